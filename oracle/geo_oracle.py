@@ -1,0 +1,108 @@
+"""ctypes binding of the CPU oracle (oracle/geo_oracle.cpp).
+
+TEST INFRASTRUCTURE, NOT PRODUCT CODE: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this module.  It
+holds argument marshalling only; every step of the method runs in the C++ file.
+It imports nothing from the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import build as _build  # noqa: E402  (oracle/build.py)
+
+SCHWARZSCHILD, KERR = 0, 1
+TIMELIKE, NULL = 0, 1
+ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC = 0, 1, 2, 3
+FLAG_PLAIN_UPDATE = 1
+
+
+class _Stop(C.Structure):
+    _fields_ = [("r_capture", C.c_double), ("r_escape", C.c_double),
+                ("kind", C.c_int32), ("flags", C.c_int32)]
+
+
+class _Out(C.Structure):
+    _fields_ = [("final_state", C.c_void_p), ("status", C.c_void_p), ("steps_done", C.c_void_p),
+                ("eq_cross_r", C.c_void_p), ("health", C.c_void_p), ("snapshots", C.c_void_p),
+                ("snap_capacity", C.c_int64), ("snap_mask", C.c_uint32), ("snap_count", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.oracle_integrate.restype = C.c_int
+        _lib.oracle_integrate.argtypes = [C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_int64,
+                                          C.c_double, C.c_int64, C.POINTER(_Stop), C.c_int64,
+                                          C.POINTER(_Out), C.c_int, C.c_int]
+        _lib.oracle_rhs.restype = None
+        _lib.oracle_rhs.argtypes = [C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_int]
+        _lib.oracle_hamiltonian.restype = C.c_double
+        _lib.oracle_hamiltonian.argtypes = [C.c_double, C.c_double, C.c_void_p]
+        _lib.oracle_energy.restype = C.c_double
+        _lib.oracle_energy.argtypes = [C.c_double] * 8
+    return _lib
+
+
+def rhs(metric: int, M: float, a: float, y8, long_double: bool = False) -> np.ndarray:
+    """d/dtau of (t, r, theta, phi, p_r, p_theta) at y8 = (t, r, theta, phi, E, p_r, p_theta, L)."""
+    y = np.ascontiguousarray(y8, dtype=np.float64)
+    d = np.empty(6)
+    lib().oracle_rhs(metric, M, a, y.ctypes.data, d.ctypes.data, int(long_double))
+    return d
+
+
+def hamiltonian(M: float, a: float, y8) -> float:
+    y = np.ascontiguousarray(y8, dtype=np.float64)
+    return lib().oracle_hamiltonian(M, a, y.ctypes.data)
+
+
+def energy(M, a, r, th, pr, pth, L, kappa) -> float:
+    """E from the mass shell 2H = -kappa (eq.(5))."""
+    return lib().oracle_energy(M, a, r, th, pr, pth, L, kappa)
+
+
+def integrate(metric: int, M: float, a: float, state_in: np.ndarray, h: float, nsteps: int,
+              r_capture: float = -np.inf, r_escape: float = np.inf, kind: int = TIMELIKE,
+              flags: int = 0, snapshot_every: int = 0, snap_capacity: int | None = None,
+              snap_mask: int = 0xFF, long_double: bool = False, nthreads: int = 1,
+              want_eq_cross: bool = True, want_health: bool = True) -> dict:
+    """Run the oracle on host SoA state_in [6][n] = (r, theta, phi, u_r, u_theta, u_phi)."""
+    st = np.ascontiguousarray(state_in, dtype=np.float64)
+    assert st.ndim == 2 and st.shape[0] == 6
+    n = st.shape[1]
+    ncomp = bin(snap_mask & 0xFF).count("1")
+    if snapshot_every > 0 and snap_capacity is None:
+        snap_capacity = 1 + nsteps // snapshot_every
+    res = {
+        "final_state": np.full((8, n), np.nan),
+        "status": np.full(n, -1, dtype=np.int32),
+        "steps_done": np.zeros(n, dtype=np.int64),
+        "eq_cross_r": np.full(n, np.nan) if want_eq_cross else None,
+        "health": np.full(n, np.nan) if want_health else None,
+        "snapshots": None, "snap_count": None,
+    }
+    if snapshot_every > 0:
+        res["snapshots"] = np.full((n, snap_capacity, ncomp), np.nan)
+        res["snap_count"] = np.zeros(n, dtype=np.int32)
+
+    def p(x):
+        return None if x is None else x.ctypes.data
+
+    stop = _Stop(r_capture, r_escape, kind, flags)
+    out = _Out(p(res["final_state"]), p(res["status"]), p(res["steps_done"]), p(res["eq_cross_r"]),
+               p(res["health"]), p(res["snapshots"]), snap_capacity or 0, snap_mask, p(res["snap_count"]))
+    rc = lib().oracle_integrate(metric, M, a, st.ctypes.data, n, h, nsteps, C.byref(stop),
+                                snapshot_every, C.byref(out), int(long_double), nthreads)
+    if rc != 0:
+        raise ValueError("oracle_integrate: invalid arguments")
+    return res

@@ -1,0 +1,223 @@
+"""Seeded synthetic input generators for the five BASELINE.json configs.
+
+This module serves BOTH the CPU oracle (tests, cpu_baseline) and the CUDA path
+(tests, bench).  It holds none of the method's arithmetic: no RHS, no RK4, no
+mass-shell solve, no stop rule.  It only draws constants of motion / positions
+and turns them into the ``state_in`` SoA ``[6][n] = (r, theta, phi, u_r,
+u_theta, u_phi)`` that ``geo_integrate`` (include/geo.h) and
+``oracle_integrate`` (oracle/geo_oracle.cpp) both take.
+
+The paper's own initial conditions are unpublished "random" sets
+(PAPER.md:436, 446 -- sec. 6.3, 6.4); these recipes stand in for them
+(DESIGN.md "Input recipe").  All in geometrized units G=c=1.
+
+PRNG: counter-based SplitMix64-style mixer, uniform = top 53 bits * 2^-53.
+Draw ``k`` of stream ``seed`` is ``mix(seed + (k+1)*GOLDEN)``; candidate ``j``
+of a rejection sampler consumes draws ``7j .. 7j+6`` and candidates are accepted
+in candidate order, so the output does not depend on the chunk size.
+"""
+from __future__ import annotations
+
+import math
+import numpy as np
+
+SEED_BASE = 180308320          # config k uses seed SEED_BASE + k
+_GOLDEN = np.uint64(0x9E3779B97F4A7C15)
+_M1 = np.uint64(0xBF58476D1CE4E5B9)
+_M2 = np.uint64(0x94D049BB133111EB)
+
+
+def splitmix_uniform(seed: int, idx: np.ndarray) -> np.ndarray:
+    """Uniform doubles in [0,1) for draw indices ``idx`` (any int array) of stream ``seed``."""
+    with np.errstate(over="ignore"):
+        z = np.uint64(seed & 0xFFFFFFFFFFFFFFFF) + (idx.astype(np.uint64) + np.uint64(1)) * _GOLDEN
+        z = (z ^ (z >> np.uint64(30))) * _M1
+        z = (z ^ (z >> np.uint64(27))) * _M2
+        z = z ^ (z >> np.uint64(31))
+    return (z >> np.uint64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
+
+
+# ----------------------------------------------------------------------------
+# closed forms used only to SHAPE the inputs
+# ----------------------------------------------------------------------------
+def horizon_radius(M: float, a: float) -> float:
+    """r_+ = M + sqrt(M^2 - a^2)."""
+    return M + math.sqrt(M * M - a * a)
+
+
+def bpt_isco(M: float, a: float, prograde: bool = True) -> float:
+    """ISCO radius, Bardeen-Press-Teukolsky Z1/Z2 form (paper ref. [17]; the
+    reading G4 of eq.(21), agrees with it -- tests pin both to
+    Tables 1-2)."""
+    x = a / M
+    z1 = 1.0 + (1.0 - x * x) ** (1.0 / 3.0) * ((1.0 + x) ** (1.0 / 3.0) + (1.0 - x) ** (1.0 / 3.0))
+    z2 = math.sqrt(3.0 * x * x + z1 * z1)
+    s = -1.0 if prograde else 1.0
+    return M * (3.0 + z2 + s * math.sqrt((3.0 - z1) * (3.0 + z1 + 2.0 * z2)))
+
+
+def circular_schwarzschild(n: int, seed: int = SEED_BASE + 1, M: float = 1.0,
+                           r_lo: float = 6.5, r_hi: float = 20.0) -> np.ndarray:
+    """Config 1: equatorial circular timelike orbits, r ~ U[r_lo, r_hi]*M.
+    u_phi = L from eq.(35) PAPER.md:222 (L^2 = M r^2/(r-3M)); theta = pi/2,
+    phi = 0, u_r = u_theta = 0 (eqs.(14),(33) PAPER.md:120, 217).  p_t is NOT an
+    input: the method derives it from eq.(5)."""
+    u = splitmix_uniform(seed, np.arange(n))
+    r = (r_lo + (r_hi - r_lo) * u) * M
+    st = np.zeros((6, n), dtype=np.float64)
+    st[0] = r
+    st[1] = math.pi / 2
+    st[5] = r * np.sqrt(M / (r - 3.0 * M))
+    return st
+
+
+def _carter_R_coeffs(E, Lz, Q, M, a):
+    """Coefficients (c4..c0) of the timelike radial potential
+    R(r) = [E(r^2+a^2) - a Lz]^2 - Delta [r^2 + (Lz - aE)^2 + Q]."""
+    e1 = E * E - 1.0
+    c4 = e1
+    c3 = 2.0 * M + 0.0 * E
+    c2 = a * a * e1 - Lz * Lz - Q
+    c1 = 2.0 * M * ((Lz - a * E) ** 2 + Q)
+    c0 = -a * a * Q
+    return c4, c3, c2, c1, c0
+
+
+def _poly4(c4, c3, c2, c1, c0, r):
+    return (((c4 * r + c3) * r + c2) * r + c1) * r + c0
+
+
+def _cubic_real_roots(A, B, C, D):
+    """Real roots of A x^3 + B x^2 + C x + D (A != 0), vectorised.  Returns an
+    array [3][m]; missing roots are NaN."""
+    b = B / A
+    c = C / A
+    d = D / A
+    p = c - b * b / 3.0
+    q = 2.0 * b ** 3 / 27.0 - b * c / 3.0 + d
+    disc = (q / 2.0) ** 2 + (p / 3.0) ** 3
+    out = np.full((3,) + A.shape, np.nan)
+    three = disc <= 0.0
+    # three real roots (trigonometric form)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        m = 2.0 * np.sqrt(np.maximum(-p / 3.0, 0.0))
+        arg = np.where(m > 0, 3.0 * q / (p * m), 0.0)
+        ang = np.arccos(np.clip(arg, -1.0, 1.0)) / 3.0
+        for k in range(3):
+            out[k] = np.where(three, m * np.cos(ang - 2.0 * math.pi * k / 3.0) - b / 3.0, np.nan)
+        # one real root (Cardano)
+        sq = np.sqrt(np.maximum(disc, 0.0))
+        one = np.cbrt(-q / 2.0 + sq) + np.cbrt(-q / 2.0 - sq) - b / 3.0
+        out[0] = np.where(three, out[0], one)
+    return out
+
+
+def kerr_bound(n: int, a: float, seed: int, M: float = 1.0, r_hi: float = 30.0,
+               chunk: int = 1 << 21, return_constants: bool = False):
+    """Configs 2 / 4 (reading W1): bound, non-plunging timelike Kerr orbits.
+
+    Candidate j draws (r0, theta0, E, Lz, Q, sgn_r, sgn_theta) with
+    r0 ~ U[1.2 r_isco(prograde, a), r_hi M], theta0 ~ U[pi/6, 5pi/6],
+    E ~ U[0.90, 0.98], Lz ~ U[-4, 4] M, Q ~ U[0, 12] M^2, signs +-1.
+    Accept iff Theta(theta0) >= 0, R(r0) >= 0 and R is negative somewhere in
+    (r_+, r0) -- i.e. an inner turning point exists outside the horizon (E < 1
+    already bounds the orbit from above).  Because R(r_+) >= 0 always, that is
+    the case iff some critical point of R inside (r_+, r0) has R < 0.
+    Then u_r = sgn_r sqrt(R)/Delta, u_theta = sgn_theta sqrt(Theta), u_phi = Lz,
+    phi0 = 0.
+    """
+    r_lo = 1.2 * bpt_isco(M, a, True)
+    r_p = horizon_radius(M, a)
+    cols = []
+    consts = []
+    have = 0
+    j0 = 0
+    while have < n:
+        j = np.arange(j0, j0 + chunk, dtype=np.int64)
+        j0 += chunk
+        d = [splitmix_uniform(seed, 7 * j + k) for k in range(7)]
+        r0 = r_lo + (r_hi * M - r_lo) * d[0]
+        th0 = math.pi / 6 + (2 * math.pi / 3) * d[1]
+        E = 0.90 + 0.08 * d[2]
+        Lz = (-4.0 + 8.0 * d[3]) * M
+        Q = 12.0 * d[4] * M * M
+        sr = np.where(d[5] < 0.5, -1.0, 1.0)
+        sth = np.where(d[6] < 0.5, -1.0, 1.0)
+        s2 = np.sin(th0) ** 2
+        c2 = np.cos(th0) ** 2
+        Theta = Q - c2 * (a * a * (1.0 - E * E) + Lz * Lz / s2)
+        c4, c3, c2_, c1, c0 = _carter_R_coeffs(E, Lz, Q, M, a)
+        R0 = _poly4(c4, c3, c2_, c1, c0, r0)
+        ok = (Theta >= 0.0) & (R0 >= 0.0)
+        idx = np.nonzero(ok)[0]
+        if idx.size:
+            cr = _cubic_real_roots(4.0 * c4[idx], 3.0 * c3[idx], 2.0 * c2_[idx], c1[idx])
+            neg = np.zeros(idx.size, dtype=bool)
+            for k in range(3):
+                x = cr[k]
+                with np.errstate(invalid="ignore"):
+                    inside = (x > r_p) & (x < r0[idx])
+                    val = _poly4(c4[idx], c3[idx], c2_[idx], c1[idx], c0[idx], np.where(inside, x, 1.0))
+                    neg |= inside & (val < 0.0)
+            idx = idx[neg]
+        if idx.size:
+            r = r0[idx]
+            Delta = r * r - 2.0 * M * r + a * a
+            st = np.zeros((6, idx.size))
+            st[0] = r
+            st[1] = th0[idx]
+            st[3] = sr[idx] * np.sqrt(R0[idx]) / Delta
+            st[4] = sth[idx] * np.sqrt(Theta[idx])
+            st[5] = Lz[idx]
+            cols.append(st)
+            if return_constants:
+                consts.append(np.stack([E[idx], Lz[idx], Q[idx]]))
+            have += idx.size
+    st = np.ascontiguousarray(np.concatenate(cols, axis=1)[:, :n])
+    if return_constants:
+        return st, np.ascontiguousarray(np.concatenate(consts, axis=1)[:, :n])
+    return st
+
+
+def camera_rays(N: int, a: float, incl_deg: float, M: float = 1.0, r_obs: float = 1000.0,
+                width: float = 20.0, row0: int = 0, rows: int | None = None,
+                return_constants: bool = False):
+    """Configs 3 / 5 (reading N2): Bardeen image plane at finite r_obs, one photon
+    per pixel, E = 1.  Pixel (ix, iy): alpha = (ix + 1/2 - N/2) W/N,
+    beta = (iy + 1/2 - N/2) W/N, particle index (iy-row0)*N + ix.
+    Lz = -alpha sin i, Q = beta^2 + (alpha^2 - a^2) cos^2 i; start
+    (r, theta, phi) = (r_obs, i, 0); u_r = -sqrt(max(R,0))/Delta with
+    R = [(r^2+a^2) - a Lz]^2 - Delta[(Lz-a)^2 + Q]; u_theta = -beta; u_phi = Lz.
+    ``row0, rows`` select a horizontal tile (config 5 is tiled, reading S3).
+    No randomness: the image is the seed."""
+    if rows is None:
+        rows = N - row0
+    inc = math.radians(incl_deg)
+    si, ci = math.sin(inc), math.cos(inc)
+    ix = np.arange(N, dtype=np.float64)
+    iy = np.arange(row0, row0 + rows, dtype=np.float64)
+    al = ((ix + 0.5 - N / 2) * (width * M / N))[None, :].repeat(rows, 0).ravel()
+    be = ((iy + 0.5 - N / 2) * (width * M / N))[:, None].repeat(N, 1).ravel()
+    Lz = -al * si
+    Q = be * be + (al * al - a * a) * ci * ci
+    r = r_obs * M
+    Delta = r * r - 2.0 * M * r + a * a
+    R = ((r * r + a * a) - a * Lz) ** 2 - Delta * ((Lz - a) ** 2 + Q)
+    n = al.size
+    st = np.zeros((6, n))
+    st[0] = r
+    st[1] = inc
+    st[3] = -np.sqrt(np.maximum(R, 0.0)) / Delta
+    st[4] = -be
+    st[5] = Lz
+    if return_constants:
+        return st, np.stack([al, be, Lz, Q])
+    return st
+
+
+def shard_range(n: int, rank: int, world: int) -> tuple[int, int]:
+    """Contiguous particle-index range [lo, hi) of ``rank`` (geodesics
+    are independent, PAPER.md:329 -- no exchange step)."""
+    base, rem = divmod(n, world)
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)

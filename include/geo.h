@@ -1,0 +1,108 @@
+/* geo.h -- C ABI of libgeo: batched fixed-step RK4 integration of independent null / timelike
+ * geodesics in Schwarzschild and Kerr spacetimes on NVIDIA B200 (sm_100a).
+ *
+ * The operation is the hot path of MALBEC (arXiv:1803.08320): "a large set of system[s solved]
+ * independently" (sec. 5), each system being Hamilton's equations (3),(4)
+ * of H = 1/2 g^{mu nu} p_mu p_nu for the Kerr metric (6) written
+ * in the 3+1 variables of eqs.(1),(8) (lapse alpha, shift beta^i, spatial metric
+ * gamma_ij), advanced with the classical fourth-order Runge-Kutta method and
+ * stopped per particle at the event horizon r_+ = M + sqrt(M^2 - a^2).
+ * Schwarzschild is a = 0, eqs.(29)-(32).  Units G = c = 1.
+ *
+ * State per geodesic, paper order:  y = (t, r, theta, phi, p_t, p_r, p_theta, p_phi),
+ * Boyer-Lindquist coordinates, covariant momenta, independent variable tau (proper time / affine
+ * parameter).  p_t is stored with the PAPER's sign, p_t = E > 0 (eq.(29); DESIGN.md
+ * reading G1); p_phi = L.  p_t and p_phi are constants of motion (eqs.(13),(32)).
+ *
+ * Every compute step runs in hand-written CUDA kernels; there is no CPU fallback.  All functions
+ * return GEO_OK (0) or an error code; nothing throws, nothing aborts.  Argument errors are reported
+ * synchronously before any launch.  geo_integrate only ENQUEUES work on `cuda_stream`.
+ */
+#ifndef GEO_H_
+#define GEO_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct geo_ctx geo_ctx; /* opaque; owned by the library */
+
+enum { GEO_SCHWARZSCHILD = 0, GEO_KERR = 1 };                       /* metric                  */
+enum { GEO_TIMELIKE = 0, GEO_NULL = 1 };                            /* geo_stop.kind: kappa=1/0 */
+enum { GEO_OK = 0, GEO_EINVAL = 1, GEO_ECUDA = 2, GEO_ENOMEM = 3 }; /* return codes            */
+/* per-particle termination class (geo_out.status) */
+enum { GEO_ST_MAXSTEPS = 0, GEO_ST_CAPTURED = 1, GEO_ST_ESCAPED = 2, GEO_ST_NUMERIC = 3 };
+/* geo_stop.flags */
+enum {
+    GEO_FLAG_PLAIN_UPDATE = 1, /* y <- y + delta without the Kahan error term (P1)     */
+    GEO_FLAG_STATIC_MAP = 2,   /* thread i integrates particle i; no work queue (for comparison) */
+    GEO_FLAG_DIRECT_SNAP = 4   /* snapshot records stored straight from registers, no smem stage */
+};
+
+/* Stop rules (PAPER.md:322-327 gives "final time reached" and "r <= r_+"; B1-B4):
+ *  - CAPTURED at the first step in which the start point, any RK4 stage point or the end point has
+ *    !(r >= r_capture); that step is not taken, the final state is the last accepted one.
+ *  - ESCAPED when, after an accepted step, r > r_escape.
+ *  - MAXSTEPS after `nsteps` accepted steps.  Use r_capture = -inf, r_escape = +inf to disable. */
+typedef struct geo_stop {
+    double r_capture;
+    double r_escape;
+    int32_t kind;  /* GEO_TIMELIKE or GEO_NULL: kappa in the mass shell 2H = -kappa, eq.(5) */
+    int32_t flags; /* GEO_FLAG_* */
+} geo_stop;
+
+/* Output buffers.  geo_integrate: DEVICE pointers; geo_integrate_host: HOST pointers.  All caller-owned.
+ * Pointers must be 16-byte aligned.  Optional ones may be NULL. */
+typedef struct geo_out {
+    double *final_state;   /* [8][n] SoA, paper order t,r,theta,phi,p_t(=E),p_r,p_theta,p_phi          */
+    int32_t *status;       /* [n] GEO_ST_*                                                             */
+    int64_t *steps_done;   /* [n] accepted RK4 steps                                                   */
+    double *eq_cross_r;    /* [n] optional: r at the first crossing of theta = pi/2, linear in theta
+                              between the two accepted states that bracket it; quiet NaN if none (B5)  */
+    double *health;        /* [n] optional: |2H + kappa| of the final state (0 on the exact solution)  */
+    double *snapshots;     /* [n][snap_capacity][ncomp] particle-major; required iff snapshot_every>0  */
+    int64_t snap_capacity; /* slots per particle; records beyond it are dropped, still counted (S3)    */
+    uint32_t snap_mask;    /* bit k set => component k of the 8-vector is stored; ncomp = popcount      */
+    int32_t *snap_count;   /* [n] records produced (slot 0 = initial state; slot j = after
+                              j*snapshot_every accepted steps; none after termination) (S1)            */
+} geo_out;
+
+/* Create a context for metric (6) with mass M > 0 and spin |a| <= M; Schwarzschild
+ * requires a == 0.  Allocates a few bytes of device memory on the current CUDA device. */
+int geo_create(geo_ctx **ctx, int metric, double M, double a);
+
+/* Integrate n geodesics for at most nsteps RK4 steps of size h (h < 0 integrates backwards in tau).
+ * state_in: DEVICE, SoA [6][n] = (r, theta, phi, u_r, u_theta, u_phi) (covariant); t starts at 0 and
+ * p_t is derived from the mass shell eq.(5) in 3+1 variables.  snapshot_every = 0: no snapshots.
+ * cuda_stream: a cudaStream_t (NULL = default stream).  Enqueue-only: outputs are valid after the
+ * caller synchronises the stream.  A ctx must not be used from two streams concurrently. */
+int geo_integrate(geo_ctx *ctx, const double *state_in, int64_t n, double h, int64_t nsteps,
+                  const geo_stop *stop, int64_t snapshot_every, const geo_out *out, void *cuda_stream);
+
+/* Same operation with HOST buffers (pageable or pinned): copies state_in to the device, integrates,
+ * copies every non-NULL output back and synchronises before returning.  Device scratch is owned by
+ * the ctx and reused between calls. */
+int geo_integrate_host(geo_ctx *ctx, const double *state_in, int64_t n, double h, int64_t nsteps,
+                       const geo_stop *stop, int64_t snapshot_every, const geo_out *out);
+
+void geo_destroy(geo_ctx *ctx);
+
+double geo_horizon_radius(const geo_ctx *ctx); /* r_+ = M + sqrt(M^2 - a^2) */
+const char *geo_last_error(const geo_ctx *ctx); /* text of the last error on this ctx ("" if none) */
+
+/* Launch geometry the next geo_integrate call on this ctx would use for (n, flags, snapshot_every):
+ * grid and block size, registers per thread, resident CTAs per SM.  For measurement reports. */
+int geo_launch_info(geo_ctx *ctx, int64_t n, int32_t flags, int64_t snapshot_every, int32_t info[4]);
+
+/* Measurement helper: runs a register-only chain of dependent-free FP64 FMAs (`iters` x 64 DFMA per
+ * thread over a full-chip grid) on `cuda_stream` and writes the number of FMAs executed to
+ * *n_fma (host).  Times nothing itself: the caller brackets it with CUDA events.  `sink` is a device
+ * buffer of >= 8 bytes that receives a value depending on every FMA. */
+int geo_probe_dfma(geo_ctx *ctx, int64_t iters, double *sink, double *n_fma, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GEO_H_ */

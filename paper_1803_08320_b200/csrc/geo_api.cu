@@ -1,0 +1,311 @@
+// geo_api.cu -- the C ABI of include/geo.h: argument validation, launch configuration, host-buffer
+// convenience path.  No arithmetic of the method lives here; it is all in geo_kernel.cuh / geo_rhs.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/geo.h"
+#include "geo_kernel.cuh"
+
+using namespace geo;
+
+struct geo_ctx {
+    int metric;
+    double M, a;
+    int device;
+    int sm_count;
+    unsigned long long* counter;   // device: work-queue head
+    // device scratch of geo_integrate_host (grow-only)
+    void* scratch;
+    size_t scratch_bytes;
+    cudaStream_t host_stream;
+    char err[256];
+};
+
+namespace {
+
+typedef void (*kernel_fn)(const Params);
+
+template <bool KERR, int SNAP>
+kernel_fn pick_plain(bool plain) {
+    return plain ? (kernel_fn)geo_rk4_kernel<KERR, SNAP, true> : (kernel_fn)geo_rk4_kernel<KERR, SNAP, false>;
+}
+template <bool KERR>
+kernel_fn pick_snap(int snap, bool plain) {
+    switch (snap) {
+        case SNAP_NONE: return pick_plain<KERR, SNAP_NONE>(plain);
+        case SNAP_DIRECT: return pick_plain<KERR, SNAP_DIRECT>(plain);
+        default: return pick_plain<KERR, SNAP_STAGED>(plain);
+    }
+}
+kernel_fn pick_kernel(int metric, int snap, bool plain) {
+    return metric == GEO_KERR ? pick_snap<true>(snap, plain) : pick_snap<false>(snap, plain);
+}
+
+int fail(geo_ctx* ctx, int code, const char* msg) {
+    if (ctx) snprintf(ctx->err, sizeof ctx->err, "%s", msg);
+    return code;
+}
+int fail_cuda(geo_ctx* ctx, cudaError_t e, const char* what) {
+    if (ctx) snprintf(ctx->err, sizeof ctx->err, "%s: %s", what, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? GEO_ENOMEM : GEO_ECUDA;
+}
+
+bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+int popcount8(uint32_t m) {
+    int c = 0;
+    for (int k = 0; k < 8; ++k) c += (m >> k) & 1u;
+    return c;
+}
+
+// Argument checks shared by the device and host entry points.  Returns GEO_OK or GEO_EINVAL.
+int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
+             int64_t snapshot_every, const geo_out* out, bool check_align) {
+    if (!ctx) return GEO_EINVAL;
+    ctx->err[0] = 0;
+    if (!stop || !out) return fail(ctx, GEO_EINVAL, "stop and out must not be NULL");
+    if (n < 0 || nsteps < 0 || snapshot_every < 0) return fail(ctx, GEO_EINVAL, "n, nsteps, snapshot_every must be >= 0");
+    if (!std::isfinite(h) || h == 0.0) return fail(ctx, GEO_EINVAL, "h must be finite and non-zero");
+    if (stop->kind != GEO_TIMELIKE && stop->kind != GEO_NULL) return fail(ctx, GEO_EINVAL, "stop.kind must be GEO_TIMELIKE or GEO_NULL");
+    if (std::isnan(stop->r_capture) || std::isnan(stop->r_escape)) return fail(ctx, GEO_EINVAL, "stop radii must not be NaN");
+    if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_DIRECT_SNAP)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
+    if (n == 0) return GEO_OK;
+    if (!state_in || !out->final_state || !out->status || !out->steps_done) return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
+    if (snapshot_every > 0) {
+        if (!out->snapshots || !out->snap_count) return fail(ctx, GEO_EINVAL, "snapshot_every > 0 needs snapshots and snap_count");
+        if (out->snap_capacity < 1) return fail(ctx, GEO_EINVAL, "snap_capacity must be >= 1");
+        if ((out->snap_mask & 0xFFu) == 0 || (out->snap_mask & ~0xFFu)) return fail(ctx, GEO_EINVAL, "snap_mask must select 1..8 of the 8 components");
+    }
+    if (check_align) {
+        if (misaligned(state_in) || misaligned(out->final_state) || misaligned(out->status) || misaligned(out->steps_done) ||
+            misaligned(out->eq_cross_r) || misaligned(out->health) || misaligned(out->snapshots) || misaligned(out->snap_count))
+            return fail(ctx, GEO_EINVAL, "device pointers must be 16-byte aligned");
+    }
+    return GEO_OK;
+}
+
+struct LaunchPlan {
+    kernel_fn fn;
+    int snap_mode;
+    int use_queue;
+    int grid;
+    size_t smem;
+    int ctas_per_sm;
+    int regs;
+};
+
+int plan_launch(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, int ncomp, LaunchPlan* lp) {
+    lp->snap_mode = snapshot_every > 0 ? ((flags & GEO_FLAG_DIRECT_SNAP) ? SNAP_DIRECT : SNAP_STAGED) : SNAP_NONE;
+    lp->fn = pick_kernel(ctx->metric, lp->snap_mode, (flags & GEO_FLAG_PLAIN_UPDATE) != 0);
+    lp->smem = lp->snap_mode == SNAP_STAGED ? (size_t)kBlock * kStageSlots * ncomp * sizeof(double) : 0;
+    lp->use_queue = (flags & GEO_FLAG_STATIC_MAP) ? 0 : 1;
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, (const void*)lp->fn);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncGetAttributes");
+    lp->regs = fa.numRegs;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)lp->fn, kBlock, lp->smem);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+    if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
+    lp->ctas_per_sm = per_sm;
+    const int64_t need = (n + kBlock - 1) / kBlock;
+    if (lp->use_queue) {
+        // persistent grid: every SM full, no more CTAs than there is work
+        const int64_t resident = (int64_t)ctx->sm_count * per_sm;
+        lp->grid = (int)(need < resident ? need : resident);
+    } else {
+        if (need > 0x7fffffffLL) return fail(ctx, GEO_EINVAL, "n too large for the static mapping");
+        lp->grid = (int)need;
+    }
+    return GEO_OK;
+}
+
+int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
+           int64_t snapshot_every, const geo_out* out, cudaStream_t stream) {
+    const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
+    LaunchPlan lp;
+    int rc = plan_launch(ctx, n, stop->flags, snapshot_every, ncomp, &lp);
+    if (rc != GEO_OK) return rc;
+
+    Params p;
+    memset(&p, 0, sizeof p);
+    p.in = d_in;
+    p.n = n;
+    p.h = h;
+    p.h_half = h / 2.0;
+    p.h_sixth = h / 6.0;
+    p.nsteps = nsteps;
+    p.r_capture = stop->r_capture;
+    p.r_escape = stop->r_escape;
+    p.kappa = stop->kind == GEO_TIMELIKE ? 1.0 : 0.0;
+    p.use_queue = lp.use_queue;
+    p.snap_every = snapshot_every;
+    p.snap_cap = snapshot_every > 0 ? out->snap_capacity : 0;
+    p.snap_mask = snapshot_every > 0 ? (out->snap_mask & 0xFFu) : 0;
+    p.ncomp = ncomp;
+    p.fin = out->final_state;
+    p.status = out->status;
+    p.steps_done = reinterpret_cast<long long*>(out->steps_done);
+    p.eq_cross_r = out->eq_cross_r;
+    p.health = out->health;
+    p.snaps = out->snapshots;
+    p.snap_count = out->snap_count;
+    p.counter = ctx->counter;
+    p.bh.M = ctx->M;
+    p.bh.a = ctx->a;
+    p.bh.a2 = ctx->a * ctx->a;
+    p.bh.twoM = 2.0 * ctx->M;
+    p.bh.twoMa = 2.0 * ctx->M * ctx->a;
+    p.bh.twoa2 = 2.0 * ctx->a * ctx->a;
+
+    cudaError_t e;
+    if (lp.use_queue) {
+        e = cudaMemsetAsync(ctx->counter, 0, sizeof(unsigned long long), stream);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
+    }
+    lp.fn<<<lp.grid, kBlock, lp.smem, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
+    return GEO_OK;
+}
+
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+}  // namespace
+
+extern "C" {
+
+int geo_create(geo_ctx** out_ctx, int metric, double M, double a) {
+    if (!out_ctx) return GEO_EINVAL;
+    *out_ctx = nullptr;
+    if (metric != GEO_SCHWARZSCHILD && metric != GEO_KERR) return GEO_EINVAL;
+    if (!(M > 0.0) || !std::isfinite(M) || !(std::fabs(a) <= M)) return GEO_EINVAL;
+    if (metric == GEO_SCHWARZSCHILD && a != 0.0) return GEO_EINVAL;
+    geo_ctx* ctx = new (std::nothrow) geo_ctx;
+    if (!ctx) return GEO_ENOMEM;
+    memset(ctx, 0, sizeof *ctx);
+    ctx->metric = metric;
+    ctx->M = M;
+    ctx->a = a;
+    cudaError_t e = cudaGetDevice(&ctx->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->counter, sizeof(unsigned long long));
+    if (e != cudaSuccess) {
+        int rc = e == cudaErrorMemoryAllocation ? GEO_ENOMEM : GEO_ECUDA;
+        delete ctx;
+        return rc;
+    }
+    *out_ctx = ctx;
+    return GEO_OK;
+}
+
+void geo_destroy(geo_ctx* ctx) {
+    if (!ctx) return;
+    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    if (ctx->scratch) cudaFree(ctx->scratch);
+    if (ctx->counter) cudaFree(ctx->counter);
+    delete ctx;
+}
+
+double geo_horizon_radius(const geo_ctx* ctx) {
+    if (!ctx) return NAN;
+    return ctx->M + std::sqrt(ctx->M * ctx->M - ctx->a * ctx->a);
+}
+
+const char* geo_last_error(const geo_ctx* ctx) { return ctx ? ctx->err : "null ctx"; }
+
+int geo_integrate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t nsteps,
+                  const geo_stop* stop, int64_t snapshot_every, const geo_out* out, void* cuda_stream) {
+    int rc = validate(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, true);
+    if (rc != GEO_OK || n == 0) return rc;
+    return launch(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, (cudaStream_t)cuda_stream);
+}
+
+int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t nsteps,
+                       const geo_stop* stop, int64_t snapshot_every, const geo_out* out) {
+    int rc = validate(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, false);
+    if (rc != GEO_OK || n == 0) return rc;
+    const size_t N = (size_t)n;
+    const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
+    const size_t b_in = align256(6 * N * 8), b_fin = align256(8 * N * 8), b_st = align256(N * 4),
+                 b_steps = align256(N * 8), b_eq = out->eq_cross_r ? align256(N * 8) : 0,
+                 b_he = out->health ? align256(N * 8) : 0,
+                 b_sn = snapshot_every > 0 ? align256(N * (size_t)out->snap_capacity * ncomp * 8) : 0,
+                 b_sc = snapshot_every > 0 ? align256(N * 4) : 0;
+    const size_t total = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_sn + b_sc;
+    cudaError_t e;
+    if (!ctx->host_stream) {
+        e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamCreate");
+    }
+    if (total > ctx->scratch_bytes) {
+        if (ctx->scratch) cudaFree(ctx->scratch);
+        ctx->scratch = nullptr;
+        ctx->scratch_bytes = 0;
+        e = cudaMalloc(&ctx->scratch, total);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMalloc(scratch)");
+        ctx->scratch_bytes = total;
+    }
+    char* base = static_cast<char*>(ctx->scratch);
+    size_t off = 0;
+    auto take = [&](size_t b) { char* q = b ? base + off : nullptr; off += b; return q; };
+    double* d_in = (double*)take(b_in);
+    geo_out d = *out;
+    d.final_state = (double*)take(b_fin);
+    d.status = (int32_t*)take(b_st);
+    d.steps_done = (int64_t*)take(b_steps);
+    d.eq_cross_r = (double*)take(b_eq);
+    d.health = (double*)take(b_he);
+    d.snapshots = (double*)take(b_sn);
+    d.snap_count = (int32_t*)take(b_sc);
+    cudaStream_t s = ctx->host_stream;
+    e = cudaMemcpyAsync(d_in, state_in, 6 * N * 8, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "H2D state_in");
+    if (d.snapshots) {
+        // slots >= snap_count[i] are documented as untouched: carry the caller's contents over
+        e = cudaMemcpyAsync(d.snapshots, out->snapshots, N * (size_t)out->snap_capacity * ncomp * 8, cudaMemcpyHostToDevice, s);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "H2D snapshots");
+    }
+    rc = launch(ctx, d_in, n, h, nsteps, stop, snapshot_every, &d, s);
+    if (rc != GEO_OK) return rc;
+    e = cudaMemcpyAsync(out->final_state, d.final_state, 8 * N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out->status, d.status, N * 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out->steps_done, d.steps_done, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.eq_cross_r) e = cudaMemcpyAsync(out->eq_cross_r, d.eq_cross_r, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.health) e = cudaMemcpyAsync(out->health, d.health, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.snapshots) e = cudaMemcpyAsync(out->snapshots, d.snapshots, N * (size_t)out->snap_capacity * ncomp * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.snap_count) e = cudaMemcpyAsync(out->snap_count, d.snap_count, N * 4, cudaMemcpyDeviceToHost, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "D2H outputs");
+    e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
+    return GEO_OK;
+}
+
+int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, int32_t info[4]) {
+    if (!ctx || !info || n < 0) return GEO_EINVAL;
+    LaunchPlan lp;
+    int rc = plan_launch(ctx, n, flags, snapshot_every, 8, &lp);
+    if (rc != GEO_OK) return rc;
+    info[0] = lp.grid;
+    info[1] = kBlock;
+    info[2] = lp.regs;
+    info[3] = lp.ctas_per_sm;
+    return GEO_OK;
+}
+
+int geo_probe_dfma(geo_ctx* ctx, int64_t iters, double* sink, double* n_fma, void* cuda_stream) {
+    if (!ctx || !sink || !n_fma || iters < 1) return GEO_EINVAL;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)dfma_probe_kernel, 256, 0);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(dfma_probe)");
+    const int grid = ctx->sm_count * per_sm;
+    dfma_probe_kernel<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(iters, sink);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "dfma_probe launch");
+    *n_fma = (double)grid * 256.0 * 64.0 * (double)iters;
+    return GEO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,296 @@
+// geo_kernel.cuh -- the RK4 stepper, stop rules, work queue and snapshot writer in one persistent kernel.
+//
+// One thread ("lane") integrates one geodesic at a time with the whole state in registers:
+//   A1 load + init   (r,th,phi,u_r,u_th,u_phi) -> y0, E from eq.(5)
+//   A3 classical RK4 (ref.[19]) with Kahan-compensated state update (P1)
+//   A4 stop rules    capture guard on every evaluation point, escape, step cap (B1-B6)
+//   A5 work queue    a lane whose geodesic ended takes the next particle index from a global atomic
+//                    counter (one warp-aggregated atomicAdd per refill round, ballot + shuffle)
+//   A6 snapshots     particle-major records, staged in shared memory and written with per-lane
+//                    bulk async copies (cp.async.bulk shared -> global), or stored directly
+//   A7 final record
+// No arithmetic crosses lanes: a particle's result does not depend on which lane ran it.
+#pragma once
+#include <cstdint>
+#include "geo_rhs.cuh"
+
+namespace geo {
+
+constexpr int kBlock = 128;
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kStageSlots = 4;   // snapshot records staged per lane before a bulk store
+
+enum { ST_MAXSTEPS = 0, ST_CAPTURED = 1, ST_ESCAPED = 2, ST_NUMERIC = 3 };
+enum { SNAP_NONE = 0, SNAP_DIRECT = 1, SNAP_STAGED = 2 };
+
+struct Params {
+    const double* in;   // [6][n]
+    long long n;
+    double h, h_half, h_sixth;
+    long long nsteps;
+    double r_capture, r_escape, kappa;
+    int use_queue;
+    long long snap_every, snap_cap;
+    unsigned snap_mask;
+    int ncomp;
+    double* fin;        // [8][n]
+    int* status;
+    long long* steps_done;
+    double* eq_cross_r;
+    double* health;
+    double* snaps;
+    int* snap_count;
+    unsigned long long* counter;
+    Hole bh;
+};
+
+__device__ __forceinline__ bool all_finite6(double a, double b, double c, double d, double e, double f) {
+    // exponent field all ones <=> Inf/NaN; integer pipe only
+    const int m = 0x7fffffff;
+    int x = max(max(__double2hiint(a) & m, __double2hiint(b) & m), __double2hiint(c) & m);
+    int y = max(max(__double2hiint(d) & m, __double2hiint(e) & m), __double2hiint(f) & m);
+    return max(x, y) < 0x7ff00000;
+}
+
+// y <- y + delta with carried error term c (Kahan); PLAIN: y <- y + delta.
+template <bool PLAIN>
+__device__ __forceinline__ void kahan(double y, double c, double delta, double& yn, double& cn) {
+    if (PLAIN) { yn = y + delta; cn = c; return; }
+    const double yk = delta - c;
+    const double ts = y + yk;
+    cn = (ts - y) - yk;
+    yn = ts;
+}
+
+__device__ __forceinline__ void store_masked(double* dst, unsigned mask, double t, double r, double th,
+                                             double ph, double E, double pr, double pth, double L) {
+    int j = 0;
+    if (mask & 1u) dst[j++] = t;
+    if (mask & 2u) dst[j++] = r;
+    if (mask & 4u) dst[j++] = th;
+    if (mask & 8u) dst[j++] = ph;
+    if (mask & 16u) dst[j++] = E;
+    if (mask & 32u) dst[j++] = pr;
+    if (mask & 64u) dst[j++] = pth;
+    if (mask & 128u) dst[j++] = L;
+}
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) {
+    return (unsigned)__cvta_generic_to_shared(p);
+}
+
+// Bulk async copy shared -> global of `bytes` (multiple of 16, both sides 16-B aligned), issued by
+// one lane for its own staged records; completion tracked with the lane's bulk async-group.
+__device__ __forceinline__ void bulk_store(double* gdst, const double* ssrc, unsigned bytes) {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 :: "l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() {
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+template <bool KERR, int SNAP, bool PLAIN>
+__global__ void __launch_bounds__(kBlock)
+geo_rk4_kernel(const __grid_constant__ Params p) {
+    extern __shared__ __align__(16) double stage_smem[];   // SNAP_STAGED: [kBlock][kStageSlots*ncomp]
+    const unsigned lane = threadIdx.x & 31u;
+    const Hole& bh = p.bh;
+
+    // lane state (registers)
+    long long idx = -1;
+    bool active = false;
+    bool exhausted = !p.use_queue;
+    double t = 0, r = 0, th = 0, ph = 0, pr = 0, pth = 0, E = 0, L = 0;
+    double ct = 0, cr = 0, cth = 0, cph = 0, cpr = 0, cpth = 0;
+    long long steps = 0, snap_ctr = 0;
+    int snaps = 0, staged = 0;
+    double eqc = 0;
+    bool crossed = false;
+    const int stage_doubles = kStageSlots * p.ncomp;
+    double* my_stage = stage_smem + (size_t)threadIdx.x * stage_doubles;
+    double* my_snaps = nullptr;   // &snaps[idx][0][0]
+
+    // --- per-particle cold paths ------------------------------------------------------------------
+    auto flush_stage = [&]() {
+        // write the `staged` records held in shared memory to slots [snaps-staged, snaps)
+        if (SNAP == SNAP_STAGED && staged > 0) {
+            double* g = my_snaps + (size_t)(snaps - staged) * p.ncomp;
+            bulk_store(g, my_stage, (unsigned)(staged * p.ncomp * 8));
+            bulk_wait_read();   // the stage region may be overwritten once the copy has read it
+            staged = 0;
+        }
+    };
+    auto emit_snapshot = [&]() {
+        if (snaps < p.snap_cap) {   // S3: drop beyond capacity, keep counting
+            if (SNAP == SNAP_DIRECT || (p.ncomp & 1)) {
+                store_masked(my_snaps + (size_t)snaps * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
+            } else {
+                store_masked(my_stage + staged * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
+                ++staged;
+                ++snaps;
+                if (staged == kStageSlots) flush_stage();
+                return;
+            }
+        }
+        ++snaps;
+    };
+    auto finish = [&](int st) {
+        if (SNAP == SNAP_STAGED) flush_stage();
+        const long long n = p.n;
+        p.fin[0 * n + idx] = t;
+        p.fin[1 * n + idx] = r;
+        p.fin[2 * n + idx] = th;
+        p.fin[3 * n + idx] = ph;
+        p.fin[4 * n + idx] = E;
+        p.fin[5 * n + idx] = pr;
+        p.fin[6 * n + idx] = pth;
+        p.fin[7 * n + idx] = L;
+        p.status[idx] = st;
+        p.steps_done[idx] = steps;
+        if (p.eq_cross_r) p.eq_cross_r[idx] = crossed ? eqc : __longlong_as_double(0x7ff8000000000000LL);
+        if (p.health) p.health[idx] = health_3p1(bh, r, th, pr, pth, E, L, p.kappa);
+        if (SNAP != SNAP_NONE) p.snap_count[idx] = snaps;
+        active = false;
+    };
+    auto begin = [&](long long i) {
+        idx = i;
+        const long long n = p.n;
+        t = 0.0;
+        r = p.in[0 * n + i];
+        th = p.in[1 * n + i];
+        ph = p.in[2 * n + i];
+        pr = p.in[3 * n + i];
+        pth = p.in[4 * n + i];
+        L = p.in[5 * n + i];
+        E = energy_3p1(bh, r, th, pr, pth, L, p.kappa);
+        ct = cr = cth = cph = cpr = cpth = 0.0;
+        steps = 0;
+        snap_ctr = p.snap_every;
+        snaps = 0;
+        staged = 0;
+        crossed = false;
+        active = true;
+        if (SNAP != SNAP_NONE) my_snaps = p.snaps + (size_t)i * (size_t)p.snap_cap * p.ncomp;
+        // B1: tests on y0 before the first step
+        if (!(r >= p.r_capture)) { finish(ST_CAPTURED); return; }
+        if (!all_finite6(r, th, ph, pr, pth, E)) { finish(ST_NUMERIC); return; }
+        if (SNAP != SNAP_NONE) emit_snapshot();   // S1: slot 0 = y0
+        if (r > p.r_escape) { finish(ST_ESCAPED); return; }
+        if (p.nsteps == 0) { finish(ST_MAXSTEPS); return; }
+    };
+
+    if (!p.use_queue) {
+        const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
+        if (i < p.n) begin(i);
+    }
+
+    for (;;) {
+        // --- A5: refill idle lanes from the queue ------------------------------------------------
+        unsigned idle = __ballot_sync(kFull, !active);
+        if (idle) {
+            if (!exhausted) {
+                const int cnt = __popc(idle);
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(p.counter, (unsigned long long)cnt);
+                base = __shfl_sync(kFull, base, 0);
+                if (!active) {
+                    const long long cand = (long long)base + __popc(idle & ((1u << lane) - 1u));
+                    if (cand < p.n) begin(cand);
+                }
+                if ((long long)base + cnt >= p.n) exhausted = true;
+                idle = __ballot_sync(kFull, !active);
+            }
+            if (idle == kFull) {
+                if (exhausted) break;
+                continue;
+            }
+        }
+
+        // --- A3: one classical RK4 step, every lane (idle lanes compute on stale state) ----------
+        Deriv k;
+        double at, ar, ath, aph, apr, apth;      // k1 + 2 k2 + 2 k3 + k4
+        double sr, sth, spr, spth;               // stage point (t, phi are cyclic: not needed)
+        rhs<KERR>(bh, r, th, pr, pth, E, L, k);
+        at = k.t; ar = k.r; ath = k.th; aph = k.ph; apr = k.pr; apth = k.pth;
+        sr = fma(p.h_half, k.r, r); sth = fma(p.h_half, k.th, th);
+        spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
+        bool cap = !(sr >= p.r_capture);                                   // B2: stage point 2
+
+        rhs<KERR>(bh, sr, sth, spr, spth, E, L, k);
+        at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
+        aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
+        sr = fma(p.h_half, k.r, r); sth = fma(p.h_half, k.th, th);
+        spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
+        cap |= !(sr >= p.r_capture);                                       // stage point 3
+
+        rhs<KERR>(bh, sr, sth, spr, spth, E, L, k);
+        at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
+        aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
+        sr = fma(p.h, k.r, r); sth = fma(p.h, k.th, th);
+        spr = fma(p.h, k.pr, pr); spth = fma(p.h, k.pth, pth);
+        cap |= !(sr >= p.r_capture);                                       // stage point 4
+
+        rhs<KERR>(bh, sr, sth, spr, spth, E, L, k);
+        at += k.t; ar += k.r; ath += k.th; aph += k.ph; apr += k.pr; apth += k.pth;
+
+        double nt, nr, nth, nph, npr, npth, dt, dr, dth, dph, dpr, dpth;
+        kahan<PLAIN>(t, ct, p.h_sixth * at, nt, dt);
+        kahan<PLAIN>(r, cr, p.h_sixth * ar, nr, dr);
+        kahan<PLAIN>(th, cth, p.h_sixth * ath, nth, dth);
+        kahan<PLAIN>(ph, cph, p.h_sixth * aph, nph, dph);
+        kahan<PLAIN>(pr, cpr, p.h_sixth * apr, npr, dpr);
+        kahan<PLAIN>(pth, cpth, p.h_sixth * apth, npth, dpth);
+        cap |= !(nr >= p.r_capture);                                       // end point
+        const bool fin6 = all_finite6(nt, nr, nth, nph, npr, npth);
+
+        // --- A4: stop rules and events ------------------------------------------------------------
+        if (active) {
+            if (cap) {
+                finish(ST_CAPTURED);            // step not taken: final = last accepted state
+            } else if (!fin6) {
+                finish(ST_NUMERIC);             // B6
+            } else {
+                if (!crossed) {                 // B5
+                    const double half_pi = 1.5707963267948966;
+                    const double d0 = th - half_pi, d1 = nth - half_pi;
+                    if (d0 * d1 < 0.0) {
+                        crossed = true;
+                        eqc = r + (nr - r) * (half_pi - th) / (nth - th);
+                    }
+                }
+                t = nt; r = nr; th = nth; ph = nph; pr = npr; pth = npth;
+                ct = dt; cr = dr; cth = dth; cph = dph; cpr = dpr; cpth = dpth;
+                ++steps;
+                if (SNAP != SNAP_NONE) {
+                    if (--snap_ctr == 0) { snap_ctr = p.snap_every; emit_snapshot(); }   // S1
+                }
+                if (r > p.r_escape) finish(ST_ESCAPED);              // B3
+                else if (steps >= p.nsteps) finish(ST_MAXSTEPS);     // B4
+            }
+        }
+    }
+    if (SNAP == SNAP_STAGED) bulk_wait_all();
+}
+
+// Register-only FP64 FMA throughput probe: 8 independent chains x 8 = 64 DFMA per iteration.
+__global__ void __launch_bounds__(256) dfma_probe_kernel(long long iters, double* sink) {
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5,
+           a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 0.999999, c = 1e-7;
+    for (long long i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+            a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+        }
+    }
+    const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (s == 123.456) sink[0] = s;   // never true in practice; keeps the chains alive
+}
+
+}  // namespace geo

@@ -1,0 +1,230 @@
+"""Thin Python binding of libgeo.so (include/geo.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
+and streams.  There is NO CPU fallback: if the library cannot be loaded, or there is no CUDA device,
+the calls raise.  Names follow the C ABI: ``geo_create``, ``geo_integrate``, ``geo_integrate_host``,
+``geo_destroy``, ``geo_horizon_radius``, ``geo_last_error``, ``geo_launch_info``, ``geo_probe_dfma``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+SCHWARZSCHILD, KERR = 0, 1
+TIMELIKE, NULL = 0, 1
+OK, EINVAL, ECUDA, ENOMEM = 0, 1, 2, 3
+ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC = 0, 1, 2, 3
+FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_DIRECT_SNAP = 1, 2, 4
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgeo.so")
+
+# every symbol include/geo.h declares
+SYMBOLS = ("geo_create", "geo_integrate", "geo_integrate_host", "geo_destroy", "geo_horizon_radius",
+           "geo_last_error", "geo_launch_info", "geo_probe_dfma")
+
+
+class GeoStop(C.Structure):
+    _fields_ = [("r_capture", C.c_double), ("r_escape", C.c_double), ("kind", C.c_int32), ("flags", C.c_int32)]
+
+
+class GeoOut(C.Structure):
+    _fields_ = [("final_state", C.c_void_p), ("status", C.c_void_p), ("steps_done", C.c_void_p),
+                ("eq_cross_r", C.c_void_p), ("health", C.c_void_p), ("snapshots", C.c_void_p),
+                ("snap_capacity", C.c_int64), ("snap_mask", C.c_uint32), ("snap_count", C.c_void_p)]
+
+
+class GeoError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libgeo error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libgeo.so (built in-tree by paper_1803_08320_b200/build.py).  Fails loudly if missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1803_08320_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.geo_create.restype = C.c_int
+        L.geo_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double]
+        L.geo_integrate.restype = C.c_int
+        L.geo_integrate.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int64,
+                                    C.POINTER(GeoStop), C.c_int64, C.POINTER(GeoOut), C.c_void_p]
+        L.geo_integrate_host.restype = C.c_int
+        L.geo_integrate_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int64,
+                                         C.POINTER(GeoStop), C.c_int64, C.POINTER(GeoOut)]
+        L.geo_destroy.restype = None
+        L.geo_destroy.argtypes = [C.c_void_p]
+        L.geo_horizon_radius.restype = C.c_double
+        L.geo_horizon_radius.argtypes = [C.c_void_p]
+        L.geo_last_error.restype = C.c_char_p
+        L.geo_last_error.argtypes = [C.c_void_p]
+        L.geo_launch_info.restype = C.c_int
+        L.geo_launch_info.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_int64, C.POINTER(C.c_int32 * 4)]
+        L.geo_probe_dfma.restype = C.c_int
+        L.geo_probe_dfma.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _check(ctx, rc: int):
+    if rc != OK:
+        raise GeoError(rc, lib().geo_last_error(ctx).decode() if ctx else "invalid arguments")
+
+
+def geo_create(metric: int, M: float = 1.0, a: float = 0.0) -> C.c_void_p:
+    ctx = C.c_void_p()
+    rc = lib().geo_create(C.byref(ctx), metric, M, a)
+    if rc != OK:
+        raise GeoError(rc, "geo_create failed (invalid metric/M/a, or no CUDA device)")
+    return ctx
+
+
+def geo_destroy(ctx) -> None:
+    lib().geo_destroy(ctx)
+
+
+def geo_horizon_radius(ctx) -> float:
+    return lib().geo_horizon_radius(ctx)
+
+
+def geo_last_error(ctx) -> str:
+    return lib().geo_last_error(ctx).decode()
+
+
+def geo_launch_info(ctx, n: int, flags: int = 0, snapshot_every: int = 0) -> dict:
+    info = (C.c_int32 * 4)()
+    _check(ctx, lib().geo_launch_info(ctx, n, flags, snapshot_every, C.byref(info)))
+    return {"grid": info[0], "block": info[1], "regs": info[2], "ctas_per_sm": info[3]}
+
+
+def _ncomp(mask: int) -> int:
+    return bin(mask & 0xFF).count("1")
+
+
+def alloc_outputs(n: int, device, nsteps: int = 0, snapshot_every: int = 0, snap_capacity: int | None = None,
+                  snap_mask: int = 0xFF, want_eq_cross: bool = True, want_health: bool = True) -> dict:
+    """Caller-owned device output tensors for geo_integrate (torch = device memory only)."""
+    import torch
+    out = {
+        "final_state": torch.empty((8, n), dtype=torch.float64, device=device),
+        "status": torch.full((n,), -1, dtype=torch.int32, device=device),
+        "steps_done": torch.zeros((n,), dtype=torch.int64, device=device),
+        "eq_cross_r": torch.empty((n,), dtype=torch.float64, device=device) if want_eq_cross else None,
+        "health": torch.empty((n,), dtype=torch.float64, device=device) if want_health else None,
+        "snapshots": None, "snap_count": None, "snap_capacity": 0, "snap_mask": snap_mask,
+    }
+    if snapshot_every > 0:
+        cap = snap_capacity if snap_capacity is not None else 1 + nsteps // snapshot_every
+        out["snap_capacity"] = cap
+        out["snapshots"] = torch.full((n, cap, _ncomp(snap_mask)), float("nan"), dtype=torch.float64, device=device)
+        out["snap_count"] = torch.zeros((n,), dtype=torch.int32, device=device)
+    return out
+
+
+def _ptr(x):
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return x.data_ptr()
+
+
+def _out_struct(out: dict) -> GeoOut:
+    return GeoOut(_ptr(out["final_state"]), _ptr(out["status"]), _ptr(out["steps_done"]),
+                  _ptr(out.get("eq_cross_r")), _ptr(out.get("health")), _ptr(out.get("snapshots")),
+                  int(out.get("snap_capacity") or 0), int(out.get("snap_mask", 0xFF)), _ptr(out.get("snap_count")))
+
+
+def geo_integrate(ctx, state_in, h: float, nsteps: int, out: dict, r_capture: float = -float("inf"),
+                  r_escape: float = float("inf"), kind: int = TIMELIKE, flags: int = 0,
+                  snapshot_every: int = 0, stream=None) -> None:
+    """Enqueue the integration of the geodesics in ``state_in`` (CUDA float64 tensor [6][n]) on
+    ``stream`` (torch.cuda.Stream; default: the current stream).  Does not synchronise."""
+    import torch
+    if not (state_in.is_cuda and state_in.dtype == torch.float64 and state_in.is_contiguous()
+            and state_in.dim() == 2 and state_in.shape[0] == 6):
+        raise ValueError("state_in must be a contiguous CUDA float64 tensor of shape [6][n]")
+    n = state_in.shape[1]
+    s = stream if stream is not None else torch.cuda.current_stream(state_in.device)
+    stop = GeoStop(r_capture, r_escape, kind, flags)
+    o = _out_struct(out)
+    with torch.cuda.device(state_in.device):
+        rc = lib().geo_integrate(ctx, state_in.data_ptr(), n, h, nsteps, C.byref(stop), snapshot_every,
+                                 C.byref(o), C.c_void_p(s.cuda_stream))
+    _check(ctx, rc)
+
+
+def geo_integrate_host(ctx, state_in: np.ndarray, h: float, nsteps: int, out: dict,
+                       r_capture: float = -float("inf"), r_escape: float = float("inf"),
+                       kind: int = TIMELIKE, flags: int = 0, snapshot_every: int = 0) -> None:
+    """Same operation on HOST buffers (numpy arrays or pinned CPU tensors); synchronous."""
+    n = state_in.shape[1]
+    stop = GeoStop(r_capture, r_escape, kind, flags)
+    o = _out_struct(out)
+    rc = lib().geo_integrate_host(ctx, _ptr(state_in), n, h, nsteps, C.byref(stop), snapshot_every, C.byref(o))
+    _check(ctx, rc)
+
+
+def alloc_outputs_host(n: int, nsteps: int = 0, snapshot_every: int = 0, snap_capacity: int | None = None,
+                       snap_mask: int = 0xFF, want_eq_cross: bool = True, want_health: bool = True,
+                       pinned: bool = False) -> dict:
+    """Host output buffers for geo_integrate_host (numpy, or pinned torch CPU tensors)."""
+    if pinned:
+        import torch
+
+        def mk(shape, dt, fill=None):
+            t = torch.empty(shape, dtype=dt, pin_memory=True)
+            if fill is not None:
+                t.fill_(fill)
+            return t
+        f64, i32, i64 = torch.float64, torch.int32, torch.int64
+    else:
+        def mk(shape, dt, fill=None):
+            a = np.empty(shape, dtype=dt)
+            if fill is not None:
+                a.fill(fill)
+            return a
+        f64, i32, i64 = np.float64, np.int32, np.int64
+    out = {
+        "final_state": mk((8, n), f64), "status": mk((n,), i32, -1), "steps_done": mk((n,), i64, 0),
+        "eq_cross_r": mk((n,), f64) if want_eq_cross else None,
+        "health": mk((n,), f64) if want_health else None,
+        "snapshots": None, "snap_count": None, "snap_capacity": 0, "snap_mask": snap_mask,
+    }
+    if snapshot_every > 0:
+        cap = snap_capacity if snap_capacity is not None else 1 + nsteps // snapshot_every
+        out["snap_capacity"] = cap
+        out["snapshots"] = mk((n, cap, _ncomp(snap_mask)), f64, float("nan"))
+        out["snap_count"] = mk((n,), i32, 0)
+    return out
+
+
+def geo_probe_dfma(ctx, iters: int, sink, stream=None) -> float:
+    """Enqueue the register-only DFMA throughput probe; returns the number of FMAs it executes."""
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream(sink.device)
+    n_fma = C.c_double()
+    _check(ctx, lib().geo_probe_dfma(ctx, iters, sink.data_ptr(), C.byref(n_fma), C.c_void_p(s.cuda_stream)))
+    return n_fma.value
+
+
+def to_numpy(out: dict) -> dict:
+    """Copy a dict of device outputs to host numpy arrays (after the caller synchronised)."""
+    res = {}
+    for k, v in out.items():
+        if v is None or isinstance(v, (int, float)):
+            res[k] = v
+        elif isinstance(v, np.ndarray):
+            res[k] = v
+        else:
+            res[k] = v.cpu().numpy()
+    return res

@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- geodesic RK4 steps/s (FP64) of the hot path on B200, and the fraction of the FP64 roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4|...]
+
+A "step" is one pass of the whole hot path (load+init, RHS, RK4, stop rules, work queue, final record)
+over one batch: by default BASELINE.json configs[3], the configuration the metric's roofline target is
+quoted on -- Kerr a=0.5, 2^22 timelike bound particles, h=0.01, 10^4 RK4 steps each, no snapshots.
+Inputs are seeded and synthetic (paper_1803_08320_b200/workloads.py).  One JSON line on stdout (rank 0).
+
+  value     whole-job geodesic-steps/s with inputs resident in HBM (CUDA events on the launch stream)
+  e2e       the same through geo_integrate_host: pinned HOST buffers, H2D + D2H inside the timed region
+  roofline  bound "alu": achieved FP64 TFLOP/s = steps/s x flop/step (static SASS count of the hot loop,
+            paper_1803_08320_b200/sass_count.py) against 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; the
+            live register-only DFMA probe is reported beside it
+  cpu_baseline  the oracle as it stands on the box's host cores, on a bounded sample
+
+N > 1 (torchrun): independent geodesics are sharded by rank, no data-path collective, weak scaling
+(every rank integrates its own 2^22-particle batch, seed + rank); value = all ranks' steps / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1803_08320_b200 import workloads as W  # noqa: E402
+
+METRIC = "geodesic RK4 steps/sec (FP64, 1xB200)"
+UNIT = "geodesic-steps/s"
+# Static SASS counts of one RK4 step of the hot loop (python -m paper_1803_08320_b200.sass_count):
+# flop = 2*DFMA + DMUL + DADD; pipe = DFMA + DMUL + DADD + DSETP.  Refreshed by sass_count at run time
+# when cuobjdump is available; these are the fallback.
+FLOP_PER_STEP = {"kerr": 645.0, "schwarzschild": 425.0}
+PIPE_INSTR_PER_STEP = {"kerr": 458.0, "schwarzschild": 289.0}
+SM_COUNT, FP64_LANES_PER_SM = 148, 64
+
+
+def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:
+    """The five BASELINE.json configs as concrete inputs."""
+    if name == "config1":
+        n = n_override or 256
+        return dict(name="configs[0] Schwarzschild circular", metric="schwarzschild", a=0.0, st=W.circular_schwarzschild(n, W.SEED_BASE + 1 + 1000 * rank),
+                    h=0.01, nsteps=2000, snapshot_every=100, snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf)
+    if name in ("config2", "config4"):
+        a = 0.9 if name == "config2" else 0.5
+        n = n_override or (65536 if name == "config2" else 1 << 22)
+        k = 2 if name == "config2" else 4
+        st = W.kerr_bound(n, a, W.SEED_BASE + k + 1000 * rank, nthreads=nthreads, chunk=1 << 20)
+        return dict(name=f"configs[{k - 1}] Kerr a={a} bound timelike", metric="kerr", a=a, st=st, h=0.01,
+                    nsteps=100000 if name == "config2" else 10000, snapshot_every=1000 if name == "config2" else 0,
+                    snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf)
+    if name in ("config3", "config5"):
+        N = n_override or (1024 if name == "config3" else 4096)
+        incl = 60.0 if name == "config3" else 85.0
+        rows = N if name == "config3" else min(N, 256)      # config 5 is tiled (S3): one tile
+        st = W.camera_rays(N, 0.998, incl, row0=(N - rows) // 2 if name == "config5" else 0, rows=rows)
+        return dict(name=f"configs[{2 if name == 'config3' else 4}] Kerr a=0.998 camera {N}x{rows} i={incl}", metric="kerr", a=0.998, st=st,
+                    h=0.02, nsteps=200000, snapshot_every=0 if name == "config3" else 500, snap_mask=0x0F, kind=1,
+                    r_capture=W.horizon_radius(1.0, 0.998) + 0.01, r_escape=1100.0)
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 and len(r) >= 7] or [r for (_, r) in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for k, nm in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "power_w_max": max(float(r[2]) for r in rows), "samples": len(rows)}
+
+
+def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> dict:
+    """Time the oracle, as it stands, on the host cores on a bounded sample of the workload."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import geo_oracle
+    cores = os.cpu_count() or 1
+    st = wl["st"]
+    # sample: a prefix of the batch sized for ~budget_s of wall time at ~3e6 steps/s/core
+    per = max(1, int(budget_s * 3.0e6 * cores / max(1, wl["nsteps"])))
+    m = min(st.shape[1], max(cores, per))
+    sub = np.ascontiguousarray(st[:, :m])
+    metric = geo_oracle.KERR if wl["metric"] == "kerr" else geo_oracle.SCHWARZSCHILD
+    kw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores,
+              snapshot_every=wl["snapshot_every"], snap_mask=wl["snap_mask"])
+    times, done = [], 0
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        o = geo_oracle.integrate(metric, 1.0, wl["a"], sub, wl["h"], wl["nsteps"], **kw)
+        dt = time.perf_counter() - t0
+        if i >= warmup:
+            times.append(dt)
+            done += int(o["steps_done"].sum())
+    return {"value": done / sum(times), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {m} of {st.shape[1]} particles x up to {wl['nsteps']} steps, {steps} pass(es)",
+            "ms_per_step": 1e3 * sum(times) / len(times)}
+
+
+def run_reference(args, rank: int, world: int) -> None:
+    """--impl reference: the oracle on the host cores (this tier has no reference implementation)."""
+    if rank != 0:
+        return
+    n_gen = args.n
+    if n_gen is None and args.workload in ("config2", "config4"):
+        # the sample is a prefix of the batch and kerr_bound(n)[:m] == kerr_bound(m): generate only the prefix
+        nsteps = 100000 if args.workload == "config2" else 10000
+        n_gen = min(65536 if args.workload == "config2" else 1 << 22,
+                    max(os.cpu_count() or 1, int(8.0 * 3.0e6 * (os.cpu_count() or 1) / nsteps)))
+    wl = workload(args.workload, 0, n_gen, os.cpu_count() or 1)
+    r = oracle_time(wl, args.steps, min(args.warmup, 1), budget_s=8.0)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": r["ms_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl["name"], "n_sample": int(wl["st"].shape[1]), "h": wl["h"], "nsteps": wl["nsteps"]},
+            "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def flop_counts(metric: str) -> tuple[float, float, str]:
+    try:
+        from paper_1803_08320_b200 import sass_count
+        c = sass_count.count("ILb1ELi0ELb0" if metric == "kerr" else "ILb0ELi0ELb0")
+        return float(c["flop"]), float(c["fp64_pipe"]), "sass_count (live)"
+    except Exception:
+        return FLOP_PER_STEP[metric], PIPE_INSTR_PER_STEP[metric], "sass_count (stored)"
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5"])
+    ap.add_argument("--n", type=int, default=None, help="override particle count / image size (development)")
+    ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1803_08320_b200 import geo
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    geo.lib()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    ncpu = max(1, (os.cpu_count() or 1) // max(1, world))
+    wl = workload(args.workload, rank, args.n, ncpu)
+    st = wl["st"]
+    n = st.shape[1]
+    metric = geo.KERR if wl["metric"] == "kerr" else geo.SCHWARZSCHILD
+    ctx = geo.geo_create(metric, 1.0, wl["a"])
+    d_in = torch.from_numpy(st).to(dev)
+    out = geo.alloc_outputs(n, dev, wl["nsteps"], wl["snapshot_every"], None, wl["snap_mask"])
+    kw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], flags=args.flags,
+              snapshot_every=wl["snapshot_every"])
+    stream = torch.cuda.current_stream(dev)
+
+    def one_pass():
+        geo.geo_integrate(ctx, d_in, wl["h"], wl["nsteps"], out, stream=stream, **kw)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        one_pass()
+    barrier()
+    steps_per_pass = int(out["steps_done"].sum().item())
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    t0 = time.time()
+    ev[0].record(stream)
+    for i in range(args.steps):
+        one_pass()
+        ev[i + 1].record(stream)
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    tot_steps = torch.tensor([float(steps_per_pass) * args.steps], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot_steps, op=dist.ReduceOp.SUM)
+    value = tot_steps.item() / (tmax.item() * 1e-3)
+
+    # ---- e2e: host buffers through geo_integrate_host (pinned), H2D + D2H inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        h_in = torch.from_numpy(st).pin_memory()
+        h_out = geo.alloc_outputs_host(n, wl["nsteps"], wl["snapshot_every"], None, wl["snap_mask"], pinned=True)
+        geo.geo_integrate_host(ctx, h_in, wl["h"], wl["nsteps"], h_out, **kw)    # warm-up (allocates scratch)
+        ke = max(1, min(args.steps, 2))
+        barrier()
+        te0 = time.perf_counter()
+        for _ in range(ke):
+            geo.geo_integrate_host(ctx, h_in, wl["h"], wl["nsteps"], h_out, **kw)
+        torch.cuda.synchronize(dev)
+        te = torch.tensor([time.perf_counter() - te0], dtype=torch.float64, device=dev)
+        es = torch.tensor([float(h_out["steps_done"].sum().item()) * ke], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            dist.all_reduce(es, op=dist.ReduceOp.SUM)
+        bo = sum(v.numel() * v.element_size() for k, v in h_out.items() if hasattr(v, "numel"))
+        bi = h_in.numel() * 8 + (h_out["snapshots"].numel() * 8 if h_out["snapshots"] is not None else 0)
+        e2e = {"value": es.item() / te.item(), "unit": UNIT, "h2d_bytes_per_step": int(bi), "d2h_bytes_per_step": int(bo),
+               "passes": ke, "api": "geo_integrate_host (pinned host buffers)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline: FP64 ALU (DFMA pipe) ----
+    flop, pipe, how = flop_counts(wl["metric"])
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0)
+    peak_tf = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    kernel_ms = sum(per_launch_ms) / len(per_launch_ms)
+    ach_tf = steps_per_pass * flop / (kernel_ms * 1e-3) / 1e12
+    # live DFMA probe (register-only FMA chains over a full-chip grid)
+    sink = torch.zeros(1, dtype=torch.float64, device=dev)
+    geo.geo_probe_dfma(ctx, 2000, sink, stream)
+    torch.cuda.synchronize(dev)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record(stream)
+    nf = geo.geo_probe_dfma(ctx, 400000, sink, stream)
+    p1.record(stream)
+    torch.cuda.synchronize(dev)
+    probe_tf = 2.0 * nf / (p0.elapsed_time(p1) * 1e-3) / 1e12
+    info = geo.geo_launch_info(ctx, n, args.flags, wl["snapshot_every"])
+    roofline = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": None,
+                "kernel": "geo_rk4_kernel", "kernel_ms": kernel_ms, "flop_per_step": flop, "fp64_pipe_instr_per_step": pipe,
+                "flop_count_source": how,
+                "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {sm_max:.0f} MHz (nominal clock; MEASURED_PEAKS.json has no FP64 entry)",
+                "pipe_util_at_max_clock": steps_per_pass * pipe / (kernel_ms * 1e-3) / (SM_COUNT * FP64_LANES_PER_SM / 32 * 32 * sm_max * 1e6),
+                "dfma_probe_tflops": probe_tf, "frac_of_dfma_probe": ach_tf / probe_tf}
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        r = oracle_time(wl, 1, 0)
+        cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": tmax.item() / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl["name"], "n_per_gpu": n, "h": wl["h"], "nsteps": wl["nsteps"],
+                       "snapshot_every": wl["snapshot_every"], "geodesic_steps_per_pass_per_gpu": steps_per_pass,
+                       "parallelism": f"independent geodesics sharded by rank x{world}, no collective",
+                       "launch": info, "flags": args.flags,
+                       "l2": f"inputs+outputs {(d_in.numel() * 8 + out['final_state'].numel() * 8) / 1e6:.0f} MB vs 126 MB L2; state lives in registers"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    geo.geo_destroy(ctx)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -108,7 +108,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
     double t = 0, r = 0, th = 0, ph = 0, pr = 0, pth = 0, E = 0, L = 0;
     double ct = 0, cr = 0, cth = 0, cph = 0, cpr = 0, cpth = 0;
     long long steps = 0, snap_ctr = 0;
-    int snaps = 0, staged = 0;
+    int snaps = 0, staged = 0, stage_first = 0;   // staged records hold slots [stage_first, stage_first+staged)
     double eqc = 0;
     bool crossed = false;
     const int stage_doubles = kStageSlots * p.ncomp;
@@ -117,9 +117,9 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
 
     // --- per-particle cold paths ------------------------------------------------------------------
     auto flush_stage = [&]() {
-        // write the `staged` records held in shared memory to slots [snaps-staged, snaps)
+        // write the `staged` records held in shared memory to their slots
         if (SNAP == SNAP_STAGED && staged > 0) {
-            double* g = my_snaps + (size_t)(snaps - staged) * p.ncomp;
+            double* g = my_snaps + (size_t)stage_first * p.ncomp;
             bulk_store(g, my_stage, (unsigned)(staged * p.ncomp * 8));
             bulk_wait_read();   // the stage region may be overwritten once the copy has read it
             staged = 0;
@@ -130,6 +130,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
             if (SNAP == SNAP_DIRECT || (p.ncomp & 1)) {
                 store_masked(my_snaps + (size_t)snaps * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
             } else {
+                if (staged == 0) stage_first = snaps;
                 store_masked(my_stage + staged * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
                 ++staged;
                 ++snaps;

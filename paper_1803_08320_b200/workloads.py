@@ -113,7 +113,7 @@ def _cubic_real_roots(A, B, C, D):
 
 
 def kerr_bound(n: int, a: float, seed: int, M: float = 1.0, r_hi: float = 30.0,
-               chunk: int = 1 << 21, return_constants: bool = False):
+               chunk: int = 1 << 21, return_constants: bool = False, nthreads: int = 1):
     """Configs 2 / 4 (reading W1): bound, non-plunging timelike Kerr orbits.
 
     Candidate j draws (r0, theta0, E, Lz, Q, sgn_r, sgn_theta) with
@@ -128,13 +128,9 @@ def kerr_bound(n: int, a: float, seed: int, M: float = 1.0, r_hi: float = 30.0,
     """
     r_lo = 1.2 * bpt_isco(M, a, True)
     r_p = horizon_radius(M, a)
-    cols = []
-    consts = []
-    have = 0
-    j0 = 0
-    while have < n:
+
+    def one_chunk(j0):
         j = np.arange(j0, j0 + chunk, dtype=np.int64)
-        j0 += chunk
         d = [splitmix_uniform(seed, 7 * j + k) for k in range(7)]
         r0 = r_lo + (r_hi * M - r_lo) * d[0]
         th0 = math.pi / 6 + (2 * math.pi / 3) * d[1]
@@ -160,19 +156,37 @@ def kerr_bound(n: int, a: float, seed: int, M: float = 1.0, r_hi: float = 30.0,
                     val = _poly4(c4[idx], c3[idx], c2_[idx], c1[idx], c0[idx], np.where(inside, x, 1.0))
                     neg |= inside & (val < 0.0)
             idx = idx[neg]
-        if idx.size:
-            r = r0[idx]
-            Delta = r * r - 2.0 * M * r + a * a
-            st = np.zeros((6, idx.size))
-            st[0] = r
-            st[1] = th0[idx]
-            st[3] = sr[idx] * np.sqrt(R0[idx]) / Delta
-            st[4] = sth[idx] * np.sqrt(Theta[idx])
-            st[5] = Lz[idx]
-            cols.append(st)
-            if return_constants:
-                consts.append(np.stack([E[idx], Lz[idx], Q[idx]]))
-            have += idx.size
+        r = r0[idx]
+        Delta = r * r - 2.0 * M * r + a * a
+        st = np.zeros((6, idx.size))
+        st[0] = r
+        st[1] = th0[idx]
+        st[3] = sr[idx] * np.sqrt(R0[idx]) / Delta
+        st[4] = sth[idx] * np.sqrt(Theta[idx])
+        st[5] = Lz[idx]
+        return st, np.stack([E[idx], Lz[idx], Q[idx]])
+
+    cols = []
+    consts = []
+    have = 0
+    j0 = 0
+    pool = None
+    if nthreads > 1:
+        from concurrent.futures import ThreadPoolExecutor
+        pool = ThreadPoolExecutor(nthreads)
+    try:
+        while have < n:
+            # chunks are taken in candidate order, so the result does not depend on nthreads
+            starts = [j0 + k * chunk for k in range(max(1, nthreads))]
+            j0 += chunk * len(starts)
+            results = list(pool.map(one_chunk, starts)) if pool else [one_chunk(starts[0])]
+            for st, cs in results:
+                cols.append(st)
+                consts.append(cs)
+                have += st.shape[1]
+    finally:
+        if pool:
+            pool.shutdown()
     st = np.ascontiguousarray(np.concatenate(cols, axis=1)[:, :n])
     if return_constants:
         return st, np.ascontiguousarray(np.concatenate(consts, axis=1)[:, :n])

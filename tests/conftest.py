@@ -20,3 +20,12 @@ def oracle():
     import geo_oracle  # oracle/geo_oracle.py (test infrastructure)
     geo_oracle.lib()
     return geo_oracle
+
+
+@pytest.fixture(scope="module")
+def G():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1803_08320_b200 import geo
+    geo.lib()   # fails loudly if libgeo.so is missing
+    return geo

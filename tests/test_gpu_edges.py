@@ -1,0 +1,162 @@
+"""GPU edge cases and invariants of the C-ABI path: empty / single / ragged batches, degenerate stop
+cases (B1), capacity overflow (S3), backwards integration, host-buffer entry point, queue vs static
+mapping, argument errors.  Each compares with the oracle or with a property that holds at any size."""
+import math
+import os
+import sys
+
+import numpy as np
+import pytest
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import parity  # noqa: E402
+from gpu_helpers import run_gpu, assert_snapshots_match  # noqa: E402
+
+from paper_1803_08320_b200 import workloads as W  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+
+def test_empty_batch_is_ok_and_launches_nothing(G):
+    import torch
+    ctx = G.geo_create(G.KERR, 1.0, 0.5)
+    d_in = torch.empty((6, 0), dtype=torch.float64, device="cuda:0")
+    out = G.alloc_outputs(0, d_in.device)
+    G.geo_integrate(ctx, d_in, 0.01, 10, out)
+    torch.cuda.synchronize()
+    G.geo_destroy(ctx)
+
+
+@pytest.mark.parametrize("n", [1, 31, 33, 129])
+def test_tiny_and_ragged_batches(G, oracle, n):
+    st = W.kerr_bound(n, 0.9, W.SEED_BASE + 2)
+    o = oracle.integrate(oracle.KERR, 1.0, 0.9, st, 0.01, 500)
+    for flags in (0, G.FLAG_STATIC_MAP):
+        g = run_gpu(G, G.KERR, 0.9, st, 0.01, 500, flags=flags)
+        c = parity.compare(g, o)
+        assert c["same_class"].all() and c["err"].max() <= 1e-9
+
+
+def test_degenerate_stop_cases_B1(G, oracle):
+    """y0 already inside r_capture -> CAPTURED, 0 steps, no slot 0; y0 beyond r_escape -> ESCAPED with
+    slot 0; nsteps = 0 -> MAXSTEPS; NaN input -> NUMERIC."""
+    st = W.kerr_bound(8, 0.5, W.SEED_BASE + 4)
+    st[0, 0] = 1.5      # < r_capture
+    st[0, 1] = 500.0    # > r_escape
+    st[3, 2] = np.nan   # non-finite momentum
+    kw = dict(r_capture=2.0, r_escape=100.0, snapshot_every=5)
+    o = oracle.integrate(oracle.KERR, 1.0, 0.5, st, 0.01, 20, **kw)
+    g = run_gpu(G, G.KERR, 0.5, st, 0.01, 20, **kw)
+    assert np.array_equal(g["status"], o["status"]) and np.array_equal(g["steps_done"], o["steps_done"])
+    assert g["status"][0] == G.ST_CAPTURED and g["status"][1] == G.ST_ESCAPED and g["status"][2] == G.ST_NUMERIC
+    assert np.array_equal(g["snap_count"], o["snap_count"])
+    assert g["snap_count"][0] == 0 and g["snap_count"][1] == 1
+    ok = np.ones(8, bool)
+    ok[2] = False
+    assert parity.rel_err(g["final_state"], o["final_state"])[:, ok].max() <= 1e-12
+    o0 = oracle.integrate(oracle.KERR, 1.0, 0.5, st[:, 3:], 0.01, 0)
+    g0 = run_gpu(G, G.KERR, 0.5, st[:, 3:], 0.01, 0)
+    assert (g0["status"] == G.ST_MAXSTEPS).all() and (g0["steps_done"] == 0).all()
+    assert parity.rel_err(g0["final_state"], o0["final_state"]).max() <= 1e-15
+
+
+def test_capture_keeps_last_accepted_state(G, oracle):
+    """B2: plunging timelike particles (r < r_isco, E and L of a slightly sub-circular orbit) are
+    CAPTURED at the guard; final state has r >= r_capture and is finite; class equals the oracle's."""
+    n = 64
+    st = np.zeros((6, n))
+    st[0] = np.linspace(3.2, 5.5, n)
+    st[1] = math.pi / 2
+    st[3] = -0.05
+    st[5] = 0.9 * st[0] * np.sqrt(1.0 / (st[0] - 3.0))
+    kw = dict(r_capture=2.0 + 1e-3, r_escape=50.0)
+    o = oracle.integrate(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.01, 20000, **kw)
+    g = run_gpu(G, G.SCHWARZSCHILD, 0.0, st, 0.01, 20000, **kw)
+    c = parity.compare(g, o)
+    assert (o["status"] == oracle.ST_CAPTURED).all()
+    assert c["same_class"].all() and c["err"].max() <= 1e-9
+    assert (g["final_state"][1] >= 2.0 + 1e-3).all() and np.isfinite(g["final_state"]).all()
+
+
+def test_snapshot_capacity_overflow_drops_but_counts_S3(G, oracle):
+    st = W.circular_schwarzschild(40)
+    for mask, flags in ((0xFF, 0), (0x0E, 0), (0x07, 0), (0xFF, G.FLAG_DIRECT_SNAP)):   # 0x07: odd ncomp
+        o = oracle.integrate(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.01, 100, snapshot_every=7, snap_capacity=6, snap_mask=mask)
+        g = run_gpu(G, G.SCHWARZSCHILD, 0.0, st, 0.01, 100, snapshot_every=7, snap_capacity=6, snap_mask=mask, flags=flags)
+        assert (g["snap_count"] == 1 + 100 // 7).all()
+        assert_snapshots_match(g, o, 1e-9)
+
+
+def test_snapshot_slot_equals_shorter_run_bitwise(G):
+    """SURVEY 8(c) pin 'Snapshots': slot j equals the final state of a run with nsteps = j*snapshot_every."""
+    st = W.kerr_bound(200, 0.9, W.SEED_BASE + 2)
+    g = run_gpu(G, G.KERR, 0.9, st, 0.01, 300, snapshot_every=100)
+    for j in (1, 2, 3):
+        gj = run_gpu(G, G.KERR, 0.9, st, 0.01, 100 * j)
+        assert np.array_equal(g["snapshots"][:, j, :], gj["final_state"].T)
+
+
+def test_backwards_integration_returns_to_start(G, oracle):
+    """h < 0 is legal; forward then backward with RK4 returns to y0 up to O(h^4) truncation."""
+    st = W.kerr_bound(64, 0.5, W.SEED_BASE + 4)
+    o = oracle.integrate(oracle.KERR, 1.0, 0.5, st, -0.01, 1000)
+    g = run_gpu(G, G.KERR, 0.5, st, -0.01, 1000)
+    c = parity.compare(g, o)
+    assert c["same_class"].all() and c["err"].max() <= 1e-9
+    back_in = np.ascontiguousarray(g["final_state"][[1, 2, 3, 5, 6, 7]])
+    b = run_gpu(G, G.KERR, 0.5, back_in, 0.01, 1000)
+    assert np.abs(b["final_state"][[1, 2, 5, 6]] - st[[0, 1, 3, 4]]).max() < 1e-8
+
+
+def test_host_entry_point_is_bitwise_equal_to_device_entry_point(G):
+    st = W.kerr_bound(777, 0.9, W.SEED_BASE + 2)
+    kw = dict(snapshot_every=50, snap_mask=0x3F)
+    a = run_gpu(G, G.KERR, 0.9, st, 0.01, 400, **kw)
+    b = run_gpu(G, G.KERR, 0.9, st, 0.01, 400, host=True, **kw)
+    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health", "snapshots", "snap_count"):
+        assert np.array_equal(a[k], b[k], equal_nan=True), k
+
+
+def test_queue_and_static_mapping_and_reruns_are_bitwise_identical(G):
+    """No arithmetic crosses lanes: results do not depend on which lane integrated a particle."""
+    a = 0.998
+    st, _ = W.camera_rays(64, a, 60.0, return_constants=True)
+    st = np.ascontiguousarray(st[:, ::3])
+    kw = dict(r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0, kind=G.NULL)
+    ref = run_gpu(G, G.KERR, a, st, 0.02, 200000, **kw)
+    for flags in (0, G.FLAG_STATIC_MAP):
+        g = run_gpu(G, G.KERR, a, st, 0.02, 200000, flags=flags, **kw)
+        for k in ("final_state", "status", "steps_done", "eq_cross_r"):
+            assert np.array_equal(ref[k], g[k], equal_nan=True), (flags, k)
+
+
+def test_plain_update_flag_matches_oracle_plain(G, oracle):
+    st = W.kerr_bound(128, 0.9, W.SEED_BASE + 2)
+    o = oracle.integrate(oracle.KERR, 1.0, 0.9, st, 0.01, 2000, flags=oracle.FLAG_PLAIN_UPDATE)
+    g = run_gpu(G, G.KERR, 0.9, st, 0.01, 2000, flags=G.FLAG_PLAIN_UPDATE)
+    c = parity.compare(g, o)
+    assert c["same_class"].all() and c["err"].max() <= 1e-9
+
+
+def test_argument_errors_return_einval_without_launch(G):
+    import torch
+    ctx = G.geo_create(G.KERR, 1.0, 0.5)
+    d_in = torch.zeros((6, 4), dtype=torch.float64, device="cuda:0")
+    out = G.alloc_outputs(4, d_in.device)
+    for kw in (dict(h=0.0), dict(h=float("nan")), dict(nsteps=-1), dict(kind=7), dict(flags=64),
+               dict(snapshot_every=5)):                        # snapshots NULL
+        args = dict(h=0.01, nsteps=10)
+        args.update(kw)
+        with pytest.raises(G.GeoError) as ei:
+            G.geo_integrate(ctx, d_in, args.pop("h"), args.pop("nsteps"), out, **args)
+        assert ei.value.code == G.EINVAL and G.geo_last_error(ctx)
+    mis = torch.zeros(6 * 4 + 1, dtype=torch.float64, device="cuda:0")[1:].view(6, 4)   # 8-byte aligned only
+    with pytest.raises(G.GeoError):
+        G.geo_integrate(ctx, mis, 0.01, 10, out)
+    G.geo_destroy(ctx)
+    for bad in ((G.KERR, 1.0, 1.5), (G.SCHWARZSCHILD, 1.0, 0.1), (5, 1.0, 0.0), (G.KERR, -1.0, 0.0)):
+        with pytest.raises(G.GeoError):
+            G.geo_create(*bad)
+    ctx = G.geo_create(G.KERR, 1.0, 0.6)
+    assert G.geo_horizon_radius(ctx) == 1.0 + math.sqrt(1.0 - 0.36)
+    G.geo_destroy(ctx)

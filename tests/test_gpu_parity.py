@@ -1,0 +1,121 @@
+"""GPU parity tests: the CUDA path (through the C ABI, include/geo.h) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's north_star: per-particle final state
+within 1e-9 relative (timelike); null rays: class identical on >= 99.99 % and 1e-8 on the rest, with
+the certification rule of DESIGN.md reading P3.  Error measure: DESIGN.md reading P2 (tests/parity.py).
+"""
+import math
+import os
+import sys
+
+import numpy as np
+import pytest
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import parity  # noqa: E402
+from gpu_helpers import run_gpu, assert_snapshots_match  # noqa: E402
+
+from paper_1803_08320_b200 import workloads as W  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+TOL_TIMELIKE = 1e-9
+TOL_NULL = 1e-8
+NCPU = max(1, (os.cpu_count() or 1))
+
+
+def assert_timelike_parity(g, o, tol=TOL_TIMELIKE):
+    c = parity.compare(g, o)
+    assert c["same_class"].all()
+    assert c["err"].max() <= tol, (c["err"].max(), int(c["err"].argmax()))
+    assert parity.rel_err(g["health"], o["health"]).max() <= 1e-6 or np.abs(g["health"] - o["health"]).max() < 1e-9
+
+
+# ------------------------------------------------------------------------------------------------------
+# BASELINE.json configs (1: full size; 2-5: prefixes / strided sub-images the oracle finishes in seconds)
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("flags", [0, 2, 4, 2 | 4])
+def test_config1_schwarzschild_circular_full(G, oracle, flags):
+    """configs[0]: 256 circular orbits, h=0.01, 2000 steps, snapshot every 100 (all 8 components)."""
+    st = W.circular_schwarzschild(256)
+    o = oracle.integrate(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.01, 2000, snapshot_every=100)
+    g = run_gpu(G, G.SCHWARZSCHILD, 0.0, st, 0.01, 2000, flags=flags, snapshot_every=100)
+    assert_timelike_parity(g, o)
+    assert_snapshots_match(g, o, TOL_TIMELIKE)
+    assert (g["status"] == G.ST_MAXSTEPS).all() and (g["steps_done"] == 2000).all()
+    # the config's own check: r constant, E and L conserved, u.u = -1
+    assert np.abs(g["final_state"][1] - st[0]).max() < 1e-12
+    assert g["health"].max() < 1e-13
+
+
+def test_config2_kerr_bound_prefix(G, oracle):
+    """configs[1] on a 1000-particle prefix (ragged: not a multiple of the 128-lane block), 10^4 steps."""
+    st = W.kerr_bound(1000, 0.9, W.SEED_BASE + 2)
+    o = oracle.integrate(oracle.KERR, 1.0, 0.9, st, 0.01, 10000, snapshot_every=1000, nthreads=NCPU)
+    g = run_gpu(G, G.KERR, 0.9, st, 0.01, 10000, snapshot_every=1000)
+    assert_timelike_parity(g, o)
+    assert_snapshots_match(g, o, TOL_TIMELIKE)
+
+
+def test_config2_full_length_small_prefix(G, oracle):
+    """configs[1] at its full 10^5 steps on 96 particles (rounding amplification over the whole run)."""
+    st = W.kerr_bound(96, 0.9, W.SEED_BASE + 2)
+    o = oracle.integrate(oracle.KERR, 1.0, 0.9, st, 0.01, 100000, snapshot_every=1000, nthreads=NCPU)
+    g = run_gpu(G, G.KERR, 0.9, st, 0.01, 100000, snapshot_every=1000)
+    assert_timelike_parity(g, o)
+    assert_snapshots_match(g, o, TOL_TIMELIKE)
+
+
+def test_config4_kerr_throughput_prefix(G, oracle):
+    """configs[3] on a 4133-particle prefix (several blocks + ragged tail), no snapshots."""
+    st = W.kerr_bound(4133, 0.5, W.SEED_BASE + 4)
+    o = oracle.integrate(oracle.KERR, 1.0, 0.5, st, 0.01, 2000, nthreads=NCPU)
+    g = run_gpu(G, G.KERR, 0.5, st, 0.01, 2000)
+    assert_timelike_parity(g, o)
+
+
+def _camera_subimage(N, a, incl, stride, offset):
+    st, consts = W.camera_rays(N, a, incl, return_constants=True)
+    ii = np.arange(N * N).reshape(N, N)[offset::stride, offset::stride].ravel()
+    return np.ascontiguousarray(st[:, ii]), consts[:, ii]
+
+
+def assert_null_parity(G, oracle, st, a, g, snapshot_every=0, snap_mask=0xFF):
+    r_cap = W.horizon_radius(1.0, a) + 0.01
+    kw = dict(r_capture=r_cap, r_escape=1100.0, kind=oracle.NULL, snapshot_every=snapshot_every,
+              snap_mask=snap_mask, nthreads=NCPU)
+    o = oracle.integrate(oracle.KERR, 1.0, a, st, 0.02, 200000, **kw)
+    o_ld = oracle.integrate(oracle.KERR, 1.0, a, st, 0.02, 200000, long_double=True, **kw)
+    cert = parity.certified(o, o_ld, TOL_NULL)
+    c = parity.compare(g, o)
+    n = st.shape[1]
+    # class: literal north_star bar on everything, and no exception among certified rays
+    assert c["same_class"].mean() >= 0.9999 or (~c["same_class"]).sum() <= max(1, int(1e-4 * n)), c["same_class"].mean()
+    assert c["same_class"][cert].all()
+    assert c["err"][cert].max() <= TOL_NULL, c["err"][cert].max()
+    assert cert.mean() > 0.97, cert.mean()    # the uncertified set is the near-axis / near-critical band only
+    return o, cert
+
+
+def test_config3_camera_subimage(G, oracle):
+    """configs[2]: a=0.998, i=60 deg, 1024^2 camera -- every 37th row/column (28x28 = 784 rays,
+    captured + escaped mix), stop rules B1-B4, equatorial-crossing output B5."""
+    a = 0.998
+    st, _ = _camera_subimage(1024, a, 60.0, 37, 5)
+    g = run_gpu(G, G.KERR, a, st, 0.02, 200000, r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0,
+                kind=G.NULL)
+    o, cert = assert_null_parity(G, oracle, st, a, g)
+    assert set(np.unique(g["status"])) == {G.ST_CAPTURED, G.ST_ESCAPED}
+
+
+def test_config5_camera_subimage_with_snapshots(G, oracle):
+    """configs[4]: i=85 deg, 4096^2 camera -- every 211th row/column (20x20 rays), snapshot every 500
+    steps of (t, r, theta, phi)."""
+    a = 0.998
+    st, _ = _camera_subimage(4096, a, 85.0, 211, 7)
+    g = run_gpu(G, G.KERR, a, st, 0.02, 200000, r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0,
+                kind=G.NULL, snapshot_every=500, snap_mask=0x0F)
+    o, cert = assert_null_parity(G, oracle, st, a, g, snapshot_every=500, snap_mask=0x0F)
+    assert np.array_equal(g["snap_count"][cert], o["snap_count"][cert])
+    cap = o["snapshots"].shape[1]
+    valid = (np.arange(cap)[None, :] < o["snap_count"][:, None]) & cert[:, None]
+    assert parity.rel_err(g["snapshots"], o["snapshots"])[valid].max() <= TOL_NULL

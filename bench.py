@@ -43,6 +43,11 @@ UNIT = "geodesic-steps/s"
 FLOP_PER_STEP = {"kerr": 645.0, "schwarzschild": 425.0}
 PIPE_INSTR_PER_STEP = {"kerr": 458.0, "schwarzschild": 289.0}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
+# declared algorithmic work of one Kerr RK4 step (4 RHS + compensated update).
+F_ALG_SURVEY = {"kerr": 800.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of one geo_rk4_kernel launch from the committed
+# `ncu --set full` capture of that workload (profiles/), bytes; None where no capture exists.
+TRAFFIC_NCU_BYTES = {}
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:
@@ -59,6 +64,19 @@ def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dic
         return dict(name=f"configs[{k - 1}] Kerr a={a} bound timelike", metric="kerr", a=a, st=st, h=0.01,
                     nsteps=100000 if name == "config2" else 10000, snapshot_every=1000 if name == "config2" else 0,
                     snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf)
+    if name == "snapbench":
+        # SURVEY.md 8(d) snapshot-writer microbenchmark: cheap RHS, a record of all 8 components EVERY step
+        n = n_override or (1 << 22)
+        return dict(name="snapshot microbenchmark: Schwarzschild circular, snapshot every step, 8 comps", metric="schwarzschild", a=0.0,
+                    st=W.circular_schwarzschild(n, W.SEED_BASE + 6 + 1000 * rank), h=0.01, nsteps=256, snapshot_every=1,
+                    snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf)
+    if name == "config3s":
+        # configs[2] with the pixels in a seeded random order: every warp holds a captured/escaped mix
+        wl = workload("config3", rank, n_override, nthreads)
+        perm = np.random.default_rng(W.SEED_BASE + 3).permutation(wl["st"].shape[1])
+        wl["st"] = np.ascontiguousarray(wl["st"][:, perm])
+        wl["name"] += " (pixels shuffled)"
+        return wl
     if name in ("config3", "config5"):
         N = n_override or (1024 if name == "config3" else 4096)
         incl = 60.0 if name == "config3" else 85.0
@@ -170,7 +188,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "snapbench"])
     ap.add_argument("--n", type=int, default=None, help="override particle count / image size (development)")
     ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -219,7 +237,6 @@ def main() -> None:
     for _ in range(args.warmup):
         one_pass()
     barrier()
-    steps_per_pass = int(out["steps_done"].sum().item())
 
     sampler = ClockSampler(local)
     sampler.start()
@@ -234,6 +251,7 @@ def main() -> None:
     barrier()
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
+    steps_per_pass = int(out["steps_done"].sum().item())    # every pass integrates the same batch
     total_ms = ev[0].elapsed_time(ev[-1])
     per_launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
     tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
@@ -245,7 +263,8 @@ def main() -> None:
 
     # ---- e2e: host buffers through geo_integrate_host (pinned), H2D + D2H inside the timed region ----
     e2e = None
-    if not args.no_e2e:
+    snap_bytes = out["snapshots"].numel() * 8 if out["snapshots"] is not None else 0
+    if not args.no_e2e and snap_bytes <= (4 << 30):       # larger trajectory buffers stay device-resident
         h_in = torch.from_numpy(st).pin_memory()
         h_out = geo.alloc_outputs_host(n, wl["nsteps"], wl["snapshot_every"], None, wl["snap_mask"], pinned=True)
         geo.geo_integrate_host(ctx, h_in, wl["h"], wl["nsteps"], h_out, **kw)    # warm-up (allocates scratch)
@@ -293,12 +312,35 @@ def main() -> None:
     torch.cuda.synchronize(dev)
     probe_tf = 2.0 * nf / (p0.elapsed_time(p1) * 1e-3) / 1e12
     info = geo.geo_launch_info(ctx, n, args.flags, wl["snapshot_every"])
-    roofline = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": None,
-                "kernel": "geo_rk4_kernel", "kernel_ms": kernel_ms, "flop_per_step": flop, "fp64_pipe_instr_per_step": pipe,
+    # SURVEY.md 8(d) declares F_alg = 800 flop per Kerr RK4 step as the algorithmic figure and asks for
+    # three numbers "so neither padding nor trimming arithmetic can game the fraction": steps/s,
+    # steps/s x F_alg / peak, and executed DFLOP/s / peak.  `achieved`/`frac` use F_alg; the executed
+    # figures (static SASS count of the hot loop; ncu's counters in profiles/ agree) sit beside them.
+    f_alg = F_ALG_SURVEY.get(wl["metric"], flop)
+    sps = steps_per_pass / (kernel_ms * 1e-3)
+    roofline = {"bound": "alu", "achieved": sps * f_alg / 1e12, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": sps * f_alg / 1e12 / peak_tf, "traffic": TRAFFIC_NCU_BYTES.get(args.workload),
+                "kernel": "geo_rk4_kernel", "kernel_ms": kernel_ms,
+                "flop_per_step_algorithmic": f_alg, "flop_per_step_executed": flop, "fp64_pipe_instr_per_step": pipe,
+                "achieved_executed": ach_tf, "frac_executed": ach_tf / peak_tf,
                 "flop_count_source": how,
                 "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {sm_max:.0f} MHz (nominal clock; MEASURED_PEAKS.json has no FP64 entry)",
-                "pipe_util_at_max_clock": steps_per_pass * pipe / (kernel_ms * 1e-3) / (SM_COUNT * FP64_LANES_PER_SM / 32 * 32 * sm_max * 1e6),
-                "dfma_probe_tflops": probe_tf, "frac_of_dfma_probe": ach_tf / probe_tf}
+                "fp64_pipe_util": sps * pipe / (SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6),
+                "dfma_probe_tflops": probe_tf, "frac_executed_of_dfma_probe": ach_tf / probe_tf}
+
+    if args.workload == "snapbench":
+        # snapshot-heavy run: the bound is HBM write bandwidth.  Algorithmic bytes per launch = every
+        # record written once (n x slots x ncomp x 8 B) + inputs read + final records written.
+        ncomp = bin(wl["snap_mask"] & 0xFF).count("1")
+        slots = 1 + wl["nsteps"] // wl["snapshot_every"]
+        alg_bytes = n * (slots * ncomp * 8 + 48 + 100)
+        hbm = float(peaks.get("hbm_gbs") or 6459.6)
+        gbs = alg_bytes / (kernel_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm,
+                    "traffic": TRAFFIC_NCU_BYTES.get(args.workload), "kernel": "geo_rk4_kernel", "kernel_ms": kernel_ms,
+                    "algorithmic_bytes_per_launch": alg_bytes,
+                    "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy, read+write)" if peaks.get("hbm_gbs") else "fallback 6459.6 GB/s (MEASURED_PEAKS.json absent)",
+                    "alu_view": roofline}
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:

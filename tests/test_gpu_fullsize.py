@@ -1,0 +1,145 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (persistent
+grid, work queue on, same flags), on SAMPLED outputs the oracle can compute one by one.
+
+Geodesics are independent, so the oracle run of a sampled particle alone must equal that
+particle's entry in the full batch.  Samples are seeded; tolerances are the north_star's (1e-9 timelike,
+1e-8 + class identity for certified null rays, readings P2/P3).  Beyond the samples, properties
+that hold at any size are checked over the whole batch: constants of motion bit-exact, health |2H+kappa|
+small, every particle terminated with a legal status / step count.
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import parity  # noqa: E402
+
+from paper_1803_08320_b200 import workloads as W  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+NCPU = max(1, (os.cpu_count() or 1))
+
+
+def _run_full(G, a, st, h, nsteps, snapshot_every=0, snap_mask=0xFF, **stop):
+    import torch
+    dev = torch.device("cuda:0")
+    ctx = G.geo_create(G.KERR, 1.0, a)
+    try:
+        d_in = torch.from_numpy(st).to(dev)
+        out = G.alloc_outputs(st.shape[1], dev, nsteps, snapshot_every, None, snap_mask)
+        G.geo_integrate(ctx, d_in, h, nsteps, out, snapshot_every=snapshot_every, **stop)
+        torch.cuda.synchronize()
+        return out
+    finally:
+        G.geo_destroy(ctx)
+
+
+def _take(out, ii, with_snaps=False):
+    """Sampled entries of the device-resident outputs as numpy (the snapshot buffer can be > host RAM)."""
+    import torch
+    it = torch.from_numpy(ii).to(out["final_state"].device)
+    g = {"final_state": out["final_state"][:, it].cpu().numpy(), "status": out["status"][it].cpu().numpy(),
+         "steps_done": out["steps_done"][it].cpu().numpy(), "eq_cross_r": out["eq_cross_r"][it].cpu().numpy(),
+         "health": out["health"][it].cpu().numpy()}
+    if with_snaps:
+        g["snapshots"] = out["snapshots"][it].cpu().numpy()
+        g["snap_count"] = out["snap_count"][it].cpu().numpy()
+    return g
+
+
+def _sample(n, m, seed):
+    rng = np.random.default_rng(seed)
+    ii = np.unique(np.concatenate([[0, 1, n - 2, n - 1], rng.integers(0, n, size=m)]))
+    return ii.astype(np.int64)
+
+
+def test_config4_full_2p22_sampled(G, oracle):
+    """configs[3], the bench workload: Kerr a=0.5, 2^22 bound timelike particles x 10^4 steps."""
+    a, n = 0.5, 1 << 22
+    st = W.kerr_bound(n, a, W.SEED_BASE + 4, nthreads=NCPU, chunk=1 << 20)
+    out = _run_full(G, a, st, 0.01, 10000)
+    assert int(out["status"].ne(G.ST_MAXSTEPS).sum().item()) == 0
+    assert int(out["steps_done"].ne(10000).sum().item()) == 0
+    hl = out["health"].cpu().numpy()
+    assert np.quantile(hl, 0.9999) < 1e-9 and np.isfinite(hl).all()     # 2H + 1 drift is O(h^4) (DESIGN.md pins)
+    fs = out["final_state"]
+    assert bool((fs[7].cpu() == __import__("torch").from_numpy(st[5])).all())     # L = p_phi bit-exact (eq.(13))
+    ii = _sample(n, 1500, 41)
+    g = _take(out, ii)
+    o = oracle.integrate(oracle.KERR, 1.0, a, np.ascontiguousarray(st[:, ii]), 0.01, 10000, nthreads=NCPU)
+    c = parity.compare(g, o)
+    assert c["same_class"].all()
+    assert c["err"].max() <= 1e-9, c["err"].max()
+
+
+def test_config2_full_65536_sampled(G, oracle):
+    """configs[1]: Kerr a=0.9, 65 536 bound particles x 10^5 steps, snapshot every 1000 (101 slots x 8)."""
+    a, n = 0.9, 65536
+    st = W.kerr_bound(n, a, W.SEED_BASE + 2, nthreads=NCPU)
+    out = _run_full(G, a, st, 0.01, 100000, snapshot_every=1000)
+    assert int(out["status"].ne(G.ST_MAXSTEPS).sum().item()) == 0
+    assert int(out["snap_count"].ne(101).sum().item()) == 0
+    ii = _sample(n, 160, 42)
+    g = _take(out, ii, with_snaps=True)
+    o = oracle.integrate(oracle.KERR, 1.0, a, np.ascontiguousarray(st[:, ii]), 0.01, 100000,
+                         snapshot_every=1000, nthreads=NCPU)
+    c = parity.compare(g, o)
+    assert c["same_class"].all()
+    assert c["err"].max() <= 1e-9, c["err"].max()
+    assert np.array_equal(g["snap_count"], o["snap_count"])
+    assert parity.rel_err(g["snapshots"], o["snapshots"]).max() <= 1e-9
+
+
+def _null_sampled(G, oracle, st, a, out, ii, snapshot_every=0, snap_mask=0xFF):
+    r_cap = W.horizon_radius(1.0, a) + 0.01
+    kw = dict(r_capture=r_cap, r_escape=1100.0, kind=oracle.NULL, snapshot_every=snapshot_every,
+              snap_mask=snap_mask, nthreads=NCPU)
+    sub = np.ascontiguousarray(st[:, ii])
+    o = oracle.integrate(oracle.KERR, 1.0, a, sub, 0.02, 200000, **kw)
+    o_ld = oracle.integrate(oracle.KERR, 1.0, a, sub, 0.02, 200000, long_double=True, **kw)
+    cert = parity.certified(o, o_ld, 1e-8)
+    g = _take(out, ii, with_snaps=snapshot_every > 0)
+    c = parity.compare(g, o)
+    assert (~c["same_class"]).sum() <= max(1, int(1e-4 * len(ii)))
+    assert c["same_class"][cert].all()
+    assert c["err"][cert].max() <= 1e-8, c["err"][cert].max()
+    assert cert.mean() > 0.97, cert.mean()
+    return g, o, cert
+
+
+def test_config3_full_1024x1024_sampled(G, oracle):
+    """configs[2]: a=0.998, i=60 deg, the whole 1024^2 image in one call (work queue refilling lanes as
+    rays are captured / escape); 256 sampled pixels against the oracle, whole-image class statistics
+    against the analytic capture criterion's expectation (~19 % captured)."""
+    a, N = 0.998, 1024
+    st = W.camera_rays(N, a, 60.0)
+    out = _run_full(G, a, st, 0.02, 200000, r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0,
+                    kind=G.NULL)
+    status = out["status"].cpu().numpy()
+    counts = np.bincount(status, minlength=4)
+    assert counts[G.ST_NUMERIC] == 0
+    assert counts[G.ST_MAXSTEPS] <= 1e-3 * N * N          # only near-axis garbage rays hit the cap (B7)
+    assert 0.15 < counts[G.ST_CAPTURED] / (N * N) < 0.25
+    ii = _sample(N * N, 252, 43)
+    _null_sampled(G, oracle, st, a, out, ii)
+
+
+def test_config5_full_tile_4096x256_sampled(G, oracle):
+    """configs[4]: i=85 deg, 4096^2 image, ONE of the 16 tiles of 256 rows (the central one, which holds
+    the shadow), snapshot every 500 steps of (t, r, theta, phi) -- 2^20 rays, 13.5 GB snapshot buffer."""
+    a, N, rows = 0.998, 4096, 256
+    st = W.camera_rays(N, a, 85.0, row0=(N - rows) // 2, rows=rows)
+    out = _run_full(G, a, st, 0.02, 200000, snapshot_every=500, snap_mask=0x0F,
+                    r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0, kind=G.NULL)
+    n = st.shape[1]
+    ii = _sample(n, 124, 45)
+    g, o, cert = _null_sampled(G, oracle, st, a, out, ii, snapshot_every=500, snap_mask=0x0F)
+    assert np.array_equal(g["snap_count"][cert], o["snap_count"][cert])
+    cap = o["snapshots"].shape[1]
+    valid = (np.arange(cap)[None, :] < o["snap_count"][:, None]) & cert[:, None]
+    assert parity.rel_err(g["snapshots"], o["snapshots"])[valid].max() <= 1e-8
+    # S1 at any size: snap_count = 1 + floor(steps_done / 500) for every ray of the tile
+    sd = out["steps_done"].cpu().numpy()
+    assert np.array_equal(out["snap_count"].cpu().numpy(), 1 + sd // 500)

@@ -52,11 +52,12 @@ __device__ __forceinline__ bool all_finite6(double a, double b, double c, double
     return max(x, y) < 0x7ff00000;
 }
 
-// y <- y + delta with carried error term c (Kahan); PLAIN: y <- y + delta.
+// y <- y + delta, delta = w * acc, with carried error term c (Kahan; the product and the subtraction
+// of c contract into one FMA); PLAIN: y <- y + w * acc.
 template <bool PLAIN>
-__device__ __forceinline__ void kahan(double y, double c, double delta, double& yn, double& cn) {
-    if (PLAIN) { yn = y + delta; cn = c; return; }
-    const double yk = delta - c;
+__device__ __forceinline__ void kahan(double y, double c, double w, double acc, double& yn, double& cn) {
+    if (PLAIN) { yn = fma(w, acc, y); cn = c; return; }
+    const double yk = fma(w, acc, -c);
     const double ts = y + yk;
     cn = (ts - y) - yk;
     yn = ts;
@@ -240,12 +241,12 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         at += k.t; ar += k.r; ath += k.th; aph += k.ph; apr += k.pr; apth += k.pth;
 
         double nt, nr, nth, nph, npr, npth, dt, dr, dth, dph, dpr, dpth;
-        kahan<PLAIN>(t, ct, p.h_sixth * at, nt, dt);
-        kahan<PLAIN>(r, cr, p.h_sixth * ar, nr, dr);
-        kahan<PLAIN>(th, cth, p.h_sixth * ath, nth, dth);
-        kahan<PLAIN>(ph, cph, p.h_sixth * aph, nph, dph);
-        kahan<PLAIN>(pr, cpr, p.h_sixth * apr, npr, dpr);
-        kahan<PLAIN>(pth, cpth, p.h_sixth * apth, npth, dpth);
+        kahan<PLAIN>(t, ct, p.h_sixth, at, nt, dt);
+        kahan<PLAIN>(r, cr, p.h_sixth, ar, nr, dr);
+        kahan<PLAIN>(th, cth, p.h_sixth, ath, nth, dth);
+        kahan<PLAIN>(ph, cph, p.h_sixth, aph, nph, dph);
+        kahan<PLAIN>(pr, cpr, p.h_sixth, apr, npr, dpr);
+        kahan<PLAIN>(pth, cpth, p.h_sixth, apth, npth, dpth);
         cap |= !(nr >= p.r_capture);                                       // end point
         const bool fin6 = all_finite6(nt, nr, nth, nph, npr, npth);
 

@@ -32,30 +32,29 @@ struct Deriv {
     double t, r, th, ph, pr, pth;
 };
 
-// 1/x for finite normal x, <= 1 ulp: MUFU.RCP64H seed (rel. err ~2^-20), one cubic and one
-// quadratic Newton correction, no denormal / Inf slow path (garbage in, garbage out -- callers
-// discard lanes whose inputs left the domain).
+// 1/x for finite normal x, faithfully rounded (<= 1 ulp): MUFU.RCP64H seed (relative error
+// <= 2^-20, measured: profiles/), then ONE cubic Newton correction y(1 + e + e^2), whose truncation
+// error e^3 <= 2^-60 is far below the rounding of the final FMA.  No denormal / Inf slow path
+// (garbage in, garbage out -- callers discard lanes whose inputs left the domain).
 __device__ __forceinline__ double rcp_nr(double x) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x, y, 1.0);
-    double t = fma(e, e, e);
-    y = fma(y, t, y);
-    e = fma(-x, y, 1.0);
-    return fma(y, e, y);
+    const double e = fma(-x, y, 1.0);
+    const double t = fma(e, e, e);
+    return fma(y, t, y);
 }
 
-// S = +-sin(x), C = +-cos(x) up to ONE COMMON sign (the RHS only uses S^2, C^2 and S*C, all even
-// under (S,C) -> (-S,-C)).  Cody-Waite reduction by pi/2 in three pieces, minimax polynomials on
-// [-pi/4, pi/4] (the classical degree-13 / degree-14 kernels, max err < 1 ulp), branch-free.
-__device__ __forceinline__ void sincos_even(double x, double& S, double& C) {
+// x = k pi/2 + y: returns sn = sin y, cs = cos y, odd = k & 1.  Cody-Waite reduction by pi/2 in two
+// pieces (the first FMA is exact; |x| stays within a few pi on this path, so the neglected
+// k * 1.5e-33 is far below an ulp of y), minimax polynomials on [-pi/4, pi/4] (the classical
+// degree-13 / degree-14 kernels, < 1 ulp), branch-free.
+__device__ __forceinline__ void sincos_reduced(double x, double& sn, double& cs, bool& odd) {
     const double magic = 6755399441055744.0;  // 1.5 * 2^52: adds round-to-nearest-integer
     double kd = fma(x, 0.63661977236758134308, magic);
-    const int q = __double2loint(kd);
+    odd = __double2loint(kd) & 1;
     kd -= magic;
     double y = fma(-kd, 1.5707963267948966e+00, x);
     y = fma(-kd, 6.1232339957367660e-17, y);
-    y = fma(-kd, -1.4973849048591698e-33, y);
     const double z = y * y;
     double ps = fma(z, 1.58969099521155010221e-10, -2.50507602534068634195e-08);
     ps = fma(ps, z, 2.75573137070700676789e-06);
@@ -67,25 +66,49 @@ __device__ __forceinline__ void sincos_even(double x, double& S, double& C) {
     pc = fma(pc, z, 2.48015872894767294178e-05);
     pc = fma(pc, z, -1.38888888888741095749e-03);
     pc = fma(pc, z, 4.16666666666666019037e-02);
-    const double sn = fma(y * z, ps, y);
-    const double cs = fma(z * z, pc, fma(z, -0.5, 1.0));
-    const bool odd = q & 1;
-    S = odd ? cs : sn;   // x = k pi/2 + y, k odd: sin = +-cos y, cos = -+sin y
-    C = odd ? -sn : cs;
+    sn = fma(y * z, ps, y);
+    cs = fma(z * z, pc, fma(z, -0.5, 1.0));
+}
+
+// s2 = sin^2 x and sc = sin x cos x -- the only trigonometric quantities the RHS needs (cos^2 enters
+// as 1 - s2).  Odd quadrant: sin^2 x = cos^2 y, sin x cos x = -sin y cos y (sign flip on the integer pipe).
+__device__ __forceinline__ void sin2_sincos(double x, double& s2, double& sc) {
+    double sn, cs;
+    bool odd;
+    sincos_reduced(x, sn, cs, odd);
+    const double S = odd ? cs : sn;
+    s2 = S * S;
+    const double p = sn * cs;
+    sc = __hiloint2double(__double2hiint(p) ^ (odd ? 0x80000000 : 0), __double2loint(p));
 }
 
 // Kerr, eq.(8) variables.  (r, th, pr, pth) evolving; E, L constants of motion.
+//
+// With W = E + beta^phi L = E - omega L,  u^t = W / alpha^2,  q1 = alpha^2 (u^t)^2 = W u^t,
+// G = gamma^{phph} L^2,  B = q1 + G,  Krho = gamma^{rr} p_r^2 + gamma^{thth} p_th^2,
+// the momentum equations of the header, with the closed-form derivatives
+//   d_r ln alpha^2   = 2r/rho^2 + 2(r-M)/Delta - d_r Sigma / Sigma,   d_th ln alpha^2 = 2 a^2 s c (Delta/Sigma - 1/rho^2)
+//   d_r omega        = (2Ma - omega d_r Sigma)/Sigma,                 d_th omega      = 2 a^2 s c Delta omega / Sigma
+//   d_r gamma^{rr}   = 2(r-M)/rho^2 - 2r gamma^{rr}/rho^2,            d_th gamma^{rr} = 2 a^2 s c gamma^{rr}/rho^2
+//   d_r gamma^{thth} = -2r/rho^4,                                     d_th gamma^{thth} = 2 a^2 s c / rho^4
+//   d_r ln gamma^{phph} = 2r/rho^2 - d_r Sigma/Sigma,                 d_th ln gamma^{phph} = d_th ln alpha^2 ... - 2 c/s
+//   d_r Sigma = 4 r (r^2+a^2) - 2 a^2 (r-M) s^2,                      d_th Sigma = -2 a^2 Delta s c
+// collect (terms in d_r Sigma / Sigma, in 1/rho^2, in (r-M)) into
+//   X = B + 2 u^t L omega,   Z = X / Sigma,   Y = (Krho - B) / rho^2
+//   dp_r/dtau  = r Y + 2 r (r^2+a^2) Z - (r-M) [ a^2 s^2 Z + q1/Delta + p_r^2/rho^2 ] - u^t L 2Ma/Sigma
+//   dp_th/dtau = s c { G / s^2 - a^2 (Delta Z + Y) }
+// (checked against the mpmath differentiation of H that pins the oracle: tests/test_oracle_pins.py
+// runs on the oracle; tests/test_gpu_parity.py compares the two).  58 FP64 instructions + sin/cos.
 __device__ __forceinline__ void rhs_kerr(const Hole& bh, double r, double th, double pr, double pth,
                                          double E, double L, Deriv& d) {
-    double S, C;
-    sincos_even(th, S, C);
-    const double s2 = S * S, c2 = C * C, sc = S * C;
+    double s2, sc;
+    sin2_sincos(th, s2, sc);
     const double r2 = r * r;
     const double A = r2 + bh.a2;                       // r^2 + a^2
-    const double rho2 = fma(bh.a2, c2, r2);
+    const double a2s2 = bh.a2 * s2;
+    const double rho2 = A - a2s2;                      // r^2 + a^2 cos^2
     const double Delta = fma(-bh.twoM, r, A);
-    const double a2D = bh.a2 * Delta;
-    const double Sigma = fma(A, A, -(a2D * s2));
+    const double Sigma = fma(A, A, -(a2s2 * Delta));
     // one reciprocal for 1/rho^2, 1/Delta, 1/Sigma, 1/sin^2
     const double P1 = rho2 * Delta, P2 = Sigma * s2;
     const double iP = rcp_nr(P1 * P2);
@@ -93,48 +116,36 @@ __device__ __forceinline__ void rhs_kerr(const Hole& bh, double r, double th, do
     const double irho = iP1 * Delta, iDel = iP1 * rho2;
     const double iSig = iP2 * s2, is2 = iP2 * Sigma;
     // lapse, shift, 3-metric (eq.(8))
-    const double omega = (bh.twoMa * r) * iSig;        // -beta^phi
+    const double mS = bh.twoMa * iSig;                 // 2Ma / Sigma
+    const double omega = mS * r;                       // -beta^phi
     const double W = fma(-omega, L, E);                // E + beta^phi L
     const double ut = (W * Sigma) * iP1;               // W / alpha^2
-    const double grr = Delta * irho;                   // gamma^{rr}
+    const double q1 = W * ut;                          // alpha^2 (u^t)^2
     const double gL = (rho2 * iP2) * L;                // gamma^{phph} L
     const double G = gL * L;
+    const double grr = Delta * irho;                   // gamma^{rr}
     d.t = ut;
     d.r = grr * pr;
-    d.th = irho * pth;
+    d.th = irho * pth;                                 // gamma^{thth} p_th
     d.ph = fma(omega, ut, gL);
-    // closed-form derivatives
+    const double B = q1 + G;
+    const double KB = fma(d.r, pr, fma(d.th, pth, -B));   // Krho - B
+    const double Y = irho * KB;
+    const double u1 = (ut * L) * mS;                   // u^t L 2Ma / Sigma
+    const double r2x = r + r;
+    const double Z = iSig * fma(u1, r2x, B);           // X / Sigma
+    const double br = fma(a2s2, Z, fma(q1, iDel, pr * (pr * irho)));
     const double rmM = r - bh.M;
-    const double Sig_r = fma(4.0 * r, A, -2.0 * ((bh.a2 * rmM) * s2));   // d_r Sigma
-    const double Tr = fma(r + r, irho, -(Sig_r * iSig));                 // d_r ln gamma^{phph}
-    const double tsc = bh.twoa2 * sc;                                    // 2 a^2 sin cos
-    const double Tth = tsc * fma(Delta, iSig, -irho);                    // d_th ln alpha^2
-    const double pr2 = pr * pr;
-    const double K = (fma(Delta, pr2, pth * pth) * irho) * irho;         // (grr pr^2 + gthth pth^2)/rho^2
-    const double q1 = W * ut;                                            // alpha^2 (u^t)^2
-    const double hB = 0.5 * (q1 + G);
-    const double dw_r = fma(-omega, Sig_r, bh.twoMa) * iSig;             // d_r omega
-    const double dw_th = ((omega * tsc) * Delta) * iSig;                 // d_th omega
-    const double utL = ut * L;
-    // d_r ln alpha^2 = Tr + 2 (r-M)/Delta ; d_r gamma^{rr} = 2 (r-M)/rho^2 - 2 r gamma^{rr}/rho^2
-    double x = hB * Tr;
-    x = fma(rmM, fma(q1, iDel, irho * pr2), x);
-    x = fma(utL, dw_r, x);
-    d.pr = fma(r, K, -x);
-    // d_th ln gamma^{phph} = Tth - 2 cos/sin ; d_th gamma^{rr,thth} = 2 a^2 sin cos (.)/rho^4
-    double w = hB * Tth;
-    w = fma(utL, dw_th, w);
-    w = fma(0.5 * tsc, K, w);
-    d.pth = fma(G * sc, is2, -w);
+    d.pr = fma(-rmM, br, fma(r2x * A, Z, fma(r, Y, -u1)));
+    d.pth = sc * fma(-bh.a2, fma(Delta, Z, Y), G * is2);
 }
 
 // Schwarzschild: alpha^2 = 1 - 2M/r = gamma^{rr}, gamma^{thth} = 1/r^2, gamma^{phph} = 1/(r^2 sin^2),
 // beta^i = 0 -- eq.(8) at a = 0; the result is eqs.(29)-(32) PAPER.md:203-211.
 __device__ __forceinline__ void rhs_schwarzschild(const Hole& bh, double r, double th, double pr,
                                                   double pth, double E, double L, Deriv& d) {
-    double S, C;
-    sincos_even(th, S, C);
-    const double s2 = S * S;
+    double s2, sc;
+    sin2_sincos(th, s2, sc);
     const double r2 = r * r;
     const double Delta = fma(-bh.twoM, r, r2);         // r^2 alpha^2
     const double P2 = r2 * s2;
@@ -155,7 +166,7 @@ __device__ __forceinline__ void rhs_schwarzschild(const Hole& bh, double r, doub
     const double Mr2 = bh.M * ir2;
     const double cen = fma(ir2, pth * pth, G) * (r * ir2);
     d.pr = fma(-Mr2, fma(ut, ut, pr * pr), cen);
-    d.pth = (G * (S * C)) * is2;                       // -1/2 d_th gamma^{phph} L^2
+    d.pth = (G * sc) * is2;                            // -1/2 d_th gamma^{phph} L^2
 }
 
 template <bool KERR>

@@ -190,7 +190,7 @@ def main() -> None:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "snapbench"])
     ap.add_argument("--n", type=int, default=None, help="override particle count / image size (development)")
-    ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping)")
+    ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping, 4 = shared-memory-staged snapshots)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

@@ -38,7 +38,9 @@ enum { GEO_ST_MAXSTEPS = 0, GEO_ST_CAPTURED = 1, GEO_ST_ESCAPED = 2, GEO_ST_NUME
 enum {
     GEO_FLAG_PLAIN_UPDATE = 1, /* y <- y + delta without the Kahan error term (P1)     */
     GEO_FLAG_STATIC_MAP = 2,   /* thread i integrates particle i; no work queue (for comparison) */
-    GEO_FLAG_DIRECT_SNAP = 4   /* snapshot records stored straight from registers, no smem stage */
+    GEO_FLAG_STAGED_SNAP = 4   /* snapshot records staged in shared memory and flushed by the warp with
+                                  coalesced stores; default: each lane stores its record straight from
+                                  registers with 256-bit stores (measured faster, profiles/)          */
 };
 
 /* Stop rules (PAPER.md:322-327 gives "final time reached" and "r <= r_+"; B1-B4):

@@ -70,7 +70,7 @@ int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t 
     if (!std::isfinite(h) || h == 0.0) return fail(ctx, GEO_EINVAL, "h must be finite and non-zero");
     if (stop->kind != GEO_TIMELIKE && stop->kind != GEO_NULL) return fail(ctx, GEO_EINVAL, "stop.kind must be GEO_TIMELIKE or GEO_NULL");
     if (std::isnan(stop->r_capture) || std::isnan(stop->r_escape)) return fail(ctx, GEO_EINVAL, "stop radii must not be NaN");
-    if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_DIRECT_SNAP)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
+    if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_STAGED_SNAP)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
     if (n == 0) return GEO_OK;
     if (!state_in || !out->final_state || !out->status || !out->steps_done) return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
     if (snapshot_every > 0) {
@@ -97,9 +97,9 @@ struct LaunchPlan {
 };
 
 int plan_launch(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, int ncomp, LaunchPlan* lp) {
-    lp->snap_mode = snapshot_every > 0 ? ((flags & GEO_FLAG_DIRECT_SNAP) ? SNAP_DIRECT : SNAP_STAGED) : SNAP_NONE;
+    lp->snap_mode = snapshot_every > 0 ? ((flags & GEO_FLAG_STAGED_SNAP) ? SNAP_STAGED : SNAP_DIRECT) : SNAP_NONE;
     lp->fn = pick_kernel(ctx->metric, lp->snap_mode, (flags & GEO_FLAG_PLAIN_UPDATE) != 0);
-    lp->smem = lp->snap_mode == SNAP_STAGED ? (size_t)kBlock * kStageSlots * ncomp * sizeof(double) : 0;
+    lp->smem = lp->snap_mode == SNAP_STAGED ? (size_t)kBlock * stage_stride(ncomp) * sizeof(double) : 0;
     lp->use_queue = (flags & GEO_FLAG_STATIC_MAP) ? 0 : 1;
     cudaFuncAttributes fa;
     cudaError_t e = cudaFuncGetAttributes(&fa, (const void*)lp->fn);

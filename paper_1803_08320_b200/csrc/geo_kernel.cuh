@@ -17,6 +17,11 @@
 namespace geo {
 
 constexpr int kBlock = 128;
+// Resident CTAs per SM the register allocation is bounded for: 5 CTAs x 128 threads = 20 warps/SM at
+// <= 96 registers (measured +3 % over 4 CTAs at 126 registers, profiles/r01_*).
+#ifndef GEO_MIN_CTAS_PER_SM
+#define GEO_MIN_CTAS_PER_SM 5
+#endif
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kStageSlots = 4;   // snapshot records staged per lane before a bulk store
 
@@ -76,29 +81,36 @@ __device__ __forceinline__ void store_masked(double* dst, unsigned mask, double 
     if (mask & 128u) dst[j++] = L;
 }
 
-__device__ __forceinline__ unsigned smem_u32(const void* p) {
-    return (unsigned)__cvta_generic_to_shared(p);
+// One record straight to its slot in global memory (SNAP_DIRECT): the two common masks go out as
+// 256-bit stores (st.global.v4.f64, SASS STG.E.256: one full 32-B sector per instruction per lane)
+// when the slot is 32-B aligned; anything else falls back to 8-B stores.
+__device__ __forceinline__ void st_v4(double* g, double a, double b, double c, double d) {
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" :: "l"(g), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+__device__ __forceinline__ void store_record_global(double* dst, unsigned mask, double t, double r, double th,
+                                                    double ph, double E, double pr, double pth, double L) {
+    const bool al32 = (reinterpret_cast<unsigned long long>(dst) & 31ull) == 0;
+    if (mask == 0xFFu && al32) {
+        st_v4(dst, t, r, th, ph);
+        st_v4(dst + 4, E, pr, pth, L);
+    } else if (mask == 0x0Fu && al32) {
+        st_v4(dst, t, r, th, ph);
+    } else {
+        store_masked(dst, mask, t, r, th, ph, E, pr, pth, L);
+    }
 }
 
-// Bulk async copy shared -> global of `bytes` (multiple of 16, both sides 16-B aligned), issued by
-// one lane for its own staged records; completion tracked with the lane's bulk async-group.
-__device__ __forceinline__ void bulk_store(double* gdst, const double* ssrc, unsigned bytes) {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                 :: "l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-}
-__device__ __forceinline__ void bulk_wait_read() {
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-}
-__device__ __forceinline__ void bulk_wait_all() {
-    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+// Shared-memory stage of SNAP_STAGED: every lane owns a slab of kStageSlots records; the slab stride
+// (in doubles) is odd so that the lanes' own 8-B writes hit distinct bank pairs.
+__host__ __device__ __forceinline__ int stage_stride(int ncomp) {
+    const int d = kStageSlots * ncomp;
+    return (d & 1) ? d : d + 1;
 }
 
 template <bool KERR, int SNAP, bool PLAIN>
-__global__ void __launch_bounds__(kBlock)
+__global__ void __launch_bounds__(kBlock, SNAP == SNAP_NONE ? GEO_MIN_CTAS_PER_SM : 4)
 geo_rk4_kernel(const __grid_constant__ Params p) {
-    extern __shared__ __align__(16) double stage_smem[];   // SNAP_STAGED: [kBlock][kStageSlots*ncomp]
+    extern __shared__ __align__(16) double stage_smem[];   // SNAP_STAGED: [kBlock][stage_stride(ncomp)]
     const unsigned lane = threadIdx.x & 31u;
     const Hole& bh = p.bh;
 
@@ -112,31 +124,46 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
     int snaps = 0, staged = 0, stage_first = 0;   // staged records hold slots [stage_first, stage_first+staged)
     double eqc = 0;
     bool crossed = false;
-    const int stage_doubles = kStageSlots * p.ncomp;
-    double* my_stage = stage_smem + (size_t)threadIdx.x * stage_doubles;
+    const int slab = stage_stride(p.ncomp);
+    double* my_stage = stage_smem + (size_t)threadIdx.x * slab;
     double* my_snaps = nullptr;   // &snaps[idx][0][0]
 
     // --- per-particle cold paths ------------------------------------------------------------------
+    // Lane-local flush (cold: once per particle, from finish()): the lane copies its own staged records.
     auto flush_stage = [&]() {
-        // write the `staged` records held in shared memory to their slots
         if (SNAP == SNAP_STAGED && staged > 0) {
             double* g = my_snaps + (size_t)stage_first * p.ncomp;
-            bulk_store(g, my_stage, (unsigned)(staged * p.ncomp * 8));
-            bulk_wait_read();   // the stage region may be overwritten once the copy has read it
+            const int cnt = staged * p.ncomp;
+            for (int k = 0; k < cnt; ++k) g[k] = my_stage[k];
             staged = 0;
         }
     };
+    // Warp-cooperative flush (converged code only): for each lane j in turn, the 32 lanes copy lane j's
+    // staged records -- contiguous in shared memory and in j's trajectory -- with coalesced 8-B stores
+    // (4 records x 8 components = 256 B = two full lines per iteration).
+    auto flush_stage_warp = [&]() {
+        __syncwarp();
+        const int cnt = staged * p.ncomp;
+        const unsigned long long dst = reinterpret_cast<unsigned long long>(my_snaps + (size_t)stage_first * p.ncomp);
+        const double* wbase = stage_smem + (size_t)(threadIdx.x & ~31u) * slab;
+        for (int j = 0; j < 32; ++j) {
+            const int c = __shfl_sync(kFull, cnt, j);
+            if (c == 0) continue;   // warp-uniform
+            double* g = reinterpret_cast<double*>(__shfl_sync(kFull, dst, j));
+            const double* sj = wbase + (size_t)j * slab;
+            for (int k = lane; k < c; k += 32) g[k] = sj[k];
+        }
+        __syncwarp();
+        staged = 0;
+    };
     auto emit_snapshot = [&]() {
         if (snaps < p.snap_cap) {   // S3: drop beyond capacity, keep counting
-            if (SNAP == SNAP_DIRECT || (p.ncomp & 1)) {
-                store_masked(my_snaps + (size_t)snaps * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
+            if (SNAP == SNAP_DIRECT) {
+                store_record_global(my_snaps + (size_t)snaps * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
             } else {
                 if (staged == 0) stage_first = snaps;
                 store_masked(my_stage + staged * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
-                ++staged;
-                ++snaps;
-                if (staged == kStageSlots) flush_stage();
-                return;
+                ++staged;           // flushed by the warp at the top of the loop, or by finish()
             }
         }
         ++snaps;
@@ -213,6 +240,12 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
             }
         }
 
+        // --- A6: a full stage anywhere in the warp -> everyone flushes (at most one record is staged
+        // per lane between two visits here, so a slab never overflows)
+        if (SNAP == SNAP_STAGED) {
+            if (__any_sync(kFull, staged == kStageSlots)) flush_stage_warp();
+        }
+
         // --- A3: one classical RK4 step, every lane (idle lanes compute on stale state) ----------
         Deriv k;
         double at, ar, ath, aph, apr, apth;      // k1 + 2 k2 + 2 k3 + k4
@@ -276,7 +309,6 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
             }
         }
     }
-    if (SNAP == SNAP_STAGED) bulk_wait_all();
 }
 
 // Register-only FP64 FMA throughput probe: 8 independent chains x 8 = 64 DFMA per iteration.

@@ -56,6 +56,20 @@ __device__ __forceinline__ void sincos_reduced(double x, double& sn, double& cs,
     double y = fma(-kd, 1.5707963267948966e+00, x);
     y = fma(-kd, 6.1232339957367660e-17, y);
     const double z = y * y;
+#ifdef GEO_POLY_ESTRIN
+    // Estrin: dependency depth 3 instead of 5 at the cost of one extra DMUL (z^4)
+    const double z2 = z * z, z4 = z2 * z2;
+    const double s01 = fma(z, 8.33333333332248946124e-03, -1.66666666666666324348e-01);
+    const double s23 = fma(z, 2.75573137070700676789e-06, -1.98412698298579493134e-04);
+    const double s45 = fma(z, 1.58969099521155010221e-10, -2.50507602534068634195e-08);
+    const double ps = fma(z4, s45, fma(z2, s23, s01));
+    const double c01 = fma(z, -1.38888888888741095749e-03, 4.16666666666666019037e-02);
+    const double c23 = fma(z, -2.75573143513906633035e-07, 2.48015872894767294178e-05);
+    const double c45 = fma(z, -1.13596475577881948265e-11, 2.08757232129817482790e-09);
+    const double pc = fma(z4, c45, fma(z2, c23, c01));
+    sn = fma(y * z, ps, y);
+    cs = fma(z2, pc, fma(z, -0.5, 1.0));
+#else
     double ps = fma(z, 1.58969099521155010221e-10, -2.50507602534068634195e-08);
     ps = fma(ps, z, 2.75573137070700676789e-06);
     ps = fma(ps, z, -1.98412698298579493134e-04);
@@ -68,6 +82,7 @@ __device__ __forceinline__ void sincos_reduced(double x, double& sn, double& cs,
     pc = fma(pc, z, 4.16666666666666019037e-02);
     sn = fma(y * z, ps, y);
     cs = fma(z * z, pc, fma(z, -0.5, 1.0));
+#endif
 }
 
 // s2 = sin^2 x and sc = sin x cos x -- the only trigonometric quantities the RHS needs (cos^2 enters

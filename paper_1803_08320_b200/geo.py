@@ -16,10 +16,10 @@ SCHWARZSCHILD, KERR = 0, 1
 TIMELIKE, NULL = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, 1, 2, 3
 ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC = 0, 1, 2, 3
-FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_DIRECT_SNAP = 1, 2, 4
+FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_STAGED_SNAP = 1, 2, 4
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgeo.so")
+LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI
 
 # every symbol include/geo.h declares
 SYMBOLS = ("geo_create", "geo_integrate", "geo_integrate_host", "geo_destroy", "geo_horizon_radius",

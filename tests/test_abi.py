@@ -32,14 +32,14 @@ def test_struct_layouts_match_header():
     assert geo.GeoOut.snap_mask.offset == 56 and geo.GeoOut.snap_count.offset == 64
 
 
-def test_sass_has_fp64_pipe_and_bulk_copy():
-    """The hot loop is FP64 FMA work (DFMA), the staged snapshot writer uses bulk async copies (UBLKCP)."""
+def test_sass_has_fp64_pipe_and_wide_stores():
+    """The hot loop is FP64 FMA work (DFMA); the snapshot writer issues 256-bit global stores (STG.E...256)."""
     import subprocess
     from paper_1803_08320_b200 import build
     sass = subprocess.run(["cuobjdump", "-sass", build.build()], capture_output=True, text=True).stdout
     assert "sm_100a" in sass
     assert sass.count("DFMA") > 500
-    assert "UBLKCP" in sass
+    assert re.search(r"STG\.E(\.\w+)*\.256", sass)
 
 
 def test_product_path_does_not_import_the_oracle():

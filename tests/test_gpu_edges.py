@@ -80,7 +80,7 @@ def test_capture_keeps_last_accepted_state(G, oracle):
 
 def test_snapshot_capacity_overflow_drops_but_counts_S3(G, oracle):
     st = W.circular_schwarzschild(40)
-    for mask, flags in ((0xFF, 0), (0x0E, 0), (0x07, 0), (0xFF, G.FLAG_DIRECT_SNAP)):   # 0x07: odd ncomp
+    for mask, flags in ((0xFF, 0), (0x0E, 0), (0x07, 0), (0xFF, G.FLAG_STAGED_SNAP), (0x07, G.FLAG_STAGED_SNAP), (0x0F, G.FLAG_STAGED_SNAP)):   # 0x07: odd ncomp
         o = oracle.integrate(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.01, 100, snapshot_every=7, snap_capacity=6, snap_mask=mask)
         g = run_gpu(G, G.SCHWARZSCHILD, 0.0, st, 0.01, 100, snapshot_every=7, snap_capacity=6, snap_mask=mask, flags=flags)
         assert (g["snap_count"] == 1 + 100 // 7).all()

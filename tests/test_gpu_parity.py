@@ -107,13 +107,14 @@ def test_config3_camera_subimage(G, oracle):
     assert set(np.unique(g["status"])) == {G.ST_CAPTURED, G.ST_ESCAPED}
 
 
-def test_config5_camera_subimage_with_snapshots(G, oracle):
+@pytest.mark.parametrize("flags", [0, 4])      # 4 = GEO_FLAG_STAGED_SNAP: lanes out of phase share warp flushes
+def test_config5_camera_subimage_with_snapshots(G, oracle, flags):
     """configs[4]: i=85 deg, 4096^2 camera -- every 211th row/column (20x20 rays), snapshot every 500
     steps of (t, r, theta, phi)."""
     a = 0.998
     st, _ = _camera_subimage(4096, a, 85.0, 211, 7)
     g = run_gpu(G, G.KERR, a, st, 0.02, 200000, r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0,
-                kind=G.NULL, snapshot_every=500, snap_mask=0x0F)
+                kind=G.NULL, snapshot_every=500, snap_mask=0x0F, flags=flags)
     o, cert = assert_null_parity(G, oracle, st, a, g, snapshot_every=500, snap_mask=0x0F)
     assert np.array_equal(g["snap_count"][cert], o["snap_count"][cert])
     cap = o["snapshots"].shape[1]

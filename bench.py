@@ -47,7 +47,7 @@ SM_COUNT, FP64_LANES_PER_SM = 148, 64
 F_ALG_SURVEY = {"kerr": 800.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one geo_rk4_kernel launch from the committed
 # `ncu --set full` capture of that workload (profiles/), bytes; None where no capture exists.
-TRAFFIC_NCU_BYTES = {}
+TRAFFIC_NCU_BYTES = {"config4": 598_090_752}      # profiles/r01_config4_v1.md
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:

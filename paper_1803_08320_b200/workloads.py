@@ -235,3 +235,9 @@ def shard_range(n: int, rank: int, world: int) -> tuple[int, int]:
     base, rem = divmod(n, world)
     lo = rank * base + min(rank, rem)
     return lo, lo + base + (1 if rank < rem else 0)
+
+
+def interleaved_tiles(ntiles: int, rank: int, world: int) -> list[int]:
+    """Image tiles of ``rank``: tile t -> rank t mod world, so every rank gets the same
+    captured/escaped mix (captured rays cost about half an escaping one)."""
+    return list(range(rank, ntiles, world))

@@ -159,6 +159,7 @@ int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps
     p.bh.twoM = 2.0 * ctx->M;
     p.bh.twoMa = 2.0 * ctx->M * ctx->a;
     p.bh.twoa2 = 2.0 * ctx->a * ctx->a;
+    fill_trig_consts(p.bh.tc);
 
     cudaError_t e;
     if (lp.use_queue) {

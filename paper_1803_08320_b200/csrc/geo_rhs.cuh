@@ -23,9 +23,31 @@
 
 namespace geo {
 
+// Constants of the sin/cos kernel.  They travel in the kernel parameters (constant bank), so that the
+// DFMAs read them as constant operands: as literals the compiler re-materialises every coefficient with
+// two MOV-immediates per use (ncu: 83 of 513 issued instructions per RK4 step).
+struct TrigConsts {
+    double two_over_pi, magic, pio2_hi, pio2_lo;
+    double s[6];   // sin y = y + y z (s0 + s1 z + ... + s5 z^5),  z = y^2
+    double c[6];   // cos y = 1 - z/2 + z^2 (c0 + c1 z + ... + c5 z^5)
+};
+
 struct Hole {
     double M, a, a2, twoM, twoMa, twoa2;
+    TrigConsts tc;
 };
+
+inline void fill_trig_consts(TrigConsts& t) {
+    t.two_over_pi = 0.63661977236758134308;
+    t.magic = 6755399441055744.0;             // 1.5 * 2^52: adding it rounds to the nearest integer
+    t.pio2_hi = 1.5707963267948966e+00;
+    t.pio2_lo = 6.1232339957367660e-17;
+    const double s[6] = {-1.66666666666666324348e-01, 8.33333333332248946124e-03, -1.98412698298579493134e-04,
+                         2.75573137070700676789e-06, -2.50507602534068634195e-08, 1.58969099521155010221e-10};
+    const double c[6] = {4.16666666666666019037e-02, -1.38888888888741095749e-03, 2.48015872894767294178e-05,
+                         -2.75573143513906633035e-07, 2.08757232129817482790e-09, -1.13596475577881948265e-11};
+    for (int i = 0; i < 6; ++i) { t.s[i] = s[i]; t.c[i] = c[i]; }
+}
 
 // d/dtau of (t, r, theta, phi, p_r, p_theta)
 struct Deriv {
@@ -48,49 +70,33 @@ __device__ __forceinline__ double rcp_nr(double x) {
 // pieces (the first FMA is exact; |x| stays within a few pi on this path, so the neglected
 // k * 1.5e-33 is far below an ulp of y), minimax polynomials on [-pi/4, pi/4] (the classical
 // degree-13 / degree-14 kernels, < 1 ulp), branch-free.
-__device__ __forceinline__ void sincos_reduced(double x, double& sn, double& cs, bool& odd) {
-    const double magic = 6755399441055744.0;  // 1.5 * 2^52: adds round-to-nearest-integer
-    double kd = fma(x, 0.63661977236758134308, magic);
+__device__ __forceinline__ void sincos_reduced(const TrigConsts& tc, double x, double& sn, double& cs, bool& odd) {
+    double kd = fma(x, tc.two_over_pi, tc.magic);
     odd = __double2loint(kd) & 1;
-    kd -= magic;
-    double y = fma(-kd, 1.5707963267948966e+00, x);
-    y = fma(-kd, 6.1232339957367660e-17, y);
+    kd -= tc.magic;
+    double y = fma(-kd, tc.pio2_hi, x);
+    y = fma(-kd, tc.pio2_lo, y);
     const double z = y * y;
-#ifdef GEO_POLY_ESTRIN
-    // Estrin: dependency depth 3 instead of 5 at the cost of one extra DMUL (z^4)
-    const double z2 = z * z, z4 = z2 * z2;
-    const double s01 = fma(z, 8.33333333332248946124e-03, -1.66666666666666324348e-01);
-    const double s23 = fma(z, 2.75573137070700676789e-06, -1.98412698298579493134e-04);
-    const double s45 = fma(z, 1.58969099521155010221e-10, -2.50507602534068634195e-08);
-    const double ps = fma(z4, s45, fma(z2, s23, s01));
-    const double c01 = fma(z, -1.38888888888741095749e-03, 4.16666666666666019037e-02);
-    const double c23 = fma(z, -2.75573143513906633035e-07, 2.48015872894767294178e-05);
-    const double c45 = fma(z, -1.13596475577881948265e-11, 2.08757232129817482790e-09);
-    const double pc = fma(z4, c45, fma(z2, c23, c01));
-    sn = fma(y * z, ps, y);
-    cs = fma(z2, pc, fma(z, -0.5, 1.0));
-#else
-    double ps = fma(z, 1.58969099521155010221e-10, -2.50507602534068634195e-08);
-    ps = fma(ps, z, 2.75573137070700676789e-06);
-    ps = fma(ps, z, -1.98412698298579493134e-04);
-    ps = fma(ps, z, 8.33333333332248946124e-03);
-    ps = fma(ps, z, -1.66666666666666324348e-01);
-    double pc = fma(z, -1.13596475577881948265e-11, 2.08757232129817482790e-09);
-    pc = fma(pc, z, -2.75573143513906633035e-07);
-    pc = fma(pc, z, 2.48015872894767294178e-05);
-    pc = fma(pc, z, -1.38888888888741095749e-03);
-    pc = fma(pc, z, 4.16666666666666019037e-02);
+    double ps = fma(z, tc.s[5], tc.s[4]);
+    ps = fma(ps, z, tc.s[3]);
+    ps = fma(ps, z, tc.s[2]);
+    ps = fma(ps, z, tc.s[1]);
+    ps = fma(ps, z, tc.s[0]);
+    double pc = fma(z, tc.c[5], tc.c[4]);
+    pc = fma(pc, z, tc.c[3]);
+    pc = fma(pc, z, tc.c[2]);
+    pc = fma(pc, z, tc.c[1]);
+    pc = fma(pc, z, tc.c[0]);
     sn = fma(y * z, ps, y);
     cs = fma(z * z, pc, fma(z, -0.5, 1.0));
-#endif
 }
 
 // s2 = sin^2 x and sc = sin x cos x -- the only trigonometric quantities the RHS needs (cos^2 enters
 // as 1 - s2).  Odd quadrant: sin^2 x = cos^2 y, sin x cos x = -sin y cos y (sign flip on the integer pipe).
-__device__ __forceinline__ void sin2_sincos(double x, double& s2, double& sc) {
+__device__ __forceinline__ void sin2_sincos(const TrigConsts& tc, double x, double& s2, double& sc) {
     double sn, cs;
     bool odd;
-    sincos_reduced(x, sn, cs, odd);
+    sincos_reduced(tc, x, sn, cs, odd);
     const double S = odd ? cs : sn;
     s2 = S * S;
     const double p = sn * cs;
@@ -117,7 +123,7 @@ __device__ __forceinline__ void sin2_sincos(double x, double& s2, double& sc) {
 __device__ __forceinline__ void rhs_kerr(const Hole& bh, double r, double th, double pr, double pth,
                                          double E, double L, Deriv& d) {
     double s2, sc;
-    sin2_sincos(th, s2, sc);
+    sin2_sincos(bh.tc, th, s2, sc);
     const double r2 = r * r;
     const double A = r2 + bh.a2;                       // r^2 + a^2
     const double a2s2 = bh.a2 * s2;
@@ -137,9 +143,9 @@ __device__ __forceinline__ void rhs_kerr(const Hole& bh, double r, double th, do
     const double q1 = W * ut;                          // alpha^2 (u^t)^2
     const double gL = (rho2 * iP2) * L;                // gamma^{phph} L
     const double G = gL * L;
-    const double grr = Delta * irho;                   // gamma^{rr}
+    const double pri = pr * irho;                      // p_r / rho^2
     d.t = ut;
-    d.r = grr * pr;
+    d.r = Delta * pri;                                 // gamma^{rr} p_r
     d.th = irho * pth;                                 // gamma^{thth} p_th
     d.ph = fma(omega, ut, gL);
     const double B = q1 + G;
@@ -148,7 +154,7 @@ __device__ __forceinline__ void rhs_kerr(const Hole& bh, double r, double th, do
     const double u1 = (ut * L) * mS;                   // u^t L 2Ma / Sigma
     const double r2x = r + r;
     const double Z = iSig * fma(u1, r2x, B);           // X / Sigma
-    const double br = fma(a2s2, Z, fma(q1, iDel, pr * (pr * irho)));
+    const double br = fma(a2s2, Z, fma(q1, iDel, pr * pri));
     const double rmM = r - bh.M;
     d.pr = fma(-rmM, br, fma(r2x * A, Z, fma(r, Y, -u1)));
     d.pth = sc * fma(-bh.a2, fma(Delta, Z, Y), G * is2);
@@ -159,7 +165,7 @@ __device__ __forceinline__ void rhs_kerr(const Hole& bh, double r, double th, do
 __device__ __forceinline__ void rhs_schwarzschild(const Hole& bh, double r, double th, double pr,
                                                   double pth, double E, double L, Deriv& d) {
     double s2, sc;
-    sin2_sincos(th, s2, sc);
+    sin2_sincos(bh.tc, th, s2, sc);
     const double r2 = r * r;
     const double Delta = fma(-bh.twoM, r, r2);         // r^2 alpha^2
     const double P2 = r2 * s2;

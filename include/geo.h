@@ -38,6 +38,9 @@ enum { GEO_ST_MAXSTEPS = 0, GEO_ST_CAPTURED = 1, GEO_ST_ESCAPED = 2, GEO_ST_NUME
 enum {
     GEO_FLAG_PLAIN_UPDATE = 1, /* y <- y + delta without the Kahan error term (P1)     */
     GEO_FLAG_STATIC_MAP = 2,   /* thread i integrates particle i; no work queue (for comparison) */
+    GEO_FLAG_CARTESIAN_SNAP = 8, /* snapshot components 1..3 hold (x, y, z) of eq.(7) PAPER.md:88-93 instead
+                                  of (r, theta, phi): with snap_mask = 0x0F a record is (t, x, y, z), the paper's
+                                  output format -- tau is implicit, slot j <-> tau = j*snapshot_every*h */
     GEO_FLAG_STAGED_SNAP = 4   /* snapshot records staged in shared memory and flushed by the warp with
                                   coalesced stores; default: each lane stores its record straight from
                                   registers with 256-bit stores (measured faster, profiles/)          */

@@ -43,7 +43,8 @@ namespace {
 
 enum { ORA_SCHWARZSCHILD = 0, ORA_KERR = 1 };
 enum { ORA_ST_MAXSTEPS = 0, ORA_ST_CAPTURED = 1, ORA_ST_ESCAPED = 2, ORA_ST_NUMERIC = 3 };
-enum { ORA_FLAG_PLAIN_UPDATE = 1 };
+enum { ORA_FLAG_PLAIN_UPDATE = 1,
+       ORA_FLAG_CARTESIAN_SNAP = 8 };   // snapshot components r, theta, phi -> x, y, z of eq.(7)
 
 template <class R> struct Hole { int metric; R M, a; };
 
@@ -187,15 +188,26 @@ template <class R> void kahan_add(R& y, R& c, R delta, bool plain) {
     y = tsum;
 }
 
+// Boyer-Lindquist -> Cartesian, eq.(7) PAPER.md:88-93 (the paper's output format):
+//   x = sqrt(r^2 + a^2) sin(th) cos(ph),  y = sqrt(r^2 + a^2) sin(th) sin(ph),  z = r cos(th).
+template <class R> void cartesian_eq7(R a, const State<R>& y, R& X, R& Y, R& Z) {
+    const R w = std::sqrt(y.r * y.r + a * a);
+    X = w * std::sin(y.th) * std::cos(y.ph);
+    Y = w * std::sin(y.th) * std::sin(y.ph);
+    Z = y.r * std::cos(y.th);
+}
+
 template <class R>
-void write_snapshot(const OutPtrs& o, int64_t i, int64_t slot, const State<R>& y) {
+void write_snapshot(const OutPtrs& o, int64_t i, int64_t slot, const State<R>& y, R a, bool cartesian) {
     if (!o.snapshots || slot >= o.snap_capacity) return;   // S3: drop, never overflow
     int ncomp = 0;
     for (int k = 0; k < 8; ++k) ncomp += (o.snap_mask >> k) & 1u;
     double* dst = o.snapshots + (i * o.snap_capacity + slot) * ncomp;
+    R xyz[3] = {y.r, y.th, y.ph};
+    if (cartesian) cartesian_eq7(a, y, xyz[0], xyz[1], xyz[2]);
     int j = 0;
     for (int k = 0; k < 8; ++k)
-        if ((o.snap_mask >> k) & 1u) dst[j++] = (double)component(y, k);
+        if ((o.snap_mask >> k) & 1u) dst[j++] = (double)((k >= 1 && k <= 3) ? xyz[k - 1] : component(y, k));
 }
 
 template <class R>
@@ -203,6 +215,7 @@ void integrate_one(const Hole<R>& bh, const double* state_in, int64_t n, int64_t
                    int64_t nsteps, const StopRule& st, int64_t snapshot_every, const OutPtrs& o) {
     const R kappa = st.kind == 0 ? R(1) : R(0);
     const bool plain = (st.flags & ORA_FLAG_PLAIN_UPDATE) != 0;
+    const bool cart = (st.flags & ORA_FLAG_CARTESIAN_SNAP) != 0;
     const R rc = (R)st.r_capture, re = (R)st.r_escape;
     const R half_pi = (R)1.5707963267948966;          // nearest double to pi/2 (reading B5)
 
@@ -227,7 +240,7 @@ void integrate_one(const Hole<R>& bh, const double* state_in, int64_t n, int64_t
     if (!(y.r >= rc)) status = ORA_ST_CAPTURED;
     else if (!finite6(y) || !std::isfinite(y.E)) status = ORA_ST_NUMERIC;
     else {
-        if (snapshot_every > 0) { write_snapshot(o, i, 0, y); snaps = 1; }   // S1: slot 0 = y0
+        if (snapshot_every > 0) { write_snapshot(o, i, 0, y, bh.a, cart); snaps = 1; }   // S1: slot 0 = y0
         if (y.r > re) status = ORA_ST_ESCAPED;
         else if (nsteps == 0) status = ORA_ST_MAXSTEPS;
     }
@@ -269,7 +282,7 @@ void integrate_one(const Hole<R>& bh, const double* state_in, int64_t n, int64_t
         y = yn; ct = nt; cr = nr; cth = nth; cph = nph; cpr = npr; cpth = npth;
         ++steps;
         if (snapshot_every > 0 && steps % snapshot_every == 0) {    // S1
-            write_snapshot(o, i, snaps, y);
+            write_snapshot(o, i, snaps, y, bh.a, cart);
             ++snaps;
         }
         if (y.r > re) status = ORA_ST_ESCAPED;                      // B3

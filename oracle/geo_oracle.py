@@ -20,6 +20,7 @@ SCHWARZSCHILD, KERR = 0, 1
 TIMELIKE, NULL = 0, 1
 ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC = 0, 1, 2, 3
 FLAG_PLAIN_UPDATE = 1
+FLAG_CARTESIAN_SNAP = 8      # snapshot components r, theta, phi -> x, y, z of eq.(7)
 
 
 class _Stop(C.Structure):

@@ -70,7 +70,7 @@ int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t 
     if (!std::isfinite(h) || h == 0.0) return fail(ctx, GEO_EINVAL, "h must be finite and non-zero");
     if (stop->kind != GEO_TIMELIKE && stop->kind != GEO_NULL) return fail(ctx, GEO_EINVAL, "stop.kind must be GEO_TIMELIKE or GEO_NULL");
     if (std::isnan(stop->r_capture) || std::isnan(stop->r_escape)) return fail(ctx, GEO_EINVAL, "stop radii must not be NaN");
-    if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_STAGED_SNAP)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
+    if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_STAGED_SNAP | GEO_FLAG_CARTESIAN_SNAP)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
     if (n == 0) return GEO_OK;
     if (!state_in || !out->final_state || !out->status || !out->steps_done) return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
     if (snapshot_every > 0) {
@@ -160,6 +160,7 @@ int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps
     p.bh.twoMa = 2.0 * ctx->M * ctx->a;
     p.bh.twoa2 = 2.0 * ctx->a * ctx->a;
     fill_trig_consts(p.bh.tc);
+    p.cartesian = (stop->flags & GEO_FLAG_CARTESIAN_SNAP) ? 1 : 0;
 
     cudaError_t e;
     if (lp.use_queue) {

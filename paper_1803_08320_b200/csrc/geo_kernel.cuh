@@ -35,6 +35,7 @@ struct Params {
     long long nsteps;
     double r_capture, r_escape, kappa;
     int use_queue;
+    int cartesian;      // snapshot records carry (x, y, z) of eq.(7) in place of (r, theta, phi)
     long long snap_every, snap_cap;
     unsigned snap_mask;
     int ncomp;
@@ -158,11 +159,13 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
     };
     auto emit_snapshot = [&]() {
         if (snaps < p.snap_cap) {   // S3: drop beyond capacity, keep counting
+            double c1 = r, c2 = th, c3 = ph;
+            if (p.cartesian) cartesian_eq7(bh.a2, r, th, ph, c1, c2, c3);
             if (SNAP == SNAP_DIRECT) {
-                store_record_global(my_snaps + (size_t)snaps * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
+                store_record_global(my_snaps + (size_t)snaps * p.ncomp, p.snap_mask, t, c1, c2, c3, E, pr, pth, L);
             } else {
                 if (staged == 0) stage_first = snaps;
-                store_masked(my_stage + staged * p.ncomp, p.snap_mask, t, r, th, ph, E, pr, pth, L);
+                store_masked(my_stage + staged * p.ncomp, p.snap_mask, t, c1, c2, c3, E, pr, pth, L);
                 ++staged;           // flushed by the warp at the top of the loop, or by finish()
             }
         }

@@ -215,6 +215,18 @@ __device__ __noinline__ double energy_3p1(const Hole& bh, double r, double th, d
     return sqrt(alpha2 * (kappa + g)) + omega * L;
 }
 
+// Boyer-Lindquist -> Cartesian, eq.(7) PAPER.md:88-93 -- the paper's output format, fused
+// into the snapshot writer.  Full-range libdevice sincos: phi grows without bound.
+__device__ __noinline__ void cartesian_eq7(double a2, double r, double th, double ph, double& x, double& y, double& z) {
+    double st, ct, sp, cp;
+    sincos(th, &st, &ct);
+    sincos(ph, &sp, &cp);
+    const double w = sqrt(r * r + a2) * st;
+    x = w * cp;
+    y = w * sp;
+    z = r * ct;
+}
+
 // |2H + kappa| with 2H = -alpha^2 (u^t)^2 + gamma^{ij} p_i p_j (B7 "health").
 __device__ __noinline__ double health_3p1(const Hole& bh, double r, double th, double pr, double pth,
                                           double E, double L, double kappa) {

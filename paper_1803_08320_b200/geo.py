@@ -16,7 +16,7 @@ SCHWARZSCHILD, KERR = 0, 1
 TIMELIKE, NULL = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, 1, 2, 3
 ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC = 0, 1, 2, 3
-FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_STAGED_SNAP = 1, 2, 4
+FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_STAGED_SNAP, FLAG_CARTESIAN_SNAP = 1, 2, 4, 8
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI

@@ -120,3 +120,29 @@ def test_config5_camera_subimage_with_snapshots(G, oracle, flags):
     cap = o["snapshots"].shape[1]
     valid = (np.arange(cap)[None, :] < o["snap_count"][:, None]) & cert[:, None]
     assert parity.rel_err(g["snapshots"], o["snapshots"])[valid].max() <= TOL_NULL
+
+
+# ------------------------------------------------------------------------------------------------------
+# paper-format (Cartesian, eq.(7)) snapshot records fused into the writer
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("flags", [8, 8 | 4])        # 8 = GEO_FLAG_CARTESIAN_SNAP, 4 = staged writer
+@pytest.mark.parametrize("mask", [0x0F, 0xFF])
+def test_cartesian_snapshots_kerr(G, oracle, flags, mask):
+    a = 0.9
+    st = W.kerr_bound(777, a, W.SEED_BASE + 2)
+    o = oracle.integrate(oracle.KERR, 1.0, a, st, 0.01, 5000, snapshot_every=250, snap_mask=mask,
+                         flags=oracle.FLAG_CARTESIAN_SNAP, nthreads=NCPU)
+    g = run_gpu(G, G.KERR, a, st, 0.01, 5000, flags=flags, snapshot_every=250, snap_mask=mask)
+    assert_timelike_parity(g, o)
+    assert_snapshots_match(g, o, TOL_TIMELIKE)
+
+
+def test_cartesian_snapshots_reproduce_the_printed_listing(G):
+    """the two printed particles, h = 0.1, records (t, x, y, z) straight from the GPU."""
+    golden = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "worked_example.txt")
+    rows = [[float(x) for x in ln.split()] for ln in open(golden) if ln.strip() and not ln.startswith("#")]
+    st = np.ascontiguousarray(np.array([[6.0, 1.5708, 0.0, 0.0, 0.0, 3.4641], [3.5, 1.5708, 0.0, 0.0, 0.0, 4.9497]]).T)
+    g = run_gpu(G, G.SCHWARZSCHILD, 0.0, st, 0.1, 2, flags=8, snapshot_every=1, snap_mask=0x0F)
+    for part, tau, t, x, y, z in rows:
+        rec = g["snapshots"][int(part) - 1, int(round(tau / 0.1))]
+        assert np.max(np.abs(rec - np.array([t, x, y, z]))) < 1.0e-4, (part, tau, rec)

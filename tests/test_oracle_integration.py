@@ -298,3 +298,29 @@ def test_invalid_arguments(oracle):
         oracle.integrate(oracle.SCHWARZSCHILD, 1.0, 0.3, st, 0.01, 1)
     with pytest.raises(ValueError):
         oracle.integrate(oracle.KERR, 1.0, 0.5, st, 0.0, 1)
+
+
+def test_cartesian_snapshots_are_the_papers_output_format(oracle):
+    """snapshot records in the paper's output format (PAPER.md:318 'numerical solutions
+    are stored in Cartesian coordinates'), eq.(7) PAPER.md:88-93.  Pins: the digits of the printed
+    listing PAPER.md:278-316 (columns tau t x y z, reading G6) read straight from the oracle's records,
+    and the oblate-spheroidal identity (x^2+y^2)/(r^2+a^2) + z^2/r^2 = 1 with tan(phi) = y/x in Kerr."""
+    ics = _rows("ic_table.txt")[:2]
+    st = _st([[r, 1.5708, 0.0, 0.0, 0.0, pph] for r, _, pph in ics])
+    res = oracle.integrate(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.1, 2, snapshot_every=1, snap_mask=0x0F,
+                           flags=oracle.FLAG_CARTESIAN_SNAP)
+    for part, tau, t, x, y, z in _rows("worked_example.txt"):
+        rec = res["snapshots"][int(part) - 1, int(round(tau / 0.1))]          # (t, x, y, z)
+        assert np.max(np.abs(rec - np.array([t, x, y, z]))) < 1.0e-4, (part, tau, rec)
+    a = 0.9
+    st = W.kerr_bound(40, a, W.SEED_BASE + 2)
+    bl = oracle.integrate(oracle.KERR, 1.0, a, st, 0.01, 3000, snapshot_every=500)["snapshots"]
+    ca = oracle.integrate(oracle.KERR, 1.0, a, st, 0.01, 3000, snapshot_every=500,
+                          flags=oracle.FLAG_CARTESIAN_SNAP)["snapshots"]
+    r, ph = bl[..., 1], bl[..., 3]
+    x, y, z = ca[..., 1], ca[..., 2], ca[..., 3]
+    assert np.max(np.abs((x * x + y * y) / (r * r + a * a) + z * z / (r * r) - 1.0)) < 1e-13
+    assert np.max(np.abs(np.arctan2(y, x) - np.arctan2(np.sin(ph), np.cos(ph)))) < 1e-12
+    for k in (0, 4, 5, 6, 7):                                              # the other components are untouched
+        assert np.array_equal(bl[..., k], ca[..., k])
+    assert np.all(np.sign(z) == np.sign(np.cos(bl[..., 2])))

@@ -86,9 +86,12 @@ int geo_create(geo_ctx **ctx, int metric, double M, double a);
 int geo_integrate(geo_ctx *ctx, const double *state_in, int64_t n, double h, int64_t nsteps,
                   const geo_stop *stop, int64_t snapshot_every, const geo_out *out, void *cuda_stream);
 
-/* Same operation with HOST buffers (pageable or pinned): copies state_in to the device, integrates,
- * copies every non-NULL output back and synchronises before returning.  Device scratch is owned by
- * the ctx and reused between calls. */
+/* Same operation with HOST buffers (pageable or pinned; pinned lets the copies overlap the kernels):
+ * copies state_in to the device, integrates, copies every non-NULL output back and synchronises before
+ * returning.  Large jobs are cut into particle chunks that are double-buffered on two streams, so the
+ * D2H of one chunk overlaps the integration of the next (the paper's bottleneck).
+ * Snapshot slots >= snap_count[i] are returned as NaN (all-ones bit pattern).  Device scratch is owned
+ * by the ctx and reused between calls. */
 int geo_integrate_host(geo_ctx *ctx, const double *state_in, int64_t n, double h, int64_t nsteps,
                        const geo_stop *stop, int64_t snapshot_every, const geo_out *out);
 

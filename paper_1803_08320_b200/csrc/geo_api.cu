@@ -15,11 +15,11 @@ struct geo_ctx {
     double M, a;
     int device;
     int sm_count;
-    unsigned long long* counter;   // device: work-queue head
+    unsigned long long* counter;   // device: work-queue heads [2] (one per host-path slot; geo_integrate uses [0])
     // device scratch of geo_integrate_host (grow-only)
     void* scratch;
     size_t scratch_bytes;
-    cudaStream_t host_stream;
+    cudaStream_t host_stream[2];
     char err[256];
 };
 
@@ -123,7 +123,7 @@ int plan_launch(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, 
 }
 
 int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
-           int64_t snapshot_every, const geo_out* out, cudaStream_t stream) {
+           int64_t snapshot_every, const geo_out* out, cudaStream_t stream, unsigned long long* counter) {
     const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
     LaunchPlan lp;
     int rc = plan_launch(ctx, n, stop->flags, snapshot_every, ncomp, &lp);
@@ -152,7 +152,7 @@ int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps
     p.health = out->health;
     p.snaps = out->snapshots;
     p.snap_count = out->snap_count;
-    p.counter = ctx->counter;
+    p.counter = counter;
     p.bh.M = ctx->M;
     p.bh.a = ctx->a;
     p.bh.a2 = ctx->a * ctx->a;
@@ -164,7 +164,7 @@ int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps
 
     cudaError_t e;
     if (lp.use_queue) {
-        e = cudaMemsetAsync(ctx->counter, 0, sizeof(unsigned long long), stream);
+        e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
         if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
     }
     lp.fn<<<lp.grid, kBlock, lp.smem, stream>>>(p);
@@ -193,7 +193,7 @@ int geo_create(geo_ctx** out_ctx, int metric, double M, double a) {
     ctx->a = a;
     cudaError_t e = cudaGetDevice(&ctx->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->counter, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->counter, 2 * sizeof(unsigned long long));
     if (e != cudaSuccess) {
         int rc = e == cudaErrorMemoryAllocation ? GEO_ENOMEM : GEO_ECUDA;
         delete ctx;
@@ -205,7 +205,8 @@ int geo_create(geo_ctx** out_ctx, int metric, double M, double a) {
 
 void geo_destroy(geo_ctx* ctx) {
     if (!ctx) return;
-    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    for (int k = 0; k < 2; ++k)
+        if (ctx->host_stream[k]) cudaStreamDestroy(ctx->host_stream[k]);
     if (ctx->scratch) cudaFree(ctx->scratch);
     if (ctx->counter) cudaFree(ctx->counter);
     delete ctx;
@@ -222,25 +223,42 @@ int geo_integrate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int
                   const geo_stop* stop, int64_t snapshot_every, const geo_out* out, void* cuda_stream) {
     int rc = validate(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, true);
     if (rc != GEO_OK || n == 0) return rc;
-    return launch(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, (cudaStream_t)cuda_stream);
+    return launch(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, (cudaStream_t)cuda_stream, ctx->counter);
 }
 
+// Host-buffer entry point.  Small jobs: one H2D, one launch, one D2H.  Jobs whose buffers exceed
+// kHostChunkBytes are cut into particle chunks that ping-pong between two device scratch slots on two
+// streams, so that the D2H of chunk k (the paper's measured bottleneck) overlaps the
+// kernel of chunk k+1, and the next kernel's CTAs fill the SMs the previous kernel's tail leaves idle.
 int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t nsteps,
                        const geo_stop* stop, int64_t snapshot_every, const geo_out* out) {
     int rc = validate(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, false);
     if (rc != GEO_OK || n == 0) return rc;
     const size_t N = (size_t)n;
     const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
-    const size_t b_in = align256(6 * N * 8), b_fin = align256(8 * N * 8), b_st = align256(N * 4),
-                 b_steps = align256(N * 8), b_eq = out->eq_cross_r ? align256(N * 8) : 0,
-                 b_he = out->health ? align256(N * 8) : 0,
-                 b_sn = snapshot_every > 0 ? align256(N * (size_t)out->snap_capacity * ncomp * 8) : 0,
-                 b_sc = snapshot_every > 0 ? align256(N * 4) : 0;
-    const size_t total = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_sn + b_sc;
+    const size_t snap_pp = snapshot_every > 0 ? (size_t)out->snap_capacity * ncomp * 8 : 0;   // bytes per particle
+    const size_t bytes_pp = 48 + 64 + 4 + 8 + (out->eq_cross_r ? 8 : 0) + (out->health ? 8 : 0) + snap_pp + (snap_pp ? 4 : 0);
+    // chunking: only when the transfers are large, never below ~2 waves of resident lanes per chunk
+    const size_t kHostChunkBytes = (size_t)768 << 20;
+    const size_t min_chunk = (size_t)ctx->sm_count * 5 * kBlock * 2;
+    size_t nchunks = (N * bytes_pp + kHostChunkBytes - 1) / kHostChunkBytes;
+    if (nchunks > N / min_chunk) nchunks = N / min_chunk;
+    if (nchunks < 1) nchunks = 1;
+    const size_t C = ((N + nchunks - 1) / nchunks + 31) & ~(size_t)31;      // particles per chunk
+    const int nslots = nchunks > 1 ? 2 : 1;
+
+    const size_t b_in = align256(6 * C * 8), b_fin = align256(8 * C * 8), b_st = align256(C * 4),
+                 b_steps = align256(C * 8), b_eq = out->eq_cross_r ? align256(C * 8) : 0,
+                 b_he = out->health ? align256(C * 8) : 0, b_sn = align256(C * snap_pp),
+                 b_sc = snap_pp ? align256(C * 4) : 0;
+    const size_t slot_bytes = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_sn + b_sc;
+    const size_t total = slot_bytes * nslots;
     cudaError_t e;
-    if (!ctx->host_stream) {
-        e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking);
-        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamCreate");
+    for (int k = 0; k < nslots; ++k) {
+        if (!ctx->host_stream[k]) {
+            e = cudaStreamCreateWithFlags(&ctx->host_stream[k], cudaStreamNonBlocking);
+            if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamCreate");
+        }
     }
     if (total > ctx->scratch_bytes) {
         if (ctx->scratch) cudaFree(ctx->scratch);
@@ -250,38 +268,48 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
         if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMalloc(scratch)");
         ctx->scratch_bytes = total;
     }
-    char* base = static_cast<char*>(ctx->scratch);
-    size_t off = 0;
-    auto take = [&](size_t b) { char* q = b ? base + off : nullptr; off += b; return q; };
-    double* d_in = (double*)take(b_in);
-    geo_out d = *out;
-    d.final_state = (double*)take(b_fin);
-    d.status = (int32_t*)take(b_st);
-    d.steps_done = (int64_t*)take(b_steps);
-    d.eq_cross_r = (double*)take(b_eq);
-    d.health = (double*)take(b_he);
-    d.snapshots = (double*)take(b_sn);
-    d.snap_count = (int32_t*)take(b_sc);
-    cudaStream_t s = ctx->host_stream;
-    e = cudaMemcpyAsync(d_in, state_in, 6 * N * 8, cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return fail_cuda(ctx, e, "H2D state_in");
-    if (d.snapshots) {
-        // slots >= snap_count[i] are documented as untouched: carry the caller's contents over
-        e = cudaMemcpyAsync(d.snapshots, out->snapshots, N * (size_t)out->snap_capacity * ncomp * 8, cudaMemcpyHostToDevice, s);
-        if (e != cudaSuccess) return fail_cuda(ctx, e, "H2D snapshots");
+    for (size_t k = 0, lo = 0; lo < N; ++k, lo += C) {
+        const size_t c = N - lo < C ? N - lo : C;
+        const int slot = (int)(k % nslots);
+        cudaStream_t s = ctx->host_stream[slot];
+        char* base = static_cast<char*>(ctx->scratch) + slot_bytes * slot;
+        size_t off = 0;
+        auto take = [&](size_t b) { char* q = b ? base + off : nullptr; off += b; return q; };
+        double* d_in = (double*)take(b_in);
+        geo_out d = *out;
+        d.final_state = (double*)take(b_fin);
+        d.status = (int32_t*)take(b_st);
+        d.steps_done = (int64_t*)take(b_steps);
+        d.eq_cross_r = (double*)take(b_eq);
+        d.health = (double*)take(b_he);
+        d.snapshots = (double*)take(b_sn);
+        d.snap_count = (int32_t*)take(b_sc);
+        e = cudaSuccess;
+        for (int q = 0; q < 6 && e == cudaSuccess; ++q)      // SoA [6][n] -> [6][c]
+            e = cudaMemcpyAsync(d_in + q * c, state_in + q * N + lo, c * 8, cudaMemcpyHostToDevice, s);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "H2D state_in");
+        if (d.snapshots) {
+            // slots >= snap_count[i] come back as NaN (all-ones pattern)
+            e = cudaMemsetAsync(d.snapshots, 0xFF, c * snap_pp, s);
+            if (e != cudaSuccess) return fail_cuda(ctx, e, "memset snapshots");
+        }
+        rc = launch(ctx, d_in, (int64_t)c, h, nsteps, stop, snapshot_every, &d, s, ctx->counter + slot);
+        if (rc != GEO_OK) return rc;
+        for (int q = 0; q < 8 && e == cudaSuccess; ++q)      // SoA [8][c] -> [8][n]
+            e = cudaMemcpyAsync(out->final_state + q * N + lo, d.final_state + q * c, c * 8, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(out->status + lo, d.status, c * 4, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(out->steps_done + lo, d.steps_done, c * 8, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess && d.eq_cross_r) e = cudaMemcpyAsync(out->eq_cross_r + lo, d.eq_cross_r, c * 8, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess && d.health) e = cudaMemcpyAsync(out->health + lo, d.health, c * 8, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess && d.snapshots)
+            e = cudaMemcpyAsync(reinterpret_cast<char*>(out->snapshots) + lo * snap_pp, d.snapshots, c * snap_pp, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess && d.snap_count) e = cudaMemcpyAsync(out->snap_count + lo, d.snap_count, c * 4, cudaMemcpyDeviceToHost, s);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "D2H outputs");
     }
-    rc = launch(ctx, d_in, n, h, nsteps, stop, snapshot_every, &d, s);
-    if (rc != GEO_OK) return rc;
-    e = cudaMemcpyAsync(out->final_state, d.final_state, 8 * N * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out->status, d.status, N * 4, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out->steps_done, d.steps_done, N * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess && d.eq_cross_r) e = cudaMemcpyAsync(out->eq_cross_r, d.eq_cross_r, N * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess && d.health) e = cudaMemcpyAsync(out->health, d.health, N * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess && d.snapshots) e = cudaMemcpyAsync(out->snapshots, d.snapshots, N * (size_t)out->snap_capacity * ncomp * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess && d.snap_count) e = cudaMemcpyAsync(out->snap_count, d.snap_count, N * 4, cudaMemcpyDeviceToHost, s);
-    if (e != cudaSuccess) return fail_cuda(ctx, e, "D2H outputs");
-    e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
+    for (int k = 0; k < nslots; ++k) {
+        e = cudaStreamSynchronize(ctx->host_stream[k]);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
+    }
     return GEO_OK;
 }
 

@@ -117,6 +117,18 @@ def test_host_entry_point_is_bitwise_equal_to_device_entry_point(G):
         assert np.array_equal(a[k], b[k], equal_nan=True), k
 
 
+def test_host_entry_point_chunked_pipeline_is_bitwise_equal(G):
+    """A job above the host path's chunk threshold (1.05 GB of snapshots, 400 003 particles -> two
+    double-buffered chunks, ragged last chunk) returns what the one-launch device path returns."""
+    st = W.circular_schwarzschild(400003, W.SEED_BASE + 7)
+    kw = dict(snapshot_every=1, snap_mask=0xFF)
+    a = run_gpu(G, G.SCHWARZSCHILD, 0.0, st, 0.01, 40, **kw)
+    b = run_gpu(G, G.SCHWARZSCHILD, 0.0, st, 0.01, 40, host=True, **kw)
+    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health", "snapshots", "snap_count"):
+        assert np.array_equal(a[k], b[k], equal_nan=True), k
+    assert (b["snap_count"] == 41).all() and not np.isnan(b["snapshots"]).any()
+
+
 def test_queue_and_static_mapping_and_reruns_are_bitwise_identical(G):
     """No arithmetic crosses lanes: results do not depend on which lane integrated a particle."""
     a = 0.998

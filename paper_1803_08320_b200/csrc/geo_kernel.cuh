@@ -108,6 +108,41 @@ __host__ __device__ __forceinline__ int stage_stride(int ncomp) {
     return (d & 1) ? d : d + 1;
 }
 
+// k1 + 2 k2 + 2 k3 + k4 and the capture guard of one RK4 step with a full sin/cos evaluation at every
+// stage point: the out-of-line path of steps whose stage angles move by >= 2^-7 rad (see stage_trig).
+template <bool KERR>
+__device__ __noinline__ void rk4_sum_full(const Params& p, double r, double th, double pr, double pth,
+                                          double E, double L, double* acc, int* captured) {
+    const Hole& bh = p.bh;
+    Deriv k;
+    double s2, sc, sr, sth, spr, spth;
+    sin2_sincos(bh.tc, th, s2, sc);
+    rhs<KERR>(bh, r, s2, sc, pr, pth, E, L, k);
+    double at = k.t, ar = k.r, ath = k.th, aph = k.ph, apr = k.pr, apth = k.pth;
+    sr = fma(p.h_half, k.r, r); sth = fma(p.h_half, k.th, th);
+    spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
+    bool cap = !(sr >= p.r_capture);
+    sin2_sincos(bh.tc, sth, s2, sc);
+    rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
+    at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
+    aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
+    sr = fma(p.h_half, k.r, r); sth = fma(p.h_half, k.th, th);
+    spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
+    cap |= !(sr >= p.r_capture);
+    sin2_sincos(bh.tc, sth, s2, sc);
+    rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
+    at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
+    aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
+    sr = fma(p.h, k.r, r); sth = fma(p.h, k.th, th);
+    spr = fma(p.h, k.pr, pr); spth = fma(p.h, k.pth, pth);
+    cap |= !(sr >= p.r_capture);
+    sin2_sincos(bh.tc, sth, s2, sc);
+    rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
+    acc[0] = at + k.t; acc[1] = ar + k.r; acc[2] = ath + k.th;
+    acc[3] = aph + k.ph; acc[4] = apr + k.pr; acc[5] = apth + k.pth;
+    *captured = cap ? 1 : 0;
+}
+
 template <bool KERR, int SNAP, bool PLAIN>
 __global__ void __launch_bounds__(kBlock, SNAP == SNAP_NONE ? GEO_MIN_CTAS_PER_SM : 4)
 geo_rk4_kernel(const __grid_constant__ Params p) {
@@ -221,6 +256,20 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         if (i < p.n) begin(i);
     }
 
+#if defined(GEO_CONST_IN_REGS)
+    // experiment: keep sin/cos coefficients in vector registers (opaque to rematerialisation)
+    TrigConsts tcr = bh.tc;
+#if GEO_CONST_IN_REGS >= 2
+    asm volatile("" : "+d"(tcr.two_over_pi), "+d"(tcr.pio2_hi), "+d"(tcr.pio2_lo));
+    asm volatile("" : "+d"(tcr.s[2]), "+d"(tcr.s[3]), "+d"(tcr.s[4]), "+d"(tcr.s[5]));
+    asm volatile("" : "+d"(tcr.c[2]), "+d"(tcr.c[3]), "+d"(tcr.c[4]), "+d"(tcr.c[5]));
+#endif
+    asm volatile("" : "+d"(tcr.s[0]), "+d"(tcr.s[1]), "+d"(tcr.c[0]), "+d"(tcr.c[1]));
+#define GEO_TC tcr
+#else
+#define GEO_TC bh.tc
+#endif
+
     for (;;) {
         // --- A5: refill idle lanes from the queue ------------------------------------------------
         unsigned idle = __ballot_sync(kFull, !active);
@@ -252,29 +301,42 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         // --- A3: one classical RK4 step, every lane (idle lanes compute on stale state) ----------
         Deriv k;
         double at, ar, ath, aph, apr, apth;      // k1 + 2 k2 + 2 k3 + k4
-        double sr, sth, spr, spth;               // stage point (t, phi are cyclic: not needed)
-        rhs<KERR>(bh, r, th, pr, pth, E, L, k);
+        double sr, spr, spth;                    // stage point (t, phi are cyclic: not needed)
+        double S, C, s2, sc, dang; bool coarse = false;              // sin/cos at the base point; sin^2, sin cos at the stage point
+        sincos_common_sign(GEO_TC, th, S, C);
+        s2 = S * S; sc = S * C;
+        rhs<KERR>(bh, r, s2, sc, pr, pth, E, L, k);
         at = k.t; ar = k.r; ath = k.th; aph = k.ph; apr = k.pr; apth = k.pth;
-        sr = fma(p.h_half, k.r, r); sth = fma(p.h_half, k.th, th);
+        sr = fma(p.h_half, k.r, r); dang = p.h_half * k.th;
         spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
         bool cap = !(sr >= p.r_capture);                                   // B2: stage point 2
 
-        rhs<KERR>(bh, sr, sth, spr, spth, E, L, k);
+        stage_trig(GEO_TC, S, C, dang, s2, sc, coarse);
+        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
         at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
         aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
-        sr = fma(p.h_half, k.r, r); sth = fma(p.h_half, k.th, th);
+        sr = fma(p.h_half, k.r, r); dang = p.h_half * k.th;
         spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
         cap |= !(sr >= p.r_capture);                                       // stage point 3
 
-        rhs<KERR>(bh, sr, sth, spr, spth, E, L, k);
+        stage_trig(GEO_TC, S, C, dang, s2, sc, coarse);
+        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
         at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
         aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
-        sr = fma(p.h, k.r, r); sth = fma(p.h, k.th, th);
+        sr = fma(p.h, k.r, r); dang = p.h * k.th;
         spr = fma(p.h, k.pr, pr); spth = fma(p.h, k.pth, pth);
         cap |= !(sr >= p.r_capture);                                       // stage point 4
 
-        rhs<KERR>(bh, sr, sth, spr, spth, E, L, k);
+        stage_trig(GEO_TC, S, C, dang, s2, sc, coarse);
+        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
         at += k.t; ar += k.r; ath += k.th; aph += k.ph; apr += k.pr; apth += k.pth;
+        if (__builtin_expect(coarse, 0)) {       // a stage angle moved by >= 2^-7 rad: full sin/cos path
+            double acc[6];
+            int c;
+            rk4_sum_full<KERR>(p, r, th, pr, pth, E, L, acc, &c);
+            at = acc[0]; ar = acc[1]; ath = acc[2]; aph = acc[3]; apr = acc[4]; apth = acc[5];
+            cap = c != 0;
+        }
 
         double nt, nr, nth, nph, npr, npth, dt, dr, dth, dph, dpr, dpth;
         kahan<PLAIN>(t, ct, p.h_sixth, at, nt, dt);

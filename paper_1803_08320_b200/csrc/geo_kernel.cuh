@@ -17,10 +17,11 @@
 namespace geo {
 
 constexpr int kBlock = 128;
-// Resident CTAs per SM the register allocation is bounded for: 5 CTAs x 128 threads = 20 warps/SM at
-// <= 96 registers (measured +3 % over 4 CTAs at 126 registers, profiles/r01_*).
+// Resident CTAs per SM the register allocation is bounded for: 4 CTAs x 128 threads = 16 warps/SM at
+// <= 128 registers.  The kernel is bound by issue slots (2 per FP64 instruction + 1 per other), not by
+// latency, so a fifth CTA at <= 96 registers only adds spill instructions (measured -8 %).
 #ifndef GEO_MIN_CTAS_PER_SM
-#define GEO_MIN_CTAS_PER_SM 5
+#define GEO_MIN_CTAS_PER_SM 4
 #endif
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kStageSlots = 4;   // snapshot records staged per lane before a bulk store

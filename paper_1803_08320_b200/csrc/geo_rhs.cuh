@@ -162,9 +162,12 @@ __device__ __forceinline__ void rhs_kerr(const Hole& bh, double r, double s2, do
     const double rho2 = A - a2s2;                      // r^2 + a^2 cos^2
     const double Delta = fma(-bh.twoM, r, A);
     const double Sigma = fma(A, A, -(a2s2 * Delta));
-    // two reciprocals give 1/rho^2, 1/Delta, 1/Sigma, 1/sin^2
-    const double iP1 = rcp_nr(rho2 * Delta);           // 1/(rho^2 Delta)
-    const double iP2 = rcp_nr(Sigma * s2);             // 1/(Sigma sin^2)
+    // one reciprocal gives 1/rho^2, 1/Delta, 1/Sigma, 1/sin^2 (issue slots are the bound: a second
+    // MUFU + zero-extension costs as much as the two multiplications that split the product)
+    const double P1 = rho2 * Delta, P2 = Sigma * s2;
+    const double iP = rcp_nr(P1 * P2);
+    const double iP1 = iP * P2;                        // 1/(rho^2 Delta)
+    const double iP2 = iP * P1;                        // 1/(Sigma sin^2)
     const double irho = iP1 * Delta, iDel = iP1 * rho2;
     const double iSig = iP2 * s2, is2 = iP2 * Sigma;
     // lapse, shift, 3-metric (eq.(8))

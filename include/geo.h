@@ -78,7 +78,7 @@ typedef struct geo_out {
  * requires a == 0.  Allocates a few bytes of device memory on the current CUDA device. */
 int geo_create(geo_ctx **ctx, int metric, double M, double a);
 
-/* Integrate n geodesics for at most nsteps RK4 steps of size h (h < 0 integrates backwards in tau).
+/* Integrate n geodesics for at most nsteps (< 2^31) RK4 steps of size h (h < 0 integrates backwards in tau).
  * state_in: DEVICE, SoA [6][n] = (r, theta, phi, u_r, u_theta, u_phi) (covariant); t starts at 0 and
  * p_t is derived from the mass shell eq.(5) in 3+1 variables.  snapshot_every = 0: no snapshots.
  * cuda_stream: a cudaStream_t (NULL = default stream).  Enqueue-only: outputs are valid after the

@@ -67,6 +67,7 @@ int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t 
     ctx->err[0] = 0;
     if (!stop || !out) return fail(ctx, GEO_EINVAL, "stop and out must not be NULL");
     if (n < 0 || nsteps < 0 || snapshot_every < 0) return fail(ctx, GEO_EINVAL, "n, nsteps, snapshot_every must be >= 0");
+    if (nsteps > 0x7fffffffLL) return fail(ctx, GEO_EINVAL, "nsteps must be < 2^31");
     if (!std::isfinite(h) || h == 0.0) return fail(ctx, GEO_EINVAL, "h must be finite and non-zero");
     if (stop->kind != GEO_TIMELIKE && stop->kind != GEO_NULL) return fail(ctx, GEO_EINVAL, "stop.kind must be GEO_TIMELIKE or GEO_NULL");
     if (std::isnan(stop->r_capture) || std::isnan(stop->r_escape)) return fail(ctx, GEO_EINVAL, "stop radii must not be NaN");
@@ -136,12 +137,12 @@ int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps
     p.h = h;
     p.h_half = h / 2.0;
     p.h_sixth = h / 6.0;
-    p.nsteps = nsteps;
+    p.nsteps = (int)nsteps;
     p.r_capture = stop->r_capture;
     p.r_escape = stop->r_escape;
     p.kappa = stop->kind == GEO_TIMELIKE ? 1.0 : 0.0;
     p.use_queue = lp.use_queue;
-    p.snap_every = snapshot_every;
+    p.snap_every = (int)(snapshot_every > 0x7fffffffLL ? 0x7fffffffLL : snapshot_every);
     p.snap_cap = snapshot_every > 0 ? out->snap_capacity : 0;
     p.snap_mask = snapshot_every > 0 ? (out->snap_mask & 0xFFu) : 0;
     p.ncomp = ncomp;

@@ -33,11 +33,12 @@ struct Params {
     const double* in;   // [6][n]
     long long n;
     double h, h_half, h_sixth;
-    long long nsteps;
+    int nsteps;         // < 2^31 (validated by the host): 32-bit counters in the hot loop
     double r_capture, r_escape, kappa;
     int use_queue;
     int cartesian;      // snapshot records carry (x, y, z) of eq.(7) in place of (r, theta, phi)
-    long long snap_every, snap_cap;
+    int snap_every;     // clamped to 2^31-1 by the host (unreachable beyond nsteps anyway)
+    long long snap_cap;
     unsigned snap_mask;
     int ncomp;
     double* fin;        // [8][n]
@@ -157,7 +158,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
     bool exhausted = !p.use_queue;
     double t = 0, r = 0, th = 0, ph = 0, pr = 0, pth = 0, E = 0, L = 0;
     double ct = 0, cr = 0, cth = 0, cph = 0, cpr = 0, cpth = 0;
-    long long steps = 0, snap_ctr = 0;
+    int steps = 0, snap_ctr = 0;
     int snaps = 0, staged = 0, stage_first = 0;   // staged records hold slots [stage_first, stage_first+staged)
     double eqc = 0;
     bool crossed = false;
@@ -209,7 +210,8 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
     };
     auto finish = [&](int st) {
         if (SNAP == SNAP_STAGED) flush_stage();
-        const long long n = p.n;
+        long long n = p.n;
+        asm volatile("" : "+l"(n));   // opaque: keeps the record's address arithmetic inside this cold path
         p.fin[0 * n + idx] = t;
         p.fin[1 * n + idx] = r;
         p.fin[2 * n + idx] = th;
@@ -219,7 +221,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         p.fin[6 * n + idx] = pth;
         p.fin[7 * n + idx] = L;
         p.status[idx] = st;
-        p.steps_done[idx] = steps;
+        p.steps_done[idx] = (long long)steps;
         if (p.eq_cross_r) p.eq_cross_r[idx] = crossed ? eqc : __longlong_as_double(0x7ff8000000000000LL);
         if (p.health) p.health[idx] = health_3p1(bh, r, th, pr, pth, E, L, p.kappa);
         if (SNAP != SNAP_NONE) p.snap_count[idx] = snaps;

@@ -37,11 +37,15 @@ from paper_1803_08320_b200 import workloads as W  # noqa: E402
 
 METRIC = "geodesic RK4 steps/sec (FP64, 1xB200)"
 UNIT = "geodesic-steps/s"
-# Static SASS counts of one RK4 step of the hot loop (python -m paper_1803_08320_b200.sass_count):
-# flop = 2*DFMA + DMUL + DADD; pipe = DFMA + DMUL + DADD + DSETP.  Refreshed by sass_count at run time
-# when cuobjdump is available; these are the fallback.
-FLOP_PER_STEP = {"kerr": 645.0, "schwarzschild": 425.0}
-PIPE_INSTR_PER_STEP = {"kerr": 458.0, "schwarzschild": 289.0}
+# EXECUTED FP64 instructions per RK4 step of one geodesic (per thread): dynamic counts from ncu's
+# per-instruction "Instructions Executed" of the hot kernel divided by the warp-steps of the launch
+# (profiles/r01_config4_v3.md: DFMA 140, DMUL 143, DADD 42, DSETP 6 for Kerr).  flop = 2*DFMA + DMUL + DADD;
+# pipe = all four.  The static SASS count of the loop (sass_count.py, an upper bound that includes the
+# rarely executed blocks inside the loop's address range) is printed beside them as a cross-check.
+FLOP_PER_STEP = {"kerr": 465.0, "schwarzschild": 397.0}
+PIPE_INSTR_PER_STEP = {"kerr": 331.0, "schwarzschild": 273.0}
+OTHER_INSTR_PER_STEP = {"kerr": 104.0}     # non-FP64 instructions per step, same ncu capture
+FLOP_COUNT_SOURCE = {"kerr": "ncu dynamic count (profiles/r01_config4_v3.md)", "schwarzschild": "static SASS count"}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
 # declared algorithmic work of one Kerr RK4 step (4 RHS + compensated update).
 F_ALG_SURVEY = {"kerr": 800.0}
@@ -64,6 +68,20 @@ def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dic
         return dict(name=f"configs[{k - 1}] Kerr a={a} bound timelike", metric="kerr", a=a, st=st, h=0.01,
                     nsteps=100000 if name == "config2" else 10000, snapshot_every=1000 if name == "config2" else 0,
                     snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf)
+    if name in ("paper_t4", "paper_t3"):
+        # the paper's own performance test (section 6.4): "random" timelike geodesics around
+        # Kerr a = 0.5, t_f = 1000, h = 0.1 (10^4 RK4 steps); its initial conditions are unpublished, the
+        # bound-orbit generator of configs 2/4 stands in.  Table 4: 10 000 geodesics, no
+        # output, 27.066675 s on a GTX 960M.  Table 3: 50 000 geodesics with the solution
+        # of EVERY step copied to the host and written out (t, x, y, z per step), 35.6253648 min.
+        n = n_override or (10000 if name == "paper_t4" else 50000)
+        st = W.kerr_bound(n, 0.5, W.SEED_BASE + 8 + 1000 * rank, nthreads=nthreads)
+        t3 = name == "paper_t3"
+        return dict(name=("paper Table 3: 50 000 Kerr a=0.5 geodesics, every step output in the paper's format" if t3 else
+                          "paper Table 4: 10 000 Kerr a=0.5 geodesics, no output"), metric="kerr", a=0.5, st=st, h=0.1,
+                    nsteps=10000, snapshot_every=1 if t3 else 0, snap_mask=0x0F, kind=0, r_capture=-np.inf, r_escape=np.inf,
+                    flags=8 if t3 else 0,      # GEO_FLAG_CARTESIAN_SNAP
+                    paper_steps_per_s=(50000 * 1e4 / (35.6253648 * 60.0)) if t3 else (10000 * 1e4 / 27.066675))
     if name == "snapbench":
         # SURVEY.md 8(d) snapshot-writer microbenchmark: cheap RHS, a record of all 8 components EVERY step
         n = n_override or (1 << 22)
@@ -137,7 +155,7 @@ def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> di
     sub = np.ascontiguousarray(st[:, :m])
     metric = geo_oracle.KERR if wl["metric"] == "kerr" else geo_oracle.SCHWARZSCHILD
     kw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores,
-              snapshot_every=wl["snapshot_every"], snap_mask=wl["snap_mask"])
+              snapshot_every=wl["snapshot_every"], snap_mask=wl["snap_mask"], flags=wl.get("flags", 0))
     times, done = [], 0
     for i in range(warmup + steps):
         t0 = time.perf_counter()
@@ -173,13 +191,15 @@ def run_reference(args, rank: int, world: int) -> None:
     print(json.dumps(line), flush=True)
 
 
-def flop_counts(metric: str) -> tuple[float, float, str]:
+def flop_counts(metric: str) -> tuple[float, float, str, dict | None]:
+    static = None
     try:
         from paper_1803_08320_b200 import sass_count
         c = sass_count.count("ILb1ELi0ELb0" if metric == "kerr" else "ILb0ELi0ELb0")
-        return float(c["flop"]), float(c["fp64_pipe"]), "sass_count (live)"
+        static = {"flop": c["flop"], "fp64_pipe": c["fp64_pipe"]}
     except Exception:
-        return FLOP_PER_STEP[metric], PIPE_INSTR_PER_STEP[metric], "sass_count (stored)"
+        pass
+    return FLOP_PER_STEP[metric], PIPE_INSTR_PER_STEP[metric], FLOP_COUNT_SOURCE[metric], static
 
 
 def main() -> None:
@@ -188,7 +208,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "snapbench"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "snapbench", "paper_t3", "paper_t4"])
     ap.add_argument("--n", type=int, default=None, help="override particle count / image size (development)")
     ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping, 4 = shared-memory-staged snapshots)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -222,7 +242,7 @@ def main() -> None:
     ctx = geo.geo_create(metric, 1.0, wl["a"])
     d_in = torch.from_numpy(st).to(dev)
     out = geo.alloc_outputs(n, dev, wl["nsteps"], wl["snapshot_every"], None, wl["snap_mask"])
-    kw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], flags=args.flags,
+    kw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], flags=args.flags | wl.get("flags", 0),
               snapshot_every=wl["snapshot_every"])
     stream = torch.cuda.current_stream(dev)
 
@@ -291,7 +311,7 @@ def main() -> None:
         return
 
     # ---- roofline: FP64 ALU (DFMA pipe) ----
-    flop, pipe, how = flop_counts(wl["metric"])
+    flop, pipe, how, static_count = flop_counts(wl["metric"])
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -323,10 +343,16 @@ def main() -> None:
                 "kernel": "geo_rk4_kernel", "kernel_ms": kernel_ms,
                 "flop_per_step_algorithmic": f_alg, "flop_per_step_executed": flop, "fp64_pipe_instr_per_step": pipe,
                 "achieved_executed": ach_tf, "frac_executed": ach_tf / peak_tf,
-                "flop_count_source": how,
+                "flop_count_source": how, "static_sass_count_of_loop": static_count,
                 "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {sm_max:.0f} MHz (nominal clock; MEASURED_PEAKS.json has no FP64 entry)",
                 "fp64_pipe_util": sps * pipe / (SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6),
                 "dfma_probe_tflops": probe_tf, "frac_executed_of_dfma_probe": ach_tf / probe_tf}
+    if wl["metric"] == "kerr":
+        # measured bound: a warp-level FP64 instruction holds the scheduler's issue port
+        # for 2 cycles (16 FP64 lanes per scheduler), any other instruction for 1
+        slots = 2.0 * pipe + OTHER_INSTR_PER_STEP["kerr"]
+        roofline["other_instr_per_step"] = OTHER_INSTR_PER_STEP["kerr"]
+        roofline["issue_slot_util"] = sps * slots / (SM_COUNT * 4 * 32 * sm_max * 1e6)
 
     if args.workload == "snapbench":
         # snapshot-heavy run: the bound is HBM write bandwidth.  Algorithmic bytes per launch = every
@@ -348,12 +374,17 @@ def main() -> None:
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": tmax.item() / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": tmax.item() / args.steps, "higher_is_better": True, "scaling": "weak",
+            # only the paper's own workloads have a published number (GTX 960M, another machine: context)
+            "vs_baseline": (value / wl["paper_steps_per_s"]) if wl.get("paper_steps_per_s") else None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl["name"], "n_per_gpu": n, "h": wl["h"], "nsteps": wl["nsteps"],
                        "snapshot_every": wl["snapshot_every"], "geodesic_steps_per_pass_per_gpu": steps_per_pass,
                        "parallelism": f"independent geodesics sharded by rank x{world}, no collective",
-                       "launch": info, "flags": args.flags,
+                       "launch": info, "flags": args.flags | wl.get("flags", 0),
+                       "paper": ({"steps_per_s": wl["paper_steps_per_s"], "hardware": "GeForce GTX 960M, CUDA 7.5 (PAPER.md:446)",
+                                  "e2e_over_paper": (e2e["value"] / wl["paper_steps_per_s"]) if e2e else None}
+                                 if wl.get("paper_steps_per_s") else None),
                        "l2": f"inputs+outputs {(d_in.numel() * 8 + out['final_state'].numel() * 8) / 1e6:.0f} MB vs 126 MB L2; state lives in registers"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)

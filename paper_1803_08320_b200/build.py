@@ -29,14 +29,15 @@ def nvcc_path() -> str:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
         return LIB
+    tmp = f"{LIB}.tmp{os.getpid()}"      # several ranks may build at once: private file, atomic rename
     cmd = [nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
            "-Xcompiler", "-fPIC,-Wall", "-shared", "-I", os.path.join(ROOT, "include"),
-           "-o", LIB + ".tmp"] + SOURCES
+           "-o", tmp] + SOURCES
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")
     subprocess.run(cmd, check=True)
-    os.replace(LIB + ".tmp", LIB)
+    os.replace(tmp, LIB)
     return LIB
 
 

@@ -333,7 +333,8 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         stage_trig(GEO_TC, S, C, dang, s2, sc, coarse);
         rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
         at += k.t; ar += k.r; ath += k.th; aph += k.ph; apr += k.pr; apth += k.pth;
-        if (__builtin_expect(coarse, 0)) {       // a stage angle moved by >= 2^-7 rad: full sin/cos path
+        if (__builtin_expect(coarse && active, 0)) {   // a stage angle moved by >= 2^-7 rad: full sin/cos path
+            // (idle lanes step on stale state -- often a captured ray next to the horizon -- and must not drag the warp here)
             double acc[6];
             int c;
             rk4_sum_full<KERR>(p, r, th, pr, pth, E, L, acc, &c);

@@ -26,6 +26,7 @@ def oracle():
 def G():
     import torch
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    from paper_1803_08320_b200 import geo
-    geo.lib()   # fails loudly if libgeo.so is missing
+    from paper_1803_08320_b200 import build, geo
+    build.build()   # (re)compiles libgeo.so in-tree if it is missing or older than its sources
+    geo.lib()       # fails loudly if libgeo.so is missing
     return geo

@@ -130,10 +130,14 @@ def test_config5_full_tile_4096x256_sampled(G, oracle):
     """configs[4]: i=85 deg, 4096^2 image, ONE of the 16 tiles of 256 rows (the central one, which holds
     the shadow), snapshot every 500 steps of (t, r, theta, phi) -- 2^20 rays, 13.5 GB snapshot buffer."""
     a, N, rows = 0.998, 4096, 256
-    st = W.camera_rays(N, a, 85.0, row0=(N - rows) // 2, rows=rows)
+    st, (al, be, Lz, Q) = W.camera_rays(N, a, 85.0, row0=(N - rows) // 2, rows=rows, return_constants=True)
     out = _run_full(G, a, st, 0.02, 200000, snapshot_every=500, snap_mask=0x0F,
                     r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0, kind=G.NULL)
     n = st.shape[1]
+    # every ray of the tile against the closed-form capture/escape criterion (see the config-3 test below)
+    wrong = (out["status"].cpu().numpy() == G.ST_ESCAPED) != _escapes_analytic(a, Lz, Q, W.horizon_radius(1.0, a), 1000.0)
+    print("config5 tile class mismatches:", int(wrong.sum()), "outside the axis columns:", int((wrong & (np.abs(al) >= 0.1)).sum()))
+    assert (wrong & (np.abs(al) >= 0.1)).sum() <= 32 and wrong.sum() <= 5e-3 * n
     ii = _sample(n, 124, 45)
     g, o, cert = _null_sampled(G, oracle, st, a, out, ii, snapshot_every=500, snap_mask=0x0F)
     assert np.array_equal(g["snap_count"][cert], o["snap_count"][cert])
@@ -143,3 +147,42 @@ def test_config5_full_tile_4096x256_sampled(G, oracle):
     # S1 at any size: snap_count = 1 + floor(steps_done / 500) for every ray of the tile
     sd = out["steps_done"].cpu().numpy()
     assert np.array_equal(out["snap_count"].cpu().numpy(), 1 + sd // 500)
+
+
+def _escapes_analytic(a, Lz, Q, r_plus, r_obs):
+    """Exact class of an incoming E = 1 photon: it escapes iff the radial potential
+    R(r) = r^4 + (a^2 - L^2 - Q) r^2 + 2[Q + (L-a)^2] r - a^2 Q has a turning point in (r_+, r_obs).  Since
+    R(r_+) = [(r_+^2 + a^2) - aL]^2 >= 0 and R(r_obs) > 0, that is: R <= 0 at an interior critical point
+    (roots of the cubic R')."""
+    c2 = a * a - Lz * Lz - Q
+    c1 = 2.0 * (Q + (Lz - a) ** 2)
+    c0 = -a * a * Q
+    roots = W._cubic_real_roots(np.full_like(Lz, 4.0), np.zeros_like(Lz), 2.0 * c2, c1)
+    esc = np.zeros(Lz.shape, dtype=bool)
+    for k in range(3):
+        rk = roots[k]
+        Rk = ((rk * rk + c2) * rk + c1) * rk + c0
+        with np.errstate(invalid="ignore"):
+            esc |= (rk > r_plus) & (rk < r_obs) & (Rk <= 0.0)
+    return esc
+
+
+def test_config3_whole_image_classes_match_the_analytic_criterion(G):
+    """Every one of the 1024^2 pixels against the closed-form capture/escape criterion (no oracle involved).
+    The method itself fails next to the polar axis (reading B7: |L_z| <~ 3h columns) and the
+    capture guard eats a sub-pixel band at the prograde edge of the critical curve; everything else must
+    agree."""
+    a, N = 0.998, 1024
+    st, (al, be, Lz, Q) = W.camera_rays(N, a, 60.0, return_constants=True)
+    rp = W.horizon_radius(1.0, a)
+    out = _run_full(G, a, st, 0.02, 200000, r_capture=rp + 0.01, r_escape=1100.0, kind=G.NULL)
+    status = out["status"].cpu().numpy()
+    esc = _escapes_analytic(a, Lz, Q, rp, 1000.0)
+    wrong = (status == G.ST_ESCAPED) != esc
+    axis = np.abs(al) < 0.1                      # 10 pixel columns around alpha = 0
+    print("mismatches:", int(wrong.sum()), "of which near-axis:", int((wrong & axis).sum()),
+          "captured fraction analytic / gpu:", float((~esc).mean()), float((status == G.ST_CAPTURED).mean()))
+    assert (wrong & ~axis).sum() <= 8             # measured: 0 (all 533 mismatches sit in the axis columns)
+    assert wrong.sum() <= 2e-3 * N * N
+    health = out["health"].cpu().numpy()
+    assert np.median(health[wrong & axis]) > 1e-9 if (wrong & axis).any() else True   # flagged as numerically invalid

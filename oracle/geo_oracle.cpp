@@ -306,6 +306,159 @@ void integrate_range(int metric, double M, double a, const double* state_in, int
         integrate_one<R>(bh, state_in, n, i, (R)h, nsteps, st, snapshot_every, o);
 }
 
+// ---------------------------------------------------------------------------
+// adaptive embedded Runge-Kutta 5(4) ("others method of the RK family will be included
+// soon").  The pair is Dormand & Prince's (J. Comput. Appl. Math. 6 (1980) 19, table 2 --
+// the DOPRI5 of Hairer, Norsett & Wanner, ref.[19] of the paper): 7 stages, first-same-as-last, the
+// 5th-order solution is propagated (local extrapolation), the difference to the embedded 4th-order
+// solution estimates the local error.  Step control, the textbook elementary controller:
+//   err = max_c |e_c| / (atol + rtol * max(|y_c|, |ynew_c|))  over the 6 evolving components,
+//   accept iff err <= 1,   h <- h * min(5, max(0.2, 0.9 * err^(-1/5))),  after a rejection never > 1.
+// "The final evolution time is reached": with a finite tau_end the step that would pass it
+// is shortened to land on it (when tau + 1.01 h >= tau_end) and the particle ends with MAXSTEPS.
+// Stop rules as for RK4 (readings B1-B5): capture guard on every stage point and the end point (the
+// attempt is not taken), escape test after an accepted step, `nsteps` caps the ATTEMPTS.
+// ---------------------------------------------------------------------------
+struct DP45 {
+    static constexpr int S = 7;
+    const long double c[S] = {0.0L, 1.0L / 5, 3.0L / 10, 4.0L / 5, 8.0L / 9, 1.0L, 1.0L};
+    const long double a[S][S] = {
+        {0},
+        {1.0L / 5},
+        {3.0L / 40, 9.0L / 40},
+        {44.0L / 45, -56.0L / 15, 32.0L / 9},
+        {19372.0L / 6561, -25360.0L / 2187, 64448.0L / 6561, -212.0L / 729},
+        {9017.0L / 3168, -355.0L / 33, 46732.0L / 5247, 49.0L / 176, -5103.0L / 18656},
+        {35.0L / 384, 0.0L, 500.0L / 1113, 125.0L / 192, -2187.0L / 6784, 11.0L / 84}};
+    // 5th-order weights = last row of a; embedded 4th-order weights:
+    const long double b4[S] = {5179.0L / 57600, 0.0L, 7571.0L / 16695, 393.0L / 640, -92097.0L / 339200,
+                               187.0L / 2100, 1.0L / 40};
+};
+
+struct AdaptiveCtl { double h0, rtol, atol, h_min, tau_end; };   // tau_end = +inf: no final time
+
+template <class R> R comp6(const State<R>& y, int c) {
+    switch (c) { case 0: return y.t; case 1: return y.r; case 2: return y.th; case 3: return y.ph;
+                 case 4: return y.pr; default: return y.pth; }
+}
+template <class R> R dcomp6(const Deriv<R>& k, int c) {
+    switch (c) { case 0: return k.t; case 1: return k.r; case 2: return k.th; case 3: return k.ph;
+                 case 4: return k.pr; default: return k.pth; }
+}
+template <class R> void set6(State<R>& y, int c, R v) {
+    switch (c) { case 0: y.t = v; break; case 1: y.r = v; break; case 2: y.th = v; break;
+                 case 3: y.ph = v; break; case 4: y.pr = v; break; default: y.pth = v; }
+}
+
+template <class R>
+void integrate_one_adaptive(const Hole<R>& bh, const double* state_in, int64_t n, int64_t i,
+                            const AdaptiveCtl& ctl, int64_t max_attempts, const StopRule& st,
+                            const OutPtrs& o, int64_t* rejected_out) {
+    static const DP45 T;
+    const R kappa = st.kind == 0 ? R(1) : R(0);
+    const R rc = (R)st.r_capture, re = (R)st.r_escape;
+    const R half_pi = (R)1.5707963267948966;
+    State<R> y;
+    y.t = R(0);
+    y.r = (R)state_in[0 * n + i];
+    y.th = (R)state_in[1 * n + i];
+    y.ph = (R)state_in[2 * n + i];
+    y.pr = (R)state_in[3 * n + i];
+    y.pth = (R)state_in[4 * n + i];
+    y.L = (R)state_in[5 * n + i];
+    y.E = energy_from_mass_shell(bh, y.r, y.th, y.pr, y.pth, y.L, kappa);
+    R cc[6] = {0, 0, 0, 0, 0, 0};                     // Kahan error terms (reading P1)
+    R h = (R)ctl.h0;
+    R tau = R(0);
+    const R tau_end = (R)ctl.tau_end;
+    int32_t status = -1;
+    int64_t steps = 0, attempts = 0, rejected = 0;
+    R eq_cross = std::numeric_limits<R>::quiet_NaN();
+    bool crossed = false;
+
+    if (!(y.r >= rc)) status = ORA_ST_CAPTURED;                      // B1
+    else if (!finite6(y) || !std::isfinite(y.E)) status = ORA_ST_NUMERIC;
+    else if (y.r > re) status = ORA_ST_ESCAPED;
+    else if (max_attempts == 0) status = ORA_ST_MAXSTEPS;
+
+    Deriv<R> k[DP45::S];
+    if (status < 0) k[0] = rhs(bh, y);
+    while (status < 0) {
+        const bool last = tau + R(1.01) * h >= tau_end;             // land on the final time
+        if (last) h = tau_end - tau;
+        bool captured = false;
+        for (int s = 1; s < DP45::S - 1; ++s) {                      // stages 2..6
+            State<R> ys = y;
+            for (int c = 0; c < 6; ++c) {
+                R acc = R(0);
+                for (int j = 0; j < s; ++j) acc += (R)T.a[s][j] * dcomp6(k[j], c);
+                set6(ys, c, comp6(y, c) + h * acc);
+            }
+            if (!(ys.r >= rc)) { captured = true; break; }           // B2 on every evaluation point
+            k[s] = rhs(bh, ys);
+        }
+        ++attempts;
+        if (captured) { status = ORA_ST_CAPTURED; break; }
+        // 5th-order solution (compensated update, committed only on acceptance); stage 7 sits on it
+        State<R> yn = y;
+        R cn[6];
+        for (int c = 0; c < 6; ++c) {
+            R acc5 = R(0);
+            for (int j = 0; j < DP45::S - 1; ++j) acc5 += (R)T.a[6][j] * dcomp6(k[j], c);
+            R v = comp6(y, c);
+            cn[c] = cc[c];
+            kahan_add(v, cn[c], h * acc5, false);
+            set6(yn, c, v);
+        }
+        if (!(yn.r >= rc)) { status = ORA_ST_CAPTURED; break; }      // B2: end point
+        const bool fin = finite6(yn);
+        R err = R(0);
+        if (fin) {
+            k[6] = rhs(bh, yn);
+            for (int c = 0; c < 6; ++c) {
+                R acce = R(0);                                       // (b5 - b4) . k, b5_7 = 0
+                for (int j = 0; j < DP45::S; ++j)
+                    acce += ((R)(j < 6 ? T.a[6][j] : 0.0L) - (R)T.b4[j]) * dcomp6(k[j], c);
+                const R sc = (R)ctl.atol + (R)ctl.rtol * std::max(std::fabs(comp6(y, c)), std::fabs(comp6(yn, c)));
+                const R ec = std::fabs(h * acce) / sc;
+                if (!(ec <= err)) err = ec;                          // max; a NaN sticks
+            }
+        }
+        R fac = err > R(0) ? R(0.9) * std::pow(err, R(-0.2)) : R(5);
+        if (!(fac >= R(0.2))) fac = R(0.2);                          // also catches NaN
+        if (fac > R(5)) fac = R(5);
+        if (std::isinf(ctl.rtol)) fac = R(1);                        // rtol = +inf: fixed step h0 (order tests)
+        if (!fin || !(err <= R(1))) {                                // reject
+            ++rejected;
+            h *= std::min(fac, R(1));
+            if (!(std::fabs(h) >= (R)ctl.h_min)) { status = ORA_ST_NUMERIC; break; }
+            if (attempts >= max_attempts) { status = ORA_ST_MAXSTEPS; break; }
+            continue;
+        }
+        if (!crossed) {                                              // B5
+            const R d0 = y.th - half_pi, d1 = yn.th - half_pi;
+            if (d0 * d1 < R(0)) {
+                crossed = true;
+                eq_cross = y.r + (yn.r - y.r) * (half_pi - y.th) / (yn.th - y.th);
+            }
+        }
+        y = yn;
+        for (int c = 0; c < 6; ++c) cc[c] = cn[c];
+        k[0] = k[6];                                                 // first same as last
+        ++steps;
+        tau += h;
+        h *= fac;
+        if (y.r > re) status = ORA_ST_ESCAPED;                       // B3
+        else if (last || attempts >= max_attempts) status = ORA_ST_MAXSTEPS;   // final time / B4 (cap on attempts)
+    }
+    for (int q = 0; q < 8; ++q) o.final_state[(int64_t)q * n + i] = (double)component(y, q);
+    o.status[i] = status;
+    o.steps_done[i] = steps;
+    if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
+    if (o.health) o.health[i] = (double)std::fabs(R(2) * hamiltonian(bh, y) + kappa);
+    if (rejected_out) rejected_out[i] = rejected;
+}
+
 }  // namespace
 
 extern "C" {
@@ -345,6 +498,56 @@ int oracle_integrate(int metric, double M, double a, const double* state_in, int
         });
     for (auto& th : pool) th.join();
     return 0;
+}
+
+// Adaptive RK5(4).  ctl = {h0, rtol, atol, h_min}; max_attempts caps accepted + rejected
+// attempts per particle; rejected: [n] or NULL.  Snapshot fields of `out` are ignored.
+int oracle_integrate_adaptive(int metric, double M, double a, const double* state_in, int64_t n,
+                              const AdaptiveCtl* ctl, int64_t max_attempts, const StopRule* stop,
+                              const OutPtrs* out, int64_t* rejected, int precision, int nthreads) {
+    if (!stop || !out || !ctl || n < 0 || max_attempts < 0) return 1;
+    if (!(M > 0) || !(std::fabs(a) <= M)) return 1;
+    if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0) || !(ctl->rtol >= 0) || !(ctl->atol >= 0) ||
+        !(ctl->rtol + ctl->atol > 0) || !(ctl->h_min >= 0) || !(ctl->tau_end > 0)) return 1;
+    if (metric != ORA_SCHWARZSCHILD && metric != ORA_KERR) return 1;
+    if (metric == ORA_SCHWARZSCHILD && a != 0.0) return 1;
+    if (n == 0) return 0;
+    if (!state_in || !out->final_state || !out->status || !out->steps_done) return 1;
+    if (nthreads < 1) nthreads = 1;
+    if ((int64_t)nthreads > n) nthreads = (int)n;
+    auto run = [&](int64_t lo, int64_t hi) {
+        for (int64_t i = lo; i < hi; ++i) {
+            if (precision == 1) {
+                Hole<long double> bh{metric, (long double)M, (long double)a};
+                integrate_one_adaptive<long double>(bh, state_in, n, i, *ctl, max_attempts, *stop, *out, rejected);
+            } else {
+                Hole<double> bh{metric, M, a};
+                integrate_one_adaptive<double>(bh, state_in, n, i, *ctl, max_attempts, *stop, *out, rejected);
+            }
+        }
+    };
+    if (nthreads == 1) { run(0, n); return 0; }
+    std::vector<std::thread> pool;
+    const int64_t block = 64;
+    const int64_t nblocks = (n + block - 1) / block;
+    for (int t = 0; t < nthreads; ++t)
+        pool.emplace_back([&, t]() {
+            for (int64_t b = t; b < nblocks; b += nthreads)
+                run(b * block, std::min<int64_t>(n, (b + 1) * block));
+        });
+    for (auto& th : pool) th.join();
+    return 0;
+}
+
+// The Butcher tableau the adaptive path uses, as doubles: c[7], a[7][7] (row-major), b5[7], b4[7].
+void oracle_dp45_tableau(double* c, double* a, double* b5, double* b4) {
+    static const DP45 T;
+    for (int i = 0; i < 7; ++i) {
+        c[i] = (double)T.c[i];
+        b5[i] = (double)(i < 6 ? T.a[6][i] : 0.0L);
+        b4[i] = (double)T.b4[i];
+        for (int j = 0; j < 7; ++j) a[7 * i + j] = (double)(j < i ? T.a[i][j] : 0.0L);
+    }
 }
 
 // d/dtau of (t, r, th, phi, p_r, p_th) at y = (t, r, th, phi, E, p_r, p_th, L).

@@ -54,6 +54,45 @@ def lib():
     return _lib
 
 
+class _Ctl(C.Structure):
+    _fields_ = [("h0", C.c_double), ("rtol", C.c_double), ("atol", C.c_double), ("h_min", C.c_double),
+                ("tau_end", C.c_double)]
+
+
+def integrate_adaptive(metric: int, M: float, a: float, state_in: np.ndarray, h0: float, rtol: float,
+                       atol: float, max_attempts: int, r_capture: float = -np.inf, r_escape: float = np.inf,
+                       kind: int = TIMELIKE, h_min: float = 1e-12, tau_end: float = np.inf,
+                       long_double: bool = False, nthreads: int = 1) -> dict:
+    """Adaptive Dormand-Prince RK5(4) on host SoA state_in [6][n].  rtol = inf: fixed step h0."""
+    st = np.ascontiguousarray(state_in, dtype=np.float64)
+    n = st.shape[1]
+    res = {"final_state": np.full((8, n), np.nan), "status": np.full(n, -1, dtype=np.int32),
+           "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan),
+           "health": np.full(n, np.nan), "rejected": np.zeros(n, dtype=np.int64)}
+    L = lib()
+    L.oracle_integrate_adaptive.restype = C.c_int
+    L.oracle_integrate_adaptive.argtypes = [C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_int64, C.POINTER(_Ctl),
+                                            C.c_int64, C.POINTER(_Stop), C.POINTER(_Out), C.c_void_p, C.c_int, C.c_int]
+    stop = _Stop(r_capture, r_escape, kind, 0)
+    out = _Out(res["final_state"].ctypes.data, res["status"].ctypes.data, res["steps_done"].ctypes.data,
+               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data, None, 0, 0, None)
+    ctl = _Ctl(h0, rtol, atol, h_min, tau_end)
+    rc = L.oracle_integrate_adaptive(metric, M, a, st.ctypes.data, n, C.byref(ctl), max_attempts, C.byref(stop),
+                                     C.byref(out), res["rejected"].ctypes.data, int(long_double), nthreads)
+    if rc != 0:
+        raise ValueError("oracle_integrate_adaptive: invalid arguments")
+    return res
+
+
+def dp45_tableau() -> dict:
+    c, a, b5, b4 = np.zeros(7), np.zeros((7, 7)), np.zeros(7), np.zeros(7)
+    L = lib()
+    L.oracle_dp45_tableau.restype = None
+    L.oracle_dp45_tableau.argtypes = [C.c_void_p] * 4
+    L.oracle_dp45_tableau(c.ctypes.data, a.ctypes.data, b5.ctypes.data, b4.ctypes.data)
+    return {"c": c, "a": a, "b5": b5, "b4": b4}
+
+
 def rhs(metric: int, M: float, a: float, y8, long_double: bool = False) -> np.ndarray:
     """d/dtau of (t, r, theta, phi, p_r, p_theta) at y8 = (t, r, theta, phi, E, p_r, p_theta, L)."""
     y = np.ascontiguousarray(y8, dtype=np.float64)

@@ -9,9 +9,9 @@ import parity  # noqa: E402
 
 
 def run_gpu(G, metric, a, st, h, nsteps, flags=0, snapshot_every=0, snap_mask=0xFF, snap_capacity=None,
-            host=False, **stop):
+            host=False, M=1.0, **stop):
     import torch
-    ctx = G.geo_create(metric, 1.0, a)
+    ctx = G.geo_create(metric, M, a)
     try:
         n = st.shape[1]
         if host:

@@ -1,0 +1,108 @@
+"""Pins of the oracle's adaptive Runge-Kutta 5(4) path (oracle/geo_oracle.cpp).
+
+The paper only announces "others method of the RK family", so there are no printed values:
+the pins are the mathematics -- the order conditions of the tableau (Butcher's rooted-tree conditions up to
+order 5 for the propagated solution, up to order 4 and NOT 5 for the embedded one), fifth-order convergence
+with the controller switched off, agreement with the pinned fixed-step RK4 path at a small step, the
+constants of motion, and the analytic capture/escape criterion for camera rays.
+"""
+import os
+import sys
+
+import numpy as np
+
+from paper_1803_08320_b200 import workloads as W
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+from test_oracle_integration import _null_class_analytic  # noqa: E402
+
+
+def test_tableau_order_conditions(oracle):
+    T = oracle.dp45_tableau()
+    A, c, b5, b4 = T["a"], T["c"], T["b5"], T["b4"]
+    assert np.allclose(A.sum(axis=1), c, atol=1e-15)                 # row-sum condition
+    assert np.allclose(A[6, :], b5, atol=0) and np.all(np.triu(A) == 0)   # FSAL: last row = weights; explicit
+    Ac = A @ c
+
+    def conds(b):
+        return {
+            1: [(b.sum(), 1.0)],
+            2: [(b @ c, 1 / 2)],
+            3: [(b @ c**2, 1 / 3), (b @ Ac, 1 / 6)],
+            4: [(b @ c**3, 1 / 4), (b @ (c * Ac), 1 / 8), (b @ (A @ c**2), 1 / 12), (b @ (A @ Ac), 1 / 24)],
+            5: [(b @ c**4, 1 / 5), (b @ (c**2 * Ac), 1 / 10), (b @ (c * (A @ c**2)), 1 / 15),
+                (b @ (c * (A @ Ac)), 1 / 30), (b @ Ac**2, 1 / 20), (b @ (A @ c**3), 1 / 20),
+                (b @ (A @ (c * Ac)), 1 / 40), (b @ (A @ (A @ c**2)), 1 / 60), (b @ (A @ (A @ Ac)), 1 / 120)],
+        }
+    for order, lst in conds(b5).items():
+        for got, want in lst:
+            assert abs(got - want) < 2e-16 * 8, (order, got, want)
+    c4 = conds(b4)
+    for order in (1, 2, 3, 4):
+        for got, want in c4[order]:
+            assert abs(got - want) < 2e-16 * 8, (order, got, want)
+    assert max(abs(g - w) for g, w in c4[5]) > 1e-4                  # the embedded solution is 4th order only
+
+
+def test_fifth_order_convergence_with_fixed_step(oracle):
+    a = 0.5
+    st = W.kerr_bound(4000, a, W.SEED_BASE + 4)
+    st = np.ascontiguousarray(st[:, np.argsort(st[0])[:10]])
+    sols = []
+    for k in (1, 2, 4):
+        n = 400 * k
+        r = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.1 / k, np.inf, 1.0, n, long_double=True)
+        assert (r["steps_done"] == n).all() and (r["rejected"] == 0).all()
+        sols.append(r["final_state"])
+    Q = np.linalg.norm(sols[0] - sols[1], axis=0) / np.linalg.norm(sols[1] - sols[2], axis=0)
+    assert Q.min() > 20.0 and Q.max() < 60.0 and abs(np.median(Q) - 32.0) < 3.0, Q   # 2^5; RK4 gives 16
+
+
+def test_adaptive_agrees_with_fixed_step_rk4_at_a_final_time(oracle):
+    """The paper's first stop condition, "the final evolution time is reached": both paths
+    integrate the same geodesics to the same tau -- bound Kerr orbits to tau = 40 and camera rays to
+    tau = 1015 (past the hole) -- and must agree to the tolerance of the coarser one (RK4 at a small h)."""
+    a = 0.9
+    st = W.kerr_bound(48, a, W.SEED_BASE + 2)
+    fx = oracle.integrate(oracle.KERR, 1.0, a, st, 0.0025, 16000, nthreads=8)
+    ad = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.01, 1e-13, 1e-13, 100000, tau_end=40.0, nthreads=8)
+    assert (ad["status"] == oracle.ST_MAXSTEPS).all() and ad["steps_done"].max() < 4000
+    d = np.abs(ad["final_state"] - fx["final_state"]) / np.maximum(np.abs(fx["final_state"]), 1.0)
+    assert d.max() < 2e-9, d.max()
+    a = 0.998
+    full = W.camera_rays(64, a, 60.0)
+    ii = np.arange(64 * 64).reshape(64, 64)[3::7, 2::7].ravel()
+    st = np.ascontiguousarray(full[:, ii])
+    rc = W.horizon_radius(1.0, a) + 0.01
+    kw = dict(r_capture=rc, r_escape=1100.0, kind=oracle.NULL, nthreads=8)
+    fx = oracle.integrate(oracle.KERR, 1.0, a, st, 0.005, 203000, **kw)
+    ad = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.02, 1e-12, 1e-12, 100000, tau_end=1015.0, **kw)
+    assert np.array_equal(fx["status"] == oracle.ST_CAPTURED, ad["status"] == oracle.ST_CAPTURED)
+    alive = fx["status"] == oracle.ST_MAXSTEPS
+    assert alive.sum() > 40 and ad["steps_done"][alive].max() < 3000      # vs 203 000 fixed steps
+    d = np.abs(ad["final_state"][:, alive] - fx["final_state"][:, alive]) / np.maximum(np.abs(fx["final_state"][:, alive]), 1.0)
+    assert d.max() < 1e-7, d.max()
+    assert ad["health"][alive].max() < 1e-9
+
+
+def test_adaptive_classes_match_the_analytic_criterion(oracle):
+    a = 0.998
+    st, (al, be, Lz, Q) = W.camera_rays(14, a, 60.0, return_constants=True)
+    rp = W.horizon_radius(1.0, a)
+    r = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.02, 1e-10, 1e-10, 100000, r_capture=rp + 0.01,
+                                  r_escape=1100.0, kind=oracle.NULL, nthreads=8)
+    esc = _null_class_analytic(a, Lz, Q, rp, 1000.0)
+    assert np.all(np.isin(r["status"], (oracle.ST_CAPTURED, oracle.ST_ESCAPED)))
+    assert np.array_equal(r["status"] == oracle.ST_ESCAPED, esc)
+    assert np.abs(r["final_state"][4] - 1.0).max() < 1e-12 and np.array_equal(r["final_state"][7], st[5])
+
+
+def test_adaptive_bound_orbits_conserve_the_constants(oracle):
+    a = 0.9
+    st, (E, Lz, Q) = W.kerr_bound(64, a, W.SEED_BASE + 2, return_constants=True)
+    r = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.01, 1e-12, 1e-12, 4000)
+    f = r["final_state"]
+    assert (r["status"] == oracle.ST_MAXSTEPS).all() and (r["steps_done"] + r["rejected"] == 4000).all()
+    assert r["health"].max() < 1e-9
+    Qf = f[6] ** 2 + np.cos(f[2]) ** 2 * (a * a * (1 - f[4] ** 2) + f[7] ** 2 / np.sin(f[2]) ** 2)
+    assert np.abs(Qf - Q).max() < 1e-8 and f[0].min() > 100.0      # far fewer steps than h = 0.01 would need

@@ -324,3 +324,30 @@ def test_cartesian_snapshots_are_the_papers_output_format(oracle):
     for k in (0, 4, 5, 6, 7):                                              # the other components are untouched
         assert np.array_equal(bl[..., k], ca[..., k])
     assert np.all(np.sign(z) == np.sign(np.cos(bl[..., 2])))
+
+
+def _scaled(st, M):
+    """Geometrized units: lengths, times, L and p_theta scale with M; p_r, E, angles do not."""
+    s = st.copy()
+    s[0] *= M          # r
+    s[4] *= M          # u_theta
+    s[5] *= M          # u_phi = L
+    return s
+
+
+def test_mass_scaling_and_spin_reflection_symmetries(oracle):
+    """Two exact symmetries of metric (6) that no implementation detail can fake:
+    (i) M-scaling: the solution for (M, aM, h M) from scaled data is the M = 1 solution with lengths, t, L,
+    p_theta multiplied by M; (ii) a -> -a together with L -> -L, phi -> -phi."""
+    a, M = 0.7, 2.5
+    st = W.kerr_bound(64, a, W.SEED_BASE + 2)
+    r1 = oracle.integrate(oracle.KERR, 1.0, a, st, 0.01, 3000, r_capture=2.0, r_escape=100.0)
+    rM = oracle.integrate(oracle.KERR, M, a * M, _scaled(st, M), 0.01 * M, 3000, r_capture=2.0 * M, r_escape=100.0 * M)
+    scale = np.array([M, M, 1, 1, 1, 1, M, M])[:, None]            # t r th ph E pr pth L
+    assert np.array_equal(r1["status"], rM["status"]) and np.array_equal(r1["steps_done"], rM["steps_done"])
+    assert np.max(np.abs(rM["final_state"] / scale - r1["final_state"]) / np.maximum(np.abs(r1["final_state"]), 1)) < 1e-11
+    flip = st.copy()
+    flip[5] *= -1.0
+    rf = oracle.integrate(oracle.KERR, 1.0, -a, flip, 0.01, 3000, r_capture=2.0, r_escape=100.0)
+    sign = np.array([1, 1, 1, -1, 1, 1, 1, -1])[:, None]
+    assert np.max(np.abs(rf["final_state"] * sign - r1["final_state"])) < 1e-11

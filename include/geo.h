@@ -95,6 +95,23 @@ int geo_integrate(geo_ctx *ctx, const double *state_in, int64_t n, double h, int
 int geo_integrate_host(geo_ctx *ctx, const double *state_in, int64_t n, double h, int64_t nsteps,
                        const geo_stop *stop, int64_t snapshot_every, const geo_out *out);
 
+/* adaptive embedded Runge-Kutta 5(4) (Dormand-Prince pair, first-same-as-last) with a step
+ * size per geodesic ("others method of the RK family will be included soon").
+ *   err = max_c |e_c| / (atol + rtol max(|y_c|, |ynew_c|)) over the 6 evolving components; a step is accepted
+ *   iff err <= 1; h <- h min(5, max(0.2, 0.9 err^(-1/5))) (not enlarged after a rejection).
+ * h0 > 0: first trial step.  rtol = +INFINITY: fixed step h0 (no error test).  h_min: a rejected step that
+ * would fall below it ends the particle with GEO_ST_NUMERIC.  tau_end: final value of the affine parameter,
+ * landed on exactly ("the final evolution time is reached"; +INFINITY: none); reaching it, or
+ * max_attempts (< 2^31, accepted + rejected), ends with GEO_ST_MAXSTEPS.  Capture / escape as in geo_stop
+ * (capture guard on every stage point; flags must be 0).  out: as for geo_integrate, the snapshot fields are
+ * ignored; steps_done = accepted steps.  rejected: DEVICE [n] int32 or NULL.  Enqueue-only on cuda_stream. */
+typedef struct geo_adaptive {
+    double h0, rtol, atol, h_min, tau_end;
+} geo_adaptive;
+int geo_integrate_adaptive(geo_ctx *ctx, const double *state_in, int64_t n, const geo_adaptive *ctl,
+                           int64_t max_attempts, const geo_stop *stop, const geo_out *out, int32_t *rejected,
+                           void *cuda_stream);
+
 void geo_destroy(geo_ctx *ctx);
 
 double geo_horizon_radius(const geo_ctx *ctx); /* r_+ = M + sqrt(M^2 - a^2) */

@@ -424,6 +424,7 @@ void integrate_one_adaptive(const Hole<R>& bh, const double* state_in, int64_t n
                 if (!(ec <= err)) err = ec;                          // max; a NaN sticks
             }
         }
+        if (fin && std::isinf(ctl.rtol)) err = R(0);                 // fixed-step mode: no error test
         R fac = err > R(0) ? R(0.9) * std::pow(err, R(-0.2)) : R(5);
         if (!(fac >= R(0.2))) fac = R(0.2);                          // also catches NaN
         if (fac > R(5)) fac = R(5);

@@ -7,6 +7,7 @@
 
 #include "../../include/geo.h"
 #include "geo_kernel.cuh"
+#include "geo_rk45.cuh"
 
 using namespace geo;
 
@@ -311,6 +312,65 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
         e = cudaStreamSynchronize(ctx->host_stream[k]);
         if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
     }
+    return GEO_OK;
+}
+
+int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl,
+                           int64_t max_attempts, const geo_stop* stop, const geo_out* out, int32_t* rejected,
+                           void* cuda_stream) {
+    int rc = validate(ctx, state_in, n, 1.0, 0, stop, 0, out, true);
+    if (rc != GEO_OK) return rc;
+    if (!ctl) return fail(ctx, GEO_EINVAL, "ctl must not be NULL");
+    if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0)) return fail(ctx, GEO_EINVAL, "h0 must be finite and > 0");
+    if (!(ctl->rtol >= 0.0) || !(ctl->atol >= 0.0) || !(ctl->rtol + ctl->atol > 0.0) || std::isinf(ctl->atol))
+        return fail(ctx, GEO_EINVAL, "rtol, atol must be >= 0, not both 0 (rtol = +inf: fixed step)");
+    if (!(ctl->h_min >= 0.0) || !(ctl->tau_end > 0.0)) return fail(ctx, GEO_EINVAL, "h_min >= 0 and tau_end > 0 required");
+    if (max_attempts < 0 || max_attempts > 0x7fffffffLL) return fail(ctx, GEO_EINVAL, "max_attempts must be in [0, 2^31)");
+    if (stop->flags != 0) return fail(ctx, GEO_EINVAL, "the adaptive path takes no flags");
+    if (misaligned(rejected)) return fail(ctx, GEO_EINVAL, "device pointers must be 16-byte aligned");
+    if (n == 0) return GEO_OK;
+    AdaptiveParams p;
+    memset(&p, 0, sizeof p);
+    p.in = state_in;
+    p.n = n;
+    p.h0 = ctl->h0;
+    p.rtol = ctl->rtol;
+    p.atol = ctl->atol;
+    p.h_min = ctl->h_min;
+    p.tau_end = ctl->tau_end;
+    p.fixed_step = std::isinf(ctl->rtol) ? 1 : 0;
+    p.max_attempts = (int)max_attempts;
+    p.r_capture = stop->r_capture;
+    p.r_escape = stop->r_escape;
+    p.kappa = stop->kind == GEO_TIMELIKE ? 1.0 : 0.0;
+    p.fin = out->final_state;
+    p.status = out->status;
+    p.steps_done = reinterpret_cast<long long*>(out->steps_done);
+    p.eq_cross_r = out->eq_cross_r;
+    p.health = out->health;
+    p.rejected = rejected;
+    p.counter = ctx->counter;
+    p.bh.M = ctx->M;
+    p.bh.a = ctx->a;
+    p.bh.a2 = ctx->a * ctx->a;
+    p.bh.twoM = 2.0 * ctx->M;
+    p.bh.twoMa = 2.0 * ctx->M * ctx->a;
+    p.bh.twoa2 = 2.0 * ctx->a * ctx->a;
+    fill_trig_consts(p.bh.tc);
+    typedef void (*fn_t)(const AdaptiveParams);
+    fn_t fn = ctx->metric == GEO_KERR ? (fn_t)geo_rk45_kernel<true> : (fn_t)geo_rk45_kernel<false>;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, 0);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(rk45)");
+    if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
+    const int64_t need = (n + kBlock - 1) / kBlock, resident = (int64_t)ctx->sm_count * per_sm;
+    const int grid = (int)(need < resident ? need : resident);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    e = cudaMemsetAsync(ctx->counter, 0, sizeof(unsigned long long), stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
+    fn<<<grid, kBlock, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
     return GEO_OK;
 }
 

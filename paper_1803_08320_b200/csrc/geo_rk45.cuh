@@ -1,0 +1,252 @@
+// geo_rk45.cuh -- adaptive embedded Runge-Kutta 5(4) stepper ("others method of the RK
+// family will be included soon"), one persistent kernel on the same 3+1 RHS, work queue and
+// stop rules as the fixed-step RK4 kernel of geo_kernel.cuh.
+//
+// Pair: Dormand & Prince 5(4) with 7 stages, first-same-as-last (DOPRI5 of ref.[19] of the paper); the
+// 5th-order solution is propagated, its difference to the embedded 4th-order solution estimates the local
+// error.  Per-geodesic step control (elementary controller):
+//     err = max_c |e_c| / (atol + rtol max(|y_c|, |ynew_c|))   over the 6 evolving components,
+//     accept iff err <= 1,   h <- h min(5, max(0.2, 0.9 err^(-1/5)))   (never enlarged after a rejection),
+// rtol = +inf: fixed step h0.  Stop rules: capture guard on every stage point and on the end point (that
+// attempt is not taken), escape after an accepted step, a finite tau_end is landed on ("the final evolution
+// time is reached"), max_attempts caps accepted + rejected attempts.
+// Step counts differ by orders of magnitude between rays (far field vs. near the hole), so the work queue
+// of DESIGN.md A5 is what keeps the lanes busy here.
+#pragma once
+#include "geo_kernel.cuh"
+
+namespace geo {
+
+struct AdaptiveParams {
+    const double* in;   // [6][n]
+    long long n;
+    double h0, rtol, atol, h_min, tau_end;
+    int fixed_step;     // rtol == +inf
+    int max_attempts;
+    double r_capture, r_escape, kappa;
+    double* fin;        // [8][n]
+    int* status;
+    long long* steps_done;
+    double* eq_cross_r;
+    double* health;
+    int* rejected;      // [n] or null
+    unsigned long long* counter;
+    Hole bh;
+};
+
+// Butcher tableau (Dormand & Prince 1980, table 2).  e = b5 - b4.
+namespace dp {
+constexpr double a21 = 1.0 / 5;
+constexpr double a31 = 3.0 / 40, a32 = 9.0 / 40;
+constexpr double a41 = 44.0 / 45, a42 = -56.0 / 15, a43 = 32.0 / 9;
+constexpr double a51 = 19372.0 / 6561, a52 = -25360.0 / 2187, a53 = 64448.0 / 6561, a54 = -212.0 / 729;
+constexpr double a61 = 9017.0 / 3168, a62 = -355.0 / 33, a63 = 46732.0 / 5247, a64 = 49.0 / 176, a65 = -5103.0 / 18656;
+constexpr double b1 = 35.0 / 384, b3 = 500.0 / 1113, b4 = 125.0 / 192, b5 = -2187.0 / 6784, b6 = 11.0 / 84;
+constexpr double e1 = 35.0 / 384 - 5179.0 / 57600, e3 = 500.0 / 1113 - 7571.0 / 16695, e4 = 125.0 / 192 - 393.0 / 640,
+                 e5 = -2187.0 / 6784 + 92097.0 / 339200, e6 = 11.0 / 84 - 187.0 / 2100, e7 = -1.0 / 40;
+}  // namespace dp
+
+// the four components that feed back into the RHS
+struct K4 {
+    double r, th, pr, pth;
+};
+
+template <bool KERR>
+__device__ __forceinline__ void rhs_at(const Hole& bh, double r, double th, double pr, double pth, double E, double L,
+                                       Deriv& d) {
+    double s2, sc;
+    sin2_sincos(bh.tc, th, s2, sc);
+    rhs<KERR>(bh, r, s2, sc, pr, pth, E, L, d);
+}
+
+__device__ __forceinline__ K4 k4_of(const Deriv& d) { return K4{d.r, d.th, d.pr, d.pth}; }
+
+template <bool KERR>
+__global__ void __launch_bounds__(kBlock, 3) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
+    const unsigned lane = threadIdx.x & 31u;
+    const Hole& bh = p.bh;
+    long long idx = -1;
+    bool active = false, exhausted = false;
+    double t = 0, r = 0, th = 0, ph = 0, pr = 0, pth = 0, E = 0, L = 0;
+    double ct = 0, cr = 0, cth = 0, cph = 0, cpr = 0, cpth = 0;     // Kahan error terms (reading P1)
+    double h = p.h0, tau = 0;
+    Deriv k1;                                                        // f(y): first same as last
+    k1.t = k1.r = k1.th = k1.ph = k1.pr = k1.pth = 0;
+    int steps = 0, attempts = 0, rejected = 0;
+    double eqc = 0;
+    bool crossed = false;
+
+    auto finish = [&](int st) {
+        long long n = p.n;
+        asm volatile("" : "+l"(n));
+        p.fin[0 * n + idx] = t;
+        p.fin[1 * n + idx] = r;
+        p.fin[2 * n + idx] = th;
+        p.fin[3 * n + idx] = ph;
+        p.fin[4 * n + idx] = E;
+        p.fin[5 * n + idx] = pr;
+        p.fin[6 * n + idx] = pth;
+        p.fin[7 * n + idx] = L;
+        p.status[idx] = st;
+        p.steps_done[idx] = (long long)steps;
+        if (p.eq_cross_r) p.eq_cross_r[idx] = crossed ? eqc : __longlong_as_double(0x7ff8000000000000LL);
+        if (p.health) p.health[idx] = health_3p1(bh, r, th, pr, pth, E, L, p.kappa);
+        if (p.rejected) p.rejected[idx] = rejected;
+        active = false;
+    };
+    auto begin = [&](long long i) {
+        idx = i;
+        const long long n = p.n;
+        t = 0.0;
+        r = p.in[0 * n + i];
+        th = p.in[1 * n + i];
+        ph = p.in[2 * n + i];
+        pr = p.in[3 * n + i];
+        pth = p.in[4 * n + i];
+        L = p.in[5 * n + i];
+        E = energy_3p1(bh, r, th, pr, pth, L, p.kappa);
+        ct = cr = cth = cph = cpr = cpth = 0.0;
+        h = p.h0;
+        tau = 0.0;
+        steps = attempts = rejected = 0;
+        crossed = false;
+        active = true;
+        if (!(r >= p.r_capture)) { finish(ST_CAPTURED); return; }               // B1
+        if (!all_finite6(r, th, ph, pr, pth, E)) { finish(ST_NUMERIC); return; }
+        if (r > p.r_escape) { finish(ST_ESCAPED); return; }
+        if (p.max_attempts == 0) { finish(ST_MAXSTEPS); return; }
+        rhs_at<KERR>(bh, r, th, pr, pth, E, L, k1);
+    };
+
+    for (;;) {
+        // --- work queue (A5) ------------------------------------------------------------------
+        unsigned idle = __ballot_sync(kFull, !active);
+        if (idle) {
+            if (!exhausted) {
+                const int cnt = __popc(idle);
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(p.counter, (unsigned long long)cnt);
+                base = __shfl_sync(kFull, base, 0);
+                if (!active) {
+                    const long long cand = (long long)base + __popc(idle & ((1u << lane) - 1u));
+                    if (cand < p.n) begin(cand);
+                }
+                if ((long long)base + cnt >= p.n) exhausted = true;
+                idle = __ballot_sync(kFull, !active);
+            }
+            if (idle == kFull) {
+                if (exhausted) break;
+                continue;
+            }
+        }
+
+        // --- one attempt of size h (every lane; idle lanes compute on stale state) ----------------------
+        const bool last = tau + 1.01 * h >= p.tau_end;                           // land on the final time
+        if (last) h = p.tau_end - tau;
+        Deriv d;
+        double sr, sth, spr, spth;
+        const K4 q1 = k4_of(k1);
+        double s5t = dp::b1 * k1.t, s5p = dp::b1 * k1.ph;                        // b5 . k for the cyclic t, phi
+        double set_ = dp::e1 * k1.t, sep = dp::e1 * k1.ph;                       // (b5 - b4) . k
+        // stage 2
+        sr = fma(h * dp::a21, q1.r, r); sth = fma(h * dp::a21, q1.th, th);
+        spr = fma(h * dp::a21, q1.pr, pr); spth = fma(h * dp::a21, q1.pth, pth);
+        bool cap = !(sr >= p.r_capture);
+        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        const K4 q2 = k4_of(d);
+        // stage 3
+        sr = fma(h, fma(dp::a32, q2.r, dp::a31 * q1.r), r); sth = fma(h, fma(dp::a32, q2.th, dp::a31 * q1.th), th);
+        spr = fma(h, fma(dp::a32, q2.pr, dp::a31 * q1.pr), pr); spth = fma(h, fma(dp::a32, q2.pth, dp::a31 * q1.pth), pth);
+        cap |= !(sr >= p.r_capture);
+        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        const K4 q3 = k4_of(d);
+        s5t = fma(dp::b3, d.t, s5t); s5p = fma(dp::b3, d.ph, s5p);
+        set_ = fma(dp::e3, d.t, set_); sep = fma(dp::e3, d.ph, sep);
+        // stage 4
+#define GEO_S4(c) fma(dp::a43, q3.c, fma(dp::a42, q2.c, dp::a41 * q1.c))
+        sr = fma(h, GEO_S4(r), r); sth = fma(h, GEO_S4(th), th); spr = fma(h, GEO_S4(pr), pr); spth = fma(h, GEO_S4(pth), pth);
+#undef GEO_S4
+        cap |= !(sr >= p.r_capture);
+        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        const K4 q4 = k4_of(d);
+        s5t = fma(dp::b4, d.t, s5t); s5p = fma(dp::b4, d.ph, s5p);
+        set_ = fma(dp::e4, d.t, set_); sep = fma(dp::e4, d.ph, sep);
+        // stage 5
+#define GEO_S5(c) fma(dp::a54, q4.c, fma(dp::a53, q3.c, fma(dp::a52, q2.c, dp::a51 * q1.c)))
+        sr = fma(h, GEO_S5(r), r); sth = fma(h, GEO_S5(th), th); spr = fma(h, GEO_S5(pr), pr); spth = fma(h, GEO_S5(pth), pth);
+#undef GEO_S5
+        cap |= !(sr >= p.r_capture);
+        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        const K4 q5 = k4_of(d);
+        s5t = fma(dp::b5, d.t, s5t); s5p = fma(dp::b5, d.ph, s5p);
+        set_ = fma(dp::e5, d.t, set_); sep = fma(dp::e5, d.ph, sep);
+        // stage 6
+#define GEO_S6(c) fma(dp::a65, q5.c, fma(dp::a64, q4.c, fma(dp::a63, q3.c, fma(dp::a62, q2.c, dp::a61 * q1.c))))
+        sr = fma(h, GEO_S6(r), r); sth = fma(h, GEO_S6(th), th); spr = fma(h, GEO_S6(pr), pr); spth = fma(h, GEO_S6(pth), pth);
+#undef GEO_S6
+        cap |= !(sr >= p.r_capture);
+        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        const K4 q6 = k4_of(d);
+        s5t = fma(dp::b6, d.t, s5t); s5p = fma(dp::b6, d.ph, s5p);
+        set_ = fma(dp::e6, d.t, set_); sep = fma(dp::e6, d.ph, sep);
+        // 5th-order solution, Kahan-compensated (committed only on acceptance); stage 7 sits on it
+#define GEO_B5(c) fma(dp::b6, q6.c, fma(dp::b5, q5.c, fma(dp::b4, q4.c, fma(dp::b3, q3.c, dp::b1 * q1.c))))
+        double nt, nr, nth, nph, npr, npth, dt, dr, dth, dph, dpr, dpth;
+        kahan<false>(t, ct, h, s5t, nt, dt);
+        kahan<false>(r, cr, h, GEO_B5(r), nr, dr);
+        kahan<false>(th, cth, h, GEO_B5(th), nth, dth);
+        kahan<false>(ph, cph, h, s5p, nph, dph);
+        kahan<false>(pr, cpr, h, GEO_B5(pr), npr, dpr);
+        kahan<false>(pth, cpth, h, GEO_B5(pth), npth, dpth);
+#undef GEO_B5
+        cap |= !(nr >= p.r_capture);                                             // B2: end point
+        const bool fin6 = all_finite6(nt, nr, nth, nph, npr, npth);
+        Deriv k7;
+        rhs_at<KERR>(bh, nr, nth, npr, npth, E, L, k7);
+        // error estimate h (b5 - b4) . k, scaled per component; a NaN sticks in the max
+#define GEO_E(c) fma(dp::e7, k7.c, fma(dp::e6, q6.c, fma(dp::e5, q5.c, fma(dp::e4, q4.c, fma(dp::e3, q3.c, dp::e1 * q1.c)))))
+        double err = 0.0, ec;
+        ec = fabs(h * fma(dp::e7, k7.t, set_)) / fma(p.rtol, fmax(fabs(t), fabs(nt)), p.atol);       if (!(ec <= err)) err = ec;
+        ec = fabs(h * GEO_E(r)) / fma(p.rtol, fmax(fabs(r), fabs(nr)), p.atol);                        if (!(ec <= err)) err = ec;
+        ec = fabs(h * GEO_E(th)) / fma(p.rtol, fmax(fabs(th), fabs(nth)), p.atol);                     if (!(ec <= err)) err = ec;
+        ec = fabs(h * fma(dp::e7, k7.ph, sep)) / fma(p.rtol, fmax(fabs(ph), fabs(nph)), p.atol);      if (!(ec <= err)) err = ec;
+        ec = fabs(h * GEO_E(pr)) / fma(p.rtol, fmax(fabs(pr), fabs(npr)), p.atol);                     if (!(ec <= err)) err = ec;
+        ec = fabs(h * GEO_E(pth)) / fma(p.rtol, fmax(fabs(pth), fabs(npth)), p.atol);                  if (!(ec <= err)) err = ec;
+#undef GEO_E
+        double fac = err > 0.0 ? 0.9 * pow(err, -0.2) : 5.0;
+        if (!(fac >= 0.2)) fac = 0.2;                                            // also catches NaN
+        if (fac > 5.0) fac = 5.0;
+        if (p.fixed_step) { fac = 1.0; err = fin6 ? 0.0 : err; }
+
+        if (active) {
+            ++attempts;
+            if (cap) {
+                finish(ST_CAPTURED);                                             // attempt not taken
+            } else if (!fin6 || !(err <= 1.0)) {                                 // reject
+                ++rejected;
+                h *= fmin(fac, 1.0);
+                if (!(fabs(h) >= p.h_min)) finish(ST_NUMERIC);
+                else if (attempts >= p.max_attempts) finish(ST_MAXSTEPS);
+            } else {
+                if (!crossed) {                                                  // B5
+                    const double half_pi = 1.5707963267948966;
+                    const double d0 = th - half_pi, d1 = nth - half_pi;
+                    if (d0 * d1 < 0.0) {
+                        crossed = true;
+                        eqc = r + (nr - r) * (half_pi - th) / (nth - th);
+                    }
+                }
+                t = nt; r = nr; th = nth; ph = nph; pr = npr; pth = npth;
+                ct = dt; cr = dr; cth = dth; cph = dph; cpr = dpr; cpth = dpth;
+                k1 = k7;                                                         // first same as last
+                ++steps;
+                tau += h;
+                h *= fac;
+                if (r > p.r_escape) finish(ST_ESCAPED);                          // B3
+                else if (last || attempts >= p.max_attempts) finish(ST_MAXSTEPS);   // final time / cap
+            }
+        }
+    }
+}
+
+}  // namespace geo

@@ -22,8 +22,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI
 
 # every symbol include/geo.h declares
-SYMBOLS = ("geo_create", "geo_integrate", "geo_integrate_host", "geo_destroy", "geo_horizon_radius",
-           "geo_last_error", "geo_launch_info", "geo_probe_dfma")
+SYMBOLS = ("geo_create", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_destroy",
+           "geo_horizon_radius", "geo_last_error", "geo_launch_info", "geo_probe_dfma")
 
 
 class GeoStop(C.Structure):
@@ -34,6 +34,11 @@ class GeoOut(C.Structure):
     _fields_ = [("final_state", C.c_void_p), ("status", C.c_void_p), ("steps_done", C.c_void_p),
                 ("eq_cross_r", C.c_void_p), ("health", C.c_void_p), ("snapshots", C.c_void_p),
                 ("snap_capacity", C.c_int64), ("snap_mask", C.c_uint32), ("snap_count", C.c_void_p)]
+
+
+class GeoAdaptive(C.Structure):
+    _fields_ = [("h0", C.c_double), ("rtol", C.c_double), ("atol", C.c_double), ("h_min", C.c_double),
+                ("tau_end", C.c_double)]
 
 
 class GeoError(RuntimeError):
@@ -160,6 +165,30 @@ def geo_integrate(ctx, state_in, h: float, nsteps: int, out: dict, r_capture: fl
     with torch.cuda.device(state_in.device):
         rc = lib().geo_integrate(ctx, state_in.data_ptr(), n, h, nsteps, C.byref(stop), snapshot_every,
                                  C.byref(o), C.c_void_p(s.cuda_stream))
+    _check(ctx, rc)
+
+
+def geo_integrate_adaptive(ctx, state_in, h0: float, rtol: float, atol: float, max_attempts: int, out: dict,
+                           r_capture: float = -float("inf"), r_escape: float = float("inf"), kind: int = TIMELIKE,
+                           h_min: float = 1e-12, tau_end: float = float("inf"), rejected=None, stream=None) -> None:
+    """Enqueue the adaptive RK5(4) integration (include/geo.h: geo_integrate_adaptive).  ``rejected``: optional
+    CUDA int32 tensor [n].  Does not synchronise."""
+    import torch
+    if not (state_in.is_cuda and state_in.dtype == torch.float64 and state_in.is_contiguous()
+            and state_in.dim() == 2 and state_in.shape[0] == 6):
+        raise ValueError("state_in must be a contiguous CUDA float64 tensor of shape [6][n]")
+    n = state_in.shape[1]
+    s = stream if stream is not None else torch.cuda.current_stream(state_in.device)
+    stop = GeoStop(r_capture, r_escape, kind, 0)
+    ctl = GeoAdaptive(h0, rtol, atol, h_min, tau_end)
+    o = _out_struct(out)
+    L = lib()
+    L.geo_integrate_adaptive.restype = C.c_int
+    L.geo_integrate_adaptive.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(GeoAdaptive), C.c_int64,
+                                         C.POINTER(GeoStop), C.POINTER(GeoOut), C.c_void_p, C.c_void_p]
+    with torch.cuda.device(state_in.device):
+        rc = L.geo_integrate_adaptive(ctx, state_in.data_ptr(), n, C.byref(ctl), max_attempts, C.byref(stop),
+                                      C.byref(o), _ptr(rejected), C.c_void_p(s.cuda_stream))
     _check(ctx, rc)
 
 

@@ -112,3 +112,20 @@ def test_adaptive_argument_errors(G):
             G.geo_integrate_adaptive(ctx, st, args["h0"], args["rtol"], args["atol"], args["max_attempts"], out, **kw)
         assert ei.value.code == G.EINVAL
     G.geo_destroy(ctx)
+
+
+def test_adaptive_whole_image_classes_match_the_analytic_criterion(G):
+    """All 1024^2 rays of config 3 with the adaptive stepper (rtol = atol = 1e-9) against the closed-form
+    capture/escape criterion -- no oracle involved.  Unlike fixed-step RK4 (reading B7) the step control also
+    resolves the passages next to the polar axis."""
+    from test_gpu_fullsize import _escapes_analytic
+    a, N = 0.998, 1024
+    st, (al, be, Lz, Q) = W.camera_rays(N, a, 60.0, return_constants=True)
+    rp = W.horizon_radius(1.0, a)
+    g = run_gpu_adaptive(G, G.KERR, a, st, 0.02, 1e-9, 1e-9, 200000, kind=G.NULL, r_capture=rp + 0.01, r_escape=1100.0)
+    esc = _escapes_analytic(a, Lz, Q, rp, 1000.0)
+    wrong = (g["status"] == G.ST_ESCAPED) != esc
+    print("adaptive: mismatches", int(wrong.sum()), "statuses", np.bincount(g["status"], minlength=4).tolist(),
+          "mean accepted steps", float(g["steps_done"].mean()), "mean rejected", float(g["rejected"].mean()))
+    assert np.isin(g["status"], (G.ST_CAPTURED, G.ST_ESCAPED)).all()
+    assert wrong.sum() <= 4                       # measured: 0 of 1 048 576

@@ -47,11 +47,14 @@ PIPE_INSTR_PER_STEP = {"kerr": 331.0, "schwarzschild": 273.0}
 OTHER_INSTR_PER_STEP = {"kerr": 103.0}     # non-FP64 instructions per step, same ncu capture
 FLOP_COUNT_SOURCE = {"kerr": "ncu dynamic count (profiles/r01_config4_v3.md)", "schwarzschild": "static SASS count"}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
+# adaptive RK5(4) kernel, per step ATTEMPT of one Kerr geodesic, executed (ncu, thread level)
+ADAPTIVE_FLOP_PER_ATTEMPT, ADAPTIVE_PIPE_PER_ATTEMPT = 1211.0, 785.0
+ADAPTIVE_SOURCE = "ncu dynamic thread-level count (profiles/r01_config3a_rk45.md): 426 DFMA + 268 DMUL + 90 DADD per attempt"
 # declared algorithmic work of one Kerr RK4 step (4 RHS + compensated update).
 F_ALG_SURVEY = {"kerr": 800.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one geo_rk4_kernel launch from the committed
 # `ncu --set full` capture of that workload (profiles/), bytes; None where no capture exists.
-TRAFFIC_NCU_BYTES = {"config4": 580_706_816, "snapbench": 69_562_443_296}      # profiles/r01_config4_v3.md, r01_snapbench_v3.md
+TRAFFIC_NCU_BYTES = {"config3a": 99_734_272, "config4": 580_706_816, "snapbench": 69_562_443_296}      # profiles/r01_config4_v3.md, r01_snapbench_v3.md
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:
@@ -94,6 +97,13 @@ def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dic
         perm = np.random.default_rng(W.SEED_BASE + 3).permutation(wl["st"].shape[1])
         wl["st"] = np.ascontiguousarray(wl["st"][:, perm])
         wl["name"] += " (pixels shuffled)"
+        return wl
+    if name == "config3a":
+        # the rays of configs[2] with the adaptive Dormand-Prince 5(4) stepper (per-ray step control);
+        # unit = one step ATTEMPT (accepted or rejected: 6 new RHS evaluations + error estimate)
+        wl = workload("config3", rank, n_override, nthreads)
+        wl["name"] += " -- adaptive RK5(4), rtol = atol = 1e-9"
+        wl["adaptive"] = dict(h0=wl["h"], rtol=1e-9, atol=1e-9, max_attempts=wl["nsteps"])
         return wl
     if name in ("config3", "config5"):
         N = n_override or (1024 if name == "config3" else 4096)
@@ -150,7 +160,8 @@ def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> di
     cores = os.cpu_count() or 1
     st = wl["st"]
     # sample: a prefix of the batch sized for ~budget_s of wall time at ~3e6 steps/s/core
-    per = max(1, int(budget_s * 3.0e6 * cores / max(1, wl["nsteps"])))
+    ad = wl.get("adaptive")
+    per = max(1, int(budget_s * 3.0e6 * cores / max(1, 300 * 2 if ad else wl["nsteps"])))   # adaptive: ~300 attempts/ray, 2x cost
     m = min(st.shape[1], max(cores, per))
     sub = np.ascontiguousarray(st[:, :m])
     metric = geo_oracle.KERR if wl["metric"] == "kerr" else geo_oracle.SCHWARZSCHILD
@@ -159,11 +170,15 @@ def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> di
     times, done = [], 0
     for i in range(warmup + steps):
         t0 = time.perf_counter()
-        o = geo_oracle.integrate(metric, 1.0, wl["a"], sub, wl["h"], wl["nsteps"], **kw)
+        if ad:
+            o = geo_oracle.integrate_adaptive(metric, 1.0, wl["a"], sub, ad["h0"], ad["rtol"], ad["atol"], ad["max_attempts"],
+                                              r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
+        else:
+            o = geo_oracle.integrate(metric, 1.0, wl["a"], sub, wl["h"], wl["nsteps"], **kw)
         dt = time.perf_counter() - t0
         if i >= warmup:
             times.append(dt)
-            done += int(o["steps_done"].sum())
+            done += int(o["steps_done"].sum()) + (int(o["rejected"].sum()) if ad else 0)
     return {"value": done / sum(times), "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"first {m} of {st.shape[1]} particles x up to {wl['nsteps']} steps, {steps} pass(es)",
             "ms_per_step": 1e3 * sum(times) / len(times)}
@@ -208,7 +223,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "snapbench", "paper_t3", "paper_t4"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "config3a", "snapbench", "paper_t3", "paper_t4"])
     ap.add_argument("--n", type=int, default=None, help="override particle count / image size (development)")
     ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping, 4 = shared-memory-staged snapshots)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -249,8 +264,15 @@ def main() -> None:
               snapshot_every=wl["snapshot_every"])
     stream = torch.cuda.current_stream(dev)
 
+    ad = wl.get("adaptive")
+    d_rej = torch.zeros(n, dtype=torch.int32, device=dev) if ad else None
+
     def one_pass():
-        geo.geo_integrate(ctx, d_in, wl["h"], wl["nsteps"], out, stream=stream, **kw)
+        if ad:
+            geo.geo_integrate_adaptive(ctx, d_in, ad["h0"], ad["rtol"], ad["atol"], ad["max_attempts"], out, r_capture=wl["r_capture"],
+                                       r_escape=wl["r_escape"], kind=wl["kind"], rejected=d_rej, stream=stream)
+        else:
+            geo.geo_integrate(ctx, d_in, wl["h"], wl["nsteps"], out, stream=stream, **kw)
 
     def barrier():
         if world > 1:
@@ -275,6 +297,8 @@ def main() -> None:
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
     steps_per_pass = int(out["steps_done"].sum().item())    # every pass integrates the same batch
+    if ad:
+        steps_per_pass += int(d_rej.sum().item())           # adaptive: unit = step attempt (accepted + rejected)
     total_ms = ev[0].elapsed_time(ev[-1])
     per_launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
     tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
@@ -287,7 +311,29 @@ def main() -> None:
     # ---- e2e: host buffers through geo_integrate_host (pinned), H2D + D2H inside the timed region ----
     e2e = None
     snap_bytes = out["snapshots"].numel() * 8 if out["snapshots"] is not None else 0
-    if not args.no_e2e and snap_bytes <= (16 << 30):      # larger trajectory buffers stay device-resident
+    if ad and not args.no_e2e:
+        # no host entry point for the adaptive stepper: pinned H2D, geo_integrate_adaptive, D2H of every output
+        h_in = torch.from_numpy(st).pin_memory()
+        keys = ("final_state", "status", "steps_done", "eq_cross_r", "health")
+        h_o = {k: torch.empty_like(out[k], device="cpu").pin_memory() for k in keys}
+        ke = max(1, min(args.steps, 2))
+        barrier()
+        te0 = time.perf_counter()
+        for _ in range(ke):
+            d_in.copy_(h_in, non_blocking=True)
+            one_pass()
+            for k in keys:
+                h_o[k].copy_(out[k], non_blocking=True)
+            torch.cuda.synchronize(dev)
+        te = torch.tensor([time.perf_counter() - te0], dtype=torch.float64, device=dev)
+        es = torch.tensor([float(steps_per_pass) * ke], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            dist.all_reduce(es, op=dist.ReduceOp.SUM)
+        e2e = {"value": es.item() / te.item(), "unit": UNIT, "h2d_bytes_per_step": int(h_in.numel() * 8),
+               "d2h_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h_o.values())), "passes": ke,
+               "api": "pinned H2D + geo_integrate_adaptive + D2H of all outputs"}
+    elif not args.no_e2e and snap_bytes <= (16 << 30):      # larger trajectory buffers stay device-resident
         h_in = torch.from_numpy(st).pin_memory()
         h_out = geo.alloc_outputs_host(n, wl["nsteps"], wl["snapshot_every"], None, wl["snap_mask"], pinned=True)
         geo.geo_integrate_host(ctx, h_in, wl["h"], wl["nsteps"], h_out, **kw)    # warm-up (allocates scratch)
@@ -315,6 +361,15 @@ def main() -> None:
 
     # ---- roofline: FP64 ALU (DFMA pipe) ----
     flop, pipe, how, static_count = flop_counts(wl["metric"])
+    if ad:
+        # unit = one step attempt of the RK5(4) kernel; executed FP64 instructions per attempt from the ncu capture
+        flop, pipe, how = ADAPTIVE_FLOP_PER_ATTEMPT, ADAPTIVE_PIPE_PER_ATTEMPT, ADAPTIVE_SOURCE
+        try:
+            from paper_1803_08320_b200 import sass_count
+            c = sass_count.count("geo_rk45_kernelILb1E")
+            static_count = {"flop": c["flop"], "fp64_pipe": c["fp64_pipe"]}
+        except Exception:
+            static_count = None
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -335,6 +390,8 @@ def main() -> None:
     torch.cuda.synchronize(dev)
     probe_tf = 2.0 * nf / (p0.elapsed_time(p1) * 1e-3) / 1e12
     info = geo.geo_launch_info(ctx, n, args.flags, wl["snapshot_every"])
+    if ad:
+        info = {"grid": SM_COUNT * 3, "block": 128, "regs": 168, "ctas_per_sm": 3}     # geo_rk45_kernel (profiles/r01_config3a_rk45.md)
     # Algorithmic work per unit: the flop of one RK4 step in the formulation built here,
     # 465 for Kerr = what the kernel executes (ncu counts) -- so `achieved` is also what ncu's
     # dadd + dmul + 2 dfma counters give, the quantity the north_star's ">= 50 % of FP64 peak in ncu" is about.
@@ -346,14 +403,17 @@ def main() -> None:
     sps = steps_per_pass / (kernel_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                 "frac": ach_tf / peak_tf, "traffic": TRAFFIC_NCU_BYTES.get(args.workload),
-                "kernel": "geo_rk4_kernel", "kernel_ms": kernel_ms,
+                "kernel": "geo_rk45_kernel" if ad else "geo_rk4_kernel", "kernel_ms": kernel_ms,
                 "flop_per_step": flop, "fp64_pipe_instr_per_step": pipe,
                 "flop_count_source": how, "static_sass_count_of_loop": static_count,
                 "flop_per_step_survey_f_alg": f_alg, "frac_survey_f_alg": sps * f_alg / 1e12 / peak_tf,
                 "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {sm_max:.0f} MHz (nominal clock; MEASURED_PEAKS.json has no FP64 entry)",
                 "fp64_pipe_util": sps * pipe / (SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6),
                 "dfma_probe_tflops": probe_tf, "frac_of_dfma_probe": ach_tf / probe_tf}
-    if wl["metric"] == "kerr":
+    if ad:
+        roofline.pop("flop_per_step_survey_f_alg"), roofline.pop("frac_survey_f_alg")
+        roofline["unit_of_work"] = "one RK5(4) step attempt (accepted or rejected)"
+    elif wl["metric"] == "kerr":
         # measured bound: a warp-level FP64 instruction holds the scheduler's issue port
         # for 2 cycles (16 FP64 lanes per scheduler), any other instruction for 1
         slots = 2.0 * pipe + OTHER_INSTR_PER_STEP["kerr"]
@@ -384,7 +444,8 @@ def main() -> None:
             # only the paper's own workloads have a published number (GTX 960M, another machine: context)
             "vs_baseline": (value / wl["paper_steps_per_s"]) if wl.get("paper_steps_per_s") else None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl["name"], "n_per_gpu": n, "h": wl["h"], "nsteps": wl["nsteps"],
+            "config": {"workload": wl["name"], "n_per_gpu": n, "h": wl["h"], "nsteps": wl["nsteps"], "adaptive": ad,
+                       "geodesics_per_s": (n * world * args.steps / (tmax.item() * 1e-3)),
                        "snapshot_every": wl["snapshot_every"], "geodesic_steps_per_pass_per_gpu": steps_per_pass,
                        "parallelism": f"independent geodesics sharded by rank x{world}, no collective",
                        "launch": info, "flags": args.flags | wl.get("flags", 0),

@@ -14,14 +14,15 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "geo_oracle.cpp")
+SRCS = [SRC, os.path.join(HERE, "geo_tab_oracle.cpp")]      # fixed-step/adaptive analytic metrics; tabulated metrics (8(f).3)
 LIB = os.path.join(HERE, "libgeo_oracle.so")
 
 
 def build(force: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(x) for x in SRCS):
         return LIB
     cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fPIC", "-shared", "-pthread",
-           "-Wall", "-Wextra", "-o", LIB + ".tmp", SRC]
+           "-Wall", "-Wextra", "-o", LIB + ".tmp"] + SRCS
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB

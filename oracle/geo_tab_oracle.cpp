@@ -1,0 +1,312 @@
+// geo_tab_oracle.cpp -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, one-particle-at-a-time CPU oracle for SURVEY 8(f).3: fixed-step classical RK4 geodesics
+// in a NUMERICALLY GIVEN (tabulated) stationary, axisymmetric 3+1 metric -- the "numerical metrics" the
+// paper names as the reason for its 3+1 formulation.  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may build, load or call
+// this file.  It shares NO code with the CUDA path (paper_1803_08320_b200/csrc/).
+//
+// What it computes (readings T1-T5):
+//   T1  Line element (1) with the structure of eq.(8): shift beta^i = (0,0,beta^phi),
+//       gamma_ij = diag(gamma_11, gamma_22, gamma_33), all five functions of (x^1, x^2) only.  They are given at
+//       the nodes x^1_i = x1_0 + i d1 (i < n1), x^2_j = x2_0 + j d2 (j < n2):  tab[f][j][i], f = 0..4 in the
+//       order alpha, beta^phi, gamma_11, gamma_22, gamma_33.  (x^1, x^2) are the metric's own coordinates;
+//       for Kerr in Boyer-Lindquist coordinates they are (r, theta).
+//   T2  Between the nodes every field is the tensor-product CUBIC CONVOLUTION interpolant (Keys 1981,
+//       parameter -1/2, "Catmull-Rom"): C^1, exact for polynomials of degree <= 2, third-order accurate.
+//       With u = (x - x_0)/d, i = floor(u), s = u - i the four weights of the nodes i-1 .. i+2 are
+//           w_-1 = (-s^3 + 2 s^2 - s)/2   w_0 = (3 s^3 - 5 s^2 + 2)/2   w_1 = (-3 s^3 + 4 s^2 + s)/2   w_2 = (s^3 - s^2)/2.
+//       The derivatives in the equations of motion are the EXACT derivatives of that interpolant
+//       (d/dx = (1/d) d/ds of the weights), so the system integrated is the Hamiltonian system (3),(4)
+//        of the interpolated metric: p_t and p_phi are constants of motion exactly.
+//   T3  Hamilton's equations of H = 1/2 [ -(p_t - beta^phi p_phi)^2/alpha^2 + p_1^2/gamma_11 + p_2^2/gamma_22
+//       + p_phi^2/gamma_33 ]  (eq.(4) with the inverse of metric (1)), p_t = -E, p_phi = L, W = E + beta^phi L,
+//       u^t = W/alpha^2:
+//           dt/dtau = u^t,  dx^k/dtau = p_k/gamma_kk (k = 1, 2),  dphi/dtau = L/gamma_33 - beta^phi u^t,
+//           dp_k/dtau = u^t L d_k beta^phi - alpha (u^t)^2 d_k alpha
+//                       + 1/2 [ d_k gamma_11 (p_1/gamma_11)^2 + d_k gamma_22 (p_2/gamma_22)^2 + d_k gamma_33 (L/gamma_33)^2 ].
+//       E from the mass shell (5): E = alpha sqrt(kappa + p_1^2/gamma_11 + p_2^2/gamma_22 + L^2/gamma_33) - beta^phi L.
+//   T4  The interpolant exists where all four nodes do:  1 <= i <= n - 3 in both directions ("the domain").
+//       An evaluation point (y0, an RK4 stage point, the end point of a step) outside the domain, or with a NaN
+//       coordinate, ends the particle with status OUTSIDE = 4; that step is not taken.
+//   T5  RK4, Kahan update (P1), stop rules B1-B6 and the equatorial-crossing event B5 exactly as in
+//       geo_oracle.cpp with r -> x^1, theta -> x^2; per evaluation point the capture test comes first,
+//       then the domain test.  No snapshots.
+//
+// Pins (tests/test_oracle_tabulated.py): the interpolant against Keys' kernel form, node values, quadratic
+// exactness, C^1 continuity; the RHS against finite differences of H on a metric with quadratic-polynomial
+// fields (where the interpolant is exact); flat space in spherical coordinates against the straight line's
+// closed form; tabulated Kerr against the pinned analytic-metric oracle with second-order convergence in
+// the grid spacing; E, L exact and 2H drift.
+//
+// Build: with geo_oracle.cpp into libgeo_oracle.so (oracle/build.py), -O2 -ffp-contract=off.
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <limits>
+#include <thread>
+#include <vector>
+
+namespace {
+
+enum { TAB_ST_MAXSTEPS = 0, TAB_ST_CAPTURED = 1, TAB_ST_ESCAPED = 2, TAB_ST_NUMERIC = 3, TAB_ST_OUTSIDE = 4 };
+enum { F_ALPHA = 0, F_BETA = 1, F_G11 = 2, F_G22 = 3, F_G33 = 4 };
+
+struct Table {
+    const double* tab;   // [5][n2][n1]
+    int64_t n1, n2;
+    double x1_0, d1, x2_0, d2;
+};
+
+template <class R> struct Fields { R f[5], d1[5], d2[5]; };   // value, d/dx^1, d/dx^2 of the five fields
+
+// T2: weights of nodes i-1, i, i+1, i+2 and their s-derivatives
+template <class R> void keys_weights(R s, R w[4], R dw[4]) {
+    const R s2 = s * s, s3 = s2 * s;
+    w[0] = (-s3 + R(2) * s2 - s) / R(2);
+    w[1] = (R(3) * s3 - R(5) * s2 + R(2)) / R(2);
+    w[2] = (-R(3) * s3 + R(4) * s2 + s) / R(2);
+    w[3] = (s3 - s2) / R(2);
+    dw[0] = (-R(3) * s2 + R(4) * s - R(1)) / R(2);
+    dw[1] = (R(9) * s2 - R(10) * s) / R(2);
+    dw[2] = (-R(9) * s2 + R(8) * s + R(1)) / R(2);
+    dw[3] = (R(3) * s2 - R(2) * s) / R(2);
+}
+
+// T2 + T4: false if (x1, x2) is outside the domain
+template <class R> bool interpolate(const Table& m, R x1, R x2, Fields<R>& F) {
+    const R u1 = (x1 - (R)m.x1_0) / (R)m.d1, u2 = (x2 - (R)m.x2_0) / (R)m.d2;
+    const R fl1 = std::floor(u1), fl2 = std::floor(u2);
+    if (!(fl1 >= R(1) && fl1 <= (R)(m.n1 - 3) && fl2 >= R(1) && fl2 <= (R)(m.n2 - 3))) return false;   // NaN-safe
+    const int64_t i = (int64_t)fl1, j = (int64_t)fl2;
+    R w1[4], dw1[4], w2[4], dw2[4];
+    keys_weights(u1 - fl1, w1, dw1);
+    keys_weights(u2 - fl2, w2, dw2);
+    for (int f = 0; f < 5; ++f) {
+        const double* T = m.tab + (int64_t)f * m.n1 * m.n2;
+        R v = 0, v1 = 0, v2 = 0;
+        for (int b = 0; b < 4; ++b)
+            for (int a = 0; a < 4; ++a) {
+                const R node = (R)T[(j - 1 + b) * m.n1 + (i - 1 + a)];
+                v += w2[b] * w1[a] * node;
+                v1 += w2[b] * dw1[a] * node;
+                v2 += dw2[b] * w1[a] * node;
+            }
+        F.f[f] = v;
+        F.d1[f] = v1 / (R)m.d1;
+        F.d2[f] = v2 / (R)m.d2;
+    }
+    return true;
+}
+
+// State: y = (t, x1, x2, phi, E, p1, p2, L) -- the paper's order with r -> x^1, theta -> x^2
+template <class R> struct State { R t, x1, x2, ph, E, p1, p2, L; };
+template <class R> struct Deriv { R t, x1, x2, ph, p1, p2; };
+
+// T3
+template <class R> Deriv<R> rhs_fields(const Fields<R>& F, const State<R>& y) {
+    const R al = F.f[F_ALPHA], be = F.f[F_BETA], g11 = F.f[F_G11], g22 = F.f[F_G22], g33 = F.f[F_G33];
+    const R W = y.E + be * y.L;
+    const R ut = W / (al * al);
+    const R v1 = y.p1 / g11, v2 = y.p2 / g22, v3 = y.L / g33;
+    Deriv<R> d;
+    d.t = ut;
+    d.x1 = v1;
+    d.x2 = v2;
+    d.ph = v3 - be * ut;
+    d.p1 = ut * y.L * F.d1[F_BETA] - al * ut * ut * F.d1[F_ALPHA]
+           + (F.d1[F_G11] * v1 * v1 + F.d1[F_G22] * v2 * v2 + F.d1[F_G33] * v3 * v3) / R(2);
+    d.p2 = ut * y.L * F.d2[F_BETA] - al * ut * ut * F.d2[F_ALPHA]
+           + (F.d2[F_G11] * v1 * v1 + F.d2[F_G22] * v2 * v2 + F.d2[F_G33] * v3 * v3) / R(2);
+    return d;
+}
+
+template <class R> R hamiltonian_fields(const Fields<R>& F, const State<R>& y) {
+    const R W = y.E + F.f[F_BETA] * y.L;
+    return (-(W * W) / (F.f[F_ALPHA] * F.f[F_ALPHA]) + y.p1 * y.p1 / F.f[F_G11] + y.p2 * y.p2 / F.f[F_G22] +
+            y.L * y.L / F.f[F_G33]) / R(2);
+}
+
+template <class R> R energy_fields(const Fields<R>& F, R p1, R p2, R L, R kappa) {
+    return F.f[F_ALPHA] * std::sqrt(kappa + p1 * p1 / F.f[F_G11] + p2 * p2 / F.f[F_G22] + L * L / F.f[F_G33]) -
+           F.f[F_BETA] * L;
+}
+
+struct StopRule { double r_capture, r_escape; int32_t kind; int32_t flags; };
+struct OutPtrs { double* final_state; int32_t* status; int64_t* steps_done; double* eq_cross_r; double* health; };
+
+template <class R> bool finite6(const State<R>& y) {
+    return std::isfinite(y.t) && std::isfinite(y.x1) && std::isfinite(y.x2) && std::isfinite(y.ph) &&
+           std::isfinite(y.p1) && std::isfinite(y.p2);
+}
+
+template <class R> State<R> shifted(const State<R>& y, R w, const Deriv<R>& k) {
+    State<R> z = y;
+    z.t = y.t + w * k.t;
+    z.x1 = y.x1 + w * k.x1;
+    z.x2 = y.x2 + w * k.x2;
+    z.ph = y.ph + w * k.ph;
+    z.p1 = y.p1 + w * k.p1;
+    z.p2 = y.p2 + w * k.p2;
+    return z;
+}
+
+template <class R> void kahan_add(R& y, R& c, R delta, bool plain) {
+    if (plain) { y = y + delta; return; }
+    const R yk = delta - c;
+    const R tsum = y + yk;
+    c = (tsum - y) - yk;
+    y = tsum;
+}
+
+template <class R>
+void integrate_one(const Table& m, const double* state_in, int64_t n, int64_t i, R h, int64_t nsteps,
+                   const StopRule& st, const OutPtrs& o) {
+    const R kappa = st.kind == 0 ? R(1) : R(0);
+    const bool plain = (st.flags & 1) != 0;
+    const R rc = (R)st.r_capture, re = (R)st.r_escape;
+    const R half_pi = (R)1.5707963267948966;
+
+    State<R> y;
+    y.t = R(0);
+    y.x1 = (R)state_in[0 * n + i];
+    y.x2 = (R)state_in[1 * n + i];
+    y.ph = (R)state_in[2 * n + i];
+    y.p1 = (R)state_in[3 * n + i];
+    y.p2 = (R)state_in[4 * n + i];
+    y.L = (R)state_in[5 * n + i];
+    y.E = std::numeric_limits<R>::quiet_NaN();
+    R ct = 0, c1 = 0, c2 = 0, cph = 0, cp1 = 0, cp2 = 0;
+
+    int32_t status = -1;
+    int64_t steps = 0;
+    R eq_cross = std::numeric_limits<R>::quiet_NaN();
+    bool crossed = false;
+    Fields<R> F;
+
+    // B1 + T4 on y0
+    if (!(y.x1 >= rc)) status = TAB_ST_CAPTURED;
+    else if (!finite6(y) || !std::isfinite(y.L)) status = TAB_ST_NUMERIC;
+    else if (!interpolate(m, y.x1, y.x2, F)) status = TAB_ST_OUTSIDE;
+    else {
+        y.E = energy_fields(F, y.p1, y.p2, y.L, kappa);
+        if (!std::isfinite(y.E)) status = TAB_ST_NUMERIC;
+        else if (y.x1 > re) status = TAB_ST_ESCAPED;
+        else if (nsteps == 0) status = TAB_ST_MAXSTEPS;
+    }
+
+    while (status < 0) {
+        // F holds the fields at y (from B1 or from the end point test of the previous step)
+        const Deriv<R> k1 = rhs_fields(F, y);
+        const State<R> y2 = shifted(y, h / R(2), k1);
+        Fields<R> G;
+        if (!(y2.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }
+        if (!interpolate(m, y2.x1, y2.x2, G)) { status = TAB_ST_OUTSIDE; break; }
+        const Deriv<R> k2 = rhs_fields(G, y2);
+        const State<R> y3 = shifted(y, h / R(2), k2);
+        if (!(y3.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }
+        if (!interpolate(m, y3.x1, y3.x2, G)) { status = TAB_ST_OUTSIDE; break; }
+        const Deriv<R> k3 = rhs_fields(G, y3);
+        const State<R> y4 = shifted(y, h, k3);
+        if (!(y4.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }
+        if (!interpolate(m, y4.x1, y4.x2, G)) { status = TAB_ST_OUTSIDE; break; }
+        const Deriv<R> k4 = rhs_fields(G, y4);
+
+        State<R> yn = y;
+        R nt = ct, n1 = c1, n2 = c2, nph = cph, np1 = cp1, np2 = cp2;
+        const R w = h / R(6);
+        kahan_add(yn.t, nt, w * (k1.t + R(2) * k2.t + R(2) * k3.t + k4.t), plain);
+        kahan_add(yn.x1, n1, w * (k1.x1 + R(2) * k2.x1 + R(2) * k3.x1 + k4.x1), plain);
+        kahan_add(yn.x2, n2, w * (k1.x2 + R(2) * k2.x2 + R(2) * k3.x2 + k4.x2), plain);
+        kahan_add(yn.ph, nph, w * (k1.ph + R(2) * k2.ph + R(2) * k3.ph + k4.ph), plain);
+        kahan_add(yn.p1, np1, w * (k1.p1 + R(2) * k2.p1 + R(2) * k3.p1 + k4.p1), plain);
+        kahan_add(yn.p2, np2, w * (k1.p2 + R(2) * k2.p2 + R(2) * k3.p2 + k4.p2), plain);
+
+        if (!(yn.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }
+        if (!finite6(yn)) { status = TAB_ST_NUMERIC; break; }
+        if (!interpolate(m, yn.x1, yn.x2, G)) { status = TAB_ST_OUTSIDE; break; }     // T4: end point
+
+        if (!crossed) {
+            const R d0 = y.x2 - half_pi, d1 = yn.x2 - half_pi;
+            if (d0 * d1 < R(0)) {
+                crossed = true;
+                eq_cross = y.x1 + (yn.x1 - y.x1) * (half_pi - y.x2) / (yn.x2 - y.x2);
+            }
+        }
+        y = yn; ct = nt; c1 = n1; c2 = n2; cph = nph; cp1 = np1; cp2 = np2;
+        F = G;
+        ++steps;
+        if (y.x1 > re) status = TAB_ST_ESCAPED;
+        else if (steps >= nsteps) status = TAB_ST_MAXSTEPS;
+    }
+
+    const R comp[8] = {y.t, y.x1, y.x2, y.ph, y.E, y.p1, y.p2, y.L};
+    for (int k = 0; k < 8; ++k) o.final_state[(int64_t)k * n + i] = (double)comp[k];
+    o.status[i] = status;
+    o.steps_done[i] = steps;
+    if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
+    if (o.health) {
+        // |2H + kappa| of the final state; NaN where the final state has no interpolant (OUTSIDE at y0, NUMERIC)
+        Fields<R> H;
+        o.health[i] = (std::isfinite(y.E) && interpolate(m, y.x1, y.x2, H))
+                          ? (double)std::fabs(R(2) * hamiltonian_fields(H, y) + kappa)
+                          : std::numeric_limits<double>::quiet_NaN();
+    }
+}
+
+template <class R>
+void integrate_range(const Table& m, const double* state_in, int64_t n, double h, int64_t nsteps,
+                     const StopRule& st, const OutPtrs& o, int64_t lo, int64_t hi) {
+    for (int64_t i = lo; i < hi; ++i) integrate_one<R>(m, state_in, n, i, (R)h, nsteps, st, o);
+}
+
+}  // namespace
+
+extern "C" {
+
+// tab: [5][n2][n1] host doubles.  precision: 0 = double, 1 = long double.  Returns 0, or 1 on invalid arguments.
+int oracle_tab_integrate(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+                         const double* state_in, int64_t n, double h, int64_t nsteps, const StopRule* st,
+                         const OutPtrs* out, int precision, int nthreads) {
+    if (!tab || n1 < 4 || n2 < 4 || !(d1 > 0) || !(d2 > 0) || n < 0 || nsteps < 0 || !st || !out) return 1;
+    const Table m{tab, n1, n2, x1_0, d1, x2_0, d2};
+    if (nthreads < 1) nthreads = 1;
+    std::vector<std::thread> pool;
+    const int64_t per = (n + nthreads - 1) / nthreads;
+    for (int t = 0; t < nthreads; ++t) {
+        const int64_t lo = t * per, hi = std::min<int64_t>(n, lo + per);
+        if (lo >= hi) break;
+        if (precision == 1)
+            pool.emplace_back(integrate_range<long double>, m, state_in, n, h, nsteps, *st, *out, lo, hi);
+        else
+            pool.emplace_back(integrate_range<double>, m, state_in, n, h, nsteps, *st, *out, lo, hi);
+    }
+    for (auto& th : pool) th.join();
+    return 0;
+}
+
+// Interpolated fields at one point: out15 = value[5], d/dx1[5], d/dx2[5].  Returns 1 inside the domain, 0 outside.
+int oracle_tab_fields(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+                      double x1, double x2, double* out15) {
+    const Table m{tab, n1, n2, x1_0, d1, x2_0, d2};
+    Fields<double> F;
+    if (!interpolate<double>(m, x1, x2, F)) return 0;
+    for (int f = 0; f < 5; ++f) { out15[f] = F.f[f]; out15[5 + f] = F.d1[f]; out15[10 + f] = F.d2[f]; }
+    return 1;
+}
+
+// RHS (T3) at y8 = (t, x1, x2, phi, E, p1, p2, L): d6 = d/dtau of (t, x1, x2, phi, p1, p2); *H = Hamiltonian.
+int oracle_tab_rhs(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+                   const double* y8, double* d6, double* H) {
+    const Table m{tab, n1, n2, x1_0, d1, x2_0, d2};
+    Fields<double> F;
+    State<double> y{y8[0], y8[1], y8[2], y8[3], y8[4], y8[5], y8[6], y8[7]};
+    if (!interpolate<double>(m, y.x1, y.x2, F)) return 0;
+    const Deriv<double> d = rhs_fields(F, y);
+    d6[0] = d.t; d6[1] = d.x1; d6[2] = d.x2; d6[3] = d.ph; d6[4] = d.p1; d6[5] = d.p2;
+    if (H) *H = hamiltonian_fields(F, y);
+    return 1;
+}
+
+}  // extern "C"

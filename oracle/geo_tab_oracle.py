@@ -1,0 +1,84 @@
+"""ctypes binding of the tabulated-metric CPU oracle (oracle/geo_tab_oracle.cpp).
+
+TEST INFRASTRUCTURE, NOT PRODUCT CODE: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this module.  Argument marshalling only; imports nothing from the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import build as _build  # noqa: E402  (oracle/build.py)
+
+TIMELIKE, NULL = 0, 1
+ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC, ST_OUTSIDE = 0, 1, 2, 3, 4
+
+
+class _Stop(C.Structure):
+    _fields_ = [("r_capture", C.c_double), ("r_escape", C.c_double), ("kind", C.c_int32), ("flags", C.c_int32)]
+
+
+class _Out(C.Structure):
+    _fields_ = [("final_state", C.c_void_p), ("status", C.c_void_p), ("steps_done", C.c_void_p),
+                ("eq_cross_r", C.c_void_p), ("health", C.c_void_p)]
+
+
+_lib = None
+_GRID = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.oracle_tab_integrate.restype = C.c_int
+        _lib.oracle_tab_integrate.argtypes = _GRID + [C.c_void_p, C.c_int64, C.c_double, C.c_int64, C.POINTER(_Stop),
+                                                      C.POINTER(_Out), C.c_int, C.c_int]
+        _lib.oracle_tab_fields.restype = C.c_int
+        _lib.oracle_tab_fields.argtypes = _GRID + [C.c_double, C.c_double, C.c_void_p]
+        _lib.oracle_tab_rhs.restype = C.c_int
+        _lib.oracle_tab_rhs.argtypes = _GRID + [C.c_void_p, C.c_void_p, C.c_void_p]
+    return _lib
+
+
+def _grid(table: dict):
+    tab = table["tab"]
+    assert tab.dtype == np.float64 and tab.flags.c_contiguous and tab.ndim == 3 and tab.shape[0] == 5
+    return [tab.ctypes.data, tab.shape[2], tab.shape[1], table["x1_0"], table["d1"], table["x2_0"], table["d2"]]
+
+
+def fields(table: dict, x1: float, x2: float):
+    """(value[5], d/dx1[5], d/dx2[5]) of the interpolated alpha, beta^phi, gamma_11, gamma_22, gamma_33; None outside."""
+    out = np.zeros(15)
+    ok = lib().oracle_tab_fields(*_grid(table), x1, x2, out.ctypes.data)
+    return (out[:5], out[5:10], out[10:]) if ok else None
+
+
+def rhs(table: dict, y8):
+    """d/dtau of (t, x1, x2, phi, p1, p2) and H at y8 = (t, x1, x2, phi, E, p1, p2, L); None outside the domain."""
+    y = np.ascontiguousarray(y8, dtype=np.float64)
+    d, H = np.zeros(6), C.c_double()
+    ok = lib().oracle_tab_rhs(*_grid(table), y.ctypes.data, d.ctypes.data, C.byref(H))
+    return (d, H.value) if ok else None
+
+
+def integrate(table: dict, state_in: np.ndarray, h: float, nsteps: int, r_capture: float = -np.inf,
+              r_escape: float = np.inf, kind: int = TIMELIKE, flags: int = 0, long_double: bool = False,
+              nthreads: int = 1) -> dict:
+    """Fixed-step RK4 through the tabulated metric on host SoA state_in [6][n] = (x1, x2, phi, p_1, p_2, p_phi)."""
+    st = np.ascontiguousarray(state_in, dtype=np.float64)
+    n = st.shape[1]
+    res = {"final_state": np.full((8, n), np.nan), "status": np.full(n, -1, dtype=np.int32),
+           "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan), "health": np.full(n, np.nan)}
+    stop = _Stop(r_capture, r_escape, kind, flags)
+    out = _Out(res["final_state"].ctypes.data, res["status"].ctypes.data, res["steps_done"].ctypes.data,
+               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data)
+    rc = lib().oracle_tab_integrate(*_grid(table), st.ctypes.data, n, h, nsteps, C.byref(stop), C.byref(out),
+                                    int(long_double), nthreads)
+    if rc != 0:
+        raise ValueError("oracle_tab_integrate: invalid arguments")
+    return res

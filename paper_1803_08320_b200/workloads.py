@@ -229,6 +229,57 @@ def camera_rays(N: int, a: float, incl_deg: float, M: float = 1.0, r_obs: float 
     return st
 
 
+# ----------------------------------------------------------------------------
+# Tabulated 3+1 metrics: input DATA for geo_create_tabulated / oracle_tab_integrate --
+# the five functions of eq.(8) sampled on a uniform (x^1, x^2) grid.  No interpolation, no
+# equations of motion here.
+# ----------------------------------------------------------------------------
+def kerr_metric_table(M: float, a: float, n1: int, n2: int, x1_lo: float, x1_hi: float,
+                      x2_lo: float = 0.0, x2_hi: float = math.pi, radial: str = "r", ghost: int = 2) -> dict:
+    """alpha, beta^phi, gamma_11, gamma_22, gamma_33 of the Kerr metric, eq.(8), at the nodes of a
+    uniform grid: ``n1 x n2`` nodes span [x1_lo, x1_hi] x [x2_lo, x2_hi] and ``ghost`` more nodes are added on every
+    side (the cubic-convolution stencil needs one; eq.(8) is analytic there, also beyond theta = 0, pi).
+    radial = "r": x^1 = r (Boyer-Lindquist);  radial = "log": x^1 = ln(r - r_+), r = r_+ + exp(x^1), so that
+    gamma_11 = gamma_rr (dr/dx^1)^2 = rho^2 (r - r_+)/(r - r_-) is regular at the horizon and a uniform grid
+    resolves both the near-horizon region and the far field.  Returns {"tab": [5][n2+2g][n1+2g], "x1_0", "d1",
+    "x2_0", "d2"} (x1_0, x2_0: coordinates of node 0, ghosts included)."""
+    d1 = (x1_hi - x1_lo) / (n1 - 1)
+    d2 = (x2_hi - x2_lo) / (n2 - 1)
+    x1 = x1_lo + d1 * (np.arange(n1 + 2 * ghost) - ghost)
+    x2 = x2_lo + d2 * (np.arange(n2 + 2 * ghost) - ghost)
+    X1, TH = np.meshgrid(x1, x2)                       # [n2][n1], x^1 fastest
+    rp, rm = M + math.sqrt(M * M - a * a), M - math.sqrt(M * M - a * a)
+    if radial == "log":
+        ex = np.exp(X1)
+        r = rp + ex
+        jac2_over_delta = ex / (r - rm)                # (dr/dx1)^2 / Delta = (r - r_+)^2 / ((r - r_+)(r - r_-))
+    elif radial == "r":
+        r = X1
+        jac2_over_delta = 1.0 / (r * r - 2.0 * M * r + a * a)
+    else:
+        raise ValueError(radial)
+    s2 = np.sin(TH) ** 2
+    rho2 = r * r + a * a * np.cos(TH) ** 2
+    Delta = r * r - 2.0 * M * r + a * a
+    Sigma = (r * r + a * a) ** 2 - a * a * Delta * s2
+    tab = np.empty((5,) + r.shape)
+    tab[0] = np.sqrt(rho2 * Delta / Sigma)
+    tab[1] = -2.0 * M * a * r / Sigma
+    tab[2] = rho2 * jac2_over_delta
+    tab[3] = rho2
+    tab[4] = Sigma / rho2 * s2
+    return {"tab": np.ascontiguousarray(tab), "x1_0": float(x1[0]), "d1": float(d1), "x2_0": float(x2[0]), "d2": float(d2),
+            "radial": radial, "r_plus": rp}
+
+
+def to_log_radial(st: np.ndarray, r_plus: float) -> np.ndarray:
+    """state_in (r, theta, phi, u_r, u_theta, u_phi) -> the same covectors in x^1 = ln(r - r_+): u_1 = u_r (r - r_+)."""
+    out = np.array(st, dtype=np.float64, copy=True)
+    out[0] = np.log(st[0] - r_plus)
+    out[3] = st[3] * (st[0] - r_plus)
+    return out
+
+
 def shard_range(n: int, rank: int, world: int) -> tuple[int, int]:
     """Contiguous particle-index range [lo, hi) of ``rank`` (geodesics
     are independent, PAPER.md:329 -- no exchange step)."""

@@ -22,6 +22,13 @@ def oracle():
     return geo_oracle
 
 
+@pytest.fixture(scope="session")
+def tab_oracle():
+    import geo_tab_oracle  # oracle/geo_tab_oracle.py (test infrastructure)
+    geo_tab_oracle.lib()
+    return geo_tab_oracle
+
+
 @pytest.fixture(scope="module")
 def G():
     import torch

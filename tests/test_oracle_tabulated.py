@@ -1,0 +1,266 @@
+"""Pins of the tabulated-metric oracle (oracle/geo_tab_oracle.cpp, readings T1-T5).
+
+The paper only announces numerical metrics, so nothing is printed: the pins are the
+mathematics.  Interpolant: Keys' cubic-convolution KERNEL form summed over all nodes (the oracle uses the four
+per-cell weight polynomials), node values, exactness on quadratics, C^1 continuity.  Equations of motion: finite
+differences of H on a metric whose fields are quadratic polynomials (there the interpolant IS the metric, so a
+dropped term, a wrong sign or swapped derivatives in the RHS fail).  Integration: flat space in spherical
+coordinates against the straight line's closed form; the Kerr metric of eq.(8) sampled on a grid against the pinned
+analytic-metric oracle, with the convergence order in the grid spacing; constants of motion; stop rules.
+"""
+import math
+
+import numpy as np
+
+from paper_1803_08320_b200 import workloads as W
+
+
+def _rand_table(n1=12, n2=10, seed=1):
+    rng = np.random.default_rng(seed)
+    return {"tab": np.ascontiguousarray(rng.uniform(0.5, 2.0, (5, n2, n1))), "x1_0": 2.0, "d1": 0.25, "x2_0": -0.3, "d2": 0.4}
+
+
+def _keys_kernel(s):
+    """Keys (1981) eq.(15): u(s) for a = -1/2."""
+    s = np.abs(s)
+    return np.where(s < 1, 1.5 * s**3 - 2.5 * s**2 + 1, np.where(s < 2, -0.5 * s**3 + 2.5 * s**2 - 4 * s + 2, 0.0))
+
+
+def _keys_kernel_prime(s):
+    sg, s = np.sign(s), np.abs(s)
+    return sg * np.where(s < 1, 4.5 * s**2 - 5 * s, np.where(s < 2, -1.5 * s**2 + 5 * s - 4, 0.0))
+
+
+def test_interpolant_equals_the_kernel_form_summed_over_all_nodes(tab_oracle):
+    tb = _rand_table()
+    n2, n1 = tb["tab"].shape[1:]
+    xs1 = tb["x1_0"] + tb["d1"] * np.arange(n1)
+    xs2 = tb["x2_0"] + tb["d2"] * np.arange(n2)
+    rng = np.random.default_rng(2)
+    for _ in range(200):
+        x1 = rng.uniform(xs1[1], xs1[n1 - 2] - 1e-9)
+        x2 = rng.uniform(xs2[1], xs2[n2 - 2] - 1e-9)
+        k1, k2 = _keys_kernel((x1 - xs1) / tb["d1"]), _keys_kernel((x2 - xs2) / tb["d2"])
+        d1, d2 = _keys_kernel_prime((x1 - xs1) / tb["d1"]) / tb["d1"], _keys_kernel_prime((x2 - xs2) / tb["d2"]) / tb["d2"]
+        v, g1, g2 = tab_oracle.fields(tb, x1, x2)
+        for f in range(5):
+            T = tb["tab"][f]
+            assert abs(v[f] - k2 @ T @ k1) < 1e-13
+            assert abs(g1[f] - k2 @ T @ d1) < 1e-12
+            assert abs(g2[f] - d2 @ T @ k1) < 1e-12
+
+
+def test_interpolant_passes_through_the_nodes_and_domain_is_where_the_stencil_exists(tab_oracle):
+    tb = _rand_table()
+    n2, n1 = tb["tab"].shape[1:]
+    for j in range(n2):
+        for i in range(n1):
+            r = tab_oracle.fields(tb, tb["x1_0"] + tb["d1"] * i, tb["x2_0"] + tb["d2"] * j)
+            inside = 1 <= i <= n1 - 3 and 1 <= j <= n2 - 3              # reading T4
+            assert (r is not None) == inside, (i, j)
+            if inside:
+                assert np.allclose(r[0], tb["tab"][:, j, i], rtol=0, atol=1e-14)
+    assert tab_oracle.fields(tb, float("nan"), 0.5) is None
+
+
+def test_interpolant_is_exact_on_quadratics_and_C1_across_cells(tab_oracle):
+    n1, n2 = 14, 11
+    tb = {"x1_0": 1.0, "d1": 0.5, "x2_0": 0.2, "d2": 0.3}
+    X1, X2 = np.meshgrid(tb["x1_0"] + tb["d1"] * np.arange(n1), tb["x2_0"] + tb["d2"] * np.arange(n2))
+    c = np.random.default_rng(3).uniform(-1, 1, (5, 3, 3))
+
+    def poly(f, x1, x2, d1=0, d2=0):
+        p1 = [np.ones_like(x1), x1, x1 * x1] if d1 == 0 else [0 * x1, np.ones_like(x1), 2 * x1]
+        p2 = [np.ones_like(x2), x2, x2 * x2] if d2 == 0 else [0 * x2, np.ones_like(x2), 2 * x2]
+        return sum(c[f, i, j] * p1[i] * p2[j] for i in range(3) for j in range(3))
+    tb["tab"] = np.ascontiguousarray(np.stack([poly(f, X1, X2) for f in range(5)]))
+    rng = np.random.default_rng(4)
+    for _ in range(100):
+        x1, x2 = np.float64(rng.uniform(1.6, 6.9)), np.float64(rng.uniform(0.55, 2.8))
+        v, g1, g2 = tab_oracle.fields(tb, x1, x2)
+        for f in range(5):
+            assert abs(v[f] - poly(f, x1, x2)) < 2e-12
+            assert abs(g1[f] - poly(f, x1, x2, d1=1)) < 2e-11
+            assert abs(g2[f] - poly(f, x1, x2, d2=1)) < 2e-11
+    # C^1 across a cell face on a NON-polynomial table
+    tr = _rand_table()
+    xb = tr["x1_0"] + 4 * tr["d1"]
+    lo, hi = tab_oracle.fields(tr, xb - 1e-10, 0.77), tab_oracle.fields(tr, xb + 1e-10, 0.77)
+    for k in range(3):
+        assert np.max(np.abs(lo[k] - hi[k])) < 1e-7
+    yb = tr["x2_0"] + 5 * tr["d2"]
+    lo, hi = tab_oracle.fields(tr, 3.21, yb - 1e-10), tab_oracle.fields(tr, 3.21, yb + 1e-10)
+    for k in range(3):
+        assert np.max(np.abs(lo[k] - hi[k])) < 1e-7
+
+
+def _quadratic_metric():
+    """A made-up stationary axisymmetric metric whose five fields are quadratics: the interpolant is exact on it."""
+    def fields(x1, x2):
+        return (1.0 + 0.05 * x1 + 0.02 * x2 * x2 - 0.01 * x1 * x2,          # alpha
+                -0.03 + 0.004 * x1 * x1 - 0.01 * x2,                        # beta^phi
+                1.5 + 0.1 * x1 * x1 + 0.05 * x2,                            # gamma_11
+                2.0 + 0.3 * x1 + 0.2 * x2 * x2,                             # gamma_22
+                1.0 + 0.5 * x1 * x2 + 0.1 * x1 * x1)                        # gamma_33
+    n1, n2 = 20, 18
+    tb = {"x1_0": 0.5, "d1": 0.2, "x2_0": 0.4, "d2": 0.15}
+    X1, X2 = np.meshgrid(tb["x1_0"] + tb["d1"] * np.arange(n1), tb["x2_0"] + tb["d2"] * np.arange(n2))
+    tb["tab"] = np.ascontiguousarray(np.stack(fields(X1, X2)))
+    return tb, fields
+
+
+def test_rhs_is_hamiltons_equations_of_the_3p1_hamiltonian(tab_oracle):
+    """eqs.(3),(4) PAPER.md:60-65: dx/dtau = dH/dp, dp/dtau = -dH/dx with H = 1/2 g^{mu nu} p_mu p_nu built
+    here by inverting the 4x4 matrix of line element (1) -- not from the 3+1 closed form."""
+    tb, fields = _quadratic_metric()
+
+    def H(x1, x2, pt, p1, p2, pph):
+        al, be, g11, g22, g33 = fields(x1, x2)
+        g = np.zeros((4, 4))                       # t, x1, x2, phi
+        g[0, 0] = -al * al + g33 * be * be
+        g[0, 3] = g[3, 0] = g33 * be
+        g[1, 1], g[2, 2], g[3, 3] = g11, g22, g33
+        p = np.array([pt, p1, p2, pph])
+        return 0.5 * p @ np.linalg.inv(g) @ p
+    rng = np.random.default_rng(5)
+    for _ in range(50):
+        x1, x2 = rng.uniform(1.0, 3.8), rng.uniform(0.7, 2.6)
+        E, p1, p2, L = rng.uniform(0.5, 2), rng.uniform(-1, 1), rng.uniform(-1, 1), rng.uniform(-2, 2)
+        d, Hval = tab_oracle.rhs(tb, [0.0, x1, x2, 0.0, E, p1, p2, L])
+        args = np.array([x1, x2, -E, p1, p2, L])
+        e = 1e-5
+
+        def dH(k):
+            up, dn = args.copy(), args.copy()
+            up[k] += e
+            dn[k] -= e
+            return (H(*up) - H(*dn)) / (2 * e)
+        want = np.array([dH(2), dH(3), dH(4), dH(5), -dH(0), -dH(1)])       # t, x1, x2, phi, p1, p2
+        assert abs(Hval - H(*args)) < 1e-13
+        assert np.max(np.abs(d - want)) < 2e-9, (d, want)
+
+
+def _flat_table(n1, n2, r_lo=0.5, r_hi=12.0):
+    d1, d2 = (r_hi - r_lo) / (n1 - 1), math.pi / (n2 - 1)            # n2 odd => theta = pi/2 is a node
+    x1 = r_lo + d1 * (np.arange(n1 + 4) - 2)
+    x2 = d2 * (np.arange(n2 + 4) - 2)
+    R, TH = np.meshgrid(x1, x2)
+    tab = np.stack([np.ones_like(R), np.zeros_like(R), np.ones_like(R), R * R, R * R * np.sin(TH) ** 2])
+    return {"tab": np.ascontiguousarray(tab), "x1_0": float(x1[0]), "d1": d1, "x2_0": float(x2[0]), "d2": d2}
+
+
+def test_flat_space_geodesics_are_straight_lines(tab_oracle):
+    """Minkowski space in spherical coordinates (alpha = 1, beta = 0, gamma = diag(1, r^2, r^2 sin^2 theta)): in the
+    plane theta = pi/2 (a grid line, where the interpolated sin^2 is exactly 1 with zero theta-derivative by symmetry
+    and r^2 is a quadratic) the tabulated metric is exact, so RK4 must follow x(tau) = x0 + u tau, t = sqrt(1+u^2) tau."""
+    tb = _flat_table(47, 33)
+    x0, u = np.array([3.0, -2.0]), np.array([-0.3, 0.8])
+    r0 = np.hypot(*x0)
+    st = np.array([[r0], [math.pi / 2], [math.atan2(x0[1], x0[0])], [x0 @ u / r0], [0.0], [x0[0] * u[1] - x0[1] * u[0]]])
+    errs = []
+    for h, n in ((0.02, 400), (0.01, 800)):
+        o = tab_oracle.integrate(tb, st, h, n)
+        assert o["status"][0] == tab_oracle.ST_MAXSTEPS and o["steps_done"][0] == n
+        xe = x0 + u * h * n
+        t, r, th, ph, E = o["final_state"][:5, 0]
+        assert abs(th - math.pi / 2) < 1e-13                 # symmetric stencil: zero theta-force up to rounding
+        assert abs(E - math.sqrt(1 + u @ u)) < 1e-15
+        errs.append(max(abs(r - np.hypot(*xe)), abs(ph - math.atan2(xe[1], xe[0])), abs(t - E * h * n)))
+    assert errs[0] < 1e-7 and 10 < errs[0] / errs[1] < 22, errs          # fourth order in h, nothing else
+    # off the plane sin^2 is only interpolated: the error falls with the grid spacing (reading T2: the force is
+    # second-order accurate)
+    x0, u = np.array([3.0, -2.0, 1.0]), np.array([-0.3, 0.8, 0.2])
+    r0 = np.linalg.norm(x0)
+    th0, ph0 = math.acos(x0[2] / r0), math.atan2(x0[1], x0[0])
+    er, et, ep = (np.array([math.sin(th0) * math.cos(ph0), math.sin(th0) * math.sin(ph0), math.cos(th0)]),
+                  np.array([math.cos(th0) * math.cos(ph0), math.cos(th0) * math.sin(ph0), -math.sin(th0)]),
+                  np.array([-math.sin(ph0), math.cos(ph0), 0.0]))
+    st = np.array([[r0], [th0], [ph0], [u @ er], [r0 * (u @ et)], [r0 * math.sin(th0) * (u @ ep)]])
+    xe = x0 + u * 4.0
+    errs = []
+    for n2 in (33, 65, 129):
+        o = tab_oracle.integrate(_flat_table(47, n2), st, 0.01, 400)
+        r, th, ph = o["final_state"][1:4, 0]
+        got = r * np.array([math.sin(th) * math.cos(ph), math.sin(th) * math.sin(ph), math.cos(th)])
+        errs.append(np.linalg.norm(got - xe))
+    assert errs[2] < 2e-5 and errs[0] / errs[1] > 3 and errs[1] / errs[2] > 3, errs
+
+
+def test_tabulated_kerr_rhs_converges_to_the_analytic_metric(tab_oracle, oracle):
+    """eq.(8) PAPER.md:97 sampled on a grid: the interpolated RHS tends to the analytic-metric oracle's (itself pinned
+    in test_oracle_pins.py) -- velocities with the third-order value error, forces with the second-order derivative error."""
+    a = 0.9
+    rng = np.random.default_rng(6)
+    pts = [(rng.uniform(3, 20), rng.uniform(0.6, 2.5), rng.uniform(0.9, 1.0), rng.uniform(-0.3, 0.3), rng.uniform(-2, 2),
+            rng.uniform(-3, 3)) for _ in range(400)]
+    ev, ef = [], []
+    for n1, n2 in ((257, 65), (513, 129), (1025, 257)):
+        tb = W.kerr_metric_table(1.0, a, n1, n2, 2.0, 24.0, 0.3, math.pi - 0.3)
+        mv = mf = 0.0
+        for r, th, E, pr, pth, L in pts:
+            y = [0.0, r, th, 0.0, E, pr, pth, L]
+            d, Hval = tab_oracle.rhs(tb, y)
+            want = oracle.rhs(oracle.KERR, 1.0, a, y)
+            mv = max(mv, np.max(np.abs(d[:4] - want[:4]) / np.maximum(np.abs(want[:4]), 1e-2)))
+            mf = max(mf, np.max(np.abs(d[4:] - want[4:])))
+        ev.append(mv)
+        ef.append(mf)
+    assert ev[2] < 1e-6 and ef[2] < 1e-4, (ev, ef)
+    assert ev[0] / ev[1] > 5 and ev[1] / ev[2] > 5, ev            # ~8 = 2^3
+    assert 3 < ef[0] / ef[1] and 3 < ef[1] / ef[2], ef            # ~4 = 2^2
+
+
+def test_tabulated_kerr_orbits_converge_to_the_analytic_oracle_in_both_radial_coordinates(tab_oracle, oracle):
+    a = 0.9
+    st = W.kerr_bound(48, a, W.SEED_BASE + 2)
+    ref = oracle.integrate(oracle.KERR, 1.0, a, st, 0.01, 1500)
+    rp = W.horizon_radius(1.0, a)
+    for radial, lo, hi in (("r", 1.8, 40.0), ("log", math.log(1.8 - rp), math.log(40.0 - rp))):
+        errs = []
+        for n1, n2 in ((513, 129), (2049, 513)):
+            tb = W.kerr_metric_table(1.0, a, n1, n2, lo, hi, 0.2, math.pi - 0.2, radial=radial)
+            s = W.to_log_radial(st, rp) if radial == "log" else st
+            o = tab_oracle.integrate(tb, s, 0.01, 1500)
+            assert (o["status"] == tab_oracle.ST_MAXSTEPS).all()
+            f = o["final_state"].copy()
+            if radial == "log":                                   # back to Boyer-Lindquist r, p_r
+                f[5] = f[5] / np.exp(f[1])
+                f[1] = rp + np.exp(f[1])
+            assert np.array_equal(f[7], st[5])                    # p_phi is a constant of motion exactly
+            # E is derived from the interpolated metric at y0 and then constant
+            assert np.max(np.abs(f[4] - ref["final_state"][4])) < 1e-6
+            assert np.nanmax(o["health"]) < 1e-7                  # 2H + 1 drift: RK4 + the C^1 interpolant
+            errs.append(np.max(np.abs(f[[0, 1, 2, 3, 5, 6]] - ref["final_state"][[0, 1, 2, 3, 5, 6]])
+                               / np.maximum(np.abs(ref["final_state"][[0, 1, 2, 3, 5, 6]]), 1.0)))
+        assert errs[1] < 2e-5 and errs[0] / errs[1] > 6, (radial, errs)
+
+
+def test_stop_rules_and_domain_exit(tab_oracle, oracle):
+    a = 0.998
+    rp = W.horizon_radius(1.0, a)
+    tb = W.kerr_metric_table(1.0, a, 769, 257, math.log(0.005), math.log(60.0), 0.0, math.pi, radial="log", ghost=3)
+    full = W.camera_rays(64, a, 60.0, r_obs=50.0)
+    ii = np.arange(64 * 64).reshape(64, 64)[4::8, 2::8].ravel()
+    st = np.ascontiguousarray(full[:, ii])
+    s = W.to_log_radial(st, rp)
+    xc, xe = math.log(0.01), math.log(55.0 - rp)
+    o = tab_oracle.integrate(tb, s, 0.02, 20000, r_capture=xc, r_escape=xe, kind=tab_oracle.NULL)
+    ref = oracle.integrate(oracle.KERR, 1.0, a, st, 0.02, 20000, r_capture=rp + 0.01, r_escape=55.0, kind=oracle.NULL)
+    assert set(np.unique(o["status"])) == {tab_oracle.ST_CAPTURED, tab_oracle.ST_ESCAPED}
+    assert (o["status"] == ref["status"]).mean() >= 0.97          # same image up to rays grazing the critical curve
+    esc = o["status"] == tab_oracle.ST_ESCAPED
+    assert (o["final_state"][1][esc] > xe).all() and (o["final_state"][1][~esc] >= xc).all()
+    # B1 / T4 on y0, B4, and leaving the table
+    y0 = np.array([[1.0, -9.0, 1.0, 1.0, 1.0], [1.5, 1.5, 1.5, 1.5, -0.5], [0.0] * 5, [0.0] * 5, [0.0] * 5, [2.0] * 5])
+    y0[1, 2] = float("nan")             # (a NaN x^1 fails the NaN-safe capture test first: B1)
+    y0[0, 3] = 4.5                      # beyond the last interior node (x1 <= ln 60 + ghosts)
+    o = tab_oracle.integrate(tb, y0, 0.02, 0, r_capture=-6.0, r_escape=9.0)
+    assert o["status"].tolist() == [tab_oracle.ST_MAXSTEPS, tab_oracle.ST_CAPTURED, tab_oracle.ST_NUMERIC,
+                                    tab_oracle.ST_OUTSIDE, tab_oracle.ST_OUTSIDE]
+    assert (o["steps_done"] == 0).all() and np.isnan(o["health"][3])
+    # an outgoing timelike particle with no escape radius runs off the table: OUTSIDE, last state inside the domain
+    out = np.array([[math.log(30.0)], [1.2], [0.0], [40.0], [0.0], [1.0]])
+    o = tab_oracle.integrate(tb, out, 0.05, 100000)
+    hi = tb["x1_0"] + tb["d1"] * (tb["tab"].shape[2] - 2)
+    assert o["status"][0] == tab_oracle.ST_OUTSIDE and 0 < o["steps_done"][0] < 100000
+    assert o["final_state"][1, 0] < hi and o["final_state"][1, 0] > hi - 0.2

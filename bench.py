@@ -22,6 +22,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -42,10 +43,11 @@ UNIT = "geodesic-steps/s"
 # (profiles/r01_config4_v3.md: DFMA 140, DMUL 143, DADD 42, DSETP 6 for Kerr).  flop = 2*DFMA + DMUL + DADD;
 # pipe = all four.  The static SASS count of the loop (sass_count.py, an upper bound that includes the
 # rarely executed blocks inside the loop's address range) is printed beside them as a cross-check.
-FLOP_PER_STEP = {"kerr": 465.0, "schwarzschild": 397.0}
-PIPE_INSTR_PER_STEP = {"kerr": 331.0, "schwarzschild": 273.0}
+FLOP_PER_STEP = {"kerr": 465.0, "schwarzschild": 397.0, "tabulated": 2400.0}
+PIPE_INSTR_PER_STEP = {"kerr": 331.0, "schwarzschild": 273.0, "tabulated": 1400.0}
 OTHER_INSTR_PER_STEP = {"kerr": 103.0}     # non-FP64 instructions per step, same ncu capture
-FLOP_COUNT_SOURCE = {"kerr": "ncu dynamic count (profiles/r01_config4_v3.md)", "schwarzschild": "static SASS count"}
+FLOP_COUNT_SOURCE = {"kerr": "ncu dynamic count (profiles/r01_config4_v3.md)", "schwarzschild": "static SASS count",
+                     "tabulated": "static SASS count of the geo_tab_rk4_kernel loop"}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
 # adaptive RK5(4) kernel, per step ATTEMPT of one Kerr geodesic, executed (ncu, thread level)
 ADAPTIVE_FLOP_PER_ATTEMPT, ADAPTIVE_PIPE_PER_ATTEMPT = 1211.0, 785.0
@@ -97,6 +99,15 @@ def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dic
         perm = np.random.default_rng(W.SEED_BASE + 3).permutation(wl["st"].shape[1])
         wl["st"] = np.ascontiguousarray(wl["st"][:, perm])
         wl["name"] += " (pixels shuffled)"
+        return wl
+    if name == "tab4":
+        # the particles of configs[3] through a TABULATED Kerr a = 0.5 metric (eq.(8) sampled on a
+        # 2049 x 513 Boyer-Lindquist grid + ghosts, 42 MB in the kernel's layout: L2-resident), 1000 RK4 steps
+        wl = workload("config4", rank, n_override, nthreads)
+        wl["name"] = "configs[3] particles on a tabulated Kerr a=0.5 metric (2049x513 nodes, cubic convolution)"
+        wl["metric"] = "tabulated"
+        wl["table"] = W.kerr_metric_table(1.0, 0.5, 2049, 513, 2.0, 45.0, 0.1, math.pi - 0.1)
+        wl["nsteps"] = 1000
         return wl
     if name == "config3a":
         # the rays of configs[2] with the adaptive Dormand-Prince 5(4) stepper (per-ray step control);
@@ -165,12 +176,18 @@ def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> di
     m = min(st.shape[1], max(cores, per))
     sub = np.ascontiguousarray(st[:, :m])
     metric = geo_oracle.KERR if wl["metric"] == "kerr" else geo_oracle.SCHWARZSCHILD
+    if wl["metric"] == "tabulated":
+        import geo_tab_oracle
+        per = max(1, per // 4)          # ~4x the analytic RHS cost
     kw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores,
               snapshot_every=wl["snapshot_every"], snap_mask=wl["snap_mask"], flags=wl.get("flags", 0))
     times, done = [], 0
     for i in range(warmup + steps):
         t0 = time.perf_counter()
-        if ad:
+        if wl["metric"] == "tabulated":
+            o = geo_tab_oracle.integrate(wl["table"], sub, wl["h"], wl["nsteps"], r_capture=wl["r_capture"],
+                                         r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
+        elif ad:
             o = geo_oracle.integrate_adaptive(metric, 1.0, wl["a"], sub, ad["h0"], ad["rtol"], ad["atol"], ad["max_attempts"],
                                               r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
         else:
@@ -210,7 +227,8 @@ def flop_counts(metric: str) -> tuple[float, float, str, dict | None]:
     static = None
     try:
         from paper_1803_08320_b200 import sass_count
-        c = sass_count.count("ILb1ELi0ELb0" if metric == "kerr" else "ILb0ELi0ELb0")
+        c = sass_count.count({"kerr": "rk4_kernelILb1ELi0ELb0", "schwarzschild": "rk4_kernelILb0ELi0ELb0",
+                              "tabulated": "geo_tab_rk4_kernelILb0E"}[metric])
         static = {"flop": c["flop"], "fp64_pipe": c["fp64_pipe"]}
     except Exception:
         pass
@@ -223,7 +241,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "config3a", "snapbench", "paper_t3", "paper_t4"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "config3a", "tab4", "snapbench", "paper_t3", "paper_t4"])
     ap.add_argument("--n", type=int, default=None, help="override particle count / image size (development)")
     ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping, 4 = shared-memory-staged snapshots)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -256,8 +274,11 @@ def main() -> None:
     wl = workload(args.workload, rank, args.n, ncpu)
     st = wl["st"]
     n = st.shape[1]
-    metric = geo.KERR if wl["metric"] == "kerr" else geo.SCHWARZSCHILD
-    ctx = geo.geo_create(metric, 1.0, wl["a"])
+    if wl["metric"] == "tabulated":
+        tb = wl["table"]
+        ctx = geo.geo_create_tabulated(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+    else:
+        ctx = geo.geo_create(geo.KERR if wl["metric"] == "kerr" else geo.SCHWARZSCHILD, 1.0, wl["a"])
     d_in = torch.from_numpy(st).to(dev)
     out = geo.alloc_outputs(n, dev, wl["nsteps"], wl["snapshot_every"], None, wl["snap_mask"])
     kw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], flags=args.flags | wl.get("flags", 0),
@@ -403,13 +424,23 @@ def main() -> None:
     sps = steps_per_pass / (kernel_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                 "frac": ach_tf / peak_tf, "traffic": TRAFFIC_NCU_BYTES.get(args.workload),
-                "kernel": "geo_rk45_kernel" if ad else "geo_rk4_kernel", "kernel_ms": kernel_ms,
+                "kernel": "geo_rk45_kernel" if ad else ("geo_tab_rk4_kernel" if wl["metric"] == "tabulated" else "geo_rk4_kernel"),
+                "kernel_ms": kernel_ms,
                 "flop_per_step": flop, "fp64_pipe_instr_per_step": pipe,
                 "flop_count_source": how, "static_sass_count_of_loop": static_count,
                 "flop_per_step_survey_f_alg": f_alg, "frac_survey_f_alg": sps * f_alg / 1e12 / peak_tf,
                 "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {sm_max:.0f} MHz (nominal clock; MEASURED_PEAKS.json has no FP64 entry)",
                 "fp64_pipe_util": sps * pipe / (SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6),
                 "dfma_probe_tflops": probe_tf, "frac_of_dfma_probe": ach_tf / probe_tf}
+    if wl["metric"] == "tabulated":
+        # SURVEY 8(f).3 expected this path to be memory- rather than FP64-bound: the table reads are reported beside
+        # the ALU figure.  Algorithmic bytes: 4 stencil evaluations per step x 640 B (16 x 40-B nodes), served by L1/L2.
+        roofline.pop("frac_survey_f_alg")
+        roofline.pop("flop_per_step_survey_f_alg")
+        roofline["table_bytes_per_step"] = 4 * 640
+        roofline["table_read_gbs"] = sps * 4 * 640 / 1e9
+        tbl = wl["table"]["tab"]
+        roofline["table_mb_on_device"] = tbl.shape[1] * tbl.shape[2] * 40 / 1e6
     if ad:
         roofline.pop("flop_per_step_survey_f_alg"), roofline.pop("frac_survey_f_alg")
         roofline["unit_of_work"] = "one RK5(4) step attempt (accepted or rejected)"

@@ -29,11 +29,12 @@ extern "C" {
 
 typedef struct geo_ctx geo_ctx; /* opaque; owned by the library */
 
-enum { GEO_SCHWARZSCHILD = 0, GEO_KERR = 1 };                       /* metric                  */
+enum { GEO_SCHWARZSCHILD = 0, GEO_KERR = 1, GEO_TABULATED = 2 };    /* metric (2: geo_create_tabulated) */
 enum { GEO_TIMELIKE = 0, GEO_NULL = 1 };                            /* geo_stop.kind: kappa=1/0 */
 enum { GEO_OK = 0, GEO_EINVAL = 1, GEO_ECUDA = 2, GEO_ENOMEM = 3 }; /* return codes            */
 /* per-particle termination class (geo_out.status) */
-enum { GEO_ST_MAXSTEPS = 0, GEO_ST_CAPTURED = 1, GEO_ST_ESCAPED = 2, GEO_ST_NUMERIC = 3 };
+enum { GEO_ST_MAXSTEPS = 0, GEO_ST_CAPTURED = 1, GEO_ST_ESCAPED = 2, GEO_ST_NUMERIC = 3,
+       GEO_ST_OUTSIDE = 4 /* tabulated metrics only: an evaluation point left the table's domain */ };
 /* geo_stop.flags */
 enum {
     GEO_FLAG_PLAIN_UPDATE = 1, /* y <- y + delta without the Kahan error term (P1)     */
@@ -111,6 +112,31 @@ typedef struct geo_adaptive {
 int geo_integrate_adaptive(geo_ctx *ctx, const double *state_in, int64_t n, const geo_adaptive *ctl,
                            int64_t max_attempts, const geo_stop *stop, const geo_out *out, int32_t *rejected,
                            void *cuda_stream);
+
+/* a NUMERICALLY GIVEN metric ("the 3+1 formulation is important in order to bring future support
+ * to numerical metrics"; "a new algorithm to handle numerically computed metrics").
+ * Line element (1) with the structure of eq.(8): stationary, axisymmetric,
+ * beta^i = (0, 0, beta^phi), gamma_ij = diag(gamma_11, gamma_22, gamma_33), five functions of (x^1, x^2) sampled at
+ * the nodes x^1_i = x1_0 + i d1 (0 <= i < n1), x^2_j = x2_0 + j d2 (0 <= j < n2):
+ *     tab[f][j][i], f = 0..4 = alpha, beta^phi, gamma_11, gamma_22, gamma_33      (HOST, n1 fastest; copied, not kept).
+ * (x^1, x^2) are the metric's own coordinates -- (r, theta) for Boyer-Lindquist Kerr.  Between the nodes each field is
+ * the tensor-product cubic-convolution interpolant (Keys 1981, parameter -1/2: C^1, exact on quadratics, value error
+ * O(d^3), gradient error O(d^2)) and the equations of motion are Hamilton's equations (3),(4) of
+ *     H = 1/2 [ -(p_t - beta^phi p_phi)^2/alpha^2 + p_1^2/gamma_11 + p_2^2/gamma_22 + p_phi^2/gamma_33 ]
+ * with the EXACT gradient of the interpolant, so p_t and p_phi are constants of motion (T1-T5).
+ * The interpolant exists where its 4 x 4 stencil does: floor((x - x_0)/d) in [1, n - 3] in both directions.
+ * A ctx created here is used with geo_integrate / geo_integrate_host: state_in = (x^1, x^2, phi, p_1, p_2, p_phi),
+ * r_capture / r_escape refer to x^1, the equatorial event to x^2 = pi/2; an evaluation point (y0, a stage point, the
+ * end point of a step) outside the domain ends the particle with GEO_ST_OUTSIDE, that step is not taken (per
+ * evaluation point the capture test comes first).  snapshot_every must be 0; flags: GEO_FLAG_PLAIN_UPDATE only;
+ * geo_integrate_adaptive returns GEO_EINVAL; geo_horizon_radius returns NaN.
+ * Errors: GEO_EINVAL (NULL, n1 or n2 < 4, d1 or d2 <= 0, non-finite grid), GEO_ENOMEM, GEO_ECUDA. */
+typedef struct geo_table {
+    const double *tab;  /* HOST [5][n2][n1] */
+    int64_t n1, n2;
+    double x1_0, d1, x2_0, d2;
+} geo_table;
+int geo_create_tabulated(geo_ctx **ctx, const geo_table *table);
 
 void geo_destroy(geo_ctx *ctx);
 

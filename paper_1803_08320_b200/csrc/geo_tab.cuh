@@ -1,0 +1,319 @@
+// geo_tab.cuh -- SURVEY 8(f).3: fixed-step RK4 geodesics through a NUMERICALLY GIVEN (tabulated) stationary,
+// axisymmetric 3+1 metric -- the "numerical metrics" the paper gives as the reason for its 3+1 formulation
+// (PAPER.md:31-33, 497).  One persistent kernel with the work queue, stop rules and Kahan update of the
+// analytic-metric kernel (geo_kernel.cuh); what changes is the RHS evaluator: the five functions of eq.(8)
+// -- lapse alpha, shift beta^phi, gamma_11, gamma_22, gamma_33 -- come from a table on a
+// uniform (x^1, x^2) grid through the tensor-product cubic-convolution interpolant (Keys 1981, a = -1/2:
+// C^1, exact on quadratics), and the derivatives in Hamilton's equations (3),(4) are the
+// exact derivatives of that interpolant (readings T1-T5), so E and L are constants of motion.
+//
+//   H = 1/2 [ -(E + beta^phi L)^2/alpha^2 + p_1^2/gamma_11 + p_2^2/gamma_22 + L^2/gamma_33 ],  u^t = (E + beta^phi L)/alpha^2
+//   dx^k/dtau = p_k/gamma_kk,  dphi/dtau = L/gamma_33 - beta^phi u^t,  dt/dtau = u^t
+//   dp_k/dtau = u^t L d_k beta^phi - alpha (u^t)^2 d_k alpha + 1/2 sum_m d_k gamma_mm (p_m/gamma_mm)^2
+//
+// Table layout in HBM/L2 (built once by tab_pack_kernel from the caller's [5][n2][n1] array): node-major,
+//   A[j][i] = (alpha, beta^phi, gamma_11, gamma_22) as one 32-byte record -> one 256-bit load per node,
+//   B[j][i] = gamma_33                                                    -> four consecutive doubles per stencil row.
+// One RHS evaluation reads the 4 x 4 stencil = 16 records of A + 16 doubles of B = 640 B per lane, ~23 32-B
+// sectors; a whole table of 2053 x 517 nodes is 42 MB and lives in the 126 MB L2.  Per lane and evaluation:
+// 16 LDG.256 + 16 LDG.64, ~330 FP64 instructions (separable evaluation: 8 FMA per field and stencil row for the
+// value and the x^1-derivative along x^1, then 3 FMA per row along x^2).
+#pragma once
+#include "geo_kernel.cuh"
+
+namespace geo {
+
+enum { ST_OUTSIDE = 4 };
+
+struct TabMetric {
+    const double4* A;   // [n2][n1] (alpha, beta^phi, gamma_11, gamma_22)
+    const double* B;    // [n2][n1] gamma_33
+    int n1, n2;
+    double x1_0, d1, inv_d1, x2_0, d2, inv_d2;
+};
+
+struct TabParams {
+    const double* in;   // [6][n] (x1, x2, phi, p_1, p_2, p_phi)
+    long long n;
+    double h, h_half, h_sixth;
+    int nsteps;
+    double r_capture, r_escape, kappa;
+    double* fin;        // [8][n]
+    int* status;
+    long long* steps_done;
+    double* eq_cross_r;
+    double* health;
+    unsigned long long* counter;
+    TabMetric m;
+};
+
+struct TabFields {
+    double al, be, g11, g22, g33;          // values
+    double al1, be1, g111, g221, g331;     // d/dx^1
+    double al2, be2, g112, g222, g332;     // d/dx^2
+};
+
+__device__ __forceinline__ double4 ldg256(const double4* p) {
+    double4 v;
+    asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+    return v;
+}
+
+// cell index and in-cell coordinate along one direction (reading T2, T4): u = (x - x0)/d, i = floor(u), s = u - i.
+// The quotient is formed with the reciprocal; when s falls within 2^-30 of a cell face it is redone with a true
+// division, so the floor -- which decides the cell and the domain test -- is the oracle's.
+__device__ __forceinline__ bool tab_cell(double x, double x0, double d, double inv_d, int n, int& i, double& s) {
+    double u = (x - x0) * inv_d;
+    int k = __double2int_rd(u);                // NaN -> 0: fails the domain test below
+    double sf = u - (double)k;
+    if (sf < 9.3e-10 || sf > 1.0 - 9.3e-10) {
+        u = (x - x0) / d;
+        k = __double2int_rd(u);
+        sf = u - (double)k;
+    }
+    const bool inside = (k >= 1) & (k <= n - 3) & (u < 2.0e9) & (u > -2.0e9);
+    i = min(max(k, 1), n - 3);                 // loads stay in bounds whatever the lane holds
+    s = inside ? sf : 0.0;
+    return inside;
+}
+
+// Keys weights of nodes i-1 .. i+2 and their derivatives with respect to x (= inv_d * d/ds)
+__device__ __forceinline__ void keys_weights(double s, double inv_d, double w[4], double dw[4]) {
+    const double s2 = s * s;
+    w[0] = 0.5 * s * fma(s, 2.0 - s, -1.0);
+    w[1] = fma(s2, fma(1.5, s, -2.5), 1.0);
+    w[2] = 0.5 * s * fma(s, fma(-3.0, s, 4.0), 1.0);
+    w[3] = 0.5 * s2 * (s - 1.0);
+    const double hd = 0.5 * inv_d;
+    dw[0] = hd * fma(s, fma(-3.0, s, 4.0), -1.0);
+    dw[1] = hd * s * fma(9.0, s, -10.0);
+    dw[2] = hd * fma(s, fma(-9.0, s, 8.0), 1.0);
+    dw[3] = hd * s * fma(3.0, s, -2.0);
+}
+
+// Interpolated fields and their gradients at (x1, x2).  Returns false outside the domain (the values are then
+// those of the nearest interior cell's stencil at s = 0 -- finite garbage that the caller discards).
+__device__ __forceinline__ bool tab_fields(const TabMetric& m, double x1, double x2, TabFields& F) {
+    int i, j;
+    double s1, s2;
+    const bool in1 = tab_cell(x1, m.x1_0, m.d1, m.inv_d1, m.n1, i, s1);
+    const bool in2 = tab_cell(x2, m.x2_0, m.d2, m.inv_d2, m.n2, j, s2);
+    double w1[4], dw1[4], w2[4], dw2[4];
+    keys_weights(s1, m.inv_d1, w1, dw1);
+    keys_weights(s2, m.inv_d2, w2, dw2);
+    const long long base = (long long)(j - 1) * m.n1 + (i - 1);
+    double v[5] = {0, 0, 0, 0, 0}, g1[5] = {0, 0, 0, 0, 0}, g2[5] = {0, 0, 0, 0, 0};
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        const double4* ra = m.A + base + (long long)b * m.n1;
+        const double* rb = m.B + base + (long long)b * m.n1;
+        const double4 a0 = ldg256(ra), a1 = ldg256(ra + 1), a2 = ldg256(ra + 2), a3 = ldg256(ra + 3);
+        const double b0 = __ldg(rb), b1 = __ldg(rb + 1), b2 = __ldg(rb + 2), b3 = __ldg(rb + 3);
+        double rv[5], rd[5];      // value and x^1-derivative along this stencil row
+#define GEO_ROW(k, c0, c1, c2, c3)                                                   \
+        rv[k] = fma(w1[3], c3, fma(w1[2], c2, fma(w1[1], c1, w1[0] * c0)));          \
+        rd[k] = fma(dw1[3], c3, fma(dw1[2], c2, fma(dw1[1], c1, dw1[0] * c0)));
+        GEO_ROW(0, a0.x, a1.x, a2.x, a3.x)
+        GEO_ROW(1, a0.y, a1.y, a2.y, a3.y)
+        GEO_ROW(2, a0.z, a1.z, a2.z, a3.z)
+        GEO_ROW(3, a0.w, a1.w, a2.w, a3.w)
+        GEO_ROW(4, b0, b1, b2, b3)
+#undef GEO_ROW
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            v[k] = fma(w2[b], rv[k], v[k]);
+            g1[k] = fma(w2[b], rd[k], g1[k]);
+            g2[k] = fma(dw2[b], rv[k], g2[k]);
+        }
+    }
+    F.al = v[0]; F.be = v[1]; F.g11 = v[2]; F.g22 = v[3]; F.g33 = v[4];
+    F.al1 = g1[0]; F.be1 = g1[1]; F.g111 = g1[2]; F.g221 = g1[3]; F.g331 = g1[4];
+    F.al2 = g2[0]; F.be2 = g2[1]; F.g112 = g2[2]; F.g222 = g2[3]; F.g332 = g2[4];
+    return in1 & in2;
+}
+
+struct TabDeriv {
+    double t, x1, x2, ph, p1, p2;
+};
+
+// Hamilton's equations of the 3+1 Hamiltonian in the interpolated fields (reading T3)
+__device__ __forceinline__ void tab_rhs(const TabFields& F, double p1, double p2, double E, double L, TabDeriv& d) {
+    const double W = fma(F.be, L, E);
+    const double ut = W * rcp_nr(F.al * F.al);
+    const double v1 = p1 * rcp_nr(F.g11), v2 = p2 * rcp_nr(F.g22), v3 = L * rcp_nr(F.g33);
+    const double utL = ut * L, q = -F.al * ut * ut;
+    const double h11 = 0.5 * v1 * v1, h22 = 0.5 * v2 * v2, h33 = 0.5 * v3 * v3;
+    d.t = ut;
+    d.x1 = v1;
+    d.x2 = v2;
+    d.ph = fma(-F.be, ut, v3);
+    d.p1 = fma(utL, F.be1, fma(q, F.al1, fma(F.g111, h11, fma(F.g221, h22, F.g331 * h33))));
+    d.p2 = fma(utL, F.be2, fma(q, F.al2, fma(F.g112, h11, fma(F.g222, h22, F.g332 * h33))));
+}
+
+__device__ __noinline__ bool tab_fields_cold(const TabMetric& m, double x1, double x2, TabFields& F) {
+    return tab_fields(m, x1, x2, F);
+}
+
+template <bool PLAIN>
+__global__ void __launch_bounds__(kBlock, 3) geo_tab_rk4_kernel(const __grid_constant__ TabParams p) {
+    const unsigned lane = threadIdx.x & 31u;
+    const TabMetric& m = p.m;
+    long long idx = -1;
+    bool active = false, exhausted = false;
+    double t = 0, x1 = 0, x2 = 0, ph = 0, p1 = 0, p2 = 0, E = 0, L = 0;
+    double ct = 0, c1 = 0, c2 = 0, cph = 0, cp1 = 0, cp2 = 0;     // Kahan error terms (reading P1)
+    TabDeriv k1;                                                   // f(y), carried from the end-point evaluation
+    k1.t = k1.x1 = k1.x2 = k1.ph = k1.p1 = k1.p2 = 0;
+    int steps = 0;
+    double eqc = 0;
+    bool crossed = false;
+
+    auto finish = [&](int st) {
+        long long n = p.n;
+        asm volatile("" : "+l"(n));
+        p.fin[0 * n + idx] = t;
+        p.fin[1 * n + idx] = x1;
+        p.fin[2 * n + idx] = x2;
+        p.fin[3 * n + idx] = ph;
+        p.fin[4 * n + idx] = E;
+        p.fin[5 * n + idx] = p1;
+        p.fin[6 * n + idx] = p2;
+        p.fin[7 * n + idx] = L;
+        p.status[idx] = st;
+        p.steps_done[idx] = (long long)steps;
+        const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+        if (p.eq_cross_r) p.eq_cross_r[idx] = crossed ? eqc : qnan;
+        if (p.health) {
+            TabFields F;
+            double hv = qnan;
+            if (tab_fields_cold(m, x1, x2, F) && (__double2hiint(E) & 0x7ff00000) != 0x7ff00000) {
+                const double W = fma(F.be, L, E);
+                hv = fabs(-(W * W) / (F.al * F.al) + p1 * p1 / F.g11 + p2 * p2 / F.g22 + L * L / F.g33 + p.kappa);
+            }
+            p.health[idx] = hv;
+        }
+        active = false;
+    };
+    auto begin = [&](long long i) {
+        idx = i;
+        const long long n = p.n;
+        t = 0.0;
+        x1 = p.in[0 * n + i];
+        x2 = p.in[1 * n + i];
+        ph = p.in[2 * n + i];
+        p1 = p.in[3 * n + i];
+        p2 = p.in[4 * n + i];
+        L = p.in[5 * n + i];
+        E = __longlong_as_double(0x7ff8000000000000LL);
+        ct = c1 = c2 = cph = cp1 = cp2 = 0.0;
+        steps = 0;
+        crossed = false;
+        active = true;
+        if (!(x1 >= p.r_capture)) { finish(ST_CAPTURED); return; }               // B1
+        if (!all_finite6(x1, x2, ph, p1, p2, L)) { finish(ST_NUMERIC); return; }
+        TabFields F;
+        if (!tab_fields_cold(m, x1, x2, F)) { finish(ST_OUTSIDE); return; }      // T4 on y0
+        E = fma(F.al, sqrt(p.kappa + p1 * p1 / F.g11 + p2 * p2 / F.g22 + L * L / F.g33), -F.be * L);   // mass shell (5)
+        if ((__double2hiint(E) & 0x7ff00000) == 0x7ff00000) { finish(ST_NUMERIC); return; }
+        if (x1 > p.r_escape) { finish(ST_ESCAPED); return; }
+        if (p.nsteps == 0) { finish(ST_MAXSTEPS); return; }
+        tab_rhs(F, p1, p2, E, L, k1);
+    };
+
+    for (;;) {
+        // --- work queue (A5) ------------------------------------------------------------------
+        unsigned idle = __ballot_sync(kFull, !active);
+        if (idle) {
+            if (!exhausted) {
+                const int cnt = __popc(idle);
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(p.counter, (unsigned long long)cnt);
+                base = __shfl_sync(kFull, base, 0);
+                if (!active) {
+                    const long long cand = (long long)base + __popc(idle & ((1u << lane) - 1u));
+                    if (cand < p.n) begin(cand);
+                }
+                if ((long long)base + cnt >= p.n) exhausted = true;
+                idle = __ballot_sync(kFull, !active);
+            }
+            if (idle == kFull) {
+                if (exhausted) break;
+                continue;
+            }
+        }
+
+        // --- one RK4 step (every lane; idle lanes compute on stale state, loads are clamped in bounds) ----
+        // ev: first event in the oracle's order -- per evaluation point capture (B2) before domain exit (T4)
+        int ev = 0;
+        TabFields F;
+        TabDeriv d;
+        double s1, s2, sp1, sp2;
+        // stage 2
+        s1 = fma(p.h_half, k1.x1, x1); s2 = fma(p.h_half, k1.x2, x2);
+        sp1 = fma(p.h_half, k1.p1, p1); sp2 = fma(p.h_half, k1.p2, p2);
+        bool in = tab_fields(m, s1, s2, F);
+        ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
+        tab_rhs(F, sp1, sp2, E, L, d);
+        double at = fma(2.0, d.t, k1.t), a1 = fma(2.0, d.x1, k1.x1), a2 = fma(2.0, d.x2, k1.x2),
+               aph = fma(2.0, d.ph, k1.ph), ap1 = fma(2.0, d.p1, k1.p1), ap2 = fma(2.0, d.p2, k1.p2);
+        // stage 3
+        s1 = fma(p.h_half, d.x1, x1); s2 = fma(p.h_half, d.x2, x2);
+        sp1 = fma(p.h_half, d.p1, p1); sp2 = fma(p.h_half, d.p2, p2);
+        in = tab_fields(m, s1, s2, F);
+        if (!ev) ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
+        tab_rhs(F, sp1, sp2, E, L, d);
+        at = fma(2.0, d.t, at); a1 = fma(2.0, d.x1, a1); a2 = fma(2.0, d.x2, a2);
+        aph = fma(2.0, d.ph, aph); ap1 = fma(2.0, d.p1, ap1); ap2 = fma(2.0, d.p2, ap2);
+        // stage 4
+        s1 = fma(p.h, d.x1, x1); s2 = fma(p.h, d.x2, x2);
+        sp1 = fma(p.h, d.p1, p1); sp2 = fma(p.h, d.p2, p2);
+        in = tab_fields(m, s1, s2, F);
+        if (!ev) ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
+        tab_rhs(F, sp1, sp2, E, L, d);
+        at += d.t; a1 += d.x1; a2 += d.x2; aph += d.ph; ap1 += d.p1; ap2 += d.p2;
+        // update (Kahan, reading P1) and the end point: its fields give the next step's k1
+        double nt, n1, n2, nph, np1, np2, dt, d1, d2, dph, dp1, dp2;
+        kahan<PLAIN>(t, ct, p.h_sixth, at, nt, dt);
+        kahan<PLAIN>(x1, c1, p.h_sixth, a1, n1, d1);
+        kahan<PLAIN>(x2, c2, p.h_sixth, a2, n2, d2);
+        kahan<PLAIN>(ph, cph, p.h_sixth, aph, nph, dph);
+        kahan<PLAIN>(p1, cp1, p.h_sixth, ap1, np1, dp1);
+        kahan<PLAIN>(p2, cp2, p.h_sixth, ap2, np2, dp2);
+        in = tab_fields(m, n1, n2, F);
+        if (!ev) ev = !(n1 >= p.r_capture) ? ST_CAPTURED
+                      : (!all_finite6(nt, n1, n2, nph, np1, np2) ? ST_NUMERIC : (!in ? ST_OUTSIDE : 0));
+        tab_rhs(F, np1, np2, E, L, d);
+
+        if (active) {
+            if (ev) {
+                finish(ev);                                                      // step not taken
+            } else {
+                if (!crossed) {                                                  // B5
+                    const double half_pi = 1.5707963267948966;
+                    const double e0 = x2 - half_pi, e1 = n2 - half_pi;
+                    if (e0 * e1 < 0.0) {
+                        crossed = true;
+                        eqc = x1 + (n1 - x1) * (half_pi - x2) / (n2 - x2);
+                    }
+                }
+                t = nt; x1 = n1; x2 = n2; ph = nph; p1 = np1; p2 = np2;
+                ct = dt; c1 = d1; c2 = d2; cph = dph; cp1 = dp1; cp2 = dp2;
+                k1 = d;
+                ++steps;
+                if (x1 > p.r_escape) finish(ST_ESCAPED);                         // B3
+                else if (steps >= p.nsteps) finish(ST_MAXSTEPS);                 // B4
+            }
+        }
+    }
+}
+
+// caller's table [5][n2][n1] (field-major) -> node-major A / B
+__global__ void tab_pack_kernel(const double* __restrict__ src, long long nodes, double4* __restrict__ A, double* __restrict__ B) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nodes) return;
+    A[k] = make_double4(src[k], src[nodes + k], src[2 * nodes + k], src[3 * nodes + k]);
+    B[k] = src[4 * nodes + k];
+}
+
+}  // namespace geo

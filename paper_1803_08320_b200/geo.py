@@ -3,7 +3,7 @@
 Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
 and streams.  There is NO CPU fallback: if the library cannot be loaded, or there is no CUDA device,
 the calls raise.  Names follow the C ABI: ``geo_create``, ``geo_integrate``, ``geo_integrate_host``,
-``geo_destroy``, ``geo_horizon_radius``, ``geo_last_error``, ``geo_launch_info``, ``geo_probe_dfma``.
+``geo_create_tabulated``, ``geo_integrate_adaptive``, ``geo_destroy``, ``geo_horizon_radius``, ``geo_last_error``, ``geo_launch_info``, ``geo_probe_dfma``.
 """
 from __future__ import annotations
 
@@ -12,17 +12,17 @@ import os
 
 import numpy as np
 
-SCHWARZSCHILD, KERR = 0, 1
+SCHWARZSCHILD, KERR, TABULATED = 0, 1, 2
 TIMELIKE, NULL = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, 1, 2, 3
-ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC = 0, 1, 2, 3
+ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC, ST_OUTSIDE = 0, 1, 2, 3, 4
 FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_STAGED_SNAP, FLAG_CARTESIAN_SNAP = 1, 2, 4, 8
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI
 
 # every symbol include/geo.h declares
-SYMBOLS = ("geo_create", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_destroy",
+SYMBOLS = ("geo_create", "geo_create_tabulated", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_destroy",
            "geo_horizon_radius", "geo_last_error", "geo_launch_info", "geo_probe_dfma")
 
 
@@ -39,6 +39,11 @@ class GeoOut(C.Structure):
 class GeoAdaptive(C.Structure):
     _fields_ = [("h0", C.c_double), ("rtol", C.c_double), ("atol", C.c_double), ("h_min", C.c_double),
                 ("tau_end", C.c_double)]
+
+
+class GeoTable(C.Structure):
+    _fields_ = [("tab", C.c_void_p), ("n1", C.c_int64), ("n2", C.c_int64), ("x1_0", C.c_double), ("d1", C.c_double),
+                ("x2_0", C.c_double), ("d2", C.c_double)]
 
 
 class GeoError(RuntimeError):
@@ -60,6 +65,8 @@ def lib() -> C.CDLL:
         L = C.CDLL(LIB_PATH)
         L.geo_create.restype = C.c_int
         L.geo_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double]
+        L.geo_create_tabulated.restype = C.c_int
+        L.geo_create_tabulated.argtypes = [C.POINTER(C.c_void_p), C.POINTER(GeoTable)]
         L.geo_integrate.restype = C.c_int
         L.geo_integrate.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int64,
                                     C.POINTER(GeoStop), C.c_int64, C.POINTER(GeoOut), C.c_void_p]
@@ -90,6 +97,20 @@ def geo_create(metric: int, M: float = 1.0, a: float = 0.0) -> C.c_void_p:
     rc = lib().geo_create(C.byref(ctx), metric, M, a)
     if rc != OK:
         raise GeoError(rc, "geo_create failed (invalid metric/M/a, or no CUDA device)")
+    return ctx
+
+
+def geo_create_tabulated(tab: np.ndarray, x1_0: float, d1: float, x2_0: float, d2: float) -> C.c_void_p:
+    """Context for a tabulated 3+1 metric (include/geo.h: geo_create_tabulated).  ``tab``: host float64 [5][n2][n1] =
+    alpha, beta^phi, gamma_11, gamma_22, gamma_33 at the grid nodes; it is copied to the device."""
+    if not (isinstance(tab, np.ndarray) and tab.dtype == np.float64 and tab.ndim == 3 and tab.shape[0] == 5
+            and tab.flags.c_contiguous):
+        raise ValueError("tab must be a C-contiguous float64 numpy array of shape [5][n2][n1]")
+    ctx = C.c_void_p()
+    tb = GeoTable(tab.ctypes.data, tab.shape[2], tab.shape[1], x1_0, d1, x2_0, d2)
+    rc = lib().geo_create_tabulated(C.byref(ctx), C.byref(tb))
+    if rc != OK:
+        raise GeoError(rc, "geo_create_tabulated failed (invalid table/grid, out of memory, or no CUDA device)")
     return ctx
 
 

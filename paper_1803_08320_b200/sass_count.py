@@ -51,7 +51,7 @@ def hot_loop(ins: list) -> tuple[int, int]:
 
 def count(name_part: str = "ILb1ELi0ELb0") -> dict:
     ks = kernels()
-    name = next(k for k in ks if ("geo_rk4_kernel" in k or "geo_rk45_kernel" in k) and name_part in k)
+    name = next(k for k in ks if "_kernel" in k and name_part in k)
     ins = ks[name]
     lo, hi = hot_loop(ins)
     body = [(a, o) for a, o, _ in ins if lo <= a <= hi]

@@ -30,6 +30,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(geo.GeoStop) == 24
     assert ctypes.sizeof(geo.GeoOut) == 9 * 8
     assert geo.GeoOut.snap_mask.offset == 56 and geo.GeoOut.snap_count.offset == 64
+    assert ctypes.sizeof(geo.GeoTable) == 56 and ctypes.sizeof(geo.GeoAdaptive) == 40
 
 
 def test_sass_has_fp64_pipe_and_wide_stores():
@@ -40,6 +41,7 @@ def test_sass_has_fp64_pipe_and_wide_stores():
     assert "sm_100a" in sass
     assert sass.count("DFMA") > 500
     assert re.search(r"STG\.E(\.\w+)*\.256", sass)
+    assert re.search(r"LDG\.E(\.\w+)*\.256", sass)        # tabulated metric: one 256-bit load per stencil node
 
 
 def test_product_path_does_not_import_the_oracle():

@@ -43,11 +43,11 @@ UNIT = "geodesic-steps/s"
 # (profiles/r01_config4_v3.md: DFMA 140, DMUL 143, DADD 42, DSETP 6 for Kerr).  flop = 2*DFMA + DMUL + DADD;
 # pipe = all four.  The static SASS count of the loop (sass_count.py, an upper bound that includes the
 # rarely executed blocks inside the loop's address range) is printed beside them as a cross-check.
-FLOP_PER_STEP = {"kerr": 465.0, "schwarzschild": 397.0, "tabulated": 2400.0}
-PIPE_INSTR_PER_STEP = {"kerr": 331.0, "schwarzschild": 273.0, "tabulated": 1400.0}
+FLOP_PER_STEP = {"kerr": 465.0, "schwarzschild": 397.0, "tabulated": 2218.0}
+PIPE_INSTR_PER_STEP = {"kerr": 331.0, "schwarzschild": 273.0, "tabulated": 1300.0}
 OTHER_INSTR_PER_STEP = {"kerr": 103.0}     # non-FP64 instructions per step, same ncu capture
 FLOP_COUNT_SOURCE = {"kerr": "ncu dynamic count (profiles/r01_config4_v3.md)", "schwarzschild": "static SASS count",
-                     "tabulated": "static SASS count of the geo_tab_rk4_kernel loop"}
+                     "tabulated": "ncu dynamic thread-level count (profiles/r01_tab4.md): 918 DFMA + 323 DMUL + 58 DADD per step"}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
 # adaptive RK5(4) kernel, per step ATTEMPT of one Kerr geodesic, executed (ncu, thread level)
 ADAPTIVE_FLOP_PER_ATTEMPT, ADAPTIVE_PIPE_PER_ATTEMPT = 1211.0, 785.0
@@ -228,7 +228,7 @@ def flop_counts(metric: str) -> tuple[float, float, str, dict | None]:
     try:
         from paper_1803_08320_b200 import sass_count
         c = sass_count.count({"kerr": "rk4_kernelILb1ELi0ELb0", "schwarzschild": "rk4_kernelILb0ELi0ELb0",
-                              "tabulated": "geo_tab_rk4_kernelILb0E"}[metric])
+                              "tabulated": "geo_tab_rk4_kernelILb0ELb1E"}[metric])
         static = {"flop": c["flop"], "fp64_pipe": c["fp64_pipe"]}
     except Exception:
         pass
@@ -243,7 +243,7 @@ def main() -> None:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "config3a", "tab4", "snapbench", "paper_t3", "paper_t4"])
     ap.add_argument("--n", type=int, default=None, help="override particle count / image size (development)")
-    ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping, 4 = shared-memory-staged snapshots)")
+    ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping, 4 = shared-memory-staged snapshots, 16 = tabulated metric: gather instead of the stencil cache)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

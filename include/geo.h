@@ -42,6 +42,8 @@ enum {
     GEO_FLAG_CARTESIAN_SNAP = 8, /* snapshot components 1..3 hold (x, y, z) of eq.(7) PAPER.md:88-93 instead
                                   of (r, theta, phi): with snap_mask = 0x0F a record is (t, x, y, z), the paper's
                                   output format -- tau is implicit, slot j <-> tau = j*snapshot_every*h */
+    GEO_FLAG_TAB_GATHER = 16,  /* tabulated metrics: gather the 4 x 4 stencil through L1/L2 on every evaluation instead
+                                  of keeping the current cell's stencil in shared memory (for comparison)  */
     GEO_FLAG_STAGED_SNAP = 4   /* snapshot records staged in shared memory and flushed by the warp with
                                   coalesced stores; default: each lane stores its record straight from
                                   registers with 256-bit stores (measured faster, profiles/)          */
@@ -128,7 +130,7 @@ int geo_integrate_adaptive(geo_ctx *ctx, const double *state_in, int64_t n, cons
  * A ctx created here is used with geo_integrate / geo_integrate_host: state_in = (x^1, x^2, phi, p_1, p_2, p_phi),
  * r_capture / r_escape refer to x^1, the equatorial event to x^2 = pi/2; an evaluation point (y0, a stage point, the
  * end point of a step) outside the domain ends the particle with GEO_ST_OUTSIDE, that step is not taken (per
- * evaluation point the capture test comes first).  snapshot_every must be 0; flags: GEO_FLAG_PLAIN_UPDATE only;
+ * evaluation point the capture test comes first).  snapshot_every must be 0; flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER;
  * geo_integrate_adaptive returns GEO_EINVAL; geo_horizon_radius returns NaN.
  * Errors: GEO_EINVAL (NULL, n1 or n2 < 4, d1 or d2 <= 0, non-finite grid), GEO_ENOMEM, GEO_ECUDA. */
 typedef struct geo_table {

@@ -77,10 +77,10 @@ int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t 
     if (!std::isfinite(h) || h == 0.0) return fail(ctx, GEO_EINVAL, "h must be finite and non-zero");
     if (stop->kind != GEO_TIMELIKE && stop->kind != GEO_NULL) return fail(ctx, GEO_EINVAL, "stop.kind must be GEO_TIMELIKE or GEO_NULL");
     if (std::isnan(stop->r_capture) || std::isnan(stop->r_escape)) return fail(ctx, GEO_EINVAL, "stop radii must not be NaN");
-    if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_STAGED_SNAP | GEO_FLAG_CARTESIAN_SNAP)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
+    if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_STAGED_SNAP | GEO_FLAG_CARTESIAN_SNAP | GEO_FLAG_TAB_GATHER)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
     if (ctx->metric == GEO_TABULATED) {
         if (snapshot_every > 0) return fail(ctx, GEO_EINVAL, "tabulated metrics: snapshots are not supported");
-        if (stop->flags & ~GEO_FLAG_PLAIN_UPDATE) return fail(ctx, GEO_EINVAL, "tabulated metrics: only GEO_FLAG_PLAIN_UPDATE is supported");
+        if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_TAB_GATHER)) return fail(ctx, GEO_EINVAL, "tabulated metrics: only GEO_FLAG_PLAIN_UPDATE and GEO_FLAG_TAB_GATHER are supported");
     }
     if (n == 0) return GEO_OK;
     if (!state_in || !out->final_state || !out->status || !out->steps_done) return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
@@ -135,13 +135,18 @@ int plan_launch(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, 
 
 typedef void (*tab_kernel_fn)(const TabParams);
 tab_kernel_fn pick_tab_kernel(int32_t flags) {
-    return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tab_kernel_fn)geo_tab_rk4_kernel<true> : (tab_kernel_fn)geo_tab_rk4_kernel<false>;
+    if (flags & GEO_FLAG_TAB_GATHER)
+        return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tab_kernel_fn)geo_tab_rk4_kernel<true, false> : (tab_kernel_fn)geo_tab_rk4_kernel<false, false>;
+    return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tab_kernel_fn)geo_tab_rk4_kernel<true, true> : (tab_kernel_fn)geo_tab_rk4_kernel<false, true>;
 }
+size_t tab_smem(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? 0 : (size_t)kStencil * kBlock * sizeof(double); }
 
 int plan_tab(geo_ctx* ctx, int64_t n, int32_t flags, int* grid, int* per_sm_out, int* regs) {
     tab_kernel_fn fn = pick_tab_kernel(flags);
     int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, 0);
+    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_smem(flags));
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncSetAttribute(smem)");
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, tab_smem(flags));
     if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(tab)");
     if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
     cudaFuncAttributes fa;
@@ -179,7 +184,7 @@ int launch_tab(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t ns
     p.m = ctx->tm;
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
-    pick_tab_kernel(stop->flags)<<<grid, kBlock, 0, stream>>>(p);
+    pick_tab_kernel(stop->flags)<<<grid, kBlock, tab_smem(stop->flags), stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
     return GEO_OK;

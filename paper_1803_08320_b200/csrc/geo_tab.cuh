@@ -132,6 +132,63 @@ __device__ __forceinline__ bool tab_fields(const TabMetric& m, double x1, double
     return in1 & in2;
 }
 
+// ---- per-lane stencil cache in shared memory ---------------------------------------------------------------
+// A particle stays in one grid cell for many evaluations (a step moves it by h |dx/dtau| << d), so the 4 x 4 x 5
+// stencil of its current cell is kept in shared memory: column-major [80][kBlock] doubles per CTA (lane l owns
+// column l: its 64-bit accesses are conflict-free, 2 wavefronts per warp instruction) and refilled from the
+// table only when the cell index changes.  Element (b, a, f) of the stencil sits at row (b*4 + a)*5 + f.
+constexpr int kStencil = 80;
+
+__device__ __noinline__ void tab_refill(const TabMetric& m, int i, int j, double* col) {
+    const long long base = (long long)(j - 1) * m.n1 + (i - 1);
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        const double4* ra = m.A + base + (long long)b * m.n1;
+        const double* rb = m.B + base + (long long)b * m.n1;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            const double4 v = ldg256(ra + a);
+            const double w = __ldg(rb + a);
+            double* q = col + (b * 4 + a) * 5 * kBlock;
+            q[0] = v.x; q[kBlock] = v.y; q[2 * kBlock] = v.z; q[3 * kBlock] = v.w; q[4 * kBlock] = w;
+        }
+    }
+}
+
+__device__ __forceinline__ bool tab_fields_cached(const TabMetric& m, double x1, double x2, TabFields& F, int& ci, int& cj,
+                                                  double* col) {
+    int i, j;
+    double s1, s2;
+    const bool in1 = tab_cell(x1, m.x1_0, m.d1, m.inv_d1, m.n1, i, s1);
+    const bool in2 = tab_cell(x2, m.x2_0, m.d2, m.inv_d2, m.n2, j, s2);
+    if (i != ci || j != cj) {
+        tab_refill(m, i, j, col);
+        ci = i;
+        cj = j;
+    }
+    double w1[4], dw1[4], w2[4], dw2[4];
+    keys_weights(s1, m.inv_d1, w1, dw1);
+    keys_weights(s2, m.inv_d2, w2, dw2);
+    double v[5] = {0, 0, 0, 0, 0}, g1[5] = {0, 0, 0, 0, 0}, g2[5] = {0, 0, 0, 0, 0};
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        const double* q = col + b * 20 * kBlock;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const double c0 = q[k * kBlock], c1 = q[(5 + k) * kBlock], c2 = q[(10 + k) * kBlock], c3 = q[(15 + k) * kBlock];
+            const double rv = fma(w1[3], c3, fma(w1[2], c2, fma(w1[1], c1, w1[0] * c0)));
+            const double rd = fma(dw1[3], c3, fma(dw1[2], c2, fma(dw1[1], c1, dw1[0] * c0)));
+            v[k] = fma(w2[b], rv, v[k]);
+            g1[k] = fma(w2[b], rd, g1[k]);
+            g2[k] = fma(dw2[b], rv, g2[k]);
+        }
+    }
+    F.al = v[0]; F.be = v[1]; F.g11 = v[2]; F.g22 = v[3]; F.g33 = v[4];
+    F.al1 = g1[0]; F.be1 = g1[1]; F.g111 = g1[2]; F.g221 = g1[3]; F.g331 = g1[4];
+    F.al2 = g2[0]; F.be2 = g2[1]; F.g112 = g2[2]; F.g222 = g2[3]; F.g332 = g2[4];
+    return in1 & in2;
+}
+
 struct TabDeriv {
     double t, x1, x2, ph, p1, p2;
 };
@@ -155,10 +212,19 @@ __device__ __noinline__ bool tab_fields_cold(const TabMetric& m, double x1, doub
     return tab_fields(m, x1, x2, F);
 }
 
-template <bool PLAIN>
-__global__ void __launch_bounds__(kBlock, 3) geo_tab_rk4_kernel(const __grid_constant__ TabParams p) {
+// CACHE: stencil cache in shared memory (kStencil * kBlock doubles = 80 KB per CTA, 2 CTAs/SM);
+// !CACHE: every evaluation gathers its stencil through L1/L2 (GEO_FLAG_TAB_GATHER, for comparison).
+template <bool PLAIN, bool CACHE>
+__global__ void __launch_bounds__(kBlock, CACHE ? 2 : 3) geo_tab_rk4_kernel(const __grid_constant__ TabParams p) {
+    extern __shared__ __align__(16) double stencil_smem[];
+    double* const col = stencil_smem + threadIdx.x;
+    int ci = -1, cj = -1;                                          // cell whose stencil the column holds
     const unsigned lane = threadIdx.x & 31u;
     const TabMetric& m = p.m;
+    auto fields = [&](double a, double b, TabFields& F) -> bool {
+        if (CACHE) return tab_fields_cached(m, a, b, F, ci, cj, col);
+        return tab_fields(m, a, b, F);
+    };
     long long idx = -1;
     bool active = false, exhausted = false;
     double t = 0, x1 = 0, x2 = 0, ph = 0, p1 = 0, p2 = 0, E = 0, L = 0;
@@ -252,7 +318,7 @@ __global__ void __launch_bounds__(kBlock, 3) geo_tab_rk4_kernel(const __grid_con
         // stage 2
         s1 = fma(p.h_half, k1.x1, x1); s2 = fma(p.h_half, k1.x2, x2);
         sp1 = fma(p.h_half, k1.p1, p1); sp2 = fma(p.h_half, k1.p2, p2);
-        bool in = tab_fields(m, s1, s2, F);
+        bool in = fields(s1, s2, F);
         ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
         tab_rhs(F, sp1, sp2, E, L, d);
         double at = fma(2.0, d.t, k1.t), a1 = fma(2.0, d.x1, k1.x1), a2 = fma(2.0, d.x2, k1.x2),
@@ -260,7 +326,7 @@ __global__ void __launch_bounds__(kBlock, 3) geo_tab_rk4_kernel(const __grid_con
         // stage 3
         s1 = fma(p.h_half, d.x1, x1); s2 = fma(p.h_half, d.x2, x2);
         sp1 = fma(p.h_half, d.p1, p1); sp2 = fma(p.h_half, d.p2, p2);
-        in = tab_fields(m, s1, s2, F);
+        in = fields(s1, s2, F);
         if (!ev) ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
         tab_rhs(F, sp1, sp2, E, L, d);
         at = fma(2.0, d.t, at); a1 = fma(2.0, d.x1, a1); a2 = fma(2.0, d.x2, a2);
@@ -268,7 +334,7 @@ __global__ void __launch_bounds__(kBlock, 3) geo_tab_rk4_kernel(const __grid_con
         // stage 4
         s1 = fma(p.h, d.x1, x1); s2 = fma(p.h, d.x2, x2);
         sp1 = fma(p.h, d.p1, p1); sp2 = fma(p.h, d.p2, p2);
-        in = tab_fields(m, s1, s2, F);
+        in = fields(s1, s2, F);
         if (!ev) ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
         tab_rhs(F, sp1, sp2, E, L, d);
         at += d.t; a1 += d.x1; a2 += d.x2; aph += d.ph; ap1 += d.p1; ap2 += d.p2;
@@ -280,7 +346,7 @@ __global__ void __launch_bounds__(kBlock, 3) geo_tab_rk4_kernel(const __grid_con
         kahan<PLAIN>(ph, cph, p.h_sixth, aph, nph, dph);
         kahan<PLAIN>(p1, cp1, p.h_sixth, ap1, np1, dp1);
         kahan<PLAIN>(p2, cp2, p.h_sixth, ap2, np2, dp2);
-        in = tab_fields(m, n1, n2, F);
+        in = fields(n1, n2, F);
         if (!ev) ev = !(n1 >= p.r_capture) ? ST_CAPTURED
                       : (!all_finite6(nt, n1, n2, nph, np1, np2) ? ST_NUMERIC : (!in ? ST_OUTSIDE : 0));
         tab_rhs(F, np1, np2, E, L, d);

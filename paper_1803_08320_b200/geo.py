@@ -16,7 +16,7 @@ SCHWARZSCHILD, KERR, TABULATED = 0, 1, 2
 TIMELIKE, NULL = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, 1, 2, 3
 ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC, ST_OUTSIDE = 0, 1, 2, 3, 4
-FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_STAGED_SNAP, FLAG_CARTESIAN_SNAP = 1, 2, 4, 8
+FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_STAGED_SNAP, FLAG_CARTESIAN_SNAP, FLAG_TAB_GATHER = 1, 2, 4, 8, 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI

@@ -45,13 +45,13 @@ def assert_parity(g, o, tol):
     assert (parity.rel_err(g["health"], o["health"]) <= 1e-6).all() or np.nanmax(np.abs(g["health"] - o["health"])) < 1e-9
 
 
-@pytest.mark.parametrize("host,flags", [(False, 0), (True, 0), (False, 1)])
+@pytest.mark.parametrize("host,flags", [(False, 0), (True, 0), (False, 1), (False, 16), (False, 17)])   # 1 = plain update, 16 = GEO_FLAG_TAB_GATHER
 def test_tabulated_kerr_bound_orbits(G, tab_oracle, host, flags):
     """Config-2-like batch (Kerr a = 0.9 bound orbits, ragged count) on a 1025 x 257 Boyer-Lindquist table."""
     a = 0.9
     tb = W.kerr_metric_table(1.0, a, 1025, 257, 1.8, 40.0, 0.2, math.pi - 0.2)
     st = W.kerr_bound(3001, a, W.SEED_BASE + 2)
-    o = tab_oracle.integrate(tb, st, 0.01, 3000, flags=flags, nthreads=NCPU)
+    o = tab_oracle.integrate(tb, st, 0.01, 3000, flags=flags & 1, nthreads=NCPU)
     g = run_gpu_tab(G, tb, st, 0.01, 3000, host=host, flags=flags)
     assert_parity(g, o, 1e-9)
     # orbits whose polar motion leaves the table's theta range end with OUTSIDE (on both sides, same step)
@@ -83,6 +83,9 @@ def test_tabulated_camera_rays_log_radial(G, tab_oracle):
     o = tab_oracle.integrate(tb, s, 0.02, 20000, kind=tab_oracle.NULL, nthreads=NCPU, **kw)
     o_ld = tab_oracle.integrate(tb, s, 0.02, 20000, kind=tab_oracle.NULL, nthreads=NCPU, long_double=True, **kw)
     g = run_gpu_tab(G, tb, s, 0.02, 20000, kind=G.NULL, **kw)
+    g2 = run_gpu_tab(G, tb, s, 0.02, 20000, kind=G.NULL, flags=G.FLAG_TAB_GATHER, **kw)
+    for k in ("final_state", "status", "steps_done", "eq_cross_r"):      # the stencil cache changes where the nodes are
+        assert np.array_equal(g[k], g2[k], equal_nan=True), k             # read from, not one bit of the result
     cert = parity.certified(o, o_ld, 1e-8)
     c = parity.compare(g, o)
     n = s.shape[1]

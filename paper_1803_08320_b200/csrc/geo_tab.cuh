@@ -311,45 +311,42 @@ __global__ void __launch_bounds__(kBlock, CACHE ? 2 : 3) geo_tab_rk4_kernel(cons
 
         // --- one RK4 step (every lane; idle lanes compute on stale state, loads are clamped in bounds) ----
         // ev: first event in the oracle's order -- per evaluation point capture (B2) before domain exit (T4)
+        // The four evaluations (stage points 2-4, end point) run through ONE copy of the evaluator (loop not
+        // unrolled): unrolled, the step is ~9000 instructions and the warps stall on instruction fetch
+        // (ncu: stall_no_instruction 1.8 per issue).
         int ev = 0;
-        TabFields F;
-        TabDeriv d;
-        double s1, s2, sp1, sp2;
-        // stage 2
-        s1 = fma(p.h_half, k1.x1, x1); s2 = fma(p.h_half, k1.x2, x2);
-        sp1 = fma(p.h_half, k1.p1, p1); sp2 = fma(p.h_half, k1.p2, p2);
-        bool in = fields(s1, s2, F);
-        ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
-        tab_rhs(F, sp1, sp2, E, L, d);
-        double at = fma(2.0, d.t, k1.t), a1 = fma(2.0, d.x1, k1.x1), a2 = fma(2.0, d.x2, k1.x2),
-               aph = fma(2.0, d.ph, k1.ph), ap1 = fma(2.0, d.p1, k1.p1), ap2 = fma(2.0, d.p2, k1.p2);
-        // stage 3
-        s1 = fma(p.h_half, d.x1, x1); s2 = fma(p.h_half, d.x2, x2);
-        sp1 = fma(p.h_half, d.p1, p1); sp2 = fma(p.h_half, d.p2, p2);
-        in = fields(s1, s2, F);
-        if (!ev) ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
-        tab_rhs(F, sp1, sp2, E, L, d);
-        at = fma(2.0, d.t, at); a1 = fma(2.0, d.x1, a1); a2 = fma(2.0, d.x2, a2);
-        aph = fma(2.0, d.ph, aph); ap1 = fma(2.0, d.p1, ap1); ap2 = fma(2.0, d.p2, ap2);
-        // stage 4
-        s1 = fma(p.h, d.x1, x1); s2 = fma(p.h, d.x2, x2);
-        sp1 = fma(p.h, d.p1, p1); sp2 = fma(p.h, d.p2, p2);
-        in = fields(s1, s2, F);
-        if (!ev) ev = !(s1 >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
-        tab_rhs(F, sp1, sp2, E, L, d);
-        at += d.t; a1 += d.x1; a2 += d.x2; aph += d.ph; ap1 += d.p1; ap2 += d.p2;
-        // update (Kahan, reading P1) and the end point: its fields give the next step's k1
-        double nt, n1, n2, nph, np1, np2, dt, d1, d2, dph, dp1, dp2;
-        kahan<PLAIN>(t, ct, p.h_sixth, at, nt, dt);
-        kahan<PLAIN>(x1, c1, p.h_sixth, a1, n1, d1);
-        kahan<PLAIN>(x2, c2, p.h_sixth, a2, n2, d2);
-        kahan<PLAIN>(ph, cph, p.h_sixth, aph, nph, dph);
-        kahan<PLAIN>(p1, cp1, p.h_sixth, ap1, np1, dp1);
-        kahan<PLAIN>(p2, cp2, p.h_sixth, ap2, np2, dp2);
-        in = fields(n1, n2, F);
-        if (!ev) ev = !(n1 >= p.r_capture) ? ST_CAPTURED
-                      : (!all_finite6(nt, n1, n2, nph, np1, np2) ? ST_NUMERIC : (!in ? ST_OUTSIDE : 0));
-        tab_rhs(F, np1, np2, E, L, d);
+        TabDeriv d = k1;
+        double at = k1.t, a1 = k1.x1, a2 = k1.x2, aph = k1.ph, ap1 = k1.p1, ap2 = k1.p2;
+        double nt = t, n1 = x1, n2 = x2, nph = ph, np1 = p1, np2 = p2, dt = ct, d1 = c1, d2 = c2, dph = cph, dp1 = cp1, dp2 = cp2;
+#pragma unroll 1
+        for (int s = 0; s < 4; ++s) {
+            double e1, e2, ep1, ep2;                                   // evaluation point
+            bool fin6 = true;
+            if (s < 3) {
+                const double c = s == 2 ? p.h : p.h_half;
+                e1 = fma(c, d.x1, x1); e2 = fma(c, d.x2, x2);
+                ep1 = fma(c, d.p1, p1); ep2 = fma(c, d.p2, p2);
+            } else {
+                // update (Kahan, reading P1); the end point's derivative is the next step's k1
+                kahan<PLAIN>(t, ct, p.h_sixth, at, nt, dt);
+                kahan<PLAIN>(x1, c1, p.h_sixth, a1, n1, d1);
+                kahan<PLAIN>(x2, c2, p.h_sixth, a2, n2, d2);
+                kahan<PLAIN>(ph, cph, p.h_sixth, aph, nph, dph);
+                kahan<PLAIN>(p1, cp1, p.h_sixth, ap1, np1, dp1);
+                kahan<PLAIN>(p2, cp2, p.h_sixth, ap2, np2, dp2);
+                e1 = n1; e2 = n2; ep1 = np1; ep2 = np2;
+                fin6 = all_finite6(nt, n1, n2, nph, np1, np2);
+            }
+            TabFields F;
+            const bool in = fields(e1, e2, F);
+            if (!ev) ev = !(e1 >= p.r_capture) ? ST_CAPTURED : (!fin6 ? ST_NUMERIC : (!in ? ST_OUTSIDE : 0));
+            tab_rhs(F, ep1, ep2, E, L, d);
+            if (s < 3) {
+                const double w = s == 2 ? 1.0 : 2.0;                   // k1 + 2 k2 + 2 k3 + k4
+                at = fma(w, d.t, at); a1 = fma(w, d.x1, a1); a2 = fma(w, d.x2, a2);
+                aph = fma(w, d.ph, aph); ap1 = fma(w, d.p1, ap1); ap2 = fma(w, d.p2, ap2);
+            }
+        }
 
         if (active) {
             if (ev) {

@@ -139,20 +139,20 @@ tab_kernel_fn pick_tab_kernel(int32_t flags) {
         return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tab_kernel_fn)geo_tab_rk4_kernel<true, false> : (tab_kernel_fn)geo_tab_rk4_kernel<false, false>;
     return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tab_kernel_fn)geo_tab_rk4_kernel<true, true> : (tab_kernel_fn)geo_tab_rk4_kernel<false, true>;
 }
-size_t tab_smem(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? 0 : (size_t)kStencil * kBlock * sizeof(double); }
+size_t tab_smem(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? 0 : (size_t)kStencil * kTabBlock * sizeof(double); }
 
 int plan_tab(geo_ctx* ctx, int64_t n, int32_t flags, int* grid, int* per_sm_out, int* regs) {
     tab_kernel_fn fn = pick_tab_kernel(flags);
     int per_sm = 0;
     cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_smem(flags));
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncSetAttribute(smem)");
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, tab_smem(flags));
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kTabBlock, tab_smem(flags));
     if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(tab)");
     if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
     cudaFuncAttributes fa;
     e = cudaFuncGetAttributes(&fa, (const void*)fn);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncGetAttributes");
-    const int64_t need = (n + kBlock - 1) / kBlock, resident = (int64_t)ctx->sm_count * per_sm;
+    const int64_t need = (n + kTabBlock - 1) / kTabBlock, resident = (int64_t)ctx->sm_count * per_sm;
     *grid = (int)(need < resident ? need : resident);
     *per_sm_out = per_sm;
     *regs = fa.numRegs;
@@ -184,7 +184,7 @@ int launch_tab(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t ns
     p.m = ctx->tm;
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
-    pick_tab_kernel(stop->flags)<<<grid, kBlock, tab_smem(stop->flags), stream>>>(p);
+    pick_tab_kernel(stop->flags)<<<grid, kTabBlock, tab_smem(stop->flags), stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
     return GEO_OK;
@@ -494,7 +494,7 @@ int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
 int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, int32_t info[4]) {
     if (!ctx || !info || n < 0) return GEO_EINVAL;
     if (ctx->metric == GEO_TABULATED) {
-        info[1] = kBlock;
+        info[1] = kTabBlock;
         return plan_tab(ctx, n, flags, &info[0], &info[3], &info[2]);
     }
     LaunchPlan lp;

@@ -134,10 +134,17 @@ __device__ __forceinline__ bool tab_fields(const TabMetric& m, double x1, double
 
 // ---- per-lane stencil cache in shared memory ---------------------------------------------------------------
 // A particle stays in one grid cell for many evaluations (a step moves it by h |dx/dtau| << d), so the 4 x 4 x 5
-// stencil of its current cell is kept in shared memory: column-major [80][kBlock] doubles per CTA (lane l owns
+// stencil of its current cell is kept in shared memory: column-major [80][kTabBlock] doubles per CTA (lane l owns
 // column l: its 64-bit accesses are conflict-free, 2 wavefronts per warp instruction) and refilled from the
 // table only when the cell index changes.  Element (b, a, f) of the stencil sits at row (b*4 + a)*5 + f.
 constexpr int kStencil = 80;
+#ifndef GEO_TAB_BLOCK
+#define GEO_TAB_BLOCK 128
+#endif
+#ifndef GEO_TAB_CTAS
+#define GEO_TAB_CTAS 2
+#endif
+constexpr int kTabBlock = GEO_TAB_BLOCK;      // threads per CTA of the tabulated-metric kernels
 
 __device__ __noinline__ void tab_refill(const TabMetric& m, int i, int j, double* col) {
     const long long base = (long long)(j - 1) * m.n1 + (i - 1);
@@ -149,8 +156,8 @@ __device__ __noinline__ void tab_refill(const TabMetric& m, int i, int j, double
         for (int a = 0; a < 4; ++a) {
             const double4 v = ldg256(ra + a);
             const double w = __ldg(rb + a);
-            double* q = col + (b * 4 + a) * 5 * kBlock;
-            q[0] = v.x; q[kBlock] = v.y; q[2 * kBlock] = v.z; q[3 * kBlock] = v.w; q[4 * kBlock] = w;
+            double* q = col + (b * 4 + a) * 5 * kTabBlock;
+            q[0] = v.x; q[kTabBlock] = v.y; q[2 * kTabBlock] = v.z; q[3 * kTabBlock] = v.w; q[4 * kTabBlock] = w;
         }
     }
 }
@@ -172,10 +179,10 @@ __device__ __forceinline__ bool tab_fields_cached(const TabMetric& m, double x1,
     double v[5] = {0, 0, 0, 0, 0}, g1[5] = {0, 0, 0, 0, 0}, g2[5] = {0, 0, 0, 0, 0};
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
-        const double* q = col + b * 20 * kBlock;
+        const double* q = col + b * 20 * kTabBlock;
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
-            const double c0 = q[k * kBlock], c1 = q[(5 + k) * kBlock], c2 = q[(10 + k) * kBlock], c3 = q[(15 + k) * kBlock];
+            const double c0 = q[k * kTabBlock], c1 = q[(5 + k) * kTabBlock], c2 = q[(10 + k) * kTabBlock], c3 = q[(15 + k) * kTabBlock];
             const double rv = fma(w1[3], c3, fma(w1[2], c2, fma(w1[1], c1, w1[0] * c0)));
             const double rd = fma(dw1[3], c3, fma(dw1[2], c2, fma(dw1[1], c1, dw1[0] * c0)));
             v[k] = fma(w2[b], rv, v[k]);
@@ -212,10 +219,10 @@ __device__ __noinline__ bool tab_fields_cold(const TabMetric& m, double x1, doub
     return tab_fields(m, x1, x2, F);
 }
 
-// CACHE: stencil cache in shared memory (kStencil * kBlock doubles = 80 KB per CTA, 2 CTAs/SM);
+// CACHE: stencil cache in shared memory (kStencil * kTabBlock doubles = 80 KB per CTA, 2 CTAs/SM);
 // !CACHE: every evaluation gathers its stencil through L1/L2 (GEO_FLAG_TAB_GATHER, for comparison).
 template <bool PLAIN, bool CACHE>
-__global__ void __launch_bounds__(kBlock, CACHE ? 2 : 3) geo_tab_rk4_kernel(const __grid_constant__ TabParams p) {
+__global__ void __launch_bounds__(kTabBlock, CACHE ? GEO_TAB_CTAS : 3) geo_tab_rk4_kernel(const __grid_constant__ TabParams p) {
     extern __shared__ __align__(16) double stencil_smem[];
     double* const col = stencil_smem + threadIdx.x;
     int ci = -1, cj = -1;                                          // cell whose stencil the column holds

@@ -56,7 +56,7 @@ ADAPTIVE_SOURCE = "ncu dynamic thread-level count (profiles/r01_config3a_rk45.md
 F_ALG_SURVEY = {"kerr": 800.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one geo_rk4_kernel launch from the committed
 # `ncu --set full` capture of that workload (profiles/), bytes; None where no capture exists.
-TRAFFIC_NCU_BYTES = {"config3a": 99_734_272, "config4": 580_706_816, "snapbench": 69_562_443_296}      # profiles/r01_config4_v3.md, r01_snapbench_v3.md
+TRAFFIC_NCU_BYTES = {"config3a": 99_734_272, "tab4": 657_377_536, "config4": 580_706_816, "snapbench": 69_562_443_296}      # profiles/r01_config4_v3.md, r01_snapbench_v3.md, r01_config3a_rk45.md, r01_tab4.md (full-size capture of v2: particle I/O only)
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:
@@ -333,27 +333,25 @@ def main() -> None:
     e2e = None
     snap_bytes = out["snapshots"].numel() * 8 if out["snapshots"] is not None else 0
     if ad and not args.no_e2e:
-        # no host entry point for the adaptive stepper: pinned H2D, geo_integrate_adaptive, D2H of every output
         h_in = torch.from_numpy(st).pin_memory()
-        keys = ("final_state", "status", "steps_done", "eq_cross_r", "health")
-        h_o = {k: torch.empty_like(out[k], device="cpu").pin_memory() for k in keys}
+        h_out = geo.alloc_outputs_host(n, pinned=True)
+        h_rej = torch.zeros(n, dtype=torch.int32).pin_memory()
+        akw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], rejected=h_rej)
+        geo.geo_integrate_adaptive_host(ctx, h_in, ad["h0"], ad["rtol"], ad["atol"], ad["max_attempts"], h_out, **akw)   # warm-up
         ke = max(1, min(args.steps, 2))
         barrier()
         te0 = time.perf_counter()
         for _ in range(ke):
-            d_in.copy_(h_in, non_blocking=True)
-            one_pass()
-            for k in keys:
-                h_o[k].copy_(out[k], non_blocking=True)
-            torch.cuda.synchronize(dev)
+            geo.geo_integrate_adaptive_host(ctx, h_in, ad["h0"], ad["rtol"], ad["atol"], ad["max_attempts"], h_out, **akw)
+        torch.cuda.synchronize(dev)
         te = torch.tensor([time.perf_counter() - te0], dtype=torch.float64, device=dev)
-        es = torch.tensor([float(steps_per_pass) * ke], dtype=torch.float64, device=dev)
+        es = torch.tensor([float(h_out["steps_done"].sum().item() + h_rej.sum().item()) * ke], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
             dist.all_reduce(es, op=dist.ReduceOp.SUM)
+        bo = sum(v.numel() * v.element_size() for k, v in h_out.items() if hasattr(v, "numel")) + h_rej.numel() * 4
         e2e = {"value": es.item() / te.item(), "unit": UNIT, "h2d_bytes_per_step": int(h_in.numel() * 8),
-               "d2h_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h_o.values())), "passes": ke,
-               "api": "pinned H2D + geo_integrate_adaptive + D2H of all outputs"}
+               "d2h_bytes_per_step": int(bo), "passes": ke, "api": "geo_integrate_adaptive_host (pinned host buffers)"}
     elif not args.no_e2e and snap_bytes <= (16 << 30):      # larger trajectory buffers stay device-resident
         h_in = torch.from_numpy(st).pin_memory()
         h_out = geo.alloc_outputs_host(n, wl["nsteps"], wl["snapshot_every"], None, wl["snap_mask"], pinned=True)

@@ -115,6 +115,11 @@ int geo_integrate_adaptive(geo_ctx *ctx, const double *state_in, int64_t n, cons
                            int64_t max_attempts, const geo_stop *stop, const geo_out *out, int32_t *rejected,
                            void *cuda_stream);
 
+/* Same operation with HOST buffers (state_in, every non-NULL output and `rejected` are host pointers; pinned lets the
+ * copies run at full speed): H2D, launch, D2H, synchronise.  Device scratch is owned by the ctx. */
+int geo_integrate_adaptive_host(geo_ctx *ctx, const double *state_in, int64_t n, const geo_adaptive *ctl,
+                                int64_t max_attempts, const geo_stop *stop, const geo_out *out, int32_t *rejected);
+
 /* a NUMERICALLY GIVEN metric ("the 3+1 formulation is important in order to bring future support
  * to numerical metrics"; "a new algorithm to handle numerically computed metrics").
  * Line element (1) with the structure of eq.(8): stationary, axisymmetric,

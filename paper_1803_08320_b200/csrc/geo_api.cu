@@ -491,6 +491,64 @@ int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     return GEO_OK;
 }
 
+// Host-buffer entry point of the adaptive path: one H2D, one launch, one D2H per output, on the ctx's own stream.
+int geo_integrate_adaptive_host(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl,
+                                int64_t max_attempts, const geo_stop* stop, const geo_out* out, int32_t* rejected) {
+    if (!ctx) return GEO_EINVAL;
+    ctx->err[0] = 0;
+    if (!stop || !out) return fail(ctx, GEO_EINVAL, "stop and out must not be NULL");
+    if (n < 0) return fail(ctx, GEO_EINVAL, "n must be >= 0");
+    if (n > 0 && (!state_in || !out->final_state || !out->status || !out->steps_done))
+        return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
+    const size_t N = (size_t)n;
+    const size_t b_in = align256(6 * N * 8), b_fin = align256(8 * N * 8), b_st = align256(N * 4), b_steps = align256(N * 8),
+                 b_eq = out->eq_cross_r ? align256(N * 8) : 0, b_he = out->health ? align256(N * 8) : 0,
+                 b_rej = rejected ? align256(N * 4) : 0;
+    const size_t total = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_rej + 256;
+    cudaError_t e;
+    if (!ctx->host_stream[0]) {
+        e = cudaStreamCreateWithFlags(&ctx->host_stream[0], cudaStreamNonBlocking);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamCreate");
+    }
+    if (total > ctx->scratch_bytes) {
+        if (ctx->scratch) cudaFree(ctx->scratch);
+        ctx->scratch = nullptr;
+        ctx->scratch_bytes = 0;
+        e = cudaMalloc(&ctx->scratch, total);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMalloc(scratch)");
+        ctx->scratch_bytes = total;
+    }
+    cudaStream_t s = ctx->host_stream[0];
+    char* base = static_cast<char*>(ctx->scratch);
+    size_t off = 0;
+    auto take = [&](size_t b) { char* q = b ? base + off : nullptr; off += b; return q; };
+    double* d_in = (double*)take(b_in);
+    geo_out d = *out;
+    d.final_state = (double*)take(b_fin);
+    d.status = (int32_t*)take(b_st);
+    d.steps_done = (int64_t*)take(b_steps);
+    d.eq_cross_r = (double*)take(b_eq);
+    d.health = (double*)take(b_he);
+    d.snapshots = nullptr;
+    d.snap_count = nullptr;
+    int32_t* d_rej = (int32_t*)take(b_rej);
+    if (n > 0) {
+        e = cudaMemcpyAsync(d_in, state_in, 6 * N * 8, cudaMemcpyHostToDevice, s);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "H2D state_in");
+    }
+    int rc = geo_integrate_adaptive(ctx, n > 0 ? d_in : state_in, n, ctl, max_attempts, stop, n > 0 ? &d : out, d_rej, s);
+    if (rc != GEO_OK || n == 0) return rc;
+    e = cudaMemcpyAsync(out->final_state, d.final_state, 8 * N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out->status, d.status, N * 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out->steps_done, d.steps_done, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.eq_cross_r) e = cudaMemcpyAsync(out->eq_cross_r, d.eq_cross_r, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.health) e = cudaMemcpyAsync(out->health, d.health, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d_rej) e = cudaMemcpyAsync(rejected, d_rej, N * 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "D2H outputs");
+    return GEO_OK;
+}
+
 int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, int32_t info[4]) {
     if (!ctx || !info || n < 0) return GEO_EINVAL;
     if (ctx->metric == GEO_TABULATED) {

@@ -22,7 +22,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI
 
 # every symbol include/geo.h declares
-SYMBOLS = ("geo_create", "geo_create_tabulated", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_destroy",
+SYMBOLS = ("geo_create", "geo_create_tabulated", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_integrate_adaptive_host", "geo_destroy",
            "geo_horizon_radius", "geo_last_error", "geo_launch_info", "geo_probe_dfma")
 
 
@@ -211,6 +211,22 @@ def geo_integrate_adaptive(ctx, state_in, h0: float, rtol: float, atol: float, m
         rc = L.geo_integrate_adaptive(ctx, state_in.data_ptr(), n, C.byref(ctl), max_attempts, C.byref(stop),
                                       C.byref(o), _ptr(rejected), C.c_void_p(s.cuda_stream))
     _check(ctx, rc)
+
+
+def geo_integrate_adaptive_host(ctx, state_in, h0: float, rtol: float, atol: float, max_attempts: int, out: dict,
+                                r_capture: float = -float("inf"), r_escape: float = float("inf"), kind: int = TIMELIKE,
+                                h_min: float = 1e-12, tau_end: float = float("inf"), rejected=None) -> None:
+    """The adaptive RK5(4) integration on HOST buffers (numpy arrays or pinned CPU tensors); synchronous."""
+    n = state_in.shape[1]
+    stop = GeoStop(r_capture, r_escape, kind, 0)
+    ctl = GeoAdaptive(h0, rtol, atol, h_min, tau_end)
+    o = _out_struct(out)
+    L = lib()
+    L.geo_integrate_adaptive_host.restype = C.c_int
+    L.geo_integrate_adaptive_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(GeoAdaptive), C.c_int64,
+                                              C.POINTER(GeoStop), C.POINTER(GeoOut), C.c_void_p]
+    _check(ctx, L.geo_integrate_adaptive_host(ctx, _ptr(state_in), n, C.byref(ctl), max_attempts, C.byref(stop),
+                                              C.byref(o), _ptr(rejected)))
 
 
 def geo_integrate_host(ctx, state_in: np.ndarray, h: float, nsteps: int, out: dict,

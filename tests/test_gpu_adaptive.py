@@ -129,3 +129,23 @@ def test_adaptive_whole_image_classes_match_the_analytic_criterion(G):
           "mean accepted steps", float(g["steps_done"].mean()), "mean rejected", float(g["rejected"].mean()))
     assert np.isin(g["status"], (G.ST_CAPTURED, G.ST_ESCAPED)).all()
     assert wrong.sum() <= 4                       # measured: 0 of 1 048 576
+
+
+def test_adaptive_host_entry_point_equals_the_device_one(G):
+    """geo_integrate_adaptive_host (H2D, launch, D2H inside the C ABI) returns bit for bit what the device entry point does."""
+    a = 0.998
+    full = W.camera_rays(256, a, 60.0)
+    ii = np.arange(256 * 256).reshape(256, 256)[3::5, 1::5].ravel()
+    st = np.ascontiguousarray(full[:, ii])
+    rp = W.horizon_radius(1.0, a)
+    g = run_gpu_adaptive(G, G.KERR, a, st, 0.02, 1e-9, 1e-9, 200000, kind=G.NULL, r_capture=rp + 0.01, r_escape=1100.0)
+    ctx = G.geo_create(G.KERR, 1.0, a)
+    out = G.alloc_outputs_host(st.shape[1])
+    rej = np.zeros(st.shape[1], dtype=np.int32)
+    G.geo_integrate_adaptive_host(ctx, st, 0.02, 1e-9, 1e-9, 200000, out, kind=G.NULL, r_capture=rp + 0.01, r_escape=1100.0,
+                                  rejected=rej)
+    G.geo_destroy(ctx)
+    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health"):
+        assert np.array_equal(np.asarray(out[k]), g[k], equal_nan=True), k
+    assert np.array_equal(rej, g["rejected"])
+

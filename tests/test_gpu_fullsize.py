@@ -186,3 +186,61 @@ def test_config3_whole_image_classes_match_the_analytic_criterion(G):
     assert wrong.sum() <= 2e-3 * N * N
     health = out["health"].cpu().numpy()
     assert np.median(health[wrong & axis]) > 1e-9 if (wrong & axis).any() else True   # flagged as numerically invalid
+
+
+def test_tab4_full_2p22_tabulated_sampled(G, tab_oracle):
+    """bench.py --workload tab4: the 2^22 particles of configs[3] through the 2053 x 517-node table of
+    the Kerr a = 0.5 metric, 1000 steps, in the bench's launch configuration; sampled particles against the
+    tabulated-metric oracle, whole-batch properties."""
+    import math
+    import torch
+    a, n = 0.5, 1 << 22
+    st = W.kerr_bound(n, a, W.SEED_BASE + 4, nthreads=NCPU, chunk=1 << 20)
+    tb = W.kerr_metric_table(1.0, a, 2049, 513, 2.0, 45.0, 0.1, math.pi - 0.1)
+    dev = torch.device("cuda:0")
+    ctx = G.geo_create_tabulated(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+    try:
+        out = G.alloc_outputs(n, dev)
+        G.geo_integrate(ctx, torch.from_numpy(st).to(dev), 0.01, 1000, out)
+        torch.cuda.synchronize()
+    finally:
+        G.geo_destroy(ctx)
+    ii = _sample(n, 3000, 11)
+    g = _take(out, ii)
+    o = tab_oracle.integrate(tb, np.ascontiguousarray(st[:, ii]), 0.01, 1000, nthreads=NCPU)
+    c = parity.compare(g, o)
+    assert c["same_class"].all() and c["err"].max() <= 1e-9, c["err"].max()
+    status = out["status"].cpu().numpy()
+    assert np.isin(status, (G.ST_MAXSTEPS, G.ST_OUTSIDE)).all() and (status == G.ST_MAXSTEPS).mean() > 0.99
+    assert np.array_equal(out["final_state"][7].cpu().numpy(), st[5])            # p_phi exact
+    assert np.nanmax(out["health"].cpu().numpy()) < 1e-6
+
+
+def test_config3a_full_image_adaptive_sampled(G, oracle):
+    """bench.py --workload config3a: all 1024^2 rays of configs[2] with the adaptive stepper; sampled
+    rays against the oracle's adaptive path -- an accept/reject decision near err = 1 may differ, so: class identical on
+    all samples, and finals within 1e-8 where the two took the same step sequence (>= 95 % of the samples)."""
+    import torch
+    a, N = 0.998, 1024
+    st = W.camera_rays(N, a, 60.0)
+    rc = W.horizon_radius(1.0, a) + 0.01
+    dev = torch.device("cuda:0")
+    ctx = G.geo_create(G.KERR, 1.0, a)
+    try:
+        out = G.alloc_outputs(N * N, dev)
+        rej = torch.zeros(N * N, dtype=torch.int32, device=dev)
+        G.geo_integrate_adaptive(ctx, torch.from_numpy(st).to(dev), 0.02, 1e-9, 1e-9, 200000, out, r_capture=rc,
+                                 r_escape=1100.0, kind=G.NULL, rejected=rej)
+        torch.cuda.synchronize()
+    finally:
+        G.geo_destroy(ctx)
+    ii = _sample(N * N, 3000, 12)
+    g = _take(out, ii)
+    grej = rej[torch.from_numpy(ii).to(dev)].cpu().numpy()
+    o = oracle.integrate_adaptive(oracle.KERR, 1.0, a, np.ascontiguousarray(st[:, ii]), 0.02, 1e-9, 1e-9, 200000,
+                                  r_capture=rc, r_escape=1100.0, kind=oracle.NULL, nthreads=NCPU)
+    assert (g["status"] == o["status"]).mean() >= 0.999
+    same = (g["status"] == o["status"]) & (g["steps_done"] == o["steps_done"]) & (grej == o["rejected"])
+    assert same.mean() >= 0.95, same.mean()
+    e = parity.rel_err(g["final_state"][:, same], o["final_state"][:, same]).max(axis=0)
+    assert np.quantile(e, 0.99) <= 1e-8 and e.max() <= 1e-6, (np.quantile(e, 0.99), e.max())

@@ -218,8 +218,8 @@ def test_tab4_full_2p22_tabulated_sampled(G, tab_oracle):
 
 def test_config3a_full_image_adaptive_sampled(G, oracle):
     """bench.py --workload config3a: all 1024^2 rays of configs[2] with the adaptive stepper; sampled
-    rays against the oracle's adaptive path -- an accept/reject decision near err = 1 may differ, so: class identical on
-    all samples, and finals within 1e-8 where the two took the same step sequence (>= 95 % of the samples)."""
+    rays against the oracle's adaptive path: class identical, the escaped photon's direction and momenta within 1e-8 on
+    certified rays (see below for what a fixed tolerance leaves undetermined)."""
     import torch
     a, N = 0.998, 1024
     st = W.camera_rays(N, a, 60.0)
@@ -237,10 +237,25 @@ def test_config3a_full_image_adaptive_sampled(G, oracle):
     ii = _sample(N * N, 3000, 12)
     g = _take(out, ii)
     grej = rej[torch.from_numpy(ii).to(dev)].cpu().numpy()
-    o = oracle.integrate_adaptive(oracle.KERR, 1.0, a, np.ascontiguousarray(st[:, ii]), 0.02, 1e-9, 1e-9, 200000,
-                                  r_capture=rc, r_escape=1100.0, kind=oracle.NULL, nthreads=NCPU)
+    kw = dict(r_capture=rc, r_escape=1100.0, kind=oracle.NULL, nthreads=NCPU)
+    sub = np.ascontiguousarray(st[:, ii])
+    o = oracle.integrate_adaptive(oracle.KERR, 1.0, a, sub, 0.02, 1e-9, 1e-9, 200000, **kw)
+    o_ld = oracle.integrate_adaptive(oracle.KERR, 1.0, a, sub, 0.02, 1e-9, 1e-9, 200000, long_double=True, **kw)
     assert (g["status"] == o["status"]).mean() >= 0.999
+    # What is unique at a fixed tolerance: the controller's error estimate is a difference of nearly equal numbers, so
+    # its rounding noise (~1e-8 relative in h, measured between the oracle's double and long double runs) moves the
+    # point ALONG the ray at which an escaping ray is stopped (t, r: ~1e-7 relative), while the ray itself -- theta,
+    # phi, p_r, p_theta of the escaped photon -- is fixed to ~1e-11.  Reading P3 carried over to those components: a
+    # ray is certified iff the oracle's double and long double runs agree in class and within 1e-9 on them.  Captured
+    # rays: class only (their record is the last accepted state next to the horizon).
+    rows = [2, 3, 5, 6]
+    esc = o["status"] == oracle.ST_ESCAPED
+    cert = esc & (o_ld["status"] == o["status"]) & (parity.rel_err(o["final_state"][rows], o_ld["final_state"][rows]).max(axis=0) <= 1e-9)
+    e_ray = parity.rel_err(g["final_state"][rows], o["final_state"][rows]).max(axis=0)
+    e_along = parity.rel_err(g["final_state"][[0, 1]], o["final_state"][[0, 1]]).max(axis=0)
     same = (g["status"] == o["status"]) & (g["steps_done"] == o["steps_done"]) & (grej == o["rejected"])
-    assert same.mean() >= 0.95, same.mean()
-    e = parity.rel_err(g["final_state"][:, same], o["final_state"][:, same]).max(axis=0)
-    assert np.quantile(e, 0.99) <= 1e-8 and e.max() <= 1e-6, (np.quantile(e, 0.99), e.max())
+    print("adaptive full image: escaped", esc.mean(), "certified", cert.mean(), "same sequence", same.mean(),
+          "max err on certified: ray", e_ray[cert].max(), "along", e_along[cert].max())
+    assert cert.sum() > 0.9 * esc.sum() and same.mean() >= 0.95
+    assert (g["status"] == o["status"])[cert].all()
+    assert e_ray[cert].max() <= 1e-8 and e_along[cert].max() <= 1e-6, (e_ray[cert].max(), e_along[cert].max())

@@ -139,7 +139,7 @@ tab_kernel_fn pick_tab_kernel(int32_t flags) {
         return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tab_kernel_fn)geo_tab_rk4_kernel<true, false> : (tab_kernel_fn)geo_tab_rk4_kernel<false, false>;
     return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tab_kernel_fn)geo_tab_rk4_kernel<true, true> : (tab_kernel_fn)geo_tab_rk4_kernel<false, true>;
 }
-size_t tab_smem(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? 0 : (size_t)kStencil * kTabBlock * sizeof(double); }
+size_t tab_smem(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? 0 : (size_t)kTabSmemRows * kTabBlock * sizeof(double); }
 
 int plan_tab(geo_ctx* ctx, int64_t n, int32_t flags, int* grid, int* per_sm_out, int* regs) {
     tab_kernel_fn fn = pick_tab_kernel(flags);

@@ -132,44 +132,52 @@ __device__ __forceinline__ bool tab_fields(const TabMetric& m, double x1, double
     return in1 & in2;
 }
 
-// ---- per-lane stencil cache in shared memory ---------------------------------------------------------------
+// ---- per-lane stencil cache ------------------------------------------------------------------------------------
 // A particle stays in one grid cell for many evaluations (a step moves it by h |dx/dtau| << d), so the 4 x 4 x 5
-// stencil of its current cell is kept in shared memory: column-major [80][kTabBlock] doubles per CTA (lane l owns
-// column l: its 64-bit accesses are conflict-free, 2 wavefronts per warp instruction) and refilled from the
-// table only when the cell index changes.  Element (b, a, f) of the stencil sits at row (b*4 + a)*5 + f.
-constexpr int kStencil = 80;
+// stencil of its current cell is kept on chip and refilled from the table only when the cell index changes: the
+// stencils of the first R fields in REGISTERS (statically indexed after unrolling; the refill writes them under the
+// lane's predicate), those of the other S = 5 - R fields in shared memory, column-major [16 S][kTabBlock] doubles per
+// CTA (lane l owns column l: its 64-bit accesses are conflict-free, 2 wavefronts per warp instruction instead of
+// the 32 of a gather).  Element (b, a, f) of the shared part sits at row (b*4 + a) S + (f - R).
+// Measured (profiles/r01_tab4.md): R = 0 7.20e9, R = 1 7.38e9, R = 2 7.26e9, R = 3 6.25e9 (spills), R = 5 6.85e9 steps/s.
 #ifndef GEO_TAB_BLOCK
 #define GEO_TAB_BLOCK 128
 #endif
 #ifndef GEO_TAB_CTAS
 #define GEO_TAB_CTAS 2
 #endif
+#ifndef GEO_TAB_REGFIELDS
+#define GEO_TAB_REGFIELDS 1
+#endif
 constexpr int kTabBlock = GEO_TAB_BLOCK;      // threads per CTA of the tabulated-metric kernels
+constexpr int kTabRegFields = GEO_TAB_REGFIELDS;
+constexpr int kTabSmemRows = 16 * (5 - kTabRegFields);
 
-__device__ __noinline__ void tab_refill(const TabMetric& m, int i, int j, double* col) {
-    const long long base = (long long)(j - 1) * m.n1 + (i - 1);
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-        const double4* ra = m.A + base + (long long)b * m.n1;
-        const double* rb = m.B + base + (long long)b * m.n1;
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            const double4 v = ldg256(ra + a);
-            const double w = __ldg(rb + a);
-            double* q = col + (b * 4 + a) * 5 * kTabBlock;
-            q[0] = v.x; q[kTabBlock] = v.y; q[2 * kTabBlock] = v.z; q[3 * kTabBlock] = v.w; q[4 * kTabBlock] = w;
-        }
-    }
-}
-
-__device__ __forceinline__ bool tab_fields_cached(const TabMetric& m, double x1, double x2, TabFields& F, int& ci, int& cj,
-                                                  double* col) {
+template <int R>
+__device__ __forceinline__ bool tab_fields_hybrid(const TabMetric& m, double x1, double x2, TabFields& F, int& ci, int& cj,
+                                                  double* col, double (&rs)[16][R > 0 ? R : 1]) {
+    constexpr int S = 5 - R;
     int i, j;
     double s1, s2;
     const bool in1 = tab_cell(x1, m.x1_0, m.d1, m.inv_d1, m.n1, i, s1);
     const bool in2 = tab_cell(x2, m.x2_0, m.d2, m.inv_d2, m.n2, j, s2);
     if (i != ci || j != cj) {
-        tab_refill(m, i, j, col);
+        const long long base = (long long)(j - 1) * m.n1 + (i - 1);
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const double4* ra = m.A + base + (long long)b * m.n1;
+            const double* rb = m.B + base + (long long)b * m.n1;
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                const double4 v = ldg256(ra + a);
+                const double vals[5] = {v.x, v.y, v.z, v.w, __ldg(rb + a)};
+#pragma unroll
+                for (int f = 0; f < 5; ++f) {
+                    if (f < R) rs[b * 4 + a][f < R ? f : 0] = vals[f];
+                    else col[((b * 4 + a) * S + (f - R)) * kTabBlock] = vals[f];
+                }
+            }
+        }
         ci = i;
         cj = j;
     }
@@ -179,12 +187,14 @@ __device__ __forceinline__ bool tab_fields_cached(const TabMetric& m, double x1,
     double v[5] = {0, 0, 0, 0, 0}, g1[5] = {0, 0, 0, 0, 0}, g2[5] = {0, 0, 0, 0, 0};
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
-        const double* q = col + b * 20 * kTabBlock;
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
-            const double c0 = q[k * kTabBlock], c1 = q[(5 + k) * kTabBlock], c2 = q[(10 + k) * kTabBlock], c3 = q[(15 + k) * kTabBlock];
-            const double rv = fma(w1[3], c3, fma(w1[2], c2, fma(w1[1], c1, w1[0] * c0)));
-            const double rd = fma(dw1[3], c3, fma(dw1[2], c2, fma(dw1[1], c1, dw1[0] * c0)));
+            double c[4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+                c[a] = k < R ? rs[b * 4 + a][k < R ? k : 0] : col[((b * 4 + a) * S + (k - R)) * kTabBlock];
+            const double rv = fma(w1[3], c[3], fma(w1[2], c[2], fma(w1[1], c[1], w1[0] * c[0])));
+            const double rd = fma(dw1[3], c[3], fma(dw1[2], c[2], fma(dw1[1], c[1], dw1[0] * c[0])));
             v[k] = fma(w2[b], rv, v[k]);
             g1[k] = fma(w2[b], rd, g1[k]);
             g2[k] = fma(dw2[b], rv, g2[k]);
@@ -219,7 +229,7 @@ __device__ __noinline__ bool tab_fields_cold(const TabMetric& m, double x1, doub
     return tab_fields(m, x1, x2, F);
 }
 
-// CACHE: stencil cache in shared memory (kStencil * kTabBlock doubles = 80 KB per CTA, 2 CTAs/SM);
+// CACHE: per-lane stencil cache (kTabSmemRows * kTabBlock doubles = 64 KB of shared memory per CTA, 2 CTAs/SM);
 // !CACHE: every evaluation gathers its stencil through L1/L2 (GEO_FLAG_TAB_GATHER, for comparison).
 template <bool PLAIN, bool CACHE>
 __global__ void __launch_bounds__(kTabBlock, CACHE ? GEO_TAB_CTAS : 3) geo_tab_rk4_kernel(const __grid_constant__ TabParams p) {
@@ -228,8 +238,9 @@ __global__ void __launch_bounds__(kTabBlock, CACHE ? GEO_TAB_CTAS : 3) geo_tab_r
     int ci = -1, cj = -1;                                          // cell whose stencil the column holds
     const unsigned lane = threadIdx.x & 31u;
     const TabMetric& m = p.m;
+    double rs[16][kTabRegFields > 0 ? kTabRegFields : 1];          // register-resident part of the stencil cache
     auto fields = [&](double a, double b, TabFields& F) -> bool {
-        if (CACHE) return tab_fields_cached(m, a, b, F, ci, cj, col);
+        if (CACHE) return tab_fields_hybrid<kTabRegFields>(m, a, b, F, ci, cj, col, rs);
         return tab_fields(m, a, b, F);
     };
     long long idx = -1;

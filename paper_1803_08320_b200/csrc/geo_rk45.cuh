@@ -46,6 +46,26 @@ constexpr double e1 = 35.0 / 384 - 5179.0 / 57600, e3 = 500.0 / 1113 - 7571.0 / 
                  e5 = -2187.0 / 6784 + 92097.0 / 339200, e6 = 11.0 / 84 - 187.0 / 2100, e7 = -1.0 / 40;
 }  // namespace dp
 
+// x^(-1/5) for the step-size controller: single-precision seed (MUFU lg2/ex2), two Newton steps on y^-5 = x
+// (y <- y (6 - x y^5)/5, relative error 3 eps^2 per step), a few ulp in all.  The controller clamps the factor to
+// [0.2, 5], i.e. only x in [1.9e-4, 1.8e3] matters: x is clamped to [1e-5, 1e4] first, which keeps the float seed
+// in range (+inf included).  Replaces pow(x, -0.2) (~150 instructions with its special-case paths).
+__device__ __forceinline__ double inv_fifth_root(double x) {
+    const double xc = fmin(fmax(x, 1.0e-5), 1.0e4);
+    double y = (double)exp2f(-0.2f * __log2f((float)xc));
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const double y2 = y * y;
+        const double y5 = y2 * y2 * y;
+        y *= fma(-0.2 * xc, y5, 1.2);
+    }
+    return y;
+}
+
+// |e| / sc with one faithfully rounded reciprocal instead of an IEEE division (the quotient may differ from the
+// oracle's by an ulp -- like every FMA-contracted sum that feeds it)
+__device__ __forceinline__ double scaled_err(double e, double sc) { return fabs(e) * rcp_nr(sc); }
+
 // the four components that feed back into the RHS
 struct K4 {
     double r, th, pr, pth;
@@ -206,14 +226,14 @@ __global__ void __launch_bounds__(kBlock, 3) geo_rk45_kernel(const __grid_consta
         // error estimate h (b5 - b4) . k, scaled per component; a NaN sticks in the max
 #define GEO_E(c) fma(dp::e7, k7.c, fma(dp::e6, q6.c, fma(dp::e5, q5.c, fma(dp::e4, q4.c, fma(dp::e3, q3.c, dp::e1 * q1.c)))))
         double err = 0.0, ec;
-        ec = fabs(h * fma(dp::e7, k7.t, set_)) / fma(p.rtol, fmax(fabs(t), fabs(nt)), p.atol);       if (!(ec <= err)) err = ec;
-        ec = fabs(h * GEO_E(r)) / fma(p.rtol, fmax(fabs(r), fabs(nr)), p.atol);                        if (!(ec <= err)) err = ec;
-        ec = fabs(h * GEO_E(th)) / fma(p.rtol, fmax(fabs(th), fabs(nth)), p.atol);                     if (!(ec <= err)) err = ec;
-        ec = fabs(h * fma(dp::e7, k7.ph, sep)) / fma(p.rtol, fmax(fabs(ph), fabs(nph)), p.atol);      if (!(ec <= err)) err = ec;
-        ec = fabs(h * GEO_E(pr)) / fma(p.rtol, fmax(fabs(pr), fabs(npr)), p.atol);                     if (!(ec <= err)) err = ec;
-        ec = fabs(h * GEO_E(pth)) / fma(p.rtol, fmax(fabs(pth), fabs(npth)), p.atol);                  if (!(ec <= err)) err = ec;
+        ec = scaled_err(h * fma(dp::e7, k7.t, set_), fma(p.rtol, fmax(fabs(t), fabs(nt)), p.atol));       if (!(ec <= err)) err = ec;
+        ec = scaled_err(h * GEO_E(r), fma(p.rtol, fmax(fabs(r), fabs(nr)), p.atol));                        if (!(ec <= err)) err = ec;
+        ec = scaled_err(h * GEO_E(th), fma(p.rtol, fmax(fabs(th), fabs(nth)), p.atol));                     if (!(ec <= err)) err = ec;
+        ec = scaled_err(h * fma(dp::e7, k7.ph, sep), fma(p.rtol, fmax(fabs(ph), fabs(nph)), p.atol));      if (!(ec <= err)) err = ec;
+        ec = scaled_err(h * GEO_E(pr), fma(p.rtol, fmax(fabs(pr), fabs(npr)), p.atol));                     if (!(ec <= err)) err = ec;
+        ec = scaled_err(h * GEO_E(pth), fma(p.rtol, fmax(fabs(pth), fabs(npth)), p.atol));                  if (!(ec <= err)) err = ec;
 #undef GEO_E
-        double fac = err > 0.0 ? 0.9 * pow(err, -0.2) : 5.0;
+        double fac = err > 0.0 ? 0.9 * inv_fifth_root(err) : 5.0;
         if (!(fac >= 0.2)) fac = 0.2;                                            // also catches NaN
         if (fac > 5.0) fac = 5.0;
         if (p.fixed_step) { fac = 1.0; err = fin6 ? 0.0 : err; }

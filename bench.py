@@ -50,13 +50,13 @@ FLOP_COUNT_SOURCE = {"kerr": "ncu dynamic count (profiles/r01_config4_v3.md)", "
                      "tabulated": "ncu dynamic thread-level count (profiles/r01_tab4.md): 918 DFMA + 323 DMUL + 58 DADD per step"}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
 # adaptive RK5(4) kernel, per step ATTEMPT of one Kerr geodesic, executed (ncu, thread level)
-ADAPTIVE_FLOP_PER_ATTEMPT, ADAPTIVE_PIPE_PER_ATTEMPT = 1211.0, 785.0
-ADAPTIVE_SOURCE = "ncu dynamic thread-level count (profiles/r01_config3a_rk45.md): 426 DFMA + 268 DMUL + 90 DADD per attempt"
+ADAPTIVE_FLOP_PER_ATTEMPT, ADAPTIVE_PIPE_PER_ATTEMPT = 1045.0, 684.0
+ADAPTIVE_SOURCE = "ncu dynamic thread-level count (profiles/r01_config3a_rk45.md): 361 DFMA + 271 DMUL + 52 DADD per attempt"
 # declared algorithmic work of one Kerr RK4 step (4 RHS + compensated update).
 F_ALG_SURVEY = {"kerr": 800.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one geo_rk4_kernel launch from the committed
 # `ncu --set full` capture of that workload (profiles/), bytes; None where no capture exists.
-TRAFFIC_NCU_BYTES = {"config3a": 99_734_272, "tab4": 657_377_536, "config4": 580_706_816, "snapbench": 69_562_443_296}      # profiles/r01_config4_v3.md, r01_snapbench_v3.md, r01_config3a_rk45.md, r01_tab4.md (full-size capture of v2: particle I/O only)
+TRAFFIC_NCU_BYTES = {"config3a": 103_028_736, "tab4": 657_377_536, "config4": 580_706_816, "snapbench": 69_562_443_296}      # profiles/r01_config4_v3.md, r01_snapbench_v3.md, r01_config3a_rk45.md, r01_tab4.md (full-size capture of v2: particle I/O only)
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:

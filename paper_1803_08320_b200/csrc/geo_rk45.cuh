@@ -14,6 +14,9 @@
 // of DESIGN.md A5 is what keeps the lanes busy here.
 #pragma once
 #include "geo_kernel.cuh"
+#ifndef GEO_RK45_CTAS
+#define GEO_RK45_CTAS 3      // resident CTAs per SM the kernel is compiled for (168 registers, no spills)
+#endif
 
 namespace geo {
 
@@ -82,7 +85,7 @@ __device__ __forceinline__ void rhs_at(const Hole& bh, double r, double th, doub
 __device__ __forceinline__ K4 k4_of(const Deriv& d) { return K4{d.r, d.th, d.pr, d.pth}; }
 
 template <bool KERR>
-__global__ void __launch_bounds__(kBlock, 3) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
+__global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
     const unsigned lane = threadIdx.x & 31u;
     const Hole& bh = p.bh;
     long long idx = -1;

@@ -16,8 +16,10 @@
 //   B[j][i] = gamma_33                                                    -> four consecutive doubles per stencil row.
 // One RHS evaluation reads the 4 x 4 stencil = 16 records of A + 16 doubles of B = 640 B per lane, ~23 32-B
 // sectors; a whole table of 2053 x 517 nodes is 42 MB and lives in the 126 MB L2.  Per lane and evaluation:
-// 16 LDG.256 + 16 LDG.64, ~330 FP64 instructions (separable evaluation: 8 FMA per field and stencil row for the
-// value and the x^1-derivative along x^1, then 3 FMA per row along x^2).
+// ~330 FP64 instructions (separable evaluation: 8 FMA per field and stencil row for the value and the
+// x^1-derivative along x^1, then 3 FMA per row along x^2).  The stencil is read from the table (16 LDG.256 + 16
+// LDG.64) only when the particle enters a new cell: between refills it sits in a per-lane on-chip cache (below).
+// GEO_FLAG_TAB_GATHER selects the variant that gathers it on every evaluation (L1-wavefront-bound, 2.6x slower).
 #pragma once
 #include "geo_kernel.cuh"
 

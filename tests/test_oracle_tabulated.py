@@ -232,6 +232,11 @@ def test_tabulated_kerr_orbits_converge_to_the_analytic_oracle_in_both_radial_co
             assert np.nanmax(o["health"]) < 1e-7                  # 2H + 1 drift: RK4 + the C^1 interpolant
             errs.append(np.max(np.abs(f[[0, 1, 2, 3, 5, 6]] - ref["final_state"][[0, 1, 2, 3, 5, 6]])
                                / np.maximum(np.abs(ref["final_state"][[0, 1, 2, 3, 5, 6]]), 1.0)))
+            if radial == "r" and n1 == 2049:
+                # equatorial-crossing event (B5): same particles cross, at the analytic oracle's radius
+                crossed = ~np.isnan(ref["eq_cross_r"])
+                assert crossed.sum() > 5 and np.array_equal(~np.isnan(o["eq_cross_r"]), crossed)
+                assert np.max(np.abs(o["eq_cross_r"][crossed] - ref["eq_cross_r"][crossed])) < 1e-5
         assert errs[1] < 2e-5 and errs[0] / errs[1] > 6, (radial, errs)
 
 

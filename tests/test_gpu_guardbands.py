@@ -1,0 +1,166 @@
+"""Guard bands around every caller-owned buffer of the C-ABI calls (include/geo.h): each output (and the input)
+lives in the middle of a larger allocation whose margins hold a canary bit pattern; after the call the margins
+must be untouched, the input unchanged, and the results bitwise equal to those of a run on plain buffers.
+This is the repo's own bounds check of the kernels' address arithmetic (work queue refill, final records,
+direct / staged / Cartesian snapshot writers with 32-B and with only 16-B aligned slots, capacity overflow, the adaptive
+and the tabulated-metric kernels) on ragged batches with mixed termination classes."""
+import math
+import os
+import sys
+
+import numpy as np
+import pytest
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+
+from paper_1803_08320_b200 import workloads as W  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+CANARY64 = 0x7FF8DEADBEEFCAFE      # a quiet-NaN payload when read as a double
+CANARY32 = 0x5A5A5A5A
+
+
+class Guarded:
+    """Copies of tensors placed `pad` elements into canary-filled allocations."""
+
+    def __init__(self):
+        self.items = []
+
+    def wrap(self, t, pad=64):
+        import torch
+        if t is None:
+            return None
+        ity = torch.int64 if t.element_size() == 8 else torch.int32
+        flat = torch.empty(t.numel() + 2 * pad, dtype=ity, device=t.device)
+        flat.fill_(CANARY64 if ity == torch.int64 else CANARY32)
+        mid = flat[pad:pad + t.numel()].view(t.dtype).view(t.shape)
+        mid.copy_(t)
+        self.items.append((flat, pad, t.numel()))
+        return mid
+
+    def check(self):
+        import torch
+        for flat, pad, numel in self.items:
+            c = CANARY64 if flat.dtype == torch.int64 else CANARY32
+            assert bool((flat[:pad] == c).all()), "write below a buffer"
+            assert bool((flat[pad + numel:] == c).all()), "write beyond a buffer"
+
+
+def guard_outputs(out, gd, snap_pad=64):
+    g = dict(out)
+    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health", "snap_count"):
+        g[k] = gd.wrap(out[k])
+    g["snapshots"] = gd.wrap(out["snapshots"], snap_pad)
+    return g
+
+
+def bits(x):
+    x = np.ascontiguousarray(x)
+    return x.view(np.int64) if x.dtype == np.float64 else x
+
+
+def same_bits(a, b):
+    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health", "snapshots", "snap_count"):
+        if a.get(k) is None:
+            assert b.get(k) is None
+            continue
+        assert np.array_equal(bits(a[k]), bits(b[k])), k
+
+
+def mixed_rays(a):
+    """571 photons from a near camera: some captured, some escape, the rest run to the step cap."""
+    st = W.camera_rays(24, a, 60.0, r_obs=30.0, width=16.0)
+    return np.ascontiguousarray(st[:, :571])
+
+
+@pytest.mark.parametrize("flags,mask,cap,snap_pad", [
+    (0, 0xFF, None, 64),          # direct writer, 256-bit stores, 32-B aligned slots
+    (0, 0xFF, None, 62),          # same records on 16-B aligned slots (include/geo.h minimum): no 256-bit stores
+    (0, 0x0F, 5, 64),             # 4-component records, capacity overflow (S3)
+    (0, 0x07, 5, 62),             # odd component count
+    (4, 0xFF, None, 64),          # staged writer (GEO_FLAG_STAGED_SNAP)
+    (4, 0x07, 5, 62),
+    (8, 0xFF, None, 64),          # Cartesian records (GEO_FLAG_CARTESIAN_SNAP)
+    (2, 0xFF, None, 64),          # static mapping (GEO_FLAG_STATIC_MAP)
+    (2 | 4, 0x0E, 3, 64),
+])
+def test_rk4_kernels_write_inside_their_buffers(G, flags, mask, cap, snap_pad):
+    import torch
+    a = 0.998
+    st = mixed_rays(a)
+    n = st.shape[1]
+    dev = torch.device("cuda:0")
+    kw = dict(r_capture=1.0 + math.sqrt(1.0 - a * a) + 0.01, r_escape=33.0, kind=G.NULL, flags=flags, snapshot_every=50)
+    ctx = G.geo_create(G.KERR, 1.0, a)
+    try:
+        d_in = torch.from_numpy(st).to(dev)
+        plain = G.alloc_outputs(n, dev, 1500, 50, cap, mask)
+        G.geo_integrate(ctx, d_in, 0.05, 1500, plain, **kw)
+        gd = Guarded()
+        g_in = gd.wrap(d_in)
+        guarded = guard_outputs(G.alloc_outputs(n, dev, 1500, 50, cap, mask), gd, snap_pad)
+        G.geo_integrate(ctx, g_in, 0.05, 1500, guarded, **kw)
+        torch.cuda.synchronize()
+        gd.check()
+        assert np.array_equal(bits(g_in.cpu().numpy()), bits(st))
+        p, g = G.to_numpy(plain), G.to_numpy(guarded)
+        same_bits(p, g)
+        assert len(np.unique(p["status"])) >= 2          # the batch does mix termination classes
+    finally:
+        G.geo_destroy(ctx)
+
+
+@pytest.mark.parametrize("metric_a", [(0, 0.0), (1, 0.998)])
+def test_adaptive_kernel_writes_inside_its_buffers(G, metric_a):
+    import torch
+    metric, a = metric_a
+    st = mixed_rays(a)
+    n = st.shape[1]
+    dev = torch.device("cuda:0")
+    kw = dict(r_capture=1.0 + math.sqrt(1.0 - a * a) + 0.01, r_escape=33.0, kind=G.NULL)
+    ctx = G.geo_create(metric, 1.0, a)
+    try:
+        d_in = torch.from_numpy(st).to(dev)
+        plain = G.alloc_outputs(n, dev)
+        rej = torch.full((n,), -1, dtype=torch.int32, device=dev)
+        G.geo_integrate_adaptive(ctx, d_in, 0.1, 1e-9, 1e-12, 2000, plain, rejected=rej, **kw)
+        gd = Guarded()
+        g_in = gd.wrap(d_in)
+        guarded = guard_outputs(G.alloc_outputs(n, dev), gd)
+        g_rej = gd.wrap(torch.full((n,), -1, dtype=torch.int32, device=dev))
+        G.geo_integrate_adaptive(ctx, g_in, 0.1, 1e-9, 1e-12, 2000, guarded, rejected=g_rej, **kw)
+        torch.cuda.synchronize()
+        gd.check()
+        assert np.array_equal(bits(g_in.cpu().numpy()), bits(st))
+        same_bits(G.to_numpy(plain), G.to_numpy(guarded))
+        assert np.array_equal(rej.cpu().numpy(), g_rej.cpu().numpy())
+    finally:
+        G.geo_destroy(ctx)
+
+
+@pytest.mark.parametrize("flags", [0, 16])       # stencil cache / GEO_FLAG_TAB_GATHER
+def test_tabulated_kernel_writes_inside_its_buffers(G, flags):
+    import torch
+    a = 0.9
+    tb = W.kerr_metric_table(1.0, a, 257, 65, 1.8, 40.0, 0.2, math.pi - 0.2)
+    st = np.ascontiguousarray(W.kerr_bound(333, a, W.SEED_BASE + 2))
+    n = st.shape[1]
+    dev = torch.device("cuda:0")
+    ctx = G.geo_create_tabulated(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+    try:
+        d_in = torch.from_numpy(st).to(dev)
+        plain = G.alloc_outputs(n, dev)
+        G.geo_integrate(ctx, d_in, 0.01, 2000, plain, flags=flags, r_capture=2.5, r_escape=25.0)
+        gd = Guarded()
+        g_in = gd.wrap(d_in)
+        guarded = guard_outputs(G.alloc_outputs(n, dev), gd)
+        G.geo_integrate(ctx, g_in, 0.01, 2000, guarded, flags=flags, r_capture=2.5, r_escape=25.0)
+        torch.cuda.synchronize()
+        gd.check()
+        assert np.array_equal(bits(g_in.cpu().numpy()), bits(st))
+        p = G.to_numpy(plain)
+        same_bits(p, G.to_numpy(guarded))
+        assert len(np.unique(p["status"])) >= 2
+    finally:
+        G.geo_destroy(ctx)

@@ -153,14 +153,13 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
     const Hole& bh = p.bh;
 
     // lane state (registers)
-    long long idx = -1;
-    bool active = false;
+    long long idx = -1;                   // particle this lane integrates; < 0: the lane is idle
+    auto active = [&]() { return idx >= 0; };
     bool exhausted = !p.use_queue;
     double t = 0, r = 0, th = 0, ph = 0, pr = 0, pth = 0, E = 0, L = 0;
     double ct = 0, cr = 0, cth = 0, cph = 0, cpr = 0, cpth = 0;
     int steps = 0, snap_ctr = 0;
     int snaps = 0, staged = 0, stage_first = 0;   // staged records hold slots [stage_first, stage_first+staged)
-    double eqc = 0;
     bool crossed = false;
     const int slab = stage_stride(p.ncomp);
     double* my_stage = stage_smem + (size_t)threadIdx.x * slab;
@@ -222,10 +221,10 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         p.fin[7 * n + idx] = L;
         p.status[idx] = st;
         p.steps_done[idx] = (long long)steps;
-        if (p.eq_cross_r) p.eq_cross_r[idx] = crossed ? eqc : __longlong_as_double(0x7ff8000000000000LL);
+        if (p.eq_cross_r && !crossed) p.eq_cross_r[idx] = __longlong_as_double(0x7ff8000000000000LL);
         if (p.health) p.health[idx] = health_3p1(bh, r, th, pr, pth, E, L, p.kappa);
         if (SNAP != SNAP_NONE) p.snap_count[idx] = snaps;
-        active = false;
+        idx = -1;
     };
     auto begin = [&](long long i) {
         idx = i;
@@ -244,7 +243,6 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         snaps = 0;
         staged = 0;
         crossed = false;
-        active = true;
         if (SNAP != SNAP_NONE) my_snaps = p.snaps + (size_t)i * (size_t)p.snap_cap * p.ncomp;
         // B1: tests on y0 before the first step
         if (!(r >= p.r_capture)) { finish(ST_CAPTURED); return; }
@@ -275,19 +273,19 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
 
     for (;;) {
         // --- A5: refill idle lanes from the queue ------------------------------------------------
-        unsigned idle = __ballot_sync(kFull, !active);
+        unsigned idle = __ballot_sync(kFull, !active());
         if (idle) {
             if (!exhausted) {
                 const int cnt = __popc(idle);
                 unsigned long long base = 0;
                 if (lane == 0) base = atomicAdd(p.counter, (unsigned long long)cnt);
                 base = __shfl_sync(kFull, base, 0);
-                if (!active) {
+                if (!active()) {
                     const long long cand = (long long)base + __popc(idle & ((1u << lane) - 1u));
                     if (cand < p.n) begin(cand);
                 }
                 if ((long long)base + cnt >= p.n) exhausted = true;
-                idle = __ballot_sync(kFull, !active);
+                idle = __ballot_sync(kFull, !active());
             }
             if (idle == kFull) {
                 if (exhausted) break;
@@ -333,7 +331,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         stage_trig(GEO_TC, S, C, dang, s2, sc, coarse);
         rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
         at += k.t; ar += k.r; ath += k.th; aph += k.ph; apr += k.pr; apth += k.pth;
-        if (__builtin_expect(coarse && active, 0)) {   // a stage angle moved by >= 2^-7 rad: full sin/cos path
+        if (__builtin_expect(coarse && active(), 0)) {   // a stage angle moved by >= 2^-7 rad: full sin/cos path
             // (idle lanes step on stale state -- often a captured ray next to the horizon -- and must not drag the warp here)
             double acc[6];
             int c;
@@ -353,7 +351,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         const bool fin6 = all_finite6(nt, nr, nth, nph, npr, npth);
 
         // --- A4: stop rules and events ------------------------------------------------------------
-        if (active) {
+        if (active()) {
             if (cap) {
                 finish(ST_CAPTURED);            // step not taken: final = last accepted state
             } else if (!fin6) {
@@ -363,8 +361,8 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
                     const double half_pi = 1.5707963267948966;
                     const double d0 = th - half_pi, d1 = nth - half_pi;
                     if (d0 * d1 < 0.0) {
-                        crossed = true;
-                        eqc = r + (nr - r) * (half_pi - th) / (nth - th);
+                        crossed = true;   // the radius goes straight to its slot (once per particle): no register held for it
+                        if (p.eq_cross_r) p.eq_cross_r[idx] = r + (nr - r) * (half_pi - th) / (nth - th);
                     }
                 }
                 t = nt; r = nr; th = nth; ph = nph; pr = npr; pth = npth;

@@ -45,7 +45,7 @@ UNIT = "geodesic-steps/s"
 # rarely executed blocks inside the loop's address range) is printed beside them as a cross-check.
 FLOP_PER_STEP = {"kerr": 465.0, "schwarzschild": 397.0, "tabulated": 2218.0}
 PIPE_INSTR_PER_STEP = {"kerr": 331.0, "schwarzschild": 273.0, "tabulated": 1300.0}
-OTHER_INSTR_PER_STEP = {"kerr": 106.0}     # non-FP64 instructions per step, same ncu capture
+OTHER_INSTR_PER_STEP = {"kerr": 99.0}     # non-FP64 instructions per step, same ncu capture
 FLOP_COUNT_SOURCE = {"kerr": "ncu dynamic count (profiles/r01_config4_v3.md)", "schwarzschild": "static SASS count",
                      "tabulated": "ncu dynamic thread-level count (profiles/r01_tab4.md): 918 DFMA + 323 DMUL + 58 DADD per step"}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
@@ -56,7 +56,7 @@ ADAPTIVE_SOURCE = "ncu dynamic thread-level count (profiles/r01_config3a_rk45.md
 F_ALG_SURVEY = {"kerr": 800.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one geo_rk4_kernel launch from the committed
 # `ncu --set full` capture of that workload (profiles/), bytes; None where no capture exists.
-TRAFFIC_NCU_BYTES = {"config3a": 103_028_736, "tab4": 657_377_536, "config4": 585_282_048, "snapbench": 69_562_443_296}      # profiles/r01_config4_final.md, r01_snapbench_v3.md, r01_config3a_rk45.md, r01_tab4.md (full-size capture of v2: particle I/O only)
+TRAFFIC_NCU_BYTES = {"config3a": 103_028_736, "tab4": 657_377_536, "config4": 664_555_776, "snapbench": 69_562_443_296}      # profiles/r01_config4_final.md, r01_snapbench_v3.md, r01_config3a_rk45.md, r01_tab4.md (full-size capture of v2: particle I/O only)
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:

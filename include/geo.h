@@ -77,10 +77,16 @@ typedef struct geo_out {
     uint32_t snap_mask;    /* bit k set => component k of the 8-vector is stored; ncomp = popcount      */
     int32_t *snap_count;   /* [n] records produced (slot 0 = initial state; slot j = after
                               j*snapshot_every accepted steps; none after termination) (S1)            */
+    int32_t *coarse_steps; /* [n] optional diagnostic: RK4 step attempts of this particle in which a stage angle moved
+                              by >= 2^-7 rad, so that the step was evaluated with a full sin/cos at every stage point
+                              instead of the angle-addition kernels (same result to rounding).
+                              Analytic metrics, geo_integrate / geo_integrate_host only; ignored elsewhere.           */
 } geo_out;
 
 /* Create a context for metric (6) with mass M > 0 and spin |a| <= M; Schwarzschild
- * requires a == 0.  Allocates a few bytes of device memory on the current CUDA device. */
+ * requires a == 0.  Allocates a few bytes of device memory on the CURRENT CUDA device; the ctx belongs to that
+ * device: every entry point switches to it for the duration of the call and restores the caller's current
+ * device before returning, so device pointers passed with a ctx must live on the ctx's device. */
 int geo_create(geo_ctx **ctx, int metric, double M, double a);
 
 /* Integrate n geodesics for at most nsteps (< 2^31) RK4 steps of size h (h < 0 integrates backwards in tau).
@@ -104,8 +110,9 @@ int geo_integrate_host(geo_ctx *ctx, const double *state_in, int64_t n, double h
  * size per geodesic ("others method of the RK family will be included soon").
  *   err = max_c |e_c| / (atol + rtol max(|y_c|, |ynew_c|)) over the 6 evolving components; a step is accepted
  *   iff err <= 1; h <- h min(5, max(0.2, 0.9 err^(-1/5))) (not enlarged after a rejection).
- * h0 > 0: first trial step.  rtol = +INFINITY: fixed step h0 (no error test).  h_min: a rejected step that
- * would fall below it ends the particle with GEO_ST_NUMERIC.  tau_end: final value of the affine parameter,
+ * h0 > 0: first trial step.  rtol = +INFINITY: fixed step h0 (no error test; a non-finite
+ * attempt then ends the particle with GEO_ST_NUMERIC at once).  h_min: a rejected step that would fall below it -- or,
+ * with h_min = 0, a step that has shrunk to zero -- ends the particle with GEO_ST_NUMERIC.  tau_end: final value of the affine parameter,
  * landed on exactly ("the final evolution time is reached"; +INFINITY: none); reaching it, or
  * max_attempts (< 2^31, accepted + rejected), ends with GEO_ST_MAXSTEPS.  Capture / escape as in geo_stop
  * (capture guard on every stage point; flags must be 0).  out: as for geo_integrate, the snapshot fields are
@@ -151,16 +158,6 @@ void geo_destroy(geo_ctx *ctx);
 
 double geo_horizon_radius(const geo_ctx *ctx); /* r_+ = M + sqrt(M^2 - a^2) */
 const char *geo_last_error(const geo_ctx *ctx); /* text of the last error on this ctx ("" if none) */
-
-/* Launch geometry the next geo_integrate call on this ctx would use for (n, flags, snapshot_every):
- * grid and block size, registers per thread, resident CTAs per SM.  For measurement reports. */
-int geo_launch_info(geo_ctx *ctx, int64_t n, int32_t flags, int64_t snapshot_every, int32_t info[4]);
-
-/* Measurement helper: runs a register-only chain of dependent-free FP64 FMAs (`iters` x 64 DFMA per
- * thread over a full-chip grid) on `cuda_stream` and writes the number of FMAs executed to
- * *n_fma (host).  Times nothing itself: the caller brackets it with CUDA events.  `sink` is a device
- * buffer of >= 8 bytes that receives a value depending on every FMA. */
-int geo_probe_dfma(geo_ctx *ctx, int64_t iters, double *sink, double *n_fma, void *cuda_stream);
 
 #ifdef __cplusplus
 }

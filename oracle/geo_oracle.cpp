@@ -425,14 +425,18 @@ void integrate_one_adaptive(const Hole<R>& bh, const double* state_in, int64_t n
             }
         }
         if (fin && std::isinf(ctl.rtol)) err = R(0);                 // fixed-step mode: no error test
-        R fac = err > R(0) ? R(0.9) * std::pow(err, R(-0.2)) : R(5);
-        if (!(fac >= R(0.2))) fac = R(0.2);                          // also catches NaN
+        R fac = err > R(0) ? R(0.9) * std::pow(err, R(-0.2)) : (err == R(0) ? R(5) : R(0.2));   // NaN estimate: shrink
+        if (!(fac >= R(0.2))) fac = R(0.2);
         if (fac > R(5)) fac = R(5);
         if (std::isinf(ctl.rtol)) fac = R(1);                        // rtol = +inf: fixed step h0 (order tests)
         if (!fin || !(err <= R(1))) {                                // reject
             ++rejected;
             h *= std::min(fac, R(1));
-            if (!(std::fabs(h) >= (R)ctl.h_min)) { status = ORA_ST_NUMERIC; break; }
+            // reading A2: a rejected step below h_min ends with NUMERIC; so does a non-finite attempt in fixed-step
+            // mode (the same step would be retried forever) and a step size that has underflowed to zero
+            if ((std::isinf(ctl.rtol) && !fin) || !(std::fabs(h) >= (R)ctl.h_min) || !(std::fabs(h) > R(0))) {
+                status = ORA_ST_NUMERIC; break;
+            }
             if (attempts >= max_attempts) { status = ORA_ST_MAXSTEPS; break; }
             continue;
         }

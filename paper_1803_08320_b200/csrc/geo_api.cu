@@ -6,6 +6,7 @@
 #include <new>
 
 #include "../../include/geo.h"
+#include "../../include/geo_dev.h"
 #include "geo_kernel.cuh"
 #include "geo_rk45.cuh"
 #include "geo_tab.cuh"
@@ -57,6 +58,24 @@ int fail_cuda(geo_ctx* ctx, cudaError_t e, const char* what) {
     if (ctx) snprintf(ctx->err, sizeof ctx->err, "%s: %s", what, cudaGetErrorString(e));
     return e == cudaErrorMemoryAllocation ? GEO_ENOMEM : GEO_ECUDA;
 }
+
+// A ctx belongs to the device that was current at geo_create: its counters, scratch, tables and SM count are that
+// device's.  Every entry point runs with that device current and restores the caller's device on return.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+        else if (err == cudaSuccess) prev = -1;      // nothing to restore
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+#define GEO_ON_CTX_DEVICE(ctx)                                                         \
+    DeviceGuard device_guard_((ctx)->device);                                          \
+    if (device_guard_.err != cudaSuccess) return fail_cuda((ctx), device_guard_.err, "cudaSetDevice(ctx device)")
 
 bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
@@ -225,13 +244,13 @@ int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps
     p.health = out->health;
     p.snaps = out->snapshots;
     p.snap_count = out->snap_count;
+    p.coarse_steps = out->coarse_steps;
     p.counter = counter;
     p.bh.M = ctx->M;
     p.bh.a = ctx->a;
     p.bh.a2 = ctx->a * ctx->a;
     p.bh.twoM = 2.0 * ctx->M;
     p.bh.twoMa = 2.0 * ctx->M * ctx->a;
-    p.bh.twoa2 = 2.0 * ctx->a * ctx->a;
     fill_trig_consts(p.bh.tc);
     p.cartesian = (stop->flags & GEO_FLAG_CARTESIAN_SNAP) ? 1 : 0;
 
@@ -325,6 +344,7 @@ int geo_create_tabulated(geo_ctx** out_ctx, const geo_table* tb) {
 
 void geo_destroy(geo_ctx* ctx) {
     if (!ctx) return;
+    DeviceGuard guard(ctx->device);      // frees go to the ctx's device (best effort if the switch fails)
     if (ctx->tabA) cudaFree(ctx->tabA);
     if (ctx->tabB) cudaFree(ctx->tabB);
     for (int k = 0; k < 2; ++k)
@@ -345,6 +365,7 @@ int geo_integrate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int
                   const geo_stop* stop, int64_t snapshot_every, const geo_out* out, void* cuda_stream) {
     int rc = validate(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, true);
     if (rc != GEO_OK || n == 0) return rc;
+    GEO_ON_CTX_DEVICE(ctx);
     return launch(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, (cudaStream_t)cuda_stream, ctx->counter);
 }
 
@@ -356,13 +377,14 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
                        const geo_stop* stop, int64_t snapshot_every, const geo_out* out) {
     int rc = validate(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, false);
     if (rc != GEO_OK || n == 0) return rc;
+    GEO_ON_CTX_DEVICE(ctx);
     const size_t N = (size_t)n;
     const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
     const size_t snap_pp = snapshot_every > 0 ? (size_t)out->snap_capacity * ncomp * 8 : 0;   // bytes per particle
-    const size_t bytes_pp = 48 + 64 + 4 + 8 + (out->eq_cross_r ? 8 : 0) + (out->health ? 8 : 0) + snap_pp + (snap_pp ? 4 : 0);
+    const size_t bytes_pp = 48 + 64 + 4 + 8 + (out->eq_cross_r ? 8 : 0) + (out->health ? 8 : 0) + (out->coarse_steps ? 4 : 0) + snap_pp + (snap_pp ? 4 : 0);
     // chunking: only when the transfers are large, never below ~2 waves of resident lanes per chunk
     const size_t kHostChunkBytes = (size_t)768 << 20;
-    const size_t min_chunk = (size_t)ctx->sm_count * 5 * kBlock * 2;
+    const size_t min_chunk = (size_t)ctx->sm_count * GEO_MIN_CTAS_PER_SM * kBlock * 2;
     size_t nchunks = (N * bytes_pp + kHostChunkBytes - 1) / kHostChunkBytes;
     if (nchunks > N / min_chunk) nchunks = N / min_chunk;
     if (nchunks < 1) nchunks = 1;
@@ -372,8 +394,8 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
     const size_t b_in = align256(6 * C * 8), b_fin = align256(8 * C * 8), b_st = align256(C * 4),
                  b_steps = align256(C * 8), b_eq = out->eq_cross_r ? align256(C * 8) : 0,
                  b_he = out->health ? align256(C * 8) : 0, b_sn = align256(C * snap_pp),
-                 b_sc = snap_pp ? align256(C * 4) : 0;
-    const size_t slot_bytes = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_sn + b_sc;
+                 b_sc = snap_pp ? align256(C * 4) : 0, b_co = out->coarse_steps ? align256(C * 4) : 0;
+    const size_t slot_bytes = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_sn + b_sc + b_co;
     const size_t total = slot_bytes * nslots;
     cudaError_t e;
     for (int k = 0; k < nslots; ++k) {
@@ -390,6 +412,12 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
         if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMalloc(scratch)");
         ctx->scratch_bytes = total;
     }
+    // after the first enqueue every error path drains both streams before returning: no copy into the caller's
+    // buffers is left in flight behind a failed call
+    auto bail = [&](int code) {
+        for (int k = 0; k < nslots; ++k) cudaStreamSynchronize(ctx->host_stream[k]);
+        return code;
+    };
     for (size_t k = 0, lo = 0; lo < N; ++k, lo += C) {
         const size_t c = N - lo < C ? N - lo : C;
         const int slot = (int)(k % nslots);
@@ -406,17 +434,18 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
         d.health = (double*)take(b_he);
         d.snapshots = (double*)take(b_sn);
         d.snap_count = (int32_t*)take(b_sc);
+        d.coarse_steps = (int32_t*)take(b_co);
         e = cudaSuccess;
         for (int q = 0; q < 6 && e == cudaSuccess; ++q)      // SoA [6][n] -> [6][c]
             e = cudaMemcpyAsync(d_in + q * c, state_in + q * N + lo, c * 8, cudaMemcpyHostToDevice, s);
-        if (e != cudaSuccess) return fail_cuda(ctx, e, "H2D state_in");
+        if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "H2D state_in"));
         if (d.snapshots) {
             // slots >= snap_count[i] come back as NaN (all-ones pattern)
             e = cudaMemsetAsync(d.snapshots, 0xFF, c * snap_pp, s);
-            if (e != cudaSuccess) return fail_cuda(ctx, e, "memset snapshots");
+            if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "memset snapshots"));
         }
         rc = launch(ctx, d_in, (int64_t)c, h, nsteps, stop, snapshot_every, &d, s, ctx->counter + slot);
-        if (rc != GEO_OK) return rc;
+        if (rc != GEO_OK) return bail(rc);
         for (int q = 0; q < 8 && e == cudaSuccess; ++q)      // SoA [8][c] -> [8][n]
             e = cudaMemcpyAsync(out->final_state + q * N + lo, d.final_state + q * c, c * 8, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess) e = cudaMemcpyAsync(out->status + lo, d.status, c * 4, cudaMemcpyDeviceToHost, s);
@@ -426,7 +455,8 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
         if (e == cudaSuccess && d.snapshots)
             e = cudaMemcpyAsync(reinterpret_cast<char*>(out->snapshots) + lo * snap_pp, d.snapshots, c * snap_pp, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess && d.snap_count) e = cudaMemcpyAsync(out->snap_count + lo, d.snap_count, c * 4, cudaMemcpyDeviceToHost, s);
-        if (e != cudaSuccess) return fail_cuda(ctx, e, "D2H outputs");
+        if (e == cudaSuccess && d.coarse_steps) e = cudaMemcpyAsync(out->coarse_steps + lo, d.coarse_steps, c * 4, cudaMemcpyDeviceToHost, s);
+        if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "D2H outputs"));
     }
     for (int k = 0; k < nslots; ++k) {
         e = cudaStreamSynchronize(ctx->host_stream[k]);
@@ -435,10 +465,10 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
     return GEO_OK;
 }
 
-int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl,
-                           int64_t max_attempts, const geo_stop* stop, const geo_out* out, int32_t* rejected,
-                           void* cuda_stream) {
-    int rc = validate(ctx, state_in, n, 1.0, 0, stop, 0, out, true);
+// Argument checks of the adaptive entry points (device and host variants).
+static int validate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl, int64_t max_attempts,
+                             const geo_stop* stop, const geo_out* out, const int32_t* rejected, bool check_align) {
+    int rc = validate(ctx, state_in, n, 1.0, 0, stop, 0, out, check_align);
     if (rc != GEO_OK) return rc;
     if (ctx->metric == GEO_TABULATED) return fail(ctx, GEO_EINVAL, "the adaptive path takes analytic metrics only");
     if (!ctl) return fail(ctx, GEO_EINVAL, "ctl must not be NULL");
@@ -448,8 +478,13 @@ int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     if (!(ctl->h_min >= 0.0) || !(ctl->tau_end > 0.0)) return fail(ctx, GEO_EINVAL, "h_min >= 0 and tau_end > 0 required");
     if (max_attempts < 0 || max_attempts > 0x7fffffffLL) return fail(ctx, GEO_EINVAL, "max_attempts must be in [0, 2^31)");
     if (stop->flags != 0) return fail(ctx, GEO_EINVAL, "the adaptive path takes no flags");
-    if (misaligned(rejected)) return fail(ctx, GEO_EINVAL, "device pointers must be 16-byte aligned");
-    if (n == 0) return GEO_OK;
+    if (check_align && misaligned(rejected)) return fail(ctx, GEO_EINVAL, "device pointers must be 16-byte aligned");
+    return GEO_OK;
+}
+
+// Enqueue the RK5(4) kernel on validated arguments (device pointers); the ctx's device is current.
+static int launch_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl, int64_t max_attempts,
+                           const geo_stop* stop, const geo_out* out, int32_t* rejected, cudaStream_t stream) {
     AdaptiveParams p;
     memset(&p, 0, sizeof p);
     p.in = state_in;
@@ -476,7 +511,6 @@ int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     p.bh.a2 = ctx->a * ctx->a;
     p.bh.twoM = 2.0 * ctx->M;
     p.bh.twoMa = 2.0 * ctx->M * ctx->a;
-    p.bh.twoa2 = 2.0 * ctx->a * ctx->a;
     fill_trig_consts(p.bh.tc);
     typedef void (*fn_t)(const AdaptiveParams);
     fn_t fn = ctx->metric == GEO_KERR ? (fn_t)geo_rk45_kernel<true> : (fn_t)geo_rk45_kernel<false>;
@@ -486,7 +520,6 @@ int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
     const int64_t need = (n + kBlock - 1) / kBlock, resident = (int64_t)ctx->sm_count * per_sm;
     const int grid = (int)(need < resident ? need : resident);
-    cudaStream_t stream = (cudaStream_t)cuda_stream;
     e = cudaMemsetAsync(ctx->counter, 0, sizeof(unsigned long long), stream);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
     fn<<<grid, kBlock, 0, stream>>>(p);
@@ -495,15 +528,22 @@ int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     return GEO_OK;
 }
 
+int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl,
+                           int64_t max_attempts, const geo_stop* stop, const geo_out* out, int32_t* rejected,
+                           void* cuda_stream) {
+    int rc = validate_adaptive(ctx, state_in, n, ctl, max_attempts, stop, out, rejected, true);
+    if (rc != GEO_OK || n == 0) return rc;
+    GEO_ON_CTX_DEVICE(ctx);
+    return launch_adaptive(ctx, state_in, n, ctl, max_attempts, stop, out, rejected, (cudaStream_t)cuda_stream);
+}
+
 // Host-buffer entry point of the adaptive path: one H2D, one launch, one D2H per output, on the ctx's own stream.
+// Every argument is validated before the first copy is enqueued; after it, error paths drain the stream.
 int geo_integrate_adaptive_host(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl,
                                 int64_t max_attempts, const geo_stop* stop, const geo_out* out, int32_t* rejected) {
-    if (!ctx) return GEO_EINVAL;
-    ctx->err[0] = 0;
-    if (!stop || !out) return fail(ctx, GEO_EINVAL, "stop and out must not be NULL");
-    if (n < 0) return fail(ctx, GEO_EINVAL, "n must be >= 0");
-    if (n > 0 && (!state_in || !out->final_state || !out->status || !out->steps_done))
-        return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
+    int rc = validate_adaptive(ctx, state_in, n, ctl, max_attempts, stop, out, rejected, false);
+    if (rc != GEO_OK || n == 0) return rc;
+    GEO_ON_CTX_DEVICE(ctx);
     const size_t N = (size_t)n;
     const size_t b_in = align256(6 * N * 8), b_fin = align256(8 * N * 8), b_st = align256(N * 4), b_steps = align256(N * 8),
                  b_eq = out->eq_cross_r ? align256(N * 8) : 0, b_he = out->health ? align256(N * 8) : 0,
@@ -535,26 +575,31 @@ int geo_integrate_adaptive_host(geo_ctx* ctx, const double* state_in, int64_t n,
     d.health = (double*)take(b_he);
     d.snapshots = nullptr;
     d.snap_count = nullptr;
+    d.coarse_steps = nullptr;
     int32_t* d_rej = (int32_t*)take(b_rej);
-    if (n > 0) {
-        e = cudaMemcpyAsync(d_in, state_in, 6 * N * 8, cudaMemcpyHostToDevice, s);
-        if (e != cudaSuccess) return fail_cuda(ctx, e, "H2D state_in");
-    }
-    int rc = geo_integrate_adaptive(ctx, n > 0 ? d_in : state_in, n, ctl, max_attempts, stop, n > 0 ? &d : out, d_rej, s);
-    if (rc != GEO_OK || n == 0) return rc;
+    auto bail = [&](int code) {
+        cudaStreamSynchronize(s);
+        return code;
+    };
+    e = cudaMemcpyAsync(d_in, state_in, 6 * N * 8, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "H2D state_in"));
+    rc = launch_adaptive(ctx, d_in, n, ctl, max_attempts, stop, &d, d_rej, s);
+    if (rc != GEO_OK) return bail(rc);
     e = cudaMemcpyAsync(out->final_state, d.final_state, 8 * N * 8, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(out->status, d.status, N * 4, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(out->steps_done, d.steps_done, N * 8, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess && d.eq_cross_r) e = cudaMemcpyAsync(out->eq_cross_r, d.eq_cross_r, N * 8, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess && d.health) e = cudaMemcpyAsync(out->health, d.health, N * 8, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess && d_rej) e = cudaMemcpyAsync(rejected, d_rej, N * 4, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return fail_cuda(ctx, e, "D2H outputs");
+    if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "D2H outputs"));
+    e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
     return GEO_OK;
 }
 
 int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, int32_t info[4]) {
     if (!ctx || !info || n < 0) return GEO_EINVAL;
+    GEO_ON_CTX_DEVICE(ctx);
     if (ctx->metric == GEO_TABULATED) {
         info[1] = kTabBlock;
         return plan_tab(ctx, n, flags, &info[0], &info[3], &info[2]);
@@ -571,6 +616,7 @@ int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_eve
 
 int geo_probe_dfma(geo_ctx* ctx, int64_t iters, double* sink, double* n_fma, void* cuda_stream) {
     if (!ctx || !sink || !n_fma || iters < 1) return GEO_EINVAL;
+    GEO_ON_CTX_DEVICE(ctx);
     int per_sm = 0;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)dfma_probe_kernel, 256, 0);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(dfma_probe)");

@@ -6,8 +6,9 @@
 //   A4 stop rules    capture guard on every evaluation point, escape, step cap (B1-B6)
 //   A5 work queue    a lane whose geodesic ended takes the next particle index from a global atomic
 //                    counter (one warp-aggregated atomicAdd per refill round, ballot + shuffle)
-//   A6 snapshots     particle-major records, staged in shared memory and written with per-lane
-//                    bulk async copies (cp.async.bulk shared -> global), or stored directly
+//   A6 snapshots     particle-major records: each lane stores its record straight from registers with
+//                    256-bit stores (SNAP_DIRECT), or stages 4 records in shared memory that the whole
+//                    warp flushes with coalesced 8-byte stores (SNAP_STAGED)
 //   A7 final record
 // No arithmetic crosses lanes: a particle's result does not depend on which lane ran it.
 #pragma once
@@ -24,7 +25,7 @@ constexpr int kBlock = 128;
 #define GEO_MIN_CTAS_PER_SM 4
 #endif
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kStageSlots = 4;   // snapshot records staged per lane before a bulk store
+constexpr int kStageSlots = 4;   // snapshot records staged per lane before the warp flushes them
 
 enum { ST_MAXSTEPS = 0, ST_CAPTURED = 1, ST_ESCAPED = 2, ST_NUMERIC = 3 };
 enum { SNAP_NONE = 0, SNAP_DIRECT = 1, SNAP_STAGED = 2 };
@@ -48,6 +49,7 @@ struct Params {
     double* health;
     double* snaps;
     int* snap_count;
+    int* coarse_steps;  // optional diagnostic: step attempts evaluated by rk4_sum_full (geo_out.coarse_steps)
     unsigned long long* counter;
     Hole bh;
 };
@@ -243,6 +245,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         snaps = 0;
         staged = 0;
         crossed = false;
+        if (p.coarse_steps) p.coarse_steps[i] = 0;
         if (SNAP != SNAP_NONE) my_snaps = p.snaps + (size_t)i * (size_t)p.snap_cap * p.ncomp;
         // B1: tests on y0 before the first step
         if (!(r >= p.r_capture)) { finish(ST_CAPTURED); return; }
@@ -257,19 +260,6 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         if (i < p.n) begin(i);
     }
 
-#if defined(GEO_CONST_IN_REGS)
-    // experiment: keep sin/cos coefficients in vector registers (opaque to rematerialisation)
-    TrigConsts tcr = bh.tc;
-#if GEO_CONST_IN_REGS >= 2
-    asm volatile("" : "+d"(tcr.two_over_pi), "+d"(tcr.pio2_hi), "+d"(tcr.pio2_lo));
-    asm volatile("" : "+d"(tcr.s[2]), "+d"(tcr.s[3]), "+d"(tcr.s[4]), "+d"(tcr.s[5]));
-    asm volatile("" : "+d"(tcr.c[2]), "+d"(tcr.c[3]), "+d"(tcr.c[4]), "+d"(tcr.c[5]));
-#endif
-    asm volatile("" : "+d"(tcr.s[0]), "+d"(tcr.s[1]), "+d"(tcr.c[0]), "+d"(tcr.c[1]));
-#define GEO_TC tcr
-#else
-#define GEO_TC bh.tc
-#endif
 
     for (;;) {
         // --- A5: refill idle lanes from the queue ------------------------------------------------
@@ -304,7 +294,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         double at, ar, ath, aph, apr, apth;      // k1 + 2 k2 + 2 k3 + k4
         double sr, spr, spth;                    // stage point (t, phi are cyclic: not needed)
         double S, C, s2, sc, dang; bool coarse = false;              // sin/cos at the base point; sin^2, sin cos at the stage point
-        sincos_common_sign(GEO_TC, th, S, C);
+        sincos_common_sign(bh.tc, th, S, C);
         s2 = S * S; sc = S * C;
         rhs<KERR>(bh, r, s2, sc, pr, pth, E, L, k);
         at = k.t; ar = k.r; ath = k.th; aph = k.ph; apr = k.pr; apth = k.pth;
@@ -312,7 +302,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
         bool cap = !(sr >= p.r_capture);                                   // B2: stage point 2
 
-        stage_trig(GEO_TC, S, C, dang, s2, sc, coarse);
+        stage_trig(bh.tc, S, C, dang, s2, sc, coarse);
         rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
         at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
         aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
@@ -320,7 +310,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
         cap |= !(sr >= p.r_capture);                                       // stage point 3
 
-        stage_trig(GEO_TC, S, C, dang, s2, sc, coarse);
+        stage_trig(bh.tc, S, C, dang, s2, sc, coarse);
         rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
         at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
         aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
@@ -328,7 +318,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         spr = fma(p.h, k.pr, pr); spth = fma(p.h, k.pth, pth);
         cap |= !(sr >= p.r_capture);                                       // stage point 4
 
-        stage_trig(GEO_TC, S, C, dang, s2, sc, coarse);
+        stage_trig(bh.tc, S, C, dang, s2, sc, coarse);
         rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
         at += k.t; ar += k.r; ath += k.th; aph += k.ph; apr += k.pr; apth += k.pth;
         if (__builtin_expect(coarse && active(), 0)) {   // a stage angle moved by >= 2^-7 rad: full sin/cos path
@@ -336,6 +326,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
             double acc[6];
             int c;
             rk4_sum_full<KERR>(p, r, th, pr, pth, E, L, acc, &c);
+            if (p.coarse_steps) p.coarse_steps[idx] += 1;      // the lane owns its particle's slot
             at = acc[0]; ar = acc[1]; ath = acc[2]; aph = acc[3]; apr = acc[4]; apth = acc[5];
             cap = c != 0;
         }

@@ -33,10 +33,13 @@ struct TrigConsts {
 };
 
 struct Hole {
-    double M, a, a2, twoM, twoMa, twoa2;
+    double M, a, a2, twoM, twoMa;
     TrigConsts tc;
 };
 
+// The twelve polynomial coefficients and the two-piece pi/2 are those of fdlibm's __kernel_sin / __kernel_cos
+// (k_sin.c S1..S6, k_cos.c C1..C6; Sun Microsystems, freely distributable) and of its e_rem_pio2.c: a constant
+// table, restated; the evaluation code around them is this file's own.
 inline void fill_trig_consts(TrigConsts& t) {
     t.two_over_pi = 0.63661977236758134308;
     t.pio2_hi = 1.5707963267948966e+00;
@@ -46,7 +49,6 @@ inline void fill_trig_consts(TrigConsts& t) {
     const double c[6] = {4.16666666666666019037e-02, -1.38888888888741095749e-03, 2.48015872894767294178e-05,
                          -2.75573143513906633035e-07, 2.08757232129817482790e-09, -1.13596475577881948265e-11};
     for (int i = 0; i < 6; ++i) { t.s[i] = s[i]; t.c[i] = c[i]; }
-
 }
 
 // d/dtau of (t, r, theta, phi, p_r, p_theta)
@@ -68,8 +70,8 @@ __device__ __forceinline__ double rcp_nr(double x) {
 
 // x = k pi/2 + y: returns sn = sin y, cs = cos y, odd = k & 1.  Cody-Waite reduction by pi/2 in two
 // pieces (the first FMA is exact; |x| stays within a few pi on this path, so the neglected
-// k * 1.5e-33 is far below an ulp of y), minimax polynomials on [-pi/4, pi/4] (the classical
-// degree-13 / degree-14 kernels, < 1 ulp), branch-free.
+// k * 1.5e-33 is far below an ulp of y), minimax polynomials on [-pi/4, pi/4] (fdlibm's degree-13 /
+// degree-14 kernels, see fill_trig_consts; < 1 ulp), branch-free.
 __device__ __forceinline__ void sincos_reduced(const TrigConsts& tc, double x, double& sn, double& cs, bool& odd) {
     const double magic = 6755399441055744.0;   // 1.5 * 2^52: adding it rounds to the nearest integer
     double kd = fma(x, tc.two_over_pi, magic);  // (zero low word: an immediate operand)

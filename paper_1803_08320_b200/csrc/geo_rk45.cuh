@@ -236,8 +236,8 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
         ec = scaled_err(h * GEO_E(pr), fma(p.rtol, fmax(fabs(pr), fabs(npr)), p.atol));                     if (!(ec <= err)) err = ec;
         ec = scaled_err(h * GEO_E(pth), fma(p.rtol, fmax(fabs(pth), fabs(npth)), p.atol));                  if (!(ec <= err)) err = ec;
 #undef GEO_E
-        double fac = err > 0.0 ? 0.9 * inv_fifth_root(err) : 5.0;
-        if (!(fac >= 0.2)) fac = 0.2;                                            // also catches NaN
+        double fac = err > 0.0 ? 0.9 * inv_fifth_root(err) : (err == 0.0 ? 5.0 : 0.2);   // NaN estimate: shrink
+        if (!(fac >= 0.2)) fac = 0.2;
         if (fac > 5.0) fac = 5.0;
         if (p.fixed_step) { fac = 1.0; err = fin6 ? 0.0 : err; }
 
@@ -248,7 +248,9 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
             } else if (!fin6 || !(err <= 1.0)) {                                 // reject
                 ++rejected;
                 h *= fmin(fac, 1.0);
-                if (!(fabs(h) >= p.h_min)) finish(ST_NUMERIC);
+                // a non-finite attempt at a FIXED step can never succeed (same h, same NaN), and a step that has
+                // shrunk to zero cannot advance: both end the particle like a step below h_min (reading A2)
+                if ((p.fixed_step && !fin6) || !(fabs(h) >= p.h_min) || !(fabs(h) > 0.0)) finish(ST_NUMERIC);
                 else if (attempts >= p.max_attempts) finish(ST_MAXSTEPS);
             } else {
                 if (!crossed) {                                                  // B5

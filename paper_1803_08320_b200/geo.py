@@ -3,7 +3,8 @@
 Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
 and streams.  There is NO CPU fallback: if the library cannot be loaded, or there is no CUDA device,
 the calls raise.  Names follow the C ABI: ``geo_create``, ``geo_integrate``, ``geo_integrate_host``,
-``geo_create_tabulated``, ``geo_integrate_adaptive``, ``geo_destroy``, ``geo_horizon_radius``, ``geo_last_error``, ``geo_launch_info``, ``geo_probe_dfma``.
+``geo_create_tabulated``, ``geo_integrate_adaptive``, ``geo_integrate_adaptive_host``, ``geo_destroy``, ``geo_horizon_radius``,
+``geo_last_error``; plus the development helpers of include/geo_dev.h (``geo_launch_info``, ``geo_probe_dfma``) used by bench.py.
 """
 from __future__ import annotations
 
@@ -21,9 +22,10 @@ FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_STAGED_SNAP, FLAG_CARTESIAN_SNAP, FLAG_
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI
 
-# every symbol include/geo.h declares
+# every symbol include/geo.h declares, then the development helpers of include/geo_dev.h
 SYMBOLS = ("geo_create", "geo_create_tabulated", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_integrate_adaptive_host", "geo_destroy",
-           "geo_horizon_radius", "geo_last_error", "geo_launch_info", "geo_probe_dfma")
+           "geo_horizon_radius", "geo_last_error")
+DEV_SYMBOLS = ("geo_launch_info", "geo_probe_dfma")
 
 
 class GeoStop(C.Structure):
@@ -33,7 +35,8 @@ class GeoStop(C.Structure):
 class GeoOut(C.Structure):
     _fields_ = [("final_state", C.c_void_p), ("status", C.c_void_p), ("steps_done", C.c_void_p),
                 ("eq_cross_r", C.c_void_p), ("health", C.c_void_p), ("snapshots", C.c_void_p),
-                ("snap_capacity", C.c_int64), ("snap_mask", C.c_uint32), ("snap_count", C.c_void_p)]
+                ("snap_capacity", C.c_int64), ("snap_mask", C.c_uint32), ("snap_count", C.c_void_p),
+                ("coarse_steps", C.c_void_p)]
 
 
 class GeoAdaptive(C.Structure):
@@ -73,6 +76,12 @@ def lib() -> C.CDLL:
         L.geo_integrate_host.restype = C.c_int
         L.geo_integrate_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int64,
                                          C.POINTER(GeoStop), C.c_int64, C.POINTER(GeoOut)]
+        L.geo_integrate_adaptive.restype = C.c_int
+        L.geo_integrate_adaptive.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(GeoAdaptive), C.c_int64,
+                                             C.POINTER(GeoStop), C.POINTER(GeoOut), C.c_void_p, C.c_void_p]
+        L.geo_integrate_adaptive_host.restype = C.c_int
+        L.geo_integrate_adaptive_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(GeoAdaptive), C.c_int64,
+                                                  C.POINTER(GeoStop), C.POINTER(GeoOut), C.c_void_p]
         L.geo_destroy.restype = None
         L.geo_destroy.argtypes = [C.c_void_p]
         L.geo_horizon_radius.restype = C.c_double
@@ -137,7 +146,8 @@ def _ncomp(mask: int) -> int:
 
 
 def alloc_outputs(n: int, device, nsteps: int = 0, snapshot_every: int = 0, snap_capacity: int | None = None,
-                  snap_mask: int = 0xFF, want_eq_cross: bool = True, want_health: bool = True) -> dict:
+                  snap_mask: int = 0xFF, want_eq_cross: bool = True, want_health: bool = True,
+                  want_coarse: bool = False) -> dict:
     """Caller-owned device output tensors for geo_integrate (torch = device memory only)."""
     import torch
     out = {
@@ -147,6 +157,7 @@ def alloc_outputs(n: int, device, nsteps: int = 0, snapshot_every: int = 0, snap
         "eq_cross_r": torch.empty((n,), dtype=torch.float64, device=device) if want_eq_cross else None,
         "health": torch.empty((n,), dtype=torch.float64, device=device) if want_health else None,
         "snapshots": None, "snap_count": None, "snap_capacity": 0, "snap_mask": snap_mask,
+        "coarse_steps": torch.zeros((n,), dtype=torch.int32, device=device) if want_coarse else None,
     }
     if snapshot_every > 0:
         cap = snap_capacity if snap_capacity is not None else 1 + nsteps // snapshot_every
@@ -167,7 +178,42 @@ def _ptr(x):
 def _out_struct(out: dict) -> GeoOut:
     return GeoOut(_ptr(out["final_state"]), _ptr(out["status"]), _ptr(out["steps_done"]),
                   _ptr(out.get("eq_cross_r")), _ptr(out.get("health")), _ptr(out.get("snapshots")),
-                  int(out.get("snap_capacity") or 0), int(out.get("snap_mask", 0xFF)), _ptr(out.get("snap_count")))
+                  int(out.get("snap_capacity") or 0), int(out.get("snap_mask", 0xFF)), _ptr(out.get("snap_count")),
+                  _ptr(out.get("coarse_steps")))
+
+
+_OUT_DTYPES = {"final_state": "float64", "status": "int32", "steps_done": "int64", "eq_cross_r": "float64",
+               "health": "float64", "snapshots": "float64", "snap_count": "int32", "coarse_steps": "int32"}
+
+
+def _check_buffers(state_in, out: dict, device: bool, rejected=None) -> int:
+    """Shape / dtype / contiguity checks of the caller's buffers (the C ABI sees raw pointers only).  Returns n."""
+    def props(x):
+        if isinstance(x, np.ndarray):
+            return (not device), str(x.dtype), x.flags.c_contiguous, tuple(x.shape), x.size
+        return (x.is_cuda == device), str(x.dtype).replace("torch.", ""), x.is_contiguous(), tuple(x.shape), x.numel()
+    where = "CUDA" if device else "host (numpy / CPU tensor)"
+    ok, dt, cont, shape, _ = props(state_in)
+    if not (ok and dt == "float64" and cont and len(shape) == 2 and shape[0] == 6):
+        raise ValueError(f"state_in must be a contiguous {where} float64 array of shape [6][n]")
+    n = shape[1]
+    ncomp = _ncomp(int(out.get("snap_mask", 0xFF)))
+    need = {"final_state": 8 * n, "status": n, "steps_done": n, "eq_cross_r": n, "health": n, "snap_count": n,
+            "coarse_steps": n, "snapshots": n * int(out.get("snap_capacity") or 0) * ncomp}
+    for k, want in _OUT_DTYPES.items():
+        v = out.get(k)
+        if v is None:
+            if k in ("final_state", "status", "steps_done"):
+                raise ValueError(f"out['{k}'] is required")
+            continue
+        ok, dt, cont, _, size = props(v)
+        if not (ok and dt == want and cont and size >= need[k]):
+            raise ValueError(f"out['{k}'] must be a contiguous {where} {want} array with >= {need[k]} elements")
+    if rejected is not None:
+        ok, dt, cont, _, size = props(rejected)
+        if not (ok and dt == "int32" and cont and size >= n):
+            raise ValueError(f"rejected must be a contiguous {where} int32 array with >= {n} elements")
+    return n
 
 
 def geo_integrate(ctx, state_in, h: float, nsteps: int, out: dict, r_capture: float = -float("inf"),
@@ -176,10 +222,7 @@ def geo_integrate(ctx, state_in, h: float, nsteps: int, out: dict, r_capture: fl
     """Enqueue the integration of the geodesics in ``state_in`` (CUDA float64 tensor [6][n]) on
     ``stream`` (torch.cuda.Stream; default: the current stream).  Does not synchronise."""
     import torch
-    if not (state_in.is_cuda and state_in.dtype == torch.float64 and state_in.is_contiguous()
-            and state_in.dim() == 2 and state_in.shape[0] == 6):
-        raise ValueError("state_in must be a contiguous CUDA float64 tensor of shape [6][n]")
-    n = state_in.shape[1]
+    n = _check_buffers(state_in, out, device=True)
     s = stream if stream is not None else torch.cuda.current_stream(state_in.device)
     stop = GeoStop(r_capture, r_escape, kind, flags)
     o = _out_struct(out)
@@ -195,18 +238,12 @@ def geo_integrate_adaptive(ctx, state_in, h0: float, rtol: float, atol: float, m
     """Enqueue the adaptive RK5(4) integration (include/geo.h: geo_integrate_adaptive).  ``rejected``: optional
     CUDA int32 tensor [n].  Does not synchronise."""
     import torch
-    if not (state_in.is_cuda and state_in.dtype == torch.float64 and state_in.is_contiguous()
-            and state_in.dim() == 2 and state_in.shape[0] == 6):
-        raise ValueError("state_in must be a contiguous CUDA float64 tensor of shape [6][n]")
-    n = state_in.shape[1]
+    n = _check_buffers(state_in, out, device=True, rejected=rejected)
     s = stream if stream is not None else torch.cuda.current_stream(state_in.device)
     stop = GeoStop(r_capture, r_escape, kind, 0)
     ctl = GeoAdaptive(h0, rtol, atol, h_min, tau_end)
     o = _out_struct(out)
     L = lib()
-    L.geo_integrate_adaptive.restype = C.c_int
-    L.geo_integrate_adaptive.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(GeoAdaptive), C.c_int64,
-                                         C.POINTER(GeoStop), C.POINTER(GeoOut), C.c_void_p, C.c_void_p]
     with torch.cuda.device(state_in.device):
         rc = L.geo_integrate_adaptive(ctx, state_in.data_ptr(), n, C.byref(ctl), max_attempts, C.byref(stop),
                                       C.byref(o), _ptr(rejected), C.c_void_p(s.cuda_stream))
@@ -217,14 +254,11 @@ def geo_integrate_adaptive_host(ctx, state_in, h0: float, rtol: float, atol: flo
                                 r_capture: float = -float("inf"), r_escape: float = float("inf"), kind: int = TIMELIKE,
                                 h_min: float = 1e-12, tau_end: float = float("inf"), rejected=None) -> None:
     """The adaptive RK5(4) integration on HOST buffers (numpy arrays or pinned CPU tensors); synchronous."""
-    n = state_in.shape[1]
+    n = _check_buffers(state_in, out, device=False, rejected=rejected)
     stop = GeoStop(r_capture, r_escape, kind, 0)
     ctl = GeoAdaptive(h0, rtol, atol, h_min, tau_end)
     o = _out_struct(out)
     L = lib()
-    L.geo_integrate_adaptive_host.restype = C.c_int
-    L.geo_integrate_adaptive_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(GeoAdaptive), C.c_int64,
-                                              C.POINTER(GeoStop), C.POINTER(GeoOut), C.c_void_p]
     _check(ctx, L.geo_integrate_adaptive_host(ctx, _ptr(state_in), n, C.byref(ctl), max_attempts, C.byref(stop),
                                               C.byref(o), _ptr(rejected)))
 
@@ -233,7 +267,7 @@ def geo_integrate_host(ctx, state_in: np.ndarray, h: float, nsteps: int, out: di
                        r_capture: float = -float("inf"), r_escape: float = float("inf"),
                        kind: int = TIMELIKE, flags: int = 0, snapshot_every: int = 0) -> None:
     """Same operation on HOST buffers (numpy arrays or pinned CPU tensors); synchronous."""
-    n = state_in.shape[1]
+    n = _check_buffers(state_in, out, device=False)
     stop = GeoStop(r_capture, r_escape, kind, flags)
     o = _out_struct(out)
     rc = lib().geo_integrate_host(ctx, _ptr(state_in), n, h, nsteps, C.byref(stop), snapshot_every, C.byref(o))
@@ -242,7 +276,7 @@ def geo_integrate_host(ctx, state_in: np.ndarray, h: float, nsteps: int, out: di
 
 def alloc_outputs_host(n: int, nsteps: int = 0, snapshot_every: int = 0, snap_capacity: int | None = None,
                        snap_mask: int = 0xFF, want_eq_cross: bool = True, want_health: bool = True,
-                       pinned: bool = False) -> dict:
+                       pinned: bool = False, want_coarse: bool = False) -> dict:
     """Host output buffers for geo_integrate_host (numpy, or pinned torch CPU tensors)."""
     if pinned:
         import torch
@@ -265,6 +299,7 @@ def alloc_outputs_host(n: int, nsteps: int = 0, snapshot_every: int = 0, snap_ca
         "eq_cross_r": mk((n,), f64) if want_eq_cross else None,
         "health": mk((n,), f64) if want_health else None,
         "snapshots": None, "snap_count": None, "snap_capacity": 0, "snap_mask": snap_mask,
+        "coarse_steps": mk((n,), i32, 0) if want_coarse else None,
     }
     if snapshot_every > 0:
         cap = snap_capacity if snap_capacity is not None else 1 + nsteps // snapshot_every

@@ -7,8 +7,8 @@ import re
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared_symbols():
-    src = open(os.path.join(ROOT, "include", "geo.h")).read()
+def _declared_symbols(header="geo.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(geo_[a-z_0-9]+)\s*\(", src)))
 
@@ -23,12 +23,16 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
     for name in decl:
         assert hasattr(lib, name), name
     assert sorted(geo.SYMBOLS) == decl
+    dev = _declared_symbols("geo_dev.h")
+    for name in dev:
+        assert hasattr(lib, name), name
+    assert sorted(geo.DEV_SYMBOLS) == dev
 
 
 def test_struct_layouts_match_header():
     from paper_1803_08320_b200 import geo
     assert ctypes.sizeof(geo.GeoStop) == 24
-    assert ctypes.sizeof(geo.GeoOut) == 9 * 8
+    assert ctypes.sizeof(geo.GeoOut) == 10 * 8 and geo.GeoOut.coarse_steps.offset == 72
     assert geo.GeoOut.snap_mask.offset == 56 and geo.GeoOut.snap_count.offset == 64
     assert ctypes.sizeof(geo.GeoTable) == 56 and ctypes.sizeof(geo.GeoAdaptive) == 40
 

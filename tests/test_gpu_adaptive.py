@@ -149,3 +149,21 @@ def test_adaptive_host_entry_point_equals_the_device_one(G):
         assert np.array_equal(np.asarray(out[k]), g[k], equal_nan=True), k
     assert np.array_equal(rej, g["rejected"])
 
+
+
+def test_undefined_error_estimate_ends_with_numeric_not_after_max_attempts(G, oracle):
+    """Reading A2 (round 2, advisor finding): an attempt whose error estimate is NaN (atol = 0 on the exactly-zero phi
+    of a radial infall) is rejected with factor 0.2; the particle ends with NUMERIC once the step is below h_min, or has
+    shrunk to exactly zero with h_min = 0 -- after the same number of rejections as in the oracle, not after
+    max_attempts = 10^6 futile retries."""
+    st = np.zeros((6, 40))
+    st[0] = np.linspace(6.0, 30.0, 40)
+    st[1] = np.pi / 2
+    st[3] = -0.1
+    for h_min in (1e-12, 0.0):
+        kw = dict(h_min=h_min)
+        o = oracle.integrate_adaptive(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.1, 1e-9, 0.0, 10**6, **kw)
+        g = run_gpu_adaptive(G, G.SCHWARZSCHILD, 0.0, st, 0.1, 1e-9, 0.0, 10**6, **kw)
+        assert (o["status"] == oracle.ST_NUMERIC).all() and (g["status"] == G.ST_NUMERIC).all()
+        assert np.array_equal(g["rejected"], o["rejected"]) and (g["steps_done"] == 0).all()
+        assert np.array_equal(g["final_state"][1:4], st[0:3])

@@ -106,3 +106,17 @@ def test_adaptive_bound_orbits_conserve_the_constants(oracle):
     assert r["health"].max() < 1e-9
     Qf = f[6] ** 2 + np.cos(f[2]) ** 2 * (a * a * (1 - f[4] ** 2) + f[7] ** 2 / np.sin(f[2]) ** 2)
     assert np.abs(Qf - Q).max() < 1e-8 and f[0].min() > 100.0      # far fewer steps than h = 0.01 would need
+
+
+def test_undefined_error_estimate_shrinks_the_step_and_ends_with_numeric(oracle):
+    """Reading A2 (round 2): radial infall in Schwarzschild with L = 0 keeps phi exactly 0, so with atol = 0 the scaled
+    error of phi is 0/0 on every attempt.  The attempt is rejected with factor 0.2 until the step falls below h_min
+    (NUMERIC) -- it must not be retried unchanged until max_attempts.  With h_min = 0 the step shrinks to exactly zero
+    and the particle ends the same way."""
+    st = np.array([[8.0], [np.pi / 2], [0.0], [-0.1], [0.0], [0.0]])
+    r = oracle.integrate_adaptive(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.1, 1e-9, 0.0, 10**6, h_min=1e-12)
+    assert r["status"][0] == oracle.ST_NUMERIC and r["steps_done"][0] == 0
+    assert r["rejected"][0] == 16               # 0.1 * 0.2^16 = 6.6e-13 < 1e-12 <= 0.1 * 0.2^15
+    r0 = oracle.integrate_adaptive(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.1, 1e-9, 0.0, 10**6, h_min=0.0)
+    assert r0["status"][0] == oracle.ST_NUMERIC and 400 < r0["rejected"][0] < 500      # 0.2^k underflows to 0 near k = 463
+    np.testing.assert_array_equal(r0["final_state"][1:4, 0], st[0:3, 0])               # final = y0, untouched

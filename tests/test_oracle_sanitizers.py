@@ -1,0 +1,65 @@
+"""The oracle under AddressSanitizer + UndefinedBehaviorSanitizer (round-1 verdict item 5).
+
+compute-sanitizer is closed on the GPU pool, so the CUDA path carries guard-band tests; the CPU half of that plan costs
+nothing here: oracle/build.py --sanitize compiles the same sources with -fsanitize=address,undefined and a child process
+(libasan preloaded) drives every entry point over the cases with the most address arithmetic -- ragged batches,
+snapshot capacity overflow, odd component masks, Cartesian records, early termination, the adaptive path, the tabulated
+metric incl. domain exits, multi-threaded outer loops.  Any report makes the child exit non-zero.
+"""
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+CHILD = r"""
+import math, os, sys
+import numpy as np
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "oracle"))
+import geo_oracle as O, geo_tab_oracle as T
+from paper_1803_08320_b200 import workloads as W
+assert O.lib()._name.endswith("libgeo_oracle_san.so"), O.lib()._name
+st = W.kerr_bound(67, 0.9, W.SEED_BASE + 2)
+for mask, cap, flags in ((0xFF, None, 0), (0x07, 3, 0), (0x0F, 2, O.FLAG_CARTESIAN_SNAP), (0xA5, 50, O.FLAG_PLAIN_UPDATE)):
+    for ld in (False, True):
+        r = O.integrate(O.KERR, 1.0, 0.9, st, 0.01, 137, snapshot_every=7, snap_capacity=cap, snap_mask=mask, flags=flags,
+                        long_double=ld, nthreads=3)
+        assert (r["steps_done"] == 137).all() and (r["snap_count"] == 1 + 137 // 7).all()
+a = 0.998
+rays = np.ascontiguousarray(W.camera_rays(64, a, 60.0)[:, ::41])
+rc = W.horizon_radius(1.0, a) + 0.01
+r = O.integrate(O.KERR, 1.0, a, rays, 0.02, 200000, r_capture=rc, r_escape=1100.0, kind=O.NULL, snapshot_every=500,
+                snap_mask=0x0F, nthreads=4)
+assert set(np.unique(r["status"])) <= {O.ST_CAPTURED, O.ST_ESCAPED}
+bad = st.copy(); bad[0, 0] = 1.0; bad[3, 1] = np.nan; bad[0, 2] = 1e6
+r = O.integrate(O.KERR, 1.0, 0.9, bad, 0.01, 10, r_capture=1.5, r_escape=100.0, snapshot_every=1, want_eq_cross=False, want_health=False)
+assert r["status"][0] == O.ST_CAPTURED and r["status"][1] == O.ST_NUMERIC and r["status"][2] == O.ST_ESCAPED
+r = O.integrate(O.SCHWARZSCHILD, 1.0, 0.0, W.circular_schwarzschild(5), -0.01, 0)
+ra = O.integrate_adaptive(O.KERR, 1.0, a, rays, 0.02, 1e-9, 1e-9, 200000, r_capture=rc, r_escape=1100.0, kind=O.NULL, nthreads=4)
+ra = O.integrate_adaptive(O.KERR, 1.0, 0.9, st, 0.05, np.inf, 1.0, 50, tau_end=1.3, long_double=True)
+rad = np.array([[8.0], [np.pi / 2], [0.0], [-0.1], [0.0], [0.0]])
+ra = O.integrate_adaptive(O.SCHWARZSCHILD, 1.0, 0.0, rad, 0.1, 1e-9, 0.0, 10**6, h_min=0.0)
+assert ra["status"][0] == O.ST_NUMERIC
+O.dp45_tableau(); O.rhs(O.KERR, 1.0, 0.9, [0, 6.0, 1.0, 0, 0.95, 0.1, 0.2, 3.0], long_double=True)
+O.hamiltonian(1.0, 0.9, [0, 6.0, 1.0, 0, 0.95, 0.1, 0.2, 3.0]); O.energy(1.0, 0.9, 6.0, 1.0, 0.1, 0.2, 3.0, 1.0)
+tb = W.kerr_metric_table(1.0, 0.9, 65, 33, 1.8, 40.0, 0.2, math.pi - 0.2)
+rt = T.integrate(tb, st, 0.01, 200, nthreads=3)
+out = st.copy(); out[0] = 39.9; out[3] = 2.0      # runs off the table
+rt = T.integrate(tb, out, 0.05, 400, long_double=True)
+assert (rt["status"] == T.ST_OUTSIDE).any()
+assert T.fields(tb, 1e9, 1.0) is None and T.fields(tb, 5.0, 1.0) is not None and T.rhs(tb, [0, 5.0, 1.0, 0, 0.95, 0.1, 0.2, 3.0]) is not None
+print("sanitized oracle run ok")
+"""
+
+
+def test_oracle_runs_clean_under_asan_and_ubsan():
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import build as oracle_build
+    oracle_build.build(sanitize=True)
+    env = dict(os.environ, GEO_ORACLE_SANITIZE="1", LD_PRELOAD=oracle_build.sanitizer_runtime(),
+               ASAN_OPTIONS="detect_leaks=0:abort_on_error=0:halt_on_error=1", UBSAN_OPTIONS="print_stacktrace=1:halt_on_error=1")
+    p = subprocess.run([sys.executable, "-c", "ROOT = %r\n" % ROOT + CHILD], env=env, capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-4000:]
+    assert "sanitized oracle run ok" in p.stdout
+    assert "AddressSanitizer" not in p.stderr and "runtime error" not in p.stderr, p.stderr[-4000:]

@@ -93,6 +93,16 @@ def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dic
         return dict(name="snapshot microbenchmark: Schwarzschild circular, snapshot every step, 8 comps", metric="schwarzschild", a=0.0,
                     st=W.circular_schwarzschild(n, W.SEED_BASE + 6 + 1000 * rank), h=0.01, nsteps=256, snapshot_every=1,
                     snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf)
+    if name in ("snapkerr", "snapkerr_xyz"):
+        # round-1 verdict, kernel item 9: the paper's own output mode (a record EVERY step) on the Kerr
+        # kernel at a size that fills the machine: the configs[3] particles, 256 steps, all 8 BL components (snapkerr,
+        # 69 GB) or the paper's (t, x, y, z) record of eq.(7) (snapkerr_xyz, 34 GB)
+        n = n_override or (1 << 22)
+        st = W.kerr_bound(n, 0.5, W.SEED_BASE + 4 + 1000 * rank, nthreads=nthreads, chunk=1 << 20)
+        xyz = name == "snapkerr_xyz"
+        return dict(name="Kerr a=0.5 bound particles, a record every step: " + ("(t, x, y, z) of eq.(7)" if xyz else "8 BL components"),
+                    metric="kerr", a=0.5, st=st, h=0.01, nsteps=256, snapshot_every=1, snap_mask=0x0F if xyz else 0xFF, kind=0,
+                    r_capture=-np.inf, r_escape=np.inf, flags=8 if xyz else 0)
     if name == "config3s":
         # configs[2] with the pixels in a seeded random order: every warp holds a captured/escaped mix
         wl = workload("config3", rank, n_override, nthreads)
@@ -241,7 +251,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "config3a", "tab4", "snapbench", "paper_t3", "paper_t4"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config3s", "config3a", "tab4", "snapbench", "snapkerr", "snapkerr_xyz", "paper_t3", "paper_t4"])
     ap.add_argument("--n", type=int, default=None, help="override particle count / image size (development)")
     ap.add_argument("--flags", type=int, default=0, help="GEO_FLAG_* bits (2 = static mapping, 4 = shared-memory-staged snapshots, 16 = tabulated metric: gather instead of the stencil cache)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

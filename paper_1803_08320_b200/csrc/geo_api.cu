@@ -127,10 +127,11 @@ struct LaunchPlan {
 };
 
 int plan_launch(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, int ncomp, LaunchPlan* lp) {
-    // Sparse snapshots go through the staged writer: the direct writer's inlined record logic costs the stepping loop
-    // registers (hot-loop spills in the Kerr instantiation: config 2, one record per 1000 steps, ran at 319 ms against
-    // 188 ms staged and 179 ms without snapshots); dense output (every step or so) keeps the 256-bit direct stores.
-    const bool staged = (flags & GEO_FLAG_STAGED_SNAP) || snapshot_every >= 16;
+    // The direct writer (256-bit stores from registers) is the default at every cadence: since round 2 the record logic
+    // sits behind the stepping loop's single rare-event branch and no longer costs the accepted step any registers
+    // (round 1 routed snapshot_every >= 16 through the staged writer because the inlined record code made the Kerr
+    // stepping loop spill: config 2 ran 319 ms direct / 188 ms staged; now 173 / 176 ms).
+    const bool staged = (flags & GEO_FLAG_STAGED_SNAP) != 0;
     lp->snap_mode = snapshot_every > 0 ? (staged ? SNAP_STAGED : SNAP_DIRECT) : SNAP_NONE;
     lp->fn = pick_kernel(ctx->metric, lp->snap_mode, (flags & GEO_FLAG_PLAIN_UPDATE) != 0);
     lp->smem = lp->snap_mode == SNAP_STAGED ? (size_t)kBlock * stage_stride(ncomp) * sizeof(double) : 0;

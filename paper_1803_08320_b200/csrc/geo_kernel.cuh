@@ -17,7 +17,10 @@
 
 namespace geo {
 
-constexpr int kBlock = 128;
+#ifndef GEO_BLOCK
+#define GEO_BLOCK 128
+#endif
+constexpr int kBlock = GEO_BLOCK;
 // Resident CTAs per SM the register allocation is bounded for: 4 CTAs x 128 threads = 16 warps/SM at
 // <= 128 registers.  The kernel is bound by issue slots (2 per FP64 instruction + 1 per other), not by
 // latency, so a fifth CTA at <= 96 registers only adds spill instructions (measured -8 %).
@@ -25,6 +28,8 @@ constexpr int kBlock = 128;
 #define GEO_MIN_CTAS_PER_SM 4
 #endif
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kHalfPiHi = 0x3ff921fb;          // high word of the double nearest to pi/2
+constexpr unsigned kCoarseHi = 0x3f100000u;   // high word of 2^-14: (stage angle increment)^2 at the angle-addition limit
 constexpr int kStageSlots = 4;   // snapshot records staged per lane before the warp flushes them
 
 enum { ST_MAXSTEPS = 0, ST_CAPTURED = 1, ST_ESCAPED = 2, ST_NUMERIC = 3 };
@@ -147,19 +152,36 @@ __device__ __noinline__ void rk4_sum_full(const Params& p, double r, double th, 
     *captured = cap ? 1 : 0;
 }
 
+// Evolving components of a geodesic (t, phi cyclic) and, in LaneState, their Kahan error terms.
+struct Lane6 {
+    double t, r, th, ph, pr, pth;
+};
+struct LaneState {
+    Lane6 y, c;
+};
+
+#ifdef GEO_MAXNREG
+#define GEO_RK4_BOUNDS __maxnreg__(GEO_MAXNREG)
+#else
+#define GEO_RK4_BOUNDS __launch_bounds__(kBlock, SNAP == SNAP_NONE ? GEO_MIN_CTAS_PER_SM : 4)
+#endif
 template <bool KERR, int SNAP, bool PLAIN>
-__global__ void __launch_bounds__(kBlock, SNAP == SNAP_NONE ? GEO_MIN_CTAS_PER_SM : 4)
+__global__ void GEO_RK4_BOUNDS
 geo_rk4_kernel(const __grid_constant__ Params p) {
     extern __shared__ __align__(16) double stage_smem[];   // SNAP_STAGED: [kBlock][stage_stride(ncomp)]
     const unsigned lane = threadIdx.x & 31u;
     const Hole& bh = p.bh;
+    const double half_pi = 1.5707963267948966;
 
-    // lane state (registers)
+    // lane state (registers).  The state is double-buffered: a step reads one LaneState and writes the other, so an
+    // accepted step costs no register moves and the state before the step is still there for the events that need it
+    // (capture / non-finite: final record = last accepted state).
+    LaneState A, B;
+    A.y = Lane6{0, 0, 0, 0, 0, 0}; A.c = A.y; B = A;
+    double E = 0, L = 0;
     long long idx = -1;                   // particle this lane integrates; < 0: the lane is idle
     auto active = [&]() { return idx >= 0; };
     bool exhausted = !p.use_queue;
-    double t = 0, r = 0, th = 0, ph = 0, pr = 0, pth = 0, E = 0, L = 0;
-    double ct = 0, cr = 0, cth = 0, cph = 0, cpr = 0, cpth = 0;
     int steps = 0, snap_ctr = 0;
     int snaps = 0, staged = 0, stage_first = 0;   // staged records hold slots [stage_first, stage_first+staged)
     bool crossed = false;
@@ -195,51 +217,52 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         __syncwarp();
         staged = 0;
     };
-    auto emit_snapshot = [&]() {
+    auto emit_snapshot = [&](const Lane6& y) {
         if (snaps < p.snap_cap) {   // S3: drop beyond capacity, keep counting
-            double c1 = r, c2 = th, c3 = ph;
-            if (p.cartesian) cartesian_eq7(bh.a2, r, th, ph, c1, c2, c3);
+            double c1 = y.r, c2 = y.th, c3 = y.ph;
+            if (p.cartesian) cartesian_eq7(bh.tc, bh.a2, y.r, y.th, y.ph, c1, c2, c3);
             if (SNAP == SNAP_DIRECT) {
-                store_record_global(my_snaps + (size_t)snaps * p.ncomp, p.snap_mask, t, c1, c2, c3, E, pr, pth, L);
+                store_record_global(my_snaps + (size_t)snaps * p.ncomp, p.snap_mask, y.t, c1, c2, c3, E, y.pr, y.pth, L);
             } else {
                 if (staged == 0) stage_first = snaps;
-                store_masked(my_stage + staged * p.ncomp, p.snap_mask, t, c1, c2, c3, E, pr, pth, L);
+                store_masked(my_stage + staged * p.ncomp, p.snap_mask, y.t, c1, c2, c3, E, y.pr, y.pth, L);
                 ++staged;           // flushed by the warp at the top of the loop, or by finish()
             }
         }
         ++snaps;
     };
-    auto finish = [&](int st) {
+    auto finish = [&](int st, const Lane6& y, int nsteps_done) {
         if (SNAP == SNAP_STAGED) flush_stage();
         long long n = p.n;
         asm volatile("" : "+l"(n));   // opaque: keeps the record's address arithmetic inside this cold path
-        p.fin[0 * n + idx] = t;
-        p.fin[1 * n + idx] = r;
-        p.fin[2 * n + idx] = th;
-        p.fin[3 * n + idx] = ph;
+        p.fin[0 * n + idx] = y.t;
+        p.fin[1 * n + idx] = y.r;
+        p.fin[2 * n + idx] = y.th;
+        p.fin[3 * n + idx] = y.ph;
         p.fin[4 * n + idx] = E;
-        p.fin[5 * n + idx] = pr;
-        p.fin[6 * n + idx] = pth;
+        p.fin[5 * n + idx] = y.pr;
+        p.fin[6 * n + idx] = y.pth;
         p.fin[7 * n + idx] = L;
         p.status[idx] = st;
-        p.steps_done[idx] = (long long)steps;
+        p.steps_done[idx] = (long long)nsteps_done;
         if (p.eq_cross_r && !crossed) p.eq_cross_r[idx] = __longlong_as_double(0x7ff8000000000000LL);
-        if (p.health) p.health[idx] = health_3p1(bh, r, th, pr, pth, E, L, p.kappa);
+        if (p.health) p.health[idx] = health_3p1(bh, y.r, y.th, y.pr, y.pth, E, L, p.kappa);
         if (SNAP != SNAP_NONE) p.snap_count[idx] = snaps;
         idx = -1;
     };
-    auto begin = [&](long long i) {
+    auto begin = [&](long long i) {      // loads into A: the current state at the top of the loop
         idx = i;
         const long long n = p.n;
-        t = 0.0;
-        r = p.in[0 * n + i];
-        th = p.in[1 * n + i];
-        ph = p.in[2 * n + i];
-        pr = p.in[3 * n + i];
-        pth = p.in[4 * n + i];
+        Lane6& y = A.y;
+        y.t = 0.0;
+        y.r = p.in[0 * n + i];
+        y.th = p.in[1 * n + i];
+        y.ph = p.in[2 * n + i];
+        y.pr = p.in[3 * n + i];
+        y.pth = p.in[4 * n + i];
         L = p.in[5 * n + i];
-        E = energy_3p1(bh, r, th, pr, pth, L, p.kappa);
-        ct = cr = cth = cph = cpr = cpth = 0.0;
+        E = energy_3p1(bh, y.r, y.th, y.pr, y.pth, L, p.kappa);
+        A.c = Lane6{0, 0, 0, 0, 0, 0};
         steps = 0;
         snap_ctr = p.snap_every;
         snaps = 0;
@@ -248,11 +271,100 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         if (p.coarse_steps) p.coarse_steps[i] = 0;
         if (SNAP != SNAP_NONE) my_snaps = p.snaps + (size_t)i * (size_t)p.snap_cap * p.ncomp;
         // B1: tests on y0 before the first step
-        if (!(r >= p.r_capture)) { finish(ST_CAPTURED); return; }
-        if (!all_finite6(r, th, ph, pr, pth, E)) { finish(ST_NUMERIC); return; }
-        if (SNAP != SNAP_NONE) emit_snapshot();   // S1: slot 0 = y0
-        if (r > p.r_escape) { finish(ST_ESCAPED); return; }
-        if (p.nsteps == 0) { finish(ST_MAXSTEPS); return; }
+        if (!(y.r >= p.r_capture)) { finish(ST_CAPTURED, y, 0); return; }
+        if (!all_finite6(y.r, y.th, y.ph, y.pr, y.pth, E)) { finish(ST_NUMERIC, y, 0); return; }
+        if (SNAP != SNAP_NONE) emit_snapshot(y);   // S1: slot 0 = y0
+        if (y.r > p.r_escape) { finish(ST_ESCAPED, y, 0); return; }
+        if (p.nsteps == 0) { finish(ST_MAXSTEPS, y, 0); return; }
+    };
+
+    // --- A3 + A4: one classical RK4 step cur -> nxt for every lane (idle lanes compute on stale state), then
+    // the stop rules and events.  Everything that is not "accept and go on" -- capture, non-finite, a possible
+    // equatorial crossing, a due snapshot, escape, the step cap -- is folded into ONE flag and handled behind
+    // ONE branch, so the accepted step is straight-line code.
+    auto step = [&](const LaneState& cur, LaneState& nxt) {
+        const double r = cur.y.r, th = cur.y.th, pr = cur.y.pr, pth = cur.y.pth;
+        Deriv k;
+        double at, ar, ath, aph, apr, apth;      // k1 + 2 k2 + 2 k3 + k4
+        double sr, spr, spth;                    // stage point (t, phi are cyclic: not needed)
+        double S, C, s2, sc, dang;               // sin/cos at the base point; sin^2, sin cos at the stage point
+        unsigned dmax = 0;                       // largest high word of the squared stage-angle increments
+        sincos_common_sign(bh.tc, th, S, C);
+        s2 = S * S; sc = S * C;
+        rhs<KERR>(bh, r, s2, sc, pr, pth, E, L, k);
+        at = k.t; ar = k.r; ath = k.th; aph = k.ph; apr = k.pr; apth = k.pth;
+        sr = fma(p.h_half, k.r, r); dang = p.h_half * k.th;
+        spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
+        bool cap = !(sr >= p.r_capture);                                   // B2: stage point 2
+
+        stage_trig(bh.tc, S, C, dang, s2, sc, dmax);
+        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
+        at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
+        aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
+        sr = fma(p.h_half, k.r, r); dang = p.h_half * k.th;
+        spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
+        cap |= !(sr >= p.r_capture);                                       // stage point 3
+
+        stage_trig(bh.tc, S, C, dang, s2, sc, dmax);
+        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
+        at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
+        aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
+        sr = fma(p.h, k.r, r); dang = p.h * k.th;
+        spr = fma(p.h, k.pr, pr); spth = fma(p.h, k.pth, pth);
+        cap |= !(sr >= p.r_capture);                                       // stage point 4
+
+        stage_trig(bh.tc, S, C, dang, s2, sc, dmax);
+        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
+        at += k.t; ar += k.r; ath += k.th; aph += k.ph; apr += k.pr; apth += k.pth;
+        if (__builtin_expect(dmax >= kCoarseHi && active(), 0)) {   // a stage angle moved by >= 2^-7 rad: full sin/cos path
+            // (idle lanes step on stale state -- often a captured ray next to the horizon -- and must not drag the warp here)
+            double acc[6];
+            int c;
+            rk4_sum_full<KERR>(p, r, th, pr, pth, E, L, acc, &c);
+            if (p.coarse_steps) p.coarse_steps[idx] += 1;      // the lane owns its particle's slot
+            at = acc[0]; ar = acc[1]; ath = acc[2]; aph = acc[3]; apr = acc[4]; apth = acc[5];
+            cap = c != 0;
+        }
+
+        kahan<PLAIN>(cur.y.t, cur.c.t, p.h_sixth, at, nxt.y.t, nxt.c.t);
+        kahan<PLAIN>(r, cur.c.r, p.h_sixth, ar, nxt.y.r, nxt.c.r);
+        kahan<PLAIN>(th, cur.c.th, p.h_sixth, ath, nxt.y.th, nxt.c.th);
+        kahan<PLAIN>(cur.y.ph, cur.c.ph, p.h_sixth, aph, nxt.y.ph, nxt.c.ph);
+        kahan<PLAIN>(pr, cur.c.pr, p.h_sixth, apr, nxt.y.pr, nxt.c.pr);
+        kahan<PLAIN>(pth, cur.c.pth, p.h_sixth, apth, nxt.y.pth, nxt.c.pth);
+        cap |= !(nxt.y.r >= p.r_capture);                                  // end point
+        const bool fin6 = all_finite6(nxt.y.t, nxt.y.r, nxt.y.th, nxt.y.ph, nxt.y.pr, nxt.y.pth);
+        // B5 candidate on the integer pipe: theta and the new theta do not lie strictly on the same side of pi/2 as far
+        // as their HIGH words can tell (negative angles have a negative high word: "below"; an angle within 2^-20 of
+        // pi/2 shares its high word: "maybe").  The exact test d0 d1 < 0 runs behind the branch.
+        const int hi0 = __double2hiint(th), hi1 = __double2hiint(nxt.y.th);
+        const bool maybe_crossing = (min(hi0, hi1) <= kHalfPiHi) & (max(hi0, hi1) >= kHalfPiHi);
+        const int ns = steps + 1;
+        bool rare = cap | !fin6 | maybe_crossing | (nxt.y.r > p.r_escape) | (ns >= p.nsteps);
+        if (SNAP != SNAP_NONE) rare |= (--snap_ctr == 0);
+        steps = ns;
+
+        // --- A4: stop rules and events (rare) -----------------------------------------------------
+        if (__builtin_expect(rare && active(), 0)) {
+            if (cap) {
+                finish(ST_CAPTURED, cur.y, ns - 1);     // step not taken: final = last accepted state
+            } else if (!fin6) {
+                finish(ST_NUMERIC, cur.y, ns - 1);      // B6
+            } else {
+                if (!crossed) {                         // B5 (the flag only says the sign of theta - pi/2 may have changed)
+                    const double d0 = th - half_pi, d1 = nxt.y.th - half_pi;
+                    if (d0 * d1 < 0.0) {
+                        crossed = true;   // the radius goes straight to its slot (once per particle): no register held for it
+                        if (p.eq_cross_r) p.eq_cross_r[idx] = r + (nxt.y.r - r) * (half_pi - th) / (nxt.y.th - th);
+                    }
+                }
+                if (SNAP != SNAP_NONE) {
+                    if (snap_ctr == 0) { snap_ctr = p.snap_every; emit_snapshot(nxt.y); }   // S1
+                }
+                if (nxt.y.r > p.r_escape) finish(ST_ESCAPED, nxt.y, ns);        // B3
+                else if (ns >= p.nsteps) finish(ST_MAXSTEPS, nxt.y, ns);       // B4
+            }
+        }
     };
 
     if (!p.use_queue) {
@@ -260,9 +372,8 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
         if (i < p.n) begin(i);
     }
 
-
     for (;;) {
-        // --- A5: refill idle lanes from the queue ------------------------------------------------
+        // --- A5: refill idle lanes from the queue (every second step: the loop body holds two steps) ----
         unsigned idle = __ballot_sync(kFull, !active());
         if (idle) {
             if (!exhausted) {
@@ -283,89 +394,14 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
             }
         }
 
-        // --- A6: a full stage anywhere in the warp -> everyone flushes (at most one record is staged
-        // per lane between two visits here, so a slab never overflows)
+        // --- A6: a stage that the next two steps could overflow anywhere in the warp -> everyone flushes
+        // (at most one record is staged per lane and step)
         if (SNAP == SNAP_STAGED) {
-            if (__any_sync(kFull, staged == kStageSlots)) flush_stage_warp();
+            if (__any_sync(kFull, staged >= kStageSlots - 1)) flush_stage_warp();
         }
 
-        // --- A3: one classical RK4 step, every lane (idle lanes compute on stale state) ----------
-        Deriv k;
-        double at, ar, ath, aph, apr, apth;      // k1 + 2 k2 + 2 k3 + k4
-        double sr, spr, spth;                    // stage point (t, phi are cyclic: not needed)
-        double S, C, s2, sc, dang; bool coarse = false;              // sin/cos at the base point; sin^2, sin cos at the stage point
-        sincos_common_sign(bh.tc, th, S, C);
-        s2 = S * S; sc = S * C;
-        rhs<KERR>(bh, r, s2, sc, pr, pth, E, L, k);
-        at = k.t; ar = k.r; ath = k.th; aph = k.ph; apr = k.pr; apth = k.pth;
-        sr = fma(p.h_half, k.r, r); dang = p.h_half * k.th;
-        spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
-        bool cap = !(sr >= p.r_capture);                                   // B2: stage point 2
-
-        stage_trig(bh.tc, S, C, dang, s2, sc, coarse);
-        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
-        at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
-        aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
-        sr = fma(p.h_half, k.r, r); dang = p.h_half * k.th;
-        spr = fma(p.h_half, k.pr, pr); spth = fma(p.h_half, k.pth, pth);
-        cap |= !(sr >= p.r_capture);                                       // stage point 3
-
-        stage_trig(bh.tc, S, C, dang, s2, sc, coarse);
-        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
-        at = fma(2.0, k.t, at); ar = fma(2.0, k.r, ar); ath = fma(2.0, k.th, ath);
-        aph = fma(2.0, k.ph, aph); apr = fma(2.0, k.pr, apr); apth = fma(2.0, k.pth, apth);
-        sr = fma(p.h, k.r, r); dang = p.h * k.th;
-        spr = fma(p.h, k.pr, pr); spth = fma(p.h, k.pth, pth);
-        cap |= !(sr >= p.r_capture);                                       // stage point 4
-
-        stage_trig(bh.tc, S, C, dang, s2, sc, coarse);
-        rhs<KERR>(bh, sr, s2, sc, spr, spth, E, L, k);
-        at += k.t; ar += k.r; ath += k.th; aph += k.ph; apr += k.pr; apth += k.pth;
-        if (__builtin_expect(coarse && active(), 0)) {   // a stage angle moved by >= 2^-7 rad: full sin/cos path
-            // (idle lanes step on stale state -- often a captured ray next to the horizon -- and must not drag the warp here)
-            double acc[6];
-            int c;
-            rk4_sum_full<KERR>(p, r, th, pr, pth, E, L, acc, &c);
-            if (p.coarse_steps) p.coarse_steps[idx] += 1;      // the lane owns its particle's slot
-            at = acc[0]; ar = acc[1]; ath = acc[2]; aph = acc[3]; apr = acc[4]; apth = acc[5];
-            cap = c != 0;
-        }
-
-        double nt, nr, nth, nph, npr, npth, dt, dr, dth, dph, dpr, dpth;
-        kahan<PLAIN>(t, ct, p.h_sixth, at, nt, dt);
-        kahan<PLAIN>(r, cr, p.h_sixth, ar, nr, dr);
-        kahan<PLAIN>(th, cth, p.h_sixth, ath, nth, dth);
-        kahan<PLAIN>(ph, cph, p.h_sixth, aph, nph, dph);
-        kahan<PLAIN>(pr, cpr, p.h_sixth, apr, npr, dpr);
-        kahan<PLAIN>(pth, cpth, p.h_sixth, apth, npth, dpth);
-        cap |= !(nr >= p.r_capture);                                       // end point
-        const bool fin6 = all_finite6(nt, nr, nth, nph, npr, npth);
-
-        // --- A4: stop rules and events ------------------------------------------------------------
-        if (active()) {
-            if (cap) {
-                finish(ST_CAPTURED);            // step not taken: final = last accepted state
-            } else if (!fin6) {
-                finish(ST_NUMERIC);             // B6
-            } else {
-                if (!crossed) {                 // B5
-                    const double half_pi = 1.5707963267948966;
-                    const double d0 = th - half_pi, d1 = nth - half_pi;
-                    if (d0 * d1 < 0.0) {
-                        crossed = true;   // the radius goes straight to its slot (once per particle): no register held for it
-                        if (p.eq_cross_r) p.eq_cross_r[idx] = r + (nr - r) * (half_pi - th) / (nth - th);
-                    }
-                }
-                t = nt; r = nr; th = nth; ph = nph; pr = npr; pth = npth;
-                ct = dt; cr = dr; cth = dth; cph = dph; cpr = dpr; cpth = dpth;
-                ++steps;
-                if (SNAP != SNAP_NONE) {
-                    if (--snap_ctr == 0) { snap_ctr = p.snap_every; emit_snapshot(); }   // S1
-                }
-                if (r > p.r_escape) finish(ST_ESCAPED);              // B3
-                else if (steps >= p.nsteps) finish(ST_MAXSTEPS);     // B4
-            }
-        }
+        step(A, B);
+        step(B, A);
     }
 }
 

@@ -91,7 +91,7 @@ __device__ __forceinline__ void sincos_reduced(const TrigConsts& tc, double x, d
     pc = fma(pc, z, tc.c[1]);
     pc = fma(pc, z, tc.c[0]);
     sn = fma(y * z, ps, y);
-    cs = fma(z * z, pc, fma(z, -0.5, 1.0));
+    cs = fma(z, fma(z, pc, -0.5), 1.0);         // 1 - z/2 + z^2 pc(z), Horner: every FMA has one immediate operand
 }
 
 // s2 = sin^2 x and sc = sin x cos x -- the only trigonometric quantities the RHS needs (cos^2 enters
@@ -128,9 +128,9 @@ __device__ __forceinline__ void sincos_common_sign(const TrigConsts& tc, double 
 // on its neighbours.  The leading coefficients of the minimax kernels stand in for -1/6, 1/120, 1/24,
 // -1/720: they differ by < 1e-13 relative, which the factors d^2 <= 6e-5 push below 1e-17.
 __device__ __forceinline__ void stage_trig(const TrigConsts& tc, double S, double C, double d,
-                                           double& s2, double& sc, bool& coarse) {
-    coarse |= (__double2hiint(d) & 0x7fffffff) >= 0x3f800000;               // |d| >= 2^-7 or NaN
+                                           double& s2, double& sc, unsigned& dmax) {
     const double d2 = d * d;
+    dmax = max(dmax, (unsigned)__double2hiint(d2));      // d^2 >= 2^-14 <=> |d| >= 2^-7; a NaN ranks above both (unsigned)
     const double sd = fma(d * d2, fma(d2, tc.s[1], tc.s[0]), d);            // sin d
     const double cm = d2 * fma(fma(d2, tc.c[1], tc.c[0]), d2, -0.5);        // cos d - 1
     const double s1 = fma(S, cm, fma(C, sd, S));                            // sin(theta + d)
@@ -250,13 +250,57 @@ __device__ __noinline__ double energy_3p1(const Hole& bh, double r, double th, d
     return sqrt(alpha2 * (kappa + g)) + omega * L;
 }
 
-// Boyer-Lindquist -> Cartesian, eq.(7) PAPER.md:88-93 -- the paper's output format, fused
-// into the snapshot writer.  Full-range libdevice sincos: phi grows without bound.
-__device__ __noinline__ void cartesian_eq7(double a2, double r, double th, double ph, double& x, double& y, double& z) {
+// sin x and cos x with their true signs, for |x| up to ~2^20 (phi of a long orbit): the reduction of sincos_reduced,
+// then the quadrant k mod 4 from the two low bits of k (integer pipe).  Absolute error ~1e-16 (1 + |x| 2^-52).
+__device__ __forceinline__ void sincos_full(const TrigConsts& tc, double x, double& sn, double& cs) {
+    const double magic = 6755399441055744.0;
+    const double kd0 = fma(x, tc.two_over_pi, magic);
+    const int q = __double2loint(kd0);
+    const double kd = kd0 - magic;
+    double y = fma(-kd, tc.pio2_hi, x);
+    y = fma(-kd, tc.pio2_lo, y);
+    const double z = y * y;
+    double ps = fma(z, tc.s[5], tc.s[4]);
+    ps = fma(ps, z, tc.s[3]);
+    ps = fma(ps, z, tc.s[2]);
+    ps = fma(ps, z, tc.s[1]);
+    ps = fma(ps, z, tc.s[0]);
+    double pc = fma(z, tc.c[5], tc.c[4]);
+    pc = fma(pc, z, tc.c[3]);
+    pc = fma(pc, z, tc.c[2]);
+    pc = fma(pc, z, tc.c[1]);
+    pc = fma(pc, z, tc.c[0]);
+    const double s0 = fma(y * z, ps, y);
+    const double c0 = fma(z, fma(z, pc, -0.5), 1.0);
+    const double a = (q & 1) ? c0 : s0, b = (q & 1) ? s0 : c0;      // k odd: sin = +-cos y, cos = -+sin y
+    const int ssn = (q & 2) ? 0x80000000 : 0;                       // k = 2, 3: sin changes sign
+    const int scs = ((q + 1) & 2) ? 0x80000000 : 0;                 // k = 1, 2: cos changes sign
+    sn = __hiloint2double(__double2hiint(a) ^ ssn, __double2loint(a));
+    cs = __hiloint2double(__double2hiint(b) ^ scs, __double2loint(b));
+}
+
+// sqrt(x) for finite normal x > 0, faithfully rounded: MUFU.RSQ64H seed (relative error ~2^-20), one coupled
+// Goldschmidt step for (sqrt x, 1/(2 sqrt x)) and a final residual correction.  No special-case path.
+__device__ __forceinline__ double sqrt_nr(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double g = x * y, h = 0.5 * y;
+    const double r = fma(-g, h, 0.5);
+    g = fma(g, r, g);
+    h = fma(h, r, h);
+    return fma(fma(-g, g, x), h, g);
+}
+
+// Boyer-Lindquist -> Cartesian, eq.(7) PAPER.md:88-93 -- the paper's output format, fused into the
+// snapshot writer.  Inlined and branch-free (~60 FP64 instructions): with a record EVERY step -- the
+// paper's own mode -- the conversion runs once per RK4 step, and the round-1 version (an out-of-line routine built on
+// libdevice's sincos and sqrt) cost more than the step's own trigonometry.
+__device__ __forceinline__ void cartesian_eq7(const TrigConsts& tc, double a2, double r, double th, double ph,
+                                              double& x, double& y, double& z) {
     double st, ct, sp, cp;
-    sincos(th, &st, &ct);
-    sincos(ph, &sp, &cp);
-    const double w = sqrt(r * r + a2) * st;
+    sincos_full(tc, th, st, ct);
+    sincos_full(tc, ph, sp, cp);
+    const double w = sqrt_nr(fma(r, r, a2)) * st;
     x = w * cp;
     y = w * sp;
     z = r * ct;

@@ -66,10 +66,12 @@ def test_config4_full_2p22_sampled(G, oracle):
     assert np.quantile(hl, 0.9999) < 1e-9 and np.isfinite(hl).all()     # 2H + 1 drift is O(h^4) (DESIGN.md pins)
     fs = out["final_state"]
     assert bool((fs[7].cpu() == __import__("torch").from_numpy(st[5])).all())     # L = p_phi bit-exact (eq.(13))
-    ii = _sample(n, 1500, 41)
+    ii = _sample(n, 100_000, 41)          # ~9.5e4 distinct particles x 10^4 steps = 1e9 oracle steps (~10 s on the box)
     g = _take(out, ii)
     o = oracle.integrate(oracle.KERR, 1.0, a, np.ascontiguousarray(st[:, ii]), 0.01, 10000, nthreads=NCPU)
     c = parity.compare(g, o)
+    print(f"config 4: {len(ii)} sampled particles vs oracle: max err {c['err'].max():.3e}, p99.9 {np.quantile(c['err'], 0.999):.3e}")
+    assert len(ii) >= 90_000
     assert c["same_class"].all()
     assert c["err"].max() <= 1e-9, c["err"].max()
 
@@ -81,72 +83,23 @@ def test_config2_full_65536_sampled(G, oracle):
     out = _run_full(G, a, st, 0.01, 100000, snapshot_every=1000)
     assert int(out["status"].ne(G.ST_MAXSTEPS).sum().item()) == 0
     assert int(out["snap_count"].ne(101).sum().item()) == 0
-    ii = _sample(n, 160, 42)
+    ii = _sample(n, 4096, 42)             # ~4e3 particles x 10^5 steps = 4e8 oracle steps
     g = _take(out, ii, with_snaps=True)
     o = oracle.integrate(oracle.KERR, 1.0, a, np.ascontiguousarray(st[:, ii]), 0.01, 100000,
                          snapshot_every=1000, nthreads=NCPU)
-    c = parity.compare(g, o)
-    assert c["same_class"].all()
-    assert c["err"].max() <= 1e-9, c["err"].max()
-    assert np.array_equal(g["snap_count"], o["snap_count"])
-    assert parity.rel_err(g["snapshots"], o["snapshots"]).max() <= 1e-9
-
-
-def _null_sampled(G, oracle, st, a, out, ii, snapshot_every=0, snap_mask=0xFF):
-    r_cap = W.horizon_radius(1.0, a) + 0.01
-    kw = dict(r_capture=r_cap, r_escape=1100.0, kind=oracle.NULL, snapshot_every=snapshot_every,
-              snap_mask=snap_mask, nthreads=NCPU)
-    sub = np.ascontiguousarray(st[:, ii])
-    o = oracle.integrate(oracle.KERR, 1.0, a, sub, 0.02, 200000, **kw)
-    o_ld = oracle.integrate(oracle.KERR, 1.0, a, sub, 0.02, 200000, long_double=True, **kw)
-    cert = parity.certified(o, o_ld, 1e-8)
-    g = _take(out, ii, with_snaps=snapshot_every > 0)
-    c = parity.compare(g, o)
-    assert (~c["same_class"]).sum() <= max(1, int(1e-4 * len(ii)))
-    assert c["same_class"][cert].all()
-    assert c["err"][cert].max() <= 1e-8, c["err"][cert].max()
-    assert cert.mean() > 0.97, cert.mean()
-    return g, o, cert
-
-
-def test_config3_full_1024x1024_sampled(G, oracle):
-    """configs[2]: a=0.998, i=60 deg, the whole 1024^2 image in one call (work queue refilling lanes as
-    rays are captured / escape); 256 sampled pixels against the oracle, whole-image class statistics
-    against the analytic capture criterion's expectation (~19 % captured)."""
-    a, N = 0.998, 1024
-    st = W.camera_rays(N, a, 60.0)
-    out = _run_full(G, a, st, 0.02, 200000, r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0,
-                    kind=G.NULL)
-    status = out["status"].cpu().numpy()
-    counts = np.bincount(status, minlength=4)
-    assert counts[G.ST_NUMERIC] == 0
-    assert counts[G.ST_MAXSTEPS] <= 1e-3 * N * N          # only near-axis garbage rays hit the cap (B7)
-    assert 0.15 < counts[G.ST_CAPTURED] / (N * N) < 0.25
-    ii = _sample(N * N, 252, 43)
-    _null_sampled(G, oracle, st, a, out, ii)
-
-
-def test_config5_full_tile_4096x256_sampled(G, oracle):
-    """configs[4]: i=85 deg, 4096^2 image, ONE of the 16 tiles of 256 rows (the central one, which holds
-    the shadow), snapshot every 500 steps of (t, r, theta, phi) -- 2^20 rays, 13.5 GB snapshot buffer."""
-    a, N, rows = 0.998, 4096, 256
-    st, (al, be, Lz, Q) = W.camera_rays(N, a, 85.0, row0=(N - rows) // 2, rows=rows, return_constants=True)
-    out = _run_full(G, a, st, 0.02, 200000, snapshot_every=500, snap_mask=0x0F,
-                    r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0, kind=G.NULL)
-    n = st.shape[1]
-    # every ray of the tile against the closed-form capture/escape criterion (see the config-3 test below)
-    wrong = (out["status"].cpu().numpy() == G.ST_ESCAPED) != _escapes_analytic(a, Lz, Q, W.horizon_radius(1.0, a), 1000.0)
-    print("config5 tile class mismatches:", int(wrong.sum()), "outside the axis columns:", int((wrong & (np.abs(al) >= 0.1)).sum()))
-    assert (wrong & (np.abs(al) >= 0.1)).sum() <= 32 and wrong.sum() <= 5e-3 * n
-    ii = _sample(n, 124, 45)
-    g, o, cert = _null_sampled(G, oracle, st, a, out, ii, snapshot_every=500, snap_mask=0x0F)
-    assert np.array_equal(g["snap_count"][cert], o["snap_count"][cert])
-    cap = o["snapshots"].shape[1]
-    valid = (np.arange(cap)[None, :] < o["snap_count"][:, None]) & cert[:, None]
-    assert parity.rel_err(g["snapshots"], o["snapshots"])[valid].max() <= 1e-8
-    # S1 at any size: snap_count = 1 + floor(steps_done / 500) for every ray of the tile
-    sd = out["steps_done"].cpu().numpy()
-    assert np.array_equal(out["snap_count"].cpu().numpy(), 1 + sd // 500)
+    # reading P3: every particle the oracle itself determines to 1e-10 (double vs long double) must be within 1e-9,
+    # final record AND all 101 trajectory records; the others (low-|L_z| orbits that pass next to the polar axis, reading
+    # B7) are counted and printed.  Round 1 compared 160 particles and met none of them.
+    def certify(jj):
+        sub = np.ascontiguousarray(st[:, ii[jj]])
+        kw = dict(snapshot_every=1000, nthreads=NCPU)
+        return [oracle.integrate(oracle.KERR, 1.0, a, sub, 0.01, 100000, long_double=True, **kw),
+                oracle.integrate(oracle.KERR, 1.0, a, parity.ulp_nudged(sub), 0.01, 100000, **kw)]
+    rep = parity.p3_report(g, o, certify, 1e-9, labels=st[[0, 1, 3, 4, 5]][:, ii], max_fail_frac=0.002,
+                           what="config 2 (labels: r0, theta0, u_r, u_theta, L_z)",
+                           extra_err=parity.snapshot_err(g, o), extra_err_fn=parity.snapshot_err)
+    print(f"config 2: {len(ii)} sampled particles incl. 101 records each vs oracle: {rep}")
+    assert len(ii) >= 3800 and rep["class_mismatch"] == 0
 
 
 def _escapes_analytic(a, Lz, Q, r_plus, r_obs):
@@ -167,25 +120,170 @@ def _escapes_analytic(a, Lz, Q, r_plus, r_obs):
     return esc
 
 
-def test_config3_whole_image_classes_match_the_analytic_criterion(G):
-    """Every one of the 1024^2 pixels against the closed-form capture/escape criterion (no oracle involved).
-    The method itself fails next to the polar axis (reading B7: |L_z| <~ 3h columns) and the
-    capture guard eats a sub-pixel band at the prograde edge of the critical curve; everything else must
-    agree."""
+def _critical_band(esc_img, px):
+    """Pixels within +-px (Chebyshev) of the analytic critical curve = the boundary between the escaping and the
+    captured region of the image: those that have both classes in their (2 px + 1)^2 neighbourhood."""
+    def dilate(m):
+        out = m.copy()
+        for _ in range(px):
+            q = out.copy()
+            q[1:, :] |= out[:-1, :]; q[:-1, :] |= out[1:, :]
+            out = q.copy()
+            q[:, 1:] |= out[:, :-1]; q[:, :-1] |= out[:, 1:]
+            out = q
+        return out
+    return dilate(esc_img) & dilate(~esc_img)
+
+
+def _null_oracle(oracle, st, a, ii, long_double=False, snapshot_every=0, snap_mask=0xFF, nudge=False):
+    sub = np.ascontiguousarray(st[:, ii])
+    return oracle.integrate(oracle.KERR, 1.0, a, parity.ulp_nudged(sub) if nudge else sub, 0.02, 200000,
+                            r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0, kind=oracle.NULL,
+                            snapshot_every=snapshot_every, snap_mask=snap_mask, long_double=long_double, nthreads=NCPU)
+
+
+def _null_sets_vs_oracle(G, oracle, st, consts, a, out, sets, snapshot_every=0, snap_mask=0xFF, cert_stat=600):
+    """Compare the rays of every named index set with the oracle under reading P3 (tests/parity.py:
+    null_parity_report).  Returns {name: report}.  A fixed sub-sample of the first set also gets the long double oracle
+    unconditionally, for the certified-fraction statistic DESIGN.md quotes."""
+    reports = {}
+    for name, ii in sets.items():
+        if len(ii) == 0:
+            continue
+        o = _null_oracle(oracle, st, a, ii, snapshot_every=snapshot_every, snap_mask=snap_mask)
+        g = _take(out, ii, with_snaps=snapshot_every > 0)
+        skw = dict(snapshot_every=snapshot_every, snap_mask=snap_mask)
+        rep = parity.p3_report(
+            g, o, lambda jj: [_null_oracle(oracle, st, a, ii[jj], long_double=True, **skw),
+                              _null_oracle(oracle, st, a, ii[jj], nudge=True, **skw)],
+            1e-8, labels=consts[:, ii], max_fail_frac=0.10 if name in ("axis", "band") else 0.03, what=name,
+            extra_err=parity.snapshot_err(g, o) if snapshot_every > 0 else None,            # trajectories: same bar
+            extra_err_fn=parity.snapshot_err if snapshot_every > 0 else None)
+        print(f"{name}: {rep}")
+        reports[name] = rep
+    first = next(iter(sets))
+    jj = sets[first][:cert_stat]
+    if len(jj):
+        o0 = _null_oracle(oracle, st, a, jj)
+        cert = (parity.certified(o0, _null_oracle(oracle, st, a, jj, long_double=True), 1e-8)
+                & parity.certified(o0, _null_oracle(oracle, st, a, jj, nudge=True), 1e-8))
+        print(f"certified fraction on {len(jj)} rays of '{first}': {cert.mean():.4f}")
+        assert cert.mean() > 0.97
+    return reports
+
+
+def test_config3_full_1024x1024_vs_oracle_at_a_resolution_that_can_fail(G, oracle):
+    """configs[2]: a=0.998, i=60 deg, the whole 1024^2 image in one call (work queue refilling lanes as rays are
+    captured / escape).  north_star: class identical on >= 99.99 % of pixels, 1e-8 on the rest -- asserted where it can
+    fail (round-1 verdict, 'what's weak' 1):
+      * every pixel against the closed-form capture/escape criterion (no oracle): mismatches only in the axis columns;
+      * 12 000 uniformly sampled pixels against the oracle: at most one class mismatch (99.99 %), all certified rays 1e-8;
+      * EVERY pixel within +-3 px of the analytic critical curve and EVERY pixel of the 10 columns next to the polar axis
+        (reading B7) against the oracle: all certified rays identical in class and within 1e-8, the others counted and
+        printed with (alpha, beta, L_z, Q) (reading P3);
+      * image-level class bar: (mismatches in band + axis, counted exhaustively) + 0 in the uniform sample of the rest
+        <= 1e-4 x 2^20 pixels."""
     a, N = 0.998, 1024
-    st, (al, be, Lz, Q) = W.camera_rays(N, a, 60.0, return_constants=True)
+    st, consts = W.camera_rays(N, a, 60.0, return_constants=True)
+    al, be, Lz, Q = consts
     rp = W.horizon_radius(1.0, a)
     out = _run_full(G, a, st, 0.02, 200000, r_capture=rp + 0.01, r_escape=1100.0, kind=G.NULL)
     status = out["status"].cpu().numpy()
+    counts = np.bincount(status, minlength=4)
+    assert counts[G.ST_NUMERIC] == 0
+    assert counts[G.ST_MAXSTEPS] <= 1e-3 * N * N          # only near-axis garbage rays hit the cap (B7)
+    assert 0.15 < counts[G.ST_CAPTURED] / (N * N) < 0.25
+    # closed form, all pixels
     esc = _escapes_analytic(a, Lz, Q, rp, 1000.0)
     wrong = (status == G.ST_ESCAPED) != esc
-    axis = np.abs(al) < 0.1                      # 10 pixel columns around alpha = 0
-    print("mismatches:", int(wrong.sum()), "of which near-axis:", int((wrong & axis).sum()),
+    axis = np.abs(al) < 0.1                      # the 10 pixel columns around alpha = 0
+    print("closed-form class mismatches:", int(wrong.sum()), "of which in the axis columns:", int((wrong & axis).sum()),
           "captured fraction analytic / gpu:", float((~esc).mean()), float((status == G.ST_CAPTURED).mean()))
-    assert (wrong & ~axis).sum() <= 8             # measured: 0 (all 533 mismatches sit in the axis columns)
+    assert (wrong & ~axis).sum() <= 8             # measured: 0
     assert wrong.sum() <= 2e-3 * N * N
     health = out["health"].cpu().numpy()
-    assert np.median(health[wrong & axis]) > 1e-9 if (wrong & axis).any() else True   # flagged as numerically invalid
+    if (wrong & axis).any():
+        assert np.median(health[wrong & axis]) > 1e-9     # flagged as numerically invalid
+    # oracle, at a resolution that can fail
+    band = _critical_band(esc.reshape(N, N), 3).ravel() & ~axis
+    rest = np.flatnonzero(~band & ~axis)
+    rng = np.random.default_rng(43)
+    sets = {"uniform": np.sort(rng.choice(rest, 12000, replace=False)), "band": np.flatnonzero(band), "axis": np.flatnonzero(axis)}
+    print({k: len(v) for k, v in sets.items()})
+    assert len(sets["band"]) > 5000 and len(sets["axis"]) == 10 * N
+    rep = _null_sets_vs_oracle(G, oracle, st, consts, a, out, sets)
+    assert rep["uniform"]["class_mismatch"] <= 1          # 99.99 % of 12 000
+    # image-level literal bar: band and axis columns are counted exhaustively, the rest has (at most) the sampled rate
+    est = rep["band"]["class_mismatch"] + rep["axis"]["class_mismatch"] + rep["uniform"]["class_mismatch"] * len(rest) / 12000.0
+    print(f"class (status AND steps_done) mismatches: band {rep['band']['class_mismatch']} of {rep['band']['n']}, axis "
+          f"{rep['axis']['class_mismatch']} of {rep['axis']['n']}, uniform {rep['uniform']['class_mismatch']} of 12000 -> image-level "
+          f"estimate {est:.0f} of {N * N} pixels ({100.0 * (1 - est / (N * N)):.4f} % identical)")
+    assert est <= 1e-4 * N * N
+
+
+def test_config5_whole_4096x4096_image_in_16_tiles(G, oracle):
+    """configs[4] as specified: i=85 deg, the WHOLE 4096^2 image, snapshot every 500 steps of (t, r, theta, phi) -- the
+    dense trajectory buffer at the step cap is 215 GB > HBM, so the harness walks 16 tiles of 256 rows (reading S3;
+    13.5 GB of records per tile, one buffer reused).  Per tile: every pixel against the closed-form capture/escape
+    criterion, S1 (snap_count = 1 + steps_done // 500) on every ray; against the oracle (final record AND trajectory,
+    reading P3): the stride-16 sub-image, every pixel within +-3 px of the analytic critical curve, and every 16th row
+    of the 40 columns next to the polar axis."""
+    import torch
+    a, N, rows, every = 0.998, 4096, 256, 500
+    rp = W.horizon_radius(1.0, a)
+    dev = torch.device("cuda:0")
+    ctx = G.geo_create(G.KERR, 1.0, a)
+    n = N * rows
+    out = G.alloc_outputs(n, dev, 200000, every, None, 0x0F)
+    tot = {"steps": 0, "records": 0, "wrong": 0, "wrong_off_axis": 0, "captured": 0, "maxsteps": 0}
+    agg = {}
+    try:
+        for t in range(N // rows):
+            row0 = t * rows
+            lo, hi = max(0, row0 - 3), min(N, row0 + rows + 3)                 # 3-row halo for the critical band
+            st_h, c_h = W.camera_rays(N, a, 85.0, row0=lo, rows=hi - lo, return_constants=True)
+            sl = slice((row0 - lo) * N, (row0 - lo) * N + n)
+            st, consts = np.ascontiguousarray(st_h[:, sl]), c_h[:, sl]
+            al = consts[0]
+            G.geo_integrate(ctx, torch.from_numpy(st).to(dev), 0.02, 200000, out, snapshot_every=every,
+                            r_capture=rp + 0.01, r_escape=1100.0, kind=G.NULL)
+            torch.cuda.synchronize()
+            status = out["status"].cpu().numpy()
+            sd = out["steps_done"].cpu().numpy()
+            sc = out["snap_count"].cpu().numpy()
+            assert np.isin(status, (G.ST_MAXSTEPS, G.ST_CAPTURED, G.ST_ESCAPED)).all()
+            assert np.array_equal(sc, 1 + sd // every)                           # S1 at any size
+            esc_h = _escapes_analytic(a, c_h[2], c_h[3], rp, 1000.0)
+            esc = esc_h[sl]
+            wrong = (status == G.ST_ESCAPED) != esc
+            axis = np.abs(al) < 0.1                                              # 40 columns around alpha = 0
+            tot["steps"] += int(sd.sum()); tot["records"] += int(sc.sum())
+            tot["wrong"] += int(wrong.sum()); tot["wrong_off_axis"] += int((wrong & ~axis).sum())
+            tot["captured"] += int((status == G.ST_CAPTURED).sum()); tot["maxsteps"] += int((status == G.ST_MAXSTEPS).sum())
+            band = _critical_band(esc_h.reshape(hi - lo, N), 3).ravel()[sl] & ~axis
+            img = np.arange(n).reshape(rows, N)
+            stride = img[8::16, 8::16].ravel()
+            stride = stride[~band[stride] & ~axis[stride]]
+            ax = img[8::16, :].ravel()
+            sets = {"stride16": stride, "band": np.flatnonzero(band), "axis": ax[axis[ax]]}
+            rep = _null_sets_vs_oracle(G, oracle, st, consts, a, out, sets, snapshot_every=every, snap_mask=0x0F,
+                                       cert_stat=100 if t in (0, 7) else 0)
+            for k, r in rep.items():
+                d = agg.setdefault(k, {"n": 0, "class_mismatch": 0, "fail": 0})
+                for q in d:
+                    d[q] += r[q]
+            print(f"tile {t}: classes captured {int((status == G.ST_CAPTURED).sum())} escaped {int((status == G.ST_ESCAPED).sum())} "
+                  f"cap {int((status == G.ST_MAXSTEPS).sum())}; closed-form mismatches {int(wrong.sum())} (off axis {int((wrong & ~axis).sum())})")
+    finally:
+        G.geo_destroy(ctx)
+    npx = N * N
+    print(f"config 5 whole image: {tot['steps']:.4e} geodesic-steps, {tot['records']} records = {tot['records'] * 32 / 1e9:.1f} GB written "
+          f"(dense buffer would be {npx * 401 * 32 / 1e9:.0f} GB), captured {tot['captured'] / npx:.4f}, at the step cap {tot['maxsteps']}, "
+          f"closed-form class mismatches {tot['wrong']} (off the axis columns: {tot['wrong_off_axis']}); vs oracle: {agg}")
+    assert tot["wrong_off_axis"] <= 64 and tot["wrong"] <= 5e-3 * npx
+    assert 0.10 < tot["captured"] / npx < 0.25
+    assert agg["stride16"]["n"] > 60000 and agg["band"]["n"] > 20000 and agg["axis"]["n"] >= 10000
+    assert agg["stride16"]["class_mismatch"] <= max(1, int(1e-4 * agg["stride16"]["n"]))      # 99.99 % on the regular sub-image
 
 
 def test_tab4_full_2p22_tabulated_sampled(G, tab_oracle):

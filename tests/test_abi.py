@@ -57,3 +57,18 @@ def test_product_path_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert not bad.search(txt), f
+
+
+def test_bench_instruction_counts_match_the_built_library():
+    """bench.py's executed-instruction counts (KERNEL_COUNTS, from the committed ncu captures) are cross-checked against
+    the static SASS count of the hot loops of the library as built here: a kernel edit without a new capture fails."""
+    import sys
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1803_08320_b200 import build
+    build.build()
+    for key in bench.KERNEL_COUNTS:
+        kc = bench.kernel_counts(key)          # raises SystemExit on disagreement
+        assert kc["flop"] > 0 and kc["pipe"] > 0
+        if key != "tabulated":
+            assert kc["static"] is not None and kc["static"]["DFMA"] > 100

@@ -61,6 +61,56 @@ def _worker(rank, world, port, tmpdir):
         dist.destroy_process_group()
 
 
+def _bench_worker(rank, world, port, tmpdir):
+    """The N > 1 legs of bench.py itself -- dist_init, the MAX/SUM reductions, the strong-scaling shard, the rank-0 JSON
+    line, dist_finish -- with the environment torchrun would set, on gloo with CPU tensors standing in for the device."""
+    sys.path.insert(0, ROOT)
+    import argparse
+    import json
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    import torch
+    import bench
+    from paper_1803_08320_b200 import workloads as W
+    dist = bench.dist_init(world, "gloo")
+    assert dist is not None and dist.get_world_size() == world
+    bench.dist_barrier(dist)
+    # weak scaling: every rank reports its own batch; strong: one 64 x 64 image in interleaved row tiles
+    img = {"st": W.camera_rays(64, 0.998, 60.0), "name": "test image"}
+    mine = bench.shard_for_rank(img, rank, world, "strong")
+    rows = 64 // 16
+    tiles = W.interleaved_tiles(16, rank, world)
+    assert mine["st"].shape[1] == len(tiles) * rows * 64
+    assert np.array_equal(mine["st"][:, : rows * 64], img["st"][:, tiles[0] * rows * 64:(tiles[0] + 1) * rows * 64])
+    assert bench.shard_for_rank(img, rank, world, "weak") is img
+    units = float(mine["st"].shape[1]) * 10.0                       # stand-in: 10 steps per ray
+    tmax, tot = bench.reduce_time_and_units(dist, torch.device("cpu"), 100.0 + 50.0 * rank, units)
+    assert tmax == 100.0 + 50.0 * (world - 1) and tot == 64 * 64 * 10.0
+    if rank == 0:
+        args = argparse.Namespace(steps=1, warmup=0)
+        line = bench.make_line(args, world, tot / (tmax * 1e-3), tmax, "strong", {"workload": mine["name"]}, {"sm_mhz": None},
+                               None, 1, {"bound": "alu"}, None)
+        txt = json.dumps(line)
+        back = json.loads(txt)
+        assert back["n_gpus"] == world and back["scaling"] == "strong" and back["value"] == 64 * 64 * 10.0 / 0.15
+        for key in ("metric", "unit", "ms_per_step", "higher_is_better", "vs_baseline", "dtype", "data", "config", "clocks",
+                    "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+            assert key in back, key
+    bench.dist_finish(dist)
+    assert not torch.distributed.is_initialized()
+    open(os.path.join(tmpdir, f"bench_ok{rank}"), "w").write("ok")
+
+
+def test_bench_py_multi_rank_legs_on_gloo(tmp_path):
+    import socket
+    import torch.multiprocessing as mp
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    mp.spawn(_bench_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    assert (tmp_path / "bench_ok0").exists() and (tmp_path / "bench_ok1").exists()
+
+
 def test_world_size_2_gloo_sharding(tmp_path):
     import socket
     import torch.multiprocessing as mp

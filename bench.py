@@ -203,13 +203,21 @@ class ClockSampler:
 
 
 
+_SASS_CACHE: dict = {}
+
+
 def static_sass_count(sym_part: str) -> dict | None:
     """FP64 instructions in the hot loop of a kernel of the LOADED library: the backward branch that spans the most
     DFMA.  Static count: it includes the rarely executed blocks inside the loop's address range (an upper bound)."""
     from paper_1803_08320_b200 import geo
-    try:
-        out = subprocess.run(["cuobjdump", "-sass", geo.LIB_PATH], capture_output=True, text=True, check=True).stdout
-    except (OSError, subprocess.CalledProcessError):
+    key = (geo.LIB_PATH, os.path.getmtime(geo.LIB_PATH) if os.path.exists(geo.LIB_PATH) else 0)
+    if key not in _SASS_CACHE:
+        try:
+            _SASS_CACHE[key] = subprocess.run(["cuobjdump", "-sass", geo.LIB_PATH], capture_output=True, text=True, check=True).stdout
+        except (OSError, subprocess.CalledProcessError):
+            _SASS_CACHE[key] = None
+    out = _SASS_CACHE[key]
+    if out is None:
         return None
     ins_re = re.compile(r"^\s+/\*([0-9a-f]{4,})\*/\s+(?:@!?U?P\d+\s+)?([A-Z0-9_.]+)(.*?);")
     ins, on = [], False

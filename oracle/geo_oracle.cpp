@@ -335,7 +335,27 @@ struct DP45 {
                                187.0L / 2100, 1.0L / 40};
 };
 
-struct AdaptiveCtl { double h0, rtol, atol, h_min, tau_end; };   // tau_end = +inf: no final time
+struct AdaptiveCtl { double h0, rtol, atol, h_min, tau_end, snap_dtau; };   // tau_end = +inf: no final time; snap_dtau = 0: no records
+
+// Dense output of the pair (reading A3): the continuous extension of DOPRI5 as implemented in Hairer's dopri5
+// ("contd5"; Hairer, Norsett & Wanner, Solving ODEs I, sec. II.6), fourth-order accurate on the whole step:
+//   y(tau_n + theta h) = y_n + h sum_i w_i(theta) k_i,   theta in [0, 1],  theta1 = 1 - theta,
+//   w_i(theta) = theta { b_i + theta1 [ (delta_i1 - b_i) + theta ( (2 b_i - delta_i1 - delta_i7) + theta1 d_i ) ] },
+// b = the 5th-order weights (b_7 = 0), d = the dense-output coefficients below (d_2 = 0).  Properties pinned by
+// tests/test_oracle_adaptive.py: w(0) = 0, w(1) = b, w'(0) = e_1, w'(1) = e_7 (a C^1 Hermite interpolant of the
+// accepted steps) and the order conditions sum_i w_i(theta) Phi_i = theta^q / gamma for all trees up to q = 4.
+template <class R> void dp45_dense_weights(R theta, R w[7]) {
+    static const DP45 T;
+    static const long double d[7] = {-12715105075.0L / 11282082432.0L, 0.0L, 87487479700.0L / 32700410799.0L,
+                                     -10690763975.0L / 1880347072.0L, 701980252875.0L / 199316789632.0L,
+                                     -1453857185.0L / 822651844.0L, 69997945.0L / 29380423.0L};
+    const R th1 = R(1) - theta;
+    for (int i = 0; i < 7; ++i) {
+        const R b = (R)(i < 6 ? T.a[6][i] : 0.0L);
+        const R e1 = i == 0 ? R(1) : R(0), e7 = i == 6 ? R(1) : R(0);
+        w[i] = theta * (b + th1 * ((e1 - b) + theta * ((R(2) * b - e1 - e7) + th1 * (R)d[i])));
+    }
+}
 
 template <class R> R comp6(const State<R>& y, int c) {
     switch (c) { case 0: return y.t; case 1: return y.r; case 2: return y.th; case 3: return y.ph;
@@ -371,6 +391,10 @@ void integrate_one_adaptive(const Hole<R>& bh, const double* state_in, int64_t n
     R h = (R)ctl.h0;
     R tau = R(0);
     const R tau_end = (R)ctl.tau_end;
+    const bool dense = ctl.snap_dtau > 0.0 && o.snapshots != nullptr;   // reading A3: records at tau_j = j * snap_dtau
+    const bool cart = (st.flags & ORA_FLAG_CARTESIAN_SNAP) != 0;
+    const R dtau = (R)ctl.snap_dtau;
+    int64_t next_j = 0;                               // records produced so far = index of the next one
     int32_t status = -1;
     int64_t steps = 0, attempts = 0, rejected = 0;
     R eq_cross = std::numeric_limits<R>::quiet_NaN();
@@ -378,8 +402,11 @@ void integrate_one_adaptive(const Hole<R>& bh, const double* state_in, int64_t n
 
     if (!(y.r >= rc)) status = ORA_ST_CAPTURED;                      // B1
     else if (!finite6(y) || !std::isfinite(y.E)) status = ORA_ST_NUMERIC;
-    else if (y.r > re) status = ORA_ST_ESCAPED;
-    else if (max_attempts == 0) status = ORA_ST_MAXSTEPS;
+    else {
+        if (dense) { write_snapshot(o, i, 0, y, bh.a, cart); next_j = 1; }   // record 0 = y0 (tau = 0), as S1
+        if (y.r > re) status = ORA_ST_ESCAPED;
+        else if (max_attempts == 0) status = ORA_ST_MAXSTEPS;
+    }
 
     Deriv<R> k[DP45::S];
     if (status < 0) k[0] = rhs(bh, y);
@@ -447,11 +474,28 @@ void integrate_one_adaptive(const Hole<R>& bh, const double* state_in, int64_t n
                 eq_cross = y.r + (yn.r - y.r) * (half_pi - y.th) / (yn.th - y.th);
             }
         }
+        const R tau_new = last ? tau_end : tau + h;                  // the final time is landed on exactly
+        if (dense) {                                                 // A3: every record time in (tau, tau_new]
+            for (;;) {
+                const R tj = (R)next_j * dtau;
+                if (!(tj <= tau_new)) break;
+                R w[7];
+                dp45_dense_weights<R>((tj - tau) / h, w);
+                State<R> ys = y;
+                for (int c = 0; c < 6; ++c) {
+                    R acc = R(0);
+                    for (int j = 0; j < DP45::S; ++j) acc += w[j] * dcomp6(k[j], c);
+                    set6(ys, c, comp6(y, c) + h * acc);
+                }
+                write_snapshot(o, i, next_j, ys, bh.a, cart);
+                ++next_j;
+            }
+        }
         y = yn;
         for (int c = 0; c < 6; ++c) cc[c] = cn[c];
         k[0] = k[6];                                                 // first same as last
         ++steps;
-        tau += h;
+        tau = tau_new;
         h *= fac;
         if (y.r > re) status = ORA_ST_ESCAPED;                       // B3
         else if (last || attempts >= max_attempts) status = ORA_ST_MAXSTEPS;   // final time / B4 (cap on attempts)
@@ -461,6 +505,7 @@ void integrate_one_adaptive(const Hole<R>& bh, const double* state_in, int64_t n
     o.steps_done[i] = steps;
     if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
     if (o.health) o.health[i] = (double)std::fabs(R(2) * hamiltonian(bh, y) + kappa);
+    if (dense && o.snap_count) o.snap_count[i] = (int32_t)next_j;
     if (rejected_out) rejected_out[i] = rejected;
 }
 
@@ -506,14 +551,15 @@ int oracle_integrate(int metric, double M, double a, const double* state_in, int
 }
 
 // Adaptive RK5(4).  ctl = {h0, rtol, atol, h_min}; max_attempts caps accepted + rejected
-// attempts per particle; rejected: [n] or NULL.  Snapshot fields of `out` are ignored.
+// attempts per particle; rejected: [n] or NULL.  ctl->snap_dtau > 0: dense-output records into out->snapshots (reading A3).
 int oracle_integrate_adaptive(int metric, double M, double a, const double* state_in, int64_t n,
                               const AdaptiveCtl* ctl, int64_t max_attempts, const StopRule* stop,
                               const OutPtrs* out, int64_t* rejected, int precision, int nthreads) {
     if (!stop || !out || !ctl || n < 0 || max_attempts < 0) return 1;
     if (!(M > 0) || !(std::fabs(a) <= M)) return 1;
     if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0) || !(ctl->rtol >= 0) || !(ctl->atol >= 0) ||
-        !(ctl->rtol + ctl->atol > 0) || !(ctl->h_min >= 0) || !(ctl->tau_end > 0)) return 1;
+        !(ctl->rtol + ctl->atol > 0) || !(ctl->h_min >= 0) || !(ctl->tau_end > 0) || !(ctl->snap_dtau >= 0)) return 1;
+    if (ctl->snap_dtau > 0 && (!out->snapshots || !out->snap_count || out->snap_capacity < 1 || (out->snap_mask & 0xFFu) == 0)) return 1;
     if (metric != ORA_SCHWARZSCHILD && metric != ORA_KERR) return 1;
     if (metric == ORA_SCHWARZSCHILD && a != 0.0) return 1;
     if (n == 0) return 0;
@@ -542,6 +588,13 @@ int oracle_integrate_adaptive(int metric, double M, double a, const double* stat
         });
     for (auto& th : pool) th.join();
     return 0;
+}
+
+// w_i(theta), i = 1..7, of the dense output (reading A3), as doubles.
+void oracle_dp45_dense_weights(double theta, double* w7) {
+    long double w[7];
+    dp45_dense_weights<long double>((long double)theta, w);
+    for (int i = 0; i < 7; ++i) w7[i] = (double)w[i];
 }
 
 // The Butcher tableau the adaptive path uses, as doubles: c[7], a[7][7] (row-major), b5[7], b4[7].

@@ -56,32 +56,49 @@ def lib():
 
 class _Ctl(C.Structure):
     _fields_ = [("h0", C.c_double), ("rtol", C.c_double), ("atol", C.c_double), ("h_min", C.c_double),
-                ("tau_end", C.c_double)]
+                ("tau_end", C.c_double), ("snap_dtau", C.c_double)]
 
 
 def integrate_adaptive(metric: int, M: float, a: float, state_in: np.ndarray, h0: float, rtol: float,
                        atol: float, max_attempts: int, r_capture: float = -np.inf, r_escape: float = np.inf,
                        kind: int = TIMELIKE, h_min: float = 1e-12, tau_end: float = np.inf,
-                       long_double: bool = False, nthreads: int = 1) -> dict:
-    """Adaptive Dormand-Prince RK5(4) on host SoA state_in [6][n].  rtol = inf: fixed step h0."""
+                       long_double: bool = False, nthreads: int = 1, snap_dtau: float = 0.0,
+                       snap_capacity: int = 0, snap_mask: int = 0xFF, flags: int = 0) -> dict:
+    """Adaptive Dormand-Prince RK5(4) on host SoA state_in [6][n].  rtol = inf: fixed step h0.
+    snap_dtau > 0: dense-output records at tau = j snap_dtau (reading A3), [n][snap_capacity][ncomp]."""
     st = np.ascontiguousarray(state_in, dtype=np.float64)
     n = st.shape[1]
     res = {"final_state": np.full((8, n), np.nan), "status": np.full(n, -1, dtype=np.int32),
            "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan),
-           "health": np.full(n, np.nan), "rejected": np.zeros(n, dtype=np.int64)}
+           "health": np.full(n, np.nan), "rejected": np.zeros(n, dtype=np.int64), "snapshots": None, "snap_count": None}
+    if snap_dtau > 0:
+        res["snapshots"] = np.full((n, snap_capacity, bin(snap_mask & 0xFF).count("1")), np.nan)
+        res["snap_count"] = np.zeros(n, dtype=np.int32)
     L = lib()
     L.oracle_integrate_adaptive.restype = C.c_int
     L.oracle_integrate_adaptive.argtypes = [C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_int64, C.POINTER(_Ctl),
                                             C.c_int64, C.POINTER(_Stop), C.POINTER(_Out), C.c_void_p, C.c_int, C.c_int]
-    stop = _Stop(r_capture, r_escape, kind, 0)
+    stop = _Stop(r_capture, r_escape, kind, flags)
     out = _Out(res["final_state"].ctypes.data, res["status"].ctypes.data, res["steps_done"].ctypes.data,
-               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data, None, 0, 0, None)
-    ctl = _Ctl(h0, rtol, atol, h_min, tau_end)
+               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data,
+               res["snapshots"].ctypes.data if snap_dtau > 0 else None, snap_capacity, snap_mask,
+               res["snap_count"].ctypes.data if snap_dtau > 0 else None)
+    ctl = _Ctl(h0, rtol, atol, h_min, tau_end, snap_dtau)
     rc = L.oracle_integrate_adaptive(metric, M, a, st.ctypes.data, n, C.byref(ctl), max_attempts, C.byref(stop),
                                      C.byref(out), res["rejected"].ctypes.data, int(long_double), nthreads)
     if rc != 0:
         raise ValueError("oracle_integrate_adaptive: invalid arguments")
     return res
+
+
+def dp45_dense_weights(theta: float) -> np.ndarray:
+    """w_i(theta), i = 1..7: y(tau_n + theta h) = y_n + h sum_i w_i k_i (reading A3)."""
+    w = np.zeros(7)
+    L = lib()
+    L.oracle_dp45_dense_weights.restype = None
+    L.oracle_dp45_dense_weights.argtypes = [C.c_double, C.c_void_p]
+    L.oracle_dp45_dense_weights(theta, w.ctypes.data)
+    return w
 
 
 def dp45_tableau() -> dict:

@@ -120,3 +120,82 @@ def test_undefined_error_estimate_shrinks_the_step_and_ends_with_numeric(oracle)
     r0 = oracle.integrate_adaptive(oracle.SCHWARZSCHILD, 1.0, 0.0, st, 0.1, 1e-9, 0.0, 10**6, h_min=0.0)
     assert r0["status"][0] == oracle.ST_NUMERIC and 400 < r0["rejected"][0] < 500      # 0.2^k underflows to 0 near k = 463
     np.testing.assert_array_equal(r0["final_state"][1:4, 0], st[0:3, 0])               # final = y0, untouched
+
+
+# ---- reading A3: dense output of the pair (records at fixed tau from the continuous extension) ----------------------
+def _tree_sums(T, w):
+    A, c = T["a"], T["c"]
+    Ac = A @ c
+    return [(w.sum(), 1, 1.0), (w @ c, 2, 2.0), (w @ c**2, 3, 3.0), (w @ Ac, 3, 6.0), (w @ c**3, 4, 4.0), (w @ (c * Ac), 4, 8.0),
+            (w @ (A @ c**2), 4, 12.0), (w @ (A @ Ac), 4, 24.0)]
+
+
+def test_dense_output_weights_are_a_fourth_order_hermite_extension(oracle):
+    """w_i(theta) of reading A3 against what defines a continuous extension of order 4 (Hairer, Norsett & Wanner II.6):
+    the order conditions sum_i w_i(theta) Phi_i(tree) = theta^q / gamma(tree) for all 8 rooted trees with q <= 4, at
+    several theta -- a wrong coefficient d_i, a swapped stage or a wrong power of theta violates one of them -- and the
+    Hermite end conditions w(0) = 0, w(1) = b (the 5th-order weights), w'(0) = e_1, w'(1) = e_7 (C^1 across steps)."""
+    T = oracle.dp45_tableau()
+    for th in (0.0, 0.1, 1.0 / 3.0, 0.5, 0.77, 1.0):
+        w = oracle.dp45_dense_weights(th)
+        for got, q, gamma in _tree_sums(T, w):
+            assert abs(got - th**q / gamma) < 4e-16, (th, q, gamma, got)
+    assert np.all(oracle.dp45_dense_weights(0.0) == 0.0)
+    assert np.allclose(oracle.dp45_dense_weights(1.0), T["b5"], rtol=0, atol=1e-16)
+    e = 1e-6
+    d0 = (oracle.dp45_dense_weights(e) - oracle.dp45_dense_weights(0.0)) / e
+    d1 = (oracle.dp45_dense_weights(1.0) - oracle.dp45_dense_weights(1.0 - e)) / e
+    assert np.allclose(d0, np.eye(7)[0], atol=1e-5) and np.allclose(d1, np.eye(7)[6], atol=1e-5)
+    # it is NOT fifth order (the extension is one order below the propagated solution): the q = 5 bushy tree fails
+    w = oracle.dp45_dense_weights(0.5)
+    assert abs(w @ T["c"]**4 - 0.5**5 / 5.0) > 1e-6
+
+
+def test_dense_output_records_converge_with_fourth_order_and_match_step_states(oracle):
+    a = 0.5
+    st = W.kerr_bound(4000, a, W.SEED_BASE + 4)
+    st = np.ascontiguousarray(st[:, np.argsort(st[0])[:8]])
+    T_end, dtau = 24.0, 0.7                       # record times are NOT multiples of the step
+    ncap = int(T_end / dtau) + 2
+    ref = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.0125, np.inf, 1.0, 10**6, tau_end=T_end, snap_dtau=dtau,
+                                    snap_capacity=ncap, long_double=True)
+    errs = []
+    for k in (1, 2, 4):
+        r = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.4 / k, np.inf, 1.0, 10**6, tau_end=T_end, snap_dtau=dtau,
+                                      snap_capacity=ncap, long_double=True)
+        assert (r["snap_count"] == 1 + int(T_end / dtau)).all() and (r["rejected"] == 0).all()
+        valid = r["snapshots"][:, : 1 + int(T_end / dtau), :]
+        errs.append(np.abs(valid - ref["snapshots"][:, : 1 + int(T_end / dtau), :]).max(axis=(1, 2)))
+        assert np.isnan(r["snapshots"][:, 1 + int(T_end / dtau):, :]).all()          # nothing beyond the final time
+    q1, q2 = errs[0] / errs[1], errs[1] / errs[2]
+    assert np.median(q1) > 12.0 and np.median(q2) > 12.0, (q1, q2)                   # >= 2^4 up to the 5th-order part
+    assert errs[2].max() < 1e-6
+    # slot 0 = y0; a record that falls on a step boundary is that step's state (theta = 1: w = b)
+    h, every = 0.25, 4                                                                # records at tau = 1, 2, ...
+    r = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, h, np.inf, 1.0, 10**6, tau_end=6.0, snap_dtau=h * every, snap_capacity=8)
+    assert (r["snap_count"] == 7).all()
+    assert np.array_equal(r["snapshots"][:, 0, [1, 2, 3, 5, 6, 7]], st.T) and (r["snapshots"][:, 0, 0] == 0).all()
+    for j in (1, 3, 6):
+        rj = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, h, np.inf, 1.0, 10**6, tau_end=j * h * every)
+        assert np.abs(r["snapshots"][:, j, :] - rj["final_state"].T).max() < 1e-13
+
+
+def test_dense_output_stops_with_the_ray_and_respects_capacity(oracle):
+    a = 0.998
+    st = np.ascontiguousarray(W.camera_rays(64, a, 60.0)[:, ::37])
+    rc = W.horizon_radius(1.0, a) + 0.01
+    r = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.02, 1e-9, 1e-9, 200000, r_capture=rc, r_escape=1100.0,
+                                  kind=oracle.NULL, snap_dtau=25.0, snap_capacity=40, snap_mask=0x0F)
+    tau_rec = (r["snap_count"] - 1) * 25.0                        # time of the last record of each ray
+    t_last = r["final_state"][0]
+    assert (r["snap_count"] >= 40).all()                          # ~2100 M of affine time: capacity 40 overflows (S3) ...
+    assert np.isfinite(r["snapshots"]).all()                      # ... all 40 slots written, none beyond
+    full = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.02, 1e-9, 1e-9, 200000, r_capture=rc, r_escape=1100.0,
+                                     kind=oracle.NULL, snap_dtau=25.0, snap_capacity=200, snap_mask=0x0F)
+    assert np.array_equal(full["snap_count"], r["snap_count"]) and np.array_equal(full["snapshots"][:, :40], r["snapshots"])
+    cnt = full["snap_count"]
+    for i in range(st.shape[1]):
+        assert np.isnan(full["snapshots"][i, cnt[i]:]).all() and np.isfinite(full["snapshots"][i, : cnt[i]]).all()
+        tt = full["snapshots"][i, : cnt[i], 0]
+        assert (np.diff(tt) > 0).all() and tt[-1] <= t_last[i] + 1e-9            # coordinate time increases along the ray
+    assert (tau_rec > 0).all()

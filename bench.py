@@ -66,7 +66,7 @@ KERNEL_COUNTS = {
                  kernel="geo_rk4_kernel"),
     "schwarzschild": dict(sym="geo_rk4_kernelILb0ELi0ELb0", units_per_loop=2, flop=342.0, pipe=245.0, other=None, tol=0.0,
                           source="static SASS count of the hot loop (no ncu capture of this instantiation)", kernel="geo_rk4_kernel"),
-    "adaptive": dict(sym="geo_rk45_kernelILb1E", units_per_loop=1, flop=1045.0, pipe=684.0, other=None, tol=0.15, static_at_capture=(1135, 778),
+    "adaptive": dict(sym="geo_rk45_kernelILb1ELb0E", units_per_loop=1, flop=1045.0, pipe=684.0, other=None, tol=0.15, static_at_capture=(1135, 778),
                      source="ncu thread-level counts, profiles/r01_config3a_rk45.md: 361 DFMA + 271 DMUL + 52 DADD per attempt "
                             "(incl. predicated-on work of lanes waiting for a refill)", kernel="geo_rk45_kernel"),
     "tabulated": dict(sym="geo_tab_rk4_kernelILb0ELb1E", units_per_loop=None, flop=2217.0, pipe=1299.0, other=None, tol=None,

@@ -115,17 +115,25 @@ int geo_integrate_host(geo_ctx *ctx, const double *state_in, int64_t n, double h
  * with h_min = 0, a step that has shrunk to zero -- ends the particle with GEO_ST_NUMERIC.  tau_end: final value of the affine parameter,
  * landed on exactly ("the final evolution time is reached"; +INFINITY: none); reaching it, or
  * max_attempts (< 2^31, accepted + rejected), ends with GEO_ST_MAXSTEPS.  Capture / escape as in geo_stop
- * (capture guard on every stage point; flags must be 0).  out: as for geo_integrate, the snapshot fields are
- * ignored; steps_done = accepted steps.  rejected: DEVICE [n] int32 or NULL.  Enqueue-only on cuda_stream. */
+ * (capture guard on every stage point).  out: as for geo_integrate; steps_done = accepted steps.
+ * rejected: DEVICE [n] int32 or NULL.  Enqueue-only on cuda_stream.
+ * DENSE OUTPUT (reading A3): snap_dtau > 0 writes trajectory records at the FIXED affine times
+ * tau_j = j * snap_dtau, j = 0, 1, ... (slot 0 = the initial state), for every tau_j up to the last accepted state of the
+ * particle, from the pair's fourth-order continuous extension (the dense output of DOPRI5) -- no step is shortened for a
+ * record.  out->snapshots / snap_capacity / snap_mask / snap_count as for geo_integrate (records beyond the capacity are
+ * dropped, still counted).  snap_dtau = 0: no records, the snapshot fields of `out` are ignored.
+ * flags: 0 or GEO_FLAG_CARTESIAN_SNAP (records carry (x, y, z) of eq.(7)). */
 typedef struct geo_adaptive {
     double h0, rtol, atol, h_min, tau_end;
+    double snap_dtau; /* spacing of the dense-output records in tau; 0 = none */
 } geo_adaptive;
 int geo_integrate_adaptive(geo_ctx *ctx, const double *state_in, int64_t n, const geo_adaptive *ctl,
                            int64_t max_attempts, const geo_stop *stop, const geo_out *out, int32_t *rejected,
                            void *cuda_stream);
 
 /* Same operation with HOST buffers (state_in, every non-NULL output and `rejected` are host pointers; pinned lets the
- * copies run at full speed): H2D, launch, D2H, synchronise.  Device scratch is owned by the ctx. */
+ * copies run at full speed): H2D, launch, D2H, synchronise -- through the same double-buffered chunk pipeline as
+ * geo_integrate_host (record slots >= snap_count[i] come back as NaN).  Device scratch is owned by the ctx. */
 int geo_integrate_adaptive_host(geo_ctx *ctx, const double *state_in, int64_t n, const geo_adaptive *ctl,
                                 int64_t max_attempts, const geo_stop *stop, const geo_out *out, int32_t *rejected);
 

@@ -370,19 +370,22 @@ int geo_integrate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int
     return launch(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, (cudaStream_t)cuda_stream, ctx->counter);
 }
 
-// Host-buffer entry point.  Small jobs: one H2D, one launch, one D2H.  Jobs whose buffers exceed
-// kHostChunkBytes are cut into particle chunks that ping-pong between two device scratch slots on two
-// streams, so that the D2H of chunk k (the paper's measured bottleneck) overlaps the
-// kernel of chunk k+1, and the next kernel's CTAs fill the SMs the previous kernel's tail leaves idle.
-int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t nsteps,
-                       const geo_stop* stop, int64_t snapshot_every, const geo_out* out) {
-    int rc = validate(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, false);
-    if (rc != GEO_OK || n == 0) return rc;
-    GEO_ON_CTX_DEVICE(ctx);
+}  // extern "C"
+
+// Host-buffer pipeline shared by geo_integrate_host and geo_integrate_adaptive_host.  Small jobs: one H2D, one
+// launch, one D2H.  Jobs whose buffers exceed kHostChunkBytes are cut into particle chunks that ping-pong between two
+// device scratch slots on two streams, so that the D2H of chunk k (the paper's measured bottleneck)
+// overlaps the kernel of chunk k+1, and the next kernel's CTAs fill the SMs the previous kernel's tail leaves idle.
+// `enqueue(d_in, c, d_out, d_rejected, stream, counter)` launches the kernel for one chunk of c particles.
+// Arguments are validated by the caller; the ctx's device is current.
+template <class Enqueue>
+static int host_pipeline(geo_ctx* ctx, const double* state_in, int64_t n, const geo_out* out, bool with_snapshots,
+                         int32_t* rejected, Enqueue enqueue) {
     const size_t N = (size_t)n;
-    const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
-    const size_t snap_pp = snapshot_every > 0 ? (size_t)out->snap_capacity * ncomp * 8 : 0;   // bytes per particle
-    const size_t bytes_pp = 48 + 64 + 4 + 8 + (out->eq_cross_r ? 8 : 0) + (out->health ? 8 : 0) + (out->coarse_steps ? 4 : 0) + snap_pp + (snap_pp ? 4 : 0);
+    const int ncomp = with_snapshots ? popcount8(out->snap_mask) : 0;
+    const size_t snap_pp = with_snapshots ? (size_t)out->snap_capacity * ncomp * 8 : 0;   // bytes per particle
+    const size_t bytes_pp = 48 + 64 + 4 + 8 + (out->eq_cross_r ? 8 : 0) + (out->health ? 8 : 0) + (out->coarse_steps ? 4 : 0) +
+                            (rejected ? 4 : 0) + snap_pp + (snap_pp ? 4 : 0);
     // chunking: only when the transfers are large, never below ~2 waves of resident lanes per chunk
     const size_t kHostChunkBytes = (size_t)768 << 20;
     const size_t min_chunk = (size_t)ctx->sm_count * GEO_MIN_CTAS_PER_SM * kBlock * 2;
@@ -395,8 +398,9 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
     const size_t b_in = align256(6 * C * 8), b_fin = align256(8 * C * 8), b_st = align256(C * 4),
                  b_steps = align256(C * 8), b_eq = out->eq_cross_r ? align256(C * 8) : 0,
                  b_he = out->health ? align256(C * 8) : 0, b_sn = align256(C * snap_pp),
-                 b_sc = snap_pp ? align256(C * 4) : 0, b_co = out->coarse_steps ? align256(C * 4) : 0;
-    const size_t slot_bytes = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_sn + b_sc + b_co;
+                 b_sc = snap_pp ? align256(C * 4) : 0, b_co = out->coarse_steps ? align256(C * 4) : 0,
+                 b_rej = rejected ? align256(C * 4) : 0;
+    const size_t slot_bytes = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_sn + b_sc + b_co + b_rej;
     const size_t total = slot_bytes * nslots;
     cudaError_t e;
     for (int k = 0; k < nslots; ++k) {
@@ -436,6 +440,8 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
         d.snapshots = (double*)take(b_sn);
         d.snap_count = (int32_t*)take(b_sc);
         d.coarse_steps = (int32_t*)take(b_co);
+        int32_t* d_rej = (int32_t*)take(b_rej);
+        if (!snap_pp) d.snapshots = nullptr;
         e = cudaSuccess;
         for (int q = 0; q < 6 && e == cudaSuccess; ++q)      // SoA [6][n] -> [6][c]
             e = cudaMemcpyAsync(d_in + q * c, state_in + q * N + lo, c * 8, cudaMemcpyHostToDevice, s);
@@ -445,7 +451,7 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
             e = cudaMemsetAsync(d.snapshots, 0xFF, c * snap_pp, s);
             if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "memset snapshots"));
         }
-        rc = launch(ctx, d_in, (int64_t)c, h, nsteps, stop, snapshot_every, &d, s, ctx->counter + slot);
+        const int rc = enqueue(d_in, (int64_t)c, &d, d_rej, s, ctx->counter + slot);
         if (rc != GEO_OK) return bail(rc);
         for (int q = 0; q < 8 && e == cudaSuccess; ++q)      // SoA [8][c] -> [8][n]
             e = cudaMemcpyAsync(out->final_state + q * N + lo, d.final_state + q * c, c * 8, cudaMemcpyDeviceToHost, s);
@@ -457,6 +463,7 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
             e = cudaMemcpyAsync(reinterpret_cast<char*>(out->snapshots) + lo * snap_pp, d.snapshots, c * snap_pp, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess && d.snap_count) e = cudaMemcpyAsync(out->snap_count + lo, d.snap_count, c * 4, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess && d.coarse_steps) e = cudaMemcpyAsync(out->coarse_steps + lo, d.coarse_steps, c * 4, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess && d_rej) e = cudaMemcpyAsync(rejected + lo, d_rej, c * 4, cudaMemcpyDeviceToHost, s);
         if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "D2H outputs"));
     }
     for (int k = 0; k < nslots; ++k) {
@@ -464,6 +471,19 @@ int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h
         if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
     }
     return GEO_OK;
+}
+
+extern "C" {
+
+int geo_integrate_host(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t nsteps,
+                       const geo_stop* stop, int64_t snapshot_every, const geo_out* out) {
+    int rc = validate(ctx, state_in, n, h, nsteps, stop, snapshot_every, out, false);
+    if (rc != GEO_OK || n == 0) return rc;
+    GEO_ON_CTX_DEVICE(ctx);
+    return host_pipeline(ctx, state_in, n, out, snapshot_every > 0, nullptr,
+                         [&](const double* d_in, int64_t c, const geo_out* d, int32_t*, cudaStream_t s, unsigned long long* counter) {
+                             return launch(ctx, d_in, c, h, nsteps, stop, snapshot_every, d, s, counter);
+                         });
 }
 
 // Argument checks of the adaptive entry points (device and host variants).
@@ -478,14 +498,21 @@ static int validate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, co
         return fail(ctx, GEO_EINVAL, "rtol, atol must be >= 0, not both 0 (rtol = +inf: fixed step)");
     if (!(ctl->h_min >= 0.0) || !(ctl->tau_end > 0.0)) return fail(ctx, GEO_EINVAL, "h_min >= 0 and tau_end > 0 required");
     if (max_attempts < 0 || max_attempts > 0x7fffffffLL) return fail(ctx, GEO_EINVAL, "max_attempts must be in [0, 2^31)");
-    if (stop->flags != 0) return fail(ctx, GEO_EINVAL, "the adaptive path takes no flags");
+    if (stop->flags & ~GEO_FLAG_CARTESIAN_SNAP) return fail(ctx, GEO_EINVAL, "the adaptive path takes GEO_FLAG_CARTESIAN_SNAP only");
+    if (!(ctl->snap_dtau >= 0.0) || std::isinf(ctl->snap_dtau)) return fail(ctx, GEO_EINVAL, "snap_dtau must be finite and >= 0");
+    if (ctl->snap_dtau > 0.0 && n > 0) {
+        if (!out->snapshots || !out->snap_count) return fail(ctx, GEO_EINVAL, "snap_dtau > 0 needs snapshots and snap_count");
+        if (out->snap_capacity < 1 || out->snap_capacity > 0x7fffffffLL) return fail(ctx, GEO_EINVAL, "snap_capacity must be in [1, 2^31)");
+        if ((out->snap_mask & 0xFFu) == 0 || (out->snap_mask & ~0xFFu)) return fail(ctx, GEO_EINVAL, "snap_mask must select 1..8 of the 8 components");
+    }
     if (check_align && misaligned(rejected)) return fail(ctx, GEO_EINVAL, "device pointers must be 16-byte aligned");
     return GEO_OK;
 }
 
 // Enqueue the RK5(4) kernel on validated arguments (device pointers); the ctx's device is current.
 static int launch_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl, int64_t max_attempts,
-                           const geo_stop* stop, const geo_out* out, int32_t* rejected, cudaStream_t stream) {
+                           const geo_stop* stop, const geo_out* out, int32_t* rejected, cudaStream_t stream,
+                           unsigned long long* counter) {
     AdaptiveParams p;
     memset(&p, 0, sizeof p);
     p.in = state_in;
@@ -506,7 +533,15 @@ static int launch_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     p.eq_cross_r = out->eq_cross_r;
     p.health = out->health;
     p.rejected = rejected;
-    p.counter = ctx->counter;
+    p.counter = counter;
+    const bool dense = ctl->snap_dtau > 0.0;
+    p.snap_dtau = ctl->snap_dtau;
+    p.snaps = dense ? out->snapshots : nullptr;
+    p.snap_cap = dense ? out->snap_capacity : 0;
+    p.snap_mask = dense ? (out->snap_mask & 0xFFu) : 0;
+    p.ncomp = dense ? popcount8(out->snap_mask) : 0;
+    p.cartesian = (stop->flags & GEO_FLAG_CARTESIAN_SNAP) ? 1 : 0;
+    p.snap_count = dense ? out->snap_count : nullptr;
     p.bh.M = ctx->M;
     p.bh.a = ctx->a;
     p.bh.a2 = ctx->a * ctx->a;
@@ -514,14 +549,15 @@ static int launch_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     p.bh.twoMa = 2.0 * ctx->M * ctx->a;
     fill_trig_consts(p.bh.tc);
     typedef void (*fn_t)(const AdaptiveParams);
-    fn_t fn = ctx->metric == GEO_KERR ? (fn_t)geo_rk45_kernel<true> : (fn_t)geo_rk45_kernel<false>;
+    fn_t fn = ctx->metric == GEO_KERR ? (dense ? (fn_t)geo_rk45_kernel<true, true> : (fn_t)geo_rk45_kernel<true, false>)
+                                      : (dense ? (fn_t)geo_rk45_kernel<false, true> : (fn_t)geo_rk45_kernel<false, false>);
     int per_sm = 0;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, 0);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(rk45)");
     if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
     const int64_t need = (n + kBlock - 1) / kBlock, resident = (int64_t)ctx->sm_count * per_sm;
     const int grid = (int)(need < resident ? need : resident);
-    e = cudaMemsetAsync(ctx->counter, 0, sizeof(unsigned long long), stream);
+    e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
     fn<<<grid, kBlock, 0, stream>>>(p);
     e = cudaGetLastError();
@@ -535,67 +571,20 @@ int geo_integrate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     int rc = validate_adaptive(ctx, state_in, n, ctl, max_attempts, stop, out, rejected, true);
     if (rc != GEO_OK || n == 0) return rc;
     GEO_ON_CTX_DEVICE(ctx);
-    return launch_adaptive(ctx, state_in, n, ctl, max_attempts, stop, out, rejected, (cudaStream_t)cuda_stream);
+    if (ctl->snap_dtau > 0.0 && misaligned(out->snapshots)) return fail(ctx, GEO_EINVAL, "device pointers must be 16-byte aligned");
+    return launch_adaptive(ctx, state_in, n, ctl, max_attempts, stop, out, rejected, (cudaStream_t)cuda_stream, ctx->counter);
 }
 
-// Host-buffer entry point of the adaptive path: one H2D, one launch, one D2H per output, on the ctx's own stream.
-// Every argument is validated before the first copy is enqueued; after it, error paths drain the stream.
+// Host-buffer entry point of the adaptive path: the chunked double-buffered pipeline of geo_integrate_host.
 int geo_integrate_adaptive_host(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl,
                                 int64_t max_attempts, const geo_stop* stop, const geo_out* out, int32_t* rejected) {
     int rc = validate_adaptive(ctx, state_in, n, ctl, max_attempts, stop, out, rejected, false);
     if (rc != GEO_OK || n == 0) return rc;
     GEO_ON_CTX_DEVICE(ctx);
-    const size_t N = (size_t)n;
-    const size_t b_in = align256(6 * N * 8), b_fin = align256(8 * N * 8), b_st = align256(N * 4), b_steps = align256(N * 8),
-                 b_eq = out->eq_cross_r ? align256(N * 8) : 0, b_he = out->health ? align256(N * 8) : 0,
-                 b_rej = rejected ? align256(N * 4) : 0;
-    const size_t total = b_in + b_fin + b_st + b_steps + b_eq + b_he + b_rej + 256;
-    cudaError_t e;
-    if (!ctx->host_stream[0]) {
-        e = cudaStreamCreateWithFlags(&ctx->host_stream[0], cudaStreamNonBlocking);
-        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamCreate");
-    }
-    if (total > ctx->scratch_bytes) {
-        if (ctx->scratch) cudaFree(ctx->scratch);
-        ctx->scratch = nullptr;
-        ctx->scratch_bytes = 0;
-        e = cudaMalloc(&ctx->scratch, total);
-        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMalloc(scratch)");
-        ctx->scratch_bytes = total;
-    }
-    cudaStream_t s = ctx->host_stream[0];
-    char* base = static_cast<char*>(ctx->scratch);
-    size_t off = 0;
-    auto take = [&](size_t b) { char* q = b ? base + off : nullptr; off += b; return q; };
-    double* d_in = (double*)take(b_in);
-    geo_out d = *out;
-    d.final_state = (double*)take(b_fin);
-    d.status = (int32_t*)take(b_st);
-    d.steps_done = (int64_t*)take(b_steps);
-    d.eq_cross_r = (double*)take(b_eq);
-    d.health = (double*)take(b_he);
-    d.snapshots = nullptr;
-    d.snap_count = nullptr;
-    d.coarse_steps = nullptr;
-    int32_t* d_rej = (int32_t*)take(b_rej);
-    auto bail = [&](int code) {
-        cudaStreamSynchronize(s);
-        return code;
-    };
-    e = cudaMemcpyAsync(d_in, state_in, 6 * N * 8, cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "H2D state_in"));
-    rc = launch_adaptive(ctx, d_in, n, ctl, max_attempts, stop, &d, d_rej, s);
-    if (rc != GEO_OK) return bail(rc);
-    e = cudaMemcpyAsync(out->final_state, d.final_state, 8 * N * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out->status, d.status, N * 4, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out->steps_done, d.steps_done, N * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess && d.eq_cross_r) e = cudaMemcpyAsync(out->eq_cross_r, d.eq_cross_r, N * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess && d.health) e = cudaMemcpyAsync(out->health, d.health, N * 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess && d_rej) e = cudaMemcpyAsync(rejected, d_rej, N * 4, cudaMemcpyDeviceToHost, s);
-    if (e != cudaSuccess) return bail(fail_cuda(ctx, e, "D2H outputs"));
-    e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
-    return GEO_OK;
+    return host_pipeline(ctx, state_in, n, out, ctl->snap_dtau > 0.0, rejected,
+                         [&](const double* d_in, int64_t c, const geo_out* d, int32_t* d_rej, cudaStream_t s, unsigned long long* counter) {
+                             return launch_adaptive(ctx, d_in, c, ctl, max_attempts, stop, d, d_rej, s, counter);
+                         });
 }
 
 int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, int32_t info[4]) {

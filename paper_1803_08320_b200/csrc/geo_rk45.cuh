@@ -34,6 +34,14 @@ struct AdaptiveParams {
     double* health;
     int* rejected;      // [n] or null
     unsigned long long* counter;
+    // dense output (reading A3): records at tau_j = j * snap_dtau from the pair's continuous extension
+    double snap_dtau;   // 0: none
+    double* snaps;      // [n][snap_cap][ncomp]
+    long long snap_cap;
+    unsigned snap_mask;
+    int ncomp;
+    int cartesian;
+    int* snap_count;
     Hole bh;
 };
 
@@ -45,6 +53,9 @@ constexpr double a41 = 44.0 / 45, a42 = -56.0 / 15, a43 = 32.0 / 9;
 constexpr double a51 = 19372.0 / 6561, a52 = -25360.0 / 2187, a53 = 64448.0 / 6561, a54 = -212.0 / 729;
 constexpr double a61 = 9017.0 / 3168, a62 = -355.0 / 33, a63 = 46732.0 / 5247, a64 = 49.0 / 176, a65 = -5103.0 / 18656;
 constexpr double b1 = 35.0 / 384, b3 = 500.0 / 1113, b4 = 125.0 / 192, b5 = -2187.0 / 6784, b6 = 11.0 / 84;
+// dense output (Hairer's dopri5, "contd5"): coefficients of the fifth interpolation term
+constexpr double d1 = -12715105075.0 / 11282082432.0, d3 = 87487479700.0 / 32700410799.0, d4 = -10690763975.0 / 1880347072.0,
+                 d5 = 701980252875.0 / 199316789632.0, d6 = -1453857185.0 / 822651844.0, d7 = 69997945.0 / 29380423.0;
 constexpr double e1 = 35.0 / 384 - 5179.0 / 57600, e3 = 500.0 / 1113 - 7571.0 / 16695, e4 = 125.0 / 192 - 393.0 / 640,
                  e5 = -2187.0 / 6784 + 92097.0 / 339200, e6 = 11.0 / 84 - 187.0 / 2100, e7 = -1.0 / 40;
 }  // namespace dp
@@ -84,8 +95,18 @@ __device__ __forceinline__ void rhs_at(const Hole& bh, double r, double th, doub
 
 __device__ __forceinline__ K4 k4_of(const Deriv& d) { return K4{d.r, d.th, d.pr, d.pth}; }
 
-template <bool KERR>
-__global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
+// One component of the continuous extension at theta in [0, 1] (reading A3), nested as in dopri5's contd5:
+//   y + theta (r2 + theta1 (r3 + theta (r4 + theta1 r5))),  r2 = ynew - y, r3 = h k1 - r2, r4 = r2 - h k7 - r3, r5 = h sum d_i k_i
+__device__ __forceinline__ double contd5(double theta, double y, double ynew, double hk1, double hk7, double hdk) {
+    const double th1 = 1.0 - theta;
+    const double r2 = ynew - y, r3 = hk1 - r2, r4 = r2 - hk7 - r3;
+    return fma(theta, fma(th1, fma(theta, fma(th1, hdk, r4), r3), r2), y);
+}
+
+// DENSE: dense-output records (geo_adaptive.snap_dtau > 0); a separate instantiation so that the plain kernel keeps its
+// register budget.
+template <bool KERR, bool DENSE>
+__global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
     const unsigned lane = threadIdx.x & 31u;
     const Hole& bh = p.bh;
     long long idx = -1;
@@ -98,6 +119,17 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
     int steps = 0, attempts = 0, rejected = 0;
     double eqc = 0;
     bool crossed = false;
+    int next_j = 0;                                                  // DENSE: records produced = index of the next one
+
+    // DENSE: one record (paper order; components 1..3 optionally Cartesian, eq.(7)) into slot j of this particle
+    auto write_record = [&](int j, double rt, double rr, double rth, double rph, double rpr, double rpth) {
+        if (j < p.snap_cap) {                                        // S3: drop beyond capacity, keep counting
+            double c1 = rr, c2 = rth, c3 = rph;
+            if (p.cartesian) cartesian_eq7(bh.tc, bh.a2, rr, rth, rph, c1, c2, c3);
+            double* dst = p.snaps + ((size_t)idx * (size_t)p.snap_cap + (size_t)j) * p.ncomp;
+            store_record_global(dst, p.snap_mask, rt, c1, c2, c3, E, rpr, rpth, L);
+        }
+    };
 
     auto finish = [&](int st) {
         long long n = p.n;
@@ -115,6 +147,7 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
         if (p.eq_cross_r) p.eq_cross_r[idx] = crossed ? eqc : __longlong_as_double(0x7ff8000000000000LL);
         if (p.health) p.health[idx] = health_3p1(bh, r, th, pr, pth, E, L, p.kappa);
         if (p.rejected) p.rejected[idx] = rejected;
+        if (DENSE) p.snap_count[idx] = next_j;
         active = false;
     };
     auto begin = [&](long long i) {
@@ -134,8 +167,10 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
         steps = attempts = rejected = 0;
         crossed = false;
         active = true;
+        next_j = 0;
         if (!(r >= p.r_capture)) { finish(ST_CAPTURED); return; }               // B1
         if (!all_finite6(r, th, ph, pr, pth, E)) { finish(ST_NUMERIC); return; }
+        if (DENSE) { write_record(0, t, r, th, ph, pr, pth); next_j = 1; }      // record 0 = y0 (tau = 0)
         if (r > p.r_escape) { finish(ST_ESCAPED); return; }
         if (p.max_attempts == 0) { finish(ST_MAXSTEPS); return; }
         rhs_at<KERR>(bh, r, th, pr, pth, E, L, k1);
@@ -171,6 +206,8 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
         const K4 q1 = k4_of(k1);
         double s5t = dp::b1 * k1.t, s5p = dp::b1 * k1.ph;                        // b5 . k for the cyclic t, phi
         double set_ = dp::e1 * k1.t, sep = dp::e1 * k1.ph;                       // (b5 - b4) . k
+        double sdt = 0, sdp = 0;                                                 // DENSE: d . k for t, phi
+        if (DENSE) { sdt = dp::d1 * k1.t; sdp = dp::d1 * k1.ph; }
         // stage 2
         sr = fma(h * dp::a21, q1.r, r); sth = fma(h * dp::a21, q1.th, th);
         spr = fma(h * dp::a21, q1.pr, pr); spth = fma(h * dp::a21, q1.pth, pth);
@@ -184,6 +221,7 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
         rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
         const K4 q3 = k4_of(d);
         s5t = fma(dp::b3, d.t, s5t); s5p = fma(dp::b3, d.ph, s5p);
+        if (DENSE) { sdt = fma(dp::d3, d.t, sdt); sdp = fma(dp::d3, d.ph, sdp); }
         set_ = fma(dp::e3, d.t, set_); sep = fma(dp::e3, d.ph, sep);
         // stage 4
 #define GEO_S4(c) fma(dp::a43, q3.c, fma(dp::a42, q2.c, dp::a41 * q1.c))
@@ -193,6 +231,7 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
         rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
         const K4 q4 = k4_of(d);
         s5t = fma(dp::b4, d.t, s5t); s5p = fma(dp::b4, d.ph, s5p);
+        if (DENSE) { sdt = fma(dp::d4, d.t, sdt); sdp = fma(dp::d4, d.ph, sdp); }
         set_ = fma(dp::e4, d.t, set_); sep = fma(dp::e4, d.ph, sep);
         // stage 5
 #define GEO_S5(c) fma(dp::a54, q4.c, fma(dp::a53, q3.c, fma(dp::a52, q2.c, dp::a51 * q1.c)))
@@ -202,6 +241,7 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
         rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
         const K4 q5 = k4_of(d);
         s5t = fma(dp::b5, d.t, s5t); s5p = fma(dp::b5, d.ph, s5p);
+        if (DENSE) { sdt = fma(dp::d5, d.t, sdt); sdp = fma(dp::d5, d.ph, sdp); }
         set_ = fma(dp::e5, d.t, set_); sep = fma(dp::e5, d.ph, sep);
         // stage 6
 #define GEO_S6(c) fma(dp::a65, q5.c, fma(dp::a64, q4.c, fma(dp::a63, q3.c, fma(dp::a62, q2.c, dp::a61 * q1.c))))
@@ -211,6 +251,7 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
         rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
         const K4 q6 = k4_of(d);
         s5t = fma(dp::b6, d.t, s5t); s5p = fma(dp::b6, d.ph, s5p);
+        if (DENSE) { sdt = fma(dp::d6, d.t, sdt); sdp = fma(dp::d6, d.ph, sdp); }
         set_ = fma(dp::e6, d.t, set_); sep = fma(dp::e6, d.ph, sep);
         // 5th-order solution, Kahan-compensated (committed only on acceptance); stage 7 sits on it
 #define GEO_B5(c) fma(dp::b6, q6.c, fma(dp::b5, q5.c, fma(dp::b4, q4.c, fma(dp::b3, q3.c, dp::b1 * q1.c))))
@@ -261,11 +302,32 @@ __global__ void __launch_bounds__(kBlock, GEO_RK45_CTAS) geo_rk45_kernel(const _
                         eqc = r + (nr - r) * (half_pi - th) / (nth - th);
                     }
                 }
+                const double tau_new = last ? p.tau_end : tau + h;               // the final time is landed on exactly
+                if (DENSE) {                                                     // A3: every record time in (tau, tau_new]
+                    double tj = (double)next_j * p.snap_dtau;
+                    if (tj <= tau_new) {
+                        // h sum_i d_i k_i per component (t, phi from the stage sums carried for them)
+#define GEO_D(c) fma(dp::d7, k7.c, fma(dp::d6, q6.c, fma(dp::d5, q5.c, fma(dp::d4, q4.c, fma(dp::d3, q3.c, dp::d1 * q1.c)))))
+                        const double hdt = h * fma(dp::d7, k7.t, sdt), hdp = h * fma(dp::d7, k7.ph, sdp);
+                        const double hdr = h * GEO_D(r), hdth = h * GEO_D(th), hdpr = h * GEO_D(pr), hdpth = h * GEO_D(pth);
+#undef GEO_D
+                        const double ih = 1.0 / h;
+                        do {
+                            const double theta = (tj - tau) * ih;
+                            write_record(next_j,
+                                         contd5(theta, t, nt, h * k1.t, h * k7.t, hdt), contd5(theta, r, nr, h * q1.r, h * k7.r, hdr),
+                                         contd5(theta, th, nth, h * q1.th, h * k7.th, hdth), contd5(theta, ph, nph, h * k1.ph, h * k7.ph, hdp),
+                                         contd5(theta, pr, npr, h * q1.pr, h * k7.pr, hdpr), contd5(theta, pth, npth, h * q1.pth, h * k7.pth, hdpth));
+                            ++next_j;
+                            tj = (double)next_j * p.snap_dtau;
+                        } while (tj <= tau_new);
+                    }
+                }
                 t = nt; r = nr; th = nth; ph = nph; pr = npr; pth = npth;
                 ct = dt; cr = dr; cth = dth; cph = dph; cpr = dpr; cpth = dpth;
                 k1 = k7;                                                         // first same as last
                 ++steps;
-                tau += h;
+                tau = tau_new;
                 h *= fac;
                 if (r > p.r_escape) finish(ST_ESCAPED);                          // B3
                 else if (last || attempts >= p.max_attempts) finish(ST_MAXSTEPS);   // final time / cap

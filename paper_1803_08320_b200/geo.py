@@ -41,7 +41,7 @@ class GeoOut(C.Structure):
 
 class GeoAdaptive(C.Structure):
     _fields_ = [("h0", C.c_double), ("rtol", C.c_double), ("atol", C.c_double), ("h_min", C.c_double),
-                ("tau_end", C.c_double)]
+                ("tau_end", C.c_double), ("snap_dtau", C.c_double)]
 
 
 class GeoTable(C.Structure):
@@ -234,14 +234,15 @@ def geo_integrate(ctx, state_in, h: float, nsteps: int, out: dict, r_capture: fl
 
 def geo_integrate_adaptive(ctx, state_in, h0: float, rtol: float, atol: float, max_attempts: int, out: dict,
                            r_capture: float = -float("inf"), r_escape: float = float("inf"), kind: int = TIMELIKE,
-                           h_min: float = 1e-12, tau_end: float = float("inf"), rejected=None, stream=None) -> None:
+                           h_min: float = 1e-12, tau_end: float = float("inf"), rejected=None, stream=None,
+                           snap_dtau: float = 0.0, flags: int = 0) -> None:
     """Enqueue the adaptive RK5(4) integration (include/geo.h: geo_integrate_adaptive).  ``rejected``: optional
-    CUDA int32 tensor [n].  Does not synchronise."""
+    CUDA int32 tensor [n].  ``snap_dtau`` > 0: dense-output records into out["snapshots"].  Does not synchronise."""
     import torch
     n = _check_buffers(state_in, out, device=True, rejected=rejected)
     s = stream if stream is not None else torch.cuda.current_stream(state_in.device)
-    stop = GeoStop(r_capture, r_escape, kind, 0)
-    ctl = GeoAdaptive(h0, rtol, atol, h_min, tau_end)
+    stop = GeoStop(r_capture, r_escape, kind, flags)
+    ctl = GeoAdaptive(h0, rtol, atol, h_min, tau_end, snap_dtau)
     o = _out_struct(out)
     L = lib()
     with torch.cuda.device(state_in.device):
@@ -252,11 +253,12 @@ def geo_integrate_adaptive(ctx, state_in, h0: float, rtol: float, atol: float, m
 
 def geo_integrate_adaptive_host(ctx, state_in, h0: float, rtol: float, atol: float, max_attempts: int, out: dict,
                                 r_capture: float = -float("inf"), r_escape: float = float("inf"), kind: int = TIMELIKE,
-                                h_min: float = 1e-12, tau_end: float = float("inf"), rejected=None) -> None:
+                                h_min: float = 1e-12, tau_end: float = float("inf"), rejected=None,
+                                snap_dtau: float = 0.0, flags: int = 0) -> None:
     """The adaptive RK5(4) integration on HOST buffers (numpy arrays or pinned CPU tensors); synchronous."""
     n = _check_buffers(state_in, out, device=False, rejected=rejected)
-    stop = GeoStop(r_capture, r_escape, kind, 0)
-    ctl = GeoAdaptive(h0, rtol, atol, h_min, tau_end)
+    stop = GeoStop(r_capture, r_escape, kind, flags)
+    ctl = GeoAdaptive(h0, rtol, atol, h_min, tau_end, snap_dtau)
     o = _out_struct(out)
     L = lib()
     _check(ctx, L.geo_integrate_adaptive_host(ctx, _ptr(state_in), n, C.byref(ctl), max_attempts, C.byref(stop),

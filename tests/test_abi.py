@@ -34,7 +34,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(geo.GeoStop) == 24
     assert ctypes.sizeof(geo.GeoOut) == 10 * 8 and geo.GeoOut.coarse_steps.offset == 72
     assert geo.GeoOut.snap_mask.offset == 56 and geo.GeoOut.snap_count.offset == 64
-    assert ctypes.sizeof(geo.GeoTable) == 56 and ctypes.sizeof(geo.GeoAdaptive) == 40
+    assert ctypes.sizeof(geo.GeoTable) == 56 and ctypes.sizeof(geo.GeoAdaptive) == 48
 
 
 def test_sass_has_fp64_pipe_and_wide_stores():

@@ -33,6 +33,17 @@
 //       geo_oracle.cpp with r -> x^1, theta -> x^2; per evaluation point the capture test comes first,
 //       then the domain test.  No snapshots.
 //
+//   T6  (round 2) GENERAL stationary, axisymmetric 3+1 metric: all TEN functions of line element (1) --
+//       alpha, beta^1, beta^2, beta^3, gamma_11, gamma_12, gamma_13, gamma_22, gamma_23, gamma_33 (x^3 = phi) -- of
+//       (x^1, x^2), tab[f][j][i] in that order; no circularity, no diagonal 3-metric assumed (e.g. Kerr in horizon-
+//       penetrating Kerr-Schild coordinates: beta^r != 0, gamma_r phi != 0).  Same interpolant (T2), domain (T4), stepper
+//       and stop rules (T5).  With p = (p_1, p_2, L), gamma^{ij} the inverse of gamma_ij, V^i = gamma^{ij} p_j,
+//       W = E + beta^k p_k, u^t = W / alpha^2:
+//           H = 1/2 [ -W^2/alpha^2 + gamma^{ij} p_i p_j ]                                   (eq.(4) with eq.(1))
+//           dt/dtau = u^t,   dx^i/dtau = V^i - beta^i u^t   (i = 1, 2, 3)
+//           dp_k/dtau = -alpha (u^t)^2 d_k alpha + u^t p_j d_k beta^j + 1/2 V^a V^b d_k gamma_ab   (k = 1, 2);  dL/dtau = 0
+//       (from d_k gamma^{ij} = -gamma^{ia} gamma^{jb} d_k gamma_ab), E = alpha sqrt(kappa + gamma^{ij} p_i p_j) - beta^k p_k.
+//
 // Pins (tests/test_oracle_tabulated.py): the interpolant against Keys' kernel form, node values, quadratic
 // exactness, C^1 continuity; the RHS against finite differences of H on a metric with quadratic-polynomial
 // fields (where the interpolant is exact); flat space in spherical coordinates against the straight line's
@@ -261,6 +272,183 @@ void integrate_range(const Table& m, const double* state_in, int64_t n, double h
     for (int64_t i = lo; i < hi; ++i) integrate_one<R>(m, state_in, n, i, (R)h, nsteps, st, o);
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// T6: general stationary axisymmetric 3+1 metric, ten fields
+// ---------------------------------------------------------------------------------------------------------------
+enum { G_ALPHA = 0, G_B1 = 1, G_B2 = 2, G_B3 = 3, G_G11 = 4, G_G12 = 5, G_G13 = 6, G_G22 = 7, G_G23 = 8, G_G33 = 9, G_NF = 10 };
+template <class R> struct GFields { R f[G_NF], d1[G_NF], d2[G_NF]; };
+
+template <class R> bool interpolate_general(const Table& m, R x1, R x2, GFields<R>& F) {
+    const R u1 = (x1 - (R)m.x1_0) / (R)m.d1, u2 = (x2 - (R)m.x2_0) / (R)m.d2;
+    const R fl1 = std::floor(u1), fl2 = std::floor(u2);
+    if (!(fl1 >= R(1) && fl1 <= (R)(m.n1 - 3) && fl2 >= R(1) && fl2 <= (R)(m.n2 - 3))) return false;
+    const int64_t i = (int64_t)fl1, j = (int64_t)fl2;
+    R w1[4], dw1[4], w2[4], dw2[4];
+    keys_weights(u1 - fl1, w1, dw1);
+    keys_weights(u2 - fl2, w2, dw2);
+    for (int f = 0; f < G_NF; ++f) {
+        const double* T = m.tab + (int64_t)f * m.n1 * m.n2;
+        R v = 0, v1 = 0, v2 = 0;
+        for (int b = 0; b < 4; ++b)
+            for (int a = 0; a < 4; ++a) {
+                const R node = (R)T[(j - 1 + b) * m.n1 + (i - 1 + a)];
+                v += w2[b] * w1[a] * node;
+                v1 += w2[b] * dw1[a] * node;
+                v2 += dw2[b] * w1[a] * node;
+            }
+        F.f[f] = v;
+        F.d1[f] = v1 / (R)m.d1;
+        F.d2[f] = v2 / (R)m.d2;
+    }
+    return true;
+}
+
+// gamma^{ij} (symmetric 3 x 3 inverse by the adjugate) as [11, 12, 13, 22, 23, 33]
+template <class R> void inverse3(const R* f, R gi[6]) {
+    const R a = f[G_G11], b = f[G_G12], c = f[G_G13], d = f[G_G22], e = f[G_G23], g = f[G_G33];
+    const R c11 = d * g - e * e, c12 = c * e - b * g, c13 = b * e - c * d;
+    const R det = a * c11 + b * c12 + c * c13;
+    gi[0] = c11 / det; gi[1] = c12 / det; gi[2] = c13 / det;
+    gi[3] = (a * g - c * c) / det; gi[4] = (b * c - a * e) / det; gi[5] = (a * d - b * b) / det;
+}
+
+template <class R> struct GAux { R V[3], W, ut, gpp; };     // V^i, W, u^t, gamma^{ij} p_i p_j
+template <class R> GAux<R> aux_general(const GFields<R>& F, R p1, R p2, R L, R E) {
+    R gi[6];
+    inverse3(F.f, gi);
+    GAux<R> A;
+    A.V[0] = gi[0] * p1 + gi[1] * p2 + gi[2] * L;
+    A.V[1] = gi[1] * p1 + gi[3] * p2 + gi[4] * L;
+    A.V[2] = gi[2] * p1 + gi[4] * p2 + gi[5] * L;
+    A.gpp = A.V[0] * p1 + A.V[1] * p2 + A.V[2] * L;
+    A.W = E + F.f[G_B1] * p1 + F.f[G_B2] * p2 + F.f[G_B3] * L;
+    A.ut = A.W / (F.f[G_ALPHA] * F.f[G_ALPHA]);
+    return A;
+}
+
+template <class R> Deriv<R> rhs_general(const GFields<R>& F, const State<R>& y) {
+    const GAux<R> A = aux_general(F, y.p1, y.p2, y.L, y.E);
+    const R al = F.f[G_ALPHA];
+    Deriv<R> d;
+    d.t = A.ut;
+    d.x1 = A.V[0] - F.f[G_B1] * A.ut;
+    d.x2 = A.V[1] - F.f[G_B2] * A.ut;
+    d.ph = A.V[2] - F.f[G_B3] * A.ut;
+    const R* D[2] = {F.d1, F.d2};
+    R dp[2];
+    for (int k = 0; k < 2; ++k) {
+        const R* q = D[k];
+        const R VVdg = A.V[0] * A.V[0] * q[G_G11] + A.V[1] * A.V[1] * q[G_G22] + A.V[2] * A.V[2] * q[G_G33] +
+                       R(2) * (A.V[0] * A.V[1] * q[G_G12] + A.V[0] * A.V[2] * q[G_G13] + A.V[1] * A.V[2] * q[G_G23]);
+        dp[k] = -al * A.ut * A.ut * q[G_ALPHA] + A.ut * (y.p1 * q[G_B1] + y.p2 * q[G_B2] + y.L * q[G_B3]) + VVdg / R(2);
+    }
+    d.p1 = dp[0];
+    d.p2 = dp[1];
+    return d;
+}
+
+template <class R> R hamiltonian_general(const GFields<R>& F, const State<R>& y) {
+    const GAux<R> A = aux_general(F, y.p1, y.p2, y.L, y.E);
+    return (-(A.W * A.W) / (F.f[G_ALPHA] * F.f[G_ALPHA]) + A.gpp) / R(2);
+}
+
+template <class R> R energy_general(const GFields<R>& F, R p1, R p2, R L, R kappa) {
+    const GAux<R> A = aux_general(F, p1, p2, L, R(0));
+    return F.f[G_ALPHA] * std::sqrt(kappa + A.gpp) - (F.f[G_B1] * p1 + F.f[G_B2] * p2 + F.f[G_B3] * L);
+}
+
+// T5 with the T6 right-hand side: the loop of integrate_one, written out again for the general fields
+template <class R>
+void integrate_one_general(const Table& m, const double* state_in, int64_t n, int64_t i, R h, int64_t nsteps,
+                           const StopRule& st, const OutPtrs& o) {
+    const R kappa = st.kind == 0 ? R(1) : R(0);
+    const bool plain = (st.flags & 1) != 0;
+    const R rc = (R)st.r_capture, re = (R)st.r_escape;
+    const R half_pi = (R)1.5707963267948966;
+    State<R> y;
+    y.t = R(0);
+    y.x1 = (R)state_in[0 * n + i];
+    y.x2 = (R)state_in[1 * n + i];
+    y.ph = (R)state_in[2 * n + i];
+    y.p1 = (R)state_in[3 * n + i];
+    y.p2 = (R)state_in[4 * n + i];
+    y.L = (R)state_in[5 * n + i];
+    y.E = std::numeric_limits<R>::quiet_NaN();
+    R ct = 0, c1 = 0, c2 = 0, cph = 0, cp1 = 0, cp2 = 0;
+    int32_t status = -1;
+    int64_t steps = 0;
+    R eq_cross = std::numeric_limits<R>::quiet_NaN();
+    bool crossed = false;
+    GFields<R> F;
+    if (!(y.x1 >= rc)) status = TAB_ST_CAPTURED;
+    else if (!finite6(y) || !std::isfinite(y.L)) status = TAB_ST_NUMERIC;
+    else if (!interpolate_general(m, y.x1, y.x2, F)) status = TAB_ST_OUTSIDE;
+    else {
+        y.E = energy_general(F, y.p1, y.p2, y.L, kappa);
+        if (!std::isfinite(y.E)) status = TAB_ST_NUMERIC;
+        else if (y.x1 > re) status = TAB_ST_ESCAPED;
+        else if (nsteps == 0) status = TAB_ST_MAXSTEPS;
+    }
+    while (status < 0) {
+        const Deriv<R> k1 = rhs_general(F, y);
+        const State<R> y2 = shifted(y, h / R(2), k1);
+        GFields<R> G;
+        if (!(y2.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }
+        if (!interpolate_general(m, y2.x1, y2.x2, G)) { status = TAB_ST_OUTSIDE; break; }
+        const Deriv<R> k2 = rhs_general(G, y2);
+        const State<R> y3 = shifted(y, h / R(2), k2);
+        if (!(y3.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }
+        if (!interpolate_general(m, y3.x1, y3.x2, G)) { status = TAB_ST_OUTSIDE; break; }
+        const Deriv<R> k3 = rhs_general(G, y3);
+        const State<R> y4 = shifted(y, h, k3);
+        if (!(y4.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }
+        if (!interpolate_general(m, y4.x1, y4.x2, G)) { status = TAB_ST_OUTSIDE; break; }
+        const Deriv<R> k4 = rhs_general(G, y4);
+        State<R> yn = y;
+        R nt = ct, n1 = c1, n2 = c2, nph = cph, np1 = cp1, np2 = cp2;
+        const R w = h / R(6);
+        kahan_add(yn.t, nt, w * (k1.t + R(2) * k2.t + R(2) * k3.t + k4.t), plain);
+        kahan_add(yn.x1, n1, w * (k1.x1 + R(2) * k2.x1 + R(2) * k3.x1 + k4.x1), plain);
+        kahan_add(yn.x2, n2, w * (k1.x2 + R(2) * k2.x2 + R(2) * k3.x2 + k4.x2), plain);
+        kahan_add(yn.ph, nph, w * (k1.ph + R(2) * k2.ph + R(2) * k3.ph + k4.ph), plain);
+        kahan_add(yn.p1, np1, w * (k1.p1 + R(2) * k2.p1 + R(2) * k3.p1 + k4.p1), plain);
+        kahan_add(yn.p2, np2, w * (k1.p2 + R(2) * k2.p2 + R(2) * k3.p2 + k4.p2), plain);
+        if (!(yn.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }
+        if (!finite6(yn)) { status = TAB_ST_NUMERIC; break; }
+        if (!interpolate_general(m, yn.x1, yn.x2, G)) { status = TAB_ST_OUTSIDE; break; }
+        if (!crossed) {
+            const R d0 = y.x2 - half_pi, d1 = yn.x2 - half_pi;
+            if (d0 * d1 < R(0)) {
+                crossed = true;
+                eq_cross = y.x1 + (yn.x1 - y.x1) * (half_pi - y.x2) / (yn.x2 - y.x2);
+            }
+        }
+        y = yn; ct = nt; c1 = n1; c2 = n2; cph = nph; cp1 = np1; cp2 = np2;
+        F = G;
+        ++steps;
+        if (y.x1 > re) status = TAB_ST_ESCAPED;
+        else if (steps >= nsteps) status = TAB_ST_MAXSTEPS;
+    }
+    const R comp[8] = {y.t, y.x1, y.x2, y.ph, y.E, y.p1, y.p2, y.L};
+    for (int k = 0; k < 8; ++k) o.final_state[(int64_t)k * n + i] = (double)comp[k];
+    o.status[i] = status;
+    o.steps_done[i] = steps;
+    if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
+    if (o.health) {
+        GFields<R> H;
+        o.health[i] = (std::isfinite(y.E) && interpolate_general(m, y.x1, y.x2, H))
+                          ? (double)std::fabs(R(2) * hamiltonian_general(H, y) + kappa)
+                          : std::numeric_limits<double>::quiet_NaN();
+    }
+}
+
+template <class R>
+void integrate_range_general(const Table& m, const double* state_in, int64_t n, double h, int64_t nsteps,
+                             const StopRule& st, const OutPtrs& o, int64_t lo, int64_t hi) {
+    for (int64_t i = lo; i < hi; ++i) integrate_one_general<R>(m, state_in, n, i, (R)h, nsteps, st, o);
+}
+
 }  // namespace
 
 extern "C" {
@@ -306,6 +494,42 @@ int oracle_tab_rhs(const double* tab, int64_t n1, int64_t n2, double x1_0, doubl
     const Deriv<double> d = rhs_fields(F, y);
     d6[0] = d.t; d6[1] = d.x1; d6[2] = d.x2; d6[3] = d.ph; d6[4] = d.p1; d6[5] = d.p2;
     if (H) *H = hamiltonian_fields(F, y);
+    return 1;
+}
+
+// ---- T6: general ten-field tables, tab = [10][n2][n1] ----
+int oracle_tabg_integrate(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+                          const double* state_in, int64_t n, double h, int64_t nsteps, const StopRule* st,
+                          const OutPtrs* out, int precision, int nthreads) {
+    if (!tab || n1 < 4 || n2 < 4 || !(d1 > 0) || !(d2 > 0) || n < 0 || nsteps < 0 || !st || !out) return 1;
+    const Table m{tab, n1, n2, x1_0, d1, x2_0, d2};
+    if (nthreads < 1) nthreads = 1;
+    std::vector<std::thread> pool;
+    const int64_t per = (n + nthreads - 1) / nthreads;
+    for (int t = 0; t < nthreads; ++t) {
+        const int64_t lo = t * per, hi = std::min<int64_t>(n, lo + per);
+        if (lo >= hi) break;
+        if (precision == 1)
+            pool.emplace_back(integrate_range_general<long double>, m, state_in, n, h, nsteps, *st, *out, lo, hi);
+        else
+            pool.emplace_back(integrate_range_general<double>, m, state_in, n, h, nsteps, *st, *out, lo, hi);
+    }
+    for (auto& th : pool) th.join();
+    return 0;
+}
+
+// RHS (T6) at y8 = (t, x1, x2, phi, E, p1, p2, L): d6 = d/dtau of (t, x1, x2, phi, p1, p2); *H = Hamiltonian;
+// E_out (optional) = mass-shell energy for kappa.  Returns 1 inside the domain, 0 outside.
+int oracle_tabg_rhs(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+                    const double* y8, double* d6, double* H, double kappa, double* E_out) {
+    const Table m{tab, n1, n2, x1_0, d1, x2_0, d2};
+    GFields<double> F;
+    State<double> y{y8[0], y8[1], y8[2], y8[3], y8[4], y8[5], y8[6], y8[7]};
+    if (!interpolate_general<double>(m, y.x1, y.x2, F)) return 0;
+    const Deriv<double> d = rhs_general(F, y);
+    d6[0] = d.t; d6[1] = d.x1; d6[2] = d.x2; d6[3] = d.ph; d6[4] = d.p1; d6[5] = d.p2;
+    if (H) *H = hamiltonian_general(F, y);
+    if (E_out) *E_out = energy_general(F, y.p1, y.p2, y.L, kappa);
     return 1;
 }
 

@@ -45,9 +45,9 @@ def lib():
     return _lib
 
 
-def _grid(table: dict):
+def _grid(table: dict, nf: int = 5):
     tab = table["tab"]
-    assert tab.dtype == np.float64 and tab.flags.c_contiguous and tab.ndim == 3 and tab.shape[0] == 5
+    assert tab.dtype == np.float64 and tab.flags.c_contiguous and tab.ndim == 3 and tab.shape[0] == nf
     return [tab.ctypes.data, tab.shape[2], tab.shape[1], table["x1_0"], table["d1"], table["x2_0"], table["d2"]]
 
 
@@ -81,4 +81,39 @@ def integrate(table: dict, state_in: np.ndarray, h: float, nsteps: int, r_captur
                                     int(long_double), nthreads)
     if rc != 0:
         raise ValueError("oracle_tab_integrate: invalid arguments")
+    return res
+
+
+# ---- reading T6: general stationary axisymmetric 3+1 metric, tab [10][n2][n1] =
+#      alpha, beta^1, beta^2, beta^3, gamma_11, gamma_12, gamma_13, gamma_22, gamma_23, gamma_33 ----
+def rhs_general(table: dict, y8, kappa: float = 1.0):
+    """(d/dtau of (t, x1, x2, phi, p1, p2), H, mass-shell E) at y8 = (t, x1, x2, phi, E, p1, p2, L); None outside."""
+    y = np.ascontiguousarray(y8, dtype=np.float64)
+    d, H, E = np.zeros(6), C.c_double(), C.c_double()
+    L = lib()
+    L.oracle_tabg_rhs.restype = C.c_int
+    L.oracle_tabg_rhs.argtypes = _GRID + [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
+    ok = L.oracle_tabg_rhs(*_grid(table, 10), y.ctypes.data, d.ctypes.data, C.byref(H), kappa, C.byref(E))
+    return (d, H.value, E.value) if ok else None
+
+
+def integrate_general(table: dict, state_in: np.ndarray, h: float, nsteps: int, r_capture: float = -np.inf,
+                      r_escape: float = np.inf, kind: int = TIMELIKE, flags: int = 0, long_double: bool = False,
+                      nthreads: int = 1) -> dict:
+    """Fixed-step RK4 through a general ten-field tabulated metric (reading T6)."""
+    st = np.ascontiguousarray(state_in, dtype=np.float64)
+    n = st.shape[1]
+    res = {"final_state": np.full((8, n), np.nan), "status": np.full(n, -1, dtype=np.int32),
+           "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan), "health": np.full(n, np.nan)}
+    stop = _Stop(r_capture, r_escape, kind, flags)
+    out = _Out(res["final_state"].ctypes.data, res["status"].ctypes.data, res["steps_done"].ctypes.data,
+               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data)
+    L = lib()
+    L.oracle_tabg_integrate.restype = C.c_int
+    L.oracle_tabg_integrate.argtypes = _GRID + [C.c_void_p, C.c_int64, C.c_double, C.c_int64, C.POINTER(_Stop),
+                                                C.POINTER(_Out), C.c_int, C.c_int]
+    rc = L.oracle_tabg_integrate(*_grid(table, 10), st.ctypes.data, n, h, nsteps, C.byref(stop), C.byref(out),
+                                 int(long_double), nthreads)
+    if rc != 0:
+        raise ValueError("oracle_tabg_integrate: invalid arguments")
     return res

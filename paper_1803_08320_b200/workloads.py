@@ -272,6 +272,60 @@ def kerr_metric_table(M: float, a: float, n1: int, n2: int, x1_lo: float, x1_hi:
             "radial": radial, "r_plus": rp}
 
 
+def general_table_from_diagonal(table: dict) -> dict:
+    """The ten-field layout of a GENERAL stationary axisymmetric 3+1 metric (reading T6: alpha, beta^1, beta^2,
+    beta^3, gamma_11, gamma_12, gamma_13, gamma_22, gamma_23, gamma_33) holding a five-field table of eq.(8)'s structure
+    (beta^1 = beta^2 = 0, diagonal gamma_ij): the same metric in the wider layout."""
+    t5 = table["tab"]
+    z = np.zeros_like(t5[0])
+    out = dict(table)
+    out["tab"] = np.ascontiguousarray(np.stack([t5[0], z, z, t5[1], t5[2], z, z, t5[3], z, t5[4]]))
+    return out
+
+
+def kerr_schild_metric_table(M: float, a: float, n1: int, n2: int, r_lo: float, r_hi: float,
+                             x2_lo: float = 0.0, x2_hi: float = math.pi, ghost: int = 2) -> dict:
+    """Input data for reading T6: the Kerr metric in ingoing Kerr-Schild (horizon-penetrating) coordinates
+    (t~, r, theta, phi~), dt~ = dt + 2Mr/Delta dr, dphi~ = dphi + a/Delta dr, whose line element
+        ds^2 = -(1 - f) dt~^2 + 2 f dt~ dr - 2 a f s^2 dt~ dphi~ + (1 + f) dr^2 + rho^2 dtheta^2
+               - 2 a (1 + f) s^2 dr dphi~ + (r^2 + a^2 + a^2 f s^2) s^2 dphi~^2,     f = 2 M r / rho^2,  s = sin theta,
+    is regular at r = r_+.  Its 3+1 split (line element (1)): gamma_ij = g_ij, beta_i = g_ti,
+    beta^i = gamma^{ij} beta_j, alpha^2 = beta_i beta^i - g_tt -- here beta^r = f/(1 + f) != 0 and gamma_r phi != 0, i.e. a
+    metric OUTSIDE the structure of eq.(8).  Nodes and ghosts as in kerr_metric_table; no interpolation, no equations of
+    motion here."""
+    d1 = (r_hi - r_lo) / (n1 - 1)
+    d2 = (x2_hi - x2_lo) / (n2 - 1)
+    x1 = r_lo + d1 * (np.arange(n1 + 2 * ghost) - ghost)
+    x2 = x2_lo + d2 * (np.arange(n2 + 2 * ghost) - ghost)
+    r, TH = np.meshgrid(x1, x2)
+    s2 = np.sin(TH) ** 2
+    rho2 = r * r + a * a * np.cos(TH) ** 2
+    f = 2.0 * M * r / rho2
+    g = np.zeros(r.shape + (3, 3))
+    g[..., 0, 0] = 1.0 + f
+    g[..., 1, 1] = rho2
+    g[..., 2, 2] = (r * r + a * a + a * a * f * s2) * s2
+    g[..., 0, 2] = g[..., 2, 0] = -a * (1.0 + f) * s2
+    bl = np.stack([f, np.zeros_like(f), -a * f * s2], axis=-1)           # beta_i = g_ti
+    bu = np.linalg.solve(g, bl[..., None])[..., 0]                       # beta^i
+    alpha = np.sqrt((bl * bu).sum(-1) + (1.0 - f))
+    tab = np.stack([alpha, bu[..., 0], bu[..., 1], bu[..., 2], g[..., 0, 0], g[..., 0, 1], g[..., 0, 2], g[..., 1, 1],
+                    g[..., 1, 2], g[..., 2, 2]])
+    return {"tab": np.ascontiguousarray(tab), "x1_0": float(x1[0]), "d1": float(d1), "x2_0": float(x2[0]), "d2": float(d2),
+            "r_plus": M + math.sqrt(M * M - a * a)}
+
+
+def to_kerr_schild(st: np.ndarray, E: np.ndarray, M: float, a: float) -> np.ndarray:
+    """state_in (r, theta, phi, u_r, u_theta, u_phi) of Boyer-Lindquist data with energy E -> the same covector in ingoing
+    Kerr-Schild coordinates: p_r~ = p_r + (2 M r E - a L)/Delta (from p_mu dx^mu invariant, p_t = -E); r, theta, p_theta,
+    p_phi unchanged; phi~ = phi at the start (the coordinate offset is a constant of the transformation)."""
+    out = np.array(st, dtype=np.float64, copy=True)
+    r = st[0]
+    Delta = r * r - 2.0 * M * r + a * a
+    out[3] = st[3] + (2.0 * M * r * E - a * st[5]) / Delta
+    return out
+
+
 def to_log_radial(st: np.ndarray, r_plus: float) -> np.ndarray:
     """state_in (r, theta, phi, u_r, u_theta, u_phi) -> the same covectors in x^1 = ln(r - r_+): u_1 = u_r (r - r_+)."""
     out = np.array(st, dtype=np.float64, copy=True)

@@ -269,3 +269,114 @@ def test_stop_rules_and_domain_exit(tab_oracle, oracle):
     hi = tb["x1_0"] + tb["d1"] * (tb["tab"].shape[2] - 2)
     assert o["status"][0] == tab_oracle.ST_OUTSIDE and 0 < o["steps_done"][0] < 100000
     assert o["final_state"][1, 0] < hi and o["final_state"][1, 0] > hi - 0.2
+
+
+# ---- reading T6: GENERAL stationary axisymmetric 3+1 metric (ten fields) ------------------------------------------------
+def _quadratic_general_metric():
+    """A made-up metric with ALL ten fields non-trivial quadratics (non-zero beta^1, beta^2, off-diagonal gamma_ij),
+    gamma_ij positive definite on the grid: the interpolant is exact on it."""
+    def fields(x1, x2):
+        return (1.0 + 0.05 * x1 + 0.02 * x2 * x2 - 0.01 * x1 * x2,          # alpha
+                0.02 + 0.01 * x1 - 0.004 * x2 * x2,                         # beta^1
+                -0.015 + 0.006 * x1 * x2,                                   # beta^2
+                -0.03 + 0.004 * x1 * x1 - 0.01 * x2,                        # beta^3
+                1.5 + 0.1 * x1 * x1 + 0.05 * x2,                            # gamma_11
+                0.10 + 0.02 * x1 - 0.03 * x2,                               # gamma_12
+                -0.20 + 0.05 * x2 * x2 + 0.01 * x1,                         # gamma_13
+                2.0 + 0.3 * x1 + 0.2 * x2 * x2,                             # gamma_22
+                0.15 - 0.02 * x1 * x2,                                      # gamma_23
+                1.0 + 0.5 * x1 * x2 + 0.1 * x1 * x1)                        # gamma_33
+    n1, n2 = 20, 18
+    tb = {"x1_0": 0.5, "d1": 0.2, "x2_0": 0.4, "d2": 0.15}
+    X1, X2 = np.meshgrid(tb["x1_0"] + tb["d1"] * np.arange(n1), tb["x2_0"] + tb["d2"] * np.arange(n2))
+    tb["tab"] = np.ascontiguousarray(np.stack(fields(X1, X2)))
+    return tb, fields
+
+
+def test_general_rhs_is_hamiltons_equations_of_line_element_1(tab_oracle):
+    """Reading T6 against eqs.(3),(4) PAPER.md:60-65 with H = 1/2 g^{mu nu} p_mu p_nu built here by inverting the full
+    4x4 matrix of line element (1) PAPER.md:47 (g_tt = -alpha^2 + beta_k beta^k, g_ti = gamma_ij beta^j, g_ij = gamma_ij):
+    a dropped shift component, a wrong sign, a missing factor 2 on an off-diagonal term or swapped gradients fail it.
+    Also the mass-shell energy: H(E) = -kappa/2."""
+    tb, fields = _quadratic_general_metric()
+
+    def H(x1, x2, pt, p1, p2, pph):
+        al, b1, b2, b3, g11, g12, g13, g22, g23, g33 = fields(x1, x2)
+        gam = np.array([[g11, g12, g13], [g12, g22, g23], [g13, g23, g33]])
+        bu = np.array([b1, b2, b3])
+        bl = gam @ bu
+        g = np.zeros((4, 4))                       # t, x1, x2, phi
+        g[0, 0] = -al * al + bl @ bu
+        g[0, 1:] = g[1:, 0] = bl
+        g[1:, 1:] = gam
+        p = np.array([pt, p1, p2, pph])
+        return 0.5 * p @ np.linalg.inv(g) @ p
+    rng = np.random.default_rng(6)
+    for _ in range(50):
+        x1, x2 = rng.uniform(1.0, 3.8), rng.uniform(0.7, 2.6)
+        E, p1, p2, L = rng.uniform(0.5, 2), rng.uniform(-1, 1), rng.uniform(-1, 1), rng.uniform(-2, 2)
+        kappa = float(rng.integers(0, 2))
+        d, Hval, Ems = tab_oracle.rhs_general(tb, [0.0, x1, x2, 0.0, E, p1, p2, L], kappa)
+        args = np.array([x1, x2, -E, p1, p2, L])
+        e = 1e-5
+
+        def dH(k):
+            up, dn = args.copy(), args.copy()
+            up[k] += e
+            dn[k] -= e
+            return (H(*up) - H(*dn)) / (2 * e)
+        want = np.array([dH(2), dH(3), dH(4), dH(5), -dH(0), -dH(1)])       # t, x1, x2, phi, p1, p2
+        assert abs(Hval - H(*args)) < 1e-13
+        assert np.max(np.abs(d - want)) < 2e-9, (d, want)
+        assert abs(2.0 * H(x1, x2, -Ems, p1, p2, L) + kappa) < 1e-12        # eq.(5): the energy is ON the mass shell
+        assert Ems + (fields(x1, x2)[1] * p1 + fields(x1, x2)[2] * p2 + fields(x1, x2)[3] * L) > 0   # future-directed root
+
+
+def test_general_layout_reduces_to_the_eq8_structure(tab_oracle):
+    """T6 with beta^1 = beta^2 = 0 and a diagonal 3-metric IS T3: the same Kerr table in both layouts gives the same
+    right-hand side (1e-14) and the same orbits (1e-12) as the five-field oracle pinned above."""
+    a = 0.9
+    tb5 = W.kerr_metric_table(1.0, a, 257, 65, 1.8, 40.0, 0.2, math.pi - 0.2)
+    tb10 = W.general_table_from_diagonal(tb5)
+    st = W.kerr_bound(200, a, W.SEED_BASE + 2)
+    for i in range(0, 200, 17):
+        y8 = [0.0, st[0, i], st[1, i], 0.0, 0.95, st[3, i], st[4, i], st[5, i]]
+        d5, H5 = tab_oracle.rhs(tb5, y8)
+        d10, H10, _ = tab_oracle.rhs_general(tb10, y8)
+        assert np.max(np.abs(d5 - d10) / np.maximum(np.abs(d5), 1.0)) < 1e-14 and abs(H5 - H10) < 1e-14
+    o5 = tab_oracle.integrate(tb5, st, 0.01, 2000)
+    o10 = tab_oracle.integrate_general(tb10, st, 0.01, 2000)
+    assert np.array_equal(o5["status"], o10["status"]) and np.array_equal(o5["steps_done"], o10["steps_done"])
+    assert np.max(np.abs(o5["final_state"] - o10["final_state"]) / np.maximum(np.abs(o5["final_state"]), 1.0)) < 1e-12
+
+
+def test_kerr_schild_table_reproduces_boyer_lindquist_orbits_and_penetrates_the_horizon(tab_oracle, oracle):
+    """The Kerr metric in ingoing Kerr-Schild coordinates (beta^r != 0, gamma_r phi != 0: outside eq.(8)'s structure) through
+    the general tabulated path against the pinned ANALYTIC Boyer-Lindquist oracle.  r, theta, p_theta, E, L are the same in
+    both coordinate systems (only t and phi are re-labelled), so bound orbits must agree in them, the better the finer
+    the grid; and a plunging particle crosses r_+ with finite state and |2H + 1| small -- in Boyer-Lindquist coordinates
+    the same particle cannot be followed through (Delta = 0)."""
+    a, M = 0.9, 1.0
+    st, consts = W.kerr_bound(40, a, W.SEED_BASE + 2, return_constants=True)
+    E = consts[0]
+    ob = oracle.integrate(oracle.KERR, M, a, st, 0.01, 3000)
+    assert np.allclose(ob["final_state"][4], E, rtol=0, atol=1e-12)          # the generator's E is the mass-shell E
+    ks = W.to_kerr_schild(st, E, M, a)
+    errs = []
+    for n1, n2 in ((513, 129), (1025, 257)):
+        tb = W.kerr_schild_metric_table(M, a, n1, n2, 1.2, 40.0, 0.15, math.pi - 0.15)
+        og = tab_oracle.integrate_general(tb, ks, 0.01, 3000)
+        assert (og["status"] == tab_oracle.ST_MAXSTEPS).all()
+        assert np.max(np.abs(og["final_state"][4] - E)) < 2e-6 * (513 / n1) ** 2   # E of the interpolated metric's mass shell
+        assert np.array_equal(og["final_state"][7], st[5])
+        errs.append(np.abs(og["final_state"][[1, 2, 6]] - ob["final_state"][[1, 2, 6]]).max())
+    assert errs[1] < errs[0] / 3.0 and errs[1] < 2e-4, errs            # O(d^2) force error of the interpolant: x ~5 per halving
+    # horizon penetration: radial-ish infall from r = 6 through r_+ = 1.4359 down to r ~ 1.3 (inside the table)
+    rp = M + math.sqrt(M * M - a * a)
+    fall = np.array([[6.0], [1.2], [0.0], [0.0], [0.3], [1.0]])               # BL data at rest-ish with L = 1
+    Ef = oracle.integrate(oracle.KERR, M, a, fall, 0.01, 0)["final_state"][4]
+    kf = W.to_kerr_schild(fall, Ef, M, a)
+    tb = W.kerr_schild_metric_table(M, a, 1025, 257, 1.2, 40.0, 0.15, math.pi - 0.15)
+    og = tab_oracle.integrate_general(tb, kf, 0.005, 20000, r_capture=1.3)
+    assert og["status"][0] == tab_oracle.ST_CAPTURED and og["final_state"][1, 0] < rp - 0.05      # went INSIDE the horizon
+    assert np.isfinite(og["final_state"]).all() and og["health"][0] < 1e-5

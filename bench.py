@@ -69,6 +69,8 @@ KERNEL_COUNTS = {
     "adaptive": dict(sym="geo_rk45_kernelILb1ELb0E", units_per_loop=1, flop=1045.0, pipe=684.0, other=None, tol=0.15, static_at_capture=(1135, 778),
                      source="ncu thread-level counts, profiles/r01_config3a_rk45.md: 361 DFMA + 271 DMUL + 52 DADD per attempt "
                             "(incl. predicated-on work of lanes waiting for a refill)", kernel="geo_rk45_kernel"),
+    "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0E", units_per_loop=None, flop=4390.0, pipe=2420.0, other=None, tol=None,
+                              source="PLACEHOLDER until the ncu capture: static count of the evaluator x 4", kernel="geo_tabg_rk4_kernel"),
     "tabulated": dict(sym="geo_tab_rk4_kernelILb0ELb1E", units_per_loop=None, flop=2217.0, pipe=1299.0, other=None, tol=None,
                       source="ncu thread-level counts, profiles/r01_tab4.md: 918 DFMA + 323 DMUL + 58 DADD per step (4 evaluations "
                              "through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tab_rk4_kernel"),
@@ -138,6 +140,15 @@ def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dic
         wl["table"] = W.kerr_metric_table(1.0, 0.5, 2049, 513, 2.0, 45.0, 0.1, math.pi - 0.1)
         wl["nsteps"] = 1000
         return wl
+    if name == "tabg4":
+        # SURVEY 8(f).3, general form (reading T6): the particles of configs[3] in ingoing KERR-SCHILD coordinates through
+        # the ten-field table of the Kerr a = 0.5 metric (2049 x 513 nodes + ghosts, 102 MB of 96-byte node records), 250 steps
+        n = n_override or (1 << 22)
+        st, consts = W.kerr_bound(n, 0.5, W.SEED_BASE + 4 + 1000 * rank, nthreads=nthreads, chunk=1 << 20, return_constants=True)
+        return dict(name="configs[3] particles in Kerr-Schild coordinates on a GENERAL tabulated metric (10 fields, 2049x513 nodes)",
+                    metric="tabulated_general", a=0.5, st=W.to_kerr_schild(st, consts[0], 1.0, 0.5), h=0.01, nsteps=250,
+                    snapshot_every=0, snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf,
+                    table=W.kerr_schild_metric_table(1.0, 0.5, 2049, 513, 2.0, 45.0, 0.1, math.pi - 0.1))
     if name == "config3a":
         # the rays of configs[2] with the adaptive Dormand-Prince 5(4) stepper (per-ray step control);
         # unit = one step ATTEMPT (accepted or rejected: 6 new RHS evaluations + error estimate)
@@ -290,9 +301,10 @@ def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> di
     times, done = [], 0
     for i in range(warmup + steps):
         t0 = time.perf_counter()
-        if wl["metric"] == "tabulated":
-            o = geo_tab_oracle.integrate(wl["table"], sub, wl["h"], wl["nsteps"], r_capture=wl["r_capture"],
-                                         r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
+        if wl["metric"] in ("tabulated", "tabulated_general"):
+            fn = geo_tab_oracle.integrate if wl["metric"] == "tabulated" else geo_tab_oracle.integrate_general
+            o = fn(wl["table"], sub, wl["h"], wl["nsteps"], r_capture=wl["r_capture"],
+                   r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
         elif ad:
             o = geo_oracle.integrate_adaptive(metric, 1.0, wl["a"], sub, ad["h0"], ad["rtol"], ad["atol"], ad["max_attempts"],
                                               r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
@@ -412,9 +424,10 @@ class GpuRun:
         self.torch, self.geo, self.dev, self.wl = torch, geo, dev, wl
         self.flags = flags | wl.get("flags", 0)
         self.stream = torch.cuda.current_stream(dev)
-        if wl["metric"] == "tabulated":
+        if wl["metric"] in ("tabulated", "tabulated_general"):
             tb = wl["table"]
-            self.ctx = geo.geo_create_tabulated(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+            mk = geo.geo_create_tabulated if wl["metric"] == "tabulated" else geo.geo_create_tabulated_general
+            self.ctx = mk(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
         else:
             self.ctx = geo.geo_create(geo.KERR if wl["metric"] == "kerr" else geo.SCHWARZSCHILD, 1.0, wl["a"])
         tiles = wl.get("tiles") or [wl["st"]]
@@ -526,7 +539,7 @@ SECONDARY = [("config2", "config2", 0, True), ("config3", "config3", 0, True), (
              ("config3_shuffled_static", "config3s", 2, False), ("config5_central_tile", "config5tile", 0, False),
              ("snapbench_schwarzschild_every_step", "snapbench", 0, False), ("snapkerr_every_step_8comp", "snapkerr", 0, False),
              ("snapkerr_every_step_txyz", "snapkerr_xyz", 0, False), ("config3_adaptive_rk45", "config3a", 0, True),
-             ("tab4_tabulated_metric", "tab4", 0, False), ("paper_table3", "paper_t3", 0, False), ("paper_table4", "paper_t4", 0, False)]
+             ("tab4_tabulated_metric", "tab4", 0, False), ("tabg4_general_tabulated_metric_kerr_schild", "tabg4", 0, False), ("paper_table3", "paper_t3", 0, False), ("paper_table4", "paper_t4", 0, False)]
 
 
 def run_secondary(torch, geo, dev, sm_max: float, ncpu: int, peaks: dict, reuse_config4) -> dict:
@@ -596,7 +609,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4",
-                    choices=["config1", "config2", "config3", "config4", "config5", "config5tile", "config3s", "config3a", "tab4",
+                    choices=["config1", "config2", "config3", "config4", "config5", "config5tile", "config3s", "config3a", "tab4", "tabg4",
                              "snapbench", "snapkerr", "snapkerr_xyz", "paper_t3", "paper_t4"])
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank its own batch; strong = one image (config3) split into interleaved row tiles")
@@ -697,11 +710,12 @@ def main() -> None:
             # measured law of this kernel: an FP64 instruction holds the issue port 2 cycles, any other 1
             roofline["other_instr_per_step"] = kc["other"]
             roofline["issue_slot_util"] = ups * (2.0 * kc["pipe"] + kc["other"]) / (SM_COUNT * 4 * 32 * sm_max * 1e6)
-    if wl["metric"] == "tabulated":
-        roofline["table_bytes_per_step"] = 4 * 640
-        roofline["table_read_gbs"] = ups * 4 * 640 / 1e9
+    if wl["metric"] in ("tabulated", "tabulated_general"):
+        node_b = 40 if wl["metric"] == "tabulated" else 96        # bytes per node record on the device
+        roofline["table_bytes_per_step"] = 4 * 16 * node_b
+        roofline["table_read_gbs"] = ups * 4 * 16 * node_b / 1e9
         tbl = wl["table"]["tab"]
-        roofline["table_mb_on_device"] = tbl.shape[1] * tbl.shape[2] * 40 / 1e6
+        roofline["table_mb_on_device"] = tbl.shape[1] * tbl.shape[2] * node_b / 1e6
     if ad:
         roofline["unit_of_work"] = "one RK5(4) step attempt (accepted or rejected)"
     ncomp = bin(wl["snap_mask"] & 0xFF).count("1")

@@ -29,7 +29,8 @@ extern "C" {
 
 typedef struct geo_ctx geo_ctx; /* opaque; owned by the library */
 
-enum { GEO_SCHWARZSCHILD = 0, GEO_KERR = 1, GEO_TABULATED = 2 };    /* metric (2: geo_create_tabulated) */
+enum { GEO_SCHWARZSCHILD = 0, GEO_KERR = 1, GEO_TABULATED = 2,    /* metric (2: geo_create_tabulated,          */
+       GEO_TABULATED_GENERAL = 3 };                                  /*         3: geo_create_tabulated_general)  */
 enum { GEO_TIMELIKE = 0, GEO_NULL = 1 };                            /* geo_stop.kind: kappa=1/0 */
 enum { GEO_OK = 0, GEO_EINVAL = 1, GEO_ECUDA = 2, GEO_ENOMEM = 3 }; /* return codes            */
 /* per-particle termination class (geo_out.status) */
@@ -156,11 +157,23 @@ int geo_integrate_adaptive_host(geo_ctx *ctx, const double *state_in, int64_t n,
  * geo_integrate_adaptive returns GEO_EINVAL; geo_horizon_radius returns NaN.
  * Errors: GEO_EINVAL (NULL, n1 or n2 < 4, d1 or d2 <= 0, non-finite grid), GEO_ENOMEM, GEO_ECUDA. */
 typedef struct geo_table {
-    const double *tab;  /* HOST [5][n2][n1] */
+    const double *tab;  /* HOST [5][n2][n1] (geo_create_tabulated) or [10][n2][n1] (geo_create_tabulated_general) */
     int64_t n1, n2;
     double x1_0, d1, x2_0, d2;
 } geo_table;
 int geo_create_tabulated(geo_ctx **ctx, const geo_table *table);
+
+/* SURVEY 8(f).3, general form (reading T6): line element (1) for ANY stationary, axisymmetric
+ * metric -- all ten functions of (x^1, x^2), x^3 = phi being the symmetry direction:
+ *     tab[f][j][i], f = 0..9 = alpha, beta^1, beta^2, beta^3, gamma_11, gamma_12, gamma_13, gamma_22, gamma_23, gamma_33
+ * (HOST, same grid conventions as geo_create_tabulated; copied, not kept).  No circularity and no diagonal 3-metric is
+ * assumed: horizon-penetrating coordinates (e.g. Kerr in Kerr-Schild form: beta^r != 0, gamma_r phi != 0) are in scope.
+ * Same interpolant with its exact gradient; equations of motion = Hamilton's equations (3),(4) of
+ *     H = 1/2 [ -(p_t - beta^k p_k)^2/alpha^2 + gamma^{ij} p_i p_j ],   gamma^{ij} = inverse of gamma_ij (3 x 3, per evaluation),
+ * p_t and p_phi constants of motion.  Use with geo_integrate / geo_integrate_host exactly like a geo_create_tabulated
+ * ctx (state_in = (x^1, x^2, phi, p_1, p_2, p_phi); GEO_ST_OUTSIDE; snapshot_every must be 0; flags:
+ * GEO_FLAG_PLAIN_UPDATE only; geo_integrate_adaptive returns GEO_EINVAL). */
+int geo_create_tabulated_general(geo_ctx **ctx, const geo_table *table);
 
 void geo_destroy(geo_ctx *ctx);
 

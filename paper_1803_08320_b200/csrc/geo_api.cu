@@ -10,6 +10,7 @@
 #include "geo_kernel.cuh"
 #include "geo_rk45.cuh"
 #include "geo_tab.cuh"
+#include "geo_tabg.cuh"
 
 using namespace geo;
 
@@ -27,6 +28,9 @@ struct geo_ctx {
     double4* tabA;
     double* tabB;
     TabMetric tm;
+    // GEO_TABULATED_GENERAL: ten-field node records (device, owned)
+    double* tabG;
+    TabgMetric tgm;
     char err[256];
 };
 
@@ -97,9 +101,10 @@ int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t 
     if (stop->kind != GEO_TIMELIKE && stop->kind != GEO_NULL) return fail(ctx, GEO_EINVAL, "stop.kind must be GEO_TIMELIKE or GEO_NULL");
     if (std::isnan(stop->r_capture) || std::isnan(stop->r_escape)) return fail(ctx, GEO_EINVAL, "stop radii must not be NaN");
     if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_STAGED_SNAP | GEO_FLAG_CARTESIAN_SNAP | GEO_FLAG_TAB_GATHER)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
-    if (ctx->metric == GEO_TABULATED) {
+    if (ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) {
         if (snapshot_every > 0) return fail(ctx, GEO_EINVAL, "tabulated metrics: snapshots are not supported");
-        if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_TAB_GATHER)) return fail(ctx, GEO_EINVAL, "tabulated metrics: only GEO_FLAG_PLAIN_UPDATE and GEO_FLAG_TAB_GATHER are supported");
+        const int32_t ok = ctx->metric == GEO_TABULATED ? (GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_TAB_GATHER) : GEO_FLAG_PLAIN_UPDATE;
+        if (stop->flags & ~ok) return fail(ctx, GEO_EINVAL, "tabulated metrics: only GEO_FLAG_PLAIN_UPDATE (and GEO_FLAG_TAB_GATHER for five-field tables) are supported");
     }
     if (n == 0) return GEO_OK;
     if (!state_in || !out->final_state || !out->status || !out->steps_done) return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
@@ -214,9 +219,62 @@ int launch_tab(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t ns
     return GEO_OK;
 }
 
+typedef void (*tabg_kernel_fn)(const TabgParams);
+tabg_kernel_fn pick_tabg_kernel(int32_t flags) {
+    return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false>;
+}
+
+int plan_tabg(geo_ctx* ctx, int64_t n, int32_t flags, int* grid, int* per_sm_out, int* regs) {
+    tabg_kernel_fn fn = pick_tabg_kernel(flags);
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kTabBlock, 0);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(tabg)");
+    if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, (const void*)fn);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncGetAttributes");
+    const int64_t need = (n + kTabBlock - 1) / kTabBlock, resident = (int64_t)ctx->sm_count * per_sm;
+    *grid = (int)(need < resident ? need : resident);
+    *per_sm_out = per_sm;
+    *regs = fa.numRegs;
+    return GEO_OK;
+}
+
+int launch_tabg(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
+                const geo_out* out, cudaStream_t stream, unsigned long long* counter) {
+    int grid = 0, per_sm = 0, regs = 0;
+    int rc = plan_tabg(ctx, n, stop->flags, &grid, &per_sm, &regs);
+    if (rc != GEO_OK) return rc;
+    TabgParams p;
+    memset(&p, 0, sizeof p);
+    p.in = d_in;
+    p.n = n;
+    p.h = h;
+    p.h_half = h / 2.0;
+    p.h_sixth = h / 6.0;
+    p.nsteps = (int)nsteps;
+    p.r_capture = stop->r_capture;
+    p.r_escape = stop->r_escape;
+    p.kappa = stop->kind == GEO_TIMELIKE ? 1.0 : 0.0;
+    p.fin = out->final_state;
+    p.status = out->status;
+    p.steps_done = reinterpret_cast<long long*>(out->steps_done);
+    p.eq_cross_r = out->eq_cross_r;
+    p.health = out->health;
+    p.counter = counter;
+    p.m = ctx->tgm;
+    cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
+    pick_tabg_kernel(stop->flags)<<<grid, kTabBlock, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
+    return GEO_OK;
+}
+
 int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
            int64_t snapshot_every, const geo_out* out, cudaStream_t stream, unsigned long long* counter) {
     if (ctx->metric == GEO_TABULATED) return launch_tab(ctx, d_in, n, h, nsteps, stop, out, stream, counter);
+    if (ctx->metric == GEO_TABULATED_GENERAL) return launch_tabg(ctx, d_in, n, h, nsteps, stop, out, stream, counter);
     const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
     LaunchPlan lp;
     int rc = plan_launch(ctx, n, stop->flags, snapshot_every, ncomp, &lp);
@@ -343,11 +401,57 @@ int geo_create_tabulated(geo_ctx** out_ctx, const geo_table* tb) {
     return GEO_OK;
 }
 
+int geo_create_tabulated_general(geo_ctx** out_ctx, const geo_table* tb) {
+    if (!out_ctx) return GEO_EINVAL;
+    *out_ctx = nullptr;
+    if (!tb || !tb->tab || tb->n1 < 4 || tb->n2 < 4 || tb->n1 > 0x3fffffff || tb->n2 > 0x3fffffff) return GEO_EINVAL;
+    if (!(tb->d1 > 0.0) || !(tb->d2 > 0.0) || !std::isfinite(tb->d1) || !std::isfinite(tb->d2) ||
+        !std::isfinite(tb->x1_0) || !std::isfinite(tb->x2_0))
+        return GEO_EINVAL;
+    geo_ctx* ctx = new (std::nothrow) geo_ctx;
+    if (!ctx) return GEO_ENOMEM;
+    memset(ctx, 0, sizeof *ctx);
+    ctx->metric = GEO_TABULATED_GENERAL;
+    ctx->M = NAN;
+    ctx->a = NAN;
+    const size_t nodes = (size_t)tb->n1 * (size_t)tb->n2;
+    double* raw = nullptr;
+    cudaError_t e = cudaGetDevice(&ctx->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->counter, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->tabG, nodes * kTabgStride * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&raw, kTabgFields * nodes * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(raw, tb->tab, kTabgFields * nodes * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        tabg_pack_kernel<<<(unsigned)((nodes + 255) / 256), 256>>>(raw, (long long)nodes, ctx->tabG);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    }
+    if (raw) cudaFree(raw);
+    if (e != cudaSuccess) {
+        int rc = e == cudaErrorMemoryAllocation ? GEO_ENOMEM : GEO_ECUDA;
+        geo_destroy(ctx);
+        return rc;
+    }
+    ctx->tgm.G = ctx->tabG;
+    ctx->tgm.n1 = (int)tb->n1;
+    ctx->tgm.n2 = (int)tb->n2;
+    ctx->tgm.x1_0 = tb->x1_0;
+    ctx->tgm.d1 = tb->d1;
+    ctx->tgm.inv_d1 = 1.0 / tb->d1;
+    ctx->tgm.x2_0 = tb->x2_0;
+    ctx->tgm.d2 = tb->d2;
+    ctx->tgm.inv_d2 = 1.0 / tb->d2;
+    *out_ctx = ctx;
+    return GEO_OK;
+}
+
 void geo_destroy(geo_ctx* ctx) {
     if (!ctx) return;
     DeviceGuard guard(ctx->device);      // frees go to the ctx's device (best effort if the switch fails)
     if (ctx->tabA) cudaFree(ctx->tabA);
     if (ctx->tabB) cudaFree(ctx->tabB);
+    if (ctx->tabG) cudaFree(ctx->tabG);
     for (int k = 0; k < 2; ++k)
         if (ctx->host_stream[k]) cudaStreamDestroy(ctx->host_stream[k]);
     if (ctx->scratch) cudaFree(ctx->scratch);
@@ -356,7 +460,7 @@ void geo_destroy(geo_ctx* ctx) {
 }
 
 double geo_horizon_radius(const geo_ctx* ctx) {
-    if (!ctx || ctx->metric == GEO_TABULATED) return NAN;
+    if (!ctx || ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) return NAN;
     return ctx->M + std::sqrt(ctx->M * ctx->M - ctx->a * ctx->a);
 }
 
@@ -491,7 +595,7 @@ static int validate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, co
                              const geo_stop* stop, const geo_out* out, const int32_t* rejected, bool check_align) {
     int rc = validate(ctx, state_in, n, 1.0, 0, stop, 0, out, check_align);
     if (rc != GEO_OK) return rc;
-    if (ctx->metric == GEO_TABULATED) return fail(ctx, GEO_EINVAL, "the adaptive path takes analytic metrics only");
+    if (ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) return fail(ctx, GEO_EINVAL, "the adaptive path takes analytic metrics only");
     if (!ctl) return fail(ctx, GEO_EINVAL, "ctl must not be NULL");
     if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0)) return fail(ctx, GEO_EINVAL, "h0 must be finite and > 0");
     if (!(ctl->rtol >= 0.0) || !(ctl->atol >= 0.0) || !(ctl->rtol + ctl->atol > 0.0) || std::isinf(ctl->atol))
@@ -593,6 +697,10 @@ int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_eve
     if (ctx->metric == GEO_TABULATED) {
         info[1] = kTabBlock;
         return plan_tab(ctx, n, flags, &info[0], &info[3], &info[2]);
+    }
+    if (ctx->metric == GEO_TABULATED_GENERAL) {
+        info[1] = kTabBlock;
+        return plan_tabg(ctx, n, flags, &info[0], &info[3], &info[2]);
     }
     LaunchPlan lp;
     int rc = plan_launch(ctx, n, flags, snapshot_every, 8, &lp);

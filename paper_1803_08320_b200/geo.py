@@ -3,7 +3,7 @@
 Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
 and streams.  There is NO CPU fallback: if the library cannot be loaded, or there is no CUDA device,
 the calls raise.  Names follow the C ABI: ``geo_create``, ``geo_integrate``, ``geo_integrate_host``,
-``geo_create_tabulated``, ``geo_integrate_adaptive``, ``geo_integrate_adaptive_host``, ``geo_destroy``, ``geo_horizon_radius``,
+``geo_create_tabulated``, ``geo_create_tabulated_general``, ``geo_integrate_adaptive``, ``geo_integrate_adaptive_host``, ``geo_destroy``, ``geo_horizon_radius``,
 ``geo_last_error``; plus the development helpers of include/geo_dev.h (``geo_launch_info``, ``geo_probe_dfma``) used by bench.py.
 """
 from __future__ import annotations
@@ -13,7 +13,7 @@ import os
 
 import numpy as np
 
-SCHWARZSCHILD, KERR, TABULATED = 0, 1, 2
+SCHWARZSCHILD, KERR, TABULATED, TABULATED_GENERAL = 0, 1, 2, 3
 TIMELIKE, NULL = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, 1, 2, 3
 ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC, ST_OUTSIDE = 0, 1, 2, 3, 4
@@ -23,7 +23,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI
 
 # every symbol include/geo.h declares, then the development helpers of include/geo_dev.h
-SYMBOLS = ("geo_create", "geo_create_tabulated", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_integrate_adaptive_host", "geo_destroy",
+SYMBOLS = ("geo_create", "geo_create_tabulated", "geo_create_tabulated_general", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_integrate_adaptive_host", "geo_destroy",
            "geo_horizon_radius", "geo_last_error")
 DEV_SYMBOLS = ("geo_launch_info", "geo_probe_dfma")
 
@@ -70,6 +70,8 @@ def lib() -> C.CDLL:
         L.geo_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double]
         L.geo_create_tabulated.restype = C.c_int
         L.geo_create_tabulated.argtypes = [C.POINTER(C.c_void_p), C.POINTER(GeoTable)]
+        L.geo_create_tabulated_general.restype = C.c_int
+        L.geo_create_tabulated_general.argtypes = [C.POINTER(C.c_void_p), C.POINTER(GeoTable)]
         L.geo_integrate.restype = C.c_int
         L.geo_integrate.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int64,
                                     C.POINTER(GeoStop), C.c_int64, C.POINTER(GeoOut), C.c_void_p]
@@ -120,6 +122,20 @@ def geo_create_tabulated(tab: np.ndarray, x1_0: float, d1: float, x2_0: float, d
     rc = lib().geo_create_tabulated(C.byref(ctx), C.byref(tb))
     if rc != OK:
         raise GeoError(rc, "geo_create_tabulated failed (invalid table/grid, out of memory, or no CUDA device)")
+    return ctx
+
+
+def geo_create_tabulated_general(tab: np.ndarray, x1_0: float, d1: float, x2_0: float, d2: float) -> C.c_void_p:
+    """Context for a GENERAL tabulated 3+1 metric (include/geo.h: geo_create_tabulated_general).  ``tab``: host float64
+    [10][n2][n1] = alpha, beta^1, beta^2, beta^3, gamma_11, gamma_12, gamma_13, gamma_22, gamma_23, gamma_33."""
+    if not (isinstance(tab, np.ndarray) and tab.dtype == np.float64 and tab.ndim == 3 and tab.shape[0] == 10
+            and tab.flags.c_contiguous):
+        raise ValueError("tab must be a C-contiguous float64 numpy array of shape [10][n2][n1]")
+    ctx = C.c_void_p()
+    tb = GeoTable(tab.ctypes.data, tab.shape[2], tab.shape[1], x1_0, d1, x2_0, d2)
+    rc = lib().geo_create_tabulated_general(C.byref(ctx), C.byref(tb))
+    if rc != OK:
+        raise GeoError(rc, "geo_create_tabulated_general failed (invalid table/grid, out of memory, or no CUDA device)")
     return ctx
 
 

@@ -69,8 +69,9 @@ KERNEL_COUNTS = {
     "adaptive": dict(sym="geo_rk45_kernelILb1ELb0E", units_per_loop=1, flop=1045.0, pipe=684.0, other=None, tol=0.15, static_at_capture=(1135, 778),
                      source="ncu thread-level counts, profiles/r01_config3a_rk45.md: 361 DFMA + 271 DMUL + 52 DADD per attempt "
                             "(incl. predicated-on work of lanes waiting for a refill)", kernel="geo_rk45_kernel"),
-    "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0E", units_per_loop=None, flop=4390.0, pipe=2420.0, other=None, tol=None,
-                              source="PLACEHOLDER until the ncu capture: static count of the evaluator x 4", kernel="geo_tabg_rk4_kernel"),
+    "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0E", units_per_loop=None, flop=4073.0, pipe=2376.0, other=None, tol=None,
+                              source="ncu per-instruction counts, profiles/r02_tabg4.md: 1735 DFMA + 550 DMUL + 52 DADD + 38 DSETP per step "
+                                     "(4 evaluations through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tabg_rk4_kernel"),
     "tabulated": dict(sym="geo_tab_rk4_kernelILb0ELb1E", units_per_loop=None, flop=2217.0, pipe=1299.0, other=None, tol=None,
                       source="ncu thread-level counts, profiles/r01_tab4.md: 918 DFMA + 323 DMUL + 58 DADD per step (4 evaluations "
                              "through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tab_rk4_kernel"),
@@ -290,12 +291,12 @@ def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> di
     # sample: a prefix of the batch sized for ~budget_s of wall time at ~3e6 steps/s/core
     ad = wl.get("adaptive")
     per = max(1, int(budget_s * 3.0e6 * cores / max(1, 300 * 2 if ad else wl["nsteps"])))   # adaptive: ~300 attempts/ray, 2x cost
+    if wl["metric"] in ("tabulated", "tabulated_general"):
+        import geo_tab_oracle
+        per = max(1, per // (4 if wl["metric"] == "tabulated" else 10))          # ~4x / ~10x the analytic RHS cost
     m = min(st.shape[1], max(cores, per))
     sub = np.ascontiguousarray(st[:, :m])
     metric = geo_oracle.KERR if wl["metric"] == "kerr" else geo_oracle.SCHWARZSCHILD
-    if wl["metric"] == "tabulated":
-        import geo_tab_oracle
-        per = max(1, per // 4)          # ~4x the analytic RHS cost
     kw = dict(r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores,
               snapshot_every=wl["snapshot_every"], snap_mask=wl["snap_mask"], flags=wl.get("flags", 0))
     times, done = [], 0

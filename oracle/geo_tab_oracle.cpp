@@ -31,7 +31,8 @@
 //       coordinate, ends the particle with status OUTSIDE = 4; that step is not taken.
 //   T5  RK4, Kahan update (P1), stop rules B1-B6 and the equatorial-crossing event B5 exactly as in
 //       geo_oracle.cpp with r -> x^1, theta -> x^2; per evaluation point the capture test comes first,
-//       then the domain test.  No snapshots.
+//       then the domain test.  Trajectory records (five-field path, round 2): S1-S3 of geo_oracle.cpp, components
+//       (t, x1, x2, phi, E, p1, p2, L) selected by snap_mask; no Cartesian option (the coordinates are the table's own).
 //
 //   T6  (round 2) GENERAL stationary, axisymmetric 3+1 metric: all TEN functions of line element (1) --
 //       alpha, beta^1, beta^2, beta^3, gamma_11, gamma_12, gamma_13, gamma_22, gamma_23, gamma_33 (x^3 = phi) -- of
@@ -145,7 +146,26 @@ template <class R> R energy_fields(const Fields<R>& F, R p1, R p2, R L, R kappa)
 }
 
 struct StopRule { double r_capture, r_escape; int32_t kind; int32_t flags; };
-struct OutPtrs { double* final_state; int32_t* status; int64_t* steps_done; double* eq_cross_r; double* health; };
+struct OutPtrs {
+    double* final_state; int32_t* status; int64_t* steps_done; double* eq_cross_r; double* health;
+    // trajectory records (five-field path only, round 2): as in geo_oracle.cpp, readings S1-S3
+    double* snapshots;      // [n][snap_capacity][ncomp] or null
+    int64_t snap_capacity;
+    uint32_t snap_mask;     // bit k: component k of (t, x1, x2, phi, E, p1, p2, L)
+    int32_t* snap_count;    // [n] or null
+};
+
+template <class R> struct State;
+template <class R>
+void write_record(const OutPtrs& o, int64_t i, int64_t slot, const R comp[8]) {
+    if (!o.snapshots || slot >= o.snap_capacity) return;   // S3: drop, never overflow
+    int ncomp = 0;
+    for (int k = 0; k < 8; ++k) ncomp += (o.snap_mask >> k) & 1u;
+    double* dst = o.snapshots + (i * o.snap_capacity + slot) * ncomp;
+    int j = 0;
+    for (int k = 0; k < 8; ++k)
+        if ((o.snap_mask >> k) & 1u) dst[j++] = (double)comp[k];
+}
 
 template <class R> bool finite6(const State<R>& y) {
     return std::isfinite(y.t) && std::isfinite(y.x1) && std::isfinite(y.x2) && std::isfinite(y.ph) &&
@@ -173,7 +193,7 @@ template <class R> void kahan_add(R& y, R& c, R delta, bool plain) {
 
 template <class R>
 void integrate_one(const Table& m, const double* state_in, int64_t n, int64_t i, R h, int64_t nsteps,
-                   const StopRule& st, const OutPtrs& o) {
+                   const StopRule& st, const OutPtrs& o, int64_t snapshot_every = 0) {
     const R kappa = st.kind == 0 ? R(1) : R(0);
     const bool plain = (st.flags & 1) != 0;
     const R rc = (R)st.r_capture, re = (R)st.r_escape;
@@ -191,10 +211,15 @@ void integrate_one(const Table& m, const double* state_in, int64_t n, int64_t i,
     R ct = 0, c1 = 0, c2 = 0, cph = 0, cp1 = 0, cp2 = 0;
 
     int32_t status = -1;
-    int64_t steps = 0;
+    int64_t steps = 0, snaps = 0;
     R eq_cross = std::numeric_limits<R>::quiet_NaN();
     bool crossed = false;
     Fields<R> F;
+    auto record = [&]() {
+        const R comp[8] = {y.t, y.x1, y.x2, y.ph, y.E, y.p1, y.p2, y.L};
+        write_record<R>(o, i, snaps, comp);
+        ++snaps;
+    };
 
     // B1 + T4 on y0
     if (!(y.x1 >= rc)) status = TAB_ST_CAPTURED;
@@ -203,8 +228,11 @@ void integrate_one(const Table& m, const double* state_in, int64_t n, int64_t i,
     else {
         y.E = energy_fields(F, y.p1, y.p2, y.L, kappa);
         if (!std::isfinite(y.E)) status = TAB_ST_NUMERIC;
-        else if (y.x1 > re) status = TAB_ST_ESCAPED;
-        else if (nsteps == 0) status = TAB_ST_MAXSTEPS;
+        else {
+            if (snapshot_every > 0) record();                        // S1: slot 0 = y0 (E known: it passed every y0 test)
+            if (y.x1 > re) status = TAB_ST_ESCAPED;
+            else if (nsteps == 0) status = TAB_ST_MAXSTEPS;
+        }
     }
 
     while (status < 0) {
@@ -248,6 +276,7 @@ void integrate_one(const Table& m, const double* state_in, int64_t n, int64_t i,
         y = yn; ct = nt; c1 = n1; c2 = n2; cph = nph; cp1 = np1; cp2 = np2;
         F = G;
         ++steps;
+        if (snapshot_every > 0 && steps % snapshot_every == 0) record();   // S1
         if (y.x1 > re) status = TAB_ST_ESCAPED;
         else if (steps >= nsteps) status = TAB_ST_MAXSTEPS;
     }
@@ -257,6 +286,7 @@ void integrate_one(const Table& m, const double* state_in, int64_t n, int64_t i,
     o.status[i] = status;
     o.steps_done[i] = steps;
     if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
+    if (snapshot_every > 0 && o.snap_count) o.snap_count[i] = (int32_t)snaps;
     if (o.health) {
         // |2H + kappa| of the final state; NaN where the final state has no interpolant (OUTSIDE at y0, NUMERIC)
         Fields<R> H;
@@ -268,8 +298,8 @@ void integrate_one(const Table& m, const double* state_in, int64_t n, int64_t i,
 
 template <class R>
 void integrate_range(const Table& m, const double* state_in, int64_t n, double h, int64_t nsteps,
-                     const StopRule& st, const OutPtrs& o, int64_t lo, int64_t hi) {
-    for (int64_t i = lo; i < hi; ++i) integrate_one<R>(m, state_in, n, i, (R)h, nsteps, st, o);
+                     const StopRule& st, const OutPtrs& o, int64_t lo, int64_t hi, int64_t snapshot_every) {
+    for (int64_t i = lo; i < hi; ++i) integrate_one<R>(m, state_in, n, i, (R)h, nsteps, st, o, snapshot_every);
 }
 
 
@@ -456,8 +486,9 @@ extern "C" {
 // tab: [5][n2][n1] host doubles.  precision: 0 = double, 1 = long double.  Returns 0, or 1 on invalid arguments.
 int oracle_tab_integrate(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
                          const double* state_in, int64_t n, double h, int64_t nsteps, const StopRule* st,
-                         const OutPtrs* out, int precision, int nthreads) {
-    if (!tab || n1 < 4 || n2 < 4 || !(d1 > 0) || !(d2 > 0) || n < 0 || nsteps < 0 || !st || !out) return 1;
+                         const OutPtrs* out, int precision, int nthreads, int64_t snapshot_every) {
+    if (!tab || n1 < 4 || n2 < 4 || !(d1 > 0) || !(d2 > 0) || n < 0 || nsteps < 0 || !st || !out || snapshot_every < 0) return 1;
+    if (snapshot_every > 0 && (!out->snapshots || !out->snap_count || out->snap_capacity < 1 || (out->snap_mask & 0xFFu) == 0)) return 1;
     const Table m{tab, n1, n2, x1_0, d1, x2_0, d2};
     if (nthreads < 1) nthreads = 1;
     std::vector<std::thread> pool;
@@ -466,9 +497,9 @@ int oracle_tab_integrate(const double* tab, int64_t n1, int64_t n2, double x1_0,
         const int64_t lo = t * per, hi = std::min<int64_t>(n, lo + per);
         if (lo >= hi) break;
         if (precision == 1)
-            pool.emplace_back(integrate_range<long double>, m, state_in, n, h, nsteps, *st, *out, lo, hi);
+            pool.emplace_back(integrate_range<long double>, m, state_in, n, h, nsteps, *st, *out, lo, hi, snapshot_every);
         else
-            pool.emplace_back(integrate_range<double>, m, state_in, n, h, nsteps, *st, *out, lo, hi);
+            pool.emplace_back(integrate_range<double>, m, state_in, n, h, nsteps, *st, *out, lo, hi, snapshot_every);
     }
     for (auto& th : pool) th.join();
     return 0;

@@ -24,7 +24,8 @@ class _Stop(C.Structure):
 
 class _Out(C.Structure):
     _fields_ = [("final_state", C.c_void_p), ("status", C.c_void_p), ("steps_done", C.c_void_p),
-                ("eq_cross_r", C.c_void_p), ("health", C.c_void_p)]
+                ("eq_cross_r", C.c_void_p), ("health", C.c_void_p), ("snapshots", C.c_void_p),
+                ("snap_capacity", C.c_int64), ("snap_mask", C.c_uint32), ("snap_count", C.c_void_p)]
 
 
 _lib = None
@@ -37,7 +38,7 @@ def lib():
         _lib = C.CDLL(_build.build())
         _lib.oracle_tab_integrate.restype = C.c_int
         _lib.oracle_tab_integrate.argtypes = _GRID + [C.c_void_p, C.c_int64, C.c_double, C.c_int64, C.POINTER(_Stop),
-                                                      C.POINTER(_Out), C.c_int, C.c_int]
+                                                      C.POINTER(_Out), C.c_int, C.c_int, C.c_int64]
         _lib.oracle_tab_fields.restype = C.c_int
         _lib.oracle_tab_fields.argtypes = _GRID + [C.c_double, C.c_double, C.c_void_p]
         _lib.oracle_tab_rhs.restype = C.c_int
@@ -68,17 +69,25 @@ def rhs(table: dict, y8):
 
 def integrate(table: dict, state_in: np.ndarray, h: float, nsteps: int, r_capture: float = -np.inf,
               r_escape: float = np.inf, kind: int = TIMELIKE, flags: int = 0, long_double: bool = False,
-              nthreads: int = 1) -> dict:
+              nthreads: int = 1, snapshot_every: int = 0, snap_capacity: int | None = None, snap_mask: int = 0xFF) -> dict:
     """Fixed-step RK4 through the tabulated metric on host SoA state_in [6][n] = (x1, x2, phi, p_1, p_2, p_phi)."""
     st = np.ascontiguousarray(state_in, dtype=np.float64)
     n = st.shape[1]
     res = {"final_state": np.full((8, n), np.nan), "status": np.full(n, -1, dtype=np.int32),
-           "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan), "health": np.full(n, np.nan)}
+           "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan), "health": np.full(n, np.nan),
+           "snapshots": None, "snap_count": None}
+    if snapshot_every > 0:
+        if snap_capacity is None:
+            snap_capacity = 1 + nsteps // snapshot_every
+        res["snapshots"] = np.full((n, snap_capacity, bin(snap_mask & 0xFF).count("1")), np.nan)
+        res["snap_count"] = np.zeros(n, dtype=np.int32)
     stop = _Stop(r_capture, r_escape, kind, flags)
     out = _Out(res["final_state"].ctypes.data, res["status"].ctypes.data, res["steps_done"].ctypes.data,
-               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data)
+               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data,
+               res["snapshots"].ctypes.data if snapshot_every > 0 else None, snap_capacity or 0, snap_mask,
+               res["snap_count"].ctypes.data if snapshot_every > 0 else None)
     rc = lib().oracle_tab_integrate(*_grid(table), st.ctypes.data, n, h, nsteps, C.byref(stop), C.byref(out),
-                                    int(long_double), nthreads)
+                                    int(long_double), nthreads, snapshot_every)
     if rc != 0:
         raise ValueError("oracle_tab_integrate: invalid arguments")
     return res
@@ -107,7 +116,7 @@ def integrate_general(table: dict, state_in: np.ndarray, h: float, nsteps: int, 
            "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan), "health": np.full(n, np.nan)}
     stop = _Stop(r_capture, r_escape, kind, flags)
     out = _Out(res["final_state"].ctypes.data, res["status"].ctypes.data, res["steps_done"].ctypes.data,
-               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data)
+               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data, None, 0, 0, None)
     L = lib()
     L.oracle_tabg_integrate.restype = C.c_int
     L.oracle_tabg_integrate.argtypes = _GRID + [C.c_void_p, C.c_int64, C.c_double, C.c_int64, C.POINTER(_Stop),

@@ -357,3 +357,58 @@ def test_config3a_full_image_adaptive_sampled(G, oracle):
     assert cert.sum() > 0.9 * esc.sum() and same.mean() >= 0.95
     assert (g["status"] == o["status"])[cert].all()
     assert e_ray[cert].max() <= 1e-8 and e_along[cert].max() <= 1e-6, (e_ray[cert].max(), e_along[cert].max())
+
+
+def test_config3a_full_image_adaptive_dense_records_cover_captured_rays_too(G, oracle):
+    """Round-1 verdict ('what's weak' 4): at full image size the adaptive path's CAPTURED rays were compared by class only,
+    because their final record is the last accepted state, and where that lies depends on the step-size noise.  With
+    dense output (reading A3) every ray -- captured or escaped -- has records at the SAME affine times tau_j = 100 j on
+    both sides: all 1024^2 rays are traced with records, 6000 sampled rays (captured ones over-sampled) are compared record
+    by record at 1e-8 under reading P3, and the number of records may differ by at most the last one."""
+    import torch
+    a, N = 0.998, 1024
+    st, consts = W.camera_rays(N, a, 60.0, return_constants=True)
+    rc = W.horizon_radius(1.0, a) + 0.01
+    dev = torch.device("cuda:0")
+    cap, dtau = 24, 100.0
+    ctx = G.geo_create(G.KERR, 1.0, a)
+    try:
+        out = G.alloc_outputs(N * N, dev, 0, 1, cap, 0x6F)              # t, r, theta, phi, p_r, p_theta
+        rej = torch.zeros(N * N, dtype=torch.int32, device=dev)
+        G.geo_integrate_adaptive(ctx, torch.from_numpy(st).to(dev), 0.02, 1e-9, 1e-9, 200000, out, r_capture=rc,
+                                 r_escape=1100.0, kind=G.NULL, rejected=rej, snap_dtau=dtau)
+        torch.cuda.synchronize()
+    finally:
+        G.geo_destroy(ctx)
+    status = out["status"].cpu().numpy()
+    rng = np.random.default_rng(14)
+    ii = np.sort(np.concatenate([rng.choice(np.flatnonzero(status == G.ST_CAPTURED), 3000, replace=False),
+                                 rng.choice(np.flatnonzero(status == G.ST_ESCAPED), 3000, replace=False)]))
+    g = _take(out, ii, with_snaps=True)
+    kw = dict(r_capture=rc, r_escape=1100.0, kind=oracle.NULL, nthreads=NCPU, snap_dtau=dtau, snap_capacity=cap, snap_mask=0x6F)
+
+    def run(sub, **extra):
+        return oracle.integrate_adaptive(oracle.KERR, 1.0, a, np.ascontiguousarray(sub), 0.02, 1e-9, 1e-9, 200000, **kw, **extra)
+    o = run(st[:, ii])
+    assert np.array_equal(g["status"], o["status"])
+    assert (np.abs(g["snap_count"].astype(int) - o["snap_count"]) <= 1).all()
+
+    def common_records_err(x, y):
+        """worst P2 error over the records BOTH runs produced (the last record may exist on one side only)."""
+        m = np.minimum(np.minimum(x["snap_count"], y["snap_count"]), cap)
+        valid = np.arange(cap)[None, :] < m[:, None]
+        return np.where(valid[:, :, None], parity.rel_err(x["snapshots"], y["snapshots"]), 0.0).max(axis=(1, 2))
+    err = common_records_err(g, o)
+    fail = np.flatnonzero(~(err <= 1e-8))
+    print(f"adaptive dense records, {len(ii)} rays (3000 captured): max err {err.max():.3e}, outside 1e-8: {len(fail)}")
+    assert len(fail) <= 0.03 * len(ii)
+    if len(fail):                                                       # reading P3: they must be uncertified
+        o_sub = parity.take(o, fail)
+        cert = np.ones(len(fail), dtype=bool)
+        for o_c in (run(st[:, ii[fail]], long_double=True), run(parity.ulp_nudged(st[:, ii[fail]]))):
+            cert &= (o_c["status"] == o_sub["status"]) & (common_records_err(o_sub, o_c) <= 1e-9)
+        for k, i in enumerate(fail[:12]):
+            print(f"   ray {ii[i]} status {g['status'][i]} err {err[i]:.3e} certified {bool(cert[k])} (alpha, beta, Lz, Q) = {consts[:, ii[i]]}")
+        assert not cert.any()
+    captured = g["status"] == G.ST_CAPTURED
+    assert (g["snap_count"][captured] >= 10).all()                      # ~1000 M of affine time to the hole: >= 10 records each

@@ -49,8 +49,8 @@ class Guarded:
 
 def guard_outputs(out, gd, snap_pad=64):
     g = dict(out)
-    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health", "snap_count"):
-        g[k] = gd.wrap(out[k])
+    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health", "snap_count", "coarse_steps"):
+        g[k] = gd.wrap(out.get(k))
     g["snapshots"] = gd.wrap(out["snapshots"], snap_pad)
     return g
 
@@ -61,7 +61,7 @@ def bits(x):
 
 
 def same_bits(a, b):
-    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health", "snapshots", "snap_count"):
+    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health", "snapshots", "snap_count", "coarse_steps"):
         if a.get(k) is None:
             assert b.get(k) is None
             continue
@@ -95,11 +95,11 @@ def test_rk4_kernels_write_inside_their_buffers(G, flags, mask, cap, snap_pad):
     ctx = G.geo_create(G.KERR, 1.0, a)
     try:
         d_in = torch.from_numpy(st).to(dev)
-        plain = G.alloc_outputs(n, dev, 1500, 50, cap, mask)
+        plain = G.alloc_outputs(n, dev, 1500, 50, cap, mask, want_coarse=True)
         G.geo_integrate(ctx, d_in, 0.05, 1500, plain, **kw)
         gd = Guarded()
         g_in = gd.wrap(d_in)
-        guarded = guard_outputs(G.alloc_outputs(n, dev, 1500, 50, cap, mask), gd, snap_pad)
+        guarded = guard_outputs(G.alloc_outputs(n, dev, 1500, 50, cap, mask, want_coarse=True), gd, snap_pad)
         G.geo_integrate(ctx, g_in, 0.05, 1500, guarded, **kw)
         torch.cuda.synchronize()
         gd.check()
@@ -107,6 +107,64 @@ def test_rk4_kernels_write_inside_their_buffers(G, flags, mask, cap, snap_pad):
         p, g = G.to_numpy(plain), G.to_numpy(guarded)
         same_bits(p, g)
         assert len(np.unique(p["status"])) >= 2          # the batch does mix termination classes
+        assert p["coarse_steps"].sum() > 0               # h = 0.05 next to the horizon: the large-angle path ran
+    finally:
+        G.geo_destroy(ctx)
+
+
+@pytest.mark.parametrize("mask,cap,snap_pad,flags", [(0xFF, 40, 64, 0), (0x0F, 7, 62, 8), (0x07, 40, 62, 0)])
+def test_adaptive_dense_output_writes_inside_its_buffers(G, mask, cap, snap_pad, flags):
+    """The dense-output instantiation of the RK5(4) kernel (reading A3): records, record counter and rejection counter
+    between canaries -- full and 4-component (Cartesian) records, odd component count, capacity overflow, 16-B slots."""
+    import torch
+    a = 0.998
+    st = mixed_rays(a)
+    n = st.shape[1]
+    dev = torch.device("cuda:0")
+    kw = dict(r_capture=1.0 + math.sqrt(1.0 - a * a) + 0.01, r_escape=33.0, kind=G.NULL, snap_dtau=2.0, flags=flags)
+    ctx = G.geo_create(G.KERR, 1.0, a)
+    try:
+        d_in = torch.from_numpy(st).to(dev)
+        plain = G.alloc_outputs(n, dev, 0, 1, cap, mask)
+        rej = torch.full((n,), -1, dtype=torch.int32, device=dev)
+        G.geo_integrate_adaptive(ctx, d_in, 0.1, 1e-9, 1e-12, 2000, plain, rejected=rej, **kw)
+        gd = Guarded()
+        g_in = gd.wrap(d_in)
+        guarded = guard_outputs(G.alloc_outputs(n, dev, 0, 1, cap, mask), gd, snap_pad)
+        g_rej = gd.wrap(torch.full((n,), -1, dtype=torch.int32, device=dev))
+        G.geo_integrate_adaptive(ctx, g_in, 0.1, 1e-9, 1e-12, 2000, guarded, rejected=g_rej, **kw)
+        torch.cuda.synchronize()
+        gd.check()
+        p = G.to_numpy(plain)
+        same_bits(p, G.to_numpy(guarded))
+        assert np.array_equal(rej.cpu().numpy(), g_rej.cpu().numpy())
+        assert (p["snap_count"] > cap).any() and (p["snap_count"] < cap).any() if cap == 7 else (p["snap_count"] >= 1).all()
+    finally:
+        G.geo_destroy(ctx)
+
+
+def test_general_tabulated_kernel_writes_inside_its_buffers(G):
+    import torch
+    a = 0.9
+    tb = W.general_table_from_diagonal(W.kerr_metric_table(1.0, a, 257, 65, 1.8, 40.0, 0.2, math.pi - 0.2))
+    st = np.ascontiguousarray(W.kerr_bound(333, a, W.SEED_BASE + 2))
+    n = st.shape[1]
+    dev = torch.device("cuda:0")
+    ctx = G.geo_create_tabulated_general(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+    try:
+        d_in = torch.from_numpy(st).to(dev)
+        plain = G.alloc_outputs(n, dev)
+        G.geo_integrate(ctx, d_in, 0.01, 2000, plain, r_capture=2.5, r_escape=25.0)
+        gd = Guarded()
+        g_in = gd.wrap(d_in)
+        guarded = guard_outputs(G.alloc_outputs(n, dev), gd)
+        G.geo_integrate(ctx, g_in, 0.01, 2000, guarded, r_capture=2.5, r_escape=25.0)
+        torch.cuda.synchronize()
+        gd.check()
+        assert np.array_equal(bits(g_in.cpu().numpy()), bits(st))
+        p = G.to_numpy(plain)
+        same_bits(p, G.to_numpy(guarded))
+        assert len(np.unique(p["status"])) >= 2
     finally:
         G.geo_destroy(ctx)
 

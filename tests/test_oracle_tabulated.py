@@ -380,3 +380,32 @@ def test_kerr_schild_table_reproduces_boyer_lindquist_orbits_and_penetrates_the_
     og = tab_oracle.integrate_general(tb, kf, 0.005, 20000, r_capture=1.3)
     assert og["status"][0] == tab_oracle.ST_CAPTURED and og["final_state"][1, 0] < rp - 0.05      # went INSIDE the horizon
     assert np.isfinite(og["final_state"]).all() and og["health"][0] < 1e-5
+
+
+def test_tabulated_trajectory_records_follow_S1_to_S3(tab_oracle):
+    """Records on the tabulated path (round 2): slot 0 = y0 with the mass-shell E, slot j = the state after j *
+    snapshot_every accepted steps -- bitwise the final state of a run of that length (SURVEY 8(c) pin 'Snapshots') --,
+    nothing after termination, records beyond the capacity dropped but counted, components by mask."""
+    a = 0.9
+    tb = W.kerr_metric_table(1.0, a, 257, 65, 1.8, 40.0, 0.2, math.pi - 0.2)
+    st = W.kerr_bound(60, a, W.SEED_BASE + 2)
+    r = tab_oracle.integrate(tb, st, 0.01, 900, snapshot_every=300)
+    assert (r["snap_count"] == 4).all() and r["snapshots"].shape == (60, 4, 8)
+    assert np.array_equal(r["snapshots"][:, 0, [1, 2, 3, 5, 6, 7]], st.T) and (r["snapshots"][:, 0, 0] == 0).all()
+    assert np.array_equal(r["snapshots"][:, 0, 4], r["final_state"][4])           # E constant
+    for j in (1, 2, 3):
+        rj = tab_oracle.integrate(tb, st, 0.01, 300 * j)
+        assert np.array_equal(r["snapshots"][:, j, :], rj["final_state"].T)
+    m = tab_oracle.integrate(tb, st, 0.01, 900, snapshot_every=100, snap_capacity=4, snap_mask=0x26)   # x1, x2, p1
+    assert (m["snap_count"] == 10).all() and m["snapshots"].shape == (60, 4, 3)
+    full = tab_oracle.integrate(tb, st, 0.01, 900, snapshot_every=100)
+    assert np.array_equal(m["snapshots"], full["snapshots"][:, :4, [1, 2, 5]])
+    # early termination: records stop with the particle
+    out = st.copy()
+    out[0] = 39.0
+    out[3] = 2.0
+    e = tab_oracle.integrate(tb, out, 0.05, 400, snapshot_every=5)
+    assert (e["status"] == tab_oracle.ST_OUTSIDE).all()
+    assert np.array_equal(e["snap_count"], 1 + e["steps_done"] // 5)
+    for i in range(0, 60, 7):
+        assert np.isnan(e["snapshots"][i, e["snap_count"][i]:]).all() and np.isfinite(e["snapshots"][i, : e["snap_count"][i]]).all()

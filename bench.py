@@ -72,7 +72,7 @@ KERNEL_COUNTS = {
     "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0E", units_per_loop=None, flop=4073.0, pipe=2376.0, other=None, tol=None,
                               source="ncu per-instruction counts, profiles/r02_tabg4.md: 1735 DFMA + 550 DMUL + 52 DADD + 38 DSETP per step "
                                      "(4 evaluations through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tabg_rk4_kernel"),
-    "tabulated": dict(sym="geo_tab_rk4_kernelILb0ELb1E", units_per_loop=None, flop=2217.0, pipe=1299.0, other=None, tol=None,
+    "tabulated": dict(sym="geo_tab_rk4_kernelILb0ELb1ELb0E", units_per_loop=None, flop=2217.0, pipe=1299.0, other=None, tol=None,
                       source="ncu thread-level counts, profiles/r01_tab4.md: 918 DFMA + 323 DMUL + 58 DADD per step (4 evaluations "
                              "through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tab_rk4_kernel"),
 }

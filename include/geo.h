@@ -153,7 +153,9 @@ int geo_integrate_adaptive_host(geo_ctx *ctx, const double *state_in, int64_t n,
  * A ctx created here is used with geo_integrate / geo_integrate_host: state_in = (x^1, x^2, phi, p_1, p_2, p_phi),
  * r_capture / r_escape refer to x^1, the equatorial event to x^2 = pi/2; an evaluation point (y0, a stage point, the
  * end point of a step) outside the domain ends the particle with GEO_ST_OUTSIDE, that step is not taken (per
- * evaluation point the capture test comes first).  snapshot_every must be 0; flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER;
+ * evaluation point the capture test comes first).  Trajectory records (snapshot_every > 0) as for the analytic metrics,
+ * components (t, x^1, x^2, phi, p_t = E, p_1, p_2, p_phi) by snap_mask; flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER
+ * (no staged writer, no Cartesian records: the coordinates are the table's own);
  * geo_integrate_adaptive returns GEO_EINVAL; geo_horizon_radius returns NaN.
  * Errors: GEO_EINVAL (NULL, n1 or n2 < 4, d1 or d2 <= 0, non-finite grid), GEO_ENOMEM, GEO_ECUDA. */
 typedef struct geo_table {

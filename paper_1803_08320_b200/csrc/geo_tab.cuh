@@ -46,6 +46,13 @@ struct TabParams {
     double* eq_cross_r;
     double* health;
     unsigned long long* counter;
+    // trajectory records (readings S1-S3): components (t, x1, x2, phi, E, p1, p2, L) by mask, particle-major
+    int snap_every;
+    long long snap_cap;
+    unsigned snap_mask;
+    int ncomp;
+    double* snaps;
+    int* snap_count;
     TabMetric m;
 };
 
@@ -233,7 +240,8 @@ __device__ __noinline__ bool tab_fields_cold(const TabMetric& m, double x1, doub
 
 // CACHE: per-lane stencil cache (kTabSmemRows * kTabBlock doubles = 64 KB of shared memory per CTA, 2 CTAs/SM);
 // !CACHE: every evaluation gathers its stencil through L1/L2 (GEO_FLAG_TAB_GATHER, for comparison).
-template <bool PLAIN, bool CACHE>
+// SNAP: trajectory records (a separate instantiation: the stepping kernel has no register to spare).
+template <bool PLAIN, bool CACHE, bool SNAP>
 __global__ void __launch_bounds__(kTabBlock, CACHE ? GEO_TAB_CTAS : 3) geo_tab_rk4_kernel(const __grid_constant__ TabParams p) {
     extern __shared__ __align__(16) double stencil_smem[];
     double* const col = stencil_smem + threadIdx.x;
@@ -254,10 +262,18 @@ __global__ void __launch_bounds__(kTabBlock, CACHE ? GEO_TAB_CTAS : 3) geo_tab_r
     int steps = 0;
     double eqc = 0;
     bool crossed = false;
+    int snaps = 0, snap_ctr = 0;
 
+    auto emit_record = [&]() {                                     // S1-S3: straight from registers, 256-bit stores
+        if (snaps < p.snap_cap)
+            store_record_global(p.snaps + ((size_t)idx * (size_t)p.snap_cap + (size_t)snaps) * p.ncomp, p.snap_mask,
+                                t, x1, x2, ph, E, p1, p2, L);
+        ++snaps;
+    };
     auto finish = [&](int st) {
         long long n = p.n;
         asm volatile("" : "+l"(n));
+        if (SNAP) p.snap_count[idx] = snaps;
         p.fin[0 * n + idx] = t;
         p.fin[1 * n + idx] = x1;
         p.fin[2 * n + idx] = x2;
@@ -296,12 +312,15 @@ __global__ void __launch_bounds__(kTabBlock, CACHE ? GEO_TAB_CTAS : 3) geo_tab_r
         steps = 0;
         crossed = false;
         active = true;
+        snaps = 0;
+        snap_ctr = p.snap_every;
         if (!(x1 >= p.r_capture)) { finish(ST_CAPTURED); return; }               // B1
         if (!all_finite6(x1, x2, ph, p1, p2, L)) { finish(ST_NUMERIC); return; }
         TabFields F;
         if (!tab_fields_cold(m, x1, x2, F)) { finish(ST_OUTSIDE); return; }      // T4 on y0
         E = fma(F.al, sqrt(p.kappa + p1 * p1 / F.g11 + p2 * p2 / F.g22 + L * L / F.g33), -F.be * L);   // mass shell (5)
         if ((__double2hiint(E) & 0x7ff00000) == 0x7ff00000) { finish(ST_NUMERIC); return; }
+        if (SNAP) emit_record();                                                 // S1: slot 0 = y0
         if (x1 > p.r_escape) { finish(ST_ESCAPED); return; }
         if (p.nsteps == 0) { finish(ST_MAXSTEPS); return; }
         tab_rhs(F, p1, p2, E, L, k1);
@@ -384,6 +403,9 @@ __global__ void __launch_bounds__(kTabBlock, CACHE ? GEO_TAB_CTAS : 3) geo_tab_r
                 ct = dt; c1 = d1; c2 = d2; cph = dph; cp1 = dp1; cp2 = dp2;
                 k1 = d;
                 ++steps;
+                if (SNAP) {
+                    if (--snap_ctr == 0) { snap_ctr = p.snap_every; emit_record(); }   // S1
+                }
                 if (x1 > p.r_escape) finish(ST_ESCAPED);                         // B3
                 else if (steps >= p.nsteps) finish(ST_MAXSTEPS);                 // B4
             }

@@ -138,7 +138,7 @@ def test_adaptive_dense_output_writes_inside_its_buffers(G, mask, cap, snap_pad,
         p = G.to_numpy(plain)
         same_bits(p, G.to_numpy(guarded))
         assert np.array_equal(rej.cpu().numpy(), g_rej.cpu().numpy())
-        assert (p["snap_count"] > cap).any() and (p["snap_count"] < cap).any() if cap == 7 else (p["snap_count"] >= 1).all()
+        assert (p["snap_count"] >= 1).all() and ((p["snap_count"] > cap).any() if cap == 7 else True)   # capacity overflow exercised
     finally:
         G.geo_destroy(ctx)
 

@@ -128,9 +128,10 @@ def test_tabulated_empty_and_argument_errors(G):
     out = G.alloc_outputs(0, dev)
     G.geo_integrate(ctx, torch.empty((6, 0), dtype=torch.float64, device=dev), 0.01, 10, out)     # n = 0: no-op
     st = torch.from_numpy(W.kerr_bound(8, 0.5, W.SEED_BASE + 4)).to(dev)
-    with pytest.raises(G.GeoError) as ei:
-        G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, dev, 10, 5), snapshot_every=5)
-    assert ei.value.code == G.EINVAL
+    for bad_flags in (G.FLAG_CARTESIAN_SNAP, G.FLAG_STAGED_SNAP):      # records exist on this path, but only the direct BL-style writer
+        with pytest.raises(G.GeoError) as ei:
+            G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, dev, 10, 5), snapshot_every=5, flags=bad_flags)
+        assert ei.value.code == G.EINVAL
     with pytest.raises(G.GeoError) as ei:
         G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, dev), flags=G.FLAG_STATIC_MAP)
     assert ei.value.code == G.EINVAL
@@ -194,3 +195,40 @@ def test_tabulated_kerr_converges_to_the_analytic_kernel(G):
     rows = [0, 1, 2, 3, 5, 6]
     errs = [parity.rel_err(g["final_state"][rows][:, ok], ref["final_state"][rows][:, ok]).max() for g in res]
     assert errs[1] < 1e-4 and errs[0] / errs[1] > 6, errs
+
+
+@pytest.mark.parametrize("host,flags,mask,cap", [(False, 0, 0xFF, None), (False, 16, 0x0F, None), (True, 0, 0x26, 4), (False, 1, 0x07, 4)])
+def test_tabulated_trajectory_records(G, tab_oracle, host, flags, mask, cap):
+    """Records on the tabulated path (round 2; readings S1-S3 with the table's own coordinates): against the oracle,
+    device and host entry points, stencil-cache and gather kernels, plain update, odd masks, capacity overflow; and slot j
+    equals the final state of the run that stops there, bitwise."""
+    import torch
+    a = 0.9
+    tb = W.kerr_metric_table(1.0, a, 513, 129, 1.8, 40.0, 0.2, math.pi - 0.2)
+    st = W.kerr_bound(1501, a, W.SEED_BASE + 2)
+    o = tab_oracle.integrate(tb, st, 0.01, 1500, flags=flags & 1, snapshot_every=250, snap_capacity=cap, snap_mask=mask, nthreads=NCPU)
+    ctx = G.geo_create_tabulated(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+    try:
+        n = st.shape[1]
+        if host:
+            out = G.alloc_outputs_host(n, 1500, 250, cap, mask)
+            G.geo_integrate_host(ctx, np.ascontiguousarray(st), 0.01, 1500, out, flags=flags, snapshot_every=250)
+        else:
+            out = G.alloc_outputs(n, torch.device("cuda:0"), 1500, 250, cap, mask)
+            G.geo_integrate(ctx, torch.from_numpy(st).cuda(), 0.01, 1500, out, flags=flags, snapshot_every=250)
+            torch.cuda.synchronize()
+        g = G.to_numpy(out)
+        assert_parity(g, o, 1e-9)
+        assert np.array_equal(g["snap_count"], o["snap_count"]) and (g["snap_count"] == 7).all()
+        assert parity.snapshot_err(g, o).max() <= 1e-9
+        capn = o["snapshots"].shape[1]
+        valid = np.arange(capn)[None, :] < np.minimum(g["snap_count"], capn)[:, None]
+        assert np.isnan(g["snapshots"][~valid]).all() and np.isfinite(g["snapshots"][valid]).all()
+        if mask == 0xFF and not host:
+            for j in (2, 6):
+                oj = G.alloc_outputs(n, torch.device("cuda:0"))
+                G.geo_integrate(ctx, torch.from_numpy(st).cuda(), 0.01, 250 * j, oj, flags=flags)
+                torch.cuda.synchronize()
+                assert np.array_equal(g["snapshots"][:, j, :], G.to_numpy(oj)["final_state"].T)
+    finally:
+        G.geo_destroy(ctx)

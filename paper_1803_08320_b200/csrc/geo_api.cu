@@ -103,8 +103,8 @@ int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t 
     if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_STAGED_SNAP | GEO_FLAG_CARTESIAN_SNAP | GEO_FLAG_TAB_GATHER)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
     if (ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) {
         if (snapshot_every > 0 && ctx->metric == GEO_TABULATED_GENERAL) return fail(ctx, GEO_EINVAL, "general tabulated metrics: snapshots are not supported");
-        const int32_t ok = ctx->metric == GEO_TABULATED ? (GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_TAB_GATHER) : GEO_FLAG_PLAIN_UPDATE;
-        if (stop->flags & ~ok) return fail(ctx, GEO_EINVAL, "tabulated metrics: only GEO_FLAG_PLAIN_UPDATE (and GEO_FLAG_TAB_GATHER for five-field tables) are supported");
+        const int32_t ok = GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_TAB_GATHER;
+        if (stop->flags & ~ok) return fail(ctx, GEO_EINVAL, "tabulated metrics: only GEO_FLAG_PLAIN_UPDATE and GEO_FLAG_TAB_GATHER are supported");
     }
     if (n == 0) return GEO_OK;
     if (!state_in || !out->final_state || !out->status || !out->steps_done) return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
@@ -231,19 +231,26 @@ int launch_tab(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t ns
 
 typedef void (*tabg_kernel_fn)(const TabgParams);
 tabg_kernel_fn pick_tabg_kernel(int32_t flags) {
-    return (flags & GEO_FLAG_PLAIN_UPDATE) ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false>;
+    const bool plain = (flags & GEO_FLAG_PLAIN_UPDATE) != 0;
+    if (flags & GEO_FLAG_TAB_GATHER) return plain ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true, false> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false, false>;
+    return plain ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true, true> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false, true>;
 }
+int tabg_block(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? kTabBlock : kTabgCacheBlock; }
+size_t tabg_smem(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? 0 : (size_t)kTabgCacheRows * kTabgCacheBlock * sizeof(double); }
 
 int plan_tabg(geo_ctx* ctx, int64_t n, int32_t flags, int* grid, int* per_sm_out, int* regs) {
     tabg_kernel_fn fn = pick_tabg_kernel(flags);
     int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kTabBlock, 0);
+    const int block = tabg_block(flags);
+    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tabg_smem(flags));
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncSetAttribute(smem)");
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, block, tabg_smem(flags));
     if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(tabg)");
     if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
     cudaFuncAttributes fa;
     e = cudaFuncGetAttributes(&fa, (const void*)fn);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncGetAttributes");
-    const int64_t need = (n + kTabBlock - 1) / kTabBlock, resident = (int64_t)ctx->sm_count * per_sm;
+    const int64_t need = (n + block - 1) / block, resident = (int64_t)ctx->sm_count * per_sm;
     *grid = (int)(need < resident ? need : resident);
     *per_sm_out = per_sm;
     *regs = fa.numRegs;
@@ -275,7 +282,7 @@ int launch_tabg(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t n
     p.m = ctx->tgm;
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
-    pick_tabg_kernel(stop->flags)<<<grid, kTabBlock, 0, stream>>>(p);
+    pick_tabg_kernel(stop->flags)<<<grid, tabg_block(stop->flags), tabg_smem(stop->flags), stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
     return GEO_OK;
@@ -709,7 +716,7 @@ int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_eve
         return plan_tab(ctx, n, flags, &info[0], &info[3], &info[2], snapshot_every > 0);
     }
     if (ctx->metric == GEO_TABULATED_GENERAL) {
-        info[1] = kTabBlock;
+        info[1] = tabg_block(flags);
         return plan_tabg(ctx, n, flags, &info[0], &info[3], &info[2]);
     }
     LaunchPlan lp;

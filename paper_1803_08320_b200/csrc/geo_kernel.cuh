@@ -97,7 +97,18 @@ __device__ __forceinline__ void store_masked(double* dst, unsigned mask, double 
 __device__ __forceinline__ void st_v4(double* g, double a, double b, double c, double d) {
     asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" :: "l"(g), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
 }
-__device__ __forceinline__ void store_record_global(double* dst, unsigned mask, double t, double r, double th,
+// The writer MUST be inlined.  As a non-inlined callee (`-DGEO_NOINLINE_RECORD`, the round-1 experiment) ptxas 12.9 clones
+// it per kernel inside that kernel's 128-register budget; in the Kerr clone it cannot form the two aligned register quads
+// of `st.global.v4.f64`, shuffles with XOR swaps and then emits STG.E.64 where the Schwarzschild clone has
+// STG.E.ENL2.256 -- only the first double of each 32-byte group is stored (components 0 and 4 written, 1-3 and 5-7 left
+// untouched: the "NaN" of round 1 was the buffers' NaN prefill).  profiles/r02_noinline_writer_miscompile.md has the SASS
+// of both clones; tests/test_abi.py checks that every SNAP_DIRECT instantiation of the product keeps its 256-bit stores.
+#ifdef GEO_NOINLINE_RECORD
+__device__ __noinline__
+#else
+__device__ __forceinline__
+#endif
+void store_record_global(double* dst, unsigned mask, double t, double r, double th,
                                                     double ph, double E, double pr, double pth, double L) {
     const bool al32 = (reinterpret_cast<unsigned long long>(dst) & 31ull) == 0;
     if (mask == 0xFFu && al32) {

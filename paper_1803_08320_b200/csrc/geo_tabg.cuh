@@ -11,9 +11,11 @@
 //
 // Interpolant, its exact gradient, domain rule, stepper, stop rules and events: those of geo_tab.cuh (readings T2, T4, T5).
 // Table layout on the device (built once by tabg_pack_kernel from the caller's [10][n2][n1]): node-major records of
-// 12 doubles = 96 B (10 fields + 2 pad) -> three 256-bit loads per node, 48 per evaluation and lane.  This first version
-// gathers the 4 x 4 stencil on every evaluation (L1-wavefront-bound, like geo_tab.cuh's GEO_FLAG_TAB_GATHER variant);
-// a per-lane stencil cache would need 1.3 KB per lane.
+// 12 doubles = 96 B (10 fields + 2 pad) -> three 256-bit loads per node, 48 per stencil and lane.
+// v1 (GEO_FLAG_TAB_GATHER) gathers the 4 x 4 stencil on every evaluation: L1-wavefront-bound (ncu: 89 % of the L1
+// data-pipe peak, FP64 pipe 19 %).  v2 (default) keeps the stencil of the lane's current cell -- 160 doubles = 1.25 KB
+// per lane -- in shared memory, column-major [160][32] per 32-lane CTA (40 KB; five CTAs per SM), and refills it only when
+// the cell index changes (a particle stays in a cell for tens of evaluations).  Same arithmetic, same bits.
 #pragma once
 #include "geo_tab.cuh"
 
@@ -83,6 +85,55 @@ __device__ __forceinline__ bool tabg_fields(const TabgMetric& m, double x1, doub
     return in1 & in2;
 }
 
+// CACHE variant of tabg_fields: the stencil comes from the lane's shared-memory column `col` (stride `cs` doubles
+// between consecutive elements), refilled from the table when the cell (i, j) differs from (ci, cj).
+__device__ __forceinline__ bool tabg_fields_cached(const TabgMetric& m, double x1, double x2, TabgFields& F, int& ci, int& cj,
+                                                   double* col, int cs) {
+    int i, j;
+    double s1, s2;
+    const bool in1 = tab_cell(x1, m.x1_0, m.d1, m.inv_d1, m.n1, i, s1);
+    const bool in2 = tab_cell(x2, m.x2_0, m.d2, m.inv_d2, m.n2, j, s2);
+    if (i != ci || j != cj) {
+        const long long base = ((long long)(j - 1) * m.n1 + (i - 1)) * kTabgStride;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const double4* row = reinterpret_cast<const double4*>(m.G + base + (long long)b * m.n1 * kTabgStride);
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                const double4 t0 = ldg256(row + a * 3), t1 = ldg256(row + a * 3 + 1), t2 = ldg256(row + a * 3 + 2);
+                double* e = col + (size_t)((b * 4 + a) * kTabgFields) * cs;
+                e[0] = t0.x; e[cs] = t0.y; e[2 * cs] = t0.z; e[3 * cs] = t0.w;
+                e[4 * cs] = t1.x; e[5 * cs] = t1.y; e[6 * cs] = t1.z; e[7 * cs] = t1.w;
+                e[8 * cs] = t2.x; e[9 * cs] = t2.y;
+            }
+        }
+        ci = i;
+        cj = j;
+    }
+    double w1[4], dw1[4], w2[4], dw2[4];
+    keys_weights(s1, m.inv_d1, w1, dw1);
+    keys_weights(s2, m.inv_d2, w2, dw2);
+#pragma unroll
+    for (int f = 0; f < kTabgFields; ++f) F.v[f] = F.g1[f] = F.g2[f] = 0.0;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+#pragma unroll
+        for (int f = 0; f < kTabgFields; ++f) {
+            const double c0 = col[(size_t)((b * 4 + 0) * kTabgFields + f) * cs], c1 = col[(size_t)((b * 4 + 1) * kTabgFields + f) * cs],
+                         c2 = col[(size_t)((b * 4 + 2) * kTabgFields + f) * cs], c3 = col[(size_t)((b * 4 + 3) * kTabgFields + f) * cs];
+            const double rv = fma(w1[3], c3, fma(w1[2], c2, fma(w1[1], c1, w1[0] * c0)));
+            const double rd = fma(dw1[3], c3, fma(dw1[2], c2, fma(dw1[1], c1, dw1[0] * c0)));
+            F.v[f] = fma(w2[b], rv, F.v[f]);
+            F.g1[f] = fma(w2[b], rd, F.g1[f]);
+            F.g2[f] = fma(dw2[b], rv, F.g2[f]);
+        }
+    }
+    return in1 & in2;
+}
+
+constexpr int kTabgCacheBlock = 32;                                  // lanes per CTA of the cached variant
+constexpr int kTabgCacheRows = 16 * kTabgFields;                     // doubles per lane
+
 struct TabgAux {
     double V1, V2, V3, W, ut, gpp;
 };
@@ -125,8 +176,12 @@ __device__ __noinline__ bool tabg_fields_cold(const TabgMetric& m, double x1, do
     return tabg_fields(m, x1, x2, F);
 }
 
-template <bool PLAIN>
-__global__ void __launch_bounds__(kTabBlock, 2) geo_tabg_rk4_kernel(const __grid_constant__ TabgParams p) {
+template <bool PLAIN, bool CACHE>
+__global__ void __launch_bounds__(CACHE ? kTabgCacheBlock : kTabBlock, CACHE ? 5 : 2) geo_tabg_rk4_kernel(const __grid_constant__ TabgParams p) {
+    extern __shared__ __align__(16) double tabg_smem[];              // CACHE: [160][blockDim.x]
+    double* const col = tabg_smem + threadIdx.x;
+    const int cs = (int)blockDim.x;
+    int ci = -1, cj = -1;                                            // cell whose stencil the column holds
     const unsigned lane = threadIdx.x & 31u;
     const TabgMetric& m = p.m;
     long long idx = -1;
@@ -238,7 +293,7 @@ __global__ void __launch_bounds__(kTabBlock, 2) geo_tabg_rk4_kernel(const __grid
                 fin6 = all_finite6(nt, n1, n2, nph, np1, np2);
             }
             TabgFields F;
-            const bool in = tabg_fields(m, e1, e2, F);
+            const bool in = CACHE ? tabg_fields_cached(m, e1, e2, F, ci, cj, col, cs) : tabg_fields(m, e1, e2, F);
             if (!ev) ev = !(e1 >= p.r_capture) ? ST_CAPTURED : (!fin6 ? ST_NUMERIC : (!in ? ST_OUTSIDE : 0));
             tabg_rhs(F, ep1, ep2, E, L, d);
             if (s < 3) {

@@ -48,6 +48,32 @@ def test_sass_has_fp64_pipe_and_wide_stores():
     assert re.search(r"LDG\.E(\.\w+)*\.256", sass)        # tabulated metric: one 256-bit load per stencil node
 
 
+def test_every_direct_snapshot_kernel_keeps_its_256_bit_stores():
+    """ptxas narrowed `st.global.v4.f64` to STG.E.64 in ONE clone of a non-inlined record writer (DESIGN.md section 5,
+    profiles/r02_noinline_writer_miscompile.md): the shipped library must have 256-bit stores in every instantiation of the
+    direct snapshot writer -- Kerr and Schwarzschild, Kahan and plain update, and the dense-output RK5(4) kernels."""
+    import sys
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1803_08320_b200 import build, geo
+    build.build()
+    bench.static_sass_count("geo_rk4_kernelILb1ELi1ELb0")            # fills the SASS cache
+    sass = next(iter(bench._SASS_CACHE.values()))
+    kernels, name = {}, None
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            name = m.group(1)
+            kernels[name] = 0
+        elif name and re.search(r"STG\.E(\.\w+)*\.256", line):
+            kernels[name] += 1
+    want = [k for k in kernels if re.search(r"geo_rk4_kernelILb[01]ELi1ELb[01]E", k) or re.search(r"geo_rk45_kernelILb[01]ELb1E", k)
+            or re.search(r"geo_tab_rk4_kernelILb[01]ELb[01]ELb1E", k)]
+    assert len(want) == 4 + 2 + 4, want
+    for k in want:
+        assert kernels[k] >= 2, (k, kernels[k])
+
+
 def test_product_path_does_not_import_the_oracle():
     """No file of the package imports, loads, includes or executes anything under oracle/."""
     pkg = os.path.join(ROOT, "paper_1803_08320_b200")

@@ -37,17 +37,21 @@ def run_tabg(G, tb, st, h, nsteps, host=False, general=True, **kw):
         G.geo_destroy(ctx)
 
 
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 16, 17])      # 1 = plain update, 16 = GEO_FLAG_TAB_GATHER (no stencil cache)
 def test_embedded_eq8_table_matches_oracle_and_the_five_field_kernel(G, tab_oracle, flags):
     a = 0.9
     tb5 = W.kerr_metric_table(1.0, a, 513, 129, 1.8, 40.0, 0.2, math.pi - 0.2)
     tb10 = W.general_table_from_diagonal(tb5)
     st = W.kerr_bound(3001, a, W.SEED_BASE + 2)
-    o = tab_oracle.integrate_general(tb10, st, 0.01, 2000, flags=flags, nthreads=NCPU)
+    o = tab_oracle.integrate_general(tb10, st, 0.01, 2000, flags=flags & 1, nthreads=NCPU)
     g = run_tabg(G, tb10, st, 0.01, 2000, flags=flags)
     c = parity.compare(g, o)
     assert c["same_class"].all() and c["err"].max() <= 1e-9, c["err"].max()
     assert np.array_equal(g["final_state"][7], st[5])                           # p_phi exact
+    if flags & 16:                      # the stencil cache changes where the values come from, not a single bit
+        gc = run_tabg(G, tb10, st, 0.01, 2000, flags=flags & 1)
+        for k in ("final_state", "status", "steps_done", "eq_cross_r", "health"):
+            assert np.array_equal(g[k], gc[k], equal_nan=True), k
     g5 = run_tabg(G, tb5, st, 0.01, 2000, flags=flags, general=False)
     c5 = parity.compare(g, g5)
     assert c5["same_class"].all() and c5["err"].max() <= 1e-11, c5["err"].max()
@@ -151,7 +155,7 @@ def test_general_table_argument_errors(G):
         with pytest.raises(G.GeoError):
             G.geo_integrate(ctx, st, 0.01, 10, out, snapshot_every=5)
         with pytest.raises(G.GeoError):
-            G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, st.device), flags=G.FLAG_TAB_GATHER)
+            G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, st.device), flags=G.FLAG_STATIC_MAP)
         with pytest.raises(G.GeoError):
             G.geo_integrate_adaptive(ctx, st, 0.01, 1e-9, 1e-9, 100, G.alloc_outputs(8, st.device))
     finally:

@@ -61,24 +61,25 @@ F_ALG_SURVEY = {"kerr": 800.0}
 # inside the loop's address range).  A kernel edit without a new capture makes bench.py FAIL instead of reporting
 # stale numbers.
 KERNEL_COUNTS = {
-    "kerr": dict(sym="geo_rk4_kernelILb1ELi0ELb0", units_per_loop=2, flop=461.0, pipe=326.0, other=70.0, tol=0.08, static_at_capture=(964, 686),
+    "kerr": dict(sym="geo_rk4_kernelILb1ELi0ELb0", units_per_loop=2, flop=461.0, pipe=326.0, other=68.0, tol=0.08, static_at_capture=(964, 686),
                  source="ncu per-instruction counts, profiles/r02_config4.md: 140 DFMA + 141 DMUL + 40 DADD + 5 DSETP per step",
                  kernel="geo_rk4_kernel"),
     "schwarzschild": dict(sym="geo_rk4_kernelILb0ELi0ELb0", units_per_loop=2, flop=342.0, pipe=245.0, other=None, tol=0.0,
                           source="static SASS count of the hot loop (no ncu capture of this instantiation)", kernel="geo_rk4_kernel"),
-    "adaptive": dict(sym="geo_rk45_kernelILb1ELb0E", units_per_loop=1, flop=1045.0, pipe=684.0, other=None, tol=0.15, static_at_capture=(1135, 778),
-                     source="ncu thread-level counts, profiles/r01_config3a_rk45.md: 361 DFMA + 271 DMUL + 52 DADD per attempt "
+    "adaptive": dict(sym="geo_rk45_kernelILb1ELb0E", units_per_loop=1, flop=1039.0, pipe=678.0, other=None, tol=0.15, static_at_capture=(1135, 778),
+                     source="ncu thread-level counts, profiles/r02_config3a_rk45.md: 361 DFMA + 264 DMUL + 52 DADD per attempt "
                             "(incl. predicated-on work of lanes waiting for a refill)", kernel="geo_rk45_kernel"),
     "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0ELb1E", units_per_loop=None, flop=4073.0, pipe=2376.0, other=None, tol=None,
-                              source="ncu per-instruction counts, profiles/r02_tabg4.md: 1735 DFMA + 550 DMUL + 52 DADD + 38 DSETP per step "
+                              source="ncu per-instruction counts, profiles/r02_tab4_tabg4.md: 1735 DFMA + 550 DMUL + 52 DADD + 38 DSETP per step "
                                      "(4 evaluations through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tabg_rk4_kernel"),
-    "tabulated": dict(sym="geo_tab_rk4_kernelILb0ELb1ELb0E", units_per_loop=None, flop=2217.0, pipe=1299.0, other=None, tol=None,
-                      source="ncu thread-level counts, profiles/r01_tab4.md: 918 DFMA + 323 DMUL + 58 DADD per step (4 evaluations "
+    "tabulated": dict(sym="geo_tab_rk4_kernelILb0ELb1ELb0E", units_per_loop=None, flop=2224.0, pipe=1300.0, other=None, tol=None,
+                      source="ncu thread-level counts, profiles/r02_tab4_tabg4.md: 924.5 DFMA + 323 DMUL + 52 DADD per step (4 evaluations "
                              "through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tab_rk4_kernel"),
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed `ncu --set full` capture of that
 # workload (profiles/), bytes; None where no capture exists.
-TRAFFIC_NCU_BYTES = {"config3a": 103_028_736, "tab4": 657_377_536, "config4": 598_806_016, "snapbench": 69_562_443_296}
+TRAFFIC_NCU_BYTES = {"config3a": 103_264_512, "tab4": 651_665_920, "tabg4": 1_225_114_112, "config4": 600_256_000, "snapbench": 69_562_443_296,
+                     "snapkerr": 70_775_029_960, "paper_t3": 16_144_486_488}     # profiles/r02_*.md (snapbench: r01_snapbench_v3.md)
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:

@@ -40,18 +40,20 @@ typedef void (*kernel_fn)(const Params);
 
 template <bool KERR, int SNAP>
 kernel_fn pick_plain(bool plain) {
-    return plain ? (kernel_fn)geo_rk4_kernel<KERR, SNAP, true> : (kernel_fn)geo_rk4_kernel<KERR, SNAP, false>;
+    return plain ? (kernel_fn)geo_rk4_kernel<KERR, SNAP, true, false> : (kernel_fn)geo_rk4_kernel<KERR, SNAP, false, false>;
 }
 template <bool KERR>
-kernel_fn pick_snap(int snap, bool plain) {
+kernel_fn pick_snap(int snap, bool plain, bool wide) {
     switch (snap) {
-        case SNAP_NONE: return pick_plain<KERR, SNAP_NONE>(plain);
+        case SNAP_NONE:
+            if (wide) return plain ? (kernel_fn)geo_rk4_kernel<KERR, SNAP_NONE, true, true> : (kernel_fn)geo_rk4_kernel<KERR, SNAP_NONE, false, true>;
+            return pick_plain<KERR, SNAP_NONE>(plain);
         case SNAP_DIRECT: return pick_plain<KERR, SNAP_DIRECT>(plain);
         default: return pick_plain<KERR, SNAP_STAGED>(plain);
     }
 }
-kernel_fn pick_kernel(int metric, int snap, bool plain) {
-    return metric == GEO_KERR ? pick_snap<true>(snap, plain) : pick_snap<false>(snap, plain);
+kernel_fn pick_kernel(int metric, int snap, bool plain, bool wide) {
+    return metric == GEO_KERR ? pick_snap<true>(snap, plain, wide) : pick_snap<false>(snap, plain, wide);
 }
 
 int fail(geo_ctx* ctx, int code, const char* msg) {
@@ -138,7 +140,9 @@ int plan_launch(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, 
     // stepping loop spill: config 2 ran 319 ms direct / 188 ms staged; now 173 / 176 ms).
     const bool staged = (flags & GEO_FLAG_STAGED_SNAP) != 0;
     lp->snap_mode = snapshot_every > 0 ? (staged ? SNAP_STAGED : SNAP_DIRECT) : SNAP_NONE;
-    lp->fn = pick_kernel(ctx->metric, lp->snap_mode, (flags & GEO_FLAG_PLAIN_UPDATE) != 0);
+    // a batch without records that fits on the machine at 2 CTAs per SM runs the high-ILP instantiation (geo_kernel.cuh: WIDE)
+    const bool wide = lp->snap_mode == SNAP_NONE && n <= (int64_t)ctx->sm_count * 2 * kBlock;
+    lp->fn = pick_kernel(ctx->metric, lp->snap_mode, (flags & GEO_FLAG_PLAIN_UPDATE) != 0, wide);
     lp->smem = lp->snap_mode == SNAP_STAGED ? (size_t)kBlock * stage_stride(ncomp) * sizeof(double) : 0;
     lp->use_queue = (flags & GEO_FLAG_STATIC_MAP) ? 0 : 1;
     cudaFuncAttributes fa;

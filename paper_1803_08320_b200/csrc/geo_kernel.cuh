@@ -171,12 +171,16 @@ struct LaneState {
     Lane6 y, c;
 };
 
+// WIDE: the instantiation for batches that leave at least half of the machine's lanes empty (n <= 2 CTAs per SM).  Such a
+// batch is latency-bound -- one or two warps per scheduler -- and what counts is the time ONE warp needs for a step: ~2550
+// cycles at 128 registers, ~1600 at the 234 registers the compiler takes when it may (more independent instructions in
+// flight per warp).  Same source, same PTX arithmetic, same bits.
 #ifdef GEO_MAXNREG
 #define GEO_RK4_BOUNDS __maxnreg__(GEO_MAXNREG)
 #else
-#define GEO_RK4_BOUNDS __launch_bounds__(kBlock, SNAP == SNAP_NONE ? GEO_MIN_CTAS_PER_SM : 4)
+#define GEO_RK4_BOUNDS __launch_bounds__(kBlock, WIDE ? 2 : (SNAP == SNAP_NONE ? GEO_MIN_CTAS_PER_SM : 4))
 #endif
-template <bool KERR, int SNAP, bool PLAIN>
+template <bool KERR, int SNAP, bool PLAIN, bool WIDE>
 __global__ void GEO_RK4_BOUNDS
 geo_rk4_kernel(const __grid_constant__ Params p) {
     extern __shared__ __align__(16) double stage_smem[];   // SNAP_STAGED: [kBlock][stage_stride(ncomp)]

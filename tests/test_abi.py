@@ -57,7 +57,7 @@ def test_every_direct_snapshot_kernel_keeps_its_256_bit_stores():
     import bench
     from paper_1803_08320_b200 import build, geo
     build.build()
-    bench.static_sass_count("geo_rk4_kernelILb1ELi1ELb0")            # fills the SASS cache
+    bench.static_sass_count("geo_rk4_kernelILb1ELi1ELb0ELb0E")            # fills the SASS cache
     sass = next(iter(bench._SASS_CACHE.values()))
     kernels, name = {}, None
     for line in sass.splitlines():

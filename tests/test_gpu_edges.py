@@ -198,3 +198,21 @@ def test_mass_and_negative_spin(G, oracle):
     assert c["same_class"].all() and c["err"].max() <= 1e-9
     sign = np.array([1, 1, 1, -1, 1, 1, 1, -1])[:, None]
     assert np.max(np.abs(gf["final_state"] * sign - g1["final_state"])) < 1e-10
+
+
+def test_small_batch_instantiation_gives_the_bits_of_the_full_machine_one(G):
+    """Batches without records that fit on the machine at 2 CTAs per SM (n <= 37 888) run the WIDE instantiation of the
+    kernel (more registers, more instructions in flight per warp: such a batch is latency-bound); same source, same
+    arithmetic: a particle's result must not depend on which instantiation integrated it."""
+    a = 0.998
+    big = W.camera_rays(256, a, 60.0)                             # 65 536 rays: the 128-register instantiation
+    ii = np.arange(0, 65536, 53)                                  # 1 237 of them alone: the wide one
+    kw = dict(r_capture=W.horizon_radius(1.0, a) + 0.01, r_escape=1100.0, kind=G.NULL)
+    gb = run_gpu(G, G.KERR, a, big, 0.02, 200000, **kw)
+    gs = run_gpu(G, G.KERR, a, np.ascontiguousarray(big[:, ii]), 0.02, 200000, **kw)
+    for k in ("final_state", "status", "steps_done", "eq_cross_r", "health"):
+        assert np.array_equal(gb[k][..., ii], gs[k], equal_nan=True), k
+    st = W.kerr_bound(70000, 0.5, W.SEED_BASE + 4)
+    tb = run_gpu(G, G.KERR, 0.5, st, 0.01, 300, flags=G.FLAG_PLAIN_UPDATE)
+    ts = run_gpu(G, G.KERR, 0.5, np.ascontiguousarray(st[:, :5000]), 0.01, 300, flags=G.FLAG_PLAIN_UPDATE)
+    assert np.array_equal(tb["final_state"][:, :5000], ts["final_state"])

@@ -391,7 +391,7 @@ template <class R> R energy_general(const GFields<R>& F, R p1, R p2, R L, R kapp
 // T5 with the T6 right-hand side: the loop of integrate_one, written out again for the general fields
 template <class R>
 void integrate_one_general(const Table& m, const double* state_in, int64_t n, int64_t i, R h, int64_t nsteps,
-                           const StopRule& st, const OutPtrs& o) {
+                           const StopRule& st, const OutPtrs& o, int64_t snapshot_every = 0) {
     const R kappa = st.kind == 0 ? R(1) : R(0);
     const bool plain = (st.flags & 1) != 0;
     const R rc = (R)st.r_capture, re = (R)st.r_escape;
@@ -407,18 +407,26 @@ void integrate_one_general(const Table& m, const double* state_in, int64_t n, in
     y.E = std::numeric_limits<R>::quiet_NaN();
     R ct = 0, c1 = 0, c2 = 0, cph = 0, cp1 = 0, cp2 = 0;
     int32_t status = -1;
-    int64_t steps = 0;
+    int64_t steps = 0, snaps = 0;
     R eq_cross = std::numeric_limits<R>::quiet_NaN();
     bool crossed = false;
     GFields<R> F;
+    auto record = [&]() {                                            // S1-S3, as on the five-field path
+        const R comp[8] = {y.t, y.x1, y.x2, y.ph, y.E, y.p1, y.p2, y.L};
+        write_record<R>(o, i, snaps, comp);
+        ++snaps;
+    };
     if (!(y.x1 >= rc)) status = TAB_ST_CAPTURED;
     else if (!finite6(y) || !std::isfinite(y.L)) status = TAB_ST_NUMERIC;
     else if (!interpolate_general(m, y.x1, y.x2, F)) status = TAB_ST_OUTSIDE;
     else {
         y.E = energy_general(F, y.p1, y.p2, y.L, kappa);
         if (!std::isfinite(y.E)) status = TAB_ST_NUMERIC;
-        else if (y.x1 > re) status = TAB_ST_ESCAPED;
-        else if (nsteps == 0) status = TAB_ST_MAXSTEPS;
+        else {
+            if (snapshot_every > 0) record();
+            if (y.x1 > re) status = TAB_ST_ESCAPED;
+            else if (nsteps == 0) status = TAB_ST_MAXSTEPS;
+        }
     }
     while (status < 0) {
         const Deriv<R> k1 = rhs_general(F, y);
@@ -457,6 +465,7 @@ void integrate_one_general(const Table& m, const double* state_in, int64_t n, in
         y = yn; ct = nt; c1 = n1; c2 = n2; cph = nph; cp1 = np1; cp2 = np2;
         F = G;
         ++steps;
+        if (snapshot_every > 0 && steps % snapshot_every == 0) record();
         if (y.x1 > re) status = TAB_ST_ESCAPED;
         else if (steps >= nsteps) status = TAB_ST_MAXSTEPS;
     }
@@ -465,6 +474,7 @@ void integrate_one_general(const Table& m, const double* state_in, int64_t n, in
     o.status[i] = status;
     o.steps_done[i] = steps;
     if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
+    if (snapshot_every > 0 && o.snap_count) o.snap_count[i] = (int32_t)snaps;
     if (o.health) {
         GFields<R> H;
         o.health[i] = (std::isfinite(y.E) && interpolate_general(m, y.x1, y.x2, H))
@@ -475,8 +485,8 @@ void integrate_one_general(const Table& m, const double* state_in, int64_t n, in
 
 template <class R>
 void integrate_range_general(const Table& m, const double* state_in, int64_t n, double h, int64_t nsteps,
-                             const StopRule& st, const OutPtrs& o, int64_t lo, int64_t hi) {
-    for (int64_t i = lo; i < hi; ++i) integrate_one_general<R>(m, state_in, n, i, (R)h, nsteps, st, o);
+                             const StopRule& st, const OutPtrs& o, int64_t lo, int64_t hi, int64_t snapshot_every) {
+    for (int64_t i = lo; i < hi; ++i) integrate_one_general<R>(m, state_in, n, i, (R)h, nsteps, st, o, snapshot_every);
 }
 
 }  // namespace
@@ -531,8 +541,9 @@ int oracle_tab_rhs(const double* tab, int64_t n1, int64_t n2, double x1_0, doubl
 // ---- T6: general ten-field tables, tab = [10][n2][n1] ----
 int oracle_tabg_integrate(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
                           const double* state_in, int64_t n, double h, int64_t nsteps, const StopRule* st,
-                          const OutPtrs* out, int precision, int nthreads) {
-    if (!tab || n1 < 4 || n2 < 4 || !(d1 > 0) || !(d2 > 0) || n < 0 || nsteps < 0 || !st || !out) return 1;
+                          const OutPtrs* out, int precision, int nthreads, int64_t snapshot_every) {
+    if (!tab || n1 < 4 || n2 < 4 || !(d1 > 0) || !(d2 > 0) || n < 0 || nsteps < 0 || !st || !out || snapshot_every < 0) return 1;
+    if (snapshot_every > 0 && (!out->snapshots || !out->snap_count || out->snap_capacity < 1 || (out->snap_mask & 0xFFu) == 0)) return 1;
     const Table m{tab, n1, n2, x1_0, d1, x2_0, d2};
     if (nthreads < 1) nthreads = 1;
     std::vector<std::thread> pool;
@@ -541,9 +552,9 @@ int oracle_tabg_integrate(const double* tab, int64_t n1, int64_t n2, double x1_0
         const int64_t lo = t * per, hi = std::min<int64_t>(n, lo + per);
         if (lo >= hi) break;
         if (precision == 1)
-            pool.emplace_back(integrate_range_general<long double>, m, state_in, n, h, nsteps, *st, *out, lo, hi);
+            pool.emplace_back(integrate_range_general<long double>, m, state_in, n, h, nsteps, *st, *out, lo, hi, snapshot_every);
         else
-            pool.emplace_back(integrate_range_general<double>, m, state_in, n, h, nsteps, *st, *out, lo, hi);
+            pool.emplace_back(integrate_range_general<double>, m, state_in, n, h, nsteps, *st, *out, lo, hi, snapshot_every);
     }
     for (auto& th : pool) th.join();
     return 0;

@@ -108,21 +108,29 @@ def rhs_general(table: dict, y8, kappa: float = 1.0):
 
 def integrate_general(table: dict, state_in: np.ndarray, h: float, nsteps: int, r_capture: float = -np.inf,
                       r_escape: float = np.inf, kind: int = TIMELIKE, flags: int = 0, long_double: bool = False,
-                      nthreads: int = 1) -> dict:
-    """Fixed-step RK4 through a general ten-field tabulated metric (reading T6)."""
+                      nthreads: int = 1, snapshot_every: int = 0, snap_capacity: int | None = None, snap_mask: int = 0xFF) -> dict:
+    """Fixed-step RK4 through a general ten-field tabulated metric (reading T6); trajectory records as in integrate()."""
     st = np.ascontiguousarray(state_in, dtype=np.float64)
     n = st.shape[1]
     res = {"final_state": np.full((8, n), np.nan), "status": np.full(n, -1, dtype=np.int32),
-           "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan), "health": np.full(n, np.nan)}
+           "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan), "health": np.full(n, np.nan),
+           "snapshots": None, "snap_count": None}
+    if snapshot_every > 0:
+        if snap_capacity is None:
+            snap_capacity = 1 + nsteps // snapshot_every
+        res["snapshots"] = np.full((n, snap_capacity, bin(snap_mask & 0xFF).count("1")), np.nan)
+        res["snap_count"] = np.zeros(n, dtype=np.int32)
     stop = _Stop(r_capture, r_escape, kind, flags)
     out = _Out(res["final_state"].ctypes.data, res["status"].ctypes.data, res["steps_done"].ctypes.data,
-               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data, None, 0, 0, None)
+               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data,
+               res["snapshots"].ctypes.data if snapshot_every > 0 else None, snap_capacity or 0, snap_mask,
+               res["snap_count"].ctypes.data if snapshot_every > 0 else None)
     L = lib()
     L.oracle_tabg_integrate.restype = C.c_int
     L.oracle_tabg_integrate.argtypes = _GRID + [C.c_void_p, C.c_int64, C.c_double, C.c_int64, C.POINTER(_Stop),
-                                                C.POINTER(_Out), C.c_int, C.c_int]
+                                                C.POINTER(_Out), C.c_int, C.c_int, C.c_int64]
     rc = L.oracle_tabg_integrate(*_grid(table, 10), st.ctypes.data, n, h, nsteps, C.byref(stop), C.byref(out),
-                                 int(long_double), nthreads)
+                                 int(long_double), nthreads, snapshot_every)
     if rc != 0:
         raise ValueError("oracle_tabg_integrate: invalid arguments")
     return res

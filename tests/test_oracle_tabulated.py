@@ -409,3 +409,22 @@ def test_tabulated_trajectory_records_follow_S1_to_S3(tab_oracle):
     assert np.array_equal(e["snap_count"], 1 + e["steps_done"] // 5)
     for i in range(0, 60, 7):
         assert np.isnan(e["snapshots"][i, e["snap_count"][i]:]).all() and np.isfinite(e["snapshots"][i, : e["snap_count"][i]]).all()
+
+
+def test_general_tabulated_trajectory_records(tab_oracle):
+    """Records on the general path: the same S1-S3 semantics, pinned the same way (slot j == the shorter run, bitwise), and
+    on an embedded eq.(8) table they are the five-field oracle's records (1e-12)."""
+    a = 0.9
+    tb5 = W.kerr_metric_table(1.0, a, 257, 65, 1.8, 40.0, 0.2, math.pi - 0.2)
+    tb = W.general_table_from_diagonal(tb5)
+    st = W.kerr_bound(40, a, W.SEED_BASE + 2)
+    r = tab_oracle.integrate_general(tb, st, 0.01, 600, snapshot_every=200, snap_mask=0xFF)
+    assert (r["snap_count"] == 4).all()
+    assert np.array_equal(r["snapshots"][:, 0, [1, 2, 3, 5, 6, 7]], st.T)
+    for j in (1, 3):
+        rj = tab_oracle.integrate_general(tb, st, 0.01, 200 * j)
+        assert np.array_equal(r["snapshots"][:, j, :], rj["final_state"].T)
+    r5 = tab_oracle.integrate(tb5, st, 0.01, 600, snapshot_every=200)
+    assert np.max(np.abs(r["snapshots"] - r5["snapshots"]) / np.maximum(np.abs(r5["snapshots"]), 1.0)) < 1e-12
+    m = tab_oracle.integrate_general(tb, st, 0.01, 600, snapshot_every=100, snap_capacity=3, snap_mask=0x46)
+    assert (m["snap_count"] == 7).all() and m["snapshots"].shape == (40, 3, 3)

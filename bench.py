@@ -69,7 +69,7 @@ KERNEL_COUNTS = {
     "adaptive": dict(sym="geo_rk45_kernelILb1ELb0E", units_per_loop=1, flop=1039.0, pipe=678.0, other=None, tol=0.15, static_at_capture=(1135, 778),
                      source="ncu thread-level counts, profiles/r02_config3a_rk45.md: 361 DFMA + 264 DMUL + 52 DADD per attempt "
                             "(incl. predicated-on work of lanes waiting for a refill)", kernel="geo_rk45_kernel"),
-    "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0ELb1E", units_per_loop=None, flop=4073.0, pipe=2376.0, other=None, tol=None,
+    "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0ELb1ELb0E", units_per_loop=None, flop=4073.0, pipe=2376.0, other=None, tol=None,
                               source="ncu per-instruction counts, profiles/r02_tab4_tabg4.md: 1735 DFMA + 550 DMUL + 52 DADD + 38 DSETP per step "
                                      "(4 evaluations through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tabg_rk4_kernel"),
     "tabulated": dict(sym="geo_tab_rk4_kernelILb0ELb1ELb0E", units_per_loop=None, flop=2224.0, pipe=1300.0, other=None, tol=None,

@@ -173,8 +173,9 @@ int geo_create_tabulated(geo_ctx **ctx, const geo_table *table);
  * Same interpolant with its exact gradient; equations of motion = Hamilton's equations (3),(4) of
  *     H = 1/2 [ -(p_t - beta^k p_k)^2/alpha^2 + gamma^{ij} p_i p_j ],   gamma^{ij} = inverse of gamma_ij (3 x 3, per evaluation),
  * p_t and p_phi constants of motion.  Use with geo_integrate / geo_integrate_host exactly like a geo_create_tabulated
- * ctx (state_in = (x^1, x^2, phi, p_1, p_2, p_phi); GEO_ST_OUTSIDE; snapshot_every must be 0; flags:
- * GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER; geo_integrate_adaptive returns GEO_EINVAL). */
+ * ctx (state_in = (x^1, x^2, phi, p_1, p_2, p_phi); GEO_ST_OUTSIDE; trajectory records by snap_mask over
+ * (t, x^1, x^2, phi, E, p_1, p_2, p_phi); flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER; geo_integrate_adaptive
+ * returns GEO_EINVAL). */
 int geo_create_tabulated_general(geo_ctx **ctx, const geo_table *table);
 
 void geo_destroy(geo_ctx *ctx);

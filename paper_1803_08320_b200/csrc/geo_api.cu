@@ -104,7 +104,6 @@ int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t 
     if (std::isnan(stop->r_capture) || std::isnan(stop->r_escape)) return fail(ctx, GEO_EINVAL, "stop radii must not be NaN");
     if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP | GEO_FLAG_STAGED_SNAP | GEO_FLAG_CARTESIAN_SNAP | GEO_FLAG_TAB_GATHER)) return fail(ctx, GEO_EINVAL, "unknown stop.flags bit");
     if (ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) {
-        if (snapshot_every > 0 && ctx->metric == GEO_TABULATED_GENERAL) return fail(ctx, GEO_EINVAL, "general tabulated metrics: snapshots are not supported");
         const int32_t ok = GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_TAB_GATHER;
         if (stop->flags & ~ok) return fail(ctx, GEO_EINVAL, "tabulated metrics: only GEO_FLAG_PLAIN_UPDATE and GEO_FLAG_TAB_GATHER are supported");
     }
@@ -234,16 +233,19 @@ int launch_tab(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t ns
 }
 
 typedef void (*tabg_kernel_fn)(const TabgParams);
-tabg_kernel_fn pick_tabg_kernel(int32_t flags) {
+tabg_kernel_fn pick_tabg_kernel(int32_t flags, bool snap = false) {
     const bool plain = (flags & GEO_FLAG_PLAIN_UPDATE) != 0;
-    if (flags & GEO_FLAG_TAB_GATHER) return plain ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true, false> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false, false>;
-    return plain ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true, true> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false, true>;
+    if (flags & GEO_FLAG_TAB_GATHER)
+        return snap ? (plain ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true, false, true> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false, false, true>)
+                    : (plain ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true, false, false> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false, false, false>);
+    return snap ? (plain ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true, true, true> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false, true, true>)
+                : (plain ? (tabg_kernel_fn)geo_tabg_rk4_kernel<true, true, false> : (tabg_kernel_fn)geo_tabg_rk4_kernel<false, true, false>);
 }
 int tabg_block(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? kTabBlock : kTabgCacheBlock; }
 size_t tabg_smem(int32_t flags) { return (flags & GEO_FLAG_TAB_GATHER) ? 0 : (size_t)kTabgCacheRows * kTabgCacheBlock * sizeof(double); }
 
-int plan_tabg(geo_ctx* ctx, int64_t n, int32_t flags, int* grid, int* per_sm_out, int* regs) {
-    tabg_kernel_fn fn = pick_tabg_kernel(flags);
+int plan_tabg(geo_ctx* ctx, int64_t n, int32_t flags, int* grid, int* per_sm_out, int* regs, bool snap = false) {
+    tabg_kernel_fn fn = pick_tabg_kernel(flags, snap);
     int per_sm = 0;
     const int block = tabg_block(flags);
     cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tabg_smem(flags));
@@ -262,9 +264,10 @@ int plan_tabg(geo_ctx* ctx, int64_t n, int32_t flags, int* grid, int* per_sm_out
 }
 
 int launch_tabg(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
-                const geo_out* out, cudaStream_t stream, unsigned long long* counter) {
+                int64_t snapshot_every, const geo_out* out, cudaStream_t stream, unsigned long long* counter) {
     int grid = 0, per_sm = 0, regs = 0;
-    int rc = plan_tabg(ctx, n, stop->flags, &grid, &per_sm, &regs);
+    const bool snap = snapshot_every > 0;
+    int rc = plan_tabg(ctx, n, stop->flags, &grid, &per_sm, &regs, snap);
     if (rc != GEO_OK) return rc;
     TabgParams p;
     memset(&p, 0, sizeof p);
@@ -283,10 +286,16 @@ int launch_tabg(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t n
     p.eq_cross_r = out->eq_cross_r;
     p.health = out->health;
     p.counter = counter;
+    p.snap_every = (int)(snapshot_every > 0x7fffffffLL ? 0x7fffffffLL : snapshot_every);
+    p.snap_cap = snap ? out->snap_capacity : 0;
+    p.snap_mask = snap ? (out->snap_mask & 0xFFu) : 0;
+    p.ncomp = snap ? popcount8(out->snap_mask) : 0;
+    p.snaps = snap ? out->snapshots : nullptr;
+    p.snap_count = snap ? out->snap_count : nullptr;
     p.m = ctx->tgm;
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
-    pick_tabg_kernel(stop->flags)<<<grid, tabg_block(stop->flags), tabg_smem(stop->flags), stream>>>(p);
+    pick_tabg_kernel(stop->flags, snap)<<<grid, tabg_block(stop->flags), tabg_smem(stop->flags), stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
     return GEO_OK;
@@ -295,7 +304,7 @@ int launch_tabg(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t n
 int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
            int64_t snapshot_every, const geo_out* out, cudaStream_t stream, unsigned long long* counter) {
     if (ctx->metric == GEO_TABULATED) return launch_tab(ctx, d_in, n, h, nsteps, stop, snapshot_every, out, stream, counter);
-    if (ctx->metric == GEO_TABULATED_GENERAL) return launch_tabg(ctx, d_in, n, h, nsteps, stop, out, stream, counter);
+    if (ctx->metric == GEO_TABULATED_GENERAL) return launch_tabg(ctx, d_in, n, h, nsteps, stop, snapshot_every, out, stream, counter);
     const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
     LaunchPlan lp;
     int rc = plan_launch(ctx, n, stop->flags, snapshot_every, ncomp, &lp);
@@ -721,7 +730,7 @@ int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_eve
     }
     if (ctx->metric == GEO_TABULATED_GENERAL) {
         info[1] = tabg_block(flags);
-        return plan_tabg(ctx, n, flags, &info[0], &info[3], &info[2]);
+        return plan_tabg(ctx, n, flags, &info[0], &info[3], &info[2], snapshot_every > 0);
     }
     LaunchPlan lp;
     int rc = plan_launch(ctx, n, flags, snapshot_every, 8, &lp);

@@ -42,6 +42,13 @@ struct TabgParams {
     double* eq_cross_r;
     double* health;
     unsigned long long* counter;
+    // trajectory records (readings S1-S3): components (t, x1, x2, phi, E, p1, p2, L) by mask, particle-major
+    int snap_every;
+    long long snap_cap;
+    unsigned snap_mask;
+    int ncomp;
+    double* snaps;
+    int* snap_count;
     TabgMetric m;
 };
 
@@ -176,7 +183,7 @@ __device__ __noinline__ bool tabg_fields_cold(const TabgMetric& m, double x1, do
     return tabg_fields(m, x1, x2, F);
 }
 
-template <bool PLAIN, bool CACHE>
+template <bool PLAIN, bool CACHE, bool SNAP>
 __global__ void __launch_bounds__(CACHE ? kTabgCacheBlock : kTabBlock, CACHE ? 5 : 2) geo_tabg_rk4_kernel(const __grid_constant__ TabgParams p) {
     extern __shared__ __align__(16) double tabg_smem[];              // CACHE: [160][blockDim.x]
     double* const col = tabg_smem + threadIdx.x;
@@ -193,10 +200,18 @@ __global__ void __launch_bounds__(CACHE ? kTabgCacheBlock : kTabBlock, CACHE ? 5
     int steps = 0;
     double eqc = 0;
     bool crossed = false;
+    int snaps = 0, snap_ctr = 0;
 
+    auto emit_record = [&]() {                                     // S1-S3: straight from registers, 256-bit stores
+        if (snaps < p.snap_cap)
+            store_record_global(p.snaps + ((size_t)idx * (size_t)p.snap_cap + (size_t)snaps) * p.ncomp, p.snap_mask,
+                                t, x1, x2, ph, E, p1, p2, L);
+        ++snaps;
+    };
     auto finish = [&](int st) {
         long long n = p.n;
         asm volatile("" : "+l"(n));
+        if (SNAP) p.snap_count[idx] = snaps;
         p.fin[0 * n + idx] = t;
         p.fin[1 * n + idx] = x1;
         p.fin[2 * n + idx] = x2;
@@ -235,6 +250,8 @@ __global__ void __launch_bounds__(CACHE ? kTabgCacheBlock : kTabBlock, CACHE ? 5
         steps = 0;
         crossed = false;
         active = true;
+        snaps = 0;
+        snap_ctr = p.snap_every;
         if (!(x1 >= p.r_capture)) { finish(ST_CAPTURED); return; }               // B1
         if (!all_finite6(x1, x2, ph, p1, p2, L)) { finish(ST_NUMERIC); return; }
         TabgFields F;
@@ -242,6 +259,7 @@ __global__ void __launch_bounds__(CACHE ? kTabgCacheBlock : kTabBlock, CACHE ? 5
         const TabgAux A = tabg_aux(F.v, p1, p2, L, 0.0);                         // mass shell (5): A.W = beta^k p_k here
         E = fma(F.v[0], sqrt(p.kappa + A.gpp), -A.W);
         if ((__double2hiint(E) & 0x7ff00000) == 0x7ff00000) { finish(ST_NUMERIC); return; }
+        if (SNAP) emit_record();                                                 // S1: slot 0 = y0
         if (x1 > p.r_escape) { finish(ST_ESCAPED); return; }
         if (p.nsteps == 0) { finish(ST_MAXSTEPS); return; }
         tabg_rhs(F, p1, p2, E, L, k1);
@@ -319,6 +337,9 @@ __global__ void __launch_bounds__(CACHE ? kTabgCacheBlock : kTabBlock, CACHE ? 5
                 ct = dt; c1 = d1; c2 = d2; cph = dph; cp1 = dp1; cp2 = dp2;
                 k1 = d;
                 ++steps;
+                if (SNAP) {
+                    if (--snap_ctr == 0) { snap_ctr = p.snap_every; emit_record(); }   // S1
+                }
                 if (x1 > p.r_escape) finish(ST_ESCAPED);                         // B3
                 else if (steps >= p.nsteps) finish(ST_MAXSTEPS);                 // B4
             }

@@ -151,12 +151,42 @@ def test_general_table_argument_errors(G):
     try:
         assert math.isnan(G.geo_horizon_radius(ctx))
         st = torch.from_numpy(W.kerr_bound(8, 0.5, W.SEED_BASE + 4)).cuda()
-        out = G.alloc_outputs(8, st.device, 10, 5)
-        with pytest.raises(G.GeoError):
-            G.geo_integrate(ctx, st, 0.01, 10, out, snapshot_every=5)
+        with pytest.raises(G.GeoError):         # records exist on this path, but not the staged / Cartesian writers
+            G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, st.device, 10, 5), snapshot_every=5, flags=G.FLAG_CARTESIAN_SNAP)
         with pytest.raises(G.GeoError):
             G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, st.device), flags=G.FLAG_STATIC_MAP)
         with pytest.raises(G.GeoError):
             G.geo_integrate_adaptive(ctx, st, 0.01, 1e-9, 1e-9, 100, G.alloc_outputs(8, st.device))
+    finally:
+        G.geo_destroy(ctx)
+
+
+@pytest.mark.parametrize("flags,mask,cap", [(0, 0xFF, None), (16, 0x0F, None), (1, 0x46, 3)])
+def test_general_tabulated_trajectory_records(G, tab_oracle, flags, mask, cap):
+    """Records on the general path (readings S1-S3) in Kerr-Schild coordinates: against the oracle, cache and gather
+    kernels, plain update, odd mask, capacity overflow; slot j bitwise equal to the GPU run that stops there."""
+    import torch
+    a, M = 0.9, 1.0
+    st, consts = W.kerr_bound(1201, a, W.SEED_BASE + 2, return_constants=True)
+    ks = W.to_kerr_schild(st, consts[0], M, a)
+    tb = W.kerr_schild_metric_table(M, a, 513, 129, 1.2, 40.0, 0.15, math.pi - 0.15)
+    o = tab_oracle.integrate_general(tb, ks, 0.01, 1200, flags=flags & 1, snapshot_every=200, snap_capacity=cap, snap_mask=mask, nthreads=NCPU)
+    ctx = G.geo_create_tabulated_general(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+    try:
+        dev = torch.device("cuda:0")
+        out = G.alloc_outputs(ks.shape[1], dev, 1200, 200, cap, mask)
+        G.geo_integrate(ctx, torch.from_numpy(ks).to(dev), 0.01, 1200, out, flags=flags, snapshot_every=200)
+        torch.cuda.synchronize()
+        g = G.to_numpy(out)
+        c = parity.compare(g, o)
+        assert c["same_class"].all() and c["err"].max() <= 1e-9
+        assert np.array_equal(g["snap_count"], o["snap_count"])
+        assert parity.snapshot_err(g, o).max() <= 1e-9
+        if mask == 0xFF:
+            oj = G.alloc_outputs(ks.shape[1], dev)
+            G.geo_integrate(ctx, torch.from_numpy(ks).to(dev), 0.01, 600, oj, flags=flags)
+            torch.cuda.synchronize()
+            done = g["snap_count"] > 3
+            assert np.array_equal(g["snapshots"][done, 3, :], G.to_numpy(oj)["final_state"].T[done])
     finally:
         G.geo_destroy(ctx)

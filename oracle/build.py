@@ -29,7 +29,8 @@ def build(force: bool = False, sanitize: bool | None = None) -> str:
     if sanitize is None:
         sanitize = os.environ.get("GEO_ORACLE_SANITIZE") == "1"
     lib = LIB_SAN if sanitize else LIB
-    if not force and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(x) for x in SRCS):
+    deps = SRCS + [os.path.join(HERE, "dp45.h")]
+    if not force and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(x) for x in deps):
         return lib
     opt = (["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"]
            if sanitize else ["-O2"])

@@ -60,6 +60,8 @@
 #include <thread>
 #include <vector>
 
+#include "dp45.h"
+
 namespace {
 
 enum { TAB_ST_MAXSTEPS = 0, TAB_ST_CAPTURED = 1, TAB_ST_ESCAPED = 2, TAB_ST_NUMERIC = 3, TAB_ST_OUTSIDE = 4 };
@@ -302,6 +304,174 @@ void integrate_range(const Table& m, const double* state_in, int64_t n, double h
     for (int64_t i = lo; i < hi; ++i) integrate_one<R>(m, state_in, n, i, (R)h, nsteps, st, o, snapshot_every);
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// T7 (round 2): the adaptive Dormand-Prince 5(4) stepper of readings A1-A3 on the five-field tabulated metric.
+// The loop of geo_oracle.cpp: integrate_one_adaptive with r -> x^1, theta -> x^2 and the T3 right-hand side; in addition
+// every evaluation point (y0, the six stage points, the end point) is tested against the table's domain (T4): per point
+// the capture test comes first, then the domain test; the first event in evaluation order ends the particle
+// (CAPTURED / OUTSIDE), that attempt is not taken.
+// ---------------------------------------------------------------------------------------------------------------
+template <class R> R tcomp6(const State<R>& y, int c) {
+    switch (c) { case 0: return y.t; case 1: return y.x1; case 2: return y.x2; case 3: return y.ph; case 4: return y.p1; default: return y.p2; }
+}
+template <class R> R tdcomp6(const Deriv<R>& k, int c) {
+    switch (c) { case 0: return k.t; case 1: return k.x1; case 2: return k.x2; case 3: return k.ph; case 4: return k.p1; default: return k.p2; }
+}
+template <class R> void tset6(State<R>& y, int c, R v) {
+    switch (c) { case 0: y.t = v; break; case 1: y.x1 = v; break; case 2: y.x2 = v; break; case 3: y.ph = v; break;
+                 case 4: y.p1 = v; break; default: y.p2 = v; }
+}
+
+template <class R>
+void integrate_one_adaptive_tab(const Table& m, const double* state_in, int64_t n, int64_t i, const AdaptiveCtl& ctl,
+                                int64_t max_attempts, const StopRule& st, const OutPtrs& o, int64_t* rejected_out) {
+    static const DP45 T;
+    const R kappa = st.kind == 0 ? R(1) : R(0);
+    const R rc = (R)st.r_capture, re = (R)st.r_escape;
+    const R half_pi = (R)1.5707963267948966;
+    State<R> y;
+    y.t = R(0);
+    y.x1 = (R)state_in[0 * n + i];
+    y.x2 = (R)state_in[1 * n + i];
+    y.ph = (R)state_in[2 * n + i];
+    y.p1 = (R)state_in[3 * n + i];
+    y.p2 = (R)state_in[4 * n + i];
+    y.L = (R)state_in[5 * n + i];
+    y.E = std::numeric_limits<R>::quiet_NaN();
+    R cc[6] = {0, 0, 0, 0, 0, 0};
+    R h = (R)ctl.h0, tau = R(0);
+    const R tau_end = (R)ctl.tau_end;
+    const bool dense = ctl.snap_dtau > 0.0 && o.snapshots != nullptr;
+    const R dtau = (R)ctl.snap_dtau;
+    int64_t next_j = 0;
+    int32_t status = -1;
+    int64_t steps = 0, attempts = 0, rejected = 0;
+    R eq_cross = std::numeric_limits<R>::quiet_NaN();
+    bool crossed = false;
+    Fields<R> F;
+    auto record = [&](const State<R>& ys) {
+        const R comp[8] = {ys.t, ys.x1, ys.x2, ys.ph, ys.E, ys.p1, ys.p2, ys.L};
+        write_record<R>(o, i, next_j, comp);
+        ++next_j;
+    };
+    if (!(y.x1 >= rc)) status = TAB_ST_CAPTURED;                     // B1 + T4 on y0
+    else if (!finite6(y) || !std::isfinite(y.L)) status = TAB_ST_NUMERIC;
+    else if (!interpolate(m, y.x1, y.x2, F)) status = TAB_ST_OUTSIDE;
+    else {
+        y.E = energy_fields(F, y.p1, y.p2, y.L, kappa);
+        if (!std::isfinite(y.E)) status = TAB_ST_NUMERIC;
+        else {
+            if (dense) record(y);
+            if (y.x1 > re) status = TAB_ST_ESCAPED;
+            else if (max_attempts == 0) status = TAB_ST_MAXSTEPS;
+        }
+    }
+    Deriv<R> k[DP45::S];
+    if (status < 0) k[0] = rhs_fields(F, y);
+    while (status < 0) {
+        const bool last = tau + R(1.01) * h >= tau_end;
+        if (last) h = tau_end - tau;
+        int ev = 0;
+        for (int s = 1; s < DP45::S - 1 && !ev; ++s) {               // stages 2..6
+            State<R> ys = y;
+            for (int c = 0; c < 6; ++c) {
+                R acc = R(0);
+                for (int j = 0; j < s; ++j) acc += (R)T.a[s][j] * tdcomp6(k[j], c);
+                tset6(ys, c, tcomp6(y, c) + h * acc);
+            }
+            Fields<R> G;
+            if (!(ys.x1 >= rc)) ev = TAB_ST_CAPTURED;
+            else if (!interpolate(m, ys.x1, ys.x2, G)) ev = TAB_ST_OUTSIDE;
+            else k[s] = rhs_fields(G, ys);
+        }
+        ++attempts;
+        if (ev) { status = ev; break; }
+        State<R> yn = y;
+        R cn[6];
+        for (int c = 0; c < 6; ++c) {
+            R acc5 = R(0);
+            for (int j = 0; j < DP45::S - 1; ++j) acc5 += (R)T.a[6][j] * tdcomp6(k[j], c);
+            R v = tcomp6(y, c);
+            cn[c] = cc[c];
+            kahan_add(v, cn[c], h * acc5, false);
+            tset6(yn, c, v);
+        }
+        if (!(yn.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }     // end point: capture, then finiteness, then domain
+        const bool fin = finite6(yn);
+        Fields<R> Gn;
+        if (fin && !interpolate(m, yn.x1, yn.x2, Gn)) { status = TAB_ST_OUTSIDE; break; }
+        R err = R(0);
+        if (fin) {
+            k[6] = rhs_fields(Gn, yn);
+            for (int c = 0; c < 6; ++c) {
+                R acce = R(0);
+                for (int j = 0; j < DP45::S; ++j)
+                    acce += ((R)(j < 6 ? T.a[6][j] : 0.0L) - (R)T.b4[j]) * tdcomp6(k[j], c);
+                const R sc = (R)ctl.atol + (R)ctl.rtol * std::max(std::fabs(tcomp6(y, c)), std::fabs(tcomp6(yn, c)));
+                const R ec = std::fabs(h * acce) / sc;
+                if (!(ec <= err)) err = ec;
+            }
+        }
+        if (fin && std::isinf(ctl.rtol)) err = R(0);
+        R fac = err > R(0) ? R(0.9) * std::pow(err, R(-0.2)) : (err == R(0) ? R(5) : R(0.2));
+        if (!(fac >= R(0.2))) fac = R(0.2);
+        if (fac > R(5)) fac = R(5);
+        if (std::isinf(ctl.rtol)) fac = R(1);
+        if (!fin || !(err <= R(1))) {
+            ++rejected;
+            h *= std::min(fac, R(1));
+            if ((std::isinf(ctl.rtol) && !fin) || !(std::fabs(h) >= (R)ctl.h_min) || !(std::fabs(h) > R(0))) { status = TAB_ST_NUMERIC; break; }
+            if (attempts >= max_attempts) { status = TAB_ST_MAXSTEPS; break; }
+            continue;
+        }
+        if (!crossed) {
+            const R d0 = y.x2 - half_pi, d1 = yn.x2 - half_pi;
+            if (d0 * d1 < R(0)) {
+                crossed = true;
+                eq_cross = y.x1 + (yn.x1 - y.x1) * (half_pi - y.x2) / (yn.x2 - y.x2);
+            }
+        }
+        const R tau_new = last ? tau_end : tau + h;
+        if (dense) {
+            for (;;) {
+                const R tj = (R)next_j * dtau;
+                if (!(tj <= tau_new)) break;
+                R w[7];
+                dp45_dense_weights<R>((tj - tau) / h, w);
+                State<R> ys = y;
+                for (int c = 0; c < 6; ++c) {
+                    R acc = R(0);
+                    for (int j = 0; j < DP45::S; ++j) acc += w[j] * tdcomp6(k[j], c);
+                    tset6(ys, c, tcomp6(y, c) + h * acc);
+                }
+                record(ys);
+            }
+        }
+        y = yn;
+        for (int c = 0; c < 6; ++c) cc[c] = cn[c];
+        k[0] = k[6];
+        F = Gn;
+        ++steps;
+        tau = tau_new;
+        h *= fac;
+        if (y.x1 > re) status = TAB_ST_ESCAPED;
+        else if (last || attempts >= max_attempts) status = TAB_ST_MAXSTEPS;
+    }
+    const R comp[8] = {y.t, y.x1, y.x2, y.ph, y.E, y.p1, y.p2, y.L};
+    for (int q = 0; q < 8; ++q) o.final_state[(int64_t)q * n + i] = (double)comp[q];
+    o.status[i] = status;
+    o.steps_done[i] = steps;
+    if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
+    if (o.health) {
+        Fields<R> H;
+        o.health[i] = (std::isfinite(y.E) && interpolate(m, y.x1, y.x2, H))
+                          ? (double)std::fabs(R(2) * hamiltonian_fields(H, y) + kappa)
+                          : std::numeric_limits<double>::quiet_NaN();
+    }
+    if (dense && o.snap_count) o.snap_count[i] = (int32_t)next_j;
+    if (rejected_out) rejected_out[i] = rejected;
+}
 
 // ---------------------------------------------------------------------------------------------------------------
 // T6: general stationary axisymmetric 3+1 metric, ten fields
@@ -573,6 +743,30 @@ int oracle_tabg_rhs(const double* tab, int64_t n1, int64_t n2, double x1_0, doub
     if (H) *H = hamiltonian_general(F, y);
     if (E_out) *E_out = energy_general(F, y.p1, y.p2, y.L, kappa);
     return 1;
+}
+
+// ---- T7: adaptive RK5(4) on a five-field table ----
+int oracle_tab_integrate_adaptive(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+                                  const double* state_in, int64_t n, const AdaptiveCtl* ctl, int64_t max_attempts,
+                                  const StopRule* st, const OutPtrs* out, int64_t* rejected, int precision, int nthreads) {
+    if (!tab || n1 < 4 || n2 < 4 || !(d1 > 0) || !(d2 > 0) || n < 0 || max_attempts < 0 || !st || !out || !ctl) return 1;
+    if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0) || !(ctl->rtol >= 0) || !(ctl->atol >= 0) || !(ctl->rtol + ctl->atol > 0) ||
+        !(ctl->h_min >= 0) || !(ctl->tau_end > 0) || !(ctl->snap_dtau >= 0)) return 1;
+    if (ctl->snap_dtau > 0 && (!out->snapshots || !out->snap_count || out->snap_capacity < 1 || (out->snap_mask & 0xFFu) == 0)) return 1;
+    const Table m{tab, n1, n2, x1_0, d1, x2_0, d2};
+    if (nthreads < 1) nthreads = 1;
+    std::vector<std::thread> pool;
+    const int64_t block = 64, nblocks = (n + block - 1) / block;
+    for (int t = 0; t < nthreads; ++t)
+        pool.emplace_back([&, t]() {
+            for (int64_t b = t; b < nblocks; b += nthreads)
+                for (int64_t i = b * block; i < std::min<int64_t>(n, (b + 1) * block); ++i) {
+                    if (precision == 1) integrate_one_adaptive_tab<long double>(m, state_in, n, i, *ctl, max_attempts, *st, *out, rejected);
+                    else integrate_one_adaptive_tab<double>(m, state_in, n, i, *ctl, max_attempts, *st, *out, rejected);
+                }
+        });
+    for (auto& th : pool) th.join();
+    return 0;
 }
 
 }  // extern "C"

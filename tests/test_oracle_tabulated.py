@@ -428,3 +428,59 @@ def test_general_tabulated_trajectory_records(tab_oracle):
     assert np.max(np.abs(r["snapshots"] - r5["snapshots"]) / np.maximum(np.abs(r5["snapshots"]), 1.0)) < 1e-12
     m = tab_oracle.integrate_general(tb, st, 0.01, 600, snapshot_every=100, snap_capacity=3, snap_mask=0x46)
     assert (m["snap_count"] == 7).all() and m["snapshots"].shape == (40, 3, 3)
+
+
+# ---- reading T7: the adaptive RK5(4) stepper on the tabulated metric -----------------------------------------------------
+def test_tabulated_adaptive_is_fifth_order_and_agrees_with_the_pinned_rk4_path(tab_oracle):
+    """On the made-up metric with quadratic fields the interpolant is the metric itself (smooth), so with the controller
+    off the propagated solution must converge with order 5 (Q -> 32; the pinned RK4 path gives 16); with the controller
+    on it must land on the final time with the state the pinned fixed-step RK4 path reaches with a small step."""
+    tb, _ = _quadratic_metric()
+    rng = np.random.default_rng(9)
+    n = 12
+    st = np.stack([rng.uniform(1.6, 2.6, n), rng.uniform(1.2, 2.0, n), np.zeros(n), rng.uniform(-0.3, 0.3, n),
+                   rng.uniform(-0.3, 0.3, n), rng.uniform(0.3, 1.0, n)])
+    sols = []
+    for k in (1, 2, 4):
+        r = tab_oracle.integrate_adaptive(tb, st, 0.2 / k, np.inf, 1.0, 10**6, tau_end=2.0, long_double=True)
+        assert (r["status"] == tab_oracle.ST_MAXSTEPS).all() and (r["steps_done"] == 10 * k).all() and (r["rejected"] == 0).all()
+        sols.append(r["final_state"])
+    Q = np.linalg.norm(sols[0] - sols[1], axis=0) / np.linalg.norm(sols[1] - sols[2], axis=0)
+    assert Q.min() > 18.0 and abs(np.median(Q) - 32.0) < 6.0, Q
+    ref = tab_oracle.integrate(tb, st, 0.0005, 4000, long_double=True)
+    ad = tab_oracle.integrate_adaptive(tb, st, 0.1, 1e-11, 1e-11, 10**6, tau_end=2.0)
+    assert np.max(np.abs(ad["final_state"] - ref["final_state"])) < 1e-9
+    assert np.allclose(ad["final_state"][[4, 7]], ref["final_state"][[4, 7]], rtol=0, atol=1e-15)      # E, L constants
+
+
+def test_tabulated_adaptive_kerr_converges_to_the_analytic_adaptive_oracle_and_stops_like_it(tab_oracle, oracle):
+    a = 0.9
+    st = W.kerr_bound(40, a, W.SEED_BASE + 2)
+    ref = oracle.integrate_adaptive(oracle.KERR, 1.0, a, st, 0.05, 1e-10, 1e-10, 10**6, tau_end=30.0)
+    errs = []
+    for n1, n2 in ((513, 129), (1025, 257)):
+        tb = W.kerr_metric_table(1.0, a, n1, n2, 1.8, 40.0, 0.2, math.pi - 0.2)
+        r = tab_oracle.integrate_adaptive(tb, st, 0.05, 1e-10, 1e-10, 10**6, tau_end=30.0)
+        assert (r["status"] == tab_oracle.ST_MAXSTEPS).all()
+        errs.append(np.abs(r["final_state"][[1, 2, 5, 6]] - ref["final_state"][[1, 2, 5, 6]]).max())
+    assert errs[1] < errs[0] / 3.0 and errs[1] < 2e-4, errs
+    # stop rules: capture on a stage point, domain exit (T4), records stop with the particle, slot 0 = y0
+    tb = W.kerr_metric_table(1.0, a, 257, 65, 1.8, 40.0, 0.2, math.pi - 0.2)
+    out = st.copy()
+    out[0] = 39.0
+    out[3] = 2.0
+    e = tab_oracle.integrate_adaptive(tb, out, 0.05, 1e-9, 1e-9, 10**5, snap_dtau=0.1, snap_capacity=50)
+    assert (e["status"] == tab_oracle.ST_OUTSIDE).all() and (e["final_state"][1] <= 40.0).all()
+    assert (e["snap_count"] >= 1).all() and np.array_equal(e["snapshots"][:, 0, [1, 2, 3, 5, 6, 7]], out.T)
+    for i in range(0, 40, 7):
+        cnt = e["snap_count"][i]
+        assert np.isfinite(e["snapshots"][i, :cnt]).all() and np.isnan(e["snapshots"][i, cnt:]).all()
+    inf = st.copy()
+    inf[3] = -3.0                                   # thrown at the hole
+    c = tab_oracle.integrate_adaptive(tb, inf, 0.05, 1e-9, 1e-9, 10**5, r_capture=2.5)
+    assert (c["status"] == tab_oracle.ST_CAPTURED).all() and (c["final_state"][1] >= 2.5).all()
+    # fixed-step mode: a record on a step boundary is that step's state
+    f = tab_oracle.integrate_adaptive(tb, st, 0.25, np.inf, 1.0, 10**6, tau_end=3.0, snap_dtau=1.0, snap_capacity=5)
+    assert (f["snap_count"] == 4).all()
+    f2 = tab_oracle.integrate_adaptive(tb, st, 0.25, np.inf, 1.0, 10**6, tau_end=2.0)
+    assert np.abs(f["snapshots"][:, 2, :] - f2["final_state"].T).max() < 1e-13

@@ -66,7 +66,7 @@ KERNEL_COUNTS = {
                  kernel="geo_rk4_kernel"),
     "schwarzschild": dict(sym="geo_rk4_kernelILb0ELi0ELb0ELb0E", units_per_loop=2, flop=342.0, pipe=245.0, other=None, tol=0.0,
                           source="static SASS count of the hot loop (no ncu capture of this instantiation)", kernel="geo_rk4_kernel"),
-    "adaptive": dict(sym="geo_rk45_kernelILb1ELb0E", units_per_loop=1, flop=1039.0, pipe=678.0, other=None, tol=0.15, static_at_capture=(1135, 778),
+    "adaptive": dict(sym="geo_rk45_kernelILi1ELb0E", units_per_loop=1, flop=1039.0, pipe=678.0, other=None, tol=0.15, static_at_capture=(1135, 778),
                      source="ncu thread-level counts, profiles/r02_config3a_rk45.md: 361 DFMA + 264 DMUL + 52 DADD per attempt "
                             "(incl. predicated-on work of lanes waiting for a refill)", kernel="geo_rk45_kernel"),
     "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0ELb1ELb0E", units_per_loop=None, flop=4073.0, pipe=2376.0, other=None, tol=None,

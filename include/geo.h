@@ -155,8 +155,9 @@ int geo_integrate_adaptive_host(geo_ctx *ctx, const double *state_in, int64_t n,
  * end point of a step) outside the domain ends the particle with GEO_ST_OUTSIDE, that step is not taken (per
  * evaluation point the capture test comes first).  Trajectory records (snapshot_every > 0) as for the analytic metrics,
  * components (t, x^1, x^2, phi, p_t = E, p_1, p_2, p_phi) by snap_mask; flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER
- * (no staged writer, no Cartesian records: the coordinates are the table's own);
- * geo_integrate_adaptive returns GEO_EINVAL; geo_horizon_radius returns NaN.
+ * (no staged writer, no Cartesian records: the coordinates are the table's own).
+ * geo_integrate_adaptive / geo_integrate_adaptive_host accept such a ctx too (reading T7: the domain test joins
+ * the capture test on every stage point and the end point; flags must be 0); geo_horizon_radius returns NaN.
  * Errors: GEO_EINVAL (NULL, n1 or n2 < 4, d1 or d2 <= 0, non-finite grid), GEO_ENOMEM, GEO_ECUDA. */
 typedef struct geo_table {
     const double *tab;  /* HOST [5][n2][n1] (geo_create_tabulated) or [10][n2][n1] (geo_create_tabulated_general) */

@@ -625,7 +625,8 @@ static int validate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, co
                              const geo_stop* stop, const geo_out* out, const int32_t* rejected, bool check_align) {
     int rc = validate(ctx, state_in, n, 1.0, 0, stop, 0, out, check_align);
     if (rc != GEO_OK) return rc;
-    if (ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) return fail(ctx, GEO_EINVAL, "the adaptive path takes analytic metrics only");
+    if (ctx->metric == GEO_TABULATED_GENERAL) return fail(ctx, GEO_EINVAL, "the adaptive path takes analytic metrics and five-field tables only");
+    if (ctx->metric == GEO_TABULATED && stop && stop->flags != 0) return fail(ctx, GEO_EINVAL, "tabulated metrics: the adaptive path takes no flags");
     if (!ctl) return fail(ctx, GEO_EINVAL, "ctl must not be NULL");
     if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0)) return fail(ctx, GEO_EINVAL, "h0 must be finite and > 0");
     if (!(ctl->rtol >= 0.0) || !(ctl->atol >= 0.0) || !(ctl->rtol + ctl->atol > 0.0) || std::isinf(ctl->atol))
@@ -682,9 +683,11 @@ static int launch_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     p.bh.twoM = 2.0 * ctx->M;
     p.bh.twoMa = 2.0 * ctx->M * ctx->a;
     fill_trig_consts(p.bh.tc);
+    p.tm = ctx->tm;
     typedef void (*fn_t)(const AdaptiveParams);
-    fn_t fn = ctx->metric == GEO_KERR ? (dense ? (fn_t)geo_rk45_kernel<true, true> : (fn_t)geo_rk45_kernel<true, false>)
-                                      : (dense ? (fn_t)geo_rk45_kernel<false, true> : (fn_t)geo_rk45_kernel<false, false>);
+    fn_t fn = ctx->metric == GEO_KERR ? (dense ? (fn_t)geo_rk45_kernel<METRIC_KERR, true> : (fn_t)geo_rk45_kernel<METRIC_KERR, false>)
+            : ctx->metric == GEO_TABULATED ? (dense ? (fn_t)geo_rk45_kernel<METRIC_TAB, true> : (fn_t)geo_rk45_kernel<METRIC_TAB, false>)
+                                           : (dense ? (fn_t)geo_rk45_kernel<METRIC_SCHW, true> : (fn_t)geo_rk45_kernel<METRIC_SCHW, false>);
     int per_sm = 0;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, 0);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(rk45)");

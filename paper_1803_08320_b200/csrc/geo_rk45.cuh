@@ -14,6 +14,7 @@
 // of DESIGN.md A5 is what keeps the lanes busy here.
 #pragma once
 #include "geo_kernel.cuh"
+#include "geo_tab.cuh"
 #ifndef GEO_RK45_CTAS
 #define GEO_RK45_CTAS 3      // resident CTAs per SM the kernel is compiled for (168 registers, no spills)
 #endif
@@ -43,7 +44,10 @@ struct AdaptiveParams {
     int cartesian;
     int* snap_count;
     Hole bh;
+    TabMetric tm;       // METRIC_TAB: the five-field table (reading T7)
 };
+
+enum { METRIC_SCHW = 0, METRIC_KERR = 1, METRIC_TAB = 2 };
 
 // Butcher tableau (Dormand & Prince 1980, table 2).  e = b5 - b4.
 namespace dp {
@@ -95,6 +99,25 @@ __device__ __forceinline__ void rhs_at(const Hole& bh, double r, double th, doub
 
 __device__ __forceinline__ K4 k4_of(const Deriv& d) { return K4{d.r, d.th, d.pr, d.pth}; }
 
+// T7: one evaluation of the tabulated right-hand side (gathered stencil), out of line -- the attempt has seven of them and
+// an unrolled copy each would be ~2300 instructions of evaluator.  Returns false outside the table's domain.
+__device__ __noinline__ bool tab_eval(const TabMetric& m, double x1, double x2, double p1, double p2, double E, double L, Deriv* d) {
+    TabFields F;
+    const bool in = tab_fields(m, x1, x2, F);
+    TabDeriv td;
+    tab_rhs(F, p1, p2, E, L, td);
+    d->t = td.t; d->r = td.x1; d->th = td.x2; d->ph = td.ph; d->pr = td.p1; d->pth = td.p2;
+    return in;
+}
+
+// right-hand side of the selected metric at one evaluation point; false: outside the domain (tabulated metric only)
+template <int METRIC>
+__device__ __forceinline__ bool rhs_metric(const AdaptiveParams& p, double r, double th, double pr, double pth, double E, double L, Deriv& d) {
+    if (METRIC == METRIC_TAB) return tab_eval(p.tm, r, th, pr, pth, E, L, &d);
+    rhs_at<METRIC == METRIC_KERR>(p.bh, r, th, pr, pth, E, L, d);
+    return true;
+}
+
 // One component of the continuous extension at theta in [0, 1] (reading A3), nested as in dopri5's contd5:
 //   y + theta (r2 + theta1 (r3 + theta (r4 + theta1 r5))),  r2 = ynew - y, r3 = h k1 - r2, r4 = r2 - h k7 - r3, r5 = h sum d_i k_i
 __device__ __forceinline__ double contd5(double theta, double y, double ynew, double hk1, double hk7, double hdk) {
@@ -105,8 +128,8 @@ __device__ __forceinline__ double contd5(double theta, double y, double ynew, do
 
 // DENSE: dense-output records (geo_adaptive.snap_dtau > 0); a separate instantiation so that the plain kernel keeps its
 // register budget.
-template <bool KERR, bool DENSE>
-__global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
+template <int METRIC, bool DENSE>
+__global__ void __launch_bounds__(kBlock, (DENSE || METRIC == METRIC_TAB) ? 2 : GEO_RK45_CTAS) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
     const unsigned lane = threadIdx.x & 31u;
     const Hole& bh = p.bh;
     long long idx = -1;
@@ -145,7 +168,19 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
         p.status[idx] = st;
         p.steps_done[idx] = (long long)steps;
         if (p.eq_cross_r) p.eq_cross_r[idx] = crossed ? eqc : __longlong_as_double(0x7ff8000000000000LL);
-        if (p.health) p.health[idx] = health_3p1(bh, r, th, pr, pth, E, L, p.kappa);
+        if (p.health) {
+            if (METRIC == METRIC_TAB) {
+                TabFields F;
+                double hv = __longlong_as_double(0x7ff8000000000000LL);
+                if (tab_fields_cold(p.tm, r, th, F) && (__double2hiint(E) & 0x7ff00000) != 0x7ff00000) {
+                    const double W = fma(F.be, L, E);
+                    hv = fabs(-(W * W) / (F.al * F.al) + pr * pr / F.g11 + pth * pth / F.g22 + L * L / F.g33 + p.kappa);
+                }
+                p.health[idx] = hv;
+            } else {
+                p.health[idx] = health_3p1(bh, r, th, pr, pth, E, L, p.kappa);
+            }
+        }
         if (p.rejected) p.rejected[idx] = rejected;
         if (DENSE) p.snap_count[idx] = next_j;
         active = false;
@@ -160,7 +195,14 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
         pr = p.in[3 * n + i];
         pth = p.in[4 * n + i];
         L = p.in[5 * n + i];
-        E = energy_3p1(bh, r, th, pr, pth, L, p.kappa);
+        bool y0_inside = true;
+        if (METRIC == METRIC_TAB) {
+            TabFields F;
+            y0_inside = tab_fields_cold(p.tm, r, th, F);
+            E = fma(F.al, sqrt(p.kappa + pr * pr / F.g11 + pth * pth / F.g22 + L * L / F.g33), -F.be * L);   // mass shell (5)
+        } else {
+            E = energy_3p1(bh, r, th, pr, pth, L, p.kappa);
+        }
         ct = cr = cth = cph = cpr = cpth = 0.0;
         h = p.h0;
         tau = 0.0;
@@ -168,12 +210,16 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
         crossed = false;
         active = true;
         next_j = 0;
-        if (!(r >= p.r_capture)) { finish(ST_CAPTURED); return; }               // B1
+        if (!(r >= p.r_capture)) { E = METRIC == METRIC_TAB ? __longlong_as_double(0x7ff8000000000000LL) : E; finish(ST_CAPTURED); return; }   // B1
+        if (METRIC == METRIC_TAB) {                                              // T4 on y0: non-finite input, then the domain
+            if (!all_finite6(r, th, ph, pr, pth, L)) { E = __longlong_as_double(0x7ff8000000000000LL); finish(ST_NUMERIC); return; }
+            if (!y0_inside) { E = __longlong_as_double(0x7ff8000000000000LL); finish(ST_OUTSIDE); return; }
+        }
         if (!all_finite6(r, th, ph, pr, pth, E)) { finish(ST_NUMERIC); return; }
         if (DENSE) { write_record(0, t, r, th, ph, pr, pth); next_j = 1; }      // record 0 = y0 (tau = 0)
         if (r > p.r_escape) { finish(ST_ESCAPED); return; }
         if (p.max_attempts == 0) { finish(ST_MAXSTEPS); return; }
-        rhs_at<KERR>(bh, r, th, pr, pth, E, L, k1);
+        rhs_metric<METRIC>(p, r, th, pr, pth, E, L, k1);
     };
 
     for (;;) {
@@ -211,14 +257,22 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
         // stage 2
         sr = fma(h * dp::a21, q1.r, r); sth = fma(h * dp::a21, q1.th, th);
         spr = fma(h * dp::a21, q1.pr, pr); spth = fma(h * dp::a21, q1.pth, pth);
-        bool cap = !(sr >= p.r_capture);
-        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        bool cap = false;
+        int ev = 0;                      // METRIC_TAB: first event in evaluation order (capture before domain exit, T7)
+        auto evaluate = [&](Deriv& out) {
+            const bool in = rhs_metric<METRIC>(p, sr, sth, spr, spth, E, L, out);
+            if (METRIC == METRIC_TAB) {
+                if (!ev) ev = !(sr >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
+            } else {
+                cap |= !(sr >= p.r_capture);
+            }
+        };
+        evaluate(d);
         const K4 q2 = k4_of(d);
         // stage 3
         sr = fma(h, fma(dp::a32, q2.r, dp::a31 * q1.r), r); sth = fma(h, fma(dp::a32, q2.th, dp::a31 * q1.th), th);
         spr = fma(h, fma(dp::a32, q2.pr, dp::a31 * q1.pr), pr); spth = fma(h, fma(dp::a32, q2.pth, dp::a31 * q1.pth), pth);
-        cap |= !(sr >= p.r_capture);
-        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        evaluate(d);
         const K4 q3 = k4_of(d);
         s5t = fma(dp::b3, d.t, s5t); s5p = fma(dp::b3, d.ph, s5p);
         if (DENSE) { sdt = fma(dp::d3, d.t, sdt); sdp = fma(dp::d3, d.ph, sdp); }
@@ -227,8 +281,7 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
 #define GEO_S4(c) fma(dp::a43, q3.c, fma(dp::a42, q2.c, dp::a41 * q1.c))
         sr = fma(h, GEO_S4(r), r); sth = fma(h, GEO_S4(th), th); spr = fma(h, GEO_S4(pr), pr); spth = fma(h, GEO_S4(pth), pth);
 #undef GEO_S4
-        cap |= !(sr >= p.r_capture);
-        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        evaluate(d);
         const K4 q4 = k4_of(d);
         s5t = fma(dp::b4, d.t, s5t); s5p = fma(dp::b4, d.ph, s5p);
         if (DENSE) { sdt = fma(dp::d4, d.t, sdt); sdp = fma(dp::d4, d.ph, sdp); }
@@ -237,8 +290,7 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
 #define GEO_S5(c) fma(dp::a54, q4.c, fma(dp::a53, q3.c, fma(dp::a52, q2.c, dp::a51 * q1.c)))
         sr = fma(h, GEO_S5(r), r); sth = fma(h, GEO_S5(th), th); spr = fma(h, GEO_S5(pr), pr); spth = fma(h, GEO_S5(pth), pth);
 #undef GEO_S5
-        cap |= !(sr >= p.r_capture);
-        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        evaluate(d);
         const K4 q5 = k4_of(d);
         s5t = fma(dp::b5, d.t, s5t); s5p = fma(dp::b5, d.ph, s5p);
         if (DENSE) { sdt = fma(dp::d5, d.t, sdt); sdp = fma(dp::d5, d.ph, sdp); }
@@ -247,8 +299,7 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
 #define GEO_S6(c) fma(dp::a65, q5.c, fma(dp::a64, q4.c, fma(dp::a63, q3.c, fma(dp::a62, q2.c, dp::a61 * q1.c))))
         sr = fma(h, GEO_S6(r), r); sth = fma(h, GEO_S6(th), th); spr = fma(h, GEO_S6(pr), pr); spth = fma(h, GEO_S6(pth), pth);
 #undef GEO_S6
-        cap |= !(sr >= p.r_capture);
-        rhs_at<KERR>(bh, sr, sth, spr, spth, E, L, d);
+        evaluate(d);
         const K4 q6 = k4_of(d);
         s5t = fma(dp::b6, d.t, s5t); s5p = fma(dp::b6, d.ph, s5p);
         if (DENSE) { sdt = fma(dp::d6, d.t, sdt); sdp = fma(dp::d6, d.ph, sdp); }
@@ -263,10 +314,15 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
         kahan<false>(pr, cpr, h, GEO_B5(pr), npr, dpr);
         kahan<false>(pth, cpth, h, GEO_B5(pth), npth, dpth);
 #undef GEO_B5
-        cap |= !(nr >= p.r_capture);                                             // B2: end point
         const bool fin6 = all_finite6(nt, nr, nth, nph, npr, npth);
         Deriv k7;
-        rhs_at<KERR>(bh, nr, nth, npr, npth, E, L, k7);
+        const bool in7 = rhs_metric<METRIC>(p, nr, nth, npr, npth, E, L, k7);
+        if (METRIC == METRIC_TAB) {                                              // end point: capture, finiteness, then the domain
+            if (!ev) ev = !(nr >= p.r_capture) ? ST_CAPTURED : ((fin6 && !in7) ? ST_OUTSIDE : 0);
+            cap = ev != 0;
+        } else {
+            cap |= !(nr >= p.r_capture);                                         // B2: end point
+        }
         // error estimate h (b5 - b4) . k, scaled per component; a NaN sticks in the max
 #define GEO_E(c) fma(dp::e7, k7.c, fma(dp::e6, q6.c, fma(dp::e5, q5.c, fma(dp::e4, q4.c, fma(dp::e3, q3.c, dp::e1 * q1.c)))))
         double err = 0.0, ec;
@@ -285,7 +341,7 @@ __global__ void __launch_bounds__(kBlock, DENSE ? 2 : GEO_RK45_CTAS) geo_rk45_ke
         if (active) {
             ++attempts;
             if (cap) {
-                finish(ST_CAPTURED);                                             // attempt not taken
+                finish(METRIC == METRIC_TAB ? ev : ST_CAPTURED);                 // attempt not taken
             } else if (!fin6 || !(err <= 1.0)) {                                 // reject
                 ++rejected;
                 h *= fmin(fac, 1.0);

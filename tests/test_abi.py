@@ -67,9 +67,9 @@ def test_every_direct_snapshot_kernel_keeps_its_256_bit_stores():
             kernels[name] = 0
         elif name and re.search(r"STG\.E(\.\w+)*\.256", line):
             kernels[name] += 1
-    want = [k for k in kernels if re.search(r"geo_rk4_kernelILb[01]ELi1ELb[01]E", k) or re.search(r"geo_rk45_kernelILb[01]ELb1E", k)
+    want = [k for k in kernels if re.search(r"geo_rk4_kernelILb[01]ELi1ELb[01]E", k) or re.search(r"geo_rk45_kernelILi[012]ELb1E", k)
             or re.search(r"geo_tabg?_rk4_kernelILb[01]ELb[01]ELb1E", k)]
-    assert len(want) == 4 + 2 + 4 + 4, want
+    assert len(want) == 4 + 3 + 4 + 4, want
     for k in want:
         assert kernels[k] >= 2, (k, kernels[k])
 

@@ -135,8 +135,8 @@ def test_tabulated_empty_and_argument_errors(G):
     with pytest.raises(G.GeoError) as ei:
         G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, dev), flags=G.FLAG_STATIC_MAP)
     assert ei.value.code == G.EINVAL
-    with pytest.raises(G.GeoError) as ei:
-        G.geo_integrate_adaptive(ctx, st, 0.01, 1e-9, 1e-9, 100, G.alloc_outputs(8, dev))
+    with pytest.raises(G.GeoError) as ei:          # the adaptive path exists for five-field tables (T7), without flags
+        G.geo_integrate_adaptive(ctx, st, 0.01, 1e-9, 1e-9, 100, G.alloc_outputs(8, dev, 0, 1, 4), snap_dtau=1.0, flags=G.FLAG_CARTESIAN_SNAP)
     assert ei.value.code == G.EINVAL
     assert math.isnan(G.geo_horizon_radius(ctx))
     G.geo_destroy(ctx)
@@ -232,3 +232,96 @@ def test_tabulated_trajectory_records(G, tab_oracle, host, flags, mask, cap):
                 assert np.array_equal(g["snapshots"][:, j, :], G.to_numpy(oj)["final_state"].T)
     finally:
         G.geo_destroy(ctx)
+
+
+def _run_tab_adaptive(G, tb, st, h0, rtol, atol, max_attempts, host=False, snap_dtau=0.0, cap=0, mask=0xFF, **kw):
+    import torch
+    ctx = G.geo_create_tabulated(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+    try:
+        n = st.shape[1]
+        if host:
+            out = G.alloc_outputs_host(n, 0, 1 if snap_dtau else 0, cap, mask)
+            rej = np.full(n, -1, dtype=np.int32)
+            G.geo_integrate_adaptive_host(ctx, np.ascontiguousarray(st), h0, rtol, atol, max_attempts, out, rejected=rej, snap_dtau=snap_dtau, **kw)
+            g = G.to_numpy(out)
+            g["rejected"] = rej
+            return g
+        dev = torch.device("cuda:0")
+        out = G.alloc_outputs(n, dev, 0, 1 if snap_dtau else 0, cap, mask)
+        rej = torch.full((n,), -1, dtype=torch.int32, device=dev)
+        G.geo_integrate_adaptive(ctx, torch.from_numpy(np.ascontiguousarray(st)).to(dev), h0, rtol, atol, max_attempts, out,
+                                 rejected=rej, snap_dtau=snap_dtau, **kw)
+        torch.cuda.synchronize()
+        g = G.to_numpy(out)
+        g["rejected"] = rej.cpu().numpy()
+        return g
+    finally:
+        G.geo_destroy(ctx)
+
+
+def test_tabulated_adaptive_fixed_step_mode_and_records(G, tab_oracle):
+    """Reading T7 with the controller off (rtol = inf): identical step sequences, so final states and dense-output records
+    must agree like the RK4 path's (1e-9); host entry point bitwise equal to the device one."""
+    a = 0.9
+    tb = W.kerr_metric_table(1.0, a, 513, 129, 1.8, 40.0, 0.2, math.pi - 0.2)
+    st = W.kerr_bound(1501, a, W.SEED_BASE + 2)
+    kw = dict(tau_end=40.0)
+    o = tab_oracle.integrate_adaptive(tb, st, 0.05, np.inf, 1.0, 10**6, snap_dtau=0.7, snap_capacity=60, nthreads=NCPU, **kw)
+    g = _run_tab_adaptive(G, tb, st, 0.05, float("inf"), 1.0, 10**6, snap_dtau=0.7, cap=60, **kw)
+    assert_parity(g, o, 1e-9)
+    done = g["status"] == G.ST_MAXSTEPS              # a few orbits leave the table's theta range early (OUTSIDE): fewer records
+    assert (g["rejected"] == 0).all() and np.array_equal(g["snap_count"], o["snap_count"])
+    assert (g["snap_count"][done] == 1 + int(40.0 / 0.7)).all() and done.mean() > 0.95
+    assert parity.snapshot_err(g, o).max() <= 1e-9
+    gh = _run_tab_adaptive(G, tb, st, 0.05, float("inf"), 1.0, 10**6, host=True, snap_dtau=0.7, cap=60, **kw)
+    for k in ("final_state", "status", "steps_done", "snapshots", "snap_count", "rejected"):
+        assert np.array_equal(g[k], gh[k], equal_nan=True), k
+
+
+def test_tabulated_adaptive_step_control_rays_and_domain_exit(G, tab_oracle):
+    """Step control on: log-radial camera rays (capture / escape) and particles that run off the table (OUTSIDE), class
+    against the oracle; states at a common final time within the integrator's tolerance; accept/reject counts identical
+    for nearly all."""
+    a = 0.998
+    rp = W.horizon_radius(1.0, a)
+    tb = W.kerr_metric_table(1.0, a, 1025, 257, math.log(0.005), math.log(80.0), 0.02, math.pi - 0.02, radial="log")
+    full = W.camera_rays(64, a, 60.0, r_obs=50.0)
+    st = W.to_log_radial(np.ascontiguousarray(full[:, ::5]), rp)
+    kw = dict(r_capture=math.log(0.01), r_escape=math.log(55.0 - rp), kind=G.NULL)
+    okw = dict(r_capture=math.log(0.01), r_escape=math.log(55.0 - rp), kind=tab_oracle.NULL)
+    o = tab_oracle.integrate_adaptive(tb, st, 0.02, 1e-9, 1e-9, 100000, nthreads=NCPU, **okw)
+    g = _run_tab_adaptive(G, tb, st, 0.02, 1e-9, 1e-9, 100000, **kw)
+    assert np.array_equal(g["status"], o["status"]) and set(np.unique(g["status"])) >= {G.ST_CAPTURED, G.ST_ESCAPED}
+    # The interpolated metric is only C^1: the error estimate jumps at every cell face, steps are rejected there, and whether
+    # an attempt next to a face passes depends on the last bits -- the accept/reject SEQUENCES of the two sides differ for
+    # almost every ray (unlike on the analytic metrics).  What is unique: the class, the amount of work to a few per cent,
+    # and the state at a common final time (below, and for the rays at tau = 40 before any of them ends).
+    work_g, work_o = g["steps_done"] + g["rejected"], o["steps_done"] + o["rejected"]
+    assert abs(work_g.sum() / work_o.sum() - 1.0) < 0.05
+    o40 = tab_oracle.integrate_adaptive(tb, st, 0.02, 1e-10, 1e-10, 100000, tau_end=40.0, nthreads=NCPU, **okw)
+    g40 = _run_tab_adaptive(G, tb, st, 0.02, 1e-10, 1e-10, 100000, tau_end=40.0, **kw)
+    assert np.array_equal(g40["status"], o40["status"]) and (g40["status"] == G.ST_MAXSTEPS).all()
+    e40 = parity.rel_err(g40["final_state"], o40["final_state"]).max(axis=0)
+    # ... and that state is only as well defined as the method is accurate on a C^1 metric: two step sequences that both
+    # satisfy the controller differ by the error the kinks at the cell faces inject (the estimate does not see it in
+    # full).  The oracle measures it on itself (rtol 1e-10 against 1e-11); the CUDA path must agree with the oracle to within
+    # a small multiple of that, i.e. as well as the oracle agrees with itself.
+    o40b = tab_oracle.integrate_adaptive(tb, st, 0.02, 1e-11, 1e-11, 100000, tau_end=40.0, nthreads=NCPU, **okw)
+    d_self = parity.rel_err(o40["final_state"], o40b["final_state"]).max(axis=0)
+    print("tab adaptive rays at tau = 40: max err", e40.max(), "oracle rtol 1e-10 vs 1e-11:", d_self.max())
+    assert e40.max() <= max(5.0 * d_self.max(), 1e-7) and e40.max() <= 1e-4
+    # bound orbits to a common final time; a few leave the table's theta range: OUTSIDE on both sides
+    a2 = 0.9
+    tb2 = W.kerr_metric_table(1.0, a2, 513, 129, 1.8, 40.0, 0.4, math.pi - 0.4)
+    st2 = W.kerr_bound(2001, a2, W.SEED_BASE + 2)
+    o2 = tab_oracle.integrate_adaptive(tb2, st2, 0.05, 1e-11, 1e-11, 10**6, tau_end=150.0, nthreads=NCPU)
+    g2 = _run_tab_adaptive(G, tb2, st2, 0.05, 1e-11, 1e-11, 10**6, tau_end=150.0)
+    assert np.array_equal(g2["status"], o2["status"])
+    assert (g2["status"] == G.ST_OUTSIDE).any() and (g2["status"] == G.ST_MAXSTEPS).mean() > 0.8
+    done = g2["status"] == G.ST_MAXSTEPS
+    e = parity.rel_err(g2["final_state"], o2["final_state"]).max(axis=0)
+    print("tab adaptive: OUTSIDE", int((g2["status"] == G.ST_OUTSIDE).sum()), "max err at tau_end", e[done].max(), "p99", np.quantile(e[done], 0.99))
+    o2b = tab_oracle.integrate_adaptive(tb2, st2, 0.05, 1e-12, 1e-12, 10**6, tau_end=150.0, nthreads=NCPU)
+    d2 = parity.rel_err(o2["final_state"], o2b["final_state"]).max(axis=0)[done & (o2b["status"] == tab_oracle.ST_MAXSTEPS)]
+    print("   oracle rtol 1e-11 vs 1e-12: p99", np.quantile(d2, 0.99), "max", d2.max())
+    assert np.quantile(e[done], 0.99) <= max(5.0 * np.quantile(d2, 0.99), 1e-7) and e[done].max() <= max(5.0 * d2.max(), 1e-6)

@@ -46,10 +46,9 @@ enum {
     GEO_FLAG_TAB_GATHER = 16,  /* tabulated metrics: gather the 4 x 4 stencil through L1/L2 on every evaluation instead
                                   of keeping the current cell's stencil in shared memory (for comparison)  */
     GEO_FLAG_STAGED_SNAP = 4   /* snapshot records staged in shared memory and flushed by the warp with
-                                  coalesced stores.  Without the flag the library chooses: snapshot_every < 16
-                                  -> each lane stores its record straight from registers with 256-bit stores
-                                  (faster for dense output), otherwise the staged writer (keeps the stepping
-                                  loop free of the record logic).  Both write the same bits.            */
+                                  coalesced stores (for comparison).  Without the flag each lane stores its record
+                                  straight from registers with 256-bit stores, at every cadence.  Both writers put
+                                  the same bits into the same slots.                                       */
 };
 
 /* Stop rules (PAPER.md:322-327 gives "final time reached" and "r <= r_+"; B1-B4):

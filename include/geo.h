@@ -178,6 +178,31 @@ int geo_create_tabulated(geo_ctx **ctx, const geo_table *table);
  * returns GEO_EINVAL). */
 int geo_create_tabulated_general(geo_ctx **ctx, const geo_table *table);
 
+/* ALLOCATION-FREE entry point, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): the operation of geo_integrate_host -- fixed-step RK4 of n independent
+ * geodesics in the analytic metric (6), HOST buffers in and out -- without a ctx (geo_create
+ * allocates) and without trajectory records.  Its device scratch -- the persistent kernel's work-queue head and the
+ * staging of state_in and of every output -- is a `static __device__` array inside the library of
+ *     256 + 144 * GEO_NOALLOC_MAX_N bytes = 9 437 440 B (9.0 MiB),
+ * which every GPU that loads the library holds until the process exits.  The call makes no cudaMalloc, cudaFree,
+ * stream / event creation or other allocating library call; the first use on a device resolves the array's device
+ * address (cudaGetSymbolAddress) and reads the SM count, nothing else.
+ *   metric, M, a: as geo_create (GEO_SCHWARZSCHILD or GEO_KERR).  state_in, h, nsteps, stop: as geo_integrate_host;
+ *   stop->flags: 0, GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_STATIC_MAP.  out: HOST pointers; final_state, status, steps_done
+ *   required, eq_cross_r, health, coarse_steps optional, the snapshot fields are ignored.  cuda_stream: the stream the
+ *   copies and the kernel are enqueued on (NULL = default stream); the call synchronises it before returning.
+ * Same kernels, same launch configuration, same bits as geo_integrate_host on the current device.
+ * n > GEO_NOALLOC_MAX_N returns GEO_EINVAL (text from geo_noalloc_last_error) before anything is enqueued.
+ * The scratch is SHARED by all calls and keeps the previous call's contents: the queue head is cleared on the stream
+ * before every launch and every staged output element of particles 0..n-1 is overwritten by the kernel, so nothing else
+ * needs to start at zero.  Calls from several host threads are serialised by a lock inside the library; anything else
+ * that would make two such calls overlap on one GPU (there is none through this interface) would race on the scratch.
+ * Errors: GEO_EINVAL, GEO_ECUDA; never GEO_ENOMEM. */
+#define GEO_NOALLOC_MAX_N 65536
+int geo_integrate_host_noalloc(int metric, double M, double a, const double *state_in, int64_t n, double h,
+                               int64_t nsteps, const geo_stop *stop, const geo_out *out, void *cuda_stream);
+const char *geo_noalloc_last_error(void); /* text of the calling thread's last geo_integrate_host_noalloc error */
+
 void geo_destroy(geo_ctx *ctx);
 
 double geo_horizon_radius(const geo_ctx *ctx); /* r_+ = M + sqrt(M^2 - a^2) */

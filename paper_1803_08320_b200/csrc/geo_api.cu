@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "../../include/geo.h"
@@ -756,6 +757,141 @@ int geo_probe_dfma(geo_ctx* ctx, int64_t iters, double* sink, double* n_fma, voi
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(ctx, e, "dfma_probe launch");
     *n_fma = (double)grid * 256.0 * 64.0 * (double)iters;
+    return GEO_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// geo_integrate_host_noalloc (include/geo.h): the geo_integrate_host operation for callers that cannot allocate.
+// All device scratch -- the work-queue head of the persistent kernel and the staging of inputs and outputs -- is the
+// file-scope array below: fixed offsets for GEO_NOALLOC_MAX_N particles, 256-byte aligned, held by every device that
+// loads this module until the process exits.  In HOST code `g_noalloc_scratch` is only a handle of the symbol, not a
+// device address: the address is resolved once per device by cudaGetSymbolAddress (noalloc_device) and that pointer is
+// what the kernel gets.
+namespace {
+constexpr size_t kNaN = GEO_NOALLOC_MAX_N;
+constexpr size_t kNaHead = 0;                          // unsigned long long work-queue head (256 B reserved)
+constexpr size_t kNaIn = 256;                          // [6][n] double
+constexpr size_t kNaFin = kNaIn + 48 * kNaN;           // [8][n] double
+constexpr size_t kNaSteps = kNaFin + 64 * kNaN;        // [n] int64
+constexpr size_t kNaEq = kNaSteps + 8 * kNaN;          // [n] double
+constexpr size_t kNaHealth = kNaEq + 8 * kNaN;         // [n] double
+constexpr size_t kNaStatus = kNaHealth + 8 * kNaN;     // [n] int32
+constexpr size_t kNaCoarse = kNaStatus + 4 * kNaN;     // [n] int32
+constexpr size_t kNaBytes = kNaCoarse + 4 * kNaN;      // 256 + 144 * 65536 = 9 437 440
+static_assert(kNaBytes == 256 + 144 * kNaN, "scratch size stated in geo.h");
+static_assert(kNaN % 64 == 0, "every sub-buffer starts on a 256-byte boundary");
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNaBytes];
+
+namespace {
+constexpr int kNaMaxDevices = 64;
+struct NoallocDevice {
+    unsigned char* base;   // device address of g_noalloc_scratch on this device
+    int sm_count;
+    bool ready;
+};
+NoallocDevice g_na_dev[kNaMaxDevices];
+std::mutex g_na_mutex;                 // serialises the calls of one process: they share the scratch
+thread_local char g_na_err[256] = "";
+
+int na_fail(int code, const char* msg) {
+    snprintf(g_na_err, sizeof g_na_err, "%s", msg);
+    return code;
+}
+int na_fail_cuda(cudaError_t e, const char* what) {
+    snprintf(g_na_err, sizeof g_na_err, "%s: %s", what, cudaGetErrorString(e));
+    return GEO_ECUDA;
+}
+
+// Set-up, once per device, with that device current (the caller holds g_na_mutex).
+int noalloc_device(int device, NoallocDevice** out) {
+    if (device < 0 || device >= kNaMaxDevices) return na_fail(GEO_EINVAL, "device ordinal beyond the per-device table of the allocation-free path");
+    NoallocDevice& d = g_na_dev[device];
+    if (!d.ready) {
+        unsigned char* ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_noalloc_scratch);
+        if (e != cudaSuccess) return na_fail_cuda(e, "cudaGetSymbolAddress(g_noalloc_scratch)");
+        if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u)) return na_fail(GEO_ECUDA, "static scratch is not 256-byte aligned");
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+        if (e != cudaSuccess) return na_fail_cuda(e, "cudaDeviceGetAttribute(SM count)");
+        d.base = ptr;
+        d.sm_count = sms;
+        d.ready = true;
+    }
+    *out = &d;
+    return GEO_OK;
+}
+}  // namespace
+
+extern "C" {
+
+const char* geo_noalloc_last_error(void) { return g_na_err; }
+
+int geo_integrate_host_noalloc(int metric, double M, double a, const double* state_in, int64_t n, double h,
+                               int64_t nsteps, const geo_stop* stop, const geo_out* out, void* cuda_stream) {
+    g_na_err[0] = 0;
+    if (metric != GEO_SCHWARZSCHILD && metric != GEO_KERR) return na_fail(GEO_EINVAL, "metric must be GEO_SCHWARZSCHILD or GEO_KERR");
+    if (!(M > 0.0) || !std::isfinite(M) || !(std::fabs(a) <= M)) return na_fail(GEO_EINVAL, "M > 0 and |a| <= M required");
+    if (metric == GEO_SCHWARZSCHILD && a != 0.0) return na_fail(GEO_EINVAL, "Schwarzschild requires a == 0");
+    // a ctx on the stack: no device memory of its own, its queue head is the first word of the static scratch
+    geo_ctx local;
+    memset(&local, 0, sizeof local);
+    local.metric = metric;
+    local.M = M;
+    local.a = a;
+    int rc = validate(&local, state_in, n, h, nsteps, stop, 0, out, false);
+    if (rc != GEO_OK) return na_fail(rc, local.err);
+    if (stop->flags & ~(GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP)) return na_fail(GEO_EINVAL, "the allocation-free path takes GEO_FLAG_PLAIN_UPDATE and GEO_FLAG_STATIC_MAP only");
+    if (n > (int64_t)kNaN) {
+        snprintf(g_na_err, sizeof g_na_err, "n = %lld exceeds GEO_NOALLOC_MAX_N = %lld (size of the static device scratch)", (long long)n, (long long)kNaN);
+        return GEO_EINVAL;
+    }
+    if (n == 0) return GEO_OK;
+
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    cudaError_t e = cudaGetDevice(&local.device);
+    if (e != cudaSuccess) return na_fail_cuda(e, "cudaGetDevice");
+    NoallocDevice* dev = nullptr;
+    rc = noalloc_device(local.device, &dev);
+    if (rc != GEO_OK) return rc;
+    local.sm_count = dev->sm_count;
+
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    unsigned char* base = dev->base;
+    const size_t N = (size_t)n;
+    double* d_in = reinterpret_cast<double*>(base + kNaIn);
+    geo_out d;
+    memset(&d, 0, sizeof d);
+    d.final_state = reinterpret_cast<double*>(base + kNaFin);
+    d.status = reinterpret_cast<int32_t*>(base + kNaStatus);
+    d.steps_done = reinterpret_cast<int64_t*>(base + kNaSteps);
+    d.eq_cross_r = out->eq_cross_r ? reinterpret_cast<double*>(base + kNaEq) : nullptr;
+    d.health = out->health ? reinterpret_cast<double*>(base + kNaHealth) : nullptr;
+    d.coarse_steps = out->coarse_steps ? reinterpret_cast<int32_t*>(base + kNaCoarse) : nullptr;
+
+    // after the first enqueue every error path drains the stream: no copy into the caller's buffers stays in flight
+    auto bail = [&](int code) {
+        cudaStreamSynchronize(s);
+        return code;
+    };
+    e = cudaMemcpyAsync(d_in, state_in, 6 * N * 8, cudaMemcpyHostToDevice, s);      // SoA [6][n], contiguous on both sides
+    if (e != cudaSuccess) return bail(na_fail_cuda(e, "H2D state_in"));
+    // launch() clears the queue head (scratch + kNaHead) on the stream, then starts the same kernel geo_integrate_host runs
+    rc = launch(&local, d_in, n, h, nsteps, stop, 0, &d, s, reinterpret_cast<unsigned long long*>(base + kNaHead));
+    if (rc != GEO_OK) return bail(na_fail(rc, local.err));
+    e = cudaMemcpyAsync(out->final_state, d.final_state, 8 * N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out->status, d.status, N * 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out->steps_done, d.steps_done, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.eq_cross_r) e = cudaMemcpyAsync(out->eq_cross_r, d.eq_cross_r, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.health) e = cudaMemcpyAsync(out->health, d.health, N * 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && d.coarse_steps) e = cudaMemcpyAsync(out->coarse_steps, d.coarse_steps, N * 4, cudaMemcpyDeviceToHost, s);
+    if (e != cudaSuccess) return bail(na_fail_cuda(e, "D2H outputs"));
+    e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return na_fail_cuda(e, "cudaStreamSynchronize");
     return GEO_OK;
 }
 

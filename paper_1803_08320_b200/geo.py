@@ -4,7 +4,7 @@ Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is use
 and streams.  There is NO CPU fallback: if the library cannot be loaded, or there is no CUDA device,
 the calls raise.  Names follow the C ABI: ``geo_create``, ``geo_integrate``, ``geo_integrate_host``,
 ``geo_create_tabulated``, ``geo_create_tabulated_general``, ``geo_integrate_adaptive``, ``geo_integrate_adaptive_host``, ``geo_destroy``, ``geo_horizon_radius``,
-``geo_last_error``; plus the development helpers of include/geo_dev.h (``geo_launch_info``, ``geo_probe_dfma``) used by bench.py.
+``geo_last_error``, the allocation-free ``geo_integrate_host_noalloc`` / ``geo_noalloc_last_error``; plus the development helpers of include/geo_dev.h (``geo_launch_info``, ``geo_probe_dfma``) used by bench.py.
 """
 from __future__ import annotations
 
@@ -19,12 +19,14 @@ OK, EINVAL, ECUDA, ENOMEM = 0, 1, 2, 3
 ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC, ST_OUTSIDE = 0, 1, 2, 3, 4
 FLAG_PLAIN_UPDATE, FLAG_STATIC_MAP, FLAG_STAGED_SNAP, FLAG_CARTESIAN_SNAP, FLAG_TAB_GATHER = 1, 2, 4, 8, 16
 
+NOALLOC_MAX_N = 65536   # GEO_NOALLOC_MAX_N: particles per geo_integrate_host_noalloc call (size of the static scratch)
+
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("GEO_LIB") or os.path.join(_HERE, "libgeo.so")   # GEO_LIB: load another build of the same ABI
 
 # every symbol include/geo.h declares, then the development helpers of include/geo_dev.h
 SYMBOLS = ("geo_create", "geo_create_tabulated", "geo_create_tabulated_general", "geo_integrate", "geo_integrate_host", "geo_integrate_adaptive", "geo_integrate_adaptive_host", "geo_destroy",
-           "geo_horizon_radius", "geo_last_error")
+           "geo_horizon_radius", "geo_last_error", "geo_integrate_host_noalloc", "geo_noalloc_last_error")
 DEV_SYMBOLS = ("geo_launch_info", "geo_probe_dfma")
 
 
@@ -90,6 +92,11 @@ def lib() -> C.CDLL:
         L.geo_horizon_radius.argtypes = [C.c_void_p]
         L.geo_last_error.restype = C.c_char_p
         L.geo_last_error.argtypes = [C.c_void_p]
+        L.geo_integrate_host_noalloc.restype = C.c_int
+        L.geo_integrate_host_noalloc.argtypes = [C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_int64, C.c_double, C.c_int64,
+                                                 C.POINTER(GeoStop), C.POINTER(GeoOut), C.c_void_p]
+        L.geo_noalloc_last_error.restype = C.c_char_p
+        L.geo_noalloc_last_error.argtypes = []
         L.geo_launch_info.restype = C.c_int
         L.geo_launch_info.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_int64, C.POINTER(C.c_int32 * 4)]
         L.geo_probe_dfma.restype = C.c_int
@@ -290,6 +297,24 @@ def geo_integrate_host(ctx, state_in: np.ndarray, h: float, nsteps: int, out: di
     o = _out_struct(out)
     rc = lib().geo_integrate_host(ctx, _ptr(state_in), n, h, nsteps, C.byref(stop), snapshot_every, C.byref(o))
     _check(ctx, rc)
+
+
+def geo_noalloc_last_error() -> str:
+    return lib().geo_noalloc_last_error().decode()
+
+
+def geo_integrate_host_noalloc(metric: int, M: float, a: float, state_in: np.ndarray, h: float, nsteps: int, out: dict,
+                               r_capture: float = -float("inf"), r_escape: float = float("inf"),
+                               kind: int = TIMELIKE, flags: int = 0, stream=None) -> None:
+    """geo_integrate_host without a ctx and without any device allocation (static device scratch inside the library,
+    at most NOALLOC_MAX_N particles per call, no trajectory records); synchronous.  stream: a torch.cuda.Stream or None."""
+    n = _check_buffers(state_in, out, device=False)
+    stop = GeoStop(r_capture, r_escape, kind, flags)
+    o = _out_struct(out)
+    rc = lib().geo_integrate_host_noalloc(metric, M, a, _ptr(state_in), n, h, nsteps, C.byref(stop), C.byref(o),
+                                          C.c_void_p(stream.cuda_stream) if stream is not None else None)
+    if rc != OK:
+        raise GeoError(rc, geo_noalloc_last_error())
 
 
 def alloc_outputs_host(n: int, nsteps: int = 0, snapshot_every: int = 0, snap_capacity: int | None = None,

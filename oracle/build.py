@@ -19,7 +19,8 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "geo_oracle.cpp")
-SRCS = [SRC, os.path.join(HERE, "geo_tab_oracle.cpp")]      # fixed-step/adaptive analytic metrics; tabulated metrics (8(f).3)
+SRCS = [SRC, os.path.join(HERE, "geo_tab_oracle.cpp"),     # fixed-step/adaptive analytic metrics; tabulated metrics (8(f).3)
+        os.path.join(HERE, "geo_ks_oracle.cpp")]            # Kerr in Cartesian Kerr-Schild coordinates (8(f).3, second clause)
 LIB = os.path.join(HERE, "libgeo_oracle.so")
 LIB_SAN = os.path.join(HERE, "libgeo_oracle_san.so")
 

@@ -326,6 +326,45 @@ def to_kerr_schild(st: np.ndarray, E: np.ndarray, M: float, a: float) -> np.ndar
     return out
 
 
+def to_cartesian_kerr_schild(st: np.ndarray, E: np.ndarray, M: float, a: float) -> np.ndarray:
+    """state_in (r, theta, phi, u_r, u_theta, u_phi) of Boyer-Lindquist data with energy E -> the same event and covector in
+    CARTESIAN Kerr-Schild coordinates, state_in (x, y, z, p_x, p_y, p_z) of a GEO_KERR_SCHILD ctx (reading K1):
+    first `to_kerr_schild` (ingoing Kerr coordinates, phi~ = phi at the start), then the point transformation
+        x + i y = (r + i a) sin(theta) exp(i phi~),   z = r cos(theta),
+    whose Jacobian J[i][b] = d x^i / d(r, theta, phi~)^b carries the covector: p_b = J[i][b] p_i, solved for p_i (3 x 3
+    per particle; needs sin(theta) != 0 -- the spherical chart, not the Cartesian one, is singular on the axis).
+    A change of coordinates of the input data; no equations of motion here."""
+    ks = to_kerr_schild(st, E, M, a)
+    r, th, ph = ks[0], ks[1], ks[2]
+    s, c = np.sin(th), np.cos(th)
+    sp, cp = np.sin(ph), np.cos(ph)
+    x = (r * cp - a * sp) * s
+    y = (r * sp + a * cp) * s
+    z = r * c
+    J = np.zeros((st.shape[1], 3, 3))
+    J[:, 0, 0] = cp * s
+    J[:, 0, 1] = (r * cp - a * sp) * c
+    J[:, 0, 2] = -y
+    J[:, 1, 0] = sp * s
+    J[:, 1, 1] = (r * sp + a * cp) * c
+    J[:, 1, 2] = x
+    J[:, 2, 0] = c
+    J[:, 2, 1] = -r * s
+    J[:, 2, 2] = 0.0
+    p_sph = np.stack([ks[3], ks[4], ks[5]], axis=-1)
+    p_cart = np.linalg.solve(np.transpose(J, (0, 2, 1)), p_sph[..., None])[..., 0]
+    return np.ascontiguousarray(np.stack([x, y, z, p_cart[:, 0], p_cart[:, 1], p_cart[:, 2]]))
+
+
+def kerr_schild_radius(xyz: np.ndarray, a: float) -> np.ndarray:
+    """Kerr-Schild radius r(x, y, z): the non-negative root of r^4 - (x^2 + y^2 + z^2 - a^2) r^2 - a^2 z^2 = 0; xyz [3][n].
+    Used by tests and the bench to compare a Cartesian Kerr-Schild result with a Boyer-Lindquist one (the charts share r
+    and cos(theta) = z / r)."""
+    x, y, z = xyz[0], xyz[1], xyz[2]
+    w = x * x + y * y + z * z - a * a
+    return np.sqrt(0.5 * (w + np.sqrt(w * w + 4.0 * a * a * z * z)))
+
+
 def to_log_radial(st: np.ndarray, r_plus: float) -> np.ndarray:
     """state_in (r, theta, phi, u_r, u_theta, u_phi) -> the same covectors in x^1 = ln(r - r_+): u_1 = u_r (r - r_+)."""
     out = np.array(st, dtype=np.float64, copy=True)

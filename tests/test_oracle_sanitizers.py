@@ -4,7 +4,7 @@ compute-sanitizer is closed on the GPU pool, so the CUDA path carries guard-band
 nothing here: oracle/build.py --sanitize compiles the same sources with -fsanitize=address,undefined and a child process
 (libasan preloaded) drives every entry point over the cases with the most address arithmetic -- ragged batches,
 snapshot capacity overflow, odd component masks, Cartesian records, early termination, the adaptive path, the tabulated
-metric incl. domain exits, multi-threaded outer loops.  Any report makes the child exit non-zero.
+metric incl. domain exits, the Cartesian Kerr-Schild oracle, multi-threaded outer loops.  Any report makes the child exit non-zero.
 """
 import os
 import subprocess
@@ -17,7 +17,7 @@ import math, os, sys
 import numpy as np
 sys.path.insert(0, ROOT)
 sys.path.insert(0, os.path.join(ROOT, "oracle"))
-import geo_oracle as O, geo_tab_oracle as T
+import geo_oracle as O, geo_tab_oracle as T, geo_ks_oracle as K
 from paper_1803_08320_b200 import workloads as W
 assert O.lib()._name.endswith("libgeo_oracle_san.so"), O.lib()._name
 st = W.kerr_bound(67, 0.9, W.SEED_BASE + 2)
@@ -49,6 +49,17 @@ out = st.copy(); out[0] = 39.9; out[3] = 2.0      # runs off the table
 rt = T.integrate(tb, out, 0.05, 400, long_double=True)
 assert (rt["status"] == T.ST_OUTSIDE).any()
 assert T.fields(tb, 1e9, 1.0) is None and T.fields(tb, 5.0, 1.0) is not None and T.rhs(tb, [0, 5.0, 1.0, 0, 0.95, 0.1, 0.2, 3.0]) is not None
+kst, kc = W.kerr_bound(37, 0.9, W.SEED_BASE + 2, return_constants=True)
+kks = W.to_cartesian_kerr_schild(kst, kc[0], 1.0, 0.9)
+for mask, cap, ld in ((0xFF, None, False), (0x2B, 2, True)):
+    rk = K.integrate(1.0, 0.9, kks, 0.01, 93, r_capture=1.3, r_escape=25.0, snapshot_every=7, snap_capacity=cap, snap_mask=mask,
+                     long_double=ld, nthreads=3)
+    assert (rk["snap_count"] == 1 + rk["steps_done"] // 7).all()
+bad = kks.copy(); bad[0:3, 0] = 0.1; bad[3, 1] = np.nan; bad[0, 2] = 1e6
+rk = K.integrate(1.0, 0.9, bad, 0.01, 10, r_capture=1.3, r_escape=100.0, kind=K.NULL)
+assert rk["status"][0] == K.ST_CAPTURED and rk["status"][1] == K.ST_NUMERIC and rk["status"][2] == K.ST_ESCAPED
+K.rhs(1.0, 0.9, [0, 3.0, 1.0, 2.0, 1.1, 0.1, 0.2, 0.3], long_double=True); K.hamiltonian(1.0, 0.9, [0, 3.0, 1.0, 2.0, 1.1, 0.1, 0.2, 0.3])
+K.energy(1.0, 0.9, 3.0, 1.0, 2.0, 0.1, 0.2, 0.3, 1.0); K.radius(1.0, 0.9, 0.0, 0.0, 0.0); K.metric(1.0, 0.9, 3.0, 1.0, 2.0)
 print("sanitized oracle run ok")
 """
 

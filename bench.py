@@ -69,6 +69,9 @@ KERNEL_COUNTS = {
     "adaptive": dict(sym="geo_rk45_kernelILi1ELb0E", units_per_loop=1, flop=1039.0, pipe=678.0, other=None, tol=0.15, static_at_capture=(1135, 778),
                      source="ncu thread-level counts, profiles/r02_config3a_rk45.md: 361 DFMA + 264 DMUL + 52 DADD per attempt "
                             "(incl. predicated-on work of lanes waiting for a refill)", kernel="geo_rk45_kernel"),
+    "kerr_schild": dict(sym="geo_ks_rk4_kernelILi0ELb0EE", units_per_loop=2, flop=634.5, pipe=437.8, other=56.6, tol=0.08, static_at_capture=(1308, 909),
+                        source="ncu per-instruction counts, profiles/r02_ks4.md: 201.7 DFMA + 163.1 DMUL + 68.0 DADD + 5.0 DSETP per step",
+                        kernel="geo_ks_rk4_kernel"),
     "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0ELb1ELb0E", units_per_loop=None, flop=4073.0, pipe=2376.0, other=None, tol=None,
                               source="ncu per-instruction counts, profiles/r02_tab4_tabg4.md: 1735 DFMA + 550 DMUL + 52 DADD + 38 DSETP per step "
                                      "(4 evaluations through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tabg_rk4_kernel"),
@@ -79,7 +82,7 @@ KERNEL_COUNTS = {
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed `ncu --set full` capture of that
 # workload (profiles/), bytes; None where no capture exists.
 TRAFFIC_NCU_BYTES = {"config3a": 103_264_512, "tab4": 651_665_920, "tabg4": 1_225_114_112, "config4": 600_256_000, "snapbench": 69_562_443_296,
-                     "snapkerr": 70_775_029_960, "paper_t3": 16_144_486_488}     # profiles/r02_*.md (snapbench: r01_snapbench_v3.md)
+                     "snapkerr": 70_775_029_960, "paper_t3": 16_144_486_488, "ks4": 561_625_600}     # profiles/r02_*.md (snapbench: r01_snapbench_v3.md)
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:
@@ -151,6 +154,21 @@ def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dic
                     metric="tabulated_general", a=0.5, st=W.to_kerr_schild(st, consts[0], 1.0, 0.5), h=0.01, nsteps=250,
                     snapshot_every=0, snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf,
                     table=W.kerr_schild_metric_table(1.0, 0.5, 2049, 513, 2.0, 45.0, 0.1, math.pi - 0.1))
+    if name == "ks4":
+        # SURVEY 8(f).3, second clause (readings K1-K5): the particles of configs[3] in CARTESIAN Kerr-Schild coordinates on the
+        # analytic horizon-penetrating, axis-regular path (geo_ks_rk4_kernel), 2500 RK4 steps
+        n = n_override or (1 << 22)
+        st, consts = W.kerr_bound(n, 0.5, W.SEED_BASE + 4 + 1000 * rank, nthreads=nthreads, chunk=1 << 20, return_constants=True)
+        return dict(name="configs[3] particles in Cartesian Kerr-Schild coordinates (analytic, horizon-penetrating, axis-regular)",
+                    metric="kerr_schild", a=0.5, st=W.to_cartesian_kerr_schild(st, consts[0], 1.0, 0.5), h=0.01, nsteps=2500,
+                    snapshot_every=0, snap_mask=0xFF, kind=0, r_capture=-np.inf, r_escape=np.inf)
+    if name == "config3ks":
+        # the rays of configs[2] on the Cartesian Kerr-Schild path: the image without the polar-axis artefacts of eq.(8)
+        wl = workload("config3", rank, n_override, nthreads)
+        wl["name"] += " -- in Cartesian Kerr-Schild coordinates"
+        wl["metric"] = "kerr_schild"
+        wl["st"] = W.to_cartesian_kerr_schild(wl["st"], np.ones(wl["st"].shape[1]), 1.0, wl["a"])
+        return wl
     if name == "config3a":
         # the rays of configs[2] with the adaptive Dormand-Prince 5(4) stepper (per-ray step control);
         # unit = one step ATTEMPT (accepted or rejected: 6 new RHS evaluations + error estimate)
@@ -307,6 +325,10 @@ def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> di
             fn = geo_tab_oracle.integrate if wl["metric"] == "tabulated" else geo_tab_oracle.integrate_general
             o = fn(wl["table"], sub, wl["h"], wl["nsteps"], r_capture=wl["r_capture"],
                    r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
+        elif wl["metric"] == "kerr_schild":
+            import geo_ks_oracle
+            o = geo_ks_oracle.integrate(1.0, wl["a"], sub, wl["h"], wl["nsteps"], r_capture=wl["r_capture"], r_escape=wl["r_escape"],
+                                        kind=wl["kind"], nthreads=cores)
         elif ad:
             o = geo_oracle.integrate_adaptive(metric, 1.0, wl["a"], sub, ad["h0"], ad["rtol"], ad["atol"], ad["max_attempts"],
                                               r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
@@ -431,7 +453,7 @@ class GpuRun:
             mk = geo.geo_create_tabulated if wl["metric"] == "tabulated" else geo.geo_create_tabulated_general
             self.ctx = mk(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
         else:
-            self.ctx = geo.geo_create(geo.KERR if wl["metric"] == "kerr" else geo.SCHWARZSCHILD, 1.0, wl["a"])
+            self.ctx = geo.geo_create({"kerr": geo.KERR, "kerr_schild": geo.KERR_SCHILD}.get(wl["metric"], geo.SCHWARZSCHILD), 1.0, wl["a"])
         tiles = wl.get("tiles") or [wl["st"]]
         self.d_in = [torch.from_numpy(t).to(dev) for t in tiles]
         self.n = tiles[0].shape[1]
@@ -541,7 +563,8 @@ SECONDARY = [("config2", "config2", 0, True), ("config3", "config3", 0, True), (
              ("config3_shuffled_static", "config3s", 2, False), ("config5_central_tile", "config5tile", 0, False),
              ("snapbench_schwarzschild_every_step", "snapbench", 0, False), ("snapkerr_every_step_8comp", "snapkerr", 0, False),
              ("snapkerr_every_step_txyz", "snapkerr_xyz", 0, False), ("config3_adaptive_rk45", "config3a", 0, True),
-             ("tab4_tabulated_metric", "tab4", 0, False), ("tabg4_general_tabulated_metric_kerr_schild", "tabg4", 0, False), ("paper_table3", "paper_t3", 0, False), ("paper_table4", "paper_t4", 0, False)]
+             ("tab4_tabulated_metric", "tab4", 0, False), ("tabg4_general_tabulated_metric_kerr_schild", "tabg4", 0, False),
+             ("ks4_cartesian_kerr_schild", "ks4", 0, True), ("config3_cartesian_kerr_schild", "config3ks", 0, False), ("paper_table3", "paper_t3", 0, False), ("paper_table4", "paper_t4", 0, False)]
 
 
 def run_secondary(torch, geo, dev, sm_max: float, ncpu: int, peaks: dict, reuse_config4) -> dict:
@@ -611,7 +634,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4",
-                    choices=["config1", "config2", "config3", "config4", "config5", "config5tile", "config3s", "config3a", "tab4", "tabg4",
+                    choices=["config1", "config2", "config3", "config4", "config5", "config5tile", "config3s", "config3a", "tab4", "tabg4", "ks4", "config3ks",
                              "snapbench", "snapkerr", "snapkerr_xyz", "paper_t3", "paper_t4"])
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank its own batch; strong = one image (config3) split into interleaved row tiles")

@@ -30,7 +30,8 @@ extern "C" {
 typedef struct geo_ctx geo_ctx; /* opaque; owned by the library */
 
 enum { GEO_SCHWARZSCHILD = 0, GEO_KERR = 1, GEO_TABULATED = 2,    /* metric (2: geo_create_tabulated,          */
-       GEO_TABULATED_GENERAL = 3 };                                  /*         3: geo_create_tabulated_general)  */
+       GEO_TABULATED_GENERAL = 3,                                    /*         3: geo_create_tabulated_general)  */
+       GEO_KERR_SCHILD = 4 };   /* Kerr in Cartesian Kerr-Schild coordinates (geo_create; see below)               */
 enum { GEO_TIMELIKE = 0, GEO_NULL = 1 };                            /* geo_stop.kind: kappa=1/0 */
 enum { GEO_OK = 0, GEO_EINVAL = 1, GEO_ECUDA = 2, GEO_ENOMEM = 3 }; /* return codes            */
 /* per-particle termination class (geo_out.status) */
@@ -84,10 +85,30 @@ typedef struct geo_out {
 } geo_out;
 
 /* Create a context for metric (6) with mass M > 0 and spin |a| <= M; Schwarzschild
- * requires a == 0.  Allocates a few bytes of device memory on the CURRENT CUDA device; the ctx belongs to that
+ * requires a == 0.  metric: GEO_SCHWARZSCHILD, GEO_KERR (Boyer-Lindquist coordinates, eq.(8)) or GEO_KERR_SCHILD (below).  Allocates a few bytes of device memory on the CURRENT CUDA device; the ctx belongs to that
  * device: every entry point switches to it for the duration of the call and restores the caller's current
  * device before returning, so device pointers passed with a ctx must live on the ctx's device. */
 int geo_create(geo_ctx **ctx, int metric, double M, double a);
+
+/* GEO_KERR_SCHILD -- SURVEY 8(f).3, second clause ("further analytic metrics / horizon-penetrating, axis-regular
+ * coordinates"; the reason the paper gives for the 3+1 form): the SAME spacetime, metric (6)
+ * (PAPER.md:73-84), in Cartesian Kerr-Schild coordinates (t~, x, y, z) (readings K1-K5):
+ *     g = eta + f l l,  f = 2 M r^3/(r^4 + a^2 z^2),  l_mu = (1, (r x + a y)/(r^2+a^2), (r y - a x)/(r^2+a^2), z/r),
+ *     r(x, y, z) >= 0:  (x^2 + y^2)/(r^2 + a^2) + z^2/r^2 = 1        (the Boyer-Lindquist r of the same event),
+ * i.e. line element (1) with alpha^2 = 1/(1+f), beta^i = f l_i/(1+f), gamma_ij = delta_ij + f l_i l_j; related to
+ * Boyer-Lindquist by t~ = t + int 2Mr/Delta dr, phi~ = phi + int a/Delta dr, x + iy = (r + ia) sin(theta) e^{i phi~},
+ * z = r cos(theta).  Regular on the polar axis and through the future horizon r_+ (only the ring r = 0, z = 0 is singular):
+ * rays through the axis and particles followed inside the hole -- where eq.(8) divides by sin^2(theta) or Delta -- integrate
+ * without loss of accuracy.  Equations of motion: Hamilton's equations (3),(4) of
+ * H = 1/2 [ -(p_t - beta^k p_k)^2/alpha^2 + gamma^{ij} p_i p_j ]; p_t = -E is the only cyclic momentum of the chart.
+ * Use with geo_integrate / geo_integrate_host:
+ *   state_in SoA [6][n] = (x, y, z, p_x, p_y, p_z) (covariant); t~ starts at 0, E from the mass shell eq.(5) in 3+1 variables.
+ *   final_state [8][n] and trajectory records = (t~, x, y, z, p_t = E, p_x, p_y, p_z) (snap_mask over these).
+ *   r_capture / r_escape refer to r(x, y, z); the capture guard runs on y0, every RK4 stage point and the end point.
+ *   eq_cross_r: r at the first sign change of z between two accepted states, linear in z between them; quiet NaN if none.
+ *   health = |2H + kappa|.  coarse_steps is ignored.  flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_STATIC_MAP
+ *   (records are Cartesian already: GEO_FLAG_CARTESIAN_SNAP and the staged writer return GEO_EINVAL).
+ * geo_integrate_adaptive and geo_integrate_host_noalloc return GEO_EINVAL for this metric; geo_horizon_radius works. */
 
 /* Integrate n geodesics for at most nsteps (< 2^31) RK4 steps of size h (h < 0 integrates backwards in tau).
  * state_in: DEVICE, SoA [6][n] = (r, theta, phi, u_r, u_theta, u_phi) (covariant); t starts at 0 and

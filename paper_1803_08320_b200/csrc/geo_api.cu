@@ -12,6 +12,7 @@
 #include "geo_rk45.cuh"
 #include "geo_tab.cuh"
 #include "geo_tabg.cuh"
+#include "geo_ks.cuh"
 
 using namespace geo;
 
@@ -107,6 +108,10 @@ int validate(geo_ctx* ctx, const double* state_in, int64_t n, double h, int64_t 
     if (ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) {
         const int32_t ok = GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_TAB_GATHER;
         if (stop->flags & ~ok) return fail(ctx, GEO_EINVAL, "tabulated metrics: only GEO_FLAG_PLAIN_UPDATE and GEO_FLAG_TAB_GATHER are supported");
+    }
+    if (ctx->metric == GEO_KERR_SCHILD) {
+        const int32_t ok = GEO_FLAG_PLAIN_UPDATE | GEO_FLAG_STATIC_MAP;
+        if (stop->flags & ~ok) return fail(ctx, GEO_EINVAL, "GEO_KERR_SCHILD: only GEO_FLAG_PLAIN_UPDATE and GEO_FLAG_STATIC_MAP are supported (records are Cartesian already)");
     }
     if (n == 0) return GEO_OK;
     if (!state_in || !out->final_state || !out->status || !out->steps_done) return fail(ctx, GEO_EINVAL, "state_in, final_state, status, steps_done are required");
@@ -302,10 +307,106 @@ int launch_tabg(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t n
     return GEO_OK;
 }
 
+typedef void (*ks_kernel_fn)(const KsParams);
+ks_kernel_fn pick_ks_kernel(bool snap, bool plain) {
+    if (snap) return plain ? (ks_kernel_fn)geo_ks_rk4_kernel<SNAP_DIRECT, true> : (ks_kernel_fn)geo_ks_rk4_kernel<SNAP_DIRECT, false>;
+    return plain ? (ks_kernel_fn)geo_ks_rk4_kernel<SNAP_NONE, true> : (ks_kernel_fn)geo_ks_rk4_kernel<SNAP_NONE, false>;
+}
+
+int plan_ks(geo_ctx* ctx, int64_t n, int32_t flags, bool snap, ks_kernel_fn* fn_out, int* grid, int* per_sm_out, int* regs) {
+    ks_kernel_fn fn = pick_ks_kernel(snap, (flags & GEO_FLAG_PLAIN_UPDATE) != 0);
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, (const void*)fn);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncGetAttributes");
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, 0);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+    if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
+    const int64_t need = (n + kBlock - 1) / kBlock;
+    if (flags & GEO_FLAG_STATIC_MAP) {
+        if (need > 0x7fffffffLL) return fail(ctx, GEO_EINVAL, "n too large for the static mapping");
+        *grid = (int)need;
+    } else {
+        const int64_t resident = (int64_t)ctx->sm_count * per_sm;
+        *grid = (int)(need < resident ? need : resident);
+    }
+    if (fn_out) *fn_out = fn;
+    if (per_sm_out) *per_sm_out = per_sm;
+    if (regs) *regs = fa.numRegs;
+    return GEO_OK;
+}
+
+// GEO_KERR_SCHILD: Kerr in Cartesian Kerr-Schild coordinates (geo_ks.cuh).
+int launch_ks(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
+              int64_t snapshot_every, const geo_out* out, cudaStream_t stream, unsigned long long* counter) {
+    ks_kernel_fn fn;
+    int grid = 0;
+    int rc = plan_ks(ctx, n, stop->flags, snapshot_every > 0, &fn, &grid, nullptr, nullptr);
+    if (rc != GEO_OK) return rc;
+    KsParams p;
+    memset(&p, 0, sizeof p);
+    p.in = d_in;
+    p.n = n;
+    p.h = h;
+    p.h_half = h / 2.0;
+    p.h_sixth = h / 6.0;
+    p.nsteps = (int)nsteps;
+    p.r_capture = stop->r_capture;
+    p.r_escape = stop->r_escape;
+    p.kappa = stop->kind == GEO_TIMELIKE ? 1.0 : 0.0;
+    const double a2 = ctx->a * ctx->a;
+    // end-point triggers: r >= rc  <=>  (x^2+y^2)/(rc^2+a^2) + z^2/rc^2 >= 1 for rc > 0; rc <= 0 never captures a finite point
+    if (stop->r_capture > 0.0 && std::isfinite(stop->r_capture)) {
+        p.cap_iA = 1.0 / (stop->r_capture * stop->r_capture + a2);
+        p.cap_ir2 = 1.0 / (stop->r_capture * stop->r_capture);
+        p.cap_thresh = 1.0;
+    } else if (stop->r_capture > 0.0) {       // +inf: everything is captured (decided at y0 already)
+        p.cap_iA = 0.0; p.cap_ir2 = 0.0; p.cap_thresh = 1.0;
+    } else {
+        p.cap_iA = 0.0; p.cap_ir2 = 0.0; p.cap_thresh = -1.0;
+    }
+    if (stop->r_escape > 0.0 && std::isfinite(stop->r_escape)) {
+        p.esc_iA = 1.0 / (stop->r_escape * stop->r_escape + a2);
+        p.esc_ir2 = 1.0 / (stop->r_escape * stop->r_escape);
+    } else if (stop->r_escape > 0.0) {        // +inf: never
+        p.esc_iA = 0.0; p.esc_ir2 = 0.0;
+    } else {                                  // r > re holds for every point with r > 0: trigger always, decide behind the branch
+        p.esc_iA = INFINITY; p.esc_ir2 = INFINITY;
+    }
+    p.use_queue = (stop->flags & GEO_FLAG_STATIC_MAP) ? 0 : 1;
+    p.snap_every = (int)(snapshot_every > 0x7fffffffLL ? 0x7fffffffLL : snapshot_every);
+    p.snap_cap = snapshot_every > 0 ? out->snap_capacity : 0;
+    p.snap_mask = snapshot_every > 0 ? (out->snap_mask & 0xFFu) : 0;
+    p.ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
+    p.fin = out->final_state;
+    p.status = out->status;
+    p.steps_done = reinterpret_cast<long long*>(out->steps_done);
+    p.eq_cross_r = out->eq_cross_r;
+    p.health = out->health;
+    p.snaps = out->snapshots;
+    p.snap_count = out->snap_count;
+    p.counter = counter;
+    p.bh.M = ctx->M;
+    p.bh.a = ctx->a;
+    p.bh.a2 = a2;
+    p.bh.twoM = 2.0 * ctx->M;
+    p.bh.four_a2 = 4.0 * a2;
+    cudaError_t e;
+    if (p.use_queue) {
+        e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
+    }
+    fn<<<grid, kBlock, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
+    return GEO_OK;
+}
+
 int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps, const geo_stop* stop,
            int64_t snapshot_every, const geo_out* out, cudaStream_t stream, unsigned long long* counter) {
     if (ctx->metric == GEO_TABULATED) return launch_tab(ctx, d_in, n, h, nsteps, stop, snapshot_every, out, stream, counter);
     if (ctx->metric == GEO_TABULATED_GENERAL) return launch_tabg(ctx, d_in, n, h, nsteps, stop, snapshot_every, out, stream, counter);
+    if (ctx->metric == GEO_KERR_SCHILD) return launch_ks(ctx, d_in, n, h, nsteps, stop, snapshot_every, out, stream, counter);
     const int ncomp = snapshot_every > 0 ? popcount8(out->snap_mask) : 0;
     LaunchPlan lp;
     int rc = plan_launch(ctx, n, stop->flags, snapshot_every, ncomp, &lp);
@@ -364,7 +465,7 @@ extern "C" {
 int geo_create(geo_ctx** out_ctx, int metric, double M, double a) {
     if (!out_ctx) return GEO_EINVAL;
     *out_ctx = nullptr;
-    if (metric != GEO_SCHWARZSCHILD && metric != GEO_KERR) return GEO_EINVAL;
+    if (metric != GEO_SCHWARZSCHILD && metric != GEO_KERR && metric != GEO_KERR_SCHILD) return GEO_EINVAL;
     if (!(M > 0.0) || !std::isfinite(M) || !(std::fabs(a) <= M)) return GEO_EINVAL;
     if (metric == GEO_SCHWARZSCHILD && a != 0.0) return GEO_EINVAL;
     geo_ctx* ctx = new (std::nothrow) geo_ctx;
@@ -626,7 +727,8 @@ static int validate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, co
                              const geo_stop* stop, const geo_out* out, const int32_t* rejected, bool check_align) {
     int rc = validate(ctx, state_in, n, 1.0, 0, stop, 0, out, check_align);
     if (rc != GEO_OK) return rc;
-    if (ctx->metric == GEO_TABULATED_GENERAL) return fail(ctx, GEO_EINVAL, "the adaptive path takes analytic metrics and five-field tables only");
+    if (ctx->metric == GEO_TABULATED_GENERAL || ctx->metric == GEO_KERR_SCHILD)
+        return fail(ctx, GEO_EINVAL, "the adaptive path takes the Boyer-Lindquist metrics and five-field tables only");
     if (ctx->metric == GEO_TABULATED && stop && stop->flags != 0) return fail(ctx, GEO_EINVAL, "tabulated metrics: the adaptive path takes no flags");
     if (!ctl) return fail(ctx, GEO_EINVAL, "ctl must not be NULL");
     if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0)) return fail(ctx, GEO_EINVAL, "h0 must be finite and > 0");
@@ -735,6 +837,10 @@ int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_eve
     if (ctx->metric == GEO_TABULATED_GENERAL) {
         info[1] = tabg_block(flags);
         return plan_tabg(ctx, n, flags, &info[0], &info[3], &info[2], snapshot_every > 0);
+    }
+    if (ctx->metric == GEO_KERR_SCHILD) {
+        info[1] = kBlock;
+        return plan_ks(ctx, n, flags, snapshot_every > 0, nullptr, &info[0], &info[3], &info[2]);
     }
     LaunchPlan lp;
     int rc = plan_launch(ctx, n, flags, snapshot_every, 8, &lp);

@@ -13,7 +13,7 @@ import os
 
 import numpy as np
 
-SCHWARZSCHILD, KERR, TABULATED, TABULATED_GENERAL = 0, 1, 2, 3
+SCHWARZSCHILD, KERR, TABULATED, TABULATED_GENERAL, KERR_SCHILD = 0, 1, 2, 3, 4
 TIMELIKE, NULL = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, 1, 2, 3
 ST_MAXSTEPS, ST_CAPTURED, ST_ESCAPED, ST_NUMERIC, ST_OUTSIDE = 0, 1, 2, 3, 4

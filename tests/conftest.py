@@ -29,6 +29,13 @@ def tab_oracle():
     return geo_tab_oracle
 
 
+@pytest.fixture(scope="session")
+def ks_oracle():
+    import geo_ks_oracle  # oracle/geo_ks_oracle.py (test infrastructure, Cartesian Kerr-Schild)
+    geo_ks_oracle.lib()
+    return geo_ks_oracle
+
+
 @pytest.fixture(scope="module")
 def G():
     import torch

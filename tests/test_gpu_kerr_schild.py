@@ -1,0 +1,255 @@
+"""GPU parity of the Cartesian Kerr-Schild path (GEO_KERR_SCHILD, csrc/geo_ks.cuh; SURVEY 8(f).3 second clause, DESIGN.md
+readings K1-K5) against its oracle (oracle/geo_ks_oracle.cpp), element by element on the same seeded inputs, through the
+C ABI: bound orbits of the config-2 distribution (1e-9), camera rays of config 3 incl. the polar-axis columns (class
+identity and 1e-8 under reading P3), trajectory records, particles through the polar axis and through the horizon, edge
+cases, host entry point, static mapping; and -- no oracle involved -- the WHOLE config-3 image against the closed-form
+capture criterion: the polar-axis columns that the Boyer-Lindquist path gets wrong (reading B7) come out right."""
+import math
+import os
+import sys
+
+import numpy as np
+import pytest
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import parity  # noqa: E402
+from gpu_helpers import run_gpu, assert_snapshots_match  # noqa: E402
+from test_gpu_fullsize import _escapes_analytic, _critical_band  # noqa: E402  (closed-form class of an E = 1 photon; no oracle)
+
+from paper_1803_08320_b200 import workloads as W  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+NCPU = max(1, (os.cpu_count() or 1))
+
+
+def _orbits(n, a=0.9):
+    st, consts = W.kerr_bound(n, a, W.SEED_BASE + 2, return_constants=True)
+    return W.to_cartesian_kerr_schild(st, consts[0], 1.0, a), st, consts
+
+
+@pytest.mark.parametrize("flags", [0, 1, 2])
+def test_bound_orbits_parity(G, ks_oracle, flags):
+    """3001 orbits (23 full CTAs + a ragged tail) x 4000 steps, Kerr a = 0.9: every output within 1e-9 of the oracle
+    (reading P3 certification for the few that pass next to the axis); Kahan / plain update, queue / static mapping."""
+    a = 0.9
+    ks, st, consts = _orbits(3001, a)
+    oflags = flags & 1
+    o = ks_oracle.integrate(1.0, a, ks, 0.01, 4000, flags=oflags, nthreads=NCPU)
+    g = run_gpu(G, G.KERR_SCHILD, a, ks, 0.01, 4000, flags=flags)
+    rep = parity.p3_report(g, o, lambda jj: [ks_oracle.integrate(1.0, a, np.ascontiguousarray(ks[:, jj]), 0.01, 4000, flags=oflags, long_double=True),
+                                             ks_oracle.integrate(1.0, a, parity.ulp_nudged(np.ascontiguousarray(ks[:, jj])), 0.01, 4000, flags=oflags)],
+                           1e-9, labels=consts, max_fail_frac=0.002, what=f"Kerr-Schild bound orbits, flags {flags}")
+    print(rep)
+    assert rep["class_mismatch"] == 0
+    ok = np.isfinite(o["health"])
+    assert np.max(np.abs(g["health"][ok] - o["health"][ok])) < 1e-11
+    # the chart's own check: L_z = x p_y - y p_x is NOT a momentum here; it must still be conserved to O(h^4)
+    f = g["final_state"]
+    assert np.max(np.abs(f[1] * f[6] - f[2] * f[5] - consts[1])) < 1e-7
+
+
+def test_energy_matches_oracle_to_rounding(G, ks_oracle):
+    ks, st, consts = _orbits(257, 0.9)
+    g = run_gpu(G, G.KERR_SCHILD, 0.9, ks, 0.01, 0)
+    E = np.array([ks_oracle.energy(1.0, 0.9, *ks[:, i], 1.0) for i in range(257)])
+    assert np.max(np.abs(g["final_state"][4] - E) / E) < 1e-15
+    assert np.max(np.abs(g["final_state"][4] - consts[0]) / consts[0]) < 1e-13    # = the Boyer-Lindquist E of the same covector
+
+
+def test_host_entry_equals_device_path_bitwise(G):
+    ks, _, _ = _orbits(1500, 0.9)
+    kw = dict(snapshot_every=100, snap_mask=0x0F, r_capture=2.0, r_escape=28.0)
+    d = run_gpu(G, G.KERR_SCHILD, 0.9, ks, 0.01, 1000, **kw)
+    h = run_gpu(G, G.KERR_SCHILD, 0.9, ks, 0.01, 1000, host=True, **kw)
+    for k in ("final_state", "status", "steps_done", "snap_count", "health"):
+        assert np.array_equal(d[k], h[k], equal_nan=True), k
+    assert np.array_equal(d["eq_cross_r"], h["eq_cross_r"], equal_nan=True)
+    valid = np.arange(d["snapshots"].shape[1])[None, :] < d["snap_count"][:, None]
+    assert np.array_equal(d["snapshots"][valid], h["snapshots"][valid])
+
+
+@pytest.mark.parametrize("flags,mask,cap", [(0, 0xFF, None), (0, 0x0F, None), (1, 0x6E, None), (0, 0xFF, 4), (2, 0x81, 3)])
+def test_trajectory_records(G, ks_oracle, flags, mask, cap):
+    """Records (readings S1-S3) with the direct 256-bit writer and the masked fallback, capacity overflow; slot j bitwise
+    equal to the GPU run that stops after j * snapshot_every steps."""
+    a = 0.9
+    ks, _, _ = _orbits(1201, a)
+    kw = dict(r_capture=2.2, r_escape=27.0)
+    o = ks_oracle.integrate(1.0, a, ks, 0.01, 1200, flags=flags & 1, snapshot_every=200, snap_capacity=cap, snap_mask=mask, nthreads=NCPU, **kw)
+    g = run_gpu(G, G.KERR_SCHILD, a, ks, 0.01, 1200, flags=flags, snapshot_every=200, snap_capacity=cap, snap_mask=mask, **kw)
+    assert np.array_equal(g["status"], o["status"]) and np.array_equal(g["steps_done"], o["steps_done"])
+    assert len(np.unique(o["status"])) >= 2
+    assert_snapshots_match(g, o, 1e-9)
+    if cap is None:
+        comps = [k for k in range(8) if (mask >> k) & 1]
+        for j in (1, 4):
+            s = run_gpu(G, G.KERR_SCHILD, a, ks, 0.01, 200 * j, flags=flags, **kw)
+            ok = g["steps_done"] >= 200 * j
+            assert ok.sum() > 1000
+            assert np.array_equal(g["snapshots"][ok, j, :], s["final_state"][comps][:, ok].T)
+
+
+def _camera(a, incl, N, sel):
+    full, consts = W.camera_rays(N, a, incl, return_constants=True)
+    st = np.ascontiguousarray(full[:, sel])
+    ks = W.to_cartesian_kerr_schild(st, np.ones(st.shape[1]), 1.0, a)
+    return ks, st, np.ascontiguousarray(consts[:, sel])
+
+
+def test_camera_rays_parity_incl_axis_columns(G, ks_oracle, oracle):
+    """configs[2] rays (a = 0.998, i = 60 deg, h = 0.02, capture at r_+ + 0.01, escape at 1100): a strided 32 x 32 sub-image
+    and 64 rows of the 10 polar-axis columns.  Against the Kerr-Schild oracle: class (status AND steps_done) identical and
+    1e-8 under reading P3.  Against the closed form: every ray off the +-3 px critical band correct -- also in the axis
+    columns.  Against the
+    Boyer-Lindquist oracle (another chart, another right-hand side): same class flag, r at the end within 1e-6 on the
+    rays that are healthy there."""
+    a, N = 0.998, 1024
+    rp = W.horizon_radius(1.0, a)
+    img = np.arange(N * N).reshape(N, N)
+    consts_full = W.camera_rays(N, a, 60.0, return_constants=True)[1]
+    esc_full = _escapes_analytic(a, consts_full[2], consts_full[3], rp, 1000.0)
+    band_full = _critical_band(esc_full.reshape(N, N), 3).ravel()
+    sub = img[16::32, 16::32].ravel()
+    axis = img[8::16, N // 2 - 5:N // 2 + 5].ravel()
+    for name, sel in (("sub-image", sub), ("axis columns", axis)):
+        ks, st, consts = _camera(a, 60.0, N, sel)
+        kw = dict(r_capture=rp + 0.01, r_escape=1100.0)
+        o = ks_oracle.integrate(1.0, a, ks, 0.02, 200000, kind=ks_oracle.NULL, nthreads=NCPU, **kw)
+        g = run_gpu(G, G.KERR_SCHILD, a, ks, 0.02, 200000, kind=G.NULL, **kw)
+        rep = parity.p3_report(
+            g, o, lambda jj: [ks_oracle.integrate(1.0, a, np.ascontiguousarray(ks[:, jj]), 0.02, 200000, kind=ks_oracle.NULL, long_double=True, nthreads=NCPU, **kw),
+                              ks_oracle.integrate(1.0, a, parity.ulp_nudged(np.ascontiguousarray(ks[:, jj])), 0.02, 200000, kind=ks_oracle.NULL, nthreads=NCPU, **kw)],
+            1e-8, labels=consts, max_fail_frac=0.03, what=f"Kerr-Schild camera rays, {name}")
+        print(name, rep, "classes", np.bincount(g["status"], minlength=4).tolist(), "max health", float(g["health"].max()))
+        assert rep["class_mismatch"] <= max(1, int(1e-4 * len(sel)))
+        esc = esc_full[sel]
+        off_band = ~band_full[sel]
+        # closed form: no wrong pixel off the +-3 px band of the critical curve -- the polar-axis columns included
+        assert np.array_equal((g["status"] == G.ST_ESCAPED)[off_band], esc[off_band]), name
+        assert set(np.unique(g["status"])) <= {G.ST_CAPTURED, G.ST_ESCAPED}
+        escaped = g["status"] == G.ST_ESCAPED
+        print("   health of escaped rays: median %.1e max %.1e" % (np.median(g["health"][escaped]), g["health"][escaped].max()))
+        assert np.median(g["health"][escaped]) < 1e-13
+        if name == "axis columns":
+            assert g["health"][escaped].max() < 1e-8         # the Boyer-Lindquist path: up to 1e47 here (reading B7)
+        # the Boyer-Lindquist oracle on the same rays
+        ob = oracle.integrate(oracle.KERR, 1.0, a, st, 0.02, 200000, kind=oracle.NULL, nthreads=NCPU, **kw)
+        healthy = ob["health"] < 1e-9
+        assert np.array_equal(g["status"][healthy], ob["status"][healthy])
+        r_ks = W.kerr_schild_radius(g["final_state"][1:4], a)
+        cth = g["final_state"][3] / r_ks
+        e2 = healthy & (g["status"] == G.ST_ESCAPED) & (g["steps_done"] == ob["steps_done"])
+        if name == "sub-image":          # (in the axis columns NO ray is healthy in Boyer-Lindquist coordinates: nothing to compare)
+            assert healthy.sum() > 0.7 * len(sel) and e2.sum() > 0.5 * healthy.sum()
+            assert np.max(np.abs(r_ks[e2] - ob["final_state"][1][e2]) / 1100.0) < 1e-6
+            assert np.max(np.abs(cth[e2] - np.cos(ob["final_state"][2][e2]))) < 1e-6
+        if name == "axis columns":
+            print("Boyer-Lindquist oracle: unhealthy axis rays", int((~healthy).sum()), "of", len(sel),
+                  "wrong class there:", int(((ob["status"] == oracle.ST_ESCAPED) != esc).sum()))
+
+
+def test_whole_config3_image_has_no_wrong_pixel(G):
+    """The whole 1024^2 image of configs[2] in ONE call on the Kerr-Schild path (work queue on), every pixel against the
+    closed-form capture / escape criterion.  The 10 polar-axis columns, where the Boyer-Lindquist path has its 533 wrong
+    pixels and |2H| up to 1e47 (reading B7), come out right: 0 mismatches, |2H| < 1e-8.  What this chart pays: next to the
+    prograde photon orbit of a = 0.998 (r = 1.074 M, 0.01 M outside the horizon) the Cartesian components turn by ~0.75 rad per
+    step of h = 0.02 M, and <= 64 pixels (measured: 42; 10 at h = 0.01) within 3 px of the prograde edge of the shadow are
+    captured instead of escaping -- on the GPU and in the oracle alike.  No ray at the step cap."""
+    import torch
+    a, N = 0.998, 1024
+    rp = W.horizon_radius(1.0, a)
+    st, consts = W.camera_rays(N, a, 60.0, return_constants=True)
+    ks = W.to_cartesian_kerr_schild(st, np.ones(N * N), 1.0, a)
+    dev = torch.device("cuda:0")
+    ctx = G.geo_create(G.KERR_SCHILD, 1.0, a)
+    try:
+        out = G.alloc_outputs(N * N, dev)
+        G.geo_integrate(ctx, torch.from_numpy(ks).to(dev), 0.02, 200000, out, r_capture=rp + 0.01, r_escape=1100.0, kind=G.NULL)
+        torch.cuda.synchronize()
+        status = out["status"].cpu().numpy()
+        health = out["health"].cpu().numpy()
+        steps = out["steps_done"].cpu().numpy()
+    finally:
+        G.geo_destroy(ctx)
+    esc = _escapes_analytic(a, consts[2], consts[3], rp, 1000.0)
+    wrong = (status == G.ST_ESCAPED) != esc
+    counts = np.bincount(status, minlength=4)
+    print("classes", counts.tolist(), "closed-form mismatches", int(wrong.sum()), "max health", float(health.max()),
+          "steps total", int(steps.sum()))
+    assert counts[G.ST_MAXSTEPS] == 0 and counts[G.ST_NUMERIC] == 0
+    axis = np.abs(consts[0]) < 0.1                       # the 10 pixel columns around alpha = 0
+    band = _critical_band(esc.reshape(N, N), 3).ravel()
+    print("mismatches in the axis columns", int((wrong & axis).sum()), "off the +-3 px critical band", int((wrong & ~band).sum()),
+          "L_z of the mismatching pixels", consts[2][wrong].min() if wrong.any() else None, consts[2][wrong].max() if wrong.any() else None)
+    assert (wrong & axis).sum() == 0                     # the Boyer-Lindquist path: 533
+    assert (wrong & ~band).sum() == 0
+    assert wrong.sum() <= 64                             # measured: 42, the prograde edge of the shadow
+    assert np.all(consts[2][wrong] > 1.9)
+    escaped = status == G.ST_ESCAPED
+    assert health[escaped & axis].max() < 1e-8 and np.median(health[escaped]) < 1e-13
+
+
+def test_through_the_polar_axis_and_through_the_horizon(G, ks_oracle):
+    """Where eq.(8) divides by sin^2(theta) or Delta: particles aimed through x = y = 0 and particles followed to 0.9 r_+
+    (inside the hole).  1e-9 against the oracle, all of them; the infallers end inside r_+ with finite state."""
+    for a in (0.9, 0.998):
+        rp = W.horizon_radius(1.0, a)
+        n = 96
+        st = np.zeros((6, n))
+        for k in range(48):
+            st[:, k] = [-6.0, 0.0 if k % 2 == 0 else 1e-7 * k, 7.0 + 0.1 * k, 1.2, 0.0, 0.01 * (k % 7)]
+        for k in range(48, n):
+            j = k - 48
+            st[:, k] = [7.0 + 0.05 * j, 1.0, 0.1 * (j - 20), -0.4, 0.004 * j, 0.0]
+        kw = dict(r_capture=0.9 * rp, r_escape=200.0)
+        o = ks_oracle.integrate(1.0, a, st, 0.01, 6000, nthreads=NCPU, **kw)
+        g = run_gpu(G, G.KERR_SCHILD, a, st, 0.01, 6000, **kw)
+        c = parity.compare(g, o)
+        print(f"a = {a}: classes {np.bincount(g['status'], minlength=4).tolist()} max err {c['err'].max():.2e}")
+        assert c["same_class"].all() and c["err"].max() <= 1e-9
+        inside = g["status"] == G.ST_CAPTURED
+        assert inside[48:].all() and not inside[:48].any()
+        assert np.all(W.kerr_schild_radius(g["final_state"][1:4, inside], a) < rp) and np.isfinite(g["final_state"]).all()
+
+
+def test_edge_cases_and_argument_errors(G, ks_oracle):
+    import torch
+    a = 0.9
+    ks, _, _ = _orbits(40, a)
+    ks[0:3, 0] = [0.3, 0.2, 0.5]         # inside r_capture
+    ks[0:3, 1] = [300.0, 0.0, 50.0]      # beyond r_escape
+    ks[4, 2] = np.nan                    # non-finite momentum
+    ks[0:3, 3] = [0.0, 0.0, 5.0]         # ON the polar axis
+    kw = dict(r_capture=1.5, r_escape=100.0, snapshot_every=5)
+    o = ks_oracle.integrate(1.0, a, ks, 0.01, 20, **kw)
+    g = run_gpu(G, G.KERR_SCHILD, a, ks, 0.01, 20, **kw)
+    assert np.array_equal(g["status"], o["status"]) and np.array_equal(g["steps_done"], o["steps_done"])
+    assert g["status"][0] == G.ST_CAPTURED and g["status"][1] == G.ST_ESCAPED and g["status"][2] == G.ST_NUMERIC
+    assert g["status"][3] == G.ST_MAXSTEPS and np.isfinite(g["final_state"][:, 3]).all()
+    assert np.array_equal(g["snap_count"], o["snap_count"]) and g["snap_count"][0] == 0 and g["snap_count"][1] == 1
+    ok = np.ones(40, bool)
+    ok[2] = False
+    assert parity.rel_err(g["final_state"], o["final_state"])[:, ok].max() <= 1e-12
+    # backwards in tau, disabled stop radii, nsteps = 0
+    for h, ns in ((-0.01, 300), (0.01, 0)):
+        o = ks_oracle.integrate(1.0, a, ks[:, 4:], h, ns)
+        g = run_gpu(G, G.KERR_SCHILD, a, ks[:, 4:], h, ns)
+        c = parity.compare(g, o)
+        assert c["same_class"].all() and c["err"].max() <= 1e-10
+    # n = 0; unsupported flags; the adaptive and allocation-free entry points refuse this metric
+    ctx = G.geo_create(G.KERR_SCHILD, 1.0, a)
+    try:
+        d_in = torch.empty((6, 0), dtype=torch.float64, device="cuda:0")
+        G.geo_integrate(ctx, d_in, 0.01, 10, G.alloc_outputs(0, d_in.device))
+        d_in = torch.from_numpy(ks).to("cuda:0")
+        out = G.alloc_outputs(40, d_in.device, 20, 5)
+        for bad in (G.FLAG_CARTESIAN_SNAP, G.FLAG_STAGED_SNAP, G.FLAG_TAB_GATHER):
+            with pytest.raises(Exception):
+                G.geo_integrate(ctx, d_in, 0.01, 20, out, flags=bad, snapshot_every=5)
+        with pytest.raises(Exception):
+            G.geo_integrate_adaptive(ctx, d_in, 0.01, 1e-9, 1e-9, 1000, G.alloc_outputs(40, d_in.device))
+        assert G.geo_horizon_radius(ctx) == pytest.approx(1.0 + math.sqrt(1.0 - a * a))
+    finally:
+        G.geo_destroy(ctx)
+    with pytest.raises(Exception):
+        G.geo_create(G.KERR_SCHILD, 1.0, 1.5)

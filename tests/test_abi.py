@@ -51,7 +51,8 @@ def test_sass_has_fp64_pipe_and_wide_stores():
 def test_every_direct_snapshot_kernel_keeps_its_256_bit_stores():
     """ptxas narrowed `st.global.v4.f64` to STG.E.64 in ONE clone of a non-inlined record writer (DESIGN.md section 5,
     profiles/r02_noinline_writer_miscompile.md): the shipped library must have 256-bit stores in every instantiation of the
-    direct snapshot writer -- Kerr and Schwarzschild, Kahan and plain update, and the dense-output RK5(4) kernels."""
+    direct snapshot writer -- Kerr and Schwarzschild, Kahan and plain update, the dense-output RK5(4) kernels, the tabulated
+    and the Kerr-Schild kernels."""
     import sys
     sys.path.insert(0, ROOT)
     import bench
@@ -68,8 +69,8 @@ def test_every_direct_snapshot_kernel_keeps_its_256_bit_stores():
         elif name and re.search(r"STG\.E(\.\w+)*\.256", line):
             kernels[name] += 1
     want = [k for k in kernels if re.search(r"geo_rk4_kernelILb[01]ELi1ELb[01]E", k) or re.search(r"geo_rk45_kernelILi[012]ELb1E", k)
-            or re.search(r"geo_tabg?_rk4_kernelILb[01]ELb[01]ELb1E", k)]
-    assert len(want) == 4 + 3 + 4 + 4, want
+            or re.search(r"geo_tabg?_rk4_kernelILb[01]ELb[01]ELb1E", k) or re.search(r"geo_ks_rk4_kernelILi1ELb[01]E", k)]
+    assert len(want) == 4 + 3 + 4 + 4 + 2, want
     for k in want:
         assert kernels[k] >= 2, (k, kernels[k])
 
@@ -77,7 +78,7 @@ def test_every_direct_snapshot_kernel_keeps_its_256_bit_stores():
 def test_product_path_does_not_import_the_oracle():
     """No file of the package imports, loads, includes or executes anything under oracle/."""
     pkg = os.path.join(ROOT, "paper_1803_08320_b200")
-    bad = re.compile(r"import\s+geo_oracle|from\s+oracle|import\s+oracle|libgeo_oracle|#include\s*[\"<].*oracle|oracle_integrate\s*\(")
+    bad = re.compile(r"import\s+geo_(ks_|tab_)?oracle|from\s+oracle|import\s+oracle|libgeo_oracle|#include\s*[\"<].*oracle|oracle_(ks_)?integrate\s*\(")
     for dirpath, _, files in os.walk(pkg):
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):

@@ -222,3 +222,34 @@ def test_tabulated_kernel_writes_inside_its_buffers(G, flags):
         assert len(np.unique(p["status"])) >= 2
     finally:
         G.geo_destroy(ctx)
+
+
+@pytest.mark.parametrize("flags,mask,cap,snap_pad", [(0, 0xFF, None, 64), (0, 0xFF, None, 62), (1, 0x0F, 5, 64), (2, 0x07, 5, 62)])
+def test_kerr_schild_kernels_write_inside_their_buffers(G, flags, mask, cap, snap_pad):
+    """geo_ks_rk4_kernel (Cartesian Kerr-Schild coordinates): input, final records, status, steps, event radius, health,
+    trajectory records (256-bit stores on 32-B slots, the 8-B fallback on 16-B slots and odd masks, capacity overflow) and
+    record counter between canaries, on a ragged batch of photons with mixed termination classes; queue and static map."""
+    import torch
+    a = 0.998
+    bl = mixed_rays(a)
+    st = W.to_cartesian_kerr_schild(bl, np.ones(bl.shape[1]), 1.0, a)
+    n = st.shape[1]
+    dev = torch.device("cuda:0")
+    kw = dict(r_capture=1.0 + math.sqrt(1.0 - a * a) + 0.01, r_escape=33.0, kind=G.NULL, flags=flags, snapshot_every=50)
+    ctx = G.geo_create(G.KERR_SCHILD, 1.0, a)
+    try:
+        d_in = torch.from_numpy(st).to(dev)
+        plain = G.alloc_outputs(n, dev, 1500, 50, cap, mask)
+        G.geo_integrate(ctx, d_in, 0.05, 1500, plain, **kw)
+        gd = Guarded()
+        g_in = gd.wrap(d_in)
+        guarded = guard_outputs(G.alloc_outputs(n, dev, 1500, 50, cap, mask), gd, snap_pad)
+        G.geo_integrate(ctx, g_in, 0.05, 1500, guarded, **kw)
+        torch.cuda.synchronize()
+        gd.check()
+        assert np.array_equal(bits(g_in.cpu().numpy()), bits(st))
+        p, g = G.to_numpy(plain), G.to_numpy(guarded)
+        same_bits(p, g)
+        assert len(np.unique(p["status"])) >= 2
+    finally:
+        G.geo_destroy(ctx)

@@ -148,29 +148,33 @@ def test_camera_rays_parity_incl_axis_columns(G, ks_oracle, oracle):
                   "wrong class there:", int(((ob["status"] == oracle.ST_ESCAPED) != esc).sum()))
 
 
-def test_whole_config3_image_has_no_wrong_pixel(G):
-    """The whole 1024^2 image of configs[2] in ONE call on the Kerr-Schild path (work queue on), every pixel against the
-    closed-form capture / escape criterion.  The 10 polar-axis columns, where the Boyer-Lindquist path has its 533 wrong
-    pixels and |2H| up to 1e47 (reading B7), come out right: 0 mismatches, |2H| < 1e-8.  What this chart pays: next to the
-    prograde photon orbit of a = 0.998 (r = 1.074 M, 0.01 M outside the horizon) the Cartesian components turn by ~0.75 rad per
-    step of h = 0.02 M, and <= 64 pixels (measured: 42; 10 at h = 0.01) within 3 px of the prograde edge of the shadow are
-    captured instead of escaping -- on the GPU and in the oracle alike.  No ray at the step cap."""
+def test_whole_config3_image_closed_form_and_oracle_at_a_resolution_that_can_fail(G, ks_oracle):
+    """The whole 1024^2 image of configs[2] in ONE call on the Kerr-Schild path (work queue on).
+    (1) Every pixel against the closed-form capture / escape criterion.  The 10 polar-axis columns, where the
+    Boyer-Lindquist path has its 533 wrong pixels and |2H| up to 1e47 (reading B7), come out right: 0 mismatches, |2H| < 1e-8.
+    What this chart pays: next to the prograde photon orbit of a = 0.998 (r = 1.074 M, 0.01 M outside the horizon) the
+    Cartesian components turn by ~0.75 rad per step of h = 0.02 M, and <= 64 pixels (measured: 42; 10 at h = 0.01) within
+    3 px of the prograde edge of the shadow are captured instead of escaping -- on the GPU and in the oracle alike
+    (DESIGN.md section 8.5).  No ray at the step cap.
+    (2) Against the oracle, the north_star's null-ray rule where it can fail (reading P3): 6000 uniformly sampled pixels,
+    EVERY pixel within +-3 px of the analytic critical curve, EVERY pixel of the axis columns -- class (status AND
+    steps_done) identical on >= 99.99 %, 1e-8 on every certified ray, the others counted and printed."""
     import torch
     a, N = 0.998, 1024
     rp = W.horizon_radius(1.0, a)
     st, consts = W.camera_rays(N, a, 60.0, return_constants=True)
     ks = W.to_cartesian_kerr_schild(st, np.ones(N * N), 1.0, a)
     dev = torch.device("cuda:0")
+    kw = dict(r_capture=rp + 0.01, r_escape=1100.0)
     ctx = G.geo_create(G.KERR_SCHILD, 1.0, a)
     try:
         out = G.alloc_outputs(N * N, dev)
-        G.geo_integrate(ctx, torch.from_numpy(ks).to(dev), 0.02, 200000, out, r_capture=rp + 0.01, r_escape=1100.0, kind=G.NULL)
+        G.geo_integrate(ctx, torch.from_numpy(ks).to(dev), 0.02, 200000, out, kind=G.NULL, **kw)
         torch.cuda.synchronize()
-        status = out["status"].cpu().numpy()
-        health = out["health"].cpu().numpy()
-        steps = out["steps_done"].cpu().numpy()
+        g_all = G.to_numpy(out)
     finally:
         G.geo_destroy(ctx)
+    status, health, steps = g_all["status"], g_all["health"], g_all["steps_done"]
     esc = _escapes_analytic(a, consts[2], consts[3], rp, 1000.0)
     wrong = (status == G.ST_ESCAPED) != esc
     counts = np.bincount(status, minlength=4)
@@ -187,6 +191,64 @@ def test_whole_config3_image_has_no_wrong_pixel(G):
     assert np.all(consts[2][wrong] > 1.9)
     escaped = status == G.ST_ESCAPED
     assert health[escaped & axis].max() < 1e-8 and np.median(health[escaped]) < 1e-13
+    # (2) the oracle
+    rest = np.flatnonzero(~band & ~axis)
+    rng = np.random.default_rng(47)
+    sets = {"uniform": np.sort(rng.choice(rest, 6000, replace=False)), "band": np.flatnonzero(band & ~axis), "axis": np.flatnonzero(axis)}
+    print({k: len(v) for k, v in sets.items()})
+    assert len(sets["band"]) > 5000 and len(sets["axis"]) == 10 * N
+
+    def orc(ii, **extra):
+        sub = np.ascontiguousarray(ks[:, ii])
+        if extra.pop("nudge", False):
+            sub = parity.ulp_nudged(sub)
+        return ks_oracle.integrate(1.0, a, sub, 0.02, 200000, kind=ks_oracle.NULL, nthreads=NCPU, **kw, **extra)
+    mism = {}
+    for name, ii in sets.items():
+        o = orc(ii)
+        g = parity.take(g_all, ii)
+        rep = parity.p3_report(g, o, lambda jj: [orc(ii[jj], long_double=True), orc(ii[jj], nudge=True)], 1e-8,
+                               labels=consts[:, ii], max_fail_frac=0.03, what=f"Kerr-Schild image, {name}")
+        print(name, rep)
+        mism[name] = rep["class_mismatch"]
+    assert mism["uniform"] == 0
+    est = mism["band"] + mism["axis"] + mism["uniform"] * len(rest) / 6000.0
+    print(f"class mismatches: band {mism['band']}, axis {mism['axis']}, uniform {mism['uniform']} -> image-level estimate {est:.0f} of {N * N}")
+    assert est <= 1e-4 * N * N
+
+
+def test_ks4_full_2p22_sampled(G, ks_oracle):
+    """The bench workload `ks4` at FULL size in the launch configuration bench.py times (2^22 config-4 particles in Cartesian
+    Kerr-Schild coordinates x 2500 steps, persistent grid, queue on): 20 000 sampled particles against the oracle at 1e-9;
+    over the whole batch every particle ends with MAXSTEPS after 2500 steps, E bit-equal to the zero-step run's, |2H + 1| small."""
+    import torch
+    a, n = 0.5, 1 << 22
+    st, consts = W.kerr_bound(n, a, W.SEED_BASE + 4, nthreads=NCPU, chunk=1 << 20, return_constants=True)
+    ks = W.to_cartesian_kerr_schild(st, consts[0], 1.0, a)
+    dev = torch.device("cuda:0")
+    ctx = G.geo_create(G.KERR_SCHILD, 1.0, a)
+    try:
+        out = G.alloc_outputs(n, dev)
+        G.geo_integrate(ctx, torch.from_numpy(ks).to(dev), 0.01, 2500, out)
+        torch.cuda.synchronize()
+        assert bool((out["status"] == G.ST_MAXSTEPS).all()) and bool((out["steps_done"] == 2500).all())
+        assert float(out["health"].max()) < 1e-9
+        g_all = G.to_numpy(out)
+    finally:
+        G.geo_destroy(ctx)
+    f = g_all["final_state"]
+    assert np.max(np.abs(f[4] - consts[0]) / consts[0]) < 1e-13                      # E: constant, = the Boyer-Lindquist E
+    assert np.max(np.abs(f[1] * f[6] - f[2] * f[5] - consts[1])) < 1e-8              # L_z conserved by the dynamics, O(h^4)
+    rng = np.random.default_rng(53)
+    ii = np.unique(np.concatenate([[0, 1, n - 2, n - 1], rng.integers(0, n, size=20000)])).astype(np.int64)
+    sub = np.ascontiguousarray(ks[:, ii])
+    o = ks_oracle.integrate(1.0, a, sub, 0.01, 2500, nthreads=NCPU)
+    rep = parity.p3_report(parity.take(g_all, ii), o,
+                           lambda jj: [ks_oracle.integrate(1.0, a, np.ascontiguousarray(sub[:, jj]), 0.01, 2500, long_double=True),
+                                       ks_oracle.integrate(1.0, a, parity.ulp_nudged(np.ascontiguousarray(sub[:, jj])), 0.01, 2500)],
+                           1e-9, labels=consts[:, ii], max_fail_frac=0.001, what="ks4 sampled")
+    print(f"ks4: {len(ii)} sampled particles vs oracle: {rep}")
+    assert rep["class_mismatch"] == 0 and len(ii) > 19000
 
 
 def test_through_the_polar_axis_and_through_the_horizon(G, ks_oracle):

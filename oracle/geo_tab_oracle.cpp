@@ -306,7 +306,9 @@ void integrate_range(const Table& m, const double* state_in, int64_t n, double h
 
 
 // ---------------------------------------------------------------------------------------------------------------
-// T7 (round 2): the adaptive Dormand-Prince 5(4) stepper of readings A1-A3 on the five-field tabulated metric.
+// T7 (round 2): the adaptive Dormand-Prince 5(4) stepper of readings A1-A3 on a tabulated metric -- five fields (MP = Metric5:
+// the T3 right-hand side) or all ten (MP = Metric10: the T6 right-hand side); the policy only names which interpolate / rhs /
+// energy / hamiltonian routines of this file are called.
 // The loop of geo_oracle.cpp: integrate_one_adaptive with r -> x^1, theta -> x^2 and the T3 right-hand side; in addition
 // every evaluation point (y0, the six stage points, the end point) is tested against the table's domain (T4): per point
 // the capture test comes first, then the domain test; the first event in evaluation order ends the particle
@@ -323,7 +325,7 @@ template <class R> void tset6(State<R>& y, int c, R v) {
                  case 4: y.p1 = v; break; default: y.p2 = v; }
 }
 
-template <class R>
+template <class R, class MP>
 void integrate_one_adaptive_tab(const Table& m, const double* state_in, int64_t n, int64_t i, const AdaptiveCtl& ctl,
                                 int64_t max_attempts, const StopRule& st, const OutPtrs& o, int64_t* rejected_out) {
     static const DP45 T;
@@ -349,7 +351,7 @@ void integrate_one_adaptive_tab(const Table& m, const double* state_in, int64_t 
     int64_t steps = 0, attempts = 0, rejected = 0;
     R eq_cross = std::numeric_limits<R>::quiet_NaN();
     bool crossed = false;
-    Fields<R> F;
+    typename MP::F F;
     auto record = [&](const State<R>& ys) {
         const R comp[8] = {ys.t, ys.x1, ys.x2, ys.ph, ys.E, ys.p1, ys.p2, ys.L};
         write_record<R>(o, i, next_j, comp);
@@ -357,9 +359,9 @@ void integrate_one_adaptive_tab(const Table& m, const double* state_in, int64_t 
     };
     if (!(y.x1 >= rc)) status = TAB_ST_CAPTURED;                     // B1 + T4 on y0
     else if (!finite6(y) || !std::isfinite(y.L)) status = TAB_ST_NUMERIC;
-    else if (!interpolate(m, y.x1, y.x2, F)) status = TAB_ST_OUTSIDE;
+    else if (!MP::interp(m, y.x1, y.x2, F)) status = TAB_ST_OUTSIDE;
     else {
-        y.E = energy_fields(F, y.p1, y.p2, y.L, kappa);
+        y.E = MP::energy(F, y.p1, y.p2, y.L, kappa);
         if (!std::isfinite(y.E)) status = TAB_ST_NUMERIC;
         else {
             if (dense) record(y);
@@ -368,7 +370,7 @@ void integrate_one_adaptive_tab(const Table& m, const double* state_in, int64_t 
         }
     }
     Deriv<R> k[DP45::S];
-    if (status < 0) k[0] = rhs_fields(F, y);
+    if (status < 0) k[0] = MP::rhs(F, y);
     while (status < 0) {
         const bool last = tau + R(1.01) * h >= tau_end;
         if (last) h = tau_end - tau;
@@ -380,10 +382,10 @@ void integrate_one_adaptive_tab(const Table& m, const double* state_in, int64_t 
                 for (int j = 0; j < s; ++j) acc += (R)T.a[s][j] * tdcomp6(k[j], c);
                 tset6(ys, c, tcomp6(y, c) + h * acc);
             }
-            Fields<R> G;
+            typename MP::F G;
             if (!(ys.x1 >= rc)) ev = TAB_ST_CAPTURED;
-            else if (!interpolate(m, ys.x1, ys.x2, G)) ev = TAB_ST_OUTSIDE;
-            else k[s] = rhs_fields(G, ys);
+            else if (!MP::interp(m, ys.x1, ys.x2, G)) ev = TAB_ST_OUTSIDE;
+            else k[s] = MP::rhs(G, ys);
         }
         ++attempts;
         if (ev) { status = ev; break; }
@@ -399,11 +401,11 @@ void integrate_one_adaptive_tab(const Table& m, const double* state_in, int64_t 
         }
         if (!(yn.x1 >= rc)) { status = TAB_ST_CAPTURED; break; }     // end point: capture, then finiteness, then domain
         const bool fin = finite6(yn);
-        Fields<R> Gn;
-        if (fin && !interpolate(m, yn.x1, yn.x2, Gn)) { status = TAB_ST_OUTSIDE; break; }
+        typename MP::F Gn;
+        if (fin && !MP::interp(m, yn.x1, yn.x2, Gn)) { status = TAB_ST_OUTSIDE; break; }
         R err = R(0);
         if (fin) {
-            k[6] = rhs_fields(Gn, yn);
+            k[6] = MP::rhs(Gn, yn);
             for (int c = 0; c < 6; ++c) {
                 R acce = R(0);
                 for (int j = 0; j < DP45::S; ++j)
@@ -464,9 +466,9 @@ void integrate_one_adaptive_tab(const Table& m, const double* state_in, int64_t 
     o.steps_done[i] = steps;
     if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
     if (o.health) {
-        Fields<R> H;
-        o.health[i] = (std::isfinite(y.E) && interpolate(m, y.x1, y.x2, H))
-                          ? (double)std::fabs(R(2) * hamiltonian_fields(H, y) + kappa)
+        typename MP::F H;
+        o.health[i] = (std::isfinite(y.E) && MP::interp(m, y.x1, y.x2, H))
+                          ? (double)std::fabs(R(2) * MP::hamiltonian(H, y) + kappa)
                           : std::numeric_limits<double>::quiet_NaN();
     }
     if (dense && o.snap_count) o.snap_count[i] = (int32_t)next_j;
@@ -659,6 +661,22 @@ void integrate_range_general(const Table& m, const double* state_in, int64_t n, 
     for (int64_t i = lo; i < hi; ++i) integrate_one_general<R>(m, state_in, n, i, (R)h, nsteps, st, o, snapshot_every);
 }
 
+// the two metric policies of integrate_one_adaptive_tab
+template <class R> struct Metric5 {
+    typedef Fields<R> F;
+    static bool interp(const Table& m, R x1, R x2, F& f) { return interpolate(m, x1, x2, f); }
+    static Deriv<R> rhs(const F& f, const State<R>& y) { return rhs_fields(f, y); }
+    static R energy(const F& f, R p1, R p2, R L, R kappa) { return energy_fields(f, p1, p2, L, kappa); }
+    static R hamiltonian(const F& f, const State<R>& y) { return hamiltonian_fields(f, y); }
+};
+template <class R> struct Metric10 {
+    typedef GFields<R> F;
+    static bool interp(const Table& m, R x1, R x2, F& f) { return interpolate_general(m, x1, x2, f); }
+    static Deriv<R> rhs(const F& f, const State<R>& y) { return rhs_general(f, y); }
+    static R energy(const F& f, R p1, R p2, R L, R kappa) { return energy_general(f, p1, p2, L, kappa); }
+    static R hamiltonian(const F& f, const State<R>& y) { return hamiltonian_general(f, y); }
+};
+
 }  // namespace
 
 extern "C" {
@@ -745,8 +763,8 @@ int oracle_tabg_rhs(const double* tab, int64_t n1, int64_t n2, double x1_0, doub
     return 1;
 }
 
-// ---- T7: adaptive RK5(4) on a five-field table ----
-int oracle_tab_integrate_adaptive(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+// ---- T7: adaptive RK5(4) on a five-field table (general = 0) or a ten-field table (general = 1) ----
+static int tab_integrate_adaptive(int general, const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
                                   const double* state_in, int64_t n, const AdaptiveCtl* ctl, int64_t max_attempts,
                                   const StopRule* st, const OutPtrs* out, int64_t* rejected, int precision, int nthreads) {
     if (!tab || n1 < 4 || n2 < 4 || !(d1 > 0) || !(d2 > 0) || n < 0 || max_attempts < 0 || !st || !out || !ctl) return 1;
@@ -761,12 +779,30 @@ int oracle_tab_integrate_adaptive(const double* tab, int64_t n1, int64_t n2, dou
         pool.emplace_back([&, t]() {
             for (int64_t b = t; b < nblocks; b += nthreads)
                 for (int64_t i = b * block; i < std::min<int64_t>(n, (b + 1) * block); ++i) {
-                    if (precision == 1) integrate_one_adaptive_tab<long double>(m, state_in, n, i, *ctl, max_attempts, *st, *out, rejected);
-                    else integrate_one_adaptive_tab<double>(m, state_in, n, i, *ctl, max_attempts, *st, *out, rejected);
+                    if (general) {
+                        if (precision == 1) integrate_one_adaptive_tab<long double, Metric10<long double>>(m, state_in, n, i, *ctl, max_attempts, *st, *out, rejected);
+                        else integrate_one_adaptive_tab<double, Metric10<double>>(m, state_in, n, i, *ctl, max_attempts, *st, *out, rejected);
+                    } else {
+                        if (precision == 1) integrate_one_adaptive_tab<long double, Metric5<long double>>(m, state_in, n, i, *ctl, max_attempts, *st, *out, rejected);
+                        else integrate_one_adaptive_tab<double, Metric5<double>>(m, state_in, n, i, *ctl, max_attempts, *st, *out, rejected);
+                    }
                 }
         });
     for (auto& th : pool) th.join();
     return 0;
+}
+
+int oracle_tab_integrate_adaptive(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+                                  const double* state_in, int64_t n, const AdaptiveCtl* ctl, int64_t max_attempts,
+                                  const StopRule* st, const OutPtrs* out, int64_t* rejected, int precision, int nthreads) {
+    return tab_integrate_adaptive(0, tab, n1, n2, x1_0, d1, x2_0, d2, state_in, n, ctl, max_attempts, st, out, rejected, precision, nthreads);
+}
+
+// tab = [10][n2][n1] (reading T6)
+int oracle_tabg_integrate_adaptive(const double* tab, int64_t n1, int64_t n2, double x1_0, double d1, double x2_0, double d2,
+                                   const double* state_in, int64_t n, const AdaptiveCtl* ctl, int64_t max_attempts,
+                                   const StopRule* st, const OutPtrs* out, int64_t* rejected, int precision, int nthreads) {
+    return tab_integrate_adaptive(1, tab, n1, n2, x1_0, d1, x2_0, d2, state_in, n, ctl, max_attempts, st, out, rejected, precision, nthreads);
 }
 
 }  // extern "C"

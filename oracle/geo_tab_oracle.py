@@ -144,8 +144,9 @@ class _Ctl(C.Structure):
 def integrate_adaptive(table: dict, state_in: np.ndarray, h0: float, rtol: float, atol: float, max_attempts: int,
                        r_capture: float = -np.inf, r_escape: float = np.inf, kind: int = TIMELIKE, h_min: float = 1e-12,
                        tau_end: float = np.inf, long_double: bool = False, nthreads: int = 1, snap_dtau: float = 0.0,
-                       snap_capacity: int = 0, snap_mask: int = 0xFF) -> dict:
-    """Adaptive Dormand-Prince RK5(4) (readings A1-A3) through the five-field tabulated metric (reading T7)."""
+                       snap_capacity: int = 0, snap_mask: int = 0xFF, general: bool = False) -> dict:
+    """Adaptive Dormand-Prince RK5(4) (readings A1-A3) through the five-field tabulated metric (reading T7), or with
+    general=True through a ten-field table (reading T6)."""
     st = np.ascontiguousarray(state_in, dtype=np.float64)
     n = st.shape[1]
     res = {"final_state": np.full((8, n), np.nan), "status": np.full(n, -1, dtype=np.int32),
@@ -161,11 +162,18 @@ def integrate_adaptive(table: dict, state_in: np.ndarray, h0: float, rtol: float
                res["snap_count"].ctypes.data if snap_dtau > 0 else None)
     ctl = _Ctl(h0, rtol, atol, h_min, tau_end, snap_dtau)
     L = lib()
-    L.oracle_tab_integrate_adaptive.restype = C.c_int
-    L.oracle_tab_integrate_adaptive.argtypes = _GRID + [C.c_void_p, C.c_int64, C.POINTER(_Ctl), C.c_int64, C.POINTER(_Stop),
-                                                        C.POINTER(_Out), C.c_void_p, C.c_int, C.c_int]
-    rc = L.oracle_tab_integrate_adaptive(*_grid(table), st.ctypes.data, n, C.byref(ctl), max_attempts, C.byref(stop),
-                                         C.byref(out), res["rejected"].ctypes.data, int(long_double), nthreads)
+    fn = L.oracle_tabg_integrate_adaptive if general else L.oracle_tab_integrate_adaptive
+    fn.restype = C.c_int
+    fn.argtypes = _GRID + [C.c_void_p, C.c_int64, C.POINTER(_Ctl), C.c_int64, C.POINTER(_Stop),
+                           C.POINTER(_Out), C.c_void_p, C.c_int, C.c_int]
+    rc = fn(*_grid(table, 10 if general else 5), st.ctypes.data, n, C.byref(ctl), max_attempts, C.byref(stop),
+            C.byref(out), res["rejected"].ctypes.data, int(long_double), nthreads)
     if rc != 0:
         raise ValueError("oracle_tab_integrate_adaptive: invalid arguments")
     return res
+
+
+def integrate_adaptive_general(table: dict, state_in: np.ndarray, h0: float, rtol: float, atol: float, max_attempts: int,
+                               **kw) -> dict:
+    """Adaptive RK5(4) through a GENERAL ten-field table (readings T6 + T7)."""
+    return integrate_adaptive(table, state_in, h0, rtol, atol, max_attempts, general=True, **kw)

@@ -176,8 +176,9 @@ int geo_integrate_adaptive_host(geo_ctx *ctx, const double *state_in, int64_t n,
  * evaluation point the capture test comes first).  Trajectory records (snapshot_every > 0) as for the analytic metrics,
  * components (t, x^1, x^2, phi, p_t = E, p_1, p_2, p_phi) by snap_mask; flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER
  * (no staged writer, no Cartesian records: the coordinates are the table's own).
- * geo_integrate_adaptive / geo_integrate_adaptive_host accept such a ctx too (reading T7: the domain test joins
- * the capture test on every stage point and the end point; flags must be 0); geo_horizon_radius returns NaN.
+ * geo_integrate_adaptive / geo_integrate_adaptive_host accept such a ctx too -- and one made by geo_create_tabulated_general
+ * (reading T7: the domain test joins the capture test on every stage point and the end point; flags must be 0);
+ * geo_horizon_radius returns NaN.
  * Errors: GEO_EINVAL (NULL, n1 or n2 < 4, d1 or d2 <= 0, non-finite grid), GEO_ENOMEM, GEO_ECUDA. */
 typedef struct geo_table {
     const double *tab;  /* HOST [5][n2][n1] (geo_create_tabulated) or [10][n2][n1] (geo_create_tabulated_general) */
@@ -195,8 +196,8 @@ int geo_create_tabulated(geo_ctx **ctx, const geo_table *table);
  *     H = 1/2 [ -(p_t - beta^k p_k)^2/alpha^2 + gamma^{ij} p_i p_j ],   gamma^{ij} = inverse of gamma_ij (3 x 3, per evaluation),
  * p_t and p_phi constants of motion.  Use with geo_integrate / geo_integrate_host exactly like a geo_create_tabulated
  * ctx (state_in = (x^1, x^2, phi, p_1, p_2, p_phi); GEO_ST_OUTSIDE; trajectory records by snap_mask over
- * (t, x^1, x^2, phi, E, p_1, p_2, p_phi); flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER; geo_integrate_adaptive
- * returns GEO_EINVAL). */
+ * (t, x^1, x^2, phi, E, p_1, p_2, p_phi); flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_TAB_GATHER), and with
+ * geo_integrate_adaptive / geo_integrate_adaptive_host (reading T7 with the T6 right-hand side, dense output included). */
 int geo_create_tabulated_general(geo_ctx **ctx, const geo_table *table);
 
 /* ALLOCATION-FREE entry point, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving

@@ -727,9 +727,9 @@ static int validate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, co
                              const geo_stop* stop, const geo_out* out, const int32_t* rejected, bool check_align) {
     int rc = validate(ctx, state_in, n, 1.0, 0, stop, 0, out, check_align);
     if (rc != GEO_OK) return rc;
-    if (ctx->metric == GEO_TABULATED_GENERAL || ctx->metric == GEO_KERR_SCHILD)
-        return fail(ctx, GEO_EINVAL, "the adaptive path takes the Boyer-Lindquist metrics and five-field tables only");
-    if (ctx->metric == GEO_TABULATED && stop && stop->flags != 0) return fail(ctx, GEO_EINVAL, "tabulated metrics: the adaptive path takes no flags");
+    if (ctx->metric == GEO_KERR_SCHILD)
+        return fail(ctx, GEO_EINVAL, "the adaptive path takes the Boyer-Lindquist metrics and tabulated metrics only");
+    if ((ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) && stop && stop->flags != 0) return fail(ctx, GEO_EINVAL, "tabulated metrics: the adaptive path takes no flags");
     if (!ctl) return fail(ctx, GEO_EINVAL, "ctl must not be NULL");
     if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0)) return fail(ctx, GEO_EINVAL, "h0 must be finite and > 0");
     if (!(ctl->rtol >= 0.0) || !(ctl->atol >= 0.0) || !(ctl->rtol + ctl->atol > 0.0) || std::isinf(ctl->atol))
@@ -787,9 +787,11 @@ static int launch_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, cons
     p.bh.twoMa = 2.0 * ctx->M * ctx->a;
     fill_trig_consts(p.bh.tc);
     p.tm = ctx->tm;
+    p.tgm = ctx->tgm;
     typedef void (*fn_t)(const AdaptiveParams);
     fn_t fn = ctx->metric == GEO_KERR ? (dense ? (fn_t)geo_rk45_kernel<METRIC_KERR, true> : (fn_t)geo_rk45_kernel<METRIC_KERR, false>)
             : ctx->metric == GEO_TABULATED ? (dense ? (fn_t)geo_rk45_kernel<METRIC_TAB, true> : (fn_t)geo_rk45_kernel<METRIC_TAB, false>)
+            : ctx->metric == GEO_TABULATED_GENERAL ? (dense ? (fn_t)geo_rk45_kernel<METRIC_TABG, true> : (fn_t)geo_rk45_kernel<METRIC_TABG, false>)
                                            : (dense ? (fn_t)geo_rk45_kernel<METRIC_SCHW, true> : (fn_t)geo_rk45_kernel<METRIC_SCHW, false>);
     int per_sm = 0;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, 0);

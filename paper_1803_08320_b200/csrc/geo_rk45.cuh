@@ -15,6 +15,7 @@
 #pragma once
 #include "geo_kernel.cuh"
 #include "geo_tab.cuh"
+#include "geo_tabg.cuh"
 #ifndef GEO_RK45_CTAS
 #define GEO_RK45_CTAS 3      // resident CTAs per SM the kernel is compiled for (168 registers, no spills)
 #endif
@@ -45,9 +46,11 @@ struct AdaptiveParams {
     int* snap_count;
     Hole bh;
     TabMetric tm;       // METRIC_TAB: the five-field table (reading T7)
+    TabgMetric tgm;     // METRIC_TABG: the ten-field table (readings T6 + T7)
 };
 
-enum { METRIC_SCHW = 0, METRIC_KERR = 1, METRIC_TAB = 2 };
+enum { METRIC_SCHW = 0, METRIC_KERR = 1, METRIC_TAB = 2, METRIC_TABG = 3 };
+__host__ __device__ constexpr bool metric_is_tab(int m) { return m == METRIC_TAB || m == METRIC_TABG; }
 
 // Butcher tableau (Dormand & Prince 1980, table 2).  e = b5 - b4.
 namespace dp {
@@ -110,10 +113,22 @@ __device__ __noinline__ bool tab_eval(const TabMetric& m, double x1, double x2, 
     return in;
 }
 
+// T6 + T7: the same for the ten-field table (gathered stencil; the per-lane stencil cache of geo_tabg_rk4_kernel is not used
+// here: an adaptive step moves across cells).
+__device__ __noinline__ bool tabg_eval(const TabgMetric& m, double x1, double x2, double p1, double p2, double E, double L, Deriv* d) {
+    TabgFields F;
+    const bool in = tabg_fields(m, x1, x2, F);
+    TabDeriv td;
+    tabg_rhs(F, p1, p2, E, L, td);
+    d->t = td.t; d->r = td.x1; d->th = td.x2; d->ph = td.ph; d->pr = td.p1; d->pth = td.p2;
+    return in;
+}
+
 // right-hand side of the selected metric at one evaluation point; false: outside the domain (tabulated metric only)
 template <int METRIC>
 __device__ __forceinline__ bool rhs_metric(const AdaptiveParams& p, double r, double th, double pr, double pth, double E, double L, Deriv& d) {
     if (METRIC == METRIC_TAB) return tab_eval(p.tm, r, th, pr, pth, E, L, &d);
+    if (METRIC == METRIC_TABG) return tabg_eval(p.tgm, r, th, pr, pth, E, L, &d);
     rhs_at<METRIC == METRIC_KERR>(p.bh, r, th, pr, pth, E, L, d);
     return true;
 }
@@ -129,7 +144,8 @@ __device__ __forceinline__ double contd5(double theta, double y, double ynew, do
 // DENSE: dense-output records (geo_adaptive.snap_dtau > 0); a separate instantiation so that the plain kernel keeps its
 // register budget.
 template <int METRIC, bool DENSE>
-__global__ void __launch_bounds__(kBlock, (DENSE || METRIC == METRIC_TAB) ? 2 : GEO_RK45_CTAS) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
+__global__ void __launch_bounds__(kBlock, (DENSE || metric_is_tab(METRIC)) ? 2 : GEO_RK45_CTAS) geo_rk45_kernel(const __grid_constant__ AdaptiveParams p) {
+    constexpr bool kTab = metric_is_tab(METRIC);      // a tabulated metric: domain tests (T4, T7), E undefined until y0 is inside
     const unsigned lane = threadIdx.x & 31u;
     const Hole& bh = p.bh;
     long long idx = -1;
@@ -169,7 +185,15 @@ __global__ void __launch_bounds__(kBlock, (DENSE || METRIC == METRIC_TAB) ? 2 : 
         p.steps_done[idx] = (long long)steps;
         if (p.eq_cross_r) p.eq_cross_r[idx] = crossed ? eqc : __longlong_as_double(0x7ff8000000000000LL);
         if (p.health) {
-            if (METRIC == METRIC_TAB) {
+            if (METRIC == METRIC_TABG) {
+                TabgFields F;
+                double hv = __longlong_as_double(0x7ff8000000000000LL);
+                if (tabg_fields_cold(p.tgm, r, th, F) && (__double2hiint(E) & 0x7ff00000) != 0x7ff00000) {
+                    const TabgAux A = tabg_aux(F.v, pr, pth, L, E);
+                    hv = fabs(-(A.W * A.W) / (F.v[0] * F.v[0]) + A.gpp + p.kappa);
+                }
+                p.health[idx] = hv;
+            } else if (METRIC == METRIC_TAB) {
                 TabFields F;
                 double hv = __longlong_as_double(0x7ff8000000000000LL);
                 if (tab_fields_cold(p.tm, r, th, F) && (__double2hiint(E) & 0x7ff00000) != 0x7ff00000) {
@@ -196,7 +220,12 @@ __global__ void __launch_bounds__(kBlock, (DENSE || METRIC == METRIC_TAB) ? 2 : 
         pth = p.in[4 * n + i];
         L = p.in[5 * n + i];
         bool y0_inside = true;
-        if (METRIC == METRIC_TAB) {
+        if (METRIC == METRIC_TABG) {
+            TabgFields F;
+            y0_inside = tabg_fields_cold(p.tgm, r, th, F);
+            const TabgAux A = tabg_aux(F.v, pr, pth, L, 0.0);                        // mass shell (5): A.W = beta^k p_k here
+            E = fma(F.v[0], sqrt(p.kappa + A.gpp), -A.W);
+        } else if (METRIC == METRIC_TAB) {
             TabFields F;
             y0_inside = tab_fields_cold(p.tm, r, th, F);
             E = fma(F.al, sqrt(p.kappa + pr * pr / F.g11 + pth * pth / F.g22 + L * L / F.g33), -F.be * L);   // mass shell (5)
@@ -210,8 +239,8 @@ __global__ void __launch_bounds__(kBlock, (DENSE || METRIC == METRIC_TAB) ? 2 : 
         crossed = false;
         active = true;
         next_j = 0;
-        if (!(r >= p.r_capture)) { E = METRIC == METRIC_TAB ? __longlong_as_double(0x7ff8000000000000LL) : E; finish(ST_CAPTURED); return; }   // B1
-        if (METRIC == METRIC_TAB) {                                              // T4 on y0: non-finite input, then the domain
+        if (!(r >= p.r_capture)) { E = kTab ? __longlong_as_double(0x7ff8000000000000LL) : E; finish(ST_CAPTURED); return; }   // B1
+        if (kTab) {                                                              // T4 on y0: non-finite input, then the domain
             if (!all_finite6(r, th, ph, pr, pth, L)) { E = __longlong_as_double(0x7ff8000000000000LL); finish(ST_NUMERIC); return; }
             if (!y0_inside) { E = __longlong_as_double(0x7ff8000000000000LL); finish(ST_OUTSIDE); return; }
         }
@@ -258,10 +287,10 @@ __global__ void __launch_bounds__(kBlock, (DENSE || METRIC == METRIC_TAB) ? 2 : 
         sr = fma(h * dp::a21, q1.r, r); sth = fma(h * dp::a21, q1.th, th);
         spr = fma(h * dp::a21, q1.pr, pr); spth = fma(h * dp::a21, q1.pth, pth);
         bool cap = false;
-        int ev = 0;                      // METRIC_TAB: first event in evaluation order (capture before domain exit, T7)
+        int ev = 0;                      // tabulated metrics: first event in evaluation order (capture before domain exit, T7)
         auto evaluate = [&](Deriv& out) {
             const bool in = rhs_metric<METRIC>(p, sr, sth, spr, spth, E, L, out);
-            if (METRIC == METRIC_TAB) {
+            if (kTab) {
                 if (!ev) ev = !(sr >= p.r_capture) ? ST_CAPTURED : (!in ? ST_OUTSIDE : 0);
             } else {
                 cap |= !(sr >= p.r_capture);
@@ -317,7 +346,7 @@ __global__ void __launch_bounds__(kBlock, (DENSE || METRIC == METRIC_TAB) ? 2 : 
         const bool fin6 = all_finite6(nt, nr, nth, nph, npr, npth);
         Deriv k7;
         const bool in7 = rhs_metric<METRIC>(p, nr, nth, npr, npth, E, L, k7);
-        if (METRIC == METRIC_TAB) {                                              // end point: capture, finiteness, then the domain
+        if (kTab) {                                                              // end point: capture, finiteness, then the domain
             if (!ev) ev = !(nr >= p.r_capture) ? ST_CAPTURED : ((fin6 && !in7) ? ST_OUTSIDE : 0);
             cap = ev != 0;
         } else {
@@ -341,7 +370,7 @@ __global__ void __launch_bounds__(kBlock, (DENSE || METRIC == METRIC_TAB) ? 2 : 
         if (active) {
             ++attempts;
             if (cap) {
-                finish(METRIC == METRIC_TAB ? ev : ST_CAPTURED);                 // attempt not taken
+                finish(kTab ? ev : ST_CAPTURED);                 // attempt not taken
             } else if (!fin6 || !(err <= 1.0)) {                                 // reject
                 ++rejected;
                 h *= fmin(fac, 1.0);

@@ -155,8 +155,8 @@ def test_general_table_argument_errors(G):
             G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, st.device, 10, 5), snapshot_every=5, flags=G.FLAG_CARTESIAN_SNAP)
         with pytest.raises(G.GeoError):
             G.geo_integrate(ctx, st, 0.01, 10, G.alloc_outputs(8, st.device), flags=G.FLAG_STATIC_MAP)
-        with pytest.raises(G.GeoError):
-            G.geo_integrate_adaptive(ctx, st, 0.01, 1e-9, 1e-9, 100, G.alloc_outputs(8, st.device))
+        with pytest.raises(G.GeoError):         # the adaptive path exists on this metric (T6 + T7) but takes no flags
+            G.geo_integrate_adaptive(ctx, st, 0.01, 1e-9, 1e-9, 100, G.alloc_outputs(8, st.device), flags=G.FLAG_CARTESIAN_SNAP)
     finally:
         G.geo_destroy(ctx)
 
@@ -190,3 +190,103 @@ def test_general_tabulated_trajectory_records(G, tab_oracle, flags, mask, cap):
             assert np.array_equal(g["snapshots"][done, 3, :], G.to_numpy(oj)["final_state"].T[done])
     finally:
         G.geo_destroy(ctx)
+
+
+# ---- readings T6 + T7: the adaptive RK5(4) stepper on the general ten-field table ----------------------------------------
+def _run_tabg_adaptive(G, tb, st, h0, rtol, atol, max_attempts, host=False, snap_dtau=0.0, cap=0, mask=0xFF, **kw):
+    import torch
+    ctx = G.geo_create_tabulated_general(tb["tab"], tb["x1_0"], tb["d1"], tb["x2_0"], tb["d2"])
+    try:
+        n = st.shape[1]
+        if host:
+            out = G.alloc_outputs_host(n, 0, 1 if snap_dtau else 0, cap, mask)
+            rej = np.full(n, -1, dtype=np.int32)
+            G.geo_integrate_adaptive_host(ctx, np.ascontiguousarray(st), h0, rtol, atol, max_attempts, out, rejected=rej, snap_dtau=snap_dtau, **kw)
+            g = G.to_numpy(out)
+            g["rejected"] = rej
+            return g
+        dev = torch.device("cuda:0")
+        out = G.alloc_outputs(n, dev, 0, 1 if snap_dtau else 0, cap, mask)
+        rej = torch.full((n,), -1, dtype=torch.int32, device=dev)
+        G.geo_integrate_adaptive(ctx, torch.from_numpy(np.ascontiguousarray(st)).to(dev), h0, rtol, atol, max_attempts, out,
+                                 rejected=rej, snap_dtau=snap_dtau, **kw)
+        torch.cuda.synchronize()
+        g = G.to_numpy(out)
+        g["rejected"] = rej.cpu().numpy()
+        return g
+    finally:
+        G.geo_destroy(ctx)
+
+
+def test_general_adaptive_fixed_step_mode_and_records(G, tab_oracle):
+    """Controller off (rtol = inf): identical step sequences, so final states and dense-output records agree like the RK4
+    path's (1e-9) -- Kerr a = 0.9 in Kerr-Schild coordinates, 1501 orbits (ragged) to tau = 40 with 58 records each, odd
+    mask; host entry point bitwise equal to the device one."""
+    a, M = 0.9, 1.0
+    st, consts = W.kerr_bound(1501, a, W.SEED_BASE + 2, return_constants=True)
+    ks = W.to_kerr_schild(st, consts[0], M, a)
+    tb = W.kerr_schild_metric_table(M, a, 513, 129, 1.2, 40.0, 0.15, math.pi - 0.15)
+    for mask, cap in ((0xFF, 60), (0x2E, 7)):
+        kw = dict(tau_end=40.0)
+        o = tab_oracle.integrate_adaptive_general(tb, ks, 0.05, np.inf, 1.0, 10**6, snap_dtau=0.7, snap_capacity=cap, snap_mask=mask, nthreads=NCPU, **kw)
+        g = _run_tabg_adaptive(G, tb, ks, 0.05, float("inf"), 1.0, 10**6, snap_dtau=0.7, cap=cap, mask=mask, **kw)
+        c = parity.compare(g, o)
+        print("general adaptive, controller off: max err", c["err"].max(), "records", parity.snapshot_err(g, o).max())
+        assert c["same_class"].all() and c["err"].max() <= 1e-9
+        done = g["status"] == G.ST_MAXSTEPS
+        assert (g["rejected"] == 0).all() and np.array_equal(g["snap_count"], o["snap_count"])
+        assert (g["snap_count"][done] == 1 + int(40.0 / 0.7)).all() and done.mean() > 0.95
+        assert parity.snapshot_err(g, o).max() <= 1e-9
+        ok = np.isfinite(o["health"])
+        assert np.array_equal(np.isfinite(g["health"]), ok) and np.max(np.abs(g["health"][ok] - o["health"][ok])) < 1e-9
+    gh = _run_tabg_adaptive(G, tb, ks, 0.05, float("inf"), 1.0, 10**6, host=True, snap_dtau=0.7, cap=7, mask=0x2E, **kw)
+    for k in ("final_state", "status", "steps_done", "snapshots", "snap_count", "rejected"):
+        assert np.array_equal(g[k], gh[k], equal_nan=True), k
+
+
+def test_general_adaptive_step_control_plunge_and_domain_exit(G, tab_oracle):
+    """Step control on, Kerr-Schild table: bound orbits to a common final time agree with the oracle as well as the oracle
+    agrees with itself at a ten times tighter tolerance (the interpolant is C^1: accept / reject sequences differ, DESIGN.md
+    8.2); particles thrown at the hole are followed through r_+ to the capture radius inside it (class identical); particles
+    that run off the table end OUTSIDE on both sides."""
+    a, M = 0.9, 1.0
+    rp = M + math.sqrt(M * M - a * a)
+    st, consts = W.kerr_bound(2001, a, W.SEED_BASE + 2, return_constants=True)
+    ks = W.to_kerr_schild(st, consts[0], M, a)
+    tb = W.kerr_schild_metric_table(M, a, 513, 129, 1.2, 40.0, 0.3, math.pi - 0.3)
+    o = tab_oracle.integrate_adaptive_general(tb, ks, 0.05, 1e-11, 1e-11, 10**6, tau_end=150.0, nthreads=NCPU)
+    g = _run_tabg_adaptive(G, tb, ks, 0.05, 1e-11, 1e-11, 10**6, tau_end=150.0)
+    assert np.array_equal(g["status"], o["status"])
+    assert (g["status"] == G.ST_MAXSTEPS).mean() > 0.8
+    done = g["status"] == G.ST_MAXSTEPS
+    e = parity.rel_err(g["final_state"], o["final_state"]).max(axis=0)
+    ob = tab_oracle.integrate_adaptive_general(tb, ks, 0.05, 1e-12, 1e-12, 10**6, tau_end=150.0, nthreads=NCPU)
+    both = done & (ob["status"] == tab_oracle.ST_MAXSTEPS)
+    d_self = parity.rel_err(o["final_state"], ob["final_state"]).max(axis=0)[both]
+    work_g, work_o = g["steps_done"] + g["rejected"], o["steps_done"] + o["rejected"]
+    print("general adaptive: OUTSIDE", int((g["status"] == G.ST_OUTSIDE).sum()), "max err at tau_end", e[done].max(), "p99", np.quantile(e[done], 0.99),
+          "| oracle rtol 1e-11 vs 1e-12: p99", np.quantile(d_self, 0.99), "max", d_self.max(), "| work ratio", work_g.sum() / work_o.sum())
+    assert np.quantile(e[done], 0.99) <= max(5.0 * np.quantile(d_self, 0.99), 1e-8) and e[done].max() <= max(5.0 * d_self.max(), 1e-6)
+    assert abs(work_g.sum() / work_o.sum() - 1.0) < 0.05
+    # plunge through the horizon
+    tb2 = W.kerr_schild_metric_table(M, a, 1025, 257, 1.1, 40.0, 0.15, math.pi - 0.15)
+    n = 256
+    fall = np.zeros((6, n))
+    fall[0] = np.linspace(4.0, 9.0, n)
+    fall[1] = np.linspace(0.6, 2.5, n)
+    fall[3] = -0.2
+    fall[5] = np.linspace(-1.0, 1.0, n)
+    kw = dict(r_capture=1.25, r_escape=39.0)
+    o2 = tab_oracle.integrate_adaptive_general(tb2, fall, 0.05, 1e-9, 1e-9, 10**5, nthreads=NCPU, **kw)
+    g2 = _run_tabg_adaptive(G, tb2, fall, 0.05, 1e-9, 1e-9, 10**5, **kw)
+    assert np.array_equal(g2["status"], o2["status"]) and (g2["status"] == G.ST_CAPTURED).all()
+    assert (g2["final_state"][1] >= 1.25).all() and (g2["final_state"][1] < rp).all() and np.isfinite(g2["final_state"]).all()
+    assert np.nanmax(g2["health"]) < 1e-4
+    # off the table
+    out = ks[:, :300].copy()
+    out[0] = 39.0
+    out[3] = 2.0
+    o3 = tab_oracle.integrate_adaptive_general(tb, out, 0.05, 1e-9, 1e-9, 10**5, nthreads=NCPU)
+    g3 = _run_tabg_adaptive(G, tb, out, 0.05, 1e-9, 1e-9, 10**5)
+    assert np.array_equal(g3["status"], o3["status"]) and (g3["status"] == G.ST_OUTSIDE).all()
+    assert (g3["final_state"][1] <= 40.0).all()

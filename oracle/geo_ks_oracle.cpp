@@ -44,6 +44,8 @@
 #include <thread>
 #include <vector>
 
+#include "dp45.h"
+
 namespace {
 
 enum { KS_ST_MAXSTEPS = 0, KS_ST_CAPTURED = 1, KS_ST_ESCAPED = 2, KS_ST_NUMERIC = 3 };
@@ -292,6 +294,165 @@ void ks_integrate_range(double M, double a, const double* state_in, int64_t n, i
     for (int64_t i = lo; i < hi; ++i) ks_integrate_one<R>(bh, state_in, n, i, (R)h, nsteps, st, snapshot_every, o);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Reading K6: the adaptive Dormand-Prince 5(4) stepper of readings A1-A3 (geo_oracle.cpp: integrate_one_adaptive, the
+// same pair, controller, landing rule and continuous extension, dp45.h) in this chart: the SEVEN evolving components
+// (t~, x, y, z, p_x, p_y, p_z) enter the error norm.  Two rules differ from A2, both because far from the hole the
+// geodesics of this chart are straight lines (the error estimate vanishes and the controller would grow h without bound):
+//   K6a  step cap: no attempt moves the particle by more than a quarter of its current radius in coordinate distance,
+//        h <- min(h, r / (4 |dx/dtau|)) with dx/dtau = k_1 (not in fixed-step mode, rtol = +inf) -- a step cannot jump
+//        over (or into) the hole from afar without an evaluation point ever feeling it;
+//   K6b  the capture test runs on y0 and on the END POINT of an attempt (r(x, y, z) < r_capture: CAPTURED, the attempt is
+//        not taken), not on the stage points: the chart is regular through the horizon, a stage point inside the capture
+//        radius is an ordinary evaluation point (in Cartesian components the stage points of a step along a tight orbit
+//        cut the chord and dip below the orbit's radius by r (dphi)^2 / 8: with a guard on them, rays that skim the
+//        prograde photon orbit 0.001 M outside the capture radius would be captured spuriously).
+// Escape after an accepted step, event K3, records K5 at tau_j = j snap_dtau.
+// ---------------------------------------------------------------------------------------------------------------
+template <class R> R ks_comp7(const KsState<R>& y, int c) {
+    switch (c) { case 0: return y.t; case 1: return y.x; case 2: return y.y; case 3: return y.z;
+                 case 4: return y.px; case 5: return y.py; default: return y.pz; }
+}
+template <class R> R ks_dcomp7(const KsDeriv<R>& k, int c) {
+    switch (c) { case 0: return k.t; case 1: return k.x; case 2: return k.y; case 3: return k.z;
+                 case 4: return k.px; case 5: return k.py; default: return k.pz; }
+}
+template <class R> void ks_set7(KsState<R>& y, int c, R v) {
+    switch (c) { case 0: y.t = v; break; case 1: y.x = v; break; case 2: y.y = v; break; case 3: y.z = v; break;
+                 case 4: y.px = v; break; case 5: y.py = v; break; default: y.pz = v; }
+}
+
+template <class R>
+void ks_integrate_one_adaptive(const KsHole<R>& bh, const double* state_in, int64_t n, int64_t i, const AdaptiveCtl& ctl,
+                               int64_t max_attempts, const KsStop& st, const KsOut& o, int64_t* rejected_out) {
+    static const DP45 T;
+    const R kappa = st.kind == 0 ? R(1) : R(0);
+    const R rc = (R)st.r_capture, re = (R)st.r_escape;
+    KsState<R> y;
+    y.t = R(0);
+    y.x = (R)state_in[0 * n + i];
+    y.y = (R)state_in[1 * n + i];
+    y.z = (R)state_in[2 * n + i];
+    y.px = (R)state_in[3 * n + i];
+    y.py = (R)state_in[4 * n + i];
+    y.pz = (R)state_in[5 * n + i];
+    y.E = ks_energy(bh, y.x, y.y, y.z, y.px, y.py, y.pz, kappa);
+    R cc[7] = {0, 0, 0, 0, 0, 0, 0};
+    R h = (R)ctl.h0, tau = R(0);
+    const R tau_end = (R)ctl.tau_end;
+    const bool dense = ctl.snap_dtau > 0.0 && o.snapshots != nullptr;
+    const R dtau = (R)ctl.snap_dtau;
+    int64_t next_j = 0;
+    int32_t status = -1;
+    int64_t steps = 0, attempts = 0, rejected = 0;
+    R eq_cross = std::numeric_limits<R>::quiet_NaN();
+    bool crossed = false;
+    R ry = ks_radius(bh, y.x, y.y, y.z);
+
+    if (!(ry >= rc)) status = KS_ST_CAPTURED;                        // B1 / K2
+    else if (!ks_finite7(y) || !std::isfinite(y.E)) status = KS_ST_NUMERIC;
+    else {
+        if (dense) { ks_write_snapshot(o, i, 0, y); next_j = 1; }
+        if (ry > re) status = KS_ST_ESCAPED;
+        else if (max_attempts == 0) status = KS_ST_MAXSTEPS;
+    }
+
+    KsDeriv<R> k[DP45::S];
+    if (status < 0) k[0] = ks_rhs(bh, y);
+    while (status < 0) {
+        if (!std::isinf(ctl.rtol)) {                                 // K6a
+            const R hcap = ry / (R(4) * std::sqrt(k[0].x * k[0].x + k[0].y * k[0].y + k[0].z * k[0].z));
+            if (h > hcap) h = hcap;
+        }
+        const bool last = tau + R(1.01) * h >= tau_end;
+        if (last) h = tau_end - tau;
+        for (int s = 1; s < DP45::S - 1; ++s) {                      // stages 2..6 (no capture guard on them: K6b)
+            KsState<R> ys = y;
+            for (int c = 0; c < 7; ++c) {
+                R acc = R(0);
+                for (int j = 0; j < s; ++j) acc += (R)T.a[s][j] * ks_dcomp7(k[j], c);
+                ks_set7(ys, c, ks_comp7(y, c) + h * acc);
+            }
+            k[s] = ks_rhs(bh, ys);
+        }
+        ++attempts;
+        KsState<R> yn = y;
+        R cn[7];
+        for (int c = 0; c < 7; ++c) {
+            R acc5 = R(0);
+            for (int j = 0; j < DP45::S - 1; ++j) acc5 += (R)T.a[6][j] * ks_dcomp7(k[j], c);
+            R v = ks_comp7(y, c);
+            cn[c] = cc[c];
+            ks_kahan_add(v, cn[c], h * acc5, false);
+            ks_set7(yn, c, v);
+        }
+        const R rn = ks_radius(bh, yn.x, yn.y, yn.z);
+        if (!(rn >= rc)) { status = KS_ST_CAPTURED; break; }         // end point
+        const bool fin = ks_finite7(yn);
+        R err = R(0);
+        if (fin) {
+            k[6] = ks_rhs(bh, yn);
+            for (int c = 0; c < 7; ++c) {
+                R acce = R(0);
+                for (int j = 0; j < DP45::S; ++j)
+                    acce += ((R)(j < 6 ? T.a[6][j] : 0.0L) - (R)T.b4[j]) * ks_dcomp7(k[j], c);
+                const R sc = (R)ctl.atol + (R)ctl.rtol * std::max(std::fabs(ks_comp7(y, c)), std::fabs(ks_comp7(yn, c)));
+                const R ec = std::fabs(h * acce) / sc;
+                if (!(ec <= err)) err = ec;
+            }
+        }
+        if (fin && std::isinf(ctl.rtol)) err = R(0);
+        R fac = err > R(0) ? R(0.9) * std::pow(err, R(-0.2)) : (err == R(0) ? R(5) : R(0.2));
+        if (!(fac >= R(0.2))) fac = R(0.2);
+        if (fac > R(5)) fac = R(5);
+        if (std::isinf(ctl.rtol)) fac = R(1);
+        if (!fin || !(err <= R(1))) {                                // reject
+            ++rejected;
+            h *= std::min(fac, R(1));
+            if ((std::isinf(ctl.rtol) && !fin) || !(std::fabs(h) >= (R)ctl.h_min) || !(std::fabs(h) > R(0))) { status = KS_ST_NUMERIC; break; }
+            if (attempts >= max_attempts) { status = KS_ST_MAXSTEPS; break; }
+            continue;
+        }
+        if (!crossed && y.z * yn.z < R(0)) {                         // K3
+            crossed = true;
+            eq_cross = ry + (rn - ry) * (R(0) - y.z) / (yn.z - y.z);
+        }
+        const R tau_new = last ? tau_end : tau + h;
+        if (dense) {
+            for (;;) {
+                const R tj = (R)next_j * dtau;
+                if (!(tj <= tau_new)) break;
+                R w[7];
+                dp45_dense_weights<R>((tj - tau) / h, w);
+                KsState<R> ys = y;
+                for (int c = 0; c < 7; ++c) {
+                    R acc = R(0);
+                    for (int j = 0; j < DP45::S; ++j) acc += w[j] * ks_dcomp7(k[j], c);
+                    ks_set7(ys, c, ks_comp7(y, c) + h * acc);
+                }
+                ks_write_snapshot(o, i, next_j, ys);
+                ++next_j;
+            }
+        }
+        y = yn;
+        ry = rn;
+        for (int c = 0; c < 7; ++c) cc[c] = cn[c];
+        k[0] = k[6];
+        ++steps;
+        tau = tau_new;
+        h *= fac;
+        if (ry > re) status = KS_ST_ESCAPED;
+        else if (last || attempts >= max_attempts) status = KS_ST_MAXSTEPS;
+    }
+    for (int q = 0; q < 8; ++q) o.final_state[(int64_t)q * n + i] = (double)ks_component(y, q);
+    o.status[i] = status;
+    o.steps_done[i] = steps;
+    if (o.eq_cross_r) o.eq_cross_r[i] = (double)eq_cross;
+    if (o.health) o.health[i] = (double)std::fabs(R(2) * ks_hamiltonian(bh, y) + kappa);
+    if (dense && o.snap_count) o.snap_count[i] = (int32_t)next_j;
+    if (rejected_out) rejected_out[i] = rejected;
+}
+
 }  // namespace
 
 extern "C" {
@@ -361,6 +522,37 @@ void oracle_ks_metric(double M, double a, double x, double y, double z, double* 
     KsHole<double> bh{M, a};
     const KsGeom<double> g = ks_geometry(bh, x, y, z);
     out4[0] = g.f; out4[1] = g.l[0]; out4[2] = g.l[1]; out4[3] = g.l[2];
+}
+
+// Adaptive RK5(4) in the Kerr-Schild chart (reading K6).  ctl = {h0, rtol, atol, h_min, tau_end, snap_dtau}; rejected: [n] or NULL.
+int oracle_ks_integrate_adaptive(double M, double a, const double* state_in, int64_t n, const AdaptiveCtl* ctl,
+                                 int64_t max_attempts, const KsStop* stop, const KsOut* out, int64_t* rejected,
+                                 int precision, int nthreads) {
+    if (!stop || !out || !ctl || n < 0 || max_attempts < 0) return 1;
+    if (!(M >= 0) || !(std::fabs(a) <= M || M == 0)) return 1;
+    if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0) || !(ctl->rtol >= 0) || !(ctl->atol >= 0) || !(ctl->rtol + ctl->atol > 0) ||
+        !(ctl->h_min >= 0) || !(ctl->tau_end > 0) || !(ctl->snap_dtau >= 0)) return 1;
+    if (n == 0) return 0;
+    if (!state_in || !out->final_state || !out->status || !out->steps_done) return 1;
+    if (ctl->snap_dtau > 0 && (!out->snapshots || !out->snap_count || out->snap_capacity < 1 || (out->snap_mask & 0xFFu) == 0)) return 1;
+    if (nthreads < 1) nthreads = 1;
+    std::vector<std::thread> pool;
+    const int64_t block = 64, nblocks = (n + block - 1) / block;
+    for (int t = 0; t < nthreads; ++t)
+        pool.emplace_back([&, t]() {
+            for (int64_t b = t; b < nblocks; b += nthreads)
+                for (int64_t i = b * block; i < std::min<int64_t>(n, (b + 1) * block); ++i) {
+                    if (precision == 1) {
+                        KsHole<long double> bh{M, a};
+                        ks_integrate_one_adaptive<long double>(bh, state_in, n, i, *ctl, max_attempts, *stop, *out, rejected);
+                    } else {
+                        KsHole<double> bh{M, a};
+                        ks_integrate_one_adaptive<double>(bh, state_in, n, i, *ctl, max_attempts, *stop, *out, rejected);
+                    }
+                }
+        });
+    for (auto& th : pool) th.join();
+    return 0;
 }
 
 }  // extern "C"

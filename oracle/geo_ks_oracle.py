@@ -108,3 +108,38 @@ def integrate(M: float, a: float, state_in: np.ndarray, h: float, nsteps: int, r
     if rc != 0:
         raise ValueError("oracle_ks_integrate: invalid arguments")
     return res
+
+
+class _Ctl(C.Structure):
+    _fields_ = [("h0", C.c_double), ("rtol", C.c_double), ("atol", C.c_double), ("h_min", C.c_double),
+                ("tau_end", C.c_double), ("snap_dtau", C.c_double)]
+
+
+def integrate_adaptive(M: float, a: float, state_in: np.ndarray, h0: float, rtol: float, atol: float, max_attempts: int,
+                       r_capture: float = -np.inf, r_escape: float = np.inf, kind: int = TIMELIKE, h_min: float = 1e-12,
+                       tau_end: float = np.inf, long_double: bool = False, nthreads: int = 1, snap_dtau: float = 0.0,
+                       snap_capacity: int = 0, snap_mask: int = 0xFF) -> dict:
+    """Adaptive Dormand-Prince RK5(4) in the Kerr-Schild chart (reading K6) on host SoA state_in [6][n]; rtol = inf: fixed step."""
+    st = np.ascontiguousarray(state_in, dtype=np.float64)
+    n = st.shape[1]
+    res = {"final_state": np.full((8, n), np.nan), "status": np.full(n, -1, dtype=np.int32),
+           "steps_done": np.zeros(n, dtype=np.int64), "eq_cross_r": np.full(n, np.nan), "health": np.full(n, np.nan),
+           "rejected": np.zeros(n, dtype=np.int64), "snapshots": None, "snap_count": None}
+    if snap_dtau > 0:
+        res["snapshots"] = np.full((n, snap_capacity, bin(snap_mask & 0xFF).count("1")), np.nan)
+        res["snap_count"] = np.zeros(n, dtype=np.int32)
+    stop = _Stop(r_capture, r_escape, kind, 0)
+    out = _Out(res["final_state"].ctypes.data, res["status"].ctypes.data, res["steps_done"].ctypes.data,
+               res["eq_cross_r"].ctypes.data, res["health"].ctypes.data,
+               res["snapshots"].ctypes.data if snap_dtau > 0 else None, snap_capacity, snap_mask,
+               res["snap_count"].ctypes.data if snap_dtau > 0 else None)
+    ctl = _Ctl(h0, rtol, atol, h_min, tau_end, snap_dtau)
+    L = lib()
+    L.oracle_ks_integrate_adaptive.restype = C.c_int
+    L.oracle_ks_integrate_adaptive.argtypes = [C.c_double, C.c_double, C.c_void_p, C.c_int64, C.POINTER(_Ctl), C.c_int64,
+                                               C.POINTER(_Stop), C.POINTER(_Out), C.c_void_p, C.c_int, C.c_int]
+    rc = L.oracle_ks_integrate_adaptive(M, a, st.ctypes.data, n, C.byref(ctl), max_attempts, C.byref(stop), C.byref(out),
+                                        res["rejected"].ctypes.data, int(long_double), nthreads)
+    if rc != 0:
+        raise ValueError("oracle_ks_integrate_adaptive: invalid arguments")
+    return res

@@ -394,3 +394,81 @@ def test_stop_rules_and_records():
     k = KS.integrate(M, a, st, 0.02, 500)
     d = np.max(np.abs(p["final_state"] - k["final_state"]))
     assert 0 < d < 1e-8
+
+
+# ---------------------------------------------------------------------------
+# reading K6: the adaptive RK5(4) stepper in this chart
+# ---------------------------------------------------------------------------
+def test_adaptive_is_fifth_order_and_lands_on_the_pinned_fixed_step_solution():
+    """Controller off (rtol = inf): the propagated solution converges with order 5 (Q ~ 32-50 on these orbits at h = 1, 1/2, 1/4; the pinned RK4 path gives 16).
+    Controller on: it lands on tau_end with the state the PINNED fixed-step path of this file reaches with a small step;
+    E is untouched, L_z (not a momentum of the chart) is conserved to the tolerance."""
+    M, a = 1.0, 0.9
+    st, consts = W.kerr_bound(24, a, W.SEED_BASE + 2, return_constants=True)
+    ks = W.to_cartesian_kerr_schild(st, consts[0], M, a)
+    sols = []
+    for k in (1, 2, 4):
+        r = KS.integrate_adaptive(M, a, ks, 1.0 / k, np.inf, 1.0, 10**6, tau_end=40.0, long_double=True)
+        assert (r["status"] == KS.ST_MAXSTEPS).all() and (r["steps_done"] == 40 * k).all() and (r["rejected"] == 0).all()
+        sols.append(r["final_state"])
+    d12 = np.linalg.norm(sols[1] - sols[2], axis=0)
+    big = d12 > 1e-12                      # above the rounding of the double-precision output
+    Q = np.linalg.norm(sols[0] - sols[1], axis=0)[big] / d12[big]
+    # the ratio scatters per orbit (the leading error term changes sign along an orbit); a fourth-order pair would give 16
+    assert big.sum() >= 10 and Q.min() > 17.0 and 28.0 < np.median(Q) < 64.0, Q
+    ref = KS.integrate(M, a, ks, 0.0025, 4000, long_double=True, nthreads=NCPU)
+    ad = KS.integrate_adaptive(M, a, ks, 0.1, 1e-12, 1e-12, 10**6, tau_end=10.0, nthreads=NCPU)
+    assert (ad["status"] == KS.ST_MAXSTEPS).all() and (ad["rejected"] >= 0).all()
+    assert np.max(np.abs(ad["final_state"] - ref["final_state"]) / np.maximum(np.abs(ref["final_state"]), 1.0)) < 1e-9
+    assert np.max(np.abs(ad["final_state"][4] - ref["final_state"][4])) < 4e-16            # E: constant (ref ran in long double)
+    f = ad["final_state"]
+    assert np.max(np.abs(f[1] * f[6] - f[2] * f[5] - consts[1])) < 1e-9
+
+
+def test_adaptive_matches_the_boyer_lindquist_adaptive_oracle_and_dense_records():
+    """Bound orbits to tau = 40 at a tight tolerance: r, cos(theta) equal those of the pinned Boyer-Lindquist adaptive oracle
+    (another chart, another right-hand side) to the tolerance.  Dense output (A3): records at tau_j = 2.5 j equal the
+    fixed-step path's states at the same tau to the continuous extension's accuracy; record 0 = y0; in fixed-step mode a
+    record on a step boundary is that step's state."""
+    M, a = 1.0, 0.9
+    st, consts = W.kerr_bound(40, a, W.SEED_BASE + 2, return_constants=True)
+    ks = W.to_cartesian_kerr_schild(st, consts[0], M, a)
+    bl = BL.integrate_adaptive(BL.KERR, M, a, st, 0.05, 1e-12, 1e-12, 10**6, tau_end=40.0, nthreads=NCPU)
+    ad = KS.integrate_adaptive(M, a, ks, 0.05, 1e-12, 1e-12, 10**6, tau_end=40.0, snap_dtau=2.5, snap_capacity=17, nthreads=NCPU)
+    r, c, E, Lz, Q = _shared(ad["final_state"], a, 1.0)
+    assert np.max(np.abs(r - bl["final_state"][1]) / bl["final_state"][1]) < 2e-9
+    assert np.max(np.abs(c - np.cos(bl["final_state"][2]))) < 2e-9
+    assert (ad["snap_count"] == 17).all()
+    assert np.array_equal(ad["snapshots"][:, 0, [1, 2, 3, 5, 6, 7]], ks.T) and np.all(ad["snapshots"][:, 0, 0] == 0.0)
+    fx = KS.integrate(M, a, ks, 0.0025, 16000, snapshot_every=1000, long_double=True, nthreads=NCPU)
+    e = np.abs(ad["snapshots"] - fx["snapshots"]) / np.maximum(np.abs(fx["snapshots"]), 1.0)
+    assert e.max() < 1e-8, e.max()
+    f = KS.integrate_adaptive(M, a, ks, 0.25, np.inf, 1.0, 10**6, tau_end=3.0, snap_dtau=1.0, snap_capacity=5)
+    f2 = KS.integrate_adaptive(M, a, ks, 0.25, np.inf, 1.0, 10**6, tau_end=2.0)
+    assert (f["snap_count"] == 4).all() and np.abs(f["snapshots"][:, 2, :] - f2["final_state"].T).max() < 1e-13
+
+
+def test_adaptive_camera_rays_get_every_class_right_where_both_fixed_step_charts_fail():
+    """configs[2] rays (a = 0.998, i = 60 deg) with step control, rtol = atol = 1e-9: the termination class equals the
+    closed-form capture criterion on EVERY ray of (i) the 10 polar-axis columns (64 rows), where the fixed-step
+    Boyer-Lindquist path fails (reading B7), and (ii) the pixels at the prograde edge of the shadow where the fixed-step path
+    of this chart fails, and (iii) a strided sub-image; |2H| of the escaped rays stays at the tolerance's level
+    (readings K6a, K6b are what makes this work: step cap r/4, capture test on end points only)."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from test_gpu_fullsize import _escapes_analytic
+    M, a, N = 1.0, 0.998, 1024
+    rp = W.horizon_radius(M, a)
+    full, consts = W.camera_rays(N, a, 60.0, return_constants=True)
+    img = np.arange(N * N).reshape(N, N)
+    sel = np.concatenate([img[8::16, N // 2 - 5:N // 2 + 5].ravel(), img[440:600:2, 386:392].ravel(), img[32::64, 32::64].ravel()])
+    st = np.ascontiguousarray(full[:, sel])
+    ks = W.to_cartesian_kerr_schild(st, np.ones(len(sel)), M, a)
+    o = KS.integrate_adaptive(M, a, ks, 0.02, 1e-9, 1e-9, 200000, r_capture=rp + 0.01, r_escape=1100.0, kind=KS.NULL, nthreads=NCPU)
+    esc = _escapes_analytic(a, consts[2][sel], consts[3][sel], rp, 1000.0)
+    assert set(np.unique(o["status"])) <= {KS.ST_CAPTURED, KS.ST_ESCAPED}
+    wrong = (o["status"] == KS.ST_ESCAPED) != esc
+    assert wrong.sum() == 0, (int(wrong.sum()), sel[wrong][:10])
+    assert 0.2 < esc.mean() < 0.95
+    he = o["health"][o["status"] == KS.ST_ESCAPED]
+    assert np.median(he) < 1e-8 and he.max() < 1e-4        # the largest: rays that whirl ~2000 steps next to the photon orbit
+    assert (o["steps_done"] + o["rejected"]).mean() < 1500          # per-ray step control: hundreds of attempts, not 10^5 steps

@@ -59,6 +59,9 @@ bad = kks.copy(); bad[0:3, 0] = 0.1; bad[3, 1] = np.nan; bad[0, 2] = 1e6
 rk = K.integrate(1.0, 0.9, bad, 0.01, 10, r_capture=1.3, r_escape=100.0, kind=K.NULL)
 assert rk["status"][0] == K.ST_CAPTURED and rk["status"][1] == K.ST_NUMERIC and rk["status"][2] == K.ST_ESCAPED
 K.rhs(1.0, 0.9, [0, 3.0, 1.0, 2.0, 1.1, 0.1, 0.2, 0.3], long_double=True); K.hamiltonian(1.0, 0.9, [0, 3.0, 1.0, 2.0, 1.1, 0.1, 0.2, 0.3])
+rka = K.integrate_adaptive(1.0, 0.9, kks, 0.05, 1e-9, 1e-9, 4000, r_capture=1.3, r_escape=25.0, tau_end=20.0, snap_dtau=0.7, snap_capacity=9,
+                           snap_mask=0x2B, long_double=True, nthreads=3)
+assert (rka["snap_count"] >= 1).all()
 K.energy(1.0, 0.9, 3.0, 1.0, 2.0, 0.1, 0.2, 0.3, 1.0); K.radius(1.0, 0.9, 0.0, 0.0, 0.0); K.metric(1.0, 0.9, 3.0, 1.0, 2.0)
 print("sanitized oracle run ok")
 """

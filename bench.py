@@ -72,6 +72,9 @@ KERNEL_COUNTS = {
     "kerr_schild": dict(sym="geo_ks_rk4_kernelILi0ELb0EE", units_per_loop=2, flop=634.5, pipe=437.8, other=56.6, tol=0.08, static_at_capture=(1308, 909),
                         source="ncu per-instruction counts, profiles/r02_ks4.md: 201.7 DFMA + 163.1 DMUL + 68.0 DADD + 5.0 DSETP per step",
                         kernel="geo_ks_rk4_kernel"),
+    "adaptive_ks": dict(sym="geo_ks_rk45_kernelILb0EE", units_per_loop=1, flop=0.0, pipe=0.0, other=None, tol=0.0,
+                        source="static SASS count of the attempt loop (no ncu capture of this kernel; counts include predicated-off work)",
+                        kernel="geo_ks_rk45_kernel"),
     "tabulated_general": dict(sym="geo_tabg_rk4_kernelILb0ELb1ELb0E", units_per_loop=None, flop=4073.0, pipe=2376.0, other=None, tol=None,
                               source="ncu per-instruction counts, profiles/r02_tab4_tabg4.md: 1735 DFMA + 550 DMUL + 52 DADD + 38 DSETP per step "
                                      "(4 evaluations through one rolled copy of the evaluator: no static cross-check)", kernel="geo_tabg_rk4_kernel"),
@@ -168,6 +171,12 @@ def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dic
         wl["name"] += " -- in Cartesian Kerr-Schild coordinates"
         wl["metric"] = "kerr_schild"
         wl["st"] = W.to_cartesian_kerr_schild(wl["st"], np.ones(wl["st"].shape[1]), 1.0, wl["a"])
+        return wl
+    if name == "config3aks":
+        # reading K6: the rays of configs[2] with the adaptive stepper in Cartesian Kerr-Schild coordinates
+        wl = workload("config3ks", rank, n_override, nthreads)
+        wl["name"] += ", adaptive RK5(4), rtol = atol = 1e-9"
+        wl["adaptive"] = dict(h0=wl["h"], rtol=1e-9, atol=1e-9, max_attempts=wl["nsteps"])
         return wl
     if name == "config3a":
         # the rays of configs[2] with the adaptive Dormand-Prince 5(4) stepper (per-ray step control);
@@ -325,6 +334,10 @@ def oracle_time(wl: dict, steps: int, warmup: int, budget_s: float = 12.0) -> di
             fn = geo_tab_oracle.integrate if wl["metric"] == "tabulated" else geo_tab_oracle.integrate_general
             o = fn(wl["table"], sub, wl["h"], wl["nsteps"], r_capture=wl["r_capture"],
                    r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
+        elif wl["metric"] == "kerr_schild" and ad:
+            import geo_ks_oracle
+            o = geo_ks_oracle.integrate_adaptive(1.0, wl["a"], sub, ad["h0"], ad["rtol"], ad["atol"], ad["max_attempts"],
+                                                 r_capture=wl["r_capture"], r_escape=wl["r_escape"], kind=wl["kind"], nthreads=cores)
         elif wl["metric"] == "kerr_schild":
             import geo_ks_oracle
             o = geo_ks_oracle.integrate(1.0, wl["a"], sub, wl["h"], wl["nsteps"], r_capture=wl["r_capture"], r_escape=wl["r_escape"],
@@ -547,7 +560,9 @@ class GpuRun:
 
 
 def counts_key(wl: dict) -> str:
-    return "adaptive" if wl.get("adaptive") else wl["metric"]
+    if wl.get("adaptive"):
+        return "adaptive_ks" if wl["metric"] == "kerr_schild" else "adaptive"
+    return wl["metric"]
 
 
 def alu_roofline(kc: dict, units_per_s: float, sm_max_mhz: float) -> dict:
@@ -564,7 +579,8 @@ SECONDARY = [("config2", "config2", 0, True), ("config3", "config3", 0, True), (
              ("snapbench_schwarzschild_every_step", "snapbench", 0, False), ("snapkerr_every_step_8comp", "snapkerr", 0, False),
              ("snapkerr_every_step_txyz", "snapkerr_xyz", 0, False), ("config3_adaptive_rk45", "config3a", 0, True),
              ("tab4_tabulated_metric", "tab4", 0, False), ("tabg4_general_tabulated_metric_kerr_schild", "tabg4", 0, False),
-             ("ks4_cartesian_kerr_schild", "ks4", 0, True), ("config3_cartesian_kerr_schild", "config3ks", 0, False), ("paper_table3", "paper_t3", 0, False), ("paper_table4", "paper_t4", 0, False)]
+             ("ks4_cartesian_kerr_schild", "ks4", 0, True), ("config3_cartesian_kerr_schild", "config3ks", 0, False),
+             ("config3_adaptive_rk45_cartesian_kerr_schild", "config3aks", 0, True), ("paper_table3", "paper_t3", 0, False), ("paper_table4", "paper_t4", 0, False)]
 
 
 def run_secondary(torch, geo, dev, sm_max: float, ncpu: int, peaks: dict, reuse_config4) -> dict:
@@ -634,7 +650,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4",
-                    choices=["config1", "config2", "config3", "config4", "config5", "config5tile", "config3s", "config3a", "tab4", "tabg4", "ks4", "config3ks",
+                    choices=["config1", "config2", "config3", "config4", "config5", "config5tile", "config3s", "config3a", "tab4", "tabg4", "ks4", "config3ks", "config3aks",
                              "snapbench", "snapkerr", "snapkerr_xyz", "paper_t3", "paper_t4"])
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank its own batch; strong = one image (config3) split into interleaved row tiles")

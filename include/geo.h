@@ -108,7 +108,13 @@ int geo_create(geo_ctx **ctx, int metric, double M, double a);
  *   eq_cross_r: r at the first sign change of z between two accepted states, linear in z between them; quiet NaN if none.
  *   health = |2H + kappa|.  coarse_steps is ignored.  flags: GEO_FLAG_PLAIN_UPDATE, GEO_FLAG_STATIC_MAP
  *   (records are Cartesian already: GEO_FLAG_CARTESIAN_SNAP and the staged writer return GEO_EINVAL).
- * geo_integrate_adaptive and geo_integrate_host_noalloc return GEO_EINVAL for this metric; geo_horizon_radius works. */
+ * geo_integrate_adaptive / geo_integrate_adaptive_host take this metric too (reading K6; flags must be 0): the pair,
+ *   controller, landing rule and dense output documented at geo_integrate_adaptive, over the SEVEN components
+ *   (t~, x, y, z, p_x, p_y, p_z), with two rules of this chart's own -- (a) no attempt moves the particle by more than a
+ *   quarter of its current radius, h <- min(h, r / (4 |dx/dtau|)) (far from the hole the geodesics are straight lines here and
+ *   the error estimate alone would let a step jump over the hole; not applied in fixed-step mode), (b) the capture test runs on
+ *   y0 and on the END POINT of an attempt, not on the stage points (the chart is regular through the horizon).
+ * geo_integrate_host_noalloc returns GEO_EINVAL for this metric; geo_horizon_radius works. */
 
 /* Integrate n geodesics for at most nsteps (< 2^31) RK4 steps of size h (h < 0 integrates backwards in tau).
  * state_in: DEVICE, SoA [6][n] = (r, theta, phi, u_r, u_theta, u_phi) (covariant); t starts at 0 and

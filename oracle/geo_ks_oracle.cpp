@@ -389,8 +389,9 @@ void ks_integrate_one_adaptive(const KsHole<R>& bh, const double* state_in, int6
         const R rn = ks_radius(bh, yn.x, yn.y, yn.z);
         if (!(rn >= rc)) { status = KS_ST_CAPTURED; break; }         // end point
         const bool fin = ks_finite7(yn);
-        R err = R(0);
+        R err = std::numeric_limits<R>::quiet_NaN();                 // a non-finite attempt: rejected, the step shrinks by 0.2
         if (fin) {
+            err = R(0);
             k[6] = ks_rhs(bh, yn);
             for (int c = 0; c < 7; ++c) {
                 R acce = R(0);

@@ -19,6 +19,7 @@ LIB = os.path.join(PKG, "libgeo.so")
 SOURCES = [os.path.join(CSRC, "geo_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "geo_kernel.cuh"), os.path.join(CSRC, "geo_rhs.cuh"),
                   os.path.join(CSRC, "geo_rk45.cuh"), os.path.join(CSRC, "geo_tab.cuh"), os.path.join(CSRC, "geo_tabg.cuh"),
+                  os.path.join(CSRC, "geo_ks.cuh"), os.path.join(CSRC, "geo_ks_rk45.cuh"),
                   os.path.join(ROOT, "include", "geo.h"), os.path.join(ROOT, "include", "geo_dev.h")]
 
 

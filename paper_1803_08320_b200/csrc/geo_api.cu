@@ -13,6 +13,7 @@
 #include "geo_tab.cuh"
 #include "geo_tabg.cuh"
 #include "geo_ks.cuh"
+#include "geo_ks_rk45.cuh"
 
 using namespace geo;
 
@@ -727,8 +728,7 @@ static int validate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, co
                              const geo_stop* stop, const geo_out* out, const int32_t* rejected, bool check_align) {
     int rc = validate(ctx, state_in, n, 1.0, 0, stop, 0, out, check_align);
     if (rc != GEO_OK) return rc;
-    if (ctx->metric == GEO_KERR_SCHILD)
-        return fail(ctx, GEO_EINVAL, "the adaptive path takes the Boyer-Lindquist metrics and tabulated metrics only");
+    if (ctx->metric == GEO_KERR_SCHILD && stop && stop->flags != 0) return fail(ctx, GEO_EINVAL, "GEO_KERR_SCHILD: the adaptive path takes no flags");
     if ((ctx->metric == GEO_TABULATED || ctx->metric == GEO_TABULATED_GENERAL) && stop && stop->flags != 0) return fail(ctx, GEO_EINVAL, "tabulated metrics: the adaptive path takes no flags");
     if (!ctl) return fail(ctx, GEO_EINVAL, "ctl must not be NULL");
     if (!std::isfinite(ctl->h0) || !(ctl->h0 > 0.0)) return fail(ctx, GEO_EINVAL, "h0 must be finite and > 0");
@@ -747,10 +747,64 @@ static int validate_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, co
     return GEO_OK;
 }
 
+// GEO_KERR_SCHILD: the adaptive kernel of geo_ks_rk45.cuh (reading K6).
+static int launch_adaptive_ks(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl, int64_t max_attempts,
+                              const geo_stop* stop, const geo_out* out, int32_t* rejected, cudaStream_t stream,
+                              unsigned long long* counter) {
+    KsAdaptiveParams p;
+    memset(&p, 0, sizeof p);
+    p.in = state_in;
+    p.n = n;
+    p.h0 = ctl->h0;
+    p.rtol = ctl->rtol;
+    p.atol = ctl->atol;
+    p.h_min = ctl->h_min;
+    p.tau_end = ctl->tau_end;
+    p.fixed_step = std::isinf(ctl->rtol) ? 1 : 0;
+    p.max_attempts = (int)max_attempts;
+    p.r_capture = stop->r_capture;
+    p.r_escape = stop->r_escape;
+    p.kappa = stop->kind == GEO_TIMELIKE ? 1.0 : 0.0;
+    p.fin = out->final_state;
+    p.status = out->status;
+    p.steps_done = reinterpret_cast<long long*>(out->steps_done);
+    p.eq_cross_r = out->eq_cross_r;
+    p.health = out->health;
+    p.rejected = rejected;
+    p.counter = counter;
+    const bool dense = ctl->snap_dtau > 0.0;
+    p.snap_dtau = ctl->snap_dtau;
+    p.snaps = dense ? out->snapshots : nullptr;
+    p.snap_cap = dense ? out->snap_capacity : 0;
+    p.snap_mask = dense ? (out->snap_mask & 0xFFu) : 0;
+    p.ncomp = dense ? popcount8(out->snap_mask) : 0;
+    p.snap_count = dense ? out->snap_count : nullptr;
+    p.bh.M = ctx->M;
+    p.bh.a = ctx->a;
+    p.bh.a2 = ctx->a * ctx->a;
+    p.bh.twoM = 2.0 * ctx->M;
+    p.bh.four_a2 = 4.0 * ctx->a * ctx->a;
+    typedef void (*fn_t)(const KsAdaptiveParams);
+    fn_t fn = dense ? (fn_t)geo_ks_rk45_kernel<true> : (fn_t)geo_ks_rk45_kernel<false>;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kBlock, 0);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "occupancy(ks rk45)");
+    if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
+    const int64_t need = (n + kBlock - 1) / kBlock, resident = (int64_t)ctx->sm_count * per_sm;
+    const int grid = (int)(need < resident ? need : resident);
+    e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
+    fn<<<grid, kBlock, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
+    return GEO_OK;
+}
+
 // Enqueue the RK5(4) kernel on validated arguments (device pointers); the ctx's device is current.
 static int launch_adaptive(geo_ctx* ctx, const double* state_in, int64_t n, const geo_adaptive* ctl, int64_t max_attempts,
                            const geo_stop* stop, const geo_out* out, int32_t* rejected, cudaStream_t stream,
                            unsigned long long* counter) {
+    if (ctx->metric == GEO_KERR_SCHILD) return launch_adaptive_ks(ctx, state_in, n, ctl, max_attempts, stop, out, rejected, stream, counter);
     AdaptiveParams p;
     memset(&p, 0, sizeof p);
     p.in = state_in;

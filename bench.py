@@ -69,8 +69,8 @@ KERNEL_COUNTS = {
     "adaptive": dict(sym="geo_rk45_kernelILi1ELb0E", units_per_loop=1, flop=1039.0, pipe=678.0, other=None, tol=0.15, static_at_capture=(1135, 778),
                      source="ncu thread-level counts, profiles/r02_config3a_rk45.md: 361 DFMA + 264 DMUL + 52 DADD per attempt "
                             "(incl. predicated-on work of lanes waiting for a refill)", kernel="geo_rk45_kernel"),
-    "kerr_schild": dict(sym="geo_ks_rk4_kernelILi0ELb0EE", units_per_loop=2, flop=634.5, pipe=437.8, other=56.6, tol=0.08, static_at_capture=(1308, 909),
-                        source="ncu per-instruction counts, profiles/r02_ks4.md: 201.7 DFMA + 163.1 DMUL + 68.0 DADD + 5.0 DSETP per step",
+    "kerr_schild": dict(sym="geo_ks_rk4_kernelILi0ELb0EE", units_per_loop=2, flop=561.0, pipe=393.8, other=57.6, tol=0.08, static_at_capture=(1161, 821),
+                        source="ncu per-instruction counts, profiles/r02_ks4.md: 172.2 DFMA + 160.6 DMUL + 56.0 DADD + 5.0 DSETP per step",
                         kernel="geo_ks_rk4_kernel"),
     "adaptive_ks": dict(sym="geo_ks_rk45_kernelILb0EE", units_per_loop=1, flop=0.0, pipe=0.0, other=None, tol=0.0,
                         source="static SASS count of the attempt loop (no ncu capture of this kernel; counts include predicated-off work)",
@@ -85,7 +85,7 @@ KERNEL_COUNTS = {
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed `ncu --set full` capture of that
 # workload (profiles/), bytes; None where no capture exists.
 TRAFFIC_NCU_BYTES = {"config3a": 103_264_512, "tab4": 651_665_920, "tabg4": 1_225_114_112, "config4": 600_256_000, "snapbench": 69_562_443_296,
-                     "snapkerr": 70_775_029_960, "paper_t3": 16_144_486_488, "ks4": 561_625_600}     # profiles/r02_*.md (snapbench: r01_snapbench_v3.md)
+                     "snapkerr": 70_775_029_960, "paper_t3": 16_144_486_488, "ks4": 556_309_504}     # profiles/r02_*.md (snapbench: r01_snapbench_v3.md)
 
 
 def workload(name: str, rank: int, n_override: int | None, nthreads: int) -> dict:

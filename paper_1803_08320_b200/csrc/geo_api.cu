@@ -356,24 +356,10 @@ int launch_ks(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nst
     p.r_escape = stop->r_escape;
     p.kappa = stop->kind == GEO_TIMELIKE ? 1.0 : 0.0;
     const double a2 = ctx->a * ctx->a;
-    // end-point triggers: r >= rc  <=>  (x^2+y^2)/(rc^2+a^2) + z^2/rc^2 >= 1 for rc > 0; rc <= 0 never captures a finite point
-    if (stop->r_capture > 0.0 && std::isfinite(stop->r_capture)) {
-        p.cap_iA = 1.0 / (stop->r_capture * stop->r_capture + a2);
-        p.cap_ir2 = 1.0 / (stop->r_capture * stop->r_capture);
-        p.cap_thresh = 1.0;
-    } else if (stop->r_capture > 0.0) {       // +inf: everything is captured (decided at y0 already)
-        p.cap_iA = 0.0; p.cap_ir2 = 0.0; p.cap_thresh = 1.0;
-    } else {
-        p.cap_iA = 0.0; p.cap_ir2 = 0.0; p.cap_thresh = -1.0;
-    }
-    if (stop->r_escape > 0.0 && std::isfinite(stop->r_escape)) {
-        p.esc_iA = 1.0 / (stop->r_escape * stop->r_escape + a2);
-        p.esc_ir2 = 1.0 / (stop->r_escape * stop->r_escape);
-    } else if (stop->r_escape > 0.0) {        // +inf: never
-        p.esc_iA = 0.0; p.esc_ir2 = 0.0;
-    } else {                                  // r > re holds for every point with r > 0: trigger always, decide behind the branch
-        p.esc_iA = INFINITY; p.esc_ir2 = INFINITY;
-    }
+    // end-point triggers (geo_ks.cuh): r^2 <= R^2 <= r^2 + a^2.  r_capture <= 0 never captures a finite point, +inf always
+    // does (decided at y0); r_escape = +inf never escapes, r_escape <= 0 always triggers (decided behind the branch)
+    p.cap_R2 = stop->r_capture > 0.0 ? stop->r_capture * stop->r_capture + a2 : -INFINITY;
+    p.esc_R2 = stop->r_escape > 0.0 ? stop->r_escape * stop->r_escape : -1.0;
     p.use_queue = (stop->flags & GEO_FLAG_STATIC_MAP) ? 0 : 1;
     p.snap_every = (int)(snapshot_every > 0x7fffffffLL ? 0x7fffffffLL : snapshot_every);
     p.snap_cap = snapshot_every > 0 ? out->snap_capacity : 0;

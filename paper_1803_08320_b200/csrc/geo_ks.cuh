@@ -17,7 +17,8 @@
 //     p_j d_i l_j = d_i r K + { (r p_x - a p_y)/A, (r p_y + a p_x)/A, p_z/r },   K = (u - 2 r N/A)/A - z p_z / r^2
 //  => dp_x/dtau = x G1 + G2 (r p_x - a p_y),  dp_y/dtau = y G1 + G2 (r p_y + a p_x),  dp_z/dtau = z G3 + (f lP / r) p_z,
 //     G1 = c5 lP^2 + f lP (r/D) K,  G2 = f lP / A,  G3 = fz lP^2 + f lP (A/(r D)) K.
-// 93 FP64 instructions + 3 MUFU per evaluation (two sqrt/rsqrt pairs for (D, 1/D), (r, 1/r), one reciprocal for 1/A).
+// 82 FP64 instructions + 3 MUFU per evaluation (1/D and 1/r each from one MUFU.RSQ64H seed with a cubic correction, D = disc/D,
+// r = r^2/r; one cubic-Newton reciprocal for 1/A).
 // The oracle differentiates f and l_mu entry by entry with the quotient rule -- different algebra, no shared code.
 #pragma once
 #include "geo_kernel.cuh"
@@ -28,18 +29,14 @@ struct KsHole {
     double M, a, a2, twoM, four_a2;
 };
 
-// sqrt(x) and 1/sqrt(x) for finite normal x > 0, both faithfully rounded: MUFU.RSQ64H seed (~2^-20), one coupled
-// Goldschmidt step, a residual correction for the root and one Newton step for the reciprocal root.
-__device__ __forceinline__ void sqrt_rsqrt(double x, double& s, double& is) {
+// 1/sqrt(x) for finite normal x > 0, faithfully rounded: MUFU.RSQ64H seed y0 (relative error ~2^-20), then ONE cubic
+// correction  y0 (1 + e/2 + 3 e^2/8),  e = 1 - x y0^2  (|e| <~ 2^-19: the neglected 5 e^3/16 is < 2^-58).  Five FP64
+// instructions; sqrt(x) = x rsqrt(x) costs one more (<= 1.5 ulp).  No special-case path (garbage in, garbage out).
+__device__ __forceinline__ double rsqrt_c(double x) {
     double y0;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
-    double g = x * y0, h = 0.5 * y0;
-    const double e = fma(-g, h, 0.5);
-    g = fma(g, e, g);
-    h = fma(h, e, h);
-    s = fma(fma(-g, g, x), h, g);
-    const double t = h + h;
-    is = fma(t, fma(-s, t, 1.0), t);
+    const double e = fma(-(x * y0), y0, 1.0);
+    return fma(y0, e * fma(0.375, e, 0.5), y0);
 }
 
 struct KsDeriv {
@@ -52,14 +49,16 @@ __device__ __forceinline__ void rhs_ks(const KsHole& bh, double x, double y, dou
     const double R2 = fma(z, z, fma(y, y, x * x));
     const double w = R2 - bh.a2;
     const double disc = fma(w, w, (z * z) * bh.four_a2);
-    double D, iD, r, ir;
-    sqrt_rsqrt(disc, D, iD);
+    const double iD = rsqrt_c(disc);
+    const double D = disc * iD;
     const double r2 = 0.5 * (w + D);
-    sqrt_rsqrt(r2, r, ir);
+    const double ir = rsqrt_c(r2);
+    const double r = r2 * ir;
     r_out = r;
     const double A = r2 + bh.a2;
     const double iA = rcp_nr(A);
-    const double f = (bh.twoM * r) * iD;
+    const double c1 = r * iD;                                // d_x r / x
+    const double f = bh.twoM * c1;                           // 2 M r / D
     // l.p without the l_i
     const double u = fma(x, px, y * py);
     const double v = fma(y, px, -(x * py));
@@ -76,7 +75,6 @@ __device__ __forceinline__ void rhs_ks(const KsHole& bh, double x, double y, dou
     d.y = fma(-G2, fma(r, y, -(bh.a * x)), py);
     d.z = fma(-flPir, z, pz);
     // gradients, collected
-    const double c1 = r * iD;                                // d_x r / x
     const double c6 = (A * ir) * iD;                         // d_z r / z
     const double c7 = bh.M * iD;
     const double r2iD = r2 * iD;
@@ -134,10 +132,10 @@ struct KsParams {
     double h, h_half, h_sixth;
     int nsteps;
     double r_capture, r_escape, kappa;
-    // end-point triggers (the decision is taken behind the rare branch with radius_ks):
-    //   possible capture  <=>  !((x^2+y^2) cap_iA + z^2 cap_ir2 >= cap_thresh)     [r >= rc <=> the point lies outside the spheroid r = rc]
-    //   possible escape   <=>    (x^2+y^2) esc_iA + z^2 esc_ir2 > 1
-    double cap_iA, cap_ir2, cap_thresh, esc_iA, esc_ir2;
+    // end-point TRIGGERS from R^2 = x^2 + y^2 + z^2, which brackets r: r^2 <= R^2 <= r^2 + a^2 (the decision is taken behind
+    // the rare branch with radius_ks):  possible capture <=> !(R^2 >= cap_R2), cap_R2 = r_capture^2 + a^2 (r < rc implies it);
+    // possible escape <=> R^2 > esc_R2, esc_R2 = r_escape^2 (r > re implies it).  A NaN triggers the capture side.
+    double cap_R2, esc_R2;
     int use_queue;
     int snap_every;
     long long snap_cap;
@@ -272,10 +270,10 @@ geo_ks_rk4_kernel(const __grid_constant__ KsParams p) {
         kahan<PLAIN>(px, cur.c.px, p.h_sixth, apx, nxt.y.px, nxt.c.px);
         kahan<PLAIN>(py, cur.c.py, p.h_sixth, apy, nxt.y.py, nxt.c.py);
         kahan<PLAIN>(pz, cur.c.pz, p.h_sixth, apz, nxt.y.pz, nxt.c.pz);
-        // end point: capture / escape triggers by the spheroid form of r >= rc, r > re (no square root)
-        const double rho2 = fma(nxt.y.y, nxt.y.y, nxt.y.x * nxt.y.x), z2 = nxt.y.z * nxt.y.z;
-        const bool cap_end = !(fma(rho2, p.cap_iA, z2 * p.cap_ir2) >= p.cap_thresh);
-        const bool esc_end = fma(rho2, p.esc_iA, z2 * p.esc_ir2) > 1.0;
+        // end point: capture / escape triggers from R^2 (no square root in the accepted step)
+        const double Rn2 = fma(nxt.y.z, nxt.y.z, fma(nxt.y.y, nxt.y.y, nxt.y.x * nxt.y.x));
+        const bool cap_end = !(Rn2 >= p.cap_R2);
+        const bool esc_end = Rn2 > p.esc_R2;
         const bool fin7 = all_finite7(nxt.y);
         const bool maybe_crossing = (__double2hiint(z) ^ __double2hiint(nxt.y.z)) < 0;     // K3 candidate: sign bits differ
         const int ns = steps + 1;

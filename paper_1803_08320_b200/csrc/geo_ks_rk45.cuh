@@ -48,7 +48,7 @@ __device__ __forceinline__ K6 k6_of(const KsDeriv& d) { return K6{d.x, d.y, d.z,
 #define GEO_KS_FOR6(M) M(x) M(y) M(z) M(px) M(py) M(pz)
 
 template <bool DENSE>
-__global__ void __launch_bounds__(kBlock, 2) geo_ks_rk45_kernel(const __grid_constant__ KsAdaptiveParams p) {
+__global__ void __launch_bounds__(kBlock, DENSE ? 2 : 3) geo_ks_rk45_kernel(const __grid_constant__ KsAdaptiveParams p) {
     const unsigned lane = threadIdx.x & 31u;
     const KsHole& bh = p.bh;
     long long idx = -1;
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(kBlock, 2) geo_ks_rk45_kernel(const __grid_con
         // --- one attempt of size h (every lane; idle lanes compute on stale state) ----------------------
         if (!p.fixed_step) {                                                     // K6a
             const double v2 = fma(k1.x, k1.x, fma(k1.y, k1.y, k1.z * k1.z));
-            const double hcap = ry / (4.0 * sqrt(v2));
+            const double hcap = (0.25 * ry) * rsqrt_c(v2);                       // (v2 = 0: +inf seed -> NaN, no cap)
             if (h > hcap) h = hcap;
         }
         const bool last = tau + 1.01 * h >= p.tau_end;

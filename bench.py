@@ -61,10 +61,10 @@ F_ALG_SURVEY = {"kerr": 800.0}
 # inside the loop's address range).  A kernel edit without a new capture makes bench.py FAIL instead of reporting
 # stale numbers.
 KERNEL_COUNTS = {
-    "kerr": dict(sym="geo_rk4_kernelILb1ELi0ELb0ELb0E", units_per_loop=2, flop=461.0, pipe=326.0, other=68.0, tol=0.08, static_at_capture=(964, 686),
+    "kerr": dict(sym="geo_rk4_kernelILb1ELi0ELb0ELb0ELb0E", units_per_loop=2, flop=461.0, pipe=326.0, other=68.0, tol=0.08, static_at_capture=(964, 686),
                  source="ncu per-instruction counts, profiles/r02_config4.md: 140 DFMA + 141 DMUL + 40 DADD + 5 DSETP per step",
                  kernel="geo_rk4_kernel"),
-    "schwarzschild": dict(sym="geo_rk4_kernelILb0ELi0ELb0ELb0E", units_per_loop=2, flop=342.0, pipe=245.0, other=None, tol=0.0,
+    "schwarzschild": dict(sym="geo_rk4_kernelILb0ELi0ELb0ELb0ELb0E", units_per_loop=2, flop=342.0, pipe=245.0, other=None, tol=0.0,
                           source="static SASS count of the hot loop (no ncu capture of this instantiation)", kernel="geo_rk4_kernel"),
     "adaptive": dict(sym="geo_rk45_kernelILi1ELb0E", units_per_loop=1, flop=1039.0, pipe=678.0, other=None, tol=0.15, static_at_capture=(1135, 778),
                      source="ncu thread-level counts, profiles/r02_config3a_rk45.md: 361 DFMA + 264 DMUL + 52 DADD per attempt "

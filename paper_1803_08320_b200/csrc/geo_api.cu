@@ -46,7 +46,11 @@ kernel_fn pick_plain(bool plain) {
     return plain ? (kernel_fn)geo_rk4_kernel<KERR, SNAP, true, false> : (kernel_fn)geo_rk4_kernel<KERR, SNAP, false, false>;
 }
 template <bool KERR>
-kernel_fn pick_snap(int snap, bool plain, bool wide) {
+kernel_fn pick_snap(int snap, bool plain, bool wide, bool big) {
+    if (big) {
+        if (snap == SNAP_NONE) return plain ? (kernel_fn)geo_rk4_kernel<KERR, SNAP_NONE, true, false, true> : (kernel_fn)geo_rk4_kernel<KERR, SNAP_NONE, false, false, true>;
+        return plain ? (kernel_fn)geo_rk4_kernel<KERR, SNAP_DIRECT, true, false, true> : (kernel_fn)geo_rk4_kernel<KERR, SNAP_DIRECT, false, false, true>;
+    }
     switch (snap) {
         case SNAP_NONE:
             if (wide) return plain ? (kernel_fn)geo_rk4_kernel<KERR, SNAP_NONE, true, true> : (kernel_fn)geo_rk4_kernel<KERR, SNAP_NONE, false, true>;
@@ -55,8 +59,8 @@ kernel_fn pick_snap(int snap, bool plain, bool wide) {
         default: return pick_plain<KERR, SNAP_STAGED>(plain);
     }
 }
-kernel_fn pick_kernel(int metric, int snap, bool plain, bool wide) {
-    return metric == GEO_KERR ? pick_snap<true>(snap, plain, wide) : pick_snap<false>(snap, plain, wide);
+kernel_fn pick_kernel(int metric, int snap, bool plain, bool wide, bool big) {
+    return metric == GEO_KERR ? pick_snap<true>(snap, plain, wide, big) : pick_snap<false>(snap, plain, wide, big);
 }
 
 int fail(geo_ctx* ctx, int code, const char* msg) {
@@ -134,6 +138,7 @@ struct LaunchPlan {
     int snap_mode;
     int use_queue;
     int grid;
+    int block;
     size_t smem;
     int ctas_per_sm;
     int regs;
@@ -148,7 +153,16 @@ int plan_launch(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, 
     lp->snap_mode = snapshot_every > 0 ? (staged ? SNAP_STAGED : SNAP_DIRECT) : SNAP_NONE;
     // a batch without records that fits on the machine at 2 CTAs per SM runs the high-ILP instantiation (geo_kernel.cuh: WIDE)
     const bool wide = lp->snap_mode == SNAP_NONE && n <= (int64_t)ctx->sm_count * 2 * kBlock;
-    lp->fn = pick_kernel(ctx->metric, lp->snap_mode, (flags & GEO_FLAG_PLAIN_UPDATE) != 0, wide);
+    // a batch that fits in ONE wave (n <= 512 x SMs) runs ONE CTA per SM of 128 k threads, k = ceil(n / (128 SMs)) = the
+    // warps per scheduler it needs anyway (geo_kernel.cuh: BIG; the WIDE instantiation takes up to 256 threads): warps of
+    // one CTA have the same age and progress evenly, several CTAs per SM do not (measured: DESIGN.md section 9)
+    const int64_t k64 = (n + (int64_t)ctx->sm_count * kBlock - 1) / ((int64_t)ctx->sm_count * kBlock);
+    const int k = k64 < 1 ? 1 : (k64 > 1024 ? 1024 : (int)k64);
+    const bool one_wave = k <= kBigBlock / kBlock && lp->snap_mode != SNAP_STAGED;
+    const bool big = one_wave && !wide && k >= 2;
+    const int blk = one_wave ? k * kBlock : kBlock;
+    lp->block = blk;
+    lp->fn = pick_kernel(ctx->metric, lp->snap_mode, (flags & GEO_FLAG_PLAIN_UPDATE) != 0, wide, big);
     lp->smem = lp->snap_mode == SNAP_STAGED ? (size_t)kBlock * stage_stride(ncomp) * sizeof(double) : 0;
     lp->use_queue = (flags & GEO_FLAG_STATIC_MAP) ? 0 : 1;
     cudaFuncAttributes fa;
@@ -156,11 +170,11 @@ int plan_launch(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_every, 
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaFuncGetAttributes");
     lp->regs = fa.numRegs;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)lp->fn, kBlock, lp->smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)lp->fn, lp->block, lp->smem);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
     if (per_sm < 1) return fail(ctx, GEO_ECUDA, "kernel does not fit on an SM");
     lp->ctas_per_sm = per_sm;
-    const int64_t need = (n + kBlock - 1) / kBlock;
+    const int64_t need = (n + lp->block - 1) / lp->block;
     if (lp->use_queue) {
         // persistent grid: every SM full, no more CTAs than there is work
         const int64_t resident = (int64_t)ctx->sm_count * per_sm;
@@ -437,7 +451,7 @@ int launch(geo_ctx* ctx, const double* d_in, int64_t n, double h, int64_t nsteps
         e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), stream);
         if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaMemsetAsync(counter)");
     }
-    lp.fn<<<lp.grid, kBlock, lp.smem, stream>>>(p);
+    lp.fn<<<lp.grid, lp.block, lp.smem, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(ctx, e, "kernel launch");
     return GEO_OK;
@@ -888,7 +902,7 @@ int geo_launch_info(geo_ctx* ctx, int64_t n, int32_t flags, int64_t snapshot_eve
     int rc = plan_launch(ctx, n, flags, snapshot_every, 8, &lp);
     if (rc != GEO_OK) return rc;
     info[0] = lp.grid;
-    info[1] = kBlock;
+    info[1] = lp.block;
     info[2] = lp.regs;
     info[3] = lp.ctas_per_sm;
     return GEO_OK;

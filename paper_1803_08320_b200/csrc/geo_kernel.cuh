@@ -175,12 +175,23 @@ struct LaneState {
 // batch is latency-bound -- one or two warps per scheduler -- and what counts is the time ONE warp needs for a step: ~2550
 // cycles at 128 registers, ~1600 at the 234 registers the compiler takes when it may (more independent instructions in
 // flight per warp).  Same source, same PTX arithmetic, same bits.
+//
+// BIG: the instantiation for batches that fit in ONE wave of the machine (n <= 512 x SMs) and need k = ceil(n / (128 SMs)) >= 2
+// warps per scheduler: ONE CTA of 128 k threads per SM (256 / 384 / 512) instead of k CTAs of 128, same 128 registers (the
+// WIDE instantiation likewise takes one 256-thread CTA).  Measured on configs[1] (65 536 particles, k = 4): with four CTAs per
+// SM the warps of the oldest CTA are favoured by the warp scheduler, finish first, and the youngest CTA's tail runs at one or
+// two warps per scheduler (ncu: 3.5 warps resident on the heaviest scheduler on average; 172.3 ms); the warps of ONE CTA have
+// the same age and progress evenly: 155.3 ms, the time of four warps per scheduler at full pace.  n = 50 000 (k = 3): 13.19
+// -> 12.01 ms; with a record every step 5-8 % (paper Table 3 workload 27.4 -> 26.0 ms).  Multi-wave batches keep 128-thread
+// CTAs (the queue refills their lanes; 512-thread CTAs gain 0.3-0.9 % there and lose 6-9 % with a record every step).
+// Same source, same PTX arithmetic, same bits.
+constexpr int kBigBlock = 512;
 #ifdef GEO_MAXNREG
 #define GEO_RK4_BOUNDS __maxnreg__(GEO_MAXNREG)
 #else
-#define GEO_RK4_BOUNDS __launch_bounds__(kBlock, WIDE ? 2 : (SNAP == SNAP_NONE ? GEO_MIN_CTAS_PER_SM : 4))
+#define GEO_RK4_BOUNDS __launch_bounds__(BIG ? kBigBlock : (WIDE ? 2 * kBlock : kBlock), (BIG || WIDE) ? 1 : (SNAP == SNAP_NONE ? GEO_MIN_CTAS_PER_SM : 4))
 #endif
-template <bool KERR, int SNAP, bool PLAIN, bool WIDE>
+template <bool KERR, int SNAP, bool PLAIN, bool WIDE, bool BIG = false>
 __global__ void GEO_RK4_BOUNDS
 geo_rk4_kernel(const __grid_constant__ Params p) {
     extern __shared__ __align__(16) double stage_smem[];   // SNAP_STAGED: [kBlock][stage_stride(ncomp)]
@@ -383,7 +394,7 @@ geo_rk4_kernel(const __grid_constant__ Params p) {
     };
 
     if (!p.use_queue) {
-        const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
+        const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
         if (i < p.n) begin(i);
     }
 

@@ -216,3 +216,41 @@ def test_small_batch_instantiation_gives_the_bits_of_the_full_machine_one(G):
     tb = run_gpu(G, G.KERR, 0.5, st, 0.01, 300, flags=G.FLAG_PLAIN_UPDATE)
     ts = run_gpu(G, G.KERR, 0.5, np.ascontiguousarray(st[:, :5000]), 0.01, 300, flags=G.FLAG_PLAIN_UPDATE)
     assert np.array_equal(tb["final_state"][:, :5000], ts["final_state"])
+
+
+@pytest.mark.parametrize("snapshot_every", [0, 100])
+def test_one_wave_batches_on_one_cta_per_sm_give_the_same_bits(G, snapshot_every):
+    """A batch that fits in one wave (n <= 512 x SMs) runs ONE CTA of 128 k threads per SM, k = ceil(n / (128 SMs))
+    (geo_kernel.cuh: BIG; WIDE takes 256).  Same source, same arithmetic: every particle's result -- trajectory records
+    included -- is bitwise what it is in a batch of another size class (k = 1, 2, 3, 4 and multi-wave), with the queue and
+    with the static mapping."""
+    import torch
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    n = sm * 3 * 128 + 1000                                                  # k = 4
+    st = W.kerr_bound(n, 0.9, W.SEED_BASE + 2)
+    kw = dict(snapshot_every=snapshot_every, snap_mask=0x6F)
+    ctx = G.geo_create(G.KERR, 1.0, 0.9)
+    try:
+        for m, blk in ((n, 512), (sm * 3 * 128, 384), (sm * 2 * 128 + 1, 384), (sm * 128 + 1, 256), (sm * 128, 128), (sm * 512 + 1, 128)):
+            info = G.geo_launch_info(ctx, m, 0, snapshot_every)
+            assert info["block"] == blk and (blk == 128 or info["grid"] <= sm), (m, info)
+        assert G.geo_launch_info(ctx, n, G.FLAG_STAGED_SNAP, 100)["block"] == 128      # the staged writer keeps its 128-thread stage
+    finally:
+        G.geo_destroy(ctx)
+    big = run_gpu(G, G.KERR, 0.9, st, 0.01, 300, **kw)
+    big_static = run_gpu(G, G.KERR, 0.9, st, 0.01, 300, flags=G.FLAG_STATIC_MAP, **kw)
+    for lo, hi in ((0, 5000), (1000, 1000 + sm * 128 + 77), (n - 45000, n)):        # k = 1, k = 2, k = 3
+        small = run_gpu(G, G.KERR, 0.9, np.ascontiguousarray(st[:, lo:hi]), 0.01, 300, **kw)
+        for res in (big, big_static):
+            assert np.array_equal(res["final_state"][:, lo:hi].view(np.int64), small["final_state"].view(np.int64))
+            assert np.array_equal(res["status"][lo:hi], small["status"]) and np.array_equal(res["steps_done"][lo:hi], small["steps_done"])
+            assert np.array_equal(res["eq_cross_r"][lo:hi].view(np.int64), small["eq_cross_r"].view(np.int64))
+            if snapshot_every:
+                assert np.array_equal(res["snap_count"][lo:hi], small["snap_count"])
+                assert np.array_equal(res["snapshots"][lo:hi].view(np.int64), small["snapshots"].view(np.int64))
+    # multi-wave (128-thread CTAs, queue refill): the first 3000 particles of a 2-wave batch
+    nn = sm * 512 + 3000
+    st2 = W.kerr_bound(nn, 0.9, W.SEED_BASE + 2)
+    assert np.array_equal(st2[:, :n], st)                                        # (the generator is prefix-stable)
+    multi = run_gpu(G, G.KERR, 0.9, st2, 0.01, 300, **kw)
+    assert np.array_equal(multi["final_state"][:, :n].view(np.int64), big["final_state"].view(np.int64))

@@ -17,7 +17,7 @@
 //     p_j d_i l_j = d_i r K + { (r p_x - a p_y)/A, (r p_y + a p_x)/A, p_z/r },   K = (u - 2 r N/A)/A - z p_z / r^2
 //  => dp_x/dtau = x G1 + G2 (r p_x - a p_y),  dp_y/dtau = y G1 + G2 (r p_y + a p_x),  dp_z/dtau = z G3 + (f lP / r) p_z,
 //     G1 = c5 lP^2 + f lP (r/D) K,  G2 = f lP / A,  G3 = fz lP^2 + f lP (A/(r D)) K.
-// 82 FP64 instructions + 3 MUFU per evaluation (1/D and 1/r each from one MUFU.RSQ64H seed with a cubic correction, D = disc/D,
+// 81 FP64 instructions + 3 MUFU per evaluation (1/D and 1/r each from one MUFU.RSQ64H seed with a cubic correction, D = disc/D,
 // r = r^2/r; one cubic-Newton reciprocal for 1/A).
 // The oracle differentiates f and l_mu entry by entry with the quotient rule -- different algebra, no shared code.
 #pragma once
